@@ -1,0 +1,124 @@
+/*
+ * hirep_b200.h -- C-ABI of the B200-native Wilson-Dirac operator for fermions in a representation R of SU(N_g).
+ *
+ * Operation definitions follow arXiv 2503.06721 (HiRep v2); citations are PAPER.md line + section/equation.
+ *
+ *   lattice      T x L^3 hypercubic, mu = 0 is time                                  (L167, Sect. 2.1)
+ *   gamma basis  e_0 = -1, e_k = -i sigma_k, gamma_mu = [[0,e_mu],[e_mu^dagger,0]]   (L171-182, Eq 1-3)
+ *   D_m psi(x) = (4+m) psi(x) - 1/2 sum_mu [ (1-gamma_mu) U^R_mu(x) psi(x+mu)
+ *                                           + (1+gamma_mu) U^R_mu(x-mu)^dagger psi(x-mu) ]   (L207, Eq 8; a = 1)
+ *   Q_m = gamma_5 D_m, gamma_5 = gamma_0 gamma_1 gamma_2 gamma_3 = diag(1,1,-1,-1)    (L230, Eq 11; A1)
+ *   even site: (t+x+y+z) mod 2 = 0; D_m = [[D_ee, D_eo],[D_oe, D_oo]]                (L793-795, Eq 41)
+ *   D_hat = (4+m)^2 - D_eo D_oe                                                      (L808, Eq 44)
+ *   boundary conditions: psi(x + L_mu) = bc_mu psi(x), bc_mu = +-1                   (L930-943, Eq 58-63)
+ *   representations FUND / ADJ / SYM / 2AS, dimensions of Tbl 1                      (L213-220)
+ *
+ * General rules
+ *   - Every function returns 0 on success and a negative HIREP_E* code on failure; nothing throws or aborts
+ *     across this boundary.  hirep_last_error() gives a thread-local NUL-terminated description.
+ *   - "device pointer" = CUDA global memory on the current device, 16-byte aligned, owned by the caller
+ *     (allocate through torch).  "host pointer" = ordinary host memory (pinned memory makes the copies faster).
+ *   - Operator calls are asynchronous on the geometry's stream (hirep_geom_set_stream; default stream 0);
+ *     launch failures are reported by the call that launched, execution failures by hirep_sync or a later call.
+ *   - `out` is overwritten, never accumulated, and must not alias `in`.
+ *   - There is NO CPU fallback: without a CUDA device every compute entry point returns HIREP_ECUDA.
+ *
+ * Canonical (interchange) layout -- used only by the import/export calls and by hirep_apply_host:
+ *     site index ix = ((t*L + x)*L + y)*L + z        (z fastest)
+ *     spinor  [ix][spin 0..3][colour 0..d_R-1]        complex (interleaved re,im)  of the working precision
+ *     links   [ix][mu 0..3][row i][col j]             complex, (U psi)_i = sum_j U_ij psi_j
+ *     half-lattice spinors list the sites of that parity in increasing ix.
+ *     represented links exported by hirep_links_rep_export: [ix][mu][i][j], REAL scalars for ADJ
+ *     (rep_is_real = 1), complex otherwise.
+ * Native layout -- private to the library, sizes from hirep_geom_sizes, described in DESIGN.md:
+ *     per parity, sites ordered (t,x,y,z/2) in tiles of 32; spinor [tile][4 d_R][32] complex;
+ *     links [parity][tile][8 directions][d*d][32]: the 8 matrices W_d that act on the 8 neighbours of a
+ *     site (W_mu = U_mu(x), W_{4+mu} = U_mu(x-mu)^dagger), so every stencil pass streams one contiguous
+ *     block per tile.  Represented links carry the boundary signs.
+ */
+#ifndef HIREP_B200_H
+#define HIREP_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hirep_geom hirep_geom; /* opaque: lattice maps, BC state, stream, workspace spinors */
+
+enum { HIREP_FUND = 0, HIREP_ADJ = 1, HIREP_SYM = 2, HIREP_ASY = 3 }; /* representation (Tbl 1, L213-220) */
+enum { HIREP_F64 = 0, HIREP_F32 = 1 };                                /* field precision (L308)          */
+enum { HIREP_EVEN = 0, HIREP_ODD = 1, HIREP_FULL = 2 };
+enum { HIREP_LINKS_STORED = 0, HIREP_LINKS_REBUILD = 1 };
+enum { HIREP_OP_DPHI = 0, HIREP_OP_DPHI_EO = 1, HIREP_OP_DPHI_OE = 2, HIREP_OP_DPHI_HAT = 3, HIREP_OP_G5DPHI_SQ = 4 };
+enum {
+    HIREP_OK = 0,
+    HIREP_EINVAL = -1,       /* bad argument: null/misaligned pointer, odd or <2 extent, unknown enum, out aliases in */
+    HIREP_EUNSUPPORTED = -2, /* (N_g, rep, prec, mode) combination not instantiated                               */
+    HIREP_ECUDA = -3,        /* CUDA runtime error (no device, launch or execution failure)                        */
+    HIREP_ENOMEM = -4        /* workspace allocation failed                                                        */
+};
+
+/* Lattice T x L^3 (both even, >= 2), gauge group SU(N_g) (2 <= N_g <= 6), representation, precision.
+ * Default boundary conditions: antiperiodic in time, periodic in space ({-1,+1,+1,+1}); link mode STORED. */
+int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep_geom **out);
+int hirep_geom_destroy(hirep_geom *g); /* frees the handle and its workspace; NULL is a no-op */
+
+/* bc_mu = +-1 per direction (Eq 58-63).  The signs are baked into the represented links by
+ * hirep_links_to_rep (the paper's implementation, L945), so call it again after changing them. */
+int hirep_geom_set_bc(hirep_geom *g, const int sign[4]);
+/* cuda_stream: a cudaStream_t / CUstream (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream */
+int hirep_geom_set_stream(hirep_geom *g, void *cuda_stream);
+/* Bytes of native buffers (any pointer may be NULL): full- and half-lattice spinor, fundamental links,
+ * represented links; d_R (Tbl 1); rep_is_real = 1 iff represented links are stored as real numbers (ADJ). */
+int hirep_geom_sizes(const hirep_geom *g, size_t *spinor_full, size_t *spinor_half, size_t *links_fund,
+                     size_t *links_rep, int *d_R, int *rep_is_real);
+
+/* canonical <-> native, all device pointers.  parity_or_full in {HIREP_EVEN, HIREP_ODD, HIREP_FULL}. */
+int hirep_spinor_import(hirep_geom *g, void *native, const void *canonical, int parity_or_full);
+int hirep_spinor_export(hirep_geom *g, void *canonical, const void *native, int parity_or_full);
+int hirep_links_import(hirep_geom *g, void *native_fund, const void *canonical_fund);
+/* forward matrices s_mu(x) U^R_mu(x) (boundary sign included) in canonical order; for tests */
+int hirep_links_rep_export(hirep_geom *g, void *canonical_rep, const void *native_rep);
+/* the stored backward matrices W_{4+mu}(x) = s U^R_mu(x-mu)^dagger, canonical [ix][mu][i][j]; for tests */
+int hirep_links_rep_export_bwd(hirep_geom *g, void *canonical_rep, const void *native_rep);
+
+/* U -> U^R for all links (Eq 7; FUND: identity map; ADJ: R_ab = 2 Re tr(T^a U T^b U^dagger);
+ * SYM/2AS: Psi -> U Psi U^T on (anti)symmetric tensors; bases in DESIGN.md A10/A11), times the boundary
+ * sign on links that cross the lattice boundary (L945).  Device pointers, native layouts. */
+int hirep_links_to_rep(hirep_geom *g, void *native_rep, const void *native_fund);
+
+/* The operators.  Device pointers to native buffers.  `links` is the represented field (mode STORED) or the
+ * fundamental field (mode REBUILD, R rebuilt in registers).  m0 is the bare mass m of Eq 8.
+ *   hirep_Dphi      out = D_m in                      full lattice            (Eq 8/10)
+ *   hirep_Dphi_eo   out_even = D_eo in_odd            (off-diagonal block of Eq 41, includes the -1/2)
+ *   hirep_Dphi_oe   out_odd  = D_oe in_even
+ *   hirep_Dphi_hat  out_even = (4+m)^2 in_even - D_eo D_oe in_even            (Eq 44)
+ *   hirep_g5Dphi_sq out = gamma_5 D_m gamma_5 D_m in  full lattice            (Eq 11)            */
+int hirep_Dphi(hirep_geom *g, double m0, void *out_full, const void *in_full, const void *links);
+int hirep_Dphi_eo(hirep_geom *g, void *out_even, const void *in_odd, const void *links);
+int hirep_Dphi_oe(hirep_geom *g, void *out_odd, const void *in_even, const void *links);
+int hirep_Dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links);
+int hirep_g5Dphi_sq(hirep_geom *g, double m0, void *out_full, const void *in_full, const void *links);
+
+int hirep_set_link_mode(hirep_geom *g, int mode); /* HIREP_LINKS_STORED | HIREP_LINKS_REBUILD */
+/* Implementation variant of the stencil kernel, for measurements: 0 = library default, >0 = explicit
+ * (list in DESIGN.md).  An unknown variant for the geometry's instantiation returns HIREP_EUNSUPPORTED. */
+int hirep_set_kernel_variant(hirep_geom *g, int variant);
+/* number of kernels this library has launched on behalf of g since creation (bench.py's gpu_launches) */
+long hirep_launch_count(const hirep_geom *g);
+
+/* End-to-end entry with HOST buffers (canonical layout): copies `in` (and `links_fund`, if non-NULL; otherwise
+ * the represented links built by the previous call are reused) to the device, imports, builds the represented
+ * links, applies `op` (HIREP_OP_*), exports and copies the result back to `out`; returns after the result is in
+ * host memory.  Spinor extents follow the op (half lattice for EO/OE/HAT, full otherwise). */
+int hirep_apply_host(hirep_geom *g, int op, double m0, void *out_host, const void *in_host, const void *links_fund_host);
+
+int hirep_sync(hirep_geom *g); /* synchronise the stream; returns any pending execution error */
+const char *hirep_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HIREP_B200_H */

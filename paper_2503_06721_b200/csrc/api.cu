@@ -1,0 +1,316 @@
+// api.cu -- the C-ABI of include/hirep_b200.h: argument checking, workspace, operator composition.
+//
+// Operator composition out of stencil passes (hop_small.cuh / hop_large.cuh), out = a*self + b*hop(in):
+//   Dphi_eo / Dphi_oe : a = 0,        b = -1/2                                  (Eq 41)
+//   Dphi              : a = 4 + m,    b = -1/2, both parities in one launch     (Eq 8,  L207)
+//   Dphi_hat          : tmp_o = D_oe in_e ; out_e = (4+m)^2 in_e + 1/2 hop(tmp_o)   (Eq 44)
+//   g5Dphi_sq         : tmp = g5 D in ; out = g5 D tmp                          (Eq 11; L772)
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/hirep_b200.h"
+#include "hop_dispatch.cuh"
+
+using namespace hirep;
+
+struct hirep_geom {
+    Geo geo;
+    int N, rep, prec, dR, real;
+    int mode, variant;
+    cudaStream_t stream;
+    void *ws_half, *ws_full;        // workspace spinors (lazy)
+    // hirep_apply_host staging (lazy)
+    void *h_links_canon, *h_links_fund, *h_links_rep, *h_in_canon, *h_in_native, *h_out_native, *h_out_canon;
+    int host_links_ready;
+    long launches;
+    size_t bytes_spinor_half, bytes_links_fund, bytes_links_rep;
+};
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+static int cuda_fail(cudaError_t e, const char *what) {
+    return fail(HIREP_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+static int kern_result(hirep_geom *g, int rc, const char *what, int nlaunch = 1) {
+    if (rc == 0) { g->launches += nlaunch; return HIREP_OK; }
+    if (rc == KERR_UNSUPPORTED)
+        return fail(HIREP_EUNSUPPORTED, "%s: no kernel instantiated for N_g=%d rep=%d prec=%d mode=%d variant=%d", what, g->N,
+                    g->rep, g->prec, g->mode, g->variant);
+    return cuda_fail((cudaError_t)rc, what);
+}
+static bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+extern "C" const char *hirep_last_error(void) { return g_err; }
+
+static int rep_dim(int N, int rep) {
+    switch (rep) {
+    case HIREP_FUND: return N;
+    case HIREP_ADJ: return N * N - 1;
+    case HIREP_SYM: return N * (N + 1) / 2;
+    case HIREP_ASY: return N * (N - 1) / 2;
+    }
+    return -1;
+}
+
+extern "C" int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep_geom **out) {
+    if (!out) return fail(HIREP_EINVAL, "hirep_geom_create: out is NULL");
+    *out = nullptr;
+    if (T < 2 || L < 2 || (T & 1) || (L & 1)) return fail(HIREP_EINVAL, "hirep_geom_create: extents must be even and >= 2 (T=%d L=%d)", T, L);
+    if (N_g < 2 || N_g > 6) return fail(HIREP_EINVAL, "hirep_geom_create: N_g=%d outside 2..6", N_g);
+    if (rep < 0 || rep > 3) return fail(HIREP_EINVAL, "hirep_geom_create: unknown representation %d", rep);
+    if (prec != HIREP_F64 && prec != HIREP_F32) return fail(HIREP_EINVAL, "hirep_geom_create: unknown precision %d", prec);
+    const long long V = (long long)T * L * L * L;
+    if (V / 2 + 32 >= (1LL << 31)) return fail(HIREP_EINVAL, "hirep_geom_create: lattice too large for 32-bit site indices");
+    const int dR = rep_dim(N_g, rep);
+    if (dR < 2) return fail(HIREP_EUNSUPPORTED, "hirep_geom_create: d_R=%d is not supported", dR);
+    hirep_geom *g = new (std::nothrow) hirep_geom;
+    if (!g) return fail(HIREP_ENOMEM, "hirep_geom_create: out of host memory");
+    memset(g, 0, sizeof(*g));
+    g->geo.T = T; g->geo.L = L; g->geo.Lh = L / 2;
+    g->geo.Nh = (int)(V / 2);
+    g->geo.n_tiles = (g->geo.Nh + TILE - 1) / TILE;
+    g->geo.bc[0] = -1; g->geo.bc[1] = g->geo.bc[2] = g->geo.bc[3] = 1;
+    g->N = N_g; g->rep = rep; g->prec = prec; g->dR = dR; g->real = (rep == HIREP_ADJ);
+    const size_t w = prec == HIREP_F64 ? 8 : 4;
+    g->bytes_spinor_half = (size_t)g->geo.n_tiles * 4 * dR * TILE * 2 * w;
+    g->bytes_links_fund = (size_t)2 * g->geo.n_tiles * 8 * N_g * N_g * TILE * 2 * w;
+    g->bytes_links_rep = (size_t)2 * g->geo.n_tiles * 8 * dR * dR * TILE * (g->real ? 1 : 2) * w;
+    *out = g;
+    return HIREP_OK;
+}
+
+extern "C" int hirep_geom_destroy(hirep_geom *g) {
+    if (!g) return HIREP_OK;
+    void *bufs[] = {g->ws_half, g->ws_full, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
+                    g->h_in_native, g->h_out_native, g->h_out_canon};
+    for (void *b : bufs)
+        if (b) cudaFree(b);
+    delete g;
+    return HIREP_OK;
+}
+
+extern "C" int hirep_geom_set_bc(hirep_geom *g, const int sign[4]) {
+    if (!g || !sign) return fail(HIREP_EINVAL, "hirep_geom_set_bc: NULL argument");
+    for (int mu = 0; mu < 4; ++mu)
+        if (sign[mu] != 1 && sign[mu] != -1) return fail(HIREP_EINVAL, "hirep_geom_set_bc: sign[%d]=%d is not +-1", mu, sign[mu]);
+    for (int mu = 0; mu < 4; ++mu) g->geo.bc[mu] = sign[mu];
+    g->host_links_ready = 0;
+    return HIREP_OK;
+}
+
+extern "C" int hirep_geom_set_stream(hirep_geom *g, void *cuda_stream) {
+    if (!g) return fail(HIREP_EINVAL, "hirep_geom_set_stream: NULL geometry");
+    g->stream = (cudaStream_t)cuda_stream;
+    return HIREP_OK;
+}
+
+extern "C" int hirep_geom_sizes(const hirep_geom *g, size_t *spinor_full, size_t *spinor_half, size_t *links_fund,
+                                size_t *links_rep, int *d_R, int *rep_is_real) {
+    if (!g) return fail(HIREP_EINVAL, "hirep_geom_sizes: NULL geometry");
+    if (spinor_full) *spinor_full = 2 * g->bytes_spinor_half;
+    if (spinor_half) *spinor_half = g->bytes_spinor_half;
+    if (links_fund) *links_fund = g->bytes_links_fund;
+    if (links_rep) *links_rep = g->bytes_links_rep;
+    if (d_R) *d_R = g->dR;
+    if (rep_is_real) *rep_is_real = g->real;
+    return HIREP_OK;
+}
+
+extern "C" int hirep_set_link_mode(hirep_geom *g, int mode) {
+    if (!g) return fail(HIREP_EINVAL, "hirep_set_link_mode: NULL geometry");
+    if (mode != HIREP_LINKS_STORED && mode != HIREP_LINKS_REBUILD) return fail(HIREP_EINVAL, "hirep_set_link_mode: unknown mode %d", mode);
+    g->mode = mode;
+    return HIREP_OK;
+}
+extern "C" int hirep_set_kernel_variant(hirep_geom *g, int variant) {
+    if (!g) return fail(HIREP_EINVAL, "hirep_set_kernel_variant: NULL geometry");
+    if (variant < 0) return fail(HIREP_EINVAL, "hirep_set_kernel_variant: negative variant");
+    g->variant = variant;
+    return HIREP_OK;
+}
+extern "C" long hirep_launch_count(const hirep_geom *g) { return g ? g->launches : 0; }
+
+#define CHECK_PTRS(name, ...)                                                                                      \
+    do {                                                                                                           \
+        if (!g) return fail(HIREP_EINVAL, name ": NULL geometry");                                                 \
+        const void *ptrs_[] = {__VA_ARGS__};                                                                       \
+        for (const void *p_ : ptrs_) {                                                                             \
+            if (!p_) return fail(HIREP_EINVAL, name ": NULL pointer argument");                                    \
+            if (misaligned(p_)) return fail(HIREP_EINVAL, name ": pointer %p is not 16-byte aligned", p_);         \
+        }                                                                                                          \
+    } while (0)
+
+extern "C" int hirep_spinor_import(hirep_geom *g, void *native, const void *canonical, int which) {
+    CHECK_PTRS("hirep_spinor_import", native, canonical);
+    if (which < 0 || which > 2) return fail(HIREP_EINVAL, "hirep_spinor_import: parity_or_full=%d", which);
+    return kern_result(g, k_spinor_import(g->geo, g->prec, g->dR, native, canonical, which, g->stream), "hirep_spinor_import",
+                       1 + (g->geo.Nh % TILE ? 1 : 0));
+}
+extern "C" int hirep_spinor_export(hirep_geom *g, void *canonical, const void *native, int which) {
+    CHECK_PTRS("hirep_spinor_export", native, canonical);
+    if (which < 0 || which > 2) return fail(HIREP_EINVAL, "hirep_spinor_export: parity_or_full=%d", which);
+    return kern_result(g, k_spinor_export(g->geo, g->prec, g->dR, canonical, native, which, g->stream), "hirep_spinor_export");
+}
+extern "C" int hirep_links_import(hirep_geom *g, void *native_fund, const void *canonical_fund) {
+    CHECK_PTRS("hirep_links_import", native_fund, canonical_fund);
+    return kern_result(g, k_links_import(g->geo, g->prec, g->N, native_fund, canonical_fund, g->stream), "hirep_links_import");
+}
+extern "C" int hirep_links_rep_export(hirep_geom *g, void *canonical_rep, const void *native_rep) {
+    CHECK_PTRS("hirep_links_rep_export", native_rep, canonical_rep);
+    return kern_result(g, k_links_rep_export(g->geo, g->prec, g->dR, g->real, canonical_rep, native_rep, 0, g->stream), "hirep_links_rep_export");
+}
+extern "C" int hirep_links_rep_export_bwd(hirep_geom *g, void *canonical_rep, const void *native_rep) {
+    CHECK_PTRS("hirep_links_rep_export_bwd", native_rep, canonical_rep);
+    return kern_result(g, k_links_rep_export(g->geo, g->prec, g->dR, g->real, canonical_rep, native_rep, 1, g->stream), "hirep_links_rep_export_bwd");
+}
+extern "C" int hirep_links_to_rep(hirep_geom *g, void *native_rep, const void *native_fund) {
+    CHECK_PTRS("hirep_links_to_rep", native_rep, native_fund);
+    if (native_rep == native_fund) return fail(HIREP_EINVAL, "hirep_links_to_rep: output aliases input");
+    return kern_result(g, k_links_to_rep(g->geo, g->prec, g->N, g->rep, native_rep, native_fund, g->stream), "hirep_links_to_rep");
+}
+
+// ---- operators ------------------------------------------------------------------------------------
+static int hop(hirep_geom *g, const HopLaunch &L, const char *what) {
+    const int rc = g->prec == HIREP_F64 ? k_hop_f64(g->geo, g->N, g->rep, g->mode, g->variant, L, g->stream)
+                                        : k_hop_f32(g->geo, g->N, g->rep, g->mode, g->variant, L, g->stream);
+    return kern_result(g, rc, what);
+}
+static const char *links_parity(const hirep_geom *g, const void *links, int p) {
+    const size_t total = g->mode == HIREP_LINKS_STORED ? g->bytes_links_rep : g->bytes_links_fund;
+    return (const char *)links + (size_t)p * (total / 2);
+}
+static int workspace(void **slot, size_t bytes) {
+    if (*slot) return HIREP_OK;
+    cudaError_t e = cudaMalloc(slot, bytes);
+    if (e != cudaSuccess) { *slot = nullptr; cudaGetLastError(); return fail(HIREP_ENOMEM, "workspace allocation of %zu bytes failed: %s", bytes, cudaGetErrorString(e)); }
+    return HIREP_OK;
+}
+
+static int offdiag(hirep_geom *g, void *out, const void *in, const void *links, int p_out, const char *what) {
+    HopLaunch L{};
+    L.nsets = 1;
+    L.set[0] = HopSet{in, out, nullptr, links_parity(g, links, p_out), p_out};
+    L.a = 0.0; L.b = -0.5; L.g5 = 0;
+    return hop(g, L, what);
+}
+
+extern "C" int hirep_Dphi_eo(hirep_geom *g, void *out_even, const void *in_odd, const void *links) {
+    CHECK_PTRS("hirep_Dphi_eo", out_even, in_odd, links);
+    if (out_even == in_odd) return fail(HIREP_EINVAL, "hirep_Dphi_eo: out aliases in");
+    return offdiag(g, out_even, in_odd, links, 0, "hirep_Dphi_eo");
+}
+extern "C" int hirep_Dphi_oe(hirep_geom *g, void *out_odd, const void *in_even, const void *links) {
+    CHECK_PTRS("hirep_Dphi_oe", out_odd, in_even, links);
+    if (out_odd == in_even) return fail(HIREP_EINVAL, "hirep_Dphi_oe: out aliases in");
+    return offdiag(g, out_odd, in_even, links, 1, "hirep_Dphi_oe");
+}
+
+static int dphi_full(hirep_geom *g, double m0, void *out, const void *in, const void *links, int g5, const char *what) {
+    const size_t hb = g->bytes_spinor_half;
+    const char *in_e = (const char *)in, *in_o = in_e + hb;
+    char *out_e = (char *)out, *out_o = out_e + hb;
+    HopLaunch L{};
+    L.nsets = 2;
+    L.set[0] = HopSet{in_o, out_e, in_e, links_parity(g, links, 0), 0};
+    L.set[1] = HopSet{in_e, out_o, in_o, links_parity(g, links, 1), 1};
+    L.a = 4.0 + m0; L.b = -0.5; L.g5 = g5;
+    return hop(g, L, what);
+}
+
+extern "C" int hirep_Dphi(hirep_geom *g, double m0, void *out_full, const void *in_full, const void *links) {
+    CHECK_PTRS("hirep_Dphi", out_full, in_full, links);
+    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Dphi: out aliases in");
+    return dphi_full(g, m0, out_full, in_full, links, 0, "hirep_Dphi");
+}
+
+extern "C" int hirep_Dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links) {
+    CHECK_PTRS("hirep_Dphi_hat", out_even, in_even, links);
+    if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_Dphi_hat: out aliases in");
+    int rc = workspace(&g->ws_half, g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = offdiag(g, g->ws_half, in_even, links, 1, "hirep_Dphi_hat (D_oe pass)");
+    if (rc) return rc;
+    HopLaunch L{};
+    L.nsets = 1;
+    L.set[0] = HopSet{g->ws_half, out_even, in_even, links_parity(g, links, 0), 0};
+    L.a = (4.0 + m0) * (4.0 + m0);
+    L.b = +0.5;   // - D_eo = -(-1/2) hop
+    L.g5 = 0;
+    return hop(g, L, "hirep_Dphi_hat (D_eo pass)");
+}
+
+extern "C" int hirep_g5Dphi_sq(hirep_geom *g, double m0, void *out_full, const void *in_full, const void *links) {
+    CHECK_PTRS("hirep_g5Dphi_sq", out_full, in_full, links);
+    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_g5Dphi_sq: out aliases in");
+    int rc = workspace(&g->ws_full, 2 * g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = dphi_full(g, m0, g->ws_full, in_full, links, 1, "hirep_g5Dphi_sq (first g5 D)");
+    if (rc) return rc;
+    return dphi_full(g, m0, out_full, g->ws_full, links, 1, "hirep_g5Dphi_sq (second g5 D)");
+}
+
+extern "C" int hirep_sync(hirep_geom *g) {
+    if (!g) return fail(HIREP_EINVAL, "hirep_sync: NULL geometry");
+    cudaError_t e = cudaStreamSynchronize(g->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "hirep_sync");
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "hirep_sync (deferred)");
+    return HIREP_OK;
+}
+
+// ---- end-to-end host entry -------------------------------------------------------------------------
+extern "C" int hirep_apply_host(hirep_geom *g, int op, double m0, void *out_host, const void *in_host, const void *links_fund_host) {
+    if (!g || !out_host || !in_host) return fail(HIREP_EINVAL, "hirep_apply_host: NULL argument");
+    if (op < HIREP_OP_DPHI || op > HIREP_OP_G5DPHI_SQ) return fail(HIREP_EINVAL, "hirep_apply_host: unknown op %d", op);
+    const bool full = (op == HIREP_OP_DPHI || op == HIREP_OP_G5DPHI_SQ);
+    const size_t w = g->prec == HIREP_F64 ? 8 : 4;
+    const size_t V = (size_t)2 * g->geo.Nh;
+    const size_t canon_links = V * 4 * g->N * g->N * 2 * w;
+    const size_t canon_sp = (full ? V : V / 2) * 4 * g->dR * 2 * w;
+    const size_t native_sp = (full ? 2 : 1) * g->bytes_spinor_half;
+    if (!links_fund_host && !g->host_links_ready) return fail(HIREP_EINVAL, "hirep_apply_host: no links given and none resident");
+    int rc;
+    if ((rc = workspace(&g->h_links_rep, g->bytes_links_rep))) return rc;
+    if ((rc = workspace(&g->h_in_canon, V * 4 * g->dR * 2 * w))) return rc;
+    if ((rc = workspace(&g->h_out_canon, V * 4 * g->dR * 2 * w))) return rc;
+    if ((rc = workspace(&g->h_in_native, 2 * g->bytes_spinor_half))) return rc;
+    if ((rc = workspace(&g->h_out_native, 2 * g->bytes_spinor_half))) return rc;
+    cudaError_t e;
+    if (links_fund_host) {
+        if ((rc = workspace(&g->h_links_canon, canon_links))) return rc;
+        if ((rc = workspace(&g->h_links_fund, g->bytes_links_fund))) return rc;
+        e = cudaMemcpyAsync(g->h_links_canon, links_fund_host, canon_links, cudaMemcpyHostToDevice, g->stream);
+        if (e != cudaSuccess) return cuda_fail(e, "hirep_apply_host: links H2D");
+        if ((rc = hirep_links_import(g, g->h_links_fund, g->h_links_canon))) return rc;
+        if ((rc = hirep_links_to_rep(g, g->h_links_rep, g->h_links_fund))) return rc;
+        g->host_links_ready = 1;
+    }
+    e = cudaMemcpyAsync(g->h_in_canon, in_host, canon_sp, cudaMemcpyHostToDevice, g->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "hirep_apply_host: spinor H2D");
+    const int in_which = full ? HIREP_FULL : (op == HIREP_OP_DPHI_EO ? HIREP_ODD : HIREP_EVEN);
+    const int out_which = full ? HIREP_FULL : (op == HIREP_OP_DPHI_OE ? HIREP_ODD : HIREP_EVEN);
+    if ((rc = hirep_spinor_import(g, g->h_in_native, g->h_in_canon, in_which))) return rc;
+    const void *links = g->mode == HIREP_LINKS_STORED ? g->h_links_rep : g->h_links_fund;
+    switch (op) {
+    case HIREP_OP_DPHI: rc = hirep_Dphi(g, m0, g->h_out_native, g->h_in_native, links); break;
+    case HIREP_OP_DPHI_EO: rc = hirep_Dphi_eo(g, g->h_out_native, g->h_in_native, links); break;
+    case HIREP_OP_DPHI_OE: rc = hirep_Dphi_oe(g, g->h_out_native, g->h_in_native, links); break;
+    case HIREP_OP_DPHI_HAT: rc = hirep_Dphi_hat(g, m0, g->h_out_native, g->h_in_native, links); break;
+    default: rc = hirep_g5Dphi_sq(g, m0, g->h_out_native, g->h_in_native, links); break;
+    }
+    if (rc) return rc;
+    if ((rc = hirep_spinor_export(g, g->h_out_canon, g->h_out_native, out_which))) return rc;
+    e = cudaMemcpyAsync(out_host, g->h_out_canon, canon_sp, cudaMemcpyDeviceToHost, g->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "hirep_apply_host: result D2H");
+    (void)native_sp;
+    return hirep_sync(g);
+}

@@ -1,0 +1,51 @@
+// hop_dispatch.cuh -- maps (N_g, rep, mode, variant) to a stencil-kernel instantiation for one precision T.
+// Included by hop_f64.cu and hop_f32.cu so the two precisions compile in parallel.
+//
+// Variants (hirep_set_kernel_variant):  0 = library default for the instantiation
+//   1 = direct-load kernel, one thread per site          (hop_small.cuh, P = 1)
+//   2 = direct-load kernel, two lanes per site           (hop_small.cuh, P = 2)
+// Large d_R (>= 8) always uses the row-group kernel of hop_large.cuh.
+#pragma once
+#include "hop_large.cuh"
+
+namespace hirep {
+
+template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
+    constexpr bool f64 = sizeof(T) == 8;
+    if (variant == 0) variant = (f64 || DR >= 5) ? 2 : 1;
+    switch (variant) {
+    case 1: return launch_hop_small<T, DR, REAL, 1, 128>(g, L, s);
+    case 2: return launch_hop_small<T, DR, REAL, 2, 128>(g, L, s);
+    }
+    return KERR_UNSUPPORTED;
+}
+
+template <typename T> int hop_by_config(const Geo &g, int N, int rep, int mode, int variant, const HopLaunch &L, cudaStream_t s) {
+    if (mode != 0) return KERR_UNSUPPORTED;
+    const int dR = (rep == 0) ? N : (rep == 1) ? N * N - 1 : (rep == 2) ? N * (N + 1) / 2 : N * (N - 1) / 2;
+    const bool real = (rep == 1);
+    if (!real) {
+        switch (dR) {
+        case 2: return hop_small_variant<T, 2, false>(g, variant, L, s);
+        case 3: return hop_small_variant<T, 3, false>(g, variant, L, s);
+        case 4: return hop_small_variant<T, 4, false>(g, variant, L, s);
+        case 5: return hop_small_variant<T, 5, false>(g, variant, L, s);
+        case 6: return hop_small_variant<T, 6, false>(g, variant, L, s);
+        case 10: return variant == 0 ? launch_hop_large<T, 10, false, 5>(g, L, s) : KERR_UNSUPPORTED;
+        case 15: return variant == 0 ? launch_hop_large<T, 15, false, 5>(g, L, s) : KERR_UNSUPPORTED;
+        }
+    } else {
+        switch (dR) {
+        case 3: return hop_small_variant<T, 3, true>(g, variant, L, s);
+        case 8: return variant == 0 ? launch_hop_large<T, 8, true, 4>(g, L, s) : KERR_UNSUPPORTED;
+        case 15: return variant == 0 ? launch_hop_large<T, 15, true, 5>(g, L, s) : KERR_UNSUPPORTED;
+        case 35: return variant == 0 ? launch_hop_large<T, 35, true, 5>(g, L, s) : KERR_UNSUPPORTED;
+        }
+    }
+    return KERR_UNSUPPORTED;
+}
+
+int k_hop_f64(const Geo &g, int N, int rep, int mode, int variant, const HopLaunch &L, cudaStream_t s);
+int k_hop_f32(const Geo &g, int N, int rep, int mode, int variant, const HopLaunch &L, cudaStream_t s);
+
+}  // namespace hirep

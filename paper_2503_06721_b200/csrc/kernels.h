@@ -1,0 +1,35 @@
+// kernels.h -- host-side launchers (type-erased on precision / representation) used by api.cu.
+// Each returns 0, a positive cudaError_t, or KERR_UNSUPPORTED when the combination is not instantiated.
+#pragma once
+#include "common.cuh"
+
+namespace hirep {
+
+constexpr int KERR_UNSUPPORTED = -2;
+
+// one stencil pass over the sites of parity p_out:  out = a*self + b*hop(in)   (optionally times gamma_5)
+//   hop(in)(x) = sum_d P_d W_d(x) in(nbr_d(x)),  P_d = (1 -+ gamma_mu)        (the bracket of Eq 8)
+struct HopSet {
+    const void *in;     // spinor on parity 1-p_out
+    void *out;          // spinor on parity p_out
+    const void *self;   // spinor on parity p_out (may be null when a == 0)
+    const void *links;  // gather block of parity p_out: represented (stored) or fundamental (rebuild)
+    int p_out;
+};
+struct HopLaunch {
+    HopSet set[2];
+    int nsets;          // 1 = half lattice, 2 = both parities in one launch
+    double a, b;
+    int g5;             // multiply the result by gamma_5 = diag(1,1,-1,-1)
+};
+
+int k_spinor_import(const Geo &g, int prec, int dR, void *native, const void *canon, int which, cudaStream_t s);
+int k_spinor_export(const Geo &g, int prec, int dR, void *canon, const void *native, int which, cudaStream_t s);
+int k_links_import(const Geo &g, int prec, int N, void *native_fund, const void *canon, cudaStream_t s);
+int k_links_rep_export(const Geo &g, int prec, int dR, int real, void *canon, const void *native, int bwd, cudaStream_t s);
+int k_links_to_rep(const Geo &g, int prec, int N, int rep, void *native_rep, const void *native_fund, cudaStream_t s);
+// variant: 0 default; see hop_dispatch.cu.  mode: 0 stored represented links, 1 rebuild from fundamental (N, rep).
+int k_hop(const Geo &g, int prec, int N, int rep, int mode, int variant, const HopLaunch &L, cudaStream_t s);
+// number of distinct kernel launches k_hop issues for this configuration (for launch accounting): always 1.
+
+}  // namespace hirep

@@ -1,0 +1,256 @@
+"""Thin ctypes binding of libhirep_b200.so (C-ABI: include/hirep_b200.h).
+
+Argument marshalling only: every step of the path runs in the library's CUDA kernels.  torch supplies device
+memory (`tensor.data_ptr()`) and the stream.  Module-level functions carry the C names and take raw pointers;
+`Geometry` is a convenience wrapper that allocates native buffers as torch tensors.
+
+There is NO CPU fallback: `load()` raises if the shared library is missing, and every compute call raises
+`HirepError` with the library's message if CUDA is unavailable.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhirep_b200.so")
+
+FUND, ADJ, SYM, ASY = 0, 1, 2, 3
+F64, F32 = 0, 1
+EVEN, ODD, FULL = 0, 1, 2
+LINKS_STORED, LINKS_REBUILD = 0, 1
+OP_DPHI, OP_DPHI_EO, OP_DPHI_OE, OP_DPHI_HAT, OP_G5DPHI_SQ = 0, 1, 2, 3, 4
+
+# every symbol include/hirep_b200.h declares
+SYMBOLS = [
+    "hirep_geom_create", "hirep_geom_destroy", "hirep_geom_set_bc", "hirep_geom_set_stream", "hirep_geom_sizes",
+    "hirep_spinor_import", "hirep_spinor_export", "hirep_links_import", "hirep_links_rep_export",
+    "hirep_links_rep_export_bwd", "hirep_links_to_rep", "hirep_Dphi", "hirep_Dphi_eo", "hirep_Dphi_oe",
+    "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_launch_count",
+    "hirep_apply_host", "hirep_sync", "hirep_last_error",
+]
+
+
+class HirepError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load():
+    """dlopen the CUDA library and check that it exports every declared symbol.  Needs no GPU."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise HirepError(
+            "CUDA library %s not found: run `python __graft_entry__.py` (nvcc, sm_100a) first. "
+            "There is no CPU fallback." % LIB_PATH)
+    lib = ctypes.CDLL(LIB_PATH)
+    for name in SYMBOLS:
+        if not hasattr(lib, name):
+            raise HirepError("libhirep_b200.so does not export %s" % name)
+    vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+    lib.hirep_geom_create.argtypes = [ci, ci, ci, ci, ci, ctypes.POINTER(vp)]
+    lib.hirep_geom_destroy.argtypes = [vp]
+    lib.hirep_geom_set_bc.argtypes = [vp, ctypes.POINTER(ci)]
+    lib.hirep_geom_set_stream.argtypes = [vp, vp]
+    lib.hirep_geom_sizes.argtypes = [vp] + [ctypes.POINTER(ctypes.c_size_t)] * 4 + [ctypes.POINTER(ci)] * 2
+    for n in ("hirep_spinor_import", "hirep_spinor_export"):
+        getattr(lib, n).argtypes = [vp, vp, vp, ci]
+    for n in ("hirep_links_import", "hirep_links_rep_export", "hirep_links_rep_export_bwd", "hirep_links_to_rep"):
+        getattr(lib, n).argtypes = [vp, vp, vp]
+    for n in ("hirep_Dphi", "hirep_Dphi_hat", "hirep_g5Dphi_sq"):
+        getattr(lib, n).argtypes = [vp, cd, vp, vp, vp]
+    for n in ("hirep_Dphi_eo", "hirep_Dphi_oe"):
+        getattr(lib, n).argtypes = [vp, vp, vp, vp]
+    lib.hirep_set_link_mode.argtypes = [vp, ci]
+    lib.hirep_set_kernel_variant.argtypes = [vp, ci]
+    lib.hirep_launch_count.argtypes = [vp]
+    lib.hirep_launch_count.restype = ctypes.c_long
+    lib.hirep_apply_host.argtypes = [vp, ci, cd, vp, vp, vp]
+    lib.hirep_sync.argtypes = [vp]
+    lib.hirep_last_error.restype = ctypes.c_char_p
+    for n in SYMBOLS:
+        if n not in ("hirep_launch_count", "hirep_last_error"):
+            getattr(lib, n).restype = ci
+    _lib = lib
+    return lib
+
+
+def hirep_last_error() -> str:
+    return load().hirep_last_error().decode()
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise HirepError("hirep error %d: %s" % (rc, hirep_last_error()))
+
+
+# ---- same-name module-level functions (raw handles / pointers) -----------------------------------------
+def hirep_geom_create(T, L, N_g, rep, prec):
+    h = ctypes.c_void_p()
+    _check(load().hirep_geom_create(T, L, N_g, rep, prec, ctypes.byref(h)))
+    return h
+
+
+def hirep_geom_destroy(g):
+    _check(load().hirep_geom_destroy(g))
+
+
+def hirep_geom_set_bc(g, sign):
+    _check(load().hirep_geom_set_bc(g, (ctypes.c_int * 4)(*[int(s) for s in sign])))
+
+
+def hirep_geom_set_stream(g, cuda_stream):
+    _check(load().hirep_geom_set_stream(g, ctypes.c_void_p(cuda_stream)))
+
+
+def hirep_geom_sizes(g):
+    sz = [ctypes.c_size_t() for _ in range(4)]
+    d, r = ctypes.c_int(), ctypes.c_int()
+    _check(load().hirep_geom_sizes(g, *[ctypes.byref(s) for s in sz], ctypes.byref(d), ctypes.byref(r)))
+    return dict(spinor_full=sz[0].value, spinor_half=sz[1].value, links_fund=sz[2].value, links_rep=sz[3].value,
+                d_R=d.value, rep_is_real=bool(r.value))
+
+
+def hirep_spinor_import(g, native, canonical, which): _check(load().hirep_spinor_import(g, native, canonical, which))
+def hirep_spinor_export(g, canonical, native, which): _check(load().hirep_spinor_export(g, canonical, native, which))
+def hirep_links_import(g, native_fund, canonical_fund): _check(load().hirep_links_import(g, native_fund, canonical_fund))
+def hirep_links_rep_export(g, canonical_rep, native_rep): _check(load().hirep_links_rep_export(g, canonical_rep, native_rep))
+def hirep_links_rep_export_bwd(g, canonical_rep, native_rep): _check(load().hirep_links_rep_export_bwd(g, canonical_rep, native_rep))
+def hirep_links_to_rep(g, native_rep, native_fund): _check(load().hirep_links_to_rep(g, native_rep, native_fund))
+def hirep_Dphi(g, m0, out, inp, links): _check(load().hirep_Dphi(g, m0, out, inp, links))
+def hirep_Dphi_eo(g, out, inp, links): _check(load().hirep_Dphi_eo(g, out, inp, links))
+def hirep_Dphi_oe(g, out, inp, links): _check(load().hirep_Dphi_oe(g, out, inp, links))
+def hirep_Dphi_hat(g, m0, out, inp, links): _check(load().hirep_Dphi_hat(g, m0, out, inp, links))
+def hirep_g5Dphi_sq(g, m0, out, inp, links): _check(load().hirep_g5Dphi_sq(g, m0, out, inp, links))
+def hirep_set_link_mode(g, mode): _check(load().hirep_set_link_mode(g, mode))
+def hirep_set_kernel_variant(g, variant): _check(load().hirep_set_kernel_variant(g, variant))
+def hirep_launch_count(g): return int(load().hirep_launch_count(g))
+def hirep_sync(g): _check(load().hirep_sync(g))
+
+
+def hirep_apply_host(g, op, m0, out_host_ptr, in_host_ptr, links_host_ptr):
+    _check(load().hirep_apply_host(g, op, m0, out_host_ptr, in_host_ptr, links_host_ptr))
+
+
+# ---- convenience wrapper ---------------------------------------------------------------------------------
+class Geometry:
+    """Owns a hirep_geom handle; allocates native buffers as uint8 torch tensors on `device`."""
+
+    def __init__(self, T, L, N_g, rep, prec="f64", device=None, bc=None):
+        import torch
+        self.torch = torch
+        self.T, self.L, self.N_g, self.rep = T, L, N_g, rep
+        self.prec = {"f64": F64, "f32": F32}[prec] if isinstance(prec, str) else prec
+        self.device = torch.device(device if device is not None else "cuda:0")
+        self.handle = hirep_geom_create(T, L, N_g, rep, self.prec)
+        self.sizes = hirep_geom_sizes(self.handle)
+        self.d_R = self.sizes["d_R"]
+        self.cdtype = torch.complex128 if self.prec == F64 else torch.complex64
+        self.rdtype = torch.float64 if self.prec == F64 else torch.float32
+        self.V = T * L ** 3
+        if bc is not None:
+            hirep_geom_set_bc(self.handle, bc)
+        self.use_current_stream()
+
+    def __del__(self):
+        try:
+            if getattr(self, "handle", None):
+                hirep_geom_destroy(self.handle)
+                self.handle = None
+        except Exception:
+            pass
+
+    def use_current_stream(self):
+        if self.device.type == "cuda" and self.torch.cuda.is_available():
+            with self.torch.cuda.device(self.device):
+                hirep_geom_set_stream(self.handle, self.torch.cuda.current_stream().cuda_stream)
+
+    def _buf(self, nbytes):
+        return self.torch.empty(nbytes, dtype=self.torch.uint8, device=self.device)
+
+    def new_spinor(self, which=FULL):
+        return self._buf(self.sizes["spinor_full" if which == FULL else "spinor_half"])
+
+    def new_links_fund(self):
+        return self._buf(self.sizes["links_fund"])
+
+    def new_links_rep(self):
+        return self._buf(self.sizes["links_rep"])
+
+    # canonical <-> native
+    def spinor_import(self, canonical, which=FULL):
+        canonical = canonical.to(self.device, self.cdtype).contiguous()
+        n = self.V if which == FULL else self.V // 2
+        assert canonical.shape == (n, 4, self.d_R), canonical.shape
+        native = self.new_spinor(which)
+        hirep_spinor_import(self.handle, native.data_ptr(), canonical.data_ptr(), which)
+        return native
+
+    def spinor_export(self, native, which=FULL):
+        n = self.V if which == FULL else self.V // 2
+        canonical = self.torch.empty((n, 4, self.d_R), dtype=self.cdtype, device=self.device)
+        hirep_spinor_export(self.handle, canonical.data_ptr(), native.data_ptr(), which)
+        return canonical
+
+    def links_import(self, canonical_fund):
+        canonical_fund = canonical_fund.to(self.device, self.cdtype).contiguous()
+        assert canonical_fund.shape == (self.V, 4, self.N_g, self.N_g), canonical_fund.shape
+        native = self.new_links_fund()
+        hirep_links_import(self.handle, native.data_ptr(), canonical_fund.data_ptr())
+        return native
+
+    def links_to_rep(self, native_fund, out=None):
+        out = self.new_links_rep() if out is None else out
+        hirep_links_to_rep(self.handle, out.data_ptr(), native_fund.data_ptr())
+        return out
+
+    def links_rep_export(self, native_rep, bwd=False):
+        dt = self.rdtype if self.sizes["rep_is_real"] else self.cdtype
+        canonical = self.torch.empty((self.V, 4, self.d_R, self.d_R), dtype=dt, device=self.device)
+        (hirep_links_rep_export_bwd if bwd else hirep_links_rep_export)(self.handle, canonical.data_ptr(), native_rep.data_ptr())
+        return canonical
+
+    # operators (allocate `out` unless given)
+    def Dphi(self, m0, inp, links, out=None):
+        out = self.new_spinor(FULL) if out is None else out
+        hirep_Dphi(self.handle, m0, out.data_ptr(), inp.data_ptr(), links.data_ptr())
+        return out
+
+    def Dphi_eo(self, inp_odd, links, out=None):
+        out = self.new_spinor(EVEN) if out is None else out
+        hirep_Dphi_eo(self.handle, out.data_ptr(), inp_odd.data_ptr(), links.data_ptr())
+        return out
+
+    def Dphi_oe(self, inp_even, links, out=None):
+        out = self.new_spinor(ODD) if out is None else out
+        hirep_Dphi_oe(self.handle, out.data_ptr(), inp_even.data_ptr(), links.data_ptr())
+        return out
+
+    def Dphi_hat(self, m0, inp_even, links, out=None):
+        out = self.new_spinor(EVEN) if out is None else out
+        hirep_Dphi_hat(self.handle, m0, out.data_ptr(), inp_even.data_ptr(), links.data_ptr())
+        return out
+
+    def g5Dphi_sq(self, m0, inp, links, out=None):
+        out = self.new_spinor(FULL) if out is None else out
+        hirep_g5Dphi_sq(self.handle, m0, out.data_ptr(), inp.data_ptr(), links.data_ptr())
+        return out
+
+    def apply_host(self, op, m0, inp_host, links_host=None):
+        """End-to-end through hirep_apply_host: host (ideally pinned) canonical tensors in, host tensor out."""
+        out = self.torch.empty_like(inp_host)
+        if inp_host.is_pinned():
+            out = out.pin_memory()
+        hirep_apply_host(self.handle, op, m0, out.data_ptr(), inp_host.data_ptr(),
+                         links_host.data_ptr() if links_host is not None else None)
+        return out
+
+    def set_link_mode(self, mode): hirep_set_link_mode(self.handle, mode)
+    def set_kernel_variant(self, v): hirep_set_kernel_variant(self.handle, v)
+    def set_bc(self, sign): hirep_geom_set_bc(self.handle, sign)
+    def sync(self): hirep_sync(self.handle)
+    def launch_count(self): return hirep_launch_count(self.handle)

@@ -184,10 +184,17 @@ def make_inputs_torch(cfg: Config, device, dtype_complex, n_spinors: int = 1, ch
             u[:, 1, 0] = torch.complex(-a[:, 2], a[:, 1])
             u[:, 1, 1] = torch.complex(a[:, 0], -a[:, 3])
         elif cfg.links == "haar":
+            # Gram-Schmidt on the columns of a complex Gaussian matrix = the Q of its QR factorisation with
+            # diag(R) > 0, i.e. the numpy recipe above, but vectorised over the batch (two passes per column)
             z = torch.randn((n, N, N), generator=g, device=device, dtype=torch.complex128)
-            q, r = torch.linalg.qr(z)
-            d = torch.diagonal(r, dim1=1, dim2=2)
-            q = q * (d / d.abs())[:, None, :]
+            cols = []
+            for j in range(N):
+                v = z[:, :, j]
+                for _ in range(2):
+                    for qk in cols:
+                        v = v - (qk.conj() * v).sum(dim=1, keepdim=True) * qk
+                cols.append(v / v.norm(dim=1, keepdim=True))
+            q = torch.stack(cols, dim=2)
             det = torch.linalg.det(q)
             u = q * torch.exp(-1j * torch.angle(det) / N)[:, None, None]
         else:

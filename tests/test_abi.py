@@ -1,0 +1,106 @@
+"""CPU-only checks of the boundary: the library loads, exports every symbol include/hirep_b200.h declares, and
+its host-side logic (argument validation, sizes, error reporting) behaves as documented.  No compute calls."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def hirep():
+    import __graft_entry__ as ge
+    ge.build_cuda()
+    from paper_2503_06721_b200 import hirep as h
+    h.load()
+    return h
+
+
+def header_symbols():
+    text = open(os.path.join(ROOT, "include", "hirep_b200.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(hirep_[A-Za-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(hirep):
+    syms = header_symbols()
+    assert len(syms) >= 20
+    lib = ctypes.CDLL(hirep.LIB_PATH)
+    for s in syms:
+        assert hasattr(lib, s), s
+    assert sorted(hirep.SYMBOLS) == syms          # the Python binding lists exactly the header's functions
+
+
+def test_geom_create_validation_and_sizes(hirep):
+    for bad in [(3, 4, 3, 0, 0), (4, 5, 3, 0, 0), (0, 4, 3, 0, 0), (4, 4, 1, 0, 0), (4, 4, 7, 0, 0), (4, 4, 3, 9, 0), (4, 4, 3, 0, 5)]:
+        with pytest.raises(hirep.HirepError):
+            hirep.hirep_geom_create(*bad)
+    assert "N_g" in hirep.hirep_last_error() or "precision" in hirep.hirep_last_error()
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_geom_create(4, 4, 2, hirep.ASY, 0)       # d_R = 1: unsupported
+    # sizes: SU(3) FUND 32^4 fp64 (BASELINE configs[1]) -- SURVEY.md 8(a) table: 201 MB spinor, 604 MB links (x2 gather copies)
+    g = hirep.hirep_geom_create(32, 32, 3, hirep.FUND, hirep.F64)
+    sz = hirep.hirep_geom_sizes(g)
+    V = 32 ** 4
+    assert sz["d_R"] == 3 and not sz["rep_is_real"]
+    assert sz["spinor_full"] == V * 12 * 16 and sz["spinor_half"] * 2 == sz["spinor_full"]
+    assert sz["links_fund"] == 2 * (V // 2) * 8 * 9 * 16 == sz["links_rep"]
+    hirep.hirep_geom_destroy(g)
+    # SU(2) ADJ fp32: real links, d_R = 3; ragged lattice pads the last tile
+    g = hirep.hirep_geom_create(2, 6, 2, hirep.ADJ, hirep.F32)
+    sz = hirep.hirep_geom_sizes(g)
+    nh = 2 * 6 ** 3 // 2
+    ntiles = (nh + 31) // 32
+    assert sz["rep_is_real"] and sz["d_R"] == 3
+    assert sz["links_rep"] == 2 * ntiles * 8 * 9 * 32 * 4
+    assert sz["spinor_half"] == ntiles * 12 * 32 * 8
+    hirep.hirep_geom_destroy(g)
+
+
+@pytest.mark.parametrize("n,rep,d", [(2, 0, 2), (3, 0, 3), (2, 1, 3), (4, 3, 6), (6, 1, 35), (3, 2, 6), (4, 2, 10), (6, 3, 15)])
+def test_rep_dimensions_table1(hirep, n, rep, d):
+    g = hirep.hirep_geom_create(4, 4, n, rep, hirep.F64)
+    assert hirep.hirep_geom_sizes(g)["d_R"] == d            # Tbl 1
+    hirep.hirep_geom_destroy(g)
+
+
+def test_argument_errors_without_gpu(hirep):
+    g = hirep.hirep_geom_create(4, 4, 3, hirep.FUND, hirep.F64)
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_geom_set_bc(g, (1, 1, 0, 1))
+    hirep.hirep_geom_set_bc(g, (1, -1, 1, 1))
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_set_link_mode(g, 7)
+    # null / misaligned / aliased pointers are rejected before any CUDA call
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_Dphi_eo(g, None, 4096, 8192)
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_Dphi_eo(g, 4096 + 8, 8192, 16384)
+    assert "aligned" in hirep.hirep_last_error()
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_Dphi(g, 0.1, 4096, 4096, 8192)
+    assert "alias" in hirep.hirep_last_error()
+    assert hirep.hirep_launch_count(g) == 0
+    hirep.hirep_geom_destroy(g)
+    hirep.hirep_geom_destroy(None)
+
+
+def test_missing_library_fails_loudly(hirep, monkeypatch):
+    """The product path must not fall back to anything when the CUDA library is absent."""
+    monkeypatch.setattr(hirep, "_lib", None)
+    monkeypatch.setattr(hirep, "LIB_PATH", os.path.join(ROOT, "no_such_dir", "libhirep_b200.so"))
+    with pytest.raises(hirep.HirepError, match="no CPU fallback"):
+        hirep.load()
+
+
+def test_product_does_not_import_oracle():
+    """Neither the package nor bench's product arm may route through oracle/ (checked textually on the package)."""
+    pkg = os.path.join(ROOT, "paper_2503_06721_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                for needle in ("import oracle", "from oracle", "liboracle", "hirep_oracle", "oracle/"):
+                    assert needle not in src, (needle, os.path.join(dirpath, f))
