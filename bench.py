@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of the Wilson-Dirac hot path (arXiv 2503.06721) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--prec f64] [--variant 0] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over one set of synthetic fields:
+    links_to_rep, Dphi_eo, Dphi_oe, Dphi, Dphi_hat, g5Dphi_sq            (8 stencil passes + 1 link build)
+Default workload: BASELINE.json configs[1] -- SU(3) fundamental, 32^4, fp64 (the configuration the metric is quoted on).
+`value` = algorithmic GFLOP (SURVEY.md 8(d) flop model) per step / device time per step, inputs resident in HBM.
+`roofline` = the dominant kernel (the Dphi_eo stencil pass): compulsory bytes (2S+8K per output site) / its own
+CUDA-event duration, against the measured copy bandwidth of MEASURED_PEAKS.json.
+`e2e` = the same step through hirep_apply_host with pinned HOST buffers (H2D of links+spinors, D2H of results, timed).
+`cpu_baseline` = the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+`--impl reference` times the oracle alone (this tier's reference arm).  N > 1: independent replicas.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "Dphi_eo GFLOP/s & effective HBM GB/s (fraction of B200 peak), per N_g/rep"
+
+
+# ------------------------------------------------------------------------------- cost model
+def cost_model(cfg, prec):
+    d = cfg.d_R
+    real = cfg.rep == 1
+    w = 8 if prec == "f64" else 4
+    S = 8 * d * w                                  # one spinor
+    K = d * d * (1 if real else 2) * w             # one represented link
+    KF = 2 * cfg.n_g ** 2 * w
+    F_hop = (64 if real else 128) * d * d + 56 * d
+    V = cfg.volume
+    ops = {
+        # name: (flops, compulsory bytes as executed by this library's link layout, paper-ideal compulsory bytes)
+        "Dphi_eo": (F_hop * V / 2, (2 * S + 8 * K) * V / 2, (2 * S + 8 * K) * V / 2),
+        "Dphi_oe": (F_hop * V / 2, (2 * S + 8 * K) * V / 2, (2 * S + 8 * K) * V / 2),
+        "Dphi": ((F_hop + 16 * d) * V, (2 * S + 8 * K) * V, (2 * S + 4 * K) * V),
+        "Dphi_hat": ((2 * F_hop + 16 * d) * V / 2, (5 * S + 16 * K) * V / 2, (5 * S + 16 * K) * V / 2),
+        "g5Dphi_sq": (2 * (F_hop + 16 * d) * V, 2 * (2 * S + 8 * K) * V, 2 * (2 * S + 4 * K) * V),
+        "links_to_rep": (0.0, 8 * V * (KF + K), 4 * V * (KF + K)),
+    }
+    return dict(S=S, K=K, KF=KF, F_hop=F_hop, ops=ops)
+
+
+OP_ORDER = ["links_to_rep", "Dphi_eo", "Dphi_oe", "Dphi", "Dphi_hat", "g5Dphi_sq"]
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi sampling during the timed region (B200_PROFILING.md 'clocks line')."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); smax = float(f[2])
+            except ValueError:
+                continue
+            for name, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# -------------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    from paper_2503_06721_b200 import hirep, synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    hirep.load()
+
+    cfg = synth.CONFIGS[args.config]
+    prec = args.prec
+    cm = cost_model(cfg, prec)
+    cdt = torch.complex128 if prec == "f64" else torch.complex64
+    links_c, (psi_c,) = synth.make_inputs_torch(cfg, dev, cdt, n_spinors=1)
+    geom = hirep.Geometry(cfg.T, cfg.L, cfg.n_g, cfg.rep, prec, device=dev)
+    geom.set_kernel_variant(args.variant)
+    lf = geom.links_import(links_c)
+    lr = geom.new_links_rep()
+    x_full = geom.spinor_import(psi_c, hirep.FULL)
+    hb = geom.sizes["spinor_half"]
+    x_e, x_o = x_full[:hb], x_full[hb:]
+    y_full, y_e, y_o = geom.new_spinor(hirep.FULL), geom.new_spinor(hirep.EVEN), geom.new_spinor(hirep.ODD)
+    m0 = cfg.m0
+    ev = {k: [] for k in OP_ORDER}
+
+    def timed(name, fn, record):
+        if record:
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record()
+            ev[name].append((a, b))
+        else:
+            fn()
+
+    def step(record=False):
+        timed("links_to_rep", lambda: geom.links_to_rep(lf, out=lr), record)
+        timed("Dphi_eo", lambda: geom.Dphi_eo(x_o, lr, out=y_e), record)
+        timed("Dphi_oe", lambda: geom.Dphi_oe(x_e, lr, out=y_o), record)
+        timed("Dphi", lambda: geom.Dphi(m0, x_full, lr, out=y_full), record)
+        timed("Dphi_hat", lambda: geom.Dphi_hat(m0, x_e, lr, out=y_e), record)
+        timed("g5Dphi_sq", lambda: geom.g5Dphi_sq(m0, x_full, lr, out=y_full), record)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = geom.launch_count()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0.record()
+    for _ in range(args.steps):
+        step(record=True)
+    t1.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = t0.elapsed_time(t1)
+    launches = geom.launch_count() - launches0
+    if dist is not None:
+        tt = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    ms_step = ms_total / args.steps
+
+    flops_step = sum(cm["ops"][k][0] for k in OP_ORDER)
+    value = world * flops_step / (ms_step * 1e-3) / 1e9
+    peak, peak_src = peaks()
+    per_op = {}
+    for k in OP_ORDER:
+        ms = sum(a.elapsed_time(b) for a, b in ev[k]) / len(ev[k])
+        fl, by, by_ideal = cm["ops"][k]
+        per_op[k] = {"ms": round(ms, 4), "gflops": round(fl / ms / 1e6, 1), "gbs": round(by / ms / 1e6, 1),
+                     "frac_hbm": round(by / ms / 1e6 / peak, 4), "gbs_paper_ideal_bytes": round(by_ideal / ms / 1e6, 1)}
+    eo = per_op["Dphi_eo"]
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get("%s_%s" % (args.config, prec), {}).get("Dphi_eo_dram_bytes")
+    roofline = {"bound": "hbm", "kernel": "hop stencil (Dphi_eo pass)", "achieved": eo["gbs"], "peak": peak,
+                "unit": "GB/s", "frac": round(eo["gbs"] / peak, 4), "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes": cm["ops"]["Dphi_eo"][1], "frac_of_8TBs_nominal": round(eo["gbs"] / 8000.0, 4)}
+
+    # ---- e2e: same step through hirep_apply_host with pinned host buffers
+    e2e = None
+    if not args.no_e2e:
+        links_h = links_c.cpu().pin_memory()
+        psi_h = psi_c.cpu().pin_memory()
+        idx = torch.arange(cfg.volume)
+        par = ((idx // cfg.L ** 3) + (idx // cfg.L ** 2) % cfg.L + (idx // cfg.L) % cfg.L + idx % cfg.L) % 2
+        psi_e_h = psi_h[par == 0].contiguous().pin_memory()
+        psi_o_h = psi_h[par == 1].contiguous().pin_memory()
+        outs = {k: torch.empty_like(v).pin_memory() for k, v in (("f", psi_h), ("e", psi_e_h), ("o", psi_o_h))}
+        H = hirep
+
+        def host_step():
+            h = geom.handle
+            H.hirep_apply_host(h, H.OP_DPHI_EO, m0, outs["e"].data_ptr(), psi_o_h.data_ptr(), links_h.data_ptr())
+            H.hirep_apply_host(h, H.OP_DPHI_OE, m0, outs["o"].data_ptr(), psi_e_h.data_ptr(), None)
+            H.hirep_apply_host(h, H.OP_DPHI, m0, outs["f"].data_ptr(), psi_h.data_ptr(), None)
+            H.hirep_apply_host(h, H.OP_DPHI_HAT, m0, outs["e"].data_ptr(), psi_e_h.data_ptr(), None)
+            H.hirep_apply_host(h, H.OP_G5DPHI_SQ, m0, outs["f"].data_ptr(), psi_h.data_ptr(), None)
+
+        nb = lambda t: t.numel() * t.element_size()
+        h2d = nb(links_h) + 2 * nb(psi_h) + 2 * nb(psi_e_h) + nb(psi_o_h)
+        d2h = 2 * nb(psi_h) + 2 * nb(psi_e_h) + nb(psi_o_h)
+        ksteps = max(1, min(args.steps, 3))
+        host_step()
+        barrier()
+        w0 = time.perf_counter()
+        for _ in range(ksteps):
+            host_step()
+        torch.cuda.synchronize()
+        w1 = time.perf_counter()
+        ms_e2e = (w1 - w0) * 1e3 / ksteps
+        if dist is not None:
+            tt = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            ms_e2e = float(tt.item())
+        e2e = {"value": round(world * flops_step / (ms_e2e * 1e-3) / 1e9, 2), "unit": "GFLOP/s", "ms_per_step": round(ms_e2e, 3),
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": ksteps,
+               "api": "hirep_apply_host (pinned host canonical buffers; links copied once per step)"}
+        del links_h, psi_h
+
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(args.config, prec)
+
+    if rank == 0:
+        out = {
+            "metric": METRIC, "value": round(value, 1), "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": prec, "data": "synthetic",
+            "config": {"workload": "%s: SU(%d) %s (d_R=%d) %dx%d^3 %s; step = links_to_rep + Dphi_eo + Dphi_oe + Dphi + Dphi_hat + g5Dphi_sq"
+                                   % (cfg.name, cfg.n_g, synth.REP_NAMES[cfg.rep], cfg.d_R, cfg.T, cfg.L, prec),
+                       "links": "stored represented links (gather layout)", "kernel_variant": args.variant,
+                       "l2": "inputs larger than L2: each step streams %.2f GB of links and spinors (L2 = 126 MB)"
+                             % (sum(cm["ops"][k][1] for k in OP_ORDER) / 1e9),
+                       "parallelism": "replicas x%d (no sharding; DESIGN.md)" % world},
+            "gpu_launches": launches,
+            "per_op": per_op,
+            "roofline": roofline,
+            "e2e": e2e,
+            "cpu_baseline": cpu,
+            "clocks": clocks,
+        }
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------- oracle arm / cpu baseline
+def prepare_sample(config, prec, T, L):
+    from paper_2503_06721_b200 import synth
+    cfg = synth.CONFIGS[config].resized(T, L)
+    U, (psi,) = synth.make_inputs(cfg)
+    U, psi = synth.round_to_precision(U, prec), synth.round_to_precision(psi, prec)
+    return cfg, U, psi, synth.parity_sites(T, L, 0), synth.parity_sites(T, L, 1)
+
+
+def oracle_step(prep):
+    """One step (the same six ops) of the oracle, as it stands, on the prepared sample; returns seconds."""
+    from oracle import oracle as orc
+    cfg, U, psi, ev, od = prep
+    T, L, d, m0 = cfg.T, cfg.L, cfg.d_R, cfg.m0
+    t0 = time.perf_counter()
+    R = orc.represent_field(cfg.n_g, cfg.rep, U)
+    orc.Dphi_eo(T, L, d, R, psi[od]); orc.Dphi_oe(T, L, d, R, psi[ev]); orc.Dphi(T, L, d, m0, R, psi)
+    orc.Dphi_hat(T, L, d, m0, R, psi[ev]); orc.g5Dphi_sq(T, L, d, m0, R, psi)
+    return time.perf_counter() - t0
+
+
+def sample_flops(prep):
+    cm = cost_model(prep[0], "f64")
+    return sum(cm["ops"][k][0] for k in OP_ORDER)
+
+
+SAMPLE = {"C1": (4, 4), "C2": (16, 16), "C3": (16, 16), "C4": (8, 8), "C5": (4, 4)}
+
+
+def cpu_baseline(config, prec):
+    from oracle import oracle as orc
+    T, L = SAMPLE[config]
+    prep = prepare_sample(config, prec, T, L)
+    secs = oracle_step(prep)
+    return {"value": round(sample_flops(prep) / secs / 1e9, 3), "unit": "GFLOP/s", "cores": orc.num_threads(), "kind": "oracle",
+            "sample": "one step (same six ops) of %s on a %dx%d^3 sub-lattice, %.1f s" % (config, T, L, secs)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    from paper_2503_06721_b200 import synth
+    T, L = SAMPLE[args.config]
+    prep = prepare_sample(args.config, args.prec, T, L)
+    for _ in range(min(args.warmup, 1)):
+        oracle_step(prep)
+    secs = [oracle_step(prep) for _ in range(args.steps)]
+    ms_step = sum(secs) * 1e3 / len(secs)
+    gf = sample_flops(prep) / (ms_step * 1e-3) / 1e9
+    cores, cfg = orc.num_threads(), synth.CONFIGS[args.config]
+    sample = "one step (same six ops) of %s on a %dx%d^3 sub-lattice" % (args.config, T, L)
+    out = {"impl": "reference", "metric": METRIC, "value": round(gf, 3), "unit": "GFLOP/s", "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms_step, 2), "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": "%s: SU(%d) %s (d_R=%d) %dx%d^3 %s; step = links_to_rep + Dphi_eo + Dphi_oe + Dphi + Dphi_hat + g5Dphi_sq"
+                                  % (cfg.name, cfg.n_g, synth.REP_NAMES[cfg.rep], cfg.d_R, cfg.T, cfg.L, args.prec),
+                      "sample": sample},
+           "gpu_launches": 0,
+           "cpu_baseline": {"value": round(gf, 3), "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
+           "e2e": {"value": round(gf, 3), "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

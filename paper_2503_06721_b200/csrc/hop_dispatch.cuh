@@ -11,8 +11,7 @@
 namespace hirep {
 
 template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
-    constexpr bool f64 = sizeof(T) == 8;
-    if (variant == 0) variant = (f64 || DR >= 5) ? 2 : 1;
+    if (variant == 0) variant = 1;   // measured on B200 (profiles/): one thread per site wins for every d_R <= 6
     switch (variant) {
     case 1: return launch_hop_small<T, DR, REAL, 1, 128>(g, L, s);
     case 2: return launch_hop_small<T, DR, REAL, 2, 128>(g, L, s);
