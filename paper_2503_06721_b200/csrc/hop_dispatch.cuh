@@ -4,17 +4,24 @@
 // Variants (hirep_set_kernel_variant):  0 = library default for the instantiation
 //   1 = direct-load kernel, one thread per site          (hop_small.cuh, P = 1)
 //   2 = direct-load kernel, two lanes per site           (hop_small.cuh, P = 2)
-// Large d_R (>= 8) always uses the row-group kernel of hop_large.cuh.
+//   3 = persistent kernel, link stream through a per-warp bulk-copy (TMA) ring in shared memory (hop_ring.cuh)
+// Default for d_R <= 6: variant 3 (measured on B200, profiles/).  Large d_R (>= 8) always uses the row-group
+// kernel of hop_large.cuh.
 #pragma once
 #include "hop_large.cuh"
+#include "hop_ring.cuh"
 
 namespace hirep {
 
 template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
-    if (variant == 0) variant = 1;   // measured on B200 (profiles/): one thread per site wins for every d_R <= 6
+    if (variant == 0) variant = 3;
     switch (variant) {
     case 1: return launch_hop_small<T, DR, REAL, 1, 128>(g, L, s);
     case 2: return launch_hop_small<T, DR, REAL, 2, 128>(g, L, s);
+    case 3: {
+        using P = RingPick<T, DR, REAL>;
+        return launch_hop_ring<T, DR, REAL, P::WARPS, P::STAGES, P::RPC>(g, L, s);
+    }
     }
     return KERR_UNSUPPORTED;
 }

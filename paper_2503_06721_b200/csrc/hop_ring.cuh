@@ -1,0 +1,275 @@
+// hop_ring.cuh -- the Wilson hopping stencil for small d_R with the link stream staged through shared memory
+// by the bulk-copy engine (TMA, cp.async.bulk) -- the sm_100a kernel of this library.
+//
+//   out(x) = a*self(x) + b * sum_{d=0..7} P_d W_d(x) in(nbr_d(x)),   x of parity p_out            (Eq 8)
+//
+// Same arithmetic as hop_small.cuh (spin projection to half spinors, d_R x d_R link matvec, reconstruction; steps
+// a2-a4 of SURVEY.md 8(a)); what differs is how the bytes move:
+//   * The kernel is persistent: one CTA per SM, WARPS warps per CTA, one warp = one tile of 32 sites at a time,
+//     tiles dealt round-robin over all warps of the grid (neighbouring tiles run at the same time on different SMs,
+//     which is what makes the 8-fold spinor reuse hit in L2).
+//   * The 8 link matrices of a tile are ONE contiguous block in the gather layout (common.cuh).  Each warp owns a
+//     ring of STAGES shared-memory slots of RPC link-matrix rows each (RPC x d_R x 32 lanes) and keeps it full with
+//     cp.async.bulk (global -> shared, completion on an mbarrier, L2 evict_first: links are streamed once).  The
+//     bytes in flight per SM are WARPS x (STAGES-1) x slot and cost no registers, so the link stream (75 % of the
+//     traffic at SU(3)) no longer depends on occupancy.  The ring runs across tile boundaries.
+//   * Neighbour spinors are gathered with plain 128-bit read-only loads; the loads of direction d+1 are issued
+//     right after direction d has been projected (the projection frees the registers), so they fly during the
+//     link matvec of direction d.  At direction 7 the first neighbour of the warp's next tile is fetched.
+// No CTA-wide barrier anywhere: every warp is its own producer/consumer pipeline (lane 0 issues the bulk copies).
+#pragma once
+#include "hop_small.cuh"
+
+namespace hirep {
+
+// ---- PTX wrappers (mbarrier + bulk async copy, PTX ISA 8.x, sm_90+) ---------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar, uint64_t pol) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol)
+        : "memory");
+}
+
+// ring geometry for one instantiation; CHUNK = RPC rows of the link block of one direction of one tile
+template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC = DR> struct RingCfg {
+    using E = link_elem<T, REAL>;
+    static constexpr int NE = DR * DR;
+    static constexpr int CPD = DR / RPC;                            // chunks per direction
+    static constexpr uint32_t CHUNK = RPC * DR * TILE * sizeof(E);  // RPC rows of one link matrix, 32 lanes
+    static_assert(DR % RPC == 0, "rows per chunk must divide d_R");
+    static constexpr size_t RING_BYTES = (size_t)WARPS * STAGES * CHUNK;
+    static constexpr size_t SMEM = RING_BYTES + (size_t)WARPS * STAGES * sizeof(uint64_t);
+    static_assert(CHUNK % 16 == 0, "bulk copies move multiples of 16 bytes");
+    static_assert(SMEM <= 227 * 1024, "ring does not fit the 227 KB of shared memory of an sm_100 CTA");
+};
+
+// Library default ring shape per instantiation, from the B200 sweeps recorded in profiles/ (r01_ring_sweep.md):
+//   fp64: 8 warps (the thread-per-site kernel needs ~200 registers); fp32: 16 warps for d_R <= 3, else 12;
+//   chunk = the largest whole number of link rows that divides d_R and stays <= 13 KB; 2..4 stages as smem allows.
+template <typename T, int DR, bool REAL> struct RingPick {
+    using E = link_elem<T, REAL>;
+    static constexpr int WARPS = sizeof(T) == 4 ? (DR <= 3 ? 16 : 12) : 8;
+    static constexpr int pick_rpc() {
+        int best = 1;
+        for (int r = 1; r <= DR; ++r)
+            if (DR % r == 0 && (size_t)r * DR * TILE * sizeof(E) <= 13 * 1024) best = r;
+        return best;
+    }
+    static constexpr int RPC = pick_rpc();
+    static constexpr size_t CHUNK = (size_t)RPC * DR * TILE * sizeof(E);
+    static constexpr int pick_stages() {
+        int st = (int)((226 * 1024) / (WARPS * (CHUNK + 8)));
+        return st > 4 ? 4 : st;
+    }
+    static constexpr int STAGES = pick_stages();
+    static_assert(STAGES >= 2, "ring needs at least two stages");
+};
+
+template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC = DR>
+__global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, const HopLaunch L) {
+    using C = cplx<T>;
+    using E = link_elem<T, REAL>;
+    using Cfg = RingCfg<T, DR, REAL, WARPS, STAGES, RPC>;
+    constexpr int NC = 4 * DR, CPD = Cfg::CPD, CPT = 8 * CPD;   // chunks per direction / per tile
+    constexpr int CE = RPC * DR * TILE;                         // link elements per chunk
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const E *ring = reinterpret_cast<const E *>(smem_raw + (size_t)warp * STAGES * Cfg::CHUNK);
+    const uint32_t ring_s = smem_u32(ring);
+    const uint32_t bars_s = smem_u32(smem_raw + Cfg::RING_BYTES) + warp * STAGES * 8;
+    if (lane == 0) {
+        for (int s = 0; s < STAGES; ++s) mbar_init(bars_s + 8 * s, 1);
+        fence_mbar_init();
+    }
+    __syncwarp();
+
+    // full-lattice launches (nsets = 2) interleave the two parities tile by tile: the `self` spinor of an even tile is
+    // the neighbour data of the odd tiles processed at the same time, so it is served by L2
+    const bool two = L.nsets == 2;
+    const int total_tiles = g.n_tiles * L.nsets;
+    const int gw = blockIdx.x * WARPS + warp, nw = gridDim.x * WARPS;
+    if (gw >= total_tiles) return;
+    const int my_tiles = (total_tiles - gw + nw - 1) / nw;
+    const int my_chunks = my_tiles * CPT;
+    const uint64_t pol = l2_policy_evict_first();
+
+    // chunk q of this warp = chunk q % CPT of its (q / CPT)-th tile; a tile's chunks are consecutive in memory
+    auto issue = [&](int q, int slot) {
+        const int gt = gw + (q / CPT) * nw;
+        const int set = two ? (gt & 1) : 0;
+        const int tile = two ? (gt >> 1) : gt;
+        const E *src = (const E *)(set ? L.set[1].links : L.set[0].links) + ((size_t)tile * CPT + (q % CPT)) * CE;
+        mbar_expect_tx(bars_s + 8 * slot, Cfg::CHUNK);
+        bulk_g2s(ring_s + slot * Cfg::CHUNK, src, Cfg::CHUNK, bars_s + 8 * slot, pol);
+    };
+    if (lane == 0) {
+        const int n0 = my_chunks < STAGES ? my_chunks : STAGES;
+        for (int q = 0; q < n0; ++q) issue(q, q);
+    }
+
+    // per-tile state
+    int set, tile, t, x, y, zh, p_out;
+    bool active;
+    const C *in;
+    auto enter_tile = [&](int k) {
+        const int gt = gw + k * nw;
+        set = two ? (gt & 1) : 0;
+        tile = two ? (gt >> 1) : gt;
+        int h = tile * TILE + lane;
+        active = h < g.Nh;
+        if (!active) h = g.Nh - 1;
+        decode_site(g, h, t, x, y, zh);
+        p_out = set ? L.set[1].p_out : L.set[0].p_out;   // selects, not L.set[set]: dynamic indexing would copy the
+        in = (const C *)(set ? L.set[1].in : L.set[0].in);   // kernel parameters to local memory
+    };
+    C nb[NC];
+    auto fetch = [&](int hn) {
+        const C *src = in + ((size_t)(hn >> 5) * NC) * TILE + (hn & 31);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) nb[c] = ld_spinor<T>(src + (size_t)c * TILE);
+    };
+
+    enter_tile(0);
+    fetch(neighbour<0>(g, p_out, t, x, y, zh));
+    int q = 0, slot = 0;
+    uint32_t phase = 0;
+    const T a = (T)L.a, b = (T)L.b;
+    const T g5s = L.g5 ? T(-1) : T(1);
+
+    for (int k = 0; k < my_tiles; ++k) {
+        // state of the tile being computed (enter_tile(k+1) below overwrites the shared variables at d = 7)
+        const int c_set = set, c_tile = tile;
+        const bool c_active = active;
+        C up[2][DR], lo[2][DR];
+#pragma unroll
+        for (int s = 0; s < 2; ++s)
+#pragma unroll
+            for (int c = 0; c < DR; ++c) up[s][c] = lo[s][c] = mk<T>(0, 0);
+
+        static_for<0, 8>([&](auto dc) {
+            constexpr int D = decltype(dc)::value;
+            using DI = DirInfo<D>;
+            // (a2) spin projection of the neighbour fetched earlier
+            C hs[2][DR];
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                const int qq = DI::swap ? 1 - s : s;
+                const T cs = (T)(DI::sg * DI::sigma(s));
+#pragma unroll
+                for (int c = 0; c < DR; ++c) {
+                    const C u = nb[s * DR + c], v = nb[(2 + qq) * DR + c];
+                    if (DI::imag) hs[s][c] = mk<T>(fma(-cs, v.y, u.x), fma(cs, v.x, u.y));   // u + i cs v
+                    else hs[s][c] = mk<T>(fma(cs, v.x, u.x), fma(cs, v.y, u.y));             // u + cs v
+                }
+            }
+            // prefetch the next neighbour (next direction, or direction 0 of this warp's next tile)
+            if constexpr (D < 7) {
+                fetch(neighbour<D + 1>(g, p_out, t, x, y, zh));
+            } else {
+                if (k + 1 < my_tiles) {
+                    enter_tile(k + 1);
+                    fetch(neighbour<0>(g, p_out, t, x, y, zh));
+                }
+            }
+            // (a3) link matvec from the ring, (a4) reconstruct + accumulate
+#pragma unroll
+            for (int i = 0; i < DR; ++i) {
+                if (i % RPC == 0) mbar_wait(bars_s + 8 * slot, phase);
+                const E *W = ring + (size_t)slot * CE + lane;
+                E w[DR];
+#pragma unroll
+                for (int j = 0; j < DR; ++j) w[j] = W[((i % RPC) * DR + j) * TILE];
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    C chi = mk<T>(0, 0);
+#pragma unroll
+                    for (int j = 0; j < DR; ++j) mac<T>(chi, w[j], hs[s][j]);
+                    up[s][i].x += chi.x;
+                    up[s][i].y += chi.y;
+                    const T cl = (T)(DI::sg * DI::sigma(s));
+                    const int qq = DI::swap ? 1 - s : s;
+                    if (DI::imag) { lo[qq][i].x += cl * chi.y; lo[qq][i].y -= cl * chi.x; }   // (-i cl) chi
+                    else { lo[qq][i].x += cl * chi.x; lo[qq][i].y += cl * chi.y; }
+                }
+                if (i % RPC == RPC - 1) {
+                    // slot consumed by every lane -> refill it with the chunk STAGES ahead
+                    __syncwarp();
+                    if (lane == 0 && q + STAGES < my_chunks) issue(q + STAGES, slot);
+                    ++q;
+                    if (++slot == STAGES) { slot = 0; phase ^= 1; }
+                }
+            }
+        });
+
+        if (c_active) {
+            C *__restrict__ out = (C *)(c_set ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
+            const C *self_base = (const C *)(c_set ? L.set[1].self : L.set[0].self);
+            const C *__restrict__ self = self_base + ((size_t)c_tile * NC) * TILE + lane;
+            const bool use_self = (self_base != nullptr) && (L.a != 0.0);
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+#pragma unroll
+                for (int c = 0; c < DR; ++c) {
+                    C vu = mk<T>(b * up[s][c].x, b * up[s][c].y);
+                    C vl = mk<T>(b * lo[s][c].x, b * lo[s][c].y);
+                    if (use_self) {
+                        const C su = self[(size_t)(s * DR + c) * TILE];
+                        const C sl = self[(size_t)((2 + s) * DR + c) * TILE];
+                        vu.x = fma(a, su.x, vu.x); vu.y = fma(a, su.y, vu.y);
+                        vl.x = fma(a, sl.x, vl.x); vl.y = fma(a, sl.y, vl.y);
+                    }
+                    out[(size_t)(s * DR + c) * TILE] = vu;
+                    out[(size_t)((2 + s) * DR + c) * TILE] = mk<T>(g5s * vl.x, g5s * vl.y);
+                }
+        }
+    }
+}
+
+template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC = DR>
+int launch_hop_ring(const Geo &g, const HopLaunch &L, cudaStream_t s) {
+    using Cfg = RingCfg<T, DR, REAL, WARPS, STAGES, RPC>;
+    auto kern = hop_ring_kernel<T, DR, REAL, WARPS, STAGES, RPC>;
+    static int n_sm = 0;
+    if (n_sm == 0) {
+        int dev = 0, sms = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        if (e != cudaSuccess) return (int)e;
+        n_sm = sms;
+    }
+    const int total_tiles = g.n_tiles * L.nsets;
+    int grid = (total_tiles + WARPS - 1) / WARPS;
+    if (grid > n_sm) grid = n_sm;
+    kern<<<grid, WARPS * 32, Cfg::SMEM, s>>>(g, L);
+    return (int)cudaGetLastError();
+}
+
+}  // namespace hirep

@@ -154,7 +154,7 @@ def test_operators_vs_oracle_reduced(env, name, T, L, prec):
 
 @pytest.mark.parametrize("name,T,L", [("C1", 4, 4), ("C2", 6, 6), ("C3", 2, 6), ("C4", 4, 6)])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 def test_kernel_variants(env, name, T, L, prec, variant):
     p = Problem(env, synth.CONFIGS[name].resized(T, L), prec)
     check_all_ops(env, p, variant)
