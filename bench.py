@@ -135,6 +135,8 @@ def run_ours(args):
     links_c, (psi_c,) = synth.make_inputs_torch(cfg, dev, cdt, n_spinors=1)
     geom = hirep.Geometry(cfg.T, cfg.L, cfg.n_g, cfg.rep, prec, device=dev)
     geom.set_kernel_variant(args.variant)
+    if args.bx != -1:
+        geom.set_tuning(hirep.TUNE_TILE_BLOCK, args.bx)
     lf = geom.links_import(links_c)
     lr = geom.new_links_rep()
     x_full = geom.spinor_import(psi_c, hirep.FULL)
@@ -348,6 +350,7 @@ def main():
     ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--bx", type=int, default=-1, help="tile traversal x-block (hirep_set_tuning); -1 = library default")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -34,6 +34,15 @@ template <typename T, bool REAL> using link_elem = std::conditional_t<REAL, T, c
 
 template <typename T> __host__ __device__ inline cplx<T> mk(T re, T im) { cplx<T> r; r.x = re; r.y = im; return r; }
 
+// compile-time loop: f(IntC<B>{}), ..., f(IntC<E-1>{})
+template <int I> struct IntC { static constexpr int value = I; };
+template <int B, int E, typename F> __device__ __forceinline__ void static_for(F &&f) {
+    if constexpr (B < E) {
+        f(IntC<B>{});
+        static_for<B + 1, E>(f);
+    }
+}
+
 // ---- site <-> coordinates ------------------------------------------------------------------
 __host__ __device__ inline void decode_site(const Geo &g, int h, int &t, int &x, int &y, int &zh) {
     zh = h % g.Lh;

@@ -5,24 +5,42 @@
 //   1 = direct-load kernel, one thread per site          (hop_small.cuh, P = 1)
 //   2 = direct-load kernel, two lanes per site           (hop_small.cuh, P = 2)
 //   3 = persistent kernel, link stream through a per-warp bulk-copy (TMA) ring in shared memory (hop_ring.cuh)
-// Default for d_R <= 6: variant 3 (measured on B200, profiles/).  Large d_R (>= 8) always uses the row-group
+//   4 = the same with two warps per tile, one per half-spinor component (hop_pair.cuh)
+// Default for d_R <= 6: variant 3, except fp64 with d_R >= 5 where one thread per site spills: variant 4
+// (measured on B200, profiles/).  Large d_R (>= 8) always uses the row-group
 // kernel of hop_large.cuh.
 #pragma once
 #include "hop_large.cuh"
-#include "hop_ring.cuh"
+#include "hop_pair.cuh"
 
 namespace hirep {
 
 template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
-    if (variant == 0) variant = 3;
+    if (variant == 0) variant = (sizeof(T) == 8 && DR >= 5) ? 4 : 3;
     switch (variant) {
     case 1: return launch_hop_small<T, DR, REAL, 1, 128>(g, L, s);
     case 2: return launch_hop_small<T, DR, REAL, 2, 128>(g, L, s);
-    case 3: {
-        using P = RingPick<T, DR, REAL>;
-        return launch_hop_ring<T, DR, REAL, P::WARPS, P::STAGES, P::RPC>(g, L, s);
+    case 3: return launch_hop_ring<T, DR, REAL>(g, L, s);
+    case 4: return launch_hop_pair<T, DR, REAL>(g, L, s);
     }
+#ifdef HIREP_SWEEP   // ring-shape sweeps (not part of the library build): variant = 1000*WARPS + 100*STAGES + RPC
+    if constexpr (DR == HIREP_SWEEP && !REAL) {
+        const bool self = (L.a != 0.0) && L.set[0].self != nullptr;
+#define SW(W, S, R)                                                                                          \
+    if (variant == 1000 * W + 100 * S + R)                                                                   \
+        return self ? launch_hop_ring_cfg<T, DR, REAL, W, S, R, true>(g, L, s) : launch_hop_ring_cfg<T, DR, REAL, W, S, R, false>(g, L, s);
+#define SWN(W, S, R)                                                                                         \
+    if (variant == 1000 * W + 100 * S + R)                                                                   \
+        return self ? launch_hop_ring<T, DR, REAL>(g, L, s) : launch_hop_ring_cfg<T, DR, REAL, W, S, R, false>(g, L, s);
+        if constexpr (sizeof(T) == 4) {
+            SW(12, 2, 3) SW(12, 4, 2) SWN(11, 2, 6) SWN(10, 2, 6) SW(8, 2, 6) SW(10, 2, 3) SW(11, 2, 3) SW(12, 3, 2) SW(8, 4, 3)
+        } else {
+            SW(8, 4, 1) SW(8, 2, 2) SW(6, 2, 3) SW(6, 3, 2) SW(4, 4, 3)
+        }
+#undef SW
+#undef SWN
     }
+#endif
     return KERR_UNSUPPORTED;
 }
 

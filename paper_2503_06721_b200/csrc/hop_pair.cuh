@@ -1,0 +1,334 @@
+// hop_pair.cuh -- the ring stencil kernel with TWO warps per tile: warp s of a pair owns half-spinor component s.
+//
+//   out(x) = a*self(x) + b * sum_{d=0..7} P_d W_d(x) in(nbr_d(x)),   x of parity p_out            (Eq 8)
+//
+// Why: with one thread per site (hop_ring.cuh) a thread holds the 4 d_R accumulators, the 2 d_R half spinor, the
+// 4 d_R prefetched neighbour and a link row -- 11 d_R + complex numbers, i.e. > 255 registers in fp64 from
+// d_R = 5 on (the paper's "register spilling for N_g > 4", L1548).  The two half-spinor components s = 0, 1 of
+// (1 -+ gamma_mu) psi are independent through the link multiply (step a3), so two warps share a tile:
+//   warp s loads psi_s and the lower component it is combined with (2 d_R numbers instead of 4 d_R), projects
+//   h_s (d_R), multiplies by the SAME link rows (read by both warps from one shared ring) and accumulates
+//   out_s (upper) and its contributions to the lower components: lo[s] for mu = 0, 3 and lo[1-s] for mu = 1, 2
+//   (e_mu is off-diagonal there, hop_small.cuh).  The cross contributions are exchanged once per tile through
+//   shared memory.  Per thread: ~5.5 d_R complex numbers -- no spills at d_R = 6 in fp64.
+// Data movement is that of hop_ring.cuh: persistent CTAs, one ring of bulk-copy (TMA) slots per PAIR for the link
+// stream with full/empty mbarriers (the producer is lane 0 of warp 0 of the pair and refills a slot once BOTH
+// warps have released it), register prefetch of the next neighbour, the tile's own spinor by one bulk copy
+// (SELF), x-blocked traversal order.
+//
+// Link mode REBUILD (NF > 0): the ring carries the FUNDAMENTAL gather block (N_g x N_g per direction) and each
+// row of R(W) is rebuilt in registers by RepMap (rep_maps.cuh) -- "rebuilding the represented field on the fly",
+// L343.  The boundary sign (Eq 61), which the stored represented field carries (L945), is applied to the
+// half spinor instead.  Both warps of the pair rebuild the rows they need (the rebuild is done twice per tile).
+#pragma once
+#include "hop_ring.cuh"
+#include "rep_maps.cuh"
+
+namespace hirep {
+
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void pair_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+
+// one lane's column of a [e][32 lanes] shared-memory tile, indexable like a register matrix
+template <typename T> struct SmemMat {
+    const cplx<T> *p;
+    __device__ __forceinline__ cplx<T> operator[](int e) const { return p[e * TILE]; }
+};
+
+// boundary factor of hop D from the site (Eq 61): bc[mu] if the hop leaves the lattice
+template <int D> __device__ __forceinline__ int hop_sign_dir(const Geo &g, int p, int t, int x, int y, int zh) {
+    constexpr int mu = D & 3;
+    constexpr bool fwd = D < 4;
+    const int c = (mu == 0) ? t : (mu == 1) ? x : (mu == 2) ? y : 2 * zh + ((t + x + y + p) & 1);
+    const int ext = (mu == 0) ? g.T : g.L;
+    return (fwd ? (c == ext - 1) : (c == 0)) ? g.bc[mu] : 1;
+}
+
+template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF> struct PairCfg {
+    using E = link_elem<T, REAL>;                                   // element type of R
+    static constexpr bool REBUILD = NF > 0;
+    static constexpr int CPD = REBUILD ? 1 : DR / RPC;              // chunks per direction
+    static constexpr uint32_t CHUNK = REBUILD ? NF * NF * TILE * sizeof(cplx<T>) : RPC * DR * TILE * sizeof(E);
+    static_assert(REBUILD || DR % RPC == 0, "rows per chunk must divide d_R");
+    static constexpr uint32_t SELF_BYTES = SELF ? 4 * DR * TILE * sizeof(cplx<T>) : 0;
+    static constexpr uint32_t X_BYTES = 2 * DR * TILE * sizeof(cplx<T>);   // cross contributions of both warps
+    static constexpr uint32_t NBAR = 2 * STAGES + 2;                // full[S], empty[S], self full, self empty
+    static constexpr size_t PER_PAIR = (size_t)STAGES * CHUNK + SELF_BYTES + X_BYTES + NBAR * 8;
+    static constexpr size_t SMEM = PER_PAIR * PAIRS;
+    static_assert(CHUNK % 16 == 0 && PER_PAIR % 16 == 0, "bulk copies need 16-byte alignment");
+    static_assert(SMEM <= 227 * 1024, "pair rings do not fit the 227 KB of shared memory of an sm_100 CTA");
+};
+
+template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF, int REP>
+__global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, const HopLaunch L) {
+    using C = cplx<T>;
+    using E = link_elem<T, REAL>;
+    using Cfg = PairCfg<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF>;
+    constexpr bool REBUILD = NF > 0;
+    constexpr int NC = 4 * DR, CPD = Cfg::CPD, CPT = 8 * CPD;
+    constexpr int RPCE = REBUILD ? DR : RPC;                        // rows of R served by one chunk
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int pair = warp >> 1, s = warp & 1;                       // s: the half-spinor component this warp owns
+    unsigned char *base = smem_raw + (size_t)pair * Cfg::PER_PAIR;
+    const unsigned char *ring = base;
+    const C *selfbuf = reinterpret_cast<const C *>(base + (size_t)STAGES * Cfg::CHUNK);
+    C *xbuf = reinterpret_cast<C *>(base + (size_t)STAGES * Cfg::CHUNK + Cfg::SELF_BYTES);
+    const uint32_t ring_s = smem_u32(ring), self_s = smem_u32(selfbuf);
+    const uint32_t full_s = smem_u32(base + (size_t)STAGES * Cfg::CHUNK + Cfg::SELF_BYTES + Cfg::X_BYTES);
+    const uint32_t empty_s = full_s + 8 * STAGES;
+    const uint32_t selffull_s = empty_s + 8 * STAGES, selfempty_s = selffull_s + 8;
+    const bool producer = (s == 0) && (lane == 0);
+    if (producer) {
+        for (int i = 0; i < STAGES; ++i) { mbar_init(full_s + 8 * i, 1); mbar_init(empty_s + 8 * i, 2); }
+        mbar_init(selffull_s, 1);
+        mbar_init(selfempty_s, 2);
+        fence_mbar_init();
+    }
+    pair_sync(1 + pair);
+
+    const bool two = L.nsets == 2;
+    const int total_tiles = g.n_tiles * L.nsets;
+    const int gp = blockIdx.x * PAIRS + pair, np = gridDim.x * PAIRS;
+    if (gp >= total_tiles) return;
+    const int my_tiles = (total_tiles - gp + np - 1) / np;
+    const int my_chunks = my_tiles * CPT;
+    const uint64_t pol = l2_policy_evict_first();
+
+    auto locate = [&](int k, int &set_, int &tile_) {
+        const int gt = gp + k * np;
+        set_ = two ? (gt & 1) : 0;
+        int sq = two ? (gt >> 1) : gt;
+        if (L.ord_BX > 0) {
+            const int r = sq % L.ord_R;
+            int u = sq / L.ord_R;
+            const int xi = u % L.ord_BX;
+            u /= L.ord_BX;
+            const int tt = u % g.T, xb = u / g.T;
+            sq = (tt * g.L + xb * L.ord_BX + xi) * L.ord_R + r;
+        }
+        tile_ = sq;
+    };
+
+    // producer state: the next chunk to issue is chunk iq_c of the pair's iq_k-th tile
+    int iq_k = 0, iq_c = 0;
+    const unsigned char *iq_base = nullptr;
+    auto iq_enter = [&]() {
+        int s_, t_;
+        locate(iq_k, s_, t_);
+        iq_base = (const unsigned char *)(s_ ? L.set[1].links : L.set[0].links) + (size_t)t_ * CPT * Cfg::CHUNK;
+    };
+    auto issue = [&](int slot) {
+        mbar_expect_tx(full_s + 8 * slot, Cfg::CHUNK);
+        bulk_g2s(ring_s + slot * Cfg::CHUNK, iq_base + (size_t)iq_c * Cfg::CHUNK, Cfg::CHUNK, full_s + 8 * slot, pol);
+        if (++iq_c == CPT) {
+            iq_c = 0;
+            if (++iq_k < my_tiles) iq_enter();
+        }
+    };
+    if (producer) {
+        iq_enter();
+        const int n0 = my_chunks < STAGES ? my_chunks : STAGES;
+        for (int i = 0; i < n0; ++i) issue(i);
+    }
+
+    int set, tile, t, x, y, zh, p_out;
+    bool active;
+    const C *in;
+    auto enter_tile = [&](int k) {
+        locate(k, set, tile);
+        int h = tile * TILE + lane;
+        active = h < g.Nh;
+        if (!active) h = g.Nh - 1;
+        decode_site(g, h, t, x, y, zh);
+        p_out = set ? L.set[1].p_out : L.set[0].p_out;
+        in = (const C *)(set ? L.set[1].in : L.set[0].in);
+    };
+    // neighbour components this warp needs for direction D: upper s and lower q_D(s)
+    C nbu[DR], nbl[DR];
+    auto fetch = [&](int hn, bool swap) {
+        const int ql = swap ? 1 - s : s;
+        const C *src = in + ((size_t)(hn >> 5) * NC) * TILE + (hn & 31);
+#pragma unroll
+        for (int c = 0; c < DR; ++c) {
+            nbu[c] = ld_spinor<T>(src + (size_t)(s * DR + c) * TILE);
+            nbl[c] = ld_spinor<T>(src + (size_t)((2 + ql) * DR + c) * TILE);
+        }
+    };
+
+    enter_tile(0);
+    fetch(neighbour<0>(g, p_out, t, x, y, zh), DirInfo<0>::swap);
+    int q = 0, slot = 0;
+    uint32_t phase = 0;
+    const T a = (T)L.a, b = (T)L.b;
+    const T g5s = L.g5 ? T(-1) : T(1);
+
+    for (int k = 0; k < my_tiles; ++k) {
+        const int c_set = set, c_tile = tile;
+        const bool c_active = active;
+        if constexpr (SELF) {
+            if (producer) {
+                if (k > 0) mbar_wait(selfempty_s, (k - 1) & 1);   // both warps have read the previous tile's block
+                const C *sp = (const C *)(c_set ? L.set[1].self : L.set[0].self) + ((size_t)c_tile * NC) * TILE;
+                mbar_expect_tx(selffull_s, Cfg::SELF_BYTES);
+                bulk_g2s_plain(self_s, sp, Cfg::SELF_BYTES, selffull_s);
+            }
+        }
+        C up[DR], ls[DR], lx[DR];   // out_s ; lower component s (mu = 0,3) ; lower component 1-s (mu = 1,2)
+#pragma unroll
+        for (int c = 0; c < DR; ++c) up[c] = ls[c] = lx[c] = mk<T>(0, 0);
+
+        static_for<0, 8>([&](auto dc) {
+            constexpr int D = decltype(dc)::value;
+            using DI = DirInfo<D>;
+            // (a2) spin projection: h_s = psi_s + sg e_mu psi_low
+            const T cs = (T)(DI::sg * ((DI::mu < 2) ? -1 : (s ? 1 : -1)));
+            T sgn = T(1);
+            if constexpr (REBUILD) sgn = (T)hop_sign_dir<D>(g, p_out, t, x, y, zh);
+            const T cv = cs * sgn;
+            C hs[DR];
+#pragma unroll
+            for (int c = 0; c < DR; ++c) {
+                const C u = nbu[c], v = nbl[c];
+                if (DI::imag) hs[c] = mk<T>(fma(-cv, v.y, sgn * u.x), fma(cv, v.x, sgn * u.y));   // sgn (u + i cs v)
+                else hs[c] = mk<T>(fma(cv, v.x, sgn * u.x), fma(cv, v.y, sgn * u.y));             // sgn (u + cs v)
+            }
+            if constexpr (D < 7) {
+                fetch(neighbour<D + 1>(g, p_out, t, x, y, zh), DirInfo<D + 1>::swap);
+            } else {
+                if (k + 1 < my_tiles) {
+                    enter_tile(k + 1);
+                    fetch(neighbour<0>(g, p_out, t, x, y, zh), DirInfo<0>::swap);
+                }
+            }
+            // (a3) link rows from the pair's ring, (a4) reconstruct + accumulate
+            static_for<0, DR>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                if constexpr (i % RPCE == 0) mbar_wait(full_s + 8 * slot, phase);
+                E w[DR];
+                if constexpr (REBUILD) {
+                    const SmemMat<T> Wm{reinterpret_cast<const C *>(ring + (size_t)slot * Cfg::CHUNK) + lane};
+                    RepMap<T, NF, REP>::template row<i>(Wm, w);
+                } else {
+                    const E *W = reinterpret_cast<const E *>(ring + (size_t)slot * Cfg::CHUNK) + lane;
+#pragma unroll
+                    for (int j = 0; j < DR; ++j) w[j] = W[((i % RPCE) * DR + j) * TILE];
+                }
+                C chi = mk<T>(0, 0);
+#pragma unroll
+                for (int j = 0; j < DR; ++j) mac<T>(chi, w[j], hs[j]);
+                up[i].x += chi.x;
+                up[i].y += chi.y;
+                C add;   // sg conj(k_mu(s)) chi
+                if (DI::imag) add = mk<T>(cs * chi.y, -cs * chi.x);
+                else add = mk<T>(cs * chi.x, cs * chi.y);
+                if (DI::swap) { lx[i].x += add.x; lx[i].y += add.y; }
+                else { ls[i].x += add.x; ls[i].y += add.y; }
+                if constexpr (i % RPCE == RPCE - 1) {
+                    // release the slot; the producer refills it once both warps have released it
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(empty_s + 8 * slot);
+                    if (producer && q + STAGES < my_chunks) {
+                        mbar_wait(empty_s + 8 * slot, phase);
+                        issue(slot);
+                    }
+                    ++q;
+                    if (++slot == STAGES) { slot = 0; phase ^= 1; }
+                }
+            });
+        });
+
+        // exchange the cross contributions: lower component s += partner's lx
+        pair_sync(1 + pair);   // partner has finished reading the previous tile's exchange
+#pragma unroll
+        for (int c = 0; c < DR; ++c) xbuf[(s * DR + c) * TILE + lane] = lx[c];
+        pair_sync(1 + pair);
+#pragma unroll
+        for (int c = 0; c < DR; ++c) {
+            const C o = xbuf[((1 - s) * DR + c) * TILE + lane];
+            ls[c].x += o.x;
+            ls[c].y += o.y;
+        }
+        if constexpr (SELF) mbar_wait(selffull_s, k & 1);
+        if (c_active) {
+            C *__restrict__ out = (C *)(c_set ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
+#pragma unroll
+            for (int c = 0; c < DR; ++c) {
+                C vu = mk<T>(b * up[c].x, b * up[c].y);
+                C vl = mk<T>(b * ls[c].x, b * ls[c].y);
+                if constexpr (SELF) {
+                    const C su = selfbuf[(s * DR + c) * TILE + lane];
+                    const C sl = selfbuf[((2 + s) * DR + c) * TILE + lane];
+                    vu.x = fma(a, su.x, vu.x); vu.y = fma(a, su.y, vu.y);
+                    vl.x = fma(a, sl.x, vl.x); vl.y = fma(a, sl.y, vl.y);
+                }
+                out[(size_t)(s * DR + c) * TILE] = vu;
+                out[(size_t)((2 + s) * DR + c) * TILE] = mk<T>(g5s * vl.x, g5s * vl.y);
+            }
+        }
+        if constexpr (SELF) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(selfempty_s);
+        }
+    }
+}
+
+template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF, int REP>
+int launch_hop_pair_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
+    using Cfg = PairCfg<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF>;
+    auto kern = hop_pair_kernel<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF, REP>;
+    static int n_sm = 0;
+    if (n_sm == 0) {
+        int dev = 0, sms = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        if (e != cudaSuccess) return (int)e;
+        n_sm = sms;
+    }
+    HopLaunch L = L0;
+    ring_tile_order<T, DR>(g, L);
+    const int grid = ring_grid(n_sm, L.max_ctas, g.n_tiles * L.nsets, PAIRS);
+    kern<<<grid, PAIRS * 64, Cfg::SMEM, s>>>(g, L);
+    return (int)cudaGetLastError();
+}
+
+// default shape of the pair kernel: PAIRS pairs per CTA; the chunk is the largest whole number of link rows that
+// divides d_R, stays <= 13 KB and leaves room for two stages; then as many stages (<= 4) as fit
+template <typename T, int DR, bool REAL, bool SELF, int NF> struct PairPick {
+    using E = link_elem<T, REAL>;
+    static constexpr int PAIRS = sizeof(T) == 4 ? 8 : 4;   // warps per SM sub-partition: 4 (fp32, <= 128 registers) or 2 (fp64, <= 255)
+    static constexpr size_t FIXED = (SELF ? 4 : 0) * DR * TILE * sizeof(cplx<T>) + 2 * DR * TILE * sizeof(cplx<T>) + 10 * 8;
+    static constexpr size_t chunk_of(int r) { return NF > 0 ? (size_t)NF * NF * TILE * sizeof(cplx<T>) : (size_t)r * DR * TILE * sizeof(E); }
+    static constexpr int stages_of(int r) {
+        const size_t per_pair = ((226 * 1024) / PAIRS) & ~(size_t)15;
+        if (per_pair < FIXED) return 0;
+        const int st = (int)((per_pair - FIXED) / chunk_of(r));
+        return st > 4 ? 4 : st;
+    }
+    static constexpr int pick_rpc() {
+        if (NF > 0) return DR;
+        int best = 1;
+        for (int r = 1; r <= DR; ++r)
+            if (DR % r == 0 && chunk_of(r) <= 13 * 1024 && stages_of(r) >= 2) best = r;
+        return best;
+    }
+    static constexpr int RPC = pick_rpc();
+    static constexpr int STAGES = stages_of(RPC);
+    static_assert(STAGES >= 2, "pair ring needs at least two stages");
+};
+
+template <typename T, int DR, bool REAL, int NF = 0, int REP = 0> int launch_hop_pair(const Geo &g, const HopLaunch &L, cudaStream_t s) {
+    const bool self = (L.a != 0.0) && L.set[0].self != nullptr;
+    if (self) {
+        using P = PairPick<T, DR, REAL, true, NF>;
+        return launch_hop_pair_cfg<T, DR, REAL, P::PAIRS, P::STAGES, P::RPC, true, NF, REP>(g, L, s);
+    }
+    using P = PairPick<T, DR, REAL, false, NF>;
+    return launch_hop_pair_cfg<T, DR, REAL, P::PAIRS, P::STAGES, P::RPC, false, NF, REP>(g, L, s);
+}
+
+}  // namespace hirep

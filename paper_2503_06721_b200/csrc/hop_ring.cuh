@@ -16,6 +16,12 @@
 //   * Neighbour spinors are gathered with plain 128-bit read-only loads; the loads of direction d+1 are issued
 //     right after direction d has been projected (the projection frees the registers), so they fly during the
 //     link matvec of direction d.  At direction 7 the first neighbour of the warp's next tile is fetched.
+//   * When the pass has a diagonal term (a != 0: Dphi, the second pass of Dphi_hat, g5Dphi_sq; template SELF) the
+//     tile's own spinor -- one contiguous 4 d_R x 32 block -- is fetched by ONE bulk copy at the start of the tile
+//     into a per-warp buffer and read in the epilogue, instead of being loaded (latency exposed) at the end.
+//   * Tile traversal order: tiles are dealt in x-blocked order (x-block, t, x in block, y, z) when the input
+//     spinor of one t-slice no longer fits comfortably in L2 (SU(4) 2AS fp64: 21 MB per slice), so that the
+//     t+-1 neighbours of a tile are processed a few MB -- not a whole t-slice -- apart (HopLaunch::ord_*).
 // No CTA-wide barrier anywhere: every warp is its own producer/consumer pipeline (lane 0 issues the bulk copies).
 #pragma once
 #include "hop_small.cuh"
@@ -56,56 +62,70 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
         : "memory");
 }
 
+__device__ __forceinline__ void bulk_g2s_plain(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+                 "r"(bytes), "r"(bar)
+                 : "memory");
+}
+
 // ring geometry for one instantiation; CHUNK = RPC rows of the link block of one direction of one tile
-template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC = DR> struct RingCfg {
+template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC, bool SELF> struct RingCfg {
     using E = link_elem<T, REAL>;
     static constexpr int NE = DR * DR;
     static constexpr int CPD = DR / RPC;                            // chunks per direction
     static constexpr uint32_t CHUNK = RPC * DR * TILE * sizeof(E);  // RPC rows of one link matrix, 32 lanes
     static_assert(DR % RPC == 0, "rows per chunk must divide d_R");
+    static constexpr uint32_t SELF_BYTES = SELF ? 4 * DR * TILE * sizeof(cplx<T>) : 0;   // one tile of the spinor
     static constexpr size_t RING_BYTES = (size_t)WARPS * STAGES * CHUNK;
-    static constexpr size_t SMEM = RING_BYTES + (size_t)WARPS * STAGES * sizeof(uint64_t);
+    static constexpr size_t BARS_OFF = RING_BYTES + (size_t)WARPS * SELF_BYTES;
+    static constexpr size_t SMEM = BARS_OFF + (size_t)WARPS * (STAGES + 1) * sizeof(uint64_t);
     static_assert(CHUNK % 16 == 0, "bulk copies move multiples of 16 bytes");
     static_assert(SMEM <= 227 * 1024, "ring does not fit the 227 KB of shared memory of an sm_100 CTA");
 };
 
-// Library default ring shape per instantiation, from the B200 sweeps recorded in profiles/ (r01_ring_sweep.md):
+// Library default ring shape per instantiation (B200 sweeps: profiles/r01_ring_sweep.md):
 //   fp64: 8 warps (the thread-per-site kernel needs ~200 registers); fp32: 16 warps for d_R <= 3, else 12;
-//   chunk = the largest whole number of link rows that divides d_R and stays <= 13 KB; 2..4 stages as smem allows.
-template <typename T, int DR, bool REAL> struct RingPick {
+//   chunk = the largest whole number of link rows that divides d_R, stays <= 13 KB and leaves room for two stages
+//   (large chunks beat deep rings: fewer barrier round trips per byte); then as many stages (<= 4) as fit.
+template <typename T, int DR, bool REAL, bool SELF> struct RingPick {
     using E = link_elem<T, REAL>;
     static constexpr int WARPS = sizeof(T) == 4 ? (DR <= 3 ? 16 : 12) : 8;
+    static constexpr size_t SELF_BYTES = SELF ? 4 * DR * TILE * sizeof(cplx<T>) : 0;
+    static constexpr size_t chunk_of(int r) { return (size_t)r * DR * TILE * sizeof(E); }
+    static constexpr int stages_of(int r) {
+        const size_t per_warp = (226 * 1024) / WARPS;
+        if (per_warp < SELF_BYTES + 8) return 0;
+        const int st = (int)((per_warp - SELF_BYTES - 8) / (chunk_of(r) + 8));
+        return st > 4 ? 4 : st;
+    }
     static constexpr int pick_rpc() {
         int best = 1;
         for (int r = 1; r <= DR; ++r)
-            if (DR % r == 0 && (size_t)r * DR * TILE * sizeof(E) <= 13 * 1024) best = r;
+            if (DR % r == 0 && chunk_of(r) <= 13 * 1024 && stages_of(r) >= 2) best = r;
         return best;
     }
     static constexpr int RPC = pick_rpc();
-    static constexpr size_t CHUNK = (size_t)RPC * DR * TILE * sizeof(E);
-    static constexpr int pick_stages() {
-        int st = (int)((226 * 1024) / (WARPS * (CHUNK + 8)));
-        return st > 4 ? 4 : st;
-    }
-    static constexpr int STAGES = pick_stages();
+    static constexpr int STAGES = stages_of(RPC);
     static_assert(STAGES >= 2, "ring needs at least two stages");
 };
 
-template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC = DR>
+template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC, bool SELF>
 __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, const HopLaunch L) {
     using C = cplx<T>;
     using E = link_elem<T, REAL>;
-    using Cfg = RingCfg<T, DR, REAL, WARPS, STAGES, RPC>;
+    using Cfg = RingCfg<T, DR, REAL, WARPS, STAGES, RPC, SELF>;
     constexpr int NC = 4 * DR, CPD = Cfg::CPD, CPT = 8 * CPD;   // chunks per direction / per tile
     constexpr int CE = RPC * DR * TILE;                         // link elements per chunk
     extern __shared__ __align__(128) unsigned char smem_raw[];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const E *ring = reinterpret_cast<const E *>(smem_raw + (size_t)warp * STAGES * Cfg::CHUNK);
-    const uint32_t ring_s = smem_u32(ring);
-    const uint32_t bars_s = smem_u32(smem_raw + Cfg::RING_BYTES) + warp * STAGES * 8;
+    const C *selfbuf = reinterpret_cast<const C *>(smem_raw + Cfg::RING_BYTES + (size_t)warp * Cfg::SELF_BYTES);
+    const uint32_t ring_s = smem_u32(ring), self_s = smem_u32(selfbuf);
+    const uint32_t bars_s = smem_u32(smem_raw + Cfg::BARS_OFF) + warp * (STAGES + 1) * 8;
+    const uint32_t selfbar_s = bars_s + 8 * STAGES;
     if (lane == 0) {
-        for (int s = 0; s < STAGES; ++s) mbar_init(bars_s + 8 * s, 1);
+        for (int s = 0; s <= STAGES; ++s) mbar_init(bars_s + 8 * s, 1);
         fence_mbar_init();
     }
     __syncwarp();
@@ -120,28 +140,38 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
     const int my_chunks = my_tiles * CPT;
     const uint64_t pol = l2_policy_evict_first();
 
-    // chunk q of this warp = chunk q % CPT of its (q / CPT)-th tile; a tile's chunks are consecutive in memory
-    auto issue = [&](int q, int slot) {
-        const int gt = gw + (q / CPT) * nw;
-        const int set = two ? (gt & 1) : 0;
-        const int tile = two ? (gt >> 1) : gt;
-        const E *src = (const E *)(set ? L.set[1].links : L.set[0].links) + ((size_t)tile * CPT + (q % CPT)) * CE;
+    // k-th tile of this warp -> (set, tile): position gw + k*nw of the traversal order (x-blocked if ord_BX > 0)
+    auto locate = [&](int k, int &set_, int &tile_) {
+        const int gt = gw + k * nw;
+        set_ = two ? (gt & 1) : 0;
+        int sq = two ? (gt >> 1) : gt;
+        if (L.ord_BX > 0) {
+            const int r = sq % L.ord_R;
+            int u = sq / L.ord_R;
+            const int xi = u % L.ord_BX;
+            u /= L.ord_BX;
+            const int tt = u % g.T, xb = u / g.T;
+            sq = (tt * g.L + xb * L.ord_BX + xi) * L.ord_R + r;
+        }
+        tile_ = sq;
+    };
+
+    // chunk qi of this warp = chunk qi % CPT of its (qi / CPT)-th tile; a tile's chunks are consecutive in memory.
+    // The ring runs at most STAGES <= CPT chunks ahead, i.e. into the warp's next tile (n_set, n_tile) at most.
+    int set, tile, c_set = 0, c_tile = 0, n_set = 0, n_tile = 0;   // being fetched / being computed / next
+    auto issue = [&](int qi, int slot, int k_cur) {
+        const int kq = qi / CPT;
+        const int set_ = kq == k_cur ? c_set : n_set, tile_ = kq == k_cur ? c_tile : n_tile;
+        const E *src = (const E *)(set_ ? L.set[1].links : L.set[0].links) + ((size_t)tile_ * CPT + (qi - kq * CPT)) * CE;
         mbar_expect_tx(bars_s + 8 * slot, Cfg::CHUNK);
         bulk_g2s(ring_s + slot * Cfg::CHUNK, src, Cfg::CHUNK, bars_s + 8 * slot, pol);
     };
-    if (lane == 0) {
-        const int n0 = my_chunks < STAGES ? my_chunks : STAGES;
-        for (int q = 0; q < n0; ++q) issue(q, q);
-    }
 
     // per-tile state
-    int set, tile, t, x, y, zh, p_out;
+    int t, x, y, zh, p_out;
     bool active;
     const C *in;
-    auto enter_tile = [&](int k) {
-        const int gt = gw + k * nw;
-        set = two ? (gt & 1) : 0;
-        tile = two ? (gt >> 1) : gt;
+    auto enter_tile = [&]() {   // (set, tile) -> coordinates and pointers
         int h = tile * TILE + lane;
         active = h < g.Nh;
         if (!active) h = g.Nh - 1;
@@ -156,7 +186,14 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
         for (int c = 0; c < NC; ++c) nb[c] = ld_spinor<T>(src + (size_t)c * TILE);
     };
 
-    enter_tile(0);
+    locate(0, set, tile);
+    c_set = set;
+    c_tile = tile;
+    if (lane == 0) {
+        const int n0 = my_chunks < STAGES ? my_chunks : STAGES;
+        for (int qi = 0; qi < n0; ++qi) issue(qi, qi, 0);
+    }
+    enter_tile();
     fetch(neighbour<0>(g, p_out, t, x, y, zh));
     int q = 0, slot = 0;
     uint32_t phase = 0;
@@ -165,8 +202,19 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
 
     for (int k = 0; k < my_tiles; ++k) {
         // state of the tile being computed (enter_tile(k+1) below overwrites the shared variables at d = 7)
-        const int c_set = set, c_tile = tile;
+        c_set = set;
+        c_tile = tile;
         const bool c_active = active;
+        if (k + 1 < my_tiles) locate(k + 1, n_set, n_tile);
+        if constexpr (SELF) {
+            // the tile's own spinor: one contiguous block -> one bulk copy, consumed in the epilogue
+            __syncwarp();   // every lane has finished reading the buffer in the previous epilogue
+            if (lane == 0) {
+                const C *sp = (const C *)(c_set ? L.set[1].self : L.set[0].self) + ((size_t)c_tile * NC) * TILE;
+                mbar_expect_tx(selfbar_s, Cfg::SELF_BYTES);
+                bulk_g2s_plain(self_s, sp, Cfg::SELF_BYTES, selfbar_s);
+            }
+        }
         C up[2][DR], lo[2][DR];
 #pragma unroll
         for (int s = 0; s < 2; ++s)
@@ -194,7 +242,9 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
                 fetch(neighbour<D + 1>(g, p_out, t, x, y, zh));
             } else {
                 if (k + 1 < my_tiles) {
-                    enter_tile(k + 1);
+                    set = n_set;
+                    tile = n_tile;
+                    enter_tile();
                     fetch(neighbour<0>(g, p_out, t, x, y, zh));
                 }
             }
@@ -221,27 +271,25 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
                 if (i % RPC == RPC - 1) {
                     // slot consumed by every lane -> refill it with the chunk STAGES ahead
                     __syncwarp();
-                    if (lane == 0 && q + STAGES < my_chunks) issue(q + STAGES, slot);
+                    if (lane == 0 && q + STAGES < my_chunks) issue(q + STAGES, slot, k);
                     ++q;
                     if (++slot == STAGES) { slot = 0; phase ^= 1; }
                 }
             }
         });
 
+        if constexpr (SELF) mbar_wait(selfbar_s, k & 1);
         if (c_active) {
             C *__restrict__ out = (C *)(c_set ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
-            const C *self_base = (const C *)(c_set ? L.set[1].self : L.set[0].self);
-            const C *__restrict__ self = self_base + ((size_t)c_tile * NC) * TILE + lane;
-            const bool use_self = (self_base != nullptr) && (L.a != 0.0);
 #pragma unroll
             for (int s = 0; s < 2; ++s)
 #pragma unroll
                 for (int c = 0; c < DR; ++c) {
                     C vu = mk<T>(b * up[s][c].x, b * up[s][c].y);
                     C vl = mk<T>(b * lo[s][c].x, b * lo[s][c].y);
-                    if (use_self) {
-                        const C su = self[(size_t)(s * DR + c) * TILE];
-                        const C sl = self[(size_t)((2 + s) * DR + c) * TILE];
+                    if constexpr (SELF) {
+                        const C su = selfbuf[(s * DR + c) * TILE + lane];
+                        const C sl = selfbuf[((2 + s) * DR + c) * TILE + lane];
                         vu.x = fma(a, su.x, vu.x); vu.y = fma(a, su.y, vu.y);
                         vl.x = fma(a, sl.x, vl.x); vl.y = fma(a, sl.y, vl.y);
                     }
@@ -252,10 +300,41 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
     }
 }
 
-template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC = DR>
-int launch_hop_ring(const Geo &g, const HopLaunch &L, cudaStream_t s) {
-    using Cfg = RingCfg<T, DR, REAL, WARPS, STAGES, RPC>;
-    auto kern = hop_ring_kernel<T, DR, REAL, WARPS, STAGES, RPC>;
+// x-blocked traversal order for one launch: ord_BX = 0 keeps the storage order.  One (t, x-block) slab of the input
+// spinor(s) is kept at or below SLAB_LIMIT bytes so that the slabs of t-1, t, t+1 stay in L2 next to the link stream.
+// L.bx_req (hirep_set_tuning) overrides the block size.
+template <typename T, int DR> void ring_tile_order(const Geo &g, HopLaunch &L) {
+    L.ord_R = 0;
+    L.ord_BX = 0;
+    const long row = (long)g.L * g.Lh;   // sites of one (t, x) row-plane
+    if (row % TILE != 0) return;
+    const int R = (int)(row / TILE);
+    int bx = 0;
+    if (L.bx_req >= 0) {
+        if (L.bx_req == 0 || g.L % L.bx_req != 0 || L.bx_req == g.L) return;
+        bx = L.bx_req;
+    } else {
+        constexpr double SLAB_LIMIT = 4.0 * 1024 * 1024;
+        const double per_x = (double)R * TILE * 4 * DR * sizeof(cplx<T>) * L.nsets;
+        if (per_x * g.L <= SLAB_LIMIT) return;   // a whole t-slice is small: storage order
+        for (int c = g.L - 1; c >= 2; --c)
+            if (g.L % c == 0 && per_x * c <= SLAB_LIMIT) { bx = c; break; }
+        if (bx == 0) bx = 2;
+    }
+    L.ord_R = R;
+    L.ord_BX = bx;
+}
+inline int ring_grid(int n_sm, int max_ctas, int total_tiles, int tiles_per_cta) {
+    int grid = (total_tiles + tiles_per_cta - 1) / tiles_per_cta;
+    if (grid > n_sm) grid = n_sm;
+    if (max_ctas > 0 && grid > max_ctas) grid = max_ctas;
+    return grid;
+}
+
+template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC, bool SELF>
+int launch_hop_ring_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
+    using Cfg = RingCfg<T, DR, REAL, WARPS, STAGES, RPC, SELF>;
+    auto kern = hop_ring_kernel<T, DR, REAL, WARPS, STAGES, RPC, SELF>;
     static int n_sm = 0;
     if (n_sm == 0) {
         int dev = 0, sms = 0;
@@ -265,11 +344,22 @@ int launch_hop_ring(const Geo &g, const HopLaunch &L, cudaStream_t s) {
         if (e != cudaSuccess) return (int)e;
         n_sm = sms;
     }
-    const int total_tiles = g.n_tiles * L.nsets;
-    int grid = (total_tiles + WARPS - 1) / WARPS;
-    if (grid > n_sm) grid = n_sm;
+    HopLaunch L = L0;
+    ring_tile_order<T, DR>(g, L);
+    const int grid = ring_grid(n_sm, L.max_ctas, g.n_tiles * L.nsets, WARPS);
     kern<<<grid, WARPS * 32, Cfg::SMEM, s>>>(g, L);
     return (int)cudaGetLastError();
+}
+
+// a pass with a diagonal term (a != 0 and a self spinor) uses the SELF instantiation, a pure hop the plain one
+template <typename T, int DR, bool REAL> int launch_hop_ring(const Geo &g, const HopLaunch &L, cudaStream_t s) {
+    const bool self = (L.a != 0.0) && L.set[0].self != nullptr;
+    if (self) {
+        using P = RingPick<T, DR, REAL, true>;
+        return launch_hop_ring_cfg<T, DR, REAL, P::WARPS, P::STAGES, P::RPC, true>(g, L, s);
+    }
+    using P = RingPick<T, DR, REAL, false>;
+    return launch_hop_ring_cfg<T, DR, REAL, P::WARPS, P::STAGES, P::RPC, false>(g, L, s);
 }
 
 }  // namespace hirep

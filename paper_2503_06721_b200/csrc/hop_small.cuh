@@ -34,14 +34,6 @@ template <int D> struct DirInfo {
     __host__ __device__ static constexpr int sigma(int s) { return (mu < 2) ? -1 : (s ? 1 : -1); }
 };
 
-template <int I> struct IntC { static constexpr int value = I; };
-template <int B, int E, typename F> __device__ __forceinline__ void static_for(F &&f) {
-    if constexpr (B < E) {
-        f(IntC<B>{});
-        static_for<B + 1, E>(f);
-    }
-}
-
 // acc += w * h  for complex or real link element
 template <typename T> __device__ __forceinline__ void mac(cplx<T> &acc, const cplx<T> &w, const cplx<T> &h) {
     acc.x = fma(w.x, h.x, acc.x);

@@ -1,5 +1,6 @@
 // rep_maps.cuh -- the maps U -> U^R (Eq 7; "functions that translate the fundamental gauge field
-// to the represented one", L339-341), one ROW of R(W) at a time, for a fundamental matrix W held in registers.
+// to the represented one", L339-341), one ROW of R(W) at a time, for a fundamental matrix W given by any accessor
+// W[e], e = i*N + j (registers, or one lane's column of a shared-memory tile).
 //
 // Used by links_to_rep (rep_kernels.cu: the stored represented field) and by the stencil kernels in link mode
 // REBUILD (R rebuilt in registers from the fundamental field, the "on-the-fly" variant of L343).
@@ -15,14 +16,6 @@
 #include "common.cuh"
 
 namespace hirep {
-
-template <int I> struct IntC { static constexpr int value = I; };
-template <int B, int E, typename F> __device__ __forceinline__ void static_for(F &&f) {
-    if constexpr (B < E) {
-        f(IntC<B>{});
-        static_for<B + 1, E>(f);
-    }
-}
 
 template <typename T> __device__ __forceinline__ cplx<T> cmul(cplx<T> a, cplx<T> b) { return mk<T>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 template <typename T> __device__ __forceinline__ cplx<T> cmulc(cplx<T> a, cplx<T> b) { return mk<T>(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }  // a * conj(b)
@@ -64,7 +57,7 @@ template <typename T, int N> struct RepMap<T, N, 0> {   // FUND
     static constexpr int DR = N;
     static constexpr bool REAL = false;
     using E = cplx<T>;
-    template <int A> __device__ __forceinline__ static void row(const cplx<T> *W, E *w) {
+    template <int A, typename WM> __device__ __forceinline__ static void row(const WM &W, E *w) {
 #pragma unroll
         for (int B = 0; B < N; ++B) w[B] = W[A * N + B];
     }
@@ -74,7 +67,7 @@ template <typename T, int N> struct RepMap<T, N, 3> {   // 2AS
     static constexpr int DR = N * (N - 1) / 2;
     static constexpr bool REAL = false;
     using E = cplx<T>;
-    template <int A> __device__ __forceinline__ static void row(const cplx<T> *W, E *w) {
+    template <int A, typename WM> __device__ __forceinline__ static void row(const WM &W, E *w) {
         constexpr PairIdx ij = pair_decode(A, N, true);
         static_for<0, DR>([&](auto bc) {
             constexpr int B = decltype(bc)::value;
@@ -90,7 +83,7 @@ template <typename T, int N> struct RepMap<T, N, 2> {   // SYM
     static constexpr int DR = N * (N + 1) / 2;
     static constexpr bool REAL = false;
     using E = cplx<T>;
-    template <int A> __device__ __forceinline__ static void row(const cplx<T> *W, E *w) {
+    template <int A, typename WM> __device__ __forceinline__ static void row(const WM &W, E *w) {
         constexpr PairIdx ij = pair_decode(A, N, false);
         constexpr int i = ij.i, j = ij.j;
         static_for<0, DR>([&](auto bc) {
@@ -117,7 +110,7 @@ template <typename T, int N> struct RepMap<T, N, 1> {   // ADJ (real matrix)
     static constexpr bool REAL = true;
     using E = T;
     // Y = W^dagger T^a W (N x N), then R_ab = 2 Re tr(Y T^b)
-    template <int A> __device__ __forceinline__ static void row(const cplx<T> *W, E *w) {
+    template <int A, typename WM> __device__ __forceinline__ static void row(const WM &W, E *w) {
         constexpr GenIdx ga = gen_decode(A);
         cplx<T> Y[N * N];
 #pragma unroll

@@ -20,13 +20,14 @@ F64, F32 = 0, 1
 EVEN, ODD, FULL = 0, 1, 2
 LINKS_STORED, LINKS_REBUILD = 0, 1
 OP_DPHI, OP_DPHI_EO, OP_DPHI_OE, OP_DPHI_HAT, OP_G5DPHI_SQ = 0, 1, 2, 3, 4
+TUNE_TILE_BLOCK, TUNE_MAX_CTAS = 0, 1
 
 # every symbol include/hirep_b200.h declares
 SYMBOLS = [
     "hirep_geom_create", "hirep_geom_destroy", "hirep_geom_set_bc", "hirep_geom_set_stream", "hirep_geom_sizes",
     "hirep_spinor_import", "hirep_spinor_export", "hirep_links_import", "hirep_links_rep_export",
     "hirep_links_rep_export_bwd", "hirep_links_to_rep", "hirep_Dphi", "hirep_Dphi_eo", "hirep_Dphi_oe",
-    "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_launch_count",
+    "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_set_tuning", "hirep_launch_count",
     "hirep_apply_host", "hirep_sync", "hirep_last_error",
 ]
 
@@ -67,6 +68,7 @@ def load():
         getattr(lib, n).argtypes = [vp, vp, vp, vp]
     lib.hirep_set_link_mode.argtypes = [vp, ci]
     lib.hirep_set_kernel_variant.argtypes = [vp, ci]
+    lib.hirep_set_tuning.argtypes = [vp, ci, ci]
     lib.hirep_launch_count.argtypes = [vp]
     lib.hirep_launch_count.restype = ctypes.c_long
     lib.hirep_apply_host.argtypes = [vp, ci, cd, vp, vp, vp]
@@ -128,6 +130,7 @@ def hirep_Dphi_hat(g, m0, out, inp, links): _check(load().hirep_Dphi_hat(g, m0, 
 def hirep_g5Dphi_sq(g, m0, out, inp, links): _check(load().hirep_g5Dphi_sq(g, m0, out, inp, links))
 def hirep_set_link_mode(g, mode): _check(load().hirep_set_link_mode(g, mode))
 def hirep_set_kernel_variant(g, variant): _check(load().hirep_set_kernel_variant(g, variant))
+def hirep_set_tuning(g, key, value): _check(load().hirep_set_tuning(g, key, value))
 def hirep_launch_count(g): return int(load().hirep_launch_count(g))
 def hirep_sync(g): _check(load().hirep_sync(g))
 
@@ -251,6 +254,7 @@ class Geometry:
 
     def set_link_mode(self, mode): hirep_set_link_mode(self.handle, mode)
     def set_kernel_variant(self, v): hirep_set_kernel_variant(self.handle, v)
+    def set_tuning(self, key, value): hirep_set_tuning(self.handle, key, value)
     def set_bc(self, sign): hirep_geom_set_bc(self.handle, sign)
     def sync(self): hirep_sync(self.handle)
     def launch_count(self): return hirep_launch_count(self.handle)

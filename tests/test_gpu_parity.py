@@ -154,9 +154,23 @@ def test_operators_vs_oracle_reduced(env, name, T, L, prec):
 
 @pytest.mark.parametrize("name,T,L", [("C1", 4, 4), ("C2", 6, 6), ("C3", 2, 6), ("C4", 4, 6)])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
 def test_kernel_variants(env, name, T, L, prec, variant):
     p = Problem(env, synth.CONFIGS[name].resized(T, L), prec)
+    check_all_ops(env, p, variant)
+
+
+@pytest.mark.parametrize("name,prec,variant", [("C2", "f64", 3), ("C2", "f32", 3), ("C3", "f64", 3), ("C4", "f32", 3),
+                                               ("C4", "f64", 4), ("C2", "f64", 4), ("C3", "f32", 4)])
+@pytest.mark.parametrize("bx,max_ctas", [(0, 1), (2, 1), (4, 3), (-1, 2)])
+def test_persistent_loop_and_tile_order(env, name, prec, variant, bx, max_ctas):
+    """Persistent kernels with MANY tiles per warp (grid capped at 1-3 CTAs: the bulk-copy ring wraps across tile
+    boundaries many times, mbarrier phases flip) and every traversal order (storage / x-blocked), on an 4x8^3
+    lattice whose (t,x) planes are whole tiles (L*L/2 = 32), so that the x-blocked order is actually taken."""
+    hirep = env["hirep"]
+    p = Problem(env, synth.CONFIGS[name].resized(4, 8), prec)
+    p.geom.set_tuning(hirep.TUNE_TILE_BLOCK, bx)
+    p.geom.set_tuning(hirep.TUNE_MAX_CTAS, max_ctas)
     check_all_ops(env, p, variant)
 
 
