@@ -30,13 +30,15 @@ METRIC = "Dphi_eo GFLOP/s & effective HBM GB/s (fraction of B200 peak), per N_g/
 
 
 # ------------------------------------------------------------------------------- cost model
-def cost_model(cfg, prec):
+def cost_model(cfg, prec, rebuild=False):
     d = cfg.d_R
     real = cfg.rep == 1
     w = 8 if prec == "f64" else 4
     S = 8 * d * w                                  # one spinor
     K = d * d * (1 if real else 2) * w             # one represented link
     KF = 2 * cfg.n_g ** 2 * w
+    if rebuild:                                    # link mode REBUILD streams fundamental links
+        K = KF
     F_hop = (64 if real else 128) * d * d + 56 * d
     V = cfg.volume
     ops = {
@@ -130,15 +132,19 @@ def run_ours(args):
 
     cfg = synth.CONFIGS[args.config]
     prec = args.prec
-    cm = cost_model(cfg, prec)
+    rebuild = args.link_mode == "rebuild"
+    cm = cost_model(cfg, prec, rebuild)
+    ops_run = [k for k in OP_ORDER if not (rebuild and k == "links_to_rep")]
     cdt = torch.complex128 if prec == "f64" else torch.complex64
     links_c, (psi_c,) = synth.make_inputs_torch(cfg, dev, cdt, n_spinors=1)
     geom = hirep.Geometry(cfg.T, cfg.L, cfg.n_g, cfg.rep, prec, device=dev)
     geom.set_kernel_variant(args.variant)
-    if args.bx != -1:
-        geom.set_tuning(hirep.TUNE_TILE_BLOCK, args.bx)
     lf = geom.links_import(links_c)
-    lr = geom.new_links_rep()
+    if rebuild:
+        geom.set_link_mode(hirep.LINKS_REBUILD)
+        lr = lf                                    # the operators read the fundamental field
+    else:
+        lr = geom.new_links_rep()
     x_full = geom.spinor_import(psi_c, hirep.FULL)
     hb = geom.sizes["spinor_half"]
     x_e, x_o = x_full[:hb], x_full[hb:]
@@ -155,7 +161,8 @@ def run_ours(args):
             fn()
 
     def step(record=False):
-        timed("links_to_rep", lambda: geom.links_to_rep(lf, out=lr), record)
+        if not rebuild:
+            timed("links_to_rep", lambda: geom.links_to_rep(lf, out=lr), record)
         timed("Dphi_eo", lambda: geom.Dphi_eo(x_o, lr, out=y_e), record)
         timed("Dphi_oe", lambda: geom.Dphi_oe(x_e, lr, out=y_o), record)
         timed("Dphi", lambda: geom.Dphi(m0, x_full, lr, out=y_full), record)
@@ -190,11 +197,11 @@ def run_ours(args):
         ms_total = float(tt.item())
     ms_step = ms_total / args.steps
 
-    flops_step = sum(cm["ops"][k][0] for k in OP_ORDER)
+    flops_step = sum(cm["ops"][k][0] for k in ops_run)
     value = world * flops_step / (ms_step * 1e-3) / 1e9
     peak, peak_src = peaks()
     per_op = {}
-    for k in OP_ORDER:
+    for k in ops_run:
         ms = sum(a.elapsed_time(b) for a, b in ev[k]) / len(ev[k])
         fl, by, by_ideal = cm["ops"][k]
         per_op[k] = {"ms": round(ms, 4), "gflops": round(fl / ms / 1e6, 1), "gbs": round(by / ms / 1e6, 1),
@@ -210,7 +217,7 @@ def run_ours(args):
 
     # ---- e2e: same step through hirep_apply_host with pinned host buffers
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not rebuild:
         links_h = links_c.cpu().pin_memory()
         psi_h = psi_c.cpu().pin_memory()
         idx = torch.arange(cfg.volume)
@@ -260,9 +267,10 @@ def run_ours(args):
             "vs_baseline": None, "dtype": prec, "data": "synthetic",
             "config": {"workload": "%s: SU(%d) %s (d_R=%d) %dx%d^3 %s; step = links_to_rep + Dphi_eo + Dphi_oe + Dphi + Dphi_hat + g5Dphi_sq"
                                    % (cfg.name, cfg.n_g, synth.REP_NAMES[cfg.rep], cfg.d_R, cfg.T, cfg.L, prec),
-                       "links": "stored represented links (gather layout)", "kernel_variant": args.variant,
+                       "links": ("fundamental links, R rebuilt in registers (link mode REBUILD; no links_to_rep in the step)" if rebuild
+                                 else "stored represented links (gather layout)"), "kernel_variant": args.variant,
                        "l2": "inputs larger than L2: each step streams %.2f GB of links and spinors (L2 = 126 MB)"
-                             % (sum(cm["ops"][k][1] for k in OP_ORDER) / 1e9),
+                             % (sum(cm["ops"][k][1] for k in ops_run) / 1e9),
                        "parallelism": "replicas x%d (no sharding; DESIGN.md)" % world},
             "gpu_launches": launches,
             "per_op": per_op,
@@ -350,7 +358,7 @@ def main():
     ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
     ap.add_argument("--variant", type=int, default=0)
-    ap.add_argument("--bx", type=int, default=-1, help="tile traversal x-block (hirep_set_tuning); -1 = library default")
+    ap.add_argument("--link-mode", default="stored", choices=["stored", "rebuild"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

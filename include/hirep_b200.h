@@ -107,10 +107,9 @@ int hirep_set_link_mode(hirep_geom *g, int mode); /* HIREP_LINKS_STORED | HIREP_
  * (list in DESIGN.md).  An unknown variant for the geometry's instantiation returns HIREP_EUNSUPPORTED. */
 int hirep_set_kernel_variant(hirep_geom *g, int variant);
 /* Measurement / test knobs of the persistent stencil kernels.  Results never depend on them.
- *   HIREP_TUNE_TILE_BLOCK  x-block size of the tile traversal order: -1 = library default (chosen from the lattice
- *                          and spinor size), 0 = storage order, n = blocks of n x-planes (ignored unless n divides L)
- *   HIREP_TUNE_MAX_CTAS    cap on the number of persistent CTAs (0 = one per SM) */
-enum { HIREP_TUNE_TILE_BLOCK = 0, HIREP_TUNE_MAX_CTAS = 1 };
+ *   HIREP_TUNE_MAX_CTAS    cap on the number of persistent CTAs (0 = one per SM); a small cap makes every warp
+ *                          walk many tiles, which the parity tests use on small lattices */
+enum { HIREP_TUNE_MAX_CTAS = 1 };
 int hirep_set_tuning(hirep_geom *g, int key, int value);
 /* number of kernels this library has launched on behalf of g since creation (bench.py's gpu_launches) */
 long hirep_launch_count(const hirep_geom *g);

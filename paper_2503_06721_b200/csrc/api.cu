@@ -19,7 +19,7 @@ struct hirep_geom {
     Geo geo;
     int N, rep, prec, dR, real;
     int mode, variant;
-    int tune_bx, tune_max_ctas;   // hirep_set_tuning
+    int tune_max_ctas;            // hirep_set_tuning
     cudaStream_t stream;
     void *ws_half, *ws_full;        // workspace spinors (lazy)
     // hirep_apply_host staging (lazy)
@@ -80,7 +80,7 @@ extern "C" int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep
     g->geo.Nh = (int)(V / 2);
     g->geo.n_tiles = (g->geo.Nh + TILE - 1) / TILE;
     g->geo.bc[0] = -1; g->geo.bc[1] = g->geo.bc[2] = g->geo.bc[3] = 1;
-    g->tune_bx = -1; g->tune_max_ctas = 0;
+    g->tune_max_ctas = 0;
     g->N = N_g; g->rep = rep; g->prec = prec; g->dR = dR; g->real = (rep == HIREP_ADJ);
     const size_t w = prec == HIREP_F64 ? 8 : 4;
     g->bytes_spinor_half = (size_t)g->geo.n_tiles * 4 * dR * TILE * 2 * w;
@@ -142,10 +142,6 @@ extern "C" int hirep_set_kernel_variant(hirep_geom *g, int variant) {
 extern "C" int hirep_set_tuning(hirep_geom *g, int key, int value) {
     if (!g) return fail(HIREP_EINVAL, "hirep_set_tuning: NULL geometry");
     switch (key) {
-    case HIREP_TUNE_TILE_BLOCK:
-        if (value < -1) return fail(HIREP_EINVAL, "hirep_set_tuning: tile block %d", value);
-        g->tune_bx = value;
-        return HIREP_OK;
     case HIREP_TUNE_MAX_CTAS:
         if (value < 0) return fail(HIREP_EINVAL, "hirep_set_tuning: max CTAs %d", value);
         g->tune_max_ctas = value;
@@ -196,7 +192,6 @@ extern "C" int hirep_links_to_rep(hirep_geom *g, void *native_rep, const void *n
 
 // ---- operators ------------------------------------------------------------------------------------
 static int hop(hirep_geom *g, HopLaunch L, const char *what) {
-    L.bx_req = g->tune_bx;
     L.max_ctas = g->tune_max_ctas;
     const int rc = g->prec == HIREP_F64 ? k_hop_f64(g->geo, g->N, g->rep, g->mode, g->variant, L, g->stream)
                                         : k_hop_f32(g->geo, g->N, g->rep, g->mode, g->variant, L, g->stream);

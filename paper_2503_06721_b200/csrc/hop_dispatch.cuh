@@ -6,8 +6,8 @@
 //   2 = direct-load kernel, two lanes per site           (hop_small.cuh, P = 2)
 //   3 = persistent kernel, link stream through a per-warp bulk-copy (TMA) ring in shared memory (hop_ring.cuh)
 //   4 = the same with two warps per tile, one per half-spinor component (hop_pair.cuh)
-// Default for d_R <= 6: variant 3, except fp64 with d_R >= 5 where one thread per site spills: variant 4
-// (measured on B200, profiles/).  Large d_R (>= 8) always uses the row-group
+// Default for d_R <= 6: variant 3, except at d_R >= 5 in fp64 (one thread per site spills) and for the fp32 passes
+// with a diagonal term: variant 4 (measured on B200, profiles/).  Link mode REBUILD always runs variant 4.  Large d_R (>= 8) always uses the row-group
 // kernel of hop_large.cuh.
 #pragma once
 #include "hop_large.cuh"
@@ -16,35 +16,46 @@
 namespace hirep {
 
 template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
-    if (variant == 0) variant = (sizeof(T) == 8 && DR >= 5) ? 4 : 3;
+    if (variant == 0) {
+        // one thread per site spills in fp64 from d_R = 5 on; in fp32 at d_R >= 5 only the passes with a diagonal
+        // term (self block in shared memory, fewer ring stages) run better with two warps per tile (profiles/)
+        const bool self = (L.a != 0.0) && L.set[0].self != nullptr;
+        variant = (DR >= 5 && (sizeof(T) == 8 || self)) ? 4 : 3;
+    }
     switch (variant) {
     case 1: return launch_hop_small<T, DR, REAL, 1, 128>(g, L, s);
     case 2: return launch_hop_small<T, DR, REAL, 2, 128>(g, L, s);
     case 3: return launch_hop_ring<T, DR, REAL>(g, L, s);
     case 4: return launch_hop_pair<T, DR, REAL>(g, L, s);
     }
-#ifdef HIREP_SWEEP   // ring-shape sweeps (not part of the library build): variant = 1000*WARPS + 100*STAGES + RPC
-    if constexpr (DR == HIREP_SWEEP && !REAL) {
-        const bool self = (L.a != 0.0) && L.set[0].self != nullptr;
-#define SW(W, S, R)                                                                                          \
-    if (variant == 1000 * W + 100 * S + R)                                                                   \
-        return self ? launch_hop_ring_cfg<T, DR, REAL, W, S, R, true>(g, L, s) : launch_hop_ring_cfg<T, DR, REAL, W, S, R, false>(g, L, s);
-#define SWN(W, S, R)                                                                                         \
-    if (variant == 1000 * W + 100 * S + R)                                                                   \
-        return self ? launch_hop_ring<T, DR, REAL>(g, L, s) : launch_hop_ring_cfg<T, DR, REAL, W, S, R, false>(g, L, s);
-        if constexpr (sizeof(T) == 4) {
-            SW(12, 2, 3) SW(12, 4, 2) SWN(11, 2, 6) SWN(10, 2, 6) SW(8, 2, 6) SW(10, 2, 3) SW(11, 2, 3) SW(12, 3, 2) SW(8, 4, 3)
-        } else {
-            SW(8, 4, 1) SW(8, 2, 2) SW(6, 2, 3) SW(6, 3, 2) SW(4, 4, 3)
-        }
-#undef SW
-#undef SWN
+    return KERR_UNSUPPORTED;
+}
+
+// link mode REBUILD: the pair kernel with the fundamental block in the ring and R rebuilt row by row (rep_maps.cuh).
+// Instantiated for every (N_g, rep) with d_R <= 6.
+template <typename T, int N, int REP> int hop_rebuild(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
+    using M = RepMap<T, N, REP>;
+    if (variant != 0 && variant != 4) return KERR_UNSUPPORTED;
+    return launch_hop_pair<T, M::DR, M::REAL, N, REP>(g, L, s);
+}
+template <typename T> int hop_rebuild_by_config(const Geo &g, int N, int rep, int variant, const HopLaunch &L, cudaStream_t s) {
+    switch (rep * 10 + N) {
+    case 2: return hop_rebuild<T, 2, 0>(g, variant, L, s);    // FUND
+    case 3: return hop_rebuild<T, 3, 0>(g, variant, L, s);
+    case 4: return hop_rebuild<T, 4, 0>(g, variant, L, s);
+    case 5: return hop_rebuild<T, 5, 0>(g, variant, L, s);
+    case 6: return hop_rebuild<T, 6, 0>(g, variant, L, s);
+    case 12: return hop_rebuild<T, 2, 1>(g, variant, L, s);   // ADJ SU(2), d_R = 3
+    case 22: return hop_rebuild<T, 2, 2>(g, variant, L, s);   // SYM SU(2), SU(3): d_R = 3, 6
+    case 23: return hop_rebuild<T, 3, 2>(g, variant, L, s);
+    case 33: return hop_rebuild<T, 3, 3>(g, variant, L, s);   // 2AS SU(3), SU(4): d_R = 3, 6
+    case 34: return hop_rebuild<T, 4, 3>(g, variant, L, s);
     }
-#endif
     return KERR_UNSUPPORTED;
 }
 
 template <typename T> int hop_by_config(const Geo &g, int N, int rep, int mode, int variant, const HopLaunch &L, cudaStream_t s) {
+    if (mode == 1) return hop_rebuild_by_config<T>(g, N, rep, variant, L, s);
     if (mode != 0) return KERR_UNSUPPORTED;
     const int dR = (rep == 0) ? N : (rep == 1) ? N * N - 1 : (rep == 2) ? N * (N + 1) / 2 : N * (N - 1) / 2;
     const bool real = (rep == 1);

@@ -14,7 +14,7 @@
 // Data movement is that of hop_ring.cuh: persistent CTAs, one ring of bulk-copy (TMA) slots per PAIR for the link
 // stream with full/empty mbarriers (the producer is lane 0 of warp 0 of the pair and refills a slot once BOTH
 // warps have released it), register prefetch of the next neighbour, the tile's own spinor by one bulk copy
-// (SELF), x-blocked traversal order.
+// (SELF).
 //
 // Link mode REBUILD (NF > 0): the ring carries the FUNDAMENTAL gather block (N_g x N_g per direction) and each
 // row of R(W) is rebuilt in registers by RepMap (rep_maps.cuh) -- "rebuilding the represented field on the fly",
@@ -102,14 +102,6 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
         const int gt = gp + k * np;
         set_ = two ? (gt & 1) : 0;
         int sq = two ? (gt >> 1) : gt;
-        if (L.ord_BX > 0) {
-            const int r = sq % L.ord_R;
-            int u = sq / L.ord_R;
-            const int xi = u % L.ord_BX;
-            u /= L.ord_BX;
-            const int tt = u % g.T, xb = u / g.T;
-            sq = (tt * g.L + xb * L.ord_BX + xi) * L.ord_R + r;
-        }
         tile_ = sq;
     };
 
@@ -289,8 +281,7 @@ int launch_hop_pair_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
         if (e != cudaSuccess) return (int)e;
         n_sm = sms;
     }
-    HopLaunch L = L0;
-    ring_tile_order<T, DR>(g, L);
+    const HopLaunch &L = L0;
     const int grid = ring_grid(n_sm, L.max_ctas, g.n_tiles * L.nsets, PAIRS);
     kern<<<grid, PAIRS * 64, Cfg::SMEM, s>>>(g, L);
     return (int)cudaGetLastError();

@@ -19,9 +19,6 @@
 //   * When the pass has a diagonal term (a != 0: Dphi, the second pass of Dphi_hat, g5Dphi_sq; template SELF) the
 //     tile's own spinor -- one contiguous 4 d_R x 32 block -- is fetched by ONE bulk copy at the start of the tile
 //     into a per-warp buffer and read in the epilogue, instead of being loaded (latency exposed) at the end.
-//   * Tile traversal order: tiles are dealt in x-blocked order (x-block, t, x in block, y, z) when the input
-//     spinor of one t-slice no longer fits comfortably in L2 (SU(4) 2AS fp64: 21 MB per slice), so that the
-//     t+-1 neighbours of a tile are processed a few MB -- not a whole t-slice -- apart (HopLaunch::ord_*).
 // No CTA-wide barrier anywhere: every warp is its own producer/consumer pipeline (lane 0 issues the bulk copies).
 #pragma once
 #include "hop_small.cuh"
@@ -140,35 +137,26 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
     const int my_chunks = my_tiles * CPT;
     const uint64_t pol = l2_policy_evict_first();
 
-    // k-th tile of this warp -> (set, tile): position gw + k*nw of the traversal order (x-blocked if ord_BX > 0)
+    // k-th tile of this warp -> (set, tile): tiles are dealt round-robin over all warps of the grid
     auto locate = [&](int k, int &set_, int &tile_) {
         const int gt = gw + k * nw;
         set_ = two ? (gt & 1) : 0;
         int sq = two ? (gt >> 1) : gt;
-        if (L.ord_BX > 0) {
-            const int r = sq % L.ord_R;
-            int u = sq / L.ord_R;
-            const int xi = u % L.ord_BX;
-            u /= L.ord_BX;
-            const int tt = u % g.T, xb = u / g.T;
-            sq = (tt * g.L + xb * L.ord_BX + xi) * L.ord_R + r;
-        }
         tile_ = sq;
     };
 
-    // chunk qi of this warp = chunk qi % CPT of its (qi / CPT)-th tile; a tile's chunks are consecutive in memory.
-    // The ring runs at most STAGES <= CPT chunks ahead, i.e. into the warp's next tile (n_set, n_tile) at most.
-    int set, tile, c_set = 0, c_tile = 0, n_set = 0, n_tile = 0;   // being fetched / being computed / next
-    auto issue = [&](int qi, int slot, int k_cur) {
+    // chunk qi of this warp = chunk qi % CPT of its (qi / CPT)-th tile; a tile's chunks are consecutive in memory
+    auto issue = [&](int qi, int slot) {
         const int kq = qi / CPT;
-        const int set_ = kq == k_cur ? c_set : n_set, tile_ = kq == k_cur ? c_tile : n_tile;
+        int set_, tile_;
+        locate(kq, set_, tile_);
         const E *src = (const E *)(set_ ? L.set[1].links : L.set[0].links) + ((size_t)tile_ * CPT + (qi - kq * CPT)) * CE;
         mbar_expect_tx(bars_s + 8 * slot, Cfg::CHUNK);
         bulk_g2s(ring_s + slot * Cfg::CHUNK, src, Cfg::CHUNK, bars_s + 8 * slot, pol);
     };
 
     // per-tile state
-    int t, x, y, zh, p_out;
+    int set, tile, t, x, y, zh, p_out;
     bool active;
     const C *in;
     auto enter_tile = [&]() {   // (set, tile) -> coordinates and pointers
@@ -186,13 +174,11 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
         for (int c = 0; c < NC; ++c) nb[c] = ld_spinor<T>(src + (size_t)c * TILE);
     };
 
-    locate(0, set, tile);
-    c_set = set;
-    c_tile = tile;
     if (lane == 0) {
         const int n0 = my_chunks < STAGES ? my_chunks : STAGES;
-        for (int qi = 0; qi < n0; ++qi) issue(qi, qi, 0);
+        for (int qi = 0; qi < n0; ++qi) issue(qi, qi);
     }
+    locate(0, set, tile);
     enter_tile();
     fetch(neighbour<0>(g, p_out, t, x, y, zh));
     int q = 0, slot = 0;
@@ -202,10 +188,8 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
 
     for (int k = 0; k < my_tiles; ++k) {
         // state of the tile being computed (enter_tile(k+1) below overwrites the shared variables at d = 7)
-        c_set = set;
-        c_tile = tile;
+        const int c_set = set, c_tile = tile;
         const bool c_active = active;
-        if (k + 1 < my_tiles) locate(k + 1, n_set, n_tile);
         if constexpr (SELF) {
             // the tile's own spinor: one contiguous block -> one bulk copy, consumed in the epilogue
             __syncwarp();   // every lane has finished reading the buffer in the previous epilogue
@@ -242,8 +226,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
                 fetch(neighbour<D + 1>(g, p_out, t, x, y, zh));
             } else {
                 if (k + 1 < my_tiles) {
-                    set = n_set;
-                    tile = n_tile;
+                    locate(k + 1, set, tile);
                     enter_tile();
                     fetch(neighbour<0>(g, p_out, t, x, y, zh));
                 }
@@ -271,7 +254,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
                 if (i % RPC == RPC - 1) {
                     // slot consumed by every lane -> refill it with the chunk STAGES ahead
                     __syncwarp();
-                    if (lane == 0 && q + STAGES < my_chunks) issue(q + STAGES, slot, k);
+                    if (lane == 0 && q + STAGES < my_chunks) issue(q + STAGES, slot);
                     ++q;
                     if (++slot == STAGES) { slot = 0; phase ^= 1; }
                 }
@@ -300,30 +283,6 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
     }
 }
 
-// x-blocked traversal order for one launch: ord_BX = 0 keeps the storage order.  One (t, x-block) slab of the input
-// spinor(s) is kept at or below SLAB_LIMIT bytes so that the slabs of t-1, t, t+1 stay in L2 next to the link stream.
-// L.bx_req (hirep_set_tuning) overrides the block size.
-template <typename T, int DR> void ring_tile_order(const Geo &g, HopLaunch &L) {
-    L.ord_R = 0;
-    L.ord_BX = 0;
-    const long row = (long)g.L * g.Lh;   // sites of one (t, x) row-plane
-    if (row % TILE != 0) return;
-    const int R = (int)(row / TILE);
-    int bx = 0;
-    if (L.bx_req >= 0) {
-        if (L.bx_req == 0 || g.L % L.bx_req != 0 || L.bx_req == g.L) return;
-        bx = L.bx_req;
-    } else {
-        constexpr double SLAB_LIMIT = 4.0 * 1024 * 1024;
-        const double per_x = (double)R * TILE * 4 * DR * sizeof(cplx<T>) * L.nsets;
-        if (per_x * g.L <= SLAB_LIMIT) return;   // a whole t-slice is small: storage order
-        for (int c = g.L - 1; c >= 2; --c)
-            if (g.L % c == 0 && per_x * c <= SLAB_LIMIT) { bx = c; break; }
-        if (bx == 0) bx = 2;
-    }
-    L.ord_R = R;
-    L.ord_BX = bx;
-}
 inline int ring_grid(int n_sm, int max_ctas, int total_tiles, int tiles_per_cta) {
     int grid = (total_tiles + tiles_per_cta - 1) / tiles_per_cta;
     if (grid > n_sm) grid = n_sm;
@@ -344,8 +303,7 @@ int launch_hop_ring_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
         if (e != cudaSuccess) return (int)e;
         n_sm = sms;
     }
-    HopLaunch L = L0;
-    ring_tile_order<T, DR>(g, L);
+    const HopLaunch &L = L0;
     const int grid = ring_grid(n_sm, L.max_ctas, g.n_tiles * L.nsets, WARPS);
     kern<<<grid, WARPS * 32, Cfg::SMEM, s>>>(g, L);
     return (int)cudaGetLastError();

@@ -21,8 +21,6 @@ struct HopLaunch {
     int nsets;          // 1 = half lattice, 2 = both parities in one launch
     double a, b;
     int g5;             // multiply the result by gamma_5 = diag(1,1,-1,-1)
-    int ord_R, ord_BX;  // tile traversal order, filled in by the launcher (hop_ring.cuh): 0 = storage order
-    int bx_req;         // requested x-block of the traversal order: -1 = library default, 0 = storage order, n = block
     int max_ctas;       // cap on the persistent grid (0 = one CTA per SM); tests use it to force many tiles per warp
 };
 

@@ -13,14 +13,14 @@ import ctypes
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libhirep_b200.so")
+LIB_PATH = os.environ.get("HIREP_B200_LIB", os.path.join(_HERE, "libhirep_b200.so"))   # override: A/B builds
 
 FUND, ADJ, SYM, ASY = 0, 1, 2, 3
 F64, F32 = 0, 1
 EVEN, ODD, FULL = 0, 1, 2
 LINKS_STORED, LINKS_REBUILD = 0, 1
 OP_DPHI, OP_DPHI_EO, OP_DPHI_OE, OP_DPHI_HAT, OP_G5DPHI_SQ = 0, 1, 2, 3, 4
-TUNE_TILE_BLOCK, TUNE_MAX_CTAS = 0, 1
+TUNE_MAX_CTAS = 1
 
 # every symbol include/hirep_b200.h declares
 SYMBOLS = [

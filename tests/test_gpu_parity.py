@@ -119,23 +119,25 @@ SMALL = [  # (config, T, L) : several tiles + ragged tail (Nh % 32 != 0) except 
 ]
 
 
-def check_all_ops(env, p, variant=0):
+def check_all_ops(env, p, variant=0, rebuild=False):
     oracle, hirep = env["oracle"], env["hirep"]
     cfg, g = p.cfg, p.geom
+    g.set_link_mode(hirep.LINKS_REBUILD if rebuild else hirep.LINKS_STORED)
+    links = p.links_fund if rebuild else p.links_rep
     T, L, d, m0 = cfg.T, cfg.L, cfg.d_R, cfg.m0
     tol = TOL[p.prec]
     g.set_kernel_variant(variant)
     psi = p.spinors[0]
     errs = {}
-    out = p.to_numpy(g.Dphi(m0, p.to_native(psi, hirep.FULL), p.links_rep), hirep.FULL)
+    out = p.to_numpy(g.Dphi(m0, p.to_native(psi, hirep.FULL), links), hirep.FULL)
     errs["Dphi"] = oracle.rel_l2(out, oracle.Dphi(T, L, d, m0, p.R, psi, p.bc))
-    out = p.to_numpy(g.Dphi_eo(p.to_native(psi[p.od], hirep.ODD), p.links_rep), hirep.EVEN)
+    out = p.to_numpy(g.Dphi_eo(p.to_native(psi[p.od], hirep.ODD), links), hirep.EVEN)
     errs["Dphi_eo"] = oracle.rel_l2(out, oracle.Dphi_eo(T, L, d, p.R, psi[p.od], p.bc))
-    out = p.to_numpy(g.Dphi_oe(p.to_native(psi[p.ev], hirep.EVEN), p.links_rep), hirep.ODD)
+    out = p.to_numpy(g.Dphi_oe(p.to_native(psi[p.ev], hirep.EVEN), links), hirep.ODD)
     errs["Dphi_oe"] = oracle.rel_l2(out, oracle.Dphi_oe(T, L, d, p.R, psi[p.ev], p.bc))
-    out = p.to_numpy(g.Dphi_hat(m0, p.to_native(psi[p.ev], hirep.EVEN), p.links_rep), hirep.EVEN)
+    out = p.to_numpy(g.Dphi_hat(m0, p.to_native(psi[p.ev], hirep.EVEN), links), hirep.EVEN)
     errs["Dphi_hat"] = oracle.rel_l2(out, oracle.Dphi_hat(T, L, d, m0, p.R, psi[p.ev], p.bc))
-    out = p.to_numpy(g.g5Dphi_sq(m0, p.to_native(psi, hirep.FULL), p.links_rep), hirep.FULL)
+    out = p.to_numpy(g.g5Dphi_sq(m0, p.to_native(psi, hirep.FULL), links), hirep.FULL)
     errs["g5Dphi_sq"] = oracle.rel_l2(out, oracle.g5Dphi_sq(T, L, d, m0, p.R, psi, p.bc))
     g.sync()
     for k, v in errs.items():
@@ -162,14 +164,12 @@ def test_kernel_variants(env, name, T, L, prec, variant):
 
 @pytest.mark.parametrize("name,prec,variant", [("C2", "f64", 3), ("C2", "f32", 3), ("C3", "f64", 3), ("C4", "f32", 3),
                                                ("C4", "f64", 4), ("C2", "f64", 4), ("C3", "f32", 4)])
-@pytest.mark.parametrize("bx,max_ctas", [(0, 1), (2, 1), (4, 3), (-1, 2)])
-def test_persistent_loop_and_tile_order(env, name, prec, variant, bx, max_ctas):
+@pytest.mark.parametrize("max_ctas", [1, 3])
+def test_persistent_loop(env, name, prec, variant, max_ctas):
     """Persistent kernels with MANY tiles per warp (grid capped at 1-3 CTAs: the bulk-copy ring wraps across tile
-    boundaries many times, mbarrier phases flip) and every traversal order (storage / x-blocked), on an 4x8^3
-    lattice whose (t,x) planes are whole tiles (L*L/2 = 32), so that the x-blocked order is actually taken."""
+    boundaries many times, mbarrier phases flip) on a 4x8^3 lattice (32 tiles per parity)."""
     hirep = env["hirep"]
     p = Problem(env, synth.CONFIGS[name].resized(4, 8), prec)
-    p.geom.set_tuning(hirep.TUNE_TILE_BLOCK, bx)
     p.geom.set_tuning(hirep.TUNE_MAX_CTAS, max_ctas)
     check_all_ops(env, p, variant)
 
@@ -178,6 +178,37 @@ def test_persistent_loop_and_tile_order(env, name, prec, variant, bx, max_ctas):
 def test_other_representations(env, n, rep):
     cfg = synth.Config("t", 4, 4, n, rep, -0.25, "haar", 500 + 10 * n + rep, ())
     check_all_ops(env, Problem(env, cfg, "f64"))
+
+
+REBUILD = [(2, FUND), (3, FUND), (4, FUND), (5, FUND), (6, FUND), (2, ADJ), (2, SYM), (3, SYM), (3, ASY), (4, ASY)]
+
+
+@pytest.mark.parametrize("n,rep", REBUILD)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_rebuild_mode(env, n, rep, prec):
+    """Link mode REBUILD (`links` = the fundamental field, R rebuilt in registers, boundary sign applied to the
+    half spinor) against the oracle, every (N_g, rep) with d_R <= 6; non-trivial signs in two directions and a
+    ragged tail."""
+    cfg = synth.Config("t", 6, 6, n, rep, -0.3, "haar", 700 + 10 * n + rep, ())
+    check_all_ops(env, Problem(env, cfg, prec, bc=(-1, 1, -1, 1)), rebuild=True)
+
+
+def test_rebuild_mode_persistent_and_unsupported(env):
+    hirep = env["hirep"]
+    p = Problem(env, synth.CONFIGS["C4"].resized(4, 8), "f64")
+    p.geom.set_tuning(hirep.TUNE_MAX_CTAS, 2)
+    check_all_ops(env, p, rebuild=True)
+    # stored and rebuilt agree with each other to rounding
+    x = p.to_native(p.spinors[0][p.ev], hirep.EVEN)
+    a = p.to_numpy(p.geom.Dphi_hat(-0.3, x, p.links_fund), hirep.EVEN)
+    p.geom.set_link_mode(hirep.LINKS_STORED)
+    b = p.to_numpy(p.geom.Dphi_hat(-0.3, x, p.links_rep), hirep.EVEN)
+    assert env["oracle"].rel_l2(a, b) < 1e-14
+    # d_R > 6 has no rebuild kernel: loud error, no fallback
+    q = Problem(env, synth.CONFIGS["C5"].resized(2, 2), "f64")
+    q.geom.set_link_mode(hirep.LINKS_REBUILD)
+    with pytest.raises(hirep.HirepError, match="no kernel instantiated"):
+        q.geom.Dphi_eo(q.to_native(q.spinors[0][q.od], hirep.ODD), q.links_fund)
 
 
 @pytest.mark.parametrize("bc", [(1, 1, 1, 1), (1, -1, 1, 1), (-1, -1, -1, -1), (-1, 1, 1, -1)])
