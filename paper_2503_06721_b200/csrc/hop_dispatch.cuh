@@ -11,6 +11,7 @@
 // kernel of hop_large.cuh.
 #pragma once
 #include "hop_large.cuh"
+#include "hop_rows.cuh"
 #include "hop_pair.cuh"
 
 namespace hirep {
@@ -28,6 +29,14 @@ template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int
     case 3: return launch_hop_ring<T, DR, REAL>(g, L, s);
     case 4: return launch_hop_pair<T, DR, REAL>(g, L, s);
     }
+    return KERR_UNSUPPORTED;
+}
+
+// d_R >= 8: variant 0 = row-group kernel with bulk-copy rings (hop_rows.cuh; R rows per warp, TP tiles per CTA),
+// variant 1 = the direct-load row-group kernel of round 1 (hop_large.cuh), kept for comparison
+template <typename T, int DR, bool REAL, int R, int TP> int hop_large_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
+    if (variant == 0) return launch_hop_rows<T, DR, REAL, R, TP>(g, L, s);
+    if (variant == 1) return launch_hop_large<T, DR, REAL, R>(g, L, s);
     return KERR_UNSUPPORTED;
 }
 
@@ -66,15 +75,17 @@ template <typename T> int hop_by_config(const Geo &g, int N, int rep, int mode, 
         case 4: return hop_small_variant<T, 4, false>(g, variant, L, s);
         case 5: return hop_small_variant<T, 5, false>(g, variant, L, s);
         case 6: return hop_small_variant<T, 6, false>(g, variant, L, s);
-        case 10: return variant == 0 ? launch_hop_large<T, 10, false, 5>(g, L, s) : KERR_UNSUPPORTED;
-        case 15: return variant == 0 ? launch_hop_large<T, 15, false, 5>(g, L, s) : KERR_UNSUPPORTED;
+        case 10: return hop_large_variant<T, 10, false, 5, 3>(g, variant, L, s);   // SU(4) SYM, SU(5) 2AS
+        case 15: return hop_large_variant<T, 15, false, 3, 2>(g, variant, L, s);   // SU(5) SYM, SU(6) 2AS
+        case 21: return hop_large_variant<T, 21, false, 3, 1>(g, variant, L, s);   // SU(6) SYM
         }
     } else {
         switch (dR) {
         case 3: return hop_small_variant<T, 3, true>(g, variant, L, s);
-        case 8: return variant == 0 ? launch_hop_large<T, 8, true, 4>(g, L, s) : KERR_UNSUPPORTED;
-        case 15: return variant == 0 ? launch_hop_large<T, 15, true, 5>(g, L, s) : KERR_UNSUPPORTED;
-        case 35: return variant == 0 ? launch_hop_large<T, 35, true, 5>(g, L, s) : KERR_UNSUPPORTED;
+        case 8: return hop_large_variant<T, 8, true, 4, 4>(g, variant, L, s);      // SU(3) ADJ
+        case 15: return hop_large_variant<T, 15, true, 3, 2>(g, variant, L, s);    // SU(4) ADJ
+        case 24: return hop_large_variant<T, 24, true, 4, 1>(g, variant, L, s);    // SU(5) ADJ
+        case 35: return hop_large_variant<T, 35, true, 5, 1>(g, variant, L, s);    // SU(6) ADJ
         }
     }
     return KERR_UNSUPPORTED;

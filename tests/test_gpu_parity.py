@@ -174,10 +174,24 @@ def test_persistent_loop(env, name, prec, variant, max_ctas):
     check_all_ops(env, p, variant)
 
 
-@pytest.mark.parametrize("n,rep", [(3, SYM), (3, ASY), (2, SYM), (4, FUND), (5, FUND), (3, ADJ), (4, SYM), (6, ASY), (4, ADJ)])
-def test_other_representations(env, n, rep):
+@pytest.mark.parametrize("n,rep", [(3, SYM), (3, ASY), (2, SYM), (4, FUND), (5, FUND), (3, ADJ), (4, SYM), (6, ASY), (4, ADJ),
+                                   (5, ASY), (5, SYM), (6, SYM), (5, ADJ)])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_other_representations(env, n, rep, prec):
+    """Every (N_g <= 6, rep) the library instantiates beyond the BASELINE configs (d_R up to 24)."""
     cfg = synth.Config("t", 4, 4, n, rep, -0.25, "haar", 500 + 10 * n + rep, ())
-    check_all_ops(env, Problem(env, cfg, "f64"))
+    check_all_ops(env, Problem(env, cfg, prec))
+
+
+@pytest.mark.parametrize("n,rep", [(3, ADJ), (4, SYM), (6, ASY), (6, ADJ)])
+@pytest.mark.parametrize("max_ctas,variant", [(1, 0), (3, 0), (0, 1)])
+def test_large_dR_kernels(env, n, rep, max_ctas, variant):
+    """d_R >= 8: the row-group ring kernel with many tiles per group (capped grid), and the direct-load kernel."""
+    hirep = env["hirep"]
+    cfg = synth.Config("t", 4, 6, n, rep, -0.4, "haar", 900 + 10 * n + rep, ())
+    p = Problem(env, cfg, "f64")
+    p.geom.set_tuning(hirep.TUNE_MAX_CTAS, max_ctas)
+    check_all_ops(env, p, variant)
 
 
 REBUILD = [(2, FUND), (3, FUND), (4, FUND), (5, FUND), (6, FUND), (2, ADJ), (2, SYM), (3, SYM), (3, ASY), (4, ASY)]
