@@ -109,14 +109,15 @@ template <typename T, int N> struct RepMap<T, N, 1> {   // ADJ (real matrix)
     static constexpr int DR = N * N - 1;
     static constexpr bool REAL = true;
     using E = T;
-    // Y = W^dagger T^a W (N x N), then R_ab = 2 Re tr(Y T^b)
+    // Y = W^dagger T^a W is Hermitian (T^a is), so only its upper triangle is built: Y[p*N+q], p <= q.  Then
+    // R_ab = 2 Re tr(Y T^b):  b = S_kl -> 2 Re Y_kl ;  b = A_kl -> -2 Im Y_kl ;  b = D_l -> diagonal combination.
     template <int A, typename WM> __device__ __forceinline__ static void row(const WM &W, E *w) {
         constexpr GenIdx ga = gen_decode(A);
         cplx<T> Y[N * N];
 #pragma unroll
         for (int p = 0; p < N; ++p)
 #pragma unroll
-            for (int q = 0; q < N; ++q) {
+            for (int q = p; q < N; ++q) {
                 if (ga.kind == 2) {
                     cplx<T> acc = mk<T>(0, 0);
 #pragma unroll
@@ -134,8 +135,8 @@ template <typename T, int N> struct RepMap<T, N, 1> {   // ADJ (real matrix)
         static_for<0, DR>([&](auto bc) {
             constexpr int B = decltype(bc)::value;
             constexpr GenIdx gb = gen_decode(B);
-            if constexpr (gb.kind == 0) w[B] = Y[gb.j * N + gb.i].x + Y[gb.i * N + gb.j].x;
-            else if constexpr (gb.kind == 1) w[B] = Y[gb.j * N + gb.i].y - Y[gb.i * N + gb.j].y;
+            if constexpr (gb.kind == 0) w[B] = 2 * Y[gb.i * N + gb.j].x;
+            else if constexpr (gb.kind == 1) w[B] = -2 * Y[gb.i * N + gb.j].y;
             else {
                 T acc = 0;
 #pragma unroll
