@@ -64,6 +64,22 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def max_over_ranks(value, dist, device=None):
+    """Timing rule of the bench contract: a multi-rank number is the MAX over ranks (all_reduce MAX; works for the
+    nccl backend on a GPU and for gloo on CPU, where the world_size-2 test runs it)."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(flops_per_replica_step, world, ms_step):
+    """Whole-job GFLOP/s of `world` independent replicas (weak scaling): units of all ranks / max time."""
+    return world * flops_per_replica_step / (ms_step * 1e-3) / 1e9
+
+
 class ClockSampler:
     """nvidia-smi sampling during the timed region (B200_PROFILING.md 'clocks line')."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -191,14 +207,11 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     ms_total = t0.elapsed_time(t1)
     launches = geom.launch_count() - launches0
-    if dist is not None:
-        tt = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
+    ms_total = max_over_ranks(ms_total, dist, dev)
     ms_step = ms_total / args.steps
 
     flops_step = sum(cm["ops"][k][0] for k in ops_run)
-    value = world * flops_step / (ms_step * 1e-3) / 1e9
+    value = aggregate_value(flops_step, world, ms_step)
     peak, peak_src = peaks()
     per_op = {}
     for k in ops_run:
@@ -247,11 +260,8 @@ def run_ours(args):
         torch.cuda.synchronize()
         w1 = time.perf_counter()
         ms_e2e = (w1 - w0) * 1e3 / ksteps
-        if dist is not None:
-            tt = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            ms_e2e = float(tt.item())
-        e2e = {"value": round(world * flops_step / (ms_e2e * 1e-3) / 1e9, 2), "unit": "GFLOP/s", "ms_per_step": round(ms_e2e, 3),
+        ms_e2e = max_over_ranks(ms_e2e, dist, dev)
+        e2e = {"value": round(aggregate_value(flops_step, world, ms_e2e), 2), "unit": "GFLOP/s", "ms_per_step": round(ms_e2e, 3),
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": ksteps,
                "api": "hirep_apply_host (pinned host canonical buffers; links copied once per step)"}
         del links_h, psi_h

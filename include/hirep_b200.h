@@ -120,6 +120,11 @@ long hirep_launch_count(const hirep_geom *g);
  * host memory.  Spinor extents follow the op (half lattice for EO/OE/HAT, full otherwise). */
 int hirep_apply_host(hirep_geom *g, int op, double m0, void *out_host, const void *in_host, const void *links_fund_host);
 
+/* Measurement utility: achieved TFLOP/s (2 flops per FMA) of a register-resident chain of
+ * FMAs in the given precision on the current device, the ALU roofline the pipe utilisation is read against.
+ * Synchronous; tflops is a host pointer. */
+int hirep_fma_peak(int prec, double *tflops);
+
 int hirep_sync(hirep_geom *g); /* synchronise the stream; returns any pending execution error */
 const char *hirep_last_error(void);
 

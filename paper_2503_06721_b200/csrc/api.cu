@@ -271,6 +271,14 @@ extern "C" int hirep_g5Dphi_sq(hirep_geom *g, double m0, void *out_full, const v
     return dphi_full(g, m0, out_full, g->ws_full, links, 1, "hirep_g5Dphi_sq (second g5 D)");
 }
 
+extern "C" int hirep_fma_peak(int prec, double *tflops) {
+    if (!tflops) return fail(HIREP_EINVAL, "hirep_fma_peak: NULL result pointer");
+    if (prec != HIREP_F64 && prec != HIREP_F32) return fail(HIREP_EINVAL, "hirep_fma_peak: unknown precision %d", prec);
+    const int rc = k_fma_peak(prec, tflops, 0);
+    if (rc != 0) return cuda_fail((cudaError_t)rc, "hirep_fma_peak");
+    return HIREP_OK;
+}
+
 extern "C" int hirep_sync(hirep_geom *g) {
     if (!g) return fail(HIREP_EINVAL, "hirep_sync: NULL geometry");
     cudaError_t e = cudaStreamSynchronize(g->stream);

@@ -31,6 +31,7 @@ int k_links_rep_export(const Geo &g, int prec, int dR, int real, void *canon, co
 int k_links_to_rep(const Geo &g, int prec, int N, int rep, void *native_rep, const void *native_fund, cudaStream_t s);
 // variant: 0 default; see hop_dispatch.cu.  mode: 0 stored represented links, 1 rebuild from fundamental (N, rep).
 int k_hop(const Geo &g, int prec, int N, int rep, int mode, int variant, const HopLaunch &L, cudaStream_t s);
+int k_fma_peak(int prec, double *tflops, cudaStream_t s);   // fma_peak.cu: measured FP64/FP32 FMA throughput
 // number of distinct kernel launches k_hop issues for this configuration (for launch accounting): always 1.
 
 }  // namespace hirep

@@ -28,7 +28,7 @@ SYMBOLS = [
     "hirep_spinor_import", "hirep_spinor_export", "hirep_links_import", "hirep_links_rep_export",
     "hirep_links_rep_export_bwd", "hirep_links_to_rep", "hirep_Dphi", "hirep_Dphi_eo", "hirep_Dphi_oe",
     "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_set_tuning", "hirep_launch_count",
-    "hirep_apply_host", "hirep_sync", "hirep_last_error",
+    "hirep_apply_host", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
 ]
 
 
@@ -72,6 +72,7 @@ def load():
     lib.hirep_launch_count.argtypes = [vp]
     lib.hirep_launch_count.restype = ctypes.c_long
     lib.hirep_apply_host.argtypes = [vp, ci, cd, vp, vp, vp]
+    lib.hirep_fma_peak.argtypes = [ci, ctypes.POINTER(cd)]
     lib.hirep_sync.argtypes = [vp]
     lib.hirep_last_error.restype = ctypes.c_char_p
     for n in SYMBOLS:
@@ -132,6 +133,12 @@ def hirep_set_link_mode(g, mode): _check(load().hirep_set_link_mode(g, mode))
 def hirep_set_kernel_variant(g, variant): _check(load().hirep_set_kernel_variant(g, variant))
 def hirep_set_tuning(g, key, value): _check(load().hirep_set_tuning(g, key, value))
 def hirep_launch_count(g): return int(load().hirep_launch_count(g))
+def hirep_fma_peak(prec):
+    out = ctypes.c_double()
+    _check(load().hirep_fma_peak(prec, ctypes.byref(out)))
+    return out.value
+
+
 def hirep_sync(g): _check(load().hirep_sync(g))
 
 
