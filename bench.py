@@ -56,6 +56,19 @@ def cost_model(cfg, prec, rebuild=False):
 OP_ORDER = ["links_to_rep", "Dphi_eo", "Dphi_oe", "Dphi", "Dphi_hat", "g5Dphi_sq"]
 
 
+def ncu_traffic(config, prec, op):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `op`, from the committed ncu capture
+    (profiles/r01b_traffic.csv; the command that made it is in profiles/r01b_summary.md)."""
+    path = os.path.join(ROOT, "profiles", "r01b_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    import csv
+    for row in csv.DictReader(open(path)):
+        if row["config"] == config and row["prec"] == prec and row["op"] == op:
+            return int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
+    return None
+
+
 def peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -81,51 +94,58 @@ def aggregate_value(flops_per_replica_step, world, ms_step):
 
 
 class ClockSampler:
-    """nvidia-smi sampling during the timed region (B200_PROFILING.md 'clocks line')."""
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons sampled DURING the timed region (B200_PROFILING.md 'clocks line') through NVML
+    (nvidia_ml_py: a sample every few ms from a thread, no process start-up); falls back to one nvidia-smi query."""
+    BAD = {"hw_slowdown": 0x8, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40, "sw_power_cap": 0x4}
 
     def __init__(self, index):
-        self.index, self.lines, self.proc = index, [], None
+        self.index, self.sm, self.mask, self.smax = index, [], 0, None
+        self.stop_flag = threading.Event()
+        self.thread = None
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.thread = threading.Thread(target=self._read, daemon=True)
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            # NVML enumerates physical devices: honour CUDA_VISIBLE_DEVICES when it is a plain index list
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+            phys = self.index
+            if vis and all(v.strip().isdigit() for v in vis.split(",")):
+                ids = [int(v) for v in vis.split(",")]
+                phys = ids[self.index] if self.index < len(ids) else self.index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.smax = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.thread = threading.Thread(target=self._loop, daemon=True)
             self.thread.start()
         except Exception:
-            self.proc = None
+            self.nv = None
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.lines.append(line.strip())
+    def _loop(self):
+        nv = self.nv
+        while not self.stop_flag.is_set():
+            try:
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                self.mask |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+            except Exception:
+                pass
+            time.sleep(0.003)
 
     def stop(self):
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=2)
-        except Exception:
-            self.proc.kill()
-        sm, smax, reasons = [], None, set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in self.lines:
-            f = [x.strip() for x in ln.split(",")]
-            if len(f) < 9:
-                continue
+        if self.thread is not None:
+            self.stop_flag.set()
+            self.thread.join(timeout=2)
+        if not self.sm:
             try:
-                sm.append(float(f[1])); smax = float(f[2])
-            except ValueError:
-                continue
-            for name, val in zip(names, f[5:9]):
-                if val.lower().startswith("active"):
-                    reasons.add(name)
-        sm.sort()
-        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
-                "samples": len(sm)}
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=clocks.sm,clocks.max.sm",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=20).stdout
+                f = [float(x) for x in out.strip().split(",")]
+                return {"sm_mhz": f[0], "sm_max_mhz": f[1], "reasons": ["sampled after the timed region (NVML unavailable)"], "samples": 1}
+            except Exception:
+                return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml and nvidia-smi unavailable"], "samples": 0}
+        sm = sorted(self.sm)
+        reasons = sorted(k for k, bit in self.BAD.items() if self.mask & bit)
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": self.smax, "reasons": reasons, "samples": len(sm)}
 
 
 # -------------------------------------------------------------------------------------------- our arm
@@ -220,10 +240,7 @@ def run_ours(args):
         per_op[k] = {"ms": round(ms, 4), "gflops": round(fl / ms / 1e6, 1), "gbs": round(by / ms / 1e6, 1),
                      "frac_hbm": round(by / ms / 1e6 / peak, 4), "gbs_paper_ideal_bytes": round(by_ideal / ms / 1e6, 1)}
     eo = per_op["Dphi_eo"]
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get("%s_%s" % (args.config, prec), {}).get("Dphi_eo_dram_bytes")
+    traffic = ncu_traffic(args.config, prec, "Dphi_eo") if not rebuild else None
     roofline = {"bound": "hbm", "kernel": "hop stencil (Dphi_eo pass)", "achieved": eo["gbs"], "peak": peak,
                 "unit": "GB/s", "frac": round(eo["gbs"] / peak, 4), "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes": cm["ops"]["Dphi_eo"][1], "frac_of_8TBs_nominal": round(eo["gbs"] / 8000.0, 4)}
@@ -362,7 +379,7 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
