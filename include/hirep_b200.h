@@ -120,6 +120,33 @@ long hirep_launch_count(const hirep_geom *g);
  * host memory.  Spinor extents follow the op (half lattice for EO/OE/HAT, full otherwise). */
 int hirep_apply_host(hirep_geom *g, int op, double m0, void *out_host, const void *in_host, const void *links_fund_host);
 
+/* ---- spinor linear algebra, reductions and the CG inverter (Sect. 4.2 / 5.1; the consumer of the hot path) ----
+ * Native spinor buffers (device pointers); `which` in {HIREP_EVEN, HIREP_ODD, HIREP_FULL} gives their extent.
+ * Complex coefficients are host pointers to {re, im}.  xi may alias eta or zeta (element-wise operations).
+ *   hirep_spinor_lc   xi = r1 eta + r2 zeta            (Eq 22)      hirep_spinor_lc1  xi <- xi + c1 eta          (Eq 24)
+ *   hirep_spinor_clc  xi = c1 eta + c2 zeta            (Eq 23)            hirep_spinor_lc2  xi <- c1 xi + c2 eta       (Eq 25)
+ *   *_add_assign      xi <- xi + (the same)            (L387)             hirep_spinor_lc3  xi <- c1 eta + c2 zeta - xi (Eq 26) */
+int hirep_spinor_lc(hirep_geom *g, int which, void *xi, double r1, const void *eta, double r2, const void *zeta);
+int hirep_spinor_clc(hirep_geom *g, int which, void *xi, const double c1[2], const void *eta, const double c2[2], const void *zeta);
+int hirep_spinor_lc_add_assign(hirep_geom *g, int which, void *xi, double r1, const void *eta, double r2, const void *zeta);
+int hirep_spinor_clc_add_assign(hirep_geom *g, int which, void *xi, const double c1[2], const void *eta, const double c2[2], const void *zeta);
+int hirep_spinor_lc1(hirep_geom *g, int which, void *xi, const double c1[2], const void *eta);
+int hirep_spinor_lc2(hirep_geom *g, int which, void *xi, const double c1[2], const double c2[2], const void *eta);
+int hirep_spinor_lc3(hirep_geom *g, int which, void *xi, const double c1[2], const void *eta, const double c2[2], const void *zeta);
+/* Reductions over the sites of the buffer (padding excluded); results are HOST doubles, the calls synchronise the
+ * stream.  Accumulation: Neumaier's compensated sum (Algorithm 2) in fp64 also for fp32 fields.
+ *   hirep_spinor_prod      out = {Re, Im} of <xi, eta> = sum conj(xi) eta            (Eq 27)
+ *   hirep_spinor_sqnorm    out = <xi, xi> = ||xi||_2^2                               (Eq 32)
+ *   hirep_spinor_max_norm  out = max over components of max(|Re|, |Im|)              (Eq 33) */
+int hirep_spinor_prod(hirep_geom *g, int which, const void *xi, const void *eta, double out[2]);
+int hirep_spinor_sqnorm(hirep_geom *g, int which, const void *xi, double *out);
+int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, double *out);
+/* Conjugate gradient (L730) for Q_m^2 x = b with Q_m^2 = g5Dphi_sq, Hermitian positive definite (L772); x starts at 0.
+ * Stops when ||r||_2 <= tol ||b||_2 (r the recurrence residual) or after maxiter iterations (not an error: check
+ * *relres).  Full-lattice native spinors; iters / relres are host pointers (may be NULL).  x must not alias b. */
+int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const void *b_full, const void *links, double tol, int maxiter,
+                       int *iters, double *relres);
+
 /* Measurement utility: achieved TFLOP/s (2 flops per FMA) of a register-resident chain of
  * FMAs in the given precision on the current device, the ALU roofline the pipe utilisation is read against.
  * Synchronous; tflops is a host pointer. */

@@ -5,6 +5,7 @@
 //   Dphi              : a = 4 + m,    b = -1/2, both parities in one launch     (Eq 8,  L207)
 //   Dphi_hat          : tmp_o = D_oe in_e ; out_e = (4+m)^2 in_e + 1/2 hop(tmp_o)   (Eq 44)
 //   g5Dphi_sq         : tmp = g5 D in ; out = g5 D tmp                          (Eq 11; L772)
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -22,6 +23,8 @@ struct hirep_geom {
     int tune_max_ctas;            // hirep_set_tuning
     cudaStream_t stream;
     void *ws_half, *ws_full;        // workspace spinors (lazy)
+    void *ws_red;                   // reduction partials + 4 result doubles (lazy)
+    void *cg_r, *cg_p, *cg_Ap;      // CG work fields (lazy)
     // hirep_apply_host staging (lazy)
     void *h_links_canon, *h_links_fund, *h_links_rep, *h_in_canon, *h_in_native, *h_out_native, *h_out_canon;
     int host_links_ready;
@@ -92,7 +95,7 @@ extern "C" int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep
 
 extern "C" int hirep_geom_destroy(hirep_geom *g) {
     if (!g) return HIREP_OK;
-    void *bufs[] = {g->ws_half, g->ws_full, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
+    void *bufs[] = {g->ws_half, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
                     g->h_in_native, g->h_out_native, g->h_out_canon};
     for (void *b : bufs)
         if (b) cudaFree(b);
@@ -269,6 +272,133 @@ extern "C" int hirep_g5Dphi_sq(hirep_geom *g, double m0, void *out_full, const v
     rc = dphi_full(g, m0, g->ws_full, in_full, links, 1, "hirep_g5Dphi_sq (first g5 D)");
     if (rc) return rc;
     return dphi_full(g, m0, out_full, g->ws_full, links, 1, "hirep_g5Dphi_sq (second g5 D)");
+}
+
+// ---- spinor linear algebra, reductions, CG ------------------------------------------
+static long spinor_elems(const hirep_geom *g, int which) {   // complex elements of a native buffer, padding included
+    return (long)g->geo.n_tiles * 4 * g->dR * TILE * (which == HIREP_FULL ? 2 : 1);
+}
+static int lincomb(hirep_geom *g, int which, void *xi, const double c0[2], int use_xi, const void *eta, const double c1[2],
+                   const void *zeta, const double c2[2], int use_zeta, const char *what) {
+    if (which < 0 || which > 2) return fail(HIREP_EINVAL, "%s: parity_or_full=%d", what, which);
+    return kern_result(g, k_lincomb(g->prec, spinor_elems(g, which), xi, c0, use_xi, eta, c1, zeta, c2, use_zeta, g->stream), what);
+}
+static const double ZERO2[2] = {0.0, 0.0}, ONE2[2] = {1.0, 0.0}, MINUS2[2] = {-1.0, 0.0};
+
+extern "C" int hirep_spinor_lc(hirep_geom *g, int which, void *xi, double r1, const void *eta, double r2, const void *zeta) {
+    CHECK_PTRS("hirep_spinor_lc", xi, eta, zeta);
+    const double c1[2] = {r1, 0.0}, c2[2] = {r2, 0.0};
+    return lincomb(g, which, xi, ZERO2, 0, eta, c1, zeta, c2, 1, "hirep_spinor_lc");
+}
+extern "C" int hirep_spinor_clc(hirep_geom *g, int which, void *xi, const double c1[2], const void *eta, const double c2[2], const void *zeta) {
+    CHECK_PTRS("hirep_spinor_clc", xi, eta, zeta);
+    if (!c1 || !c2) return fail(HIREP_EINVAL, "hirep_spinor_clc: NULL coefficient");
+    return lincomb(g, which, xi, ZERO2, 0, eta, c1, zeta, c2, 1, "hirep_spinor_clc");
+}
+extern "C" int hirep_spinor_lc_add_assign(hirep_geom *g, int which, void *xi, double r1, const void *eta, double r2, const void *zeta) {
+    CHECK_PTRS("hirep_spinor_lc_add_assign", xi, eta, zeta);
+    const double c1[2] = {r1, 0.0}, c2[2] = {r2, 0.0};
+    return lincomb(g, which, xi, ONE2, 1, eta, c1, zeta, c2, 1, "hirep_spinor_lc_add_assign");
+}
+extern "C" int hirep_spinor_clc_add_assign(hirep_geom *g, int which, void *xi, const double c1[2], const void *eta, const double c2[2], const void *zeta) {
+    CHECK_PTRS("hirep_spinor_clc_add_assign", xi, eta, zeta);
+    if (!c1 || !c2) return fail(HIREP_EINVAL, "hirep_spinor_clc_add_assign: NULL coefficient");
+    return lincomb(g, which, xi, ONE2, 1, eta, c1, zeta, c2, 1, "hirep_spinor_clc_add_assign");
+}
+extern "C" int hirep_spinor_lc1(hirep_geom *g, int which, void *xi, const double c1[2], const void *eta) {
+    CHECK_PTRS("hirep_spinor_lc1", xi, eta);
+    if (!c1) return fail(HIREP_EINVAL, "hirep_spinor_lc1: NULL coefficient");
+    return lincomb(g, which, xi, ONE2, 1, eta, c1, eta, ZERO2, 0, "hirep_spinor_lc1");
+}
+extern "C" int hirep_spinor_lc2(hirep_geom *g, int which, void *xi, const double c1[2], const double c2[2], const void *eta) {
+    CHECK_PTRS("hirep_spinor_lc2", xi, eta);
+    if (!c1 || !c2) return fail(HIREP_EINVAL, "hirep_spinor_lc2: NULL coefficient");
+    return lincomb(g, which, xi, c1, 1, eta, c2, eta, ZERO2, 0, "hirep_spinor_lc2");
+}
+extern "C" int hirep_spinor_lc3(hirep_geom *g, int which, void *xi, const double c1[2], const void *eta, const double c2[2], const void *zeta) {
+    CHECK_PTRS("hirep_spinor_lc3", xi, eta, zeta);
+    if (!c1 || !c2) return fail(HIREP_EINVAL, "hirep_spinor_lc3: NULL coefficient");
+    return lincomb(g, which, xi, MINUS2, 1, eta, c1, zeta, c2, 1, "hirep_spinor_lc3");
+}
+
+static int red_workspace(hirep_geom *g) { return workspace(&g->ws_red, (size_t)k_reduce_workspace_bytes() + 64); }
+static double *red_out(hirep_geom *g) { return (double *)((char *)g->ws_red + k_reduce_workspace_bytes()); }
+static int fetch_result(hirep_geom *g, double *host, int n, const char *what) {
+    cudaError_t e = cudaMemcpyAsync(host, red_out(g), n * sizeof(double), cudaMemcpyDeviceToHost, g->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
+    if (e != cudaSuccess) return cuda_fail(e, what);
+    return HIREP_OK;
+}
+static int reduce_prod(hirep_geom *g, int which, int mode, const void *xi, const void *eta, double *host, const char *what) {
+    if (which < 0 || which > 2) return fail(HIREP_EINVAL, "%s: parity_or_full=%d", what, which);
+    int rc = red_workspace(g);
+    if (rc) return rc;
+    rc = kern_result(g, k_prod(g->geo, g->prec, g->dR, which == HIREP_FULL ? 2 : 1, mode, xi, eta, g->ws_red, red_out(g), g->stream), what, 2);
+    if (rc) return rc;
+    return fetch_result(g, host, 2, what);
+}
+extern "C" int hirep_spinor_prod(hirep_geom *g, int which, const void *xi, const void *eta, double out[2]) {
+    CHECK_PTRS("hirep_spinor_prod", xi, eta);
+    if (!out) return fail(HIREP_EINVAL, "hirep_spinor_prod: NULL result pointer");
+    return reduce_prod(g, which, 0, xi, eta, out, "hirep_spinor_prod");
+}
+extern "C" int hirep_spinor_sqnorm(hirep_geom *g, int which, const void *xi, double *out) {
+    CHECK_PTRS("hirep_spinor_sqnorm", xi);
+    if (!out) return fail(HIREP_EINVAL, "hirep_spinor_sqnorm: NULL result pointer");
+    double r[2];
+    const int rc = reduce_prod(g, which, 1, xi, xi, r, "hirep_spinor_sqnorm");
+    if (rc == HIREP_OK) *out = r[0];
+    return rc;
+}
+extern "C" int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, double *out) {
+    CHECK_PTRS("hirep_spinor_max_norm", eta);
+    if (!out) return fail(HIREP_EINVAL, "hirep_spinor_max_norm: NULL result pointer");
+    if (which < 0 || which > 2) return fail(HIREP_EINVAL, "hirep_spinor_max_norm: parity_or_full=%d", which);
+    int rc = red_workspace(g);
+    if (rc) return rc;
+    rc = kern_result(g, k_maxnorm(g->geo, g->prec, g->dR, which == HIREP_FULL ? 2 : 1, eta, g->ws_red, red_out(g), g->stream), "hirep_spinor_max_norm", 2);
+    if (rc) return rc;
+    return fetch_result(g, out, 1, "hirep_spinor_max_norm");
+}
+
+// Conjugate gradient for Q_m^2 x = b, Q_m^2 = g5Dphi_sq (Hermitian positive definite).  Textbook recurrence
+// (reading A19): r = b - A x0 with x0 = 0; p = r; repeat { Ap; alpha = rr/<p,Ap>; x += alpha p; r -= alpha Ap;
+// rr' = <r,r>; stop if rr' <= tol^2 <b,b>; beta = rr'/rr; p = r + beta p }.  7 launches per iteration: two stencil
+// launches, <p,Ap> (2), the fused update + ||r||^2 (2), the p update (1).
+extern "C" int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const void *b_full, const void *links, double tol,
+                                  int maxiter, int *iters, double *relres) {
+    CHECK_PTRS("hirep_cg_g5Dphi_sq", x_full, b_full, links);
+    if (x_full == b_full) return fail(HIREP_EINVAL, "hirep_cg_g5Dphi_sq: x aliases b");
+    if (!(tol > 0.0) || maxiter < 0) return fail(HIREP_EINVAL, "hirep_cg_g5Dphi_sq: tol=%g maxiter=%d", tol, maxiter);
+    const size_t fb = 2 * g->bytes_spinor_half;
+    int rc;
+    if ((rc = workspace(&g->cg_r, fb)) || (rc = workspace(&g->cg_p, fb)) || (rc = workspace(&g->cg_Ap, fb)) || (rc = red_workspace(g))) return rc;
+    cudaError_t e = cudaMemsetAsync(x_full, 0, fb, g->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(g->cg_r, b_full, fb, cudaMemcpyDeviceToDevice, g->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(g->cg_p, b_full, fb, cudaMemcpyDeviceToDevice, g->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "hirep_cg_g5Dphi_sq: setup");
+    double bb, rr, res[2];
+    if ((rc = hirep_spinor_sqnorm(g, HIREP_FULL, b_full, &bb))) return rc;
+    rr = bb;
+    int it = 0;
+    while (bb > 0.0 && it < maxiter && rr > tol * tol * bb) {
+        if ((rc = hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links))) return rc;
+        if ((rc = reduce_prod(g, HIREP_FULL, 0, g->cg_p, g->cg_Ap, res, "hirep_cg_g5Dphi_sq: <p,Ap>"))) return rc;
+        if (!(res[0] > 0.0)) return fail(HIREP_EINVAL, "hirep_cg_g5Dphi_sq: <p,Ap> = %g is not positive (operator not positive definite?)", res[0]);
+        const double alpha = rr / res[0];
+        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, 2, alpha, x_full, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, red_out(g), g->stream),
+                         "hirep_cg_g5Dphi_sq: update", 2);
+        if (rc) return rc;
+        if ((rc = fetch_result(g, res, 2, "hirep_cg_g5Dphi_sq: ||r||^2"))) return rc;
+        const double rr_new = res[0];
+        ++it;
+        const double beta[2] = {rr_new / rr, 0.0};
+        if ((rc = lincomb(g, HIREP_FULL, g->cg_p, beta, 1, g->cg_r, ONE2, g->cg_r, ZERO2, 0, "hirep_cg_g5Dphi_sq: p update"))) return rc;
+        rr = rr_new;
+    }
+    if (iters) *iters = it;
+    if (relres) *relres = bb > 0.0 ? sqrt(rr / bb) : 0.0;
+    return hirep_sync(g);
 }
 
 extern "C" int hirep_fma_peak(int prec, double *tflops) {

@@ -1,0 +1,277 @@
+// linalg.cu -- spinor linear algebra and reductions on native-layout spinors.
+//
+//   linear combinations   Eq 22-26: every form is xi = c0*xi + c1*eta + c2*zeta with complex
+//                         coefficients (a real coefficient is a complex one with zero imaginary part), one fused
+//                         kernel -- "fusing together one or more linear algebra kernels" (L379)
+//   reductions            Eq 27 (L402) <xi,eta>, Eq 32 (L426) ||xi||^2, Eq 33 (L430) max norm, accumulated with
+//                         Neumaier's compensated sum, Algorithm 2 (L662) -- the paper's default -- per thread, and
+//                         merged across lanes / warps / blocks with the branch-free two-sum (L654: "either variant
+//                         can be used"); fp32 fields are accumulated in fp64 (their products are exact in fp64)
+//   cg_update             the fused CG step  x += alpha p ; r -= alpha Ap ; ||r||^2  (one pass over four fields)
+//
+// All kernels are HBM-bound streaming passes: 128-bit accesses, grid = 4 CTAs per SM, grid-stride loops.  The
+// padding lanes of the last tile (sites h >= Nh) are excluded from every reduction.
+#include "kernels.h"
+
+namespace hirep {
+
+namespace {
+
+constexpr int RED_THREADS = 256;
+
+struct Acc {   // running compensated sum: value = s + c
+    double s, c;
+};
+__device__ __forceinline__ void two_sum(double a, double b, double &s, double &e) {   // branch-free variant of Alg 1
+    s = __dadd_rn(a, b);
+    const double bb = __dsub_rn(s, a);
+    e = __dadd_rn(__dsub_rn(a, __dsub_rn(s, bb)), __dsub_rn(b, bb));
+}
+__device__ __forceinline__ void acc_add(Acc &A, double x) {   // one step of Algorithm 2 (Neumaier)
+    double s, e;
+    two_sum(A.s, x, s, e);
+    A.s = s;
+    A.c = __dadd_rn(A.c, e);
+}
+__device__ __forceinline__ void acc_merge(Acc &A, const Acc &B) {
+    double s, e;
+    two_sum(A.s, B.s, s, e);
+    A.s = s;
+    A.c = __dadd_rn(__dadd_rn(A.c, B.c), e);
+}
+__device__ __forceinline__ Acc acc_shfl_down(const Acc &A, int off) {
+    Acc B;
+    B.s = __shfl_down_sync(0xffffffffu, A.s, off);
+    B.c = __shfl_down_sync(0xffffffffu, A.c, off);
+    return B;
+}
+// block-wide merge of NV accumulators per thread; result valid in thread 0
+template <int NV> __device__ void block_merge(Acc (&a)[NV]) {
+    __shared__ Acc sh[NV][RED_THREADS / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            const Acc b = acc_shfl_down(a[v], off);
+            acc_merge(a[v], b);
+        }
+        if (lane == 0) sh[v][warp] = a[v];
+    }
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            Acc x = lane < RED_THREADS / 32 ? sh[v][lane] : Acc{0.0, 0.0};
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+                const Acc b = acc_shfl_down(x, off);
+                acc_merge(x, b);
+            }
+            a[v] = x;
+        }
+    }
+}
+
+// Which elements of a native spinor buffer are real sites: element i = (row r = i >> 5, lane = i & 31), row =
+// (half, tile, component); only the LAST tile of each half lattice has padding lanes (lane >= Nh % 32).  No division.
+struct Pad {
+    long rows_per_half;   // n_tiles * ncomp
+    int ncomp, valid;     // valid lanes of the last tile (32 = no padding)
+};
+__device__ __forceinline__ bool is_site(const Pad &P, long i) {
+    if (P.valid == TILE) return true;
+    long r = i >> 5;
+    if (r >= P.rows_per_half) r -= P.rows_per_half;
+    return r < P.rows_per_half - P.ncomp || (int)(i & (TILE - 1)) < P.valid;
+}
+
+// ---- xi = c0*xi + c1*eta + c2*zeta --------------------------------------------------------------------------
+template <typename T, bool USE_XI, bool USE_ZETA>
+__global__ void __launch_bounds__(256) lincomb_kernel(long n, cplx<T> *__restrict__ xi, double2 c0, const cplx<T> *__restrict__ eta,
+                                                      double2 c1, const cplx<T> *__restrict__ zeta, double2 c2) {
+    const T c0x = (T)c0.x, c0y = (T)c0.y, c1x = (T)c1.x, c1y = (T)c1.y, c2x = (T)c2.x, c2y = (T)c2.y;
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
+        const cplx<T> e = eta[i];
+        T re = c1x * e.x - c1y * e.y, im = c1x * e.y + c1y * e.x;
+        if (USE_ZETA) {
+            const cplx<T> z = zeta[i];
+            re += c2x * z.x - c2y * z.y;
+            im += c2x * z.y + c2y * z.x;
+        }
+        if (USE_XI) {
+            const cplx<T> x = xi[i];
+            re += c0x * x.x - c0y * x.y;
+            im += c0x * x.y + c0y * x.x;
+        }
+        xi[i] = mk<T>(re, im);
+    }
+}
+
+// ---- partial reductions: one Acc pair (or quadruple) per block -------------------------------------------------
+// mode 0: <xi,eta> (re, im)   mode 1: ||xi||^2 (re only)
+template <typename T, int MODE>
+__global__ void __launch_bounds__(RED_THREADS) prod_partial_kernel(Pad P, long n, const cplx<T> *__restrict__ xi,
+                                                                   const cplx<T> *__restrict__ eta, Acc *__restrict__ partial) {
+    Acc a[2] = {{0.0, 0.0}, {0.0, 0.0}};
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
+        if (!is_site(P, i)) continue;
+        const cplx<T> x = xi[i];
+        const double xr = (double)x.x, xm = (double)x.y;
+        if (MODE == 1) {
+            acc_add(a[0], __dmul_rn(xr, xr));
+            acc_add(a[0], __dmul_rn(xm, xm));
+        } else {
+            const cplx<T> e = eta[i];
+            const double er = (double)e.x, em = (double)e.y;
+            acc_add(a[0], __dmul_rn(xr, er));
+            acc_add(a[0], __dmul_rn(xm, em));
+            acc_add(a[1], __dmul_rn(xr, em));
+            acc_add(a[1], -__dmul_rn(xm, er));
+        }
+    }
+    block_merge<2>(a);
+    if (threadIdx.x == 0) { partial[2 * blockIdx.x] = a[0]; partial[2 * blockIdx.x + 1] = a[1]; }
+}
+
+// fused CG step: x += alpha p ; r -= alpha Ap ; partial ||r||^2          (alpha real: A is Hermitian positive definite)
+template <typename T>
+__global__ void __launch_bounds__(RED_THREADS) cg_update_kernel(Pad P, long n, double alpha, cplx<T> *__restrict__ x,
+                                                                cplx<T> *__restrict__ r, const cplx<T> *__restrict__ p,
+                                                                const cplx<T> *__restrict__ Ap, Acc *__restrict__ partial) {
+    Acc a[2] = {{0.0, 0.0}, {0.0, 0.0}};
+    const T al = (T)alpha;
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
+        const cplx<T> pv = p[i], av = Ap[i];
+        cplx<T> xv = x[i], rv = r[i];
+        xv.x += al * pv.x; xv.y += al * pv.y;
+        rv.x -= al * av.x; rv.y -= al * av.y;
+        x[i] = xv;
+        r[i] = rv;
+        if (is_site(P, i)) {
+            acc_add(a[0], __dmul_rn((double)rv.x, (double)rv.x));
+            acc_add(a[0], __dmul_rn((double)rv.y, (double)rv.y));
+        }
+    }
+    block_merge<2>(a);
+    if (threadIdx.x == 0) { partial[2 * blockIdx.x] = a[0]; partial[2 * blockIdx.x + 1] = a[1]; }
+}
+
+// second stage: merge the per-block accumulators (fixed order: deterministic), out[v] = s + c  (last line of Alg 2)
+__global__ void __launch_bounds__(RED_THREADS) reduce_final_kernel(int nblocks, const Acc *__restrict__ partial, double *__restrict__ out) {
+    Acc a[2] = {{0.0, 0.0}, {0.0, 0.0}};
+    for (int b = threadIdx.x; b < nblocks; b += RED_THREADS) {
+        acc_merge(a[0], partial[2 * b]);
+        acc_merge(a[1], partial[2 * b + 1]);
+    }
+    block_merge<2>(a);
+    if (threadIdx.x == 0) { out[0] = __dadd_rn(a[0].s, a[0].c); out[1] = __dadd_rn(a[1].s, a[1].c); }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(RED_THREADS) maxnorm_partial_kernel(Pad P, long n, const cplx<T> *__restrict__ xi, double *__restrict__ partial) {
+    double m = 0.0;
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
+        if (!is_site(P, i)) continue;
+        const cplx<T> x = xi[i];
+        m = fmax(m, fmax(fabs((double)x.x), fabs((double)x.y)));
+    }
+    __shared__ double sh[RED_THREADS / 32];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) m = fmax(m, __shfl_down_sync(0xffffffffu, m, off));
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < RED_THREADS / 32; ++w) m = fmax(m, sh[w]);
+        partial[blockIdx.x] = m;
+    }
+}
+__global__ void maxnorm_final_kernel(int nblocks, const double *__restrict__ partial, double *__restrict__ out) {
+    double m = 0.0;
+    for (int b = 0; b < nblocks; ++b) m = fmax(m, partial[b]);
+    out[0] = m;
+}
+
+int red_blocks() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 148;
+        n = 4 * sms;
+    }
+    return n;
+}
+int blocks_for(long n) {
+    const long need = (n + RED_THREADS - 1) / RED_THREADS;
+    const int cap = red_blocks();
+    return (int)(need < cap ? (need > 0 ? need : 1) : cap);
+}
+
+template <typename T>
+int lincomb_t(long n, void *xi, double2 c0, bool use_xi, const void *eta, double2 c1, const void *zeta, double2 c2, bool use_zeta, cudaStream_t s) {
+    const int nb = blocks_for(n);
+    auto X = (cplx<T> *)xi;
+    auto E = (const cplx<T> *)eta;
+    auto Z = (const cplx<T> *)zeta;
+    if (use_xi && use_zeta) lincomb_kernel<T, true, true><<<nb, 256, 0, s>>>(n, X, c0, E, c1, Z, c2);
+    else if (use_xi) lincomb_kernel<T, true, false><<<nb, 256, 0, s>>>(n, X, c0, E, c1, Z, c2);
+    else if (use_zeta) lincomb_kernel<T, false, true><<<nb, 256, 0, s>>>(n, X, c0, E, c1, Z, c2);
+    else lincomb_kernel<T, false, false><<<nb, 256, 0, s>>>(n, X, c0, E, c1, Z, c2);
+    return (int)cudaGetLastError();
+}
+
+}  // namespace
+
+int k_reduce_workspace_bytes() { return red_blocks() * 2 * (int)sizeof(Acc) + 64; }
+
+// n = number of complex elements of the buffer (padding included); halves = 1 or 2
+int k_lincomb(int prec, long n, void *xi, const double c0[2], int use_xi, const void *eta, const double c1[2], const void *zeta,
+              const double c2[2], int use_zeta, cudaStream_t s) {
+    const double2 a = make_double2(c0[0], c0[1]), b = make_double2(c1[0], c1[1]), c = make_double2(c2[0], c2[1]);
+    return prec == 0 ? lincomb_t<double>(n, xi, a, use_xi, eta, b, zeta, c, use_zeta, s)
+                     : lincomb_t<float>(n, xi, a, use_xi, eta, b, zeta, c, use_zeta, s);
+}
+
+// mode 0: <xi,eta> -> out_dev[0..1] ; mode 1: ||xi||^2 -> out_dev[0] ; ws = k_reduce_workspace_bytes() device bytes
+int k_prod(const Geo &g, int prec, int dR, int halves, int mode, const void *xi, const void *eta, void *ws, double *out_dev, cudaStream_t s) {
+    const int ncomp = 4 * dR;
+    const long half_elems = (long)g.n_tiles * ncomp * TILE, n = half_elems * halves;
+    const Pad P{(long)g.n_tiles * ncomp, ncomp, g.Nh % TILE == 0 ? TILE : g.Nh % TILE};
+    const int nb = blocks_for(n);
+    Acc *partial = (Acc *)ws;
+    if (prec == 0) {
+        if (mode == 0) prod_partial_kernel<double, 0><<<nb, RED_THREADS, 0, s>>>(P, n, (const double2 *)xi, (const double2 *)eta, partial);
+        else prod_partial_kernel<double, 1><<<nb, RED_THREADS, 0, s>>>(P, n, (const double2 *)xi, (const double2 *)eta, partial);
+    } else {
+        if (mode == 0) prod_partial_kernel<float, 0><<<nb, RED_THREADS, 0, s>>>(P, n, (const float2 *)xi, (const float2 *)eta, partial);
+        else prod_partial_kernel<float, 1><<<nb, RED_THREADS, 0, s>>>(P, n, (const float2 *)xi, (const float2 *)eta, partial);
+    }
+    reduce_final_kernel<<<1, RED_THREADS, 0, s>>>(nb, partial, out_dev);
+    return (int)cudaGetLastError();
+}
+
+int k_maxnorm(const Geo &g, int prec, int dR, int halves, const void *xi, void *ws, double *out_dev, cudaStream_t s) {
+    const int ncomp = 4 * dR;
+    const long half_elems = (long)g.n_tiles * ncomp * TILE, n = half_elems * halves;
+    const Pad P{(long)g.n_tiles * ncomp, ncomp, g.Nh % TILE == 0 ? TILE : g.Nh % TILE};
+    const int nb = blocks_for(n);
+    if (prec == 0) maxnorm_partial_kernel<double><<<nb, RED_THREADS, 0, s>>>(P, n, (const double2 *)xi, (double *)ws);
+    else maxnorm_partial_kernel<float><<<nb, RED_THREADS, 0, s>>>(P, n, (const float2 *)xi, (double *)ws);
+    maxnorm_final_kernel<<<1, 1, 0, s>>>(nb, (const double *)ws, out_dev);
+    return (int)cudaGetLastError();
+}
+
+int k_cg_update(const Geo &g, int prec, int dR, int halves, double alpha, void *x, void *r, const void *p, const void *Ap, void *ws,
+                double *out_dev, cudaStream_t s) {
+    const int ncomp = 4 * dR;
+    const long half_elems = (long)g.n_tiles * ncomp * TILE, n = half_elems * halves;
+    const Pad P{(long)g.n_tiles * ncomp, ncomp, g.Nh % TILE == 0 ? TILE : g.Nh % TILE};
+    const int nb = blocks_for(n);
+    Acc *partial = (Acc *)ws;
+    if (prec == 0) cg_update_kernel<double><<<nb, RED_THREADS, 0, s>>>(P, n, alpha, (double2 *)x, (double2 *)r, (const double2 *)p, (const double2 *)Ap, partial);
+    else cg_update_kernel<float><<<nb, RED_THREADS, 0, s>>>(P, n, alpha, (float2 *)x, (float2 *)r, (const float2 *)p, (const float2 *)Ap, partial);
+    reduce_final_kernel<<<1, RED_THREADS, 0, s>>>(nb, partial, out_dev);
+    return (int)cudaGetLastError();
+}
+
+}  // namespace hirep

@@ -28,7 +28,9 @@ SYMBOLS = [
     "hirep_spinor_import", "hirep_spinor_export", "hirep_links_import", "hirep_links_rep_export",
     "hirep_links_rep_export_bwd", "hirep_links_to_rep", "hirep_Dphi", "hirep_Dphi_eo", "hirep_Dphi_oe",
     "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_set_tuning", "hirep_launch_count",
-    "hirep_apply_host", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
+    "hirep_apply_host", "hirep_spinor_lc", "hirep_spinor_clc", "hirep_spinor_lc_add_assign", "hirep_spinor_clc_add_assign",
+    "hirep_spinor_lc1", "hirep_spinor_lc2", "hirep_spinor_lc3", "hirep_spinor_prod", "hirep_spinor_sqnorm",
+    "hirep_spinor_max_norm", "hirep_cg_g5Dphi_sq", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
 ]
 
 
@@ -72,6 +74,17 @@ def load():
     lib.hirep_launch_count.argtypes = [vp]
     lib.hirep_launch_count.restype = ctypes.c_long
     lib.hirep_apply_host.argtypes = [vp, ci, cd, vp, vp, vp]
+    c2p = ctypes.POINTER(cd)
+    for n in ("hirep_spinor_lc", "hirep_spinor_lc_add_assign"):
+        getattr(lib, n).argtypes = [vp, ci, vp, cd, vp, cd, vp]
+    for n in ("hirep_spinor_clc", "hirep_spinor_clc_add_assign", "hirep_spinor_lc3"):
+        getattr(lib, n).argtypes = [vp, ci, vp, c2p, vp, c2p, vp]
+    lib.hirep_spinor_lc1.argtypes = [vp, ci, vp, c2p, vp]
+    lib.hirep_spinor_lc2.argtypes = [vp, ci, vp, c2p, c2p, vp]
+    lib.hirep_spinor_prod.argtypes = [vp, ci, vp, vp, c2p]
+    lib.hirep_spinor_sqnorm.argtypes = [vp, ci, vp, c2p]
+    lib.hirep_spinor_max_norm.argtypes = [vp, ci, vp, c2p]
+    lib.hirep_cg_g5Dphi_sq.argtypes = [vp, cd, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_fma_peak.argtypes = [ci, ctypes.POINTER(cd)]
     lib.hirep_sync.argtypes = [vp]
     lib.hirep_last_error.restype = ctypes.c_char_p
@@ -133,6 +146,44 @@ def hirep_set_link_mode(g, mode): _check(load().hirep_set_link_mode(g, mode))
 def hirep_set_kernel_variant(g, variant): _check(load().hirep_set_kernel_variant(g, variant))
 def hirep_set_tuning(g, key, value): _check(load().hirep_set_tuning(g, key, value))
 def hirep_launch_count(g): return int(load().hirep_launch_count(g))
+def _c2(z):
+    z = complex(z)
+    return (ctypes.c_double * 2)(z.real, z.imag)
+
+
+def hirep_spinor_lc(g, which, xi, r1, eta, r2, zeta): _check(load().hirep_spinor_lc(g, which, xi, r1, eta, r2, zeta))
+def hirep_spinor_clc(g, which, xi, c1, eta, c2, zeta): _check(load().hirep_spinor_clc(g, which, xi, _c2(c1), eta, _c2(c2), zeta))
+def hirep_spinor_lc_add_assign(g, which, xi, r1, eta, r2, zeta): _check(load().hirep_spinor_lc_add_assign(g, which, xi, r1, eta, r2, zeta))
+def hirep_spinor_clc_add_assign(g, which, xi, c1, eta, c2, zeta): _check(load().hirep_spinor_clc_add_assign(g, which, xi, _c2(c1), eta, _c2(c2), zeta))
+def hirep_spinor_lc1(g, which, xi, c1, eta): _check(load().hirep_spinor_lc1(g, which, xi, _c2(c1), eta))
+def hirep_spinor_lc2(g, which, xi, c1, c2, eta): _check(load().hirep_spinor_lc2(g, which, xi, _c2(c1), _c2(c2), eta))
+def hirep_spinor_lc3(g, which, xi, c1, eta, c2, zeta): _check(load().hirep_spinor_lc3(g, which, xi, _c2(c1), eta, _c2(c2), zeta))
+
+
+def hirep_spinor_prod(g, which, xi, eta):
+    out = (ctypes.c_double * 2)()
+    _check(load().hirep_spinor_prod(g, which, xi, eta, out))
+    return complex(out[0], out[1])
+
+
+def hirep_spinor_sqnorm(g, which, xi):
+    out = (ctypes.c_double * 2)()
+    _check(load().hirep_spinor_sqnorm(g, which, xi, out))
+    return out[0]
+
+
+def hirep_spinor_max_norm(g, which, eta):
+    out = (ctypes.c_double * 2)()
+    _check(load().hirep_spinor_max_norm(g, which, eta, out))
+    return out[0]
+
+
+def hirep_cg_g5Dphi_sq(g, m0, x, b, links, tol, maxiter):
+    it, res = ctypes.c_int(), (ctypes.c_double * 2)()
+    _check(load().hirep_cg_g5Dphi_sq(g, m0, x, b, links, tol, maxiter, ctypes.byref(it), res))
+    return it.value, res[0]
+
+
 def hirep_fma_peak(prec):
     out = ctypes.c_double()
     _check(load().hirep_fma_peak(prec, ctypes.byref(out)))
@@ -258,6 +309,23 @@ class Geometry:
         hirep_apply_host(self.handle, op, m0, out.data_ptr(), inp_host.data_ptr(),
                          links_host.data_ptr() if links_host is not None else None)
         return out
+
+    # linear algebra / reductions / CG on native buffers (tensors); `which` gives the extent
+    def lc(self, which, xi, r1, eta, r2, zeta): hirep_spinor_lc(self.handle, which, xi.data_ptr(), r1, eta.data_ptr(), r2, zeta.data_ptr())
+    def clc(self, which, xi, c1, eta, c2, zeta): hirep_spinor_clc(self.handle, which, xi.data_ptr(), c1, eta.data_ptr(), c2, zeta.data_ptr())
+    def lc_add_assign(self, which, xi, r1, eta, r2, zeta): hirep_spinor_lc_add_assign(self.handle, which, xi.data_ptr(), r1, eta.data_ptr(), r2, zeta.data_ptr())
+    def clc_add_assign(self, which, xi, c1, eta, c2, zeta): hirep_spinor_clc_add_assign(self.handle, which, xi.data_ptr(), c1, eta.data_ptr(), c2, zeta.data_ptr())
+    def lc1(self, which, xi, c1, eta): hirep_spinor_lc1(self.handle, which, xi.data_ptr(), c1, eta.data_ptr())
+    def lc2(self, which, xi, c1, c2, eta): hirep_spinor_lc2(self.handle, which, xi.data_ptr(), c1, c2, eta.data_ptr())
+    def lc3(self, which, xi, c1, eta, c2, zeta): hirep_spinor_lc3(self.handle, which, xi.data_ptr(), c1, eta.data_ptr(), c2, zeta.data_ptr())
+    def prod(self, which, xi, eta): return hirep_spinor_prod(self.handle, which, xi.data_ptr(), eta.data_ptr())
+    def sqnorm(self, which, xi): return hirep_spinor_sqnorm(self.handle, which, xi.data_ptr())
+    def max_norm(self, which, eta): return hirep_spinor_max_norm(self.handle, which, eta.data_ptr())
+
+    def cg_g5Dphi_sq(self, m0, b, links, tol, maxiter, out=None):
+        out = self.new_spinor(FULL) if out is None else out
+        it, res = hirep_cg_g5Dphi_sq(self.handle, m0, out.data_ptr(), b.data_ptr(), links.data_ptr(), tol, maxiter)
+        return out, it, res
 
     def set_link_mode(self, mode): hirep_set_link_mode(self.handle, mode)
     def set_kernel_variant(self, v): hirep_set_kernel_variant(self.handle, v)

@@ -1,0 +1,127 @@
+"""GPU parity of the spinor linear algebra, the reductions and the CG inverter against
+oracle/linalg.py, through the C-ABI binding.
+
+Tolerances: linear combinations -- relative L2 <= 1e-13 (fp64) / 1e-5 (fp32) like the operators (one or two
+roundings per element); reductions -- the GPU's Neumaier sum against the correctly rounded sum of the same fp64
+products: |diff| <= 4 ulp of sum|terms| (compensated summation leaves O(eps) relative to the result plus the
+products' own rounding, which both sides share); max norm -- bit exact; CG -- both sides run the same recurrence to
+tol = 1e-10, so the two solutions differ by at most ~2 tol cond(Q^2): checked at 1e-7, and the true residual of the
+GPU solution (oracle operator) at 1e-9.
+"""
+import numpy as np
+import pytest
+
+from oracle import linalg as la
+from paper_2503_06721_b200 import synth
+from tests.gpu_helpers import BC
+from tests.test_gpu_parity import Problem, env, np_c  # noqa: F401  (env is a fixture)
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-13, "f32": 1e-5}
+CASES = [("C2", 6, 6), ("C3", 4, 8), ("C4", 2, 6)]     # ragged tail (Nh % 32 != 0) and whole tiles
+
+
+def fields(p, n, seed):
+    rng = np.random.default_rng(seed)
+    out = []
+    for _ in range(n):
+        f = synth.gaussian_spinor(rng, p.cfg.volume, p.cfg.d_R)
+        out.append(synth.round_to_precision(f, p.prec))
+    return out
+
+
+@pytest.mark.parametrize("name,T,L", CASES)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("which", ["full", "even", "odd"])
+def test_linear_combinations(env, name, T, L, prec, which):
+    hirep, oracle = env["hirep"], env["oracle"]
+    p = Problem(env, synth.CONFIGS[name].resized(T, L), prec)
+    w = {"full": hirep.FULL, "even": hirep.EVEN, "odd": hirep.ODD}[which]
+    sel = {"full": slice(None), "even": p.ev, "odd": p.od}[which]
+    xi0, eta0, zeta0 = [f[sel] for f in fields(p, 3, 42)]
+    g = p.geom
+    nat = lambda f: p.to_native(f, w)
+    c1, c2, r1, r2 = 0.75 - 1.25j, -0.5 + 2.0j, 1.5, -0.625
+    cases = [
+        ("lc", lambda xi, e, z: g.lc(w, xi, r1, e, r2, z), la.lc(r1, eta0, r2, zeta0)),
+        ("clc", lambda xi, e, z: g.clc(w, xi, c1, e, c2, z), la.clc(c1, eta0, c2, zeta0)),
+        ("lc_add_assign", lambda xi, e, z: g.lc_add_assign(w, xi, r1, e, r2, z), la.lc_add_assign(xi0, r1, eta0, r2, zeta0)),
+        ("clc_add_assign", lambda xi, e, z: g.clc_add_assign(w, xi, c1, e, c2, z), la.clc_add_assign(xi0, c1, eta0, c2, zeta0)),
+        ("lc1", lambda xi, e, z: g.lc1(w, xi, c1, e), la.lc1(xi0, c1, eta0)),
+        ("lc2", lambda xi, e, z: g.lc2(w, xi, c1, c2, e), la.lc2(xi0, c1, c2, eta0)),
+        ("lc3", lambda xi, e, z: g.lc3(w, xi, c1, e, c2, z), la.lc3(xi0, c1, eta0, c2, zeta0)),
+    ]
+    for nm, run, ref in cases:
+        xi, e, z = nat(xi0), nat(eta0), nat(zeta0)
+        run(xi, e, z)
+        got = p.to_numpy(xi, w)
+        assert oracle.rel_l2(got, ref) < TOL[prec], nm
+        # inputs untouched
+        assert np.array_equal(p.to_numpy(e, w), eta0) and np.array_equal(p.to_numpy(z, w), zeta0), nm
+
+
+@pytest.mark.parametrize("name,T,L", CASES)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_reductions(env, name, T, L, prec):
+    hirep = env["hirep"]
+    p = Problem(env, synth.CONFIGS[name].resized(T, L), prec)
+    xi0, eta0 = fields(p, 2, 7)
+    # plant the maximum on an imaginary part with negative sign, and make the sum ill conditioned
+    xi0[5, 1, 0] = complex(0.25, -7.5)
+    eps = 2.0 ** -52
+    for w, sel in ((hirep.FULL, slice(None)), (hirep.EVEN, p.ev), (hirep.ODD, p.od)):
+        a, b = xi0[sel], eta0[sel]
+        xa, xb = p.to_native(a, w), p.to_native(b, w)
+        mag = float(np.sum(np.abs(a.real * b.real)) + np.sum(np.abs(a.imag * b.imag)) + np.sum(np.abs(a.real * b.imag)) + np.sum(np.abs(a.imag * b.real)))
+        got, ref = p.geom.prod(w, xa, xb), la.prod(a, b)
+        assert abs(got - ref) <= 4 * eps * mag
+        assert abs(got - ref) <= 1e-13 * abs(ref) + 4 * eps * mag
+        n_got, n_ref = p.geom.sqnorm(w, xa), la.sqnorm(a)
+        assert abs(n_got - n_ref) <= 4 * eps * n_ref
+        assert p.geom.max_norm(w, xa) == la.max_norm(a)              # bit exact
+    # conj on the left: <xi,eta> = conj <eta,xi>
+    xa, xb = p.to_native(xi0, hirep.FULL), p.to_native(eta0, hirep.FULL)
+    assert p.geom.prod(hirep.FULL, xb, xa) == p.geom.prod(hirep.FULL, xa, xb).conjugate()
+
+
+def test_reduction_is_compensated(env):
+    """A sum that naive fp64 accumulation gets wrong by many ulps: 2^20 terms of size ~1 plus a few of size 2^40.
+    The GPU result must be within 2 ulp of the exact sum (Algorithm 2), far below the naive error."""
+    hirep = env["hirep"]
+    cfg = synth.CONFIGS["C2"].resized(8, 8)
+    p = Problem(env, cfg, "f64")
+    rng = np.random.default_rng(99)
+    f = (rng.uniform(0.5, 1.5, size=(cfg.volume, 4, cfg.d_R)) + 1j * rng.uniform(0.5, 1.5, size=(cfg.volume, 4, cfg.d_R)))
+    f[::997, 0, 0] = 2.0 ** 20
+    ref = la.sqnorm(f)
+    got = p.geom.sqnorm(hirep.FULL, p.to_native(f, hirep.FULL))
+    assert abs(got - ref) <= 2 * 2.0 ** -52 * ref
+    naive = la.naive_sum(np.concatenate([f.real.ravel() ** 2, f.imag.ravel() ** 2]).tolist())
+    assert abs(naive - ref) > 8 * 2.0 ** -52 * ref
+
+
+@pytest.mark.parametrize("name,T,L,prec,m0", [("C1", 4, 4, "f64", 0.6), ("C2", 4, 4, "f64", 0.4), ("C3", 4, 4, "f64", 0.5), ("C2", 4, 4, "f32", 0.6)])
+def test_cg_vs_oracle(env, name, T, L, prec, m0):
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS[name].resized(T, L)
+    p = Problem(env, cfg, prec)
+    b = p.spinors[0]
+    d = cfg.d_R
+    apply_A = lambda v: oracle.g5Dphi_sq(T, L, d, m0, p.R, v, BC)
+    tol = 1e-10 if prec == "f64" else 1e-5
+    x_ref, it_ref, res_ref, _ = la.cg(apply_A, b, tol, 3000)
+    x_nat, it, res = p.geom.cg_g5Dphi_sq(m0, p.to_native(b, hirep.FULL), p.links_rep, tol, 3000)
+    x = p.to_numpy(x_nat, hirep.FULL)
+    assert res <= tol and abs(it - it_ref) <= max(2, it_ref // 20), (it, it_ref)
+    bn = np.linalg.norm(b.ravel())
+    true_res = np.linalg.norm((b - apply_A(x)).ravel()) / bn
+    if prec == "f64":
+        assert oracle.rel_l2(x, x_ref) < 1e-7
+        assert true_res < 1e-9
+    else:
+        assert oracle.rel_l2(x, x_ref) < 1e-3
+        assert true_res < 1e-4
+    # maxiter is honoured and reported, not an error
+    _, it2, res2 = p.geom.cg_g5Dphi_sq(m0, p.to_native(b, hirep.FULL), p.links_rep, tol, 3)
+    assert it2 == 3 and res2 > tol
