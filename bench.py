@@ -283,6 +283,11 @@ def run_ours(args):
                "api": "hirep_apply_host (pinned host canonical buffers; links copied once per step)"}
         del links_h, psi_h
 
+    # ---- NEXT-1 row: linear algebra, reductions and CG on the same fields; outside the timed step
+    extras = None
+    if not args.no_extras and not rebuild:
+        extras = measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, peak)
+
     cpu = None
     if rank == 0 and not args.no_cpu_baseline:
         cpu = cpu_baseline(args.config, prec)
@@ -303,12 +308,59 @@ def run_ours(args):
             "per_op": per_op,
             "roofline": roofline,
             "e2e": e2e,
+            "next1_linalg_cg": extras,
             "cpu_baseline": cpu,
             "clocks": clocks,
         }
         print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, peak):
+    """GB/s of the streaming kernels (full-lattice spinors) and ms per CG iteration of hirep_cg_g5Dphi_sq."""
+    V, S = cfg.volume, cm["S"]
+    z_full = geom.new_spinor(hirep.FULL)
+    z_full.copy_(x_full)
+
+    def timeit(fn, reps=20):
+        fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    out = {}
+    ms = timeit(lambda: geom.lc(hirep.FULL, y_full, 0.5, x_full, -1.5, z_full))
+    out["lc"] = {"ms": round(ms, 4), "gbs": round(3 * S * V / ms / 1e6, 1), "frac_hbm": round(3 * S * V / ms / 1e6 / peak, 3)}
+    ms = timeit(lambda: geom.lc1(hirep.FULL, y_full, 0.5 + 0.25j, x_full))
+    out["lc1"] = {"ms": round(ms, 4), "gbs": round(3 * S * V / ms / 1e6, 1), "frac_hbm": round(3 * S * V / ms / 1e6 / peak, 3)}
+    ms = timeit(lambda: geom.sqnorm(hirep.FULL, x_full))
+    out["sqnorm"] = {"ms": round(ms, 4), "gbs": round(S * V / ms / 1e6, 1), "frac_hbm": round(S * V / ms / 1e6 / peak, 3),
+                     "note": "includes the result read-back and stream synchronisation"}
+    ms = timeit(lambda: geom.prod(hirep.FULL, x_full, z_full))
+    out["prod"] = {"ms": round(ms, 4), "gbs": round(2 * S * V / ms / 1e6, 1), "frac_hbm": round(2 * S * V / ms / 1e6 / peak, 3)}
+    # CG: a fixed number of iterations on a well-conditioned mass so that every iteration does the same work
+    iters = 20
+    geom.cg_g5Dphi_sq(2.0, x_full, lr, 1e-30, 2, out=y_full)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    _, it, res = geom.cg_g5Dphi_sq(2.0, x_full, lr, 1e-30, iters, out=y_full)
+    torch.cuda.synchronize()
+    ms_it = (time.perf_counter() - t0) * 1e3 / max(it, 1)
+    fl_it = cm["ops"]["g5Dphi_sq"][0]
+    by_it = cm["ops"]["g5Dphi_sq"][1] + (2 + 6 + 3) * S * V      # stencils + <p,Ap> + fused update + p update
+    out["cg_g5Dphi_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gflops_operator": round(fl_it / ms_it / 1e6, 1),
+                           "gbs": round(by_it / ms_it / 1e6, 1), "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3),
+                           "launches_per_iteration": 7, "relres_after": res}
+    try:
+        out["fma_peak_tflops"] = {"f64": round(hirep.hirep_fma_peak(hirep.F64), 2), "f32": round(hirep.hirep_fma_peak(hirep.F32), 2)}
+    except Exception as e:   # measurement utility only
+        out["fma_peak_tflops"] = {"error": str(e)}
+    return out
 
 
 # ------------------------------------------------------------------------------- oracle arm / cpu baseline
@@ -337,16 +389,32 @@ def sample_flops(prep):
     return sum(cm["ops"][k][0] for k in OP_ORDER)
 
 
-SAMPLE = {"C1": (4, 4), "C2": (16, 16), "C3": (16, 16), "C4": (8, 8), "C5": (4, 4)}
+SAMPLE = {"C1": (4, 4), "C2": (16, 16), "C3": (16, 16), "C4": (8, 8), "C5": (4, 4)}   # small sub-lattice samples
+SAMPLE_BIG = {"C1": (4, 4), "C2": (32, 32), "C3": (24, 24), "C4": (12, 12), "C5": (8, 4)}  # larger ones (C1, C2: the full lattice)
+
+
+def pick_sample(config, prec, n_steps, budget_s):
+    """The larger of the two sample lattices if n_steps oracle steps on it fit budget_s: one step of the small sample is
+    timed and the big one extrapolated by volume (the oracle's cost is linear in the number of sites)."""
+    small = prepare_sample(config, prec, *SAMPLE[config])
+    t_small = oracle_step(small)
+    Tb, Lb = SAMPLE_BIG[config]
+    ratio = (Tb * Lb ** 3) / float(SAMPLE[config][0] * SAMPLE[config][1] ** 3)
+    if ratio > 1 and t_small * ratio * n_steps * 1.3 <= budget_s:
+        return prepare_sample(config, prec, Tb, Lb), (Tb, Lb)
+    return small, SAMPLE[config]
 
 
 def cpu_baseline(config, prec):
+    """The oracle as it stands on the host cores: whole steps on a bounded sample, repeated for about 10-20 s."""
     from oracle import oracle as orc
-    T, L = SAMPLE[config]
-    prep = prepare_sample(config, prec, T, L)
-    secs = oracle_step(prep)
-    return {"value": round(sample_flops(prep) / secs / 1e9, 3), "unit": "GFLOP/s", "cores": orc.num_threads(), "kind": "oracle",
-            "sample": "one step (same six ops) of %s on a %dx%d^3 sub-lattice, %.1f s" % (config, T, L, secs)}
+    prep, (T, L) = pick_sample(config, prec, 3, 30.0)
+    secs, n = 0.0, 0
+    while n < 1 or (secs < 10.0 and n < 200):
+        secs += oracle_step(prep)
+        n += 1
+    return {"value": round(n * sample_flops(prep) / secs / 1e9, 3), "unit": "GFLOP/s", "cores": orc.num_threads(), "kind": "oracle",
+            "sample": "%d steps (same six ops) of %s on a %dx%d^3 lattice, %.1f s of oracle time" % (n, config, T, L, secs)}
 
 
 def run_reference(args):
@@ -355,15 +423,14 @@ def run_reference(args):
         return
     from oracle import oracle as orc
     from paper_2503_06721_b200 import synth
-    T, L = SAMPLE[args.config]
-    prep = prepare_sample(args.config, args.prec, T, L)
+    prep, (T, L) = pick_sample(args.config, args.prec, args.steps + min(args.warmup, 1), 150.0)
     for _ in range(min(args.warmup, 1)):
         oracle_step(prep)
     secs = [oracle_step(prep) for _ in range(args.steps)]
     ms_step = sum(secs) * 1e3 / len(secs)
     gf = sample_flops(prep) / (ms_step * 1e-3) / 1e9
     cores, cfg = orc.num_threads(), synth.CONFIGS[args.config]
-    sample = "one step (same six ops) of %s on a %dx%d^3 sub-lattice" % (args.config, T, L)
+    sample = "one step (same six ops) of %s on a %dx%d^3 lattice" % (args.config, T, L)
     out = {"impl": "reference", "metric": METRIC, "value": round(gf, 3), "unit": "GFLOP/s", "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms_step, 2), "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -387,6 +454,7 @@ def main():
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--link-mode", default="stored", choices=["stored", "rebuild"])
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the linear-algebra / CG measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
