@@ -80,7 +80,7 @@ template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC, bool SE
     static_assert(SMEM <= 227 * 1024, "ring does not fit the 227 KB of shared memory of an sm_100 CTA");
 };
 
-// Library default ring shape per instantiation (B200 sweeps: profiles/r01_ring_sweep.md):
+// Library default ring shape per instantiation (B200 sweeps: profiles/r01b_summary.md):
 //   fp64: 8 warps (the thread-per-site kernel needs ~200 registers); fp32: 16 warps for d_R <= 3, else 12;
 //   chunk = the largest whole number of link rows that divides d_R, stays <= 13 KB and leaves room for two stages
 //   (large chunks beat deep rings: fewer barrier round trips per byte); then as many stages (<= 4) as fit.
