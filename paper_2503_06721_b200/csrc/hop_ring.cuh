@@ -276,8 +276,8 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
                         vu.x = fma(a, su.x, vu.x); vu.y = fma(a, su.y, vu.y);
                         vl.x = fma(a, sl.x, vl.x); vl.y = fma(a, sl.y, vl.y);
                     }
-                    out[(size_t)(s * DR + c) * TILE] = vu;
-                    out[(size_t)((2 + s) * DR + c) * TILE] = mk<T>(g5s * vl.x, g5s * vl.y);
+                    st_spinor(out + (size_t)(s * DR + c) * TILE, vu);
+                    st_spinor(out + (size_t)((2 + s) * DR + c) * TILE, mk<T>(g5s * vl.x, g5s * vl.y));
                 }
         }
     }

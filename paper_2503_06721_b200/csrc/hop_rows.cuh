@@ -216,8 +216,8 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
                         vu.x = fma(a, su.x, vu.x); vu.y = fma(a, su.y, vu.y);
                         vl.x = fma(a, sl.x, vl.x); vl.y = fma(a, sl.y, vl.y);
                     }
-                    out[(size_t)(s * DR + i) * TILE] = vu;
-                    out[(size_t)((2 + s) * DR + i) * TILE] = mk<T>(g5s * vl.x, g5s * vl.y);
+                    st_spinor(out + (size_t)(s * DR + i) * TILE, vu);
+                    st_spinor(out + (size_t)((2 + s) * DR + i) * TILE, mk<T>(g5s * vl.x, g5s * vl.y));
                 }
         }
     }
