@@ -87,6 +87,46 @@ def test_argument_errors_without_gpu(hirep):
     hirep.hirep_geom_destroy(None)
 
 
+def test_new_entry_points_argument_errors_without_gpu(hirep):
+    g = hirep.hirep_geom_create(4, 4, 3, hirep.FUND, hirep.F64)
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_spinor_lc(g, hirep.FULL, None, 1.0, 4096, 1.0, 8192)
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_spinor_lc(g, 5, 4096, 1.0, 8192, 1.0, 12288)          # bad extent selector
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_spinor_prod(g, hirep.EVEN, 4096 + 4, 8192)            # misaligned
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_cg_g5Dphi_sq(g, 0.1, 4096, 4096, 8192, 1e-8, 10)      # x aliases b
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_cg_g5Dphi_sq(g, 0.1, 4096, 8192, 12288, 0.0, 10)      # tol must be positive
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_set_tuning(g, 99, 1)
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_set_tuning(g, hirep.TUNE_MAX_CTAS, -2)
+    hirep.hirep_set_tuning(g, hirep.TUNE_MAX_CTAS, 4)
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_fma_peak(7)
+    assert hirep.hirep_launch_count(g) == 0
+    hirep.hirep_geom_destroy(g)
+
+
+def test_compute_without_device_is_an_error_not_a_fallback(hirep):
+    """On a box without a GPU every compute entry point reports HIREP_ECUDA (-3); nothing is computed on the CPU."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("needs a box without a CUDA device")
+    g = hirep.hirep_geom_create(4, 4, 3, hirep.FUND, hirep.F64)
+    buf = (ctypes.c_char * (1 << 20))()
+    base = (ctypes.addressof(buf) + 255) & ~255
+    with pytest.raises(hirep.HirepError, match="hirep error -3"):
+        hirep.hirep_Dphi_eo(g, base, base + 65536, base + 131072)
+    with pytest.raises(hirep.HirepError, match="hirep error -3"):
+        hirep.hirep_links_to_rep(g, base, base + 262144)
+    with pytest.raises(hirep.HirepError, match="hirep error -3"):
+        hirep.hirep_spinor_lc(g, hirep.EVEN, base, 1.0, base + 65536, 1.0, base + 131072)
+    hirep.hirep_geom_destroy(g)
+
+
 def test_missing_library_fails_loudly(hirep, monkeypatch):
     """The product path must not fall back to anything when the CUDA library is absent."""
     monkeypatch.setattr(hirep, "_lib", None)
