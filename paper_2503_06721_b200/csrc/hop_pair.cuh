@@ -115,7 +115,9 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
     };
     auto issue = [&](int slot) {
         mbar_expect_tx(full_s + 8 * slot, Cfg::CHUNK);
-        bulk_g2s(ring_s + slot * Cfg::CHUNK, iq_base + (size_t)iq_c * Cfg::CHUNK, Cfg::CHUNK, full_s + 8 * slot, pol);
+        // chunk iq_c of the tile = step iq_c / CPD of the walk -> direction dir_of<true>(step) of the gather block
+        const int step = iq_c / CPD, chunk = dir_of<true>(step) * CPD + (iq_c - step * CPD);
+        bulk_g2s(ring_s + slot * Cfg::CHUNK, iq_base + (size_t)chunk * Cfg::CHUNK, Cfg::CHUNK, full_s + 8 * slot, pol);
         if (++iq_c == CPT) {
             iq_c = 0;
             if (++iq_k < my_tiles) iq_enter();
@@ -152,7 +154,7 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
     };
 
     enter_tile(0);
-    fetch(neighbour<0>(g, p_out, t, x, y, zh), DirInfo<0>::swap);
+    fetch(neighbour<dir_of<true>(0)>(g, p_out, t, x, y, zh), DirInfo<dir_of<true>(0)>::swap);
     int q = 0, slot = 0;
     uint32_t phase = 0;
     const T a = (T)L.a, b = (T)L.b;
@@ -174,7 +176,7 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
         for (int c = 0; c < DR; ++c) up[c] = ls[c] = lx[c] = mk<T>(0, 0);
 
         static_for<0, 8>([&](auto dc) {
-            constexpr int D = decltype(dc)::value;
+            constexpr int I = decltype(dc)::value, D = dir_of<true>(I);
             using DI = DirInfo<D>;
             // (a2) spin projection: h_s = psi_s + sg e_mu psi_low
             const T cs = (T)(DI::sg * ((DI::mu < 2) ? -1 : (s ? 1 : -1)));
@@ -188,12 +190,13 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
                 if (DI::imag) hs[c] = mk<T>(fma(-cv, v.y, sgn * u.x), fma(cv, v.x, sgn * u.y));   // sgn (u + i cs v)
                 else hs[c] = mk<T>(fma(cv, v.x, sgn * u.x), fma(cv, v.y, sgn * u.y));             // sgn (u + cs v)
             }
-            if constexpr (D < 7) {
-                fetch(neighbour<D + 1>(g, p_out, t, x, y, zh), DirInfo<D + 1>::swap);
+            if constexpr (I < 7) {
+                constexpr int DN = dir_of<true>(I + 1);
+                fetch(neighbour<DN>(g, p_out, t, x, y, zh), DirInfo<DN>::swap);
             } else {
                 if (k + 1 < my_tiles) {
                     enter_tile(k + 1);
-                    fetch(neighbour<0>(g, p_out, t, x, y, zh), DirInfo<0>::swap);
+                    fetch(neighbour<dir_of<true>(0)>(g, p_out, t, x, y, zh), DirInfo<dir_of<true>(0)>::swap);
                 }
             }
             // (a3) link rows from the pair's ring, (a4) reconstruct + accumulate

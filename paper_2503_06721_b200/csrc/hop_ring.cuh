@@ -113,6 +113,8 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
     using Cfg = RingCfg<T, DR, REAL, WARPS, STAGES, RPC, SELF>;
     constexpr int NC = 4 * DR, CPD = Cfg::CPD, CPT = 8 * CPD;   // chunks per direction / per tile
     constexpr int CE = RPC * DR * TILE;                         // link elements per chunk
+    constexpr bool IL = !(sizeof(T) == 4 && DR >= 5);           // hop order (common.cuh): the 168-register fp32 kernels
+                                                                // at d_R = 5, 6 lose 13 % with the interleaved walk
     extern __shared__ __align__(128) unsigned char smem_raw[];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -150,7 +152,9 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
         const int kq = qi / CPT;
         int set_, tile_;
         locate(kq, set_, tile_);
-        const E *src = (const E *)(set_ ? L.set[1].links : L.set[0].links) + ((size_t)tile_ * CPT + (qi - kq * CPT)) * CE;
+        // chunk c of the tile = step c / CPD of the walk -> direction dir_of<IL>(step) of the gather block
+        const int c = qi - kq * CPT, step = c / CPD, chunk = dir_of<IL>(step) * CPD + (c - step * CPD);
+        const E *src = (const E *)(set_ ? L.set[1].links : L.set[0].links) + ((size_t)tile_ * CPT + chunk) * CE;
         mbar_expect_tx(bars_s + 8 * slot, Cfg::CHUNK);
         bulk_g2s(ring_s + slot * Cfg::CHUNK, src, Cfg::CHUNK, bars_s + 8 * slot, pol);
     };
@@ -180,7 +184,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
     }
     locate(0, set, tile);
     enter_tile();
-    fetch(neighbour<0>(g, p_out, t, x, y, zh));
+    fetch(neighbour<dir_of<IL>(0)>(g, p_out, t, x, y, zh));
     int q = 0, slot = 0;
     uint32_t phase = 0;
     const T a = (T)L.a, b = (T)L.b;
@@ -206,7 +210,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
             for (int c = 0; c < DR; ++c) up[s][c] = lo[s][c] = mk<T>(0, 0);
 
         static_for<0, 8>([&](auto dc) {
-            constexpr int D = decltype(dc)::value;
+            constexpr int I = decltype(dc)::value, D = dir_of<IL>(I);
             using DI = DirInfo<D>;
             // (a2) spin projection of the neighbour fetched earlier
             C hs[2][DR];
@@ -222,13 +226,13 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
                 }
             }
             // prefetch the next neighbour (next direction, or direction 0 of this warp's next tile)
-            if constexpr (D < 7) {
-                fetch(neighbour<D + 1>(g, p_out, t, x, y, zh));
+            if constexpr (I < 7) {
+                fetch(neighbour<dir_of<IL>(I + 1)>(g, p_out, t, x, y, zh));
             } else {
                 if (k + 1 < my_tiles) {
                     locate(k + 1, set, tile);
                     enter_tile();
-                    fetch(neighbour<0>(g, p_out, t, x, y, zh));
+                    fetch(neighbour<dir_of<IL>(0)>(g, p_out, t, x, y, zh));
                 }
             }
             // (a3) link matvec from the ring, (a4) reconstruct + accumulate

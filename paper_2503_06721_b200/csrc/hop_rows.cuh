@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
     // chunk qi of this warp: tile qi / CPT, direction (qi % CPT) / NJB, column block qi % NJB; R row segments
     auto issue = [&](int qi, int slot) {
         const int kq = qi / CPT, rem = qi - kq * CPT;
-        const int d = rem / NJB, jb = rem - d * NJB;
+        const int step = rem / NJB, jb = rem - step * NJB, d = dir_of<false>(step);   // the walk of common.cuh
         int set_, tile_;
         locate(kq, set_, tile_);
         const E *src = (const E *)(set_ ? L.set[1].links : L.set[0].links) +
@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
     };
 
     enter_tile(0);
-    fetch(neighbour<0>(g, p_out, t, x, y, zh));
+    fetch(neighbour<dir_of<false>(0)>(g, p_out, t, x, y, zh));
     int q = 0, slot = 0;
     uint32_t phase = 0;
     const T a = (T)L.a, b = (T)L.b;
@@ -131,9 +131,9 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
             for (int r = 0; r < R; ++r) up[s][r] = lo[s][r] = mk<T>(0, 0);
 
         static_for<0, 8>([&](auto dc) {
-            constexpr int D = decltype(dc)::value;
+            constexpr int I = decltype(dc)::value, D = dir_of<false>(I);
             using DI = DirInfo<D>;
-            C *hb = hbuf + (D & 1) * (2 * DR * TILE);
+            C *hb = hbuf + (I & 1) * (2 * DR * TILE);
             // (a2) projection of this warp's colours into the group's half-spinor buffer
 #pragma unroll
             for (int m = 0; m < R; ++m)
@@ -148,15 +148,15 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
                     hb[(s * DR + wg + NG * m) * TILE + lane] = hv;
                 }
             // prefetch the next neighbour (next direction, or direction 0 of the group's next tile)
-            if constexpr (D < 7) {
-                fetch(neighbour<D + 1>(g, p_out, t, x, y, zh));
+            if constexpr (I < 7) {
+                fetch(neighbour<dir_of<false>(I + 1)>(g, p_out, t, x, y, zh));
             } else {
                 if (k + 1 < my_tiles) {
                     enter_tile(k + 1);
-                    fetch(neighbour<0>(g, p_out, t, x, y, zh));
+                    fetch(neighbour<dir_of<false>(0)>(g, p_out, t, x, y, zh));
                 }
             }
-            group_sync(1 + grp, NG * 32);   // h of direction D complete; buffer (D&1) was last read at direction D-2
+            group_sync(1 + grp, NG * 32);   // h of step I complete; buffer (I&1) was last read at step I-2
             // (a3) rows i0 .. i0+R-1 times both half-spinor components, column block by column block
             C chi[2][R];
 #pragma unroll
