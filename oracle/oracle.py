@@ -177,6 +177,17 @@ def g5Dphi_sq(T, L, d_R, m0, Rlinks, psi, bc=DEFAULT_BC) -> np.ndarray:
     return out
 
 
+def g5Dphi_hat(T, L, d_R, m0, Rlinks, psi_even, bc=DEFAULT_BC) -> np.ndarray:
+    """Q_hat psi_e = gamma_5 D_hat psi_e (Eq 45) with D_hat in the normalisation of Eq 44 (L808): the literal
+    composition of the two oracle functions above (reading A22 of DESIGN.md)."""
+    return g5(Dphi_hat(T, L, d_R, m0, Rlinks, psi_even, bc))
+
+
+def g5Dphi_hat_sq(T, L, d_R, m0, Rlinks, psi_even, bc=DEFAULT_BC) -> np.ndarray:
+    """Q_hat^2 psi_e: the operator the even-odd preconditioned CG inverts (L772, L806)."""
+    return g5Dphi_hat(T, L, d_R, m0, Rlinks, g5Dphi_hat(T, L, d_R, m0, Rlinks, psi_even, bc), bc)
+
+
 def rel_l2(a: np.ndarray, b: np.ndarray) -> float:
     """||a - b||_2 / ||b||_2 in fp64 with compensated (math.fsum) accumulation."""
     import math
