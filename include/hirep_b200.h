@@ -101,6 +101,11 @@ int hirep_Dphi_eo(hirep_geom *g, void *out_even, const void *in_odd, const void 
 int hirep_Dphi_oe(hirep_geom *g, void *out_odd, const void *in_even, const void *links);
 int hirep_Dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links);
 int hirep_g5Dphi_sq(hirep_geom *g, double m0, void *out_full, const void *in_full, const void *links);
+/* The Hermitian even-odd preconditioned operator (Eq 45) in the normalisation of Eq 44 (A22):
+ *   hirep_g5Dphi_hat     out_even = gamma_5 ((4+m)^2 - D_eo D_oe) in_even = Q_hat in_even
+ *   hirep_g5Dphi_hat_sq  out_even = Q_hat Q_hat in_even      (Hermitian positive definite: what CG inverts in HMC, L772/L806) */
+int hirep_g5Dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links);
+int hirep_g5Dphi_hat_sq(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links);
 
 int hirep_set_link_mode(hirep_geom *g, int mode); /* HIREP_LINKS_STORED | HIREP_LINKS_REBUILD */
 /* Implementation variant of the stencil kernel, for measurements: 0 = library default, >0 = explicit
@@ -146,6 +151,9 @@ int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, double *out
  * *relres).  Full-lattice native spinors; iters / relres are host pointers (may be NULL).  x must not alias b. */
 int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const void *b_full, const void *links, double tol, int maxiter,
                        int *iters, double *relres);
+/* The same for Q_hat^2 x = b on the even sites (hirep_g5Dphi_hat_sq): even-odd preconditioned CG. */
+int hirep_cg_g5Dphi_hat_sq(hirep_geom *g, double m0, void *x_even, const void *b_even, const void *links, double tol, int maxiter,
+                           int *iters, double *relres);
 
 /* Measurement utility: achieved TFLOP/s (2 flops per FMA) of a register-resident chain of
  * FMAs in the given precision on the current device, the ALU roofline the pipe utilisation is read against.

@@ -22,7 +22,7 @@ struct hirep_geom {
     int mode, variant;
     int tune_max_ctas;            // hirep_set_tuning
     cudaStream_t stream;
-    void *ws_half, *ws_full;        // workspace spinors (lazy)
+    void *ws_half, *ws_half2, *ws_full;   // workspace spinors (lazy)
     void *ws_red;                   // reduction partials + 4 result doubles (lazy)
     void *cg_r, *cg_p, *cg_Ap;      // CG work fields (lazy)
     // hirep_apply_host staging (lazy)
@@ -95,7 +95,7 @@ extern "C" int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep
 
 extern "C" int hirep_geom_destroy(hirep_geom *g) {
     if (!g) return HIREP_OK;
-    void *bufs[] = {g->ws_half, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
+    void *bufs[] = {g->ws_half, g->ws_half2, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
                     g->h_in_native, g->h_out_native, g->h_out_canon};
     for (void *b : bufs)
         if (b) cudaFree(b);
@@ -248,20 +248,41 @@ extern "C" int hirep_Dphi(hirep_geom *g, double m0, void *out_full, const void *
     return dphi_full(g, m0, out_full, in_full, links, 0, "hirep_Dphi");
 }
 
-extern "C" int hirep_Dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links) {
-    CHECK_PTRS("hirep_Dphi_hat", out_even, in_even, links);
-    if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_Dphi_hat: out aliases in");
+// out_even = [gamma_5] ((4+m)^2 in_even - D_eo D_oe in_even): two half-lattice passes through the odd workspace
+static int dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links, int g5, const char *what) {
     int rc = workspace(&g->ws_half, g->bytes_spinor_half);
     if (rc) return rc;
-    rc = offdiag(g, g->ws_half, in_even, links, 1, "hirep_Dphi_hat (D_oe pass)");
+    rc = offdiag(g, g->ws_half, in_even, links, 1, what);
     if (rc) return rc;
     HopLaunch L{};
     L.nsets = 1;
     L.set[0] = HopSet{g->ws_half, out_even, in_even, links_parity(g, links, 0), 0};
     L.a = (4.0 + m0) * (4.0 + m0);
     L.b = +0.5;   // - D_eo = -(-1/2) hop
-    L.g5 = 0;
-    return hop(g, L, "hirep_Dphi_hat (D_eo pass)");
+    L.g5 = g5;
+    return hop(g, L, what);
+}
+
+extern "C" int hirep_Dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links) {
+    CHECK_PTRS("hirep_Dphi_hat", out_even, in_even, links);
+    if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_Dphi_hat: out aliases in");
+    return dphi_hat(g, m0, out_even, in_even, links, 0, "hirep_Dphi_hat");
+}
+
+extern "C" int hirep_g5Dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links) {
+    CHECK_PTRS("hirep_g5Dphi_hat", out_even, in_even, links);
+    if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_g5Dphi_hat: out aliases in");
+    return dphi_hat(g, m0, out_even, in_even, links, 1, "hirep_g5Dphi_hat");
+}
+
+extern "C" int hirep_g5Dphi_hat_sq(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links) {
+    CHECK_PTRS("hirep_g5Dphi_hat_sq", out_even, in_even, links);
+    if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_g5Dphi_hat_sq: out aliases in");
+    int rc = workspace(&g->ws_half2, g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = dphi_hat(g, m0, g->ws_half2, in_even, links, 1, "hirep_g5Dphi_hat_sq (first Q_hat)");
+    if (rc) return rc;
+    return dphi_hat(g, m0, out_even, g->ws_half2, links, 1, "hirep_g5Dphi_hat_sq (second Q_hat)");
 }
 
 extern "C" int hirep_g5Dphi_sq(hirep_geom *g, double m0, void *out_full, const void *in_full, const void *links) {
@@ -361,44 +382,58 @@ extern "C" int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, 
     return fetch_result(g, out, 1, "hirep_spinor_max_norm");
 }
 
-// Conjugate gradient for Q_m^2 x = b, Q_m^2 = g5Dphi_sq (Hermitian positive definite).  Textbook recurrence
-// (reading A19): r = b - A x0 with x0 = 0; p = r; repeat { Ap; alpha = rr/<p,Ap>; x += alpha p; r -= alpha Ap;
-// rr' = <r,r>; stop if rr' <= tol^2 <b,b>; beta = rr'/rr; p = r + beta p }.  7 launches per iteration: two stencil
-// launches, <p,Ap> (2), the fused update + ||r||^2 (2), the p update (1).
-extern "C" int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const void *b_full, const void *links, double tol,
-                                  int maxiter, int *iters, double *relres) {
-    CHECK_PTRS("hirep_cg_g5Dphi_sq", x_full, b_full, links);
-    if (x_full == b_full) return fail(HIREP_EINVAL, "hirep_cg_g5Dphi_sq: x aliases b");
-    if (!(tol > 0.0) || maxiter < 0) return fail(HIREP_EINVAL, "hirep_cg_g5Dphi_sq: tol=%g maxiter=%d", tol, maxiter);
-    const size_t fb = 2 * g->bytes_spinor_half;
+// Conjugate gradient for A x = b with A = Q_m^2 = g5Dphi_sq (full lattice) or A = Q_hat^2 = g5Dphi_hat_sq (even
+// sites), both Hermitian positive definite (L772, L815).  Textbook recurrence (reading A19): x0 = 0; r = b;
+// p = r; repeat { Ap; alpha = rr/<p,Ap>; x += alpha p; r -= alpha Ap; rr' = <r,r>; stop if rr' <= tol^2 <b,b>;
+// beta = rr'/rr; p = r + beta p }.  Per iteration: the operator (2 or 4 stencil launches), <p,Ap> (2 launches), the
+// fused update + ||r||^2 (2), the p update (1).
+static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, const void *links, double tol, int maxiter, int *iters,
+                    double *relres, const char *what) {
+    if (x == b) return fail(HIREP_EINVAL, "%s: x aliases b", what);
+    if (!(tol > 0.0) || maxiter < 0) return fail(HIREP_EINVAL, "%s: tol=%g maxiter=%d", what, tol, maxiter);
+    const int which = full ? HIREP_FULL : HIREP_EVEN, halves = full ? 2 : 1;
+    const size_t fb = halves * g->bytes_spinor_half;
     int rc;
-    if ((rc = workspace(&g->cg_r, fb)) || (rc = workspace(&g->cg_p, fb)) || (rc = workspace(&g->cg_Ap, fb)) || (rc = red_workspace(g))) return rc;
-    cudaError_t e = cudaMemsetAsync(x_full, 0, fb, g->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(g->cg_r, b_full, fb, cudaMemcpyDeviceToDevice, g->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(g->cg_p, b_full, fb, cudaMemcpyDeviceToDevice, g->stream);
-    if (e != cudaSuccess) return cuda_fail(e, "hirep_cg_g5Dphi_sq: setup");
+    // work fields are allocated at full-lattice size once and serve both operators
+    const size_t wb = 2 * g->bytes_spinor_half;
+    if ((rc = workspace(&g->cg_r, wb)) || (rc = workspace(&g->cg_p, wb)) || (rc = workspace(&g->cg_Ap, wb)) || (rc = red_workspace(g))) return rc;
+    cudaError_t e = cudaMemsetAsync(x, 0, fb, g->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(g->cg_r, b, fb, cudaMemcpyDeviceToDevice, g->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(g->cg_p, b, fb, cudaMemcpyDeviceToDevice, g->stream);
+    if (e != cudaSuccess) return cuda_fail(e, what);
     double bb, rr, res[2];
-    if ((rc = hirep_spinor_sqnorm(g, HIREP_FULL, b_full, &bb))) return rc;
+    if ((rc = hirep_spinor_sqnorm(g, which, b, &bb))) return rc;
     rr = bb;
     int it = 0;
     while (bb > 0.0 && it < maxiter && rr > tol * tol * bb) {
-        if ((rc = hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links))) return rc;
-        if ((rc = reduce_prod(g, HIREP_FULL, 0, g->cg_p, g->cg_Ap, res, "hirep_cg_g5Dphi_sq: <p,Ap>"))) return rc;
-        if (!(res[0] > 0.0)) return fail(HIREP_EINVAL, "hirep_cg_g5Dphi_sq: <p,Ap> = %g is not positive (operator not positive definite?)", res[0]);
-        const double alpha = rr / res[0];
-        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, 2, alpha, x_full, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, red_out(g), g->stream),
-                         "hirep_cg_g5Dphi_sq: update", 2);
+        rc = full ? hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links) : hirep_g5Dphi_hat_sq(g, m0, g->cg_Ap, g->cg_p, links);
         if (rc) return rc;
-        if ((rc = fetch_result(g, res, 2, "hirep_cg_g5Dphi_sq: ||r||^2"))) return rc;
+        if ((rc = reduce_prod(g, which, 0, g->cg_p, g->cg_Ap, res, what))) return rc;
+        if (!(res[0] > 0.0)) return fail(HIREP_EINVAL, "%s: <p,Ap> = %g is not positive (operator not positive definite?)", what, res[0]);
+        const double alpha = rr / res[0];
+        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, halves, alpha, x, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, red_out(g), g->stream), what, 2);
+        if (rc) return rc;
+        if ((rc = fetch_result(g, res, 2, what))) return rc;
         const double rr_new = res[0];
         ++it;
         const double beta[2] = {rr_new / rr, 0.0};
-        if ((rc = lincomb(g, HIREP_FULL, g->cg_p, beta, 1, g->cg_r, ONE2, g->cg_r, ZERO2, 0, "hirep_cg_g5Dphi_sq: p update"))) return rc;
+        if ((rc = lincomb(g, which, g->cg_p, beta, 1, g->cg_r, ONE2, g->cg_r, ZERO2, 0, what))) return rc;
         rr = rr_new;
     }
     if (iters) *iters = it;
     if (relres) *relres = bb > 0.0 ? sqrt(rr / bb) : 0.0;
     return hirep_sync(g);
+}
+
+extern "C" int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const void *b_full, const void *links, double tol,
+                                  int maxiter, int *iters, double *relres) {
+    CHECK_PTRS("hirep_cg_g5Dphi_sq", x_full, b_full, links);
+    return cg_solve(g, 1, m0, x_full, b_full, links, tol, maxiter, iters, relres, "hirep_cg_g5Dphi_sq");
+}
+extern "C" int hirep_cg_g5Dphi_hat_sq(hirep_geom *g, double m0, void *x_even, const void *b_even, const void *links, double tol,
+                                      int maxiter, int *iters, double *relres) {
+    CHECK_PTRS("hirep_cg_g5Dphi_hat_sq", x_even, b_even, links);
+    return cg_solve(g, 0, m0, x_even, b_even, links, tol, maxiter, iters, relres, "hirep_cg_g5Dphi_hat_sq");
 }
 
 extern "C" int hirep_fma_peak(int prec, double *tflops) {

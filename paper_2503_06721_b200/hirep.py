@@ -27,7 +27,7 @@ SYMBOLS = [
     "hirep_geom_create", "hirep_geom_destroy", "hirep_geom_set_bc", "hirep_geom_set_stream", "hirep_geom_sizes",
     "hirep_spinor_import", "hirep_spinor_export", "hirep_links_import", "hirep_links_rep_export",
     "hirep_links_rep_export_bwd", "hirep_links_to_rep", "hirep_Dphi", "hirep_Dphi_eo", "hirep_Dphi_oe",
-    "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_set_tuning", "hirep_launch_count",
+    "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_g5Dphi_hat", "hirep_g5Dphi_hat_sq", "hirep_cg_g5Dphi_hat_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_set_tuning", "hirep_launch_count",
     "hirep_apply_host", "hirep_spinor_lc", "hirep_spinor_clc", "hirep_spinor_lc_add_assign", "hirep_spinor_clc_add_assign",
     "hirep_spinor_lc1", "hirep_spinor_lc2", "hirep_spinor_lc3", "hirep_spinor_prod", "hirep_spinor_sqnorm",
     "hirep_spinor_max_norm", "hirep_cg_g5Dphi_sq", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
@@ -64,7 +64,7 @@ def load():
         getattr(lib, n).argtypes = [vp, vp, vp, ci]
     for n in ("hirep_links_import", "hirep_links_rep_export", "hirep_links_rep_export_bwd", "hirep_links_to_rep"):
         getattr(lib, n).argtypes = [vp, vp, vp]
-    for n in ("hirep_Dphi", "hirep_Dphi_hat", "hirep_g5Dphi_sq"):
+    for n in ("hirep_Dphi", "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_g5Dphi_hat", "hirep_g5Dphi_hat_sq"):
         getattr(lib, n).argtypes = [vp, cd, vp, vp, vp]
     for n in ("hirep_Dphi_eo", "hirep_Dphi_oe"):
         getattr(lib, n).argtypes = [vp, vp, vp, vp]
@@ -85,6 +85,7 @@ def load():
     lib.hirep_spinor_sqnorm.argtypes = [vp, ci, vp, c2p]
     lib.hirep_spinor_max_norm.argtypes = [vp, ci, vp, c2p]
     lib.hirep_cg_g5Dphi_sq.argtypes = [vp, cd, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
+    lib.hirep_cg_g5Dphi_hat_sq.argtypes = [vp, cd, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_fma_peak.argtypes = [ci, ctypes.POINTER(cd)]
     lib.hirep_sync.argtypes = [vp]
     lib.hirep_last_error.restype = ctypes.c_char_p
@@ -142,6 +143,8 @@ def hirep_Dphi_eo(g, out, inp, links): _check(load().hirep_Dphi_eo(g, out, inp, 
 def hirep_Dphi_oe(g, out, inp, links): _check(load().hirep_Dphi_oe(g, out, inp, links))
 def hirep_Dphi_hat(g, m0, out, inp, links): _check(load().hirep_Dphi_hat(g, m0, out, inp, links))
 def hirep_g5Dphi_sq(g, m0, out, inp, links): _check(load().hirep_g5Dphi_sq(g, m0, out, inp, links))
+def hirep_g5Dphi_hat(g, m0, out, inp, links): _check(load().hirep_g5Dphi_hat(g, m0, out, inp, links))
+def hirep_g5Dphi_hat_sq(g, m0, out, inp, links): _check(load().hirep_g5Dphi_hat_sq(g, m0, out, inp, links))
 def hirep_set_link_mode(g, mode): _check(load().hirep_set_link_mode(g, mode))
 def hirep_set_kernel_variant(g, variant): _check(load().hirep_set_kernel_variant(g, variant))
 def hirep_set_tuning(g, key, value): _check(load().hirep_set_tuning(g, key, value))
@@ -181,6 +184,12 @@ def hirep_spinor_max_norm(g, which, eta):
 def hirep_cg_g5Dphi_sq(g, m0, x, b, links, tol, maxiter):
     it, res = ctypes.c_int(), (ctypes.c_double * 2)()
     _check(load().hirep_cg_g5Dphi_sq(g, m0, x, b, links, tol, maxiter, ctypes.byref(it), res))
+    return it.value, res[0]
+
+
+def hirep_cg_g5Dphi_hat_sq(g, m0, x, b, links, tol, maxiter):
+    it, res = ctypes.c_int(), (ctypes.c_double * 2)()
+    _check(load().hirep_cg_g5Dphi_hat_sq(g, m0, x, b, links, tol, maxiter, ctypes.byref(it), res))
     return it.value, res[0]
 
 
@@ -301,6 +310,16 @@ class Geometry:
         hirep_g5Dphi_sq(self.handle, m0, out.data_ptr(), inp.data_ptr(), links.data_ptr())
         return out
 
+    def g5Dphi_hat(self, m0, inp_even, links, out=None):
+        out = self.new_spinor(EVEN) if out is None else out
+        hirep_g5Dphi_hat(self.handle, m0, out.data_ptr(), inp_even.data_ptr(), links.data_ptr())
+        return out
+
+    def g5Dphi_hat_sq(self, m0, inp_even, links, out=None):
+        out = self.new_spinor(EVEN) if out is None else out
+        hirep_g5Dphi_hat_sq(self.handle, m0, out.data_ptr(), inp_even.data_ptr(), links.data_ptr())
+        return out
+
     def apply_host(self, op, m0, inp_host, links_host=None):
         """End-to-end through hirep_apply_host: host (ideally pinned) canonical tensors in, host tensor out."""
         out = self.torch.empty_like(inp_host)
@@ -325,6 +344,11 @@ class Geometry:
     def cg_g5Dphi_sq(self, m0, b, links, tol, maxiter, out=None):
         out = self.new_spinor(FULL) if out is None else out
         it, res = hirep_cg_g5Dphi_sq(self.handle, m0, out.data_ptr(), b.data_ptr(), links.data_ptr(), tol, maxiter)
+        return out, it, res
+
+    def cg_g5Dphi_hat_sq(self, m0, b_even, links, tol, maxiter, out=None):
+        out = self.new_spinor(EVEN) if out is None else out
+        it, res = hirep_cg_g5Dphi_hat_sq(self.handle, m0, out.data_ptr(), b_even.data_ptr(), links.data_ptr(), tol, maxiter)
         return out, it, res
 
     def set_link_mode(self, mode): hirep_set_link_mode(self.handle, mode)

@@ -125,3 +125,51 @@ def test_cg_vs_oracle(env, name, T, L, prec, m0):
     # maxiter is honoured and reported, not an error
     _, it2, res2 = p.geom.cg_g5Dphi_sq(m0, p.to_native(b, hirep.FULL), p.links_rep, tol, 3)
     assert it2 == 3 and res2 > tol
+
+
+@pytest.mark.parametrize("name,T,L,prec", [("C1", 4, 4, "f64"), ("C2", 6, 6, "f64"), ("C3", 4, 6, "f32"), ("C4", 4, 6, "f64"), ("C5", 2, 4, "f64")])
+def test_g5Dphi_hat_and_square(env, name, T, L, prec):
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS[name].resized(T, L)
+    p = Problem(env, cfg, prec)
+    psi_e = p.spinors[0][p.ev]
+    x = p.to_native(psi_e, hirep.EVEN)
+    tol = TOL[prec]
+    got = p.to_numpy(p.geom.g5Dphi_hat(cfg.m0, x, p.links_rep), hirep.EVEN)
+    assert oracle.rel_l2(got, oracle.g5Dphi_hat(T, L, cfg.d_R, cfg.m0, p.R, psi_e, BC)) < tol
+    got = p.to_numpy(p.geom.g5Dphi_hat_sq(cfg.m0, x, p.links_rep), hirep.EVEN)
+    assert oracle.rel_l2(got, oracle.g5Dphi_hat_sq(T, L, cfg.d_R, cfg.m0, p.R, psi_e, BC)) < tol
+    # Hermitian positive definite: <phi, Q^2 psi> = conj <psi, Q^2 phi>, <psi, Q^2 psi> = ||Q psi||^2 > 0 (GPU reductions)
+    q = p.geom.g5Dphi_hat(cfg.m0, x, p.links_rep)
+    q2 = p.geom.g5Dphi_hat_sq(cfg.m0, x, p.links_rep)
+    lhs, rhs = p.geom.prod(hirep.EVEN, x, q2).real, p.geom.sqnorm(hirep.EVEN, q)
+    assert abs(lhs - rhs) <= (1e-12 if prec == "f64" else 1e-5) * rhs and rhs > 0
+
+
+def test_eo_preconditioned_solve_on_gpu(env):
+    """The production solve: D_m x = b through the Schur complement with every step on the GPU (Dphi_eo, lc, Q_hat,
+    CG on Q_hat^2, Dphi_oe), against the oracle's CG and a direct check of the residual of the FULL system."""
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS["C2"].resized(4, 4)
+    T, L, d, m0 = 4, 4, cfg.d_R, 0.3
+    a = 4.0 + m0
+    p = Problem(env, cfg, "f64")
+    g, b = p.geom, p.spinors[0]
+    b_e, b_o = p.to_native(b[p.ev], hirep.EVEN), p.to_native(b[p.od], hirep.ODD)
+    c = g.Dphi_eo(b_o, p.links_rep)                                   # D_eo b_o
+    g.lc(hirep.EVEN, c, a, b_e, -1.0, c)                              # c = a b_e - D_eo b_o     (xi aliases zeta)
+    c_np = oracle.g5(p.to_numpy(c, hirep.EVEN))                       # gamma_5 c (host: no standalone gamma_5 entry)
+    rhs = g.g5Dphi_hat(m0, p.to_native(c_np, hirep.EVEN), p.links_rep)
+    x_e, it, res = g.cg_g5Dphi_hat_sq(m0, rhs, p.links_rep, 1e-12, 2000)
+    assert res <= 1e-12 and it > 3
+    x_o = g.Dphi_oe(x_e, p.links_rep)
+    g.lc(hirep.ODD, x_o, 1.0 / a, b_o, -1.0 / a, x_o)                 # x_o = (b_o - D_oe x_e) / a
+    x = np.zeros_like(b)
+    x[p.ev], x[p.od] = p.to_numpy(x_e, hirep.EVEN), p.to_numpy(x_o, hirep.ODD)
+    resid = np.linalg.norm((b - oracle.Dphi(T, L, d, m0, p.R, x, BC)).ravel()) / np.linalg.norm(b.ravel())
+    assert resid < 1e-10
+    # the oracle's CG on the same preconditioned system needs the same number of iterations (+-2) and agrees
+    rhs_np = p.to_numpy(rhs, hirep.EVEN)
+    x_ref, it_ref, _, _ = la.cg(lambda v: oracle.g5Dphi_hat_sq(T, L, d, m0, p.R, v, BC), rhs_np, 1e-12, 2000)
+    assert abs(it - it_ref) <= 2
+    assert oracle.rel_l2(p.to_numpy(x_e, hirep.EVEN), x_ref) < 1e-8
