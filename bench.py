@@ -356,6 +356,19 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
     out["cg_g5Dphi_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gflops_operator": round(fl_it / ms_it / 1e6, 1),
                            "gbs": round(by_it / ms_it / 1e6, 1), "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3),
                            "launches_per_iteration": 7, "relres_after": res}
+    hb = geom.sizes["spinor_half"]
+    x_e, y_e = x_full[:hb], y_full[:hb]
+    geom.cg_g5Dphi_hat_sq(2.0, x_e, lr, 1e-30, 2, out=y_e)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    _, it, res = geom.cg_g5Dphi_hat_sq(2.0, x_e, lr, 1e-30, iters, out=y_e)
+    torch.cuda.synchronize()
+    ms_it = (time.perf_counter() - t0) * 1e3 / max(it, 1)
+    fl_it = 2 * cm["ops"]["Dphi_hat"][0]
+    by_it = 2 * cm["ops"]["Dphi_hat"][1] + (2 + 6 + 3) * S * V / 2
+    out["cg_g5Dphi_hat_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gflops_operator": round(fl_it / ms_it / 1e6, 1),
+                               "gbs": round(by_it / ms_it / 1e6, 1), "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3),
+                               "launches_per_iteration": 9, "relres_after": res}
     try:
         out["fma_peak_tflops"] = {"f64": round(hirep.hirep_fma_peak(hirep.F64), 2), "f32": round(hirep.hirep_fma_peak(hirep.F32), 2)}
     except Exception as e:   # measurement utility only
