@@ -147,4 +147,65 @@ template <typename T, int N> struct RepMap<T, N, 1> {   // ADJ (real matrix)
     }
 };
 
+// ADJ row with a RUNTIME row index a, for the large adjoints (SU(4..6): d_R = 15, 24, 35).  The compile-time version
+// above unrolls d_R rows of ~500 instructions each; at d_R = 35 that is ~280 KB of code and the kernel stalls on
+// instruction fetch (ncu: 88 % "no instruction").  Here only the generator (kind, i, j) of row a is a run-time value:
+// it selects which rows of W are read (W = any accessor with operator[], e.g. a shared-memory tile), the N x N
+// arithmetic and the d_R outputs stay unrolled -- one row body of code.  Same formulas as RepMap<T, N, 1>::row.
+template <typename T, int N, typename WM> __device__ __forceinline__ void adj_row_runtime(const WM &W, int a, T *w) {
+    constexpr int DR = N * N - 1;
+    const GenIdx ga = gen_decode(a);
+    cplx<T> Y[N * N];
+    if (ga.kind != 2) {
+        cplx<T> wi[N], wj[N];
+#pragma unroll
+        for (int q = 0; q < N; ++q) { wi[q] = W[ga.i * N + q]; wj[q] = W[ga.j * N + q]; }
+#pragma unroll
+        for (int p = 0; p < N; ++p)
+#pragma unroll
+            for (int q = p; q < N; ++q) {
+                const cplx<T> u = ccmul<T>(wi[p], wj[q]);   // conj(W_ip) W_jq
+                const cplx<T> v = ccmul<T>(wj[p], wi[q]);   // conj(W_jp) W_iq
+                if (ga.kind == 0) Y[p * N + q] = mk<T>(T(0.5) * (u.x + v.x), T(0.5) * (u.y + v.y));
+                else Y[p * N + q] = mk<T>(T(0.5) * (u.y - v.y), T(0.5) * (v.x - u.x));   // (-i/2)(u - v)
+            }
+    } else {
+#pragma unroll
+        for (int p = 0; p < N; ++p)
+#pragma unroll
+            for (int q = p; q < N; ++q) Y[p * N + q] = mk<T>(0, 0);
+        for (int r = 0; r <= ga.j; ++r) {
+            cplx<T> wr[N];
+#pragma unroll
+            for (int q = 0; q < N; ++q) wr[q] = W[r * N + q];
+            const T f = (r < ga.j) ? T(1) : T(-ga.j);
+#pragma unroll
+            for (int p = 0; p < N; ++p)
+#pragma unroll
+                for (int q = p; q < N; ++q) {
+                    const cplx<T> u = ccmul<T>(wr[p], wr[q]);
+                    Y[p * N + q].x += f * u.x;
+                    Y[p * N + q].y += f * u.y;
+                }
+        }
+        const T nrm = (T)diag_norm(ga.j);
+#pragma unroll
+        for (int p = 0; p < N; ++p)
+#pragma unroll
+            for (int q = p; q < N; ++q) { Y[p * N + q].x *= nrm; Y[p * N + q].y *= nrm; }
+    }
+    static_for<0, DR>([&](auto bc) {
+        constexpr int B = decltype(bc)::value;
+        constexpr GenIdx gb = gen_decode(B);
+        if constexpr (gb.kind == 0) w[B] = 2 * Y[gb.i * N + gb.j].x;
+        else if constexpr (gb.kind == 1) w[B] = -2 * Y[gb.i * N + gb.j].y;
+        else {
+            T acc = 0;
+#pragma unroll
+            for (int r = 0; r < gb.j; ++r) acc += Y[r * N + r].x;
+            w[B] = (T)(2.0 * diag_norm(gb.j)) * (acc - gb.j * Y[gb.j * N + gb.j].x);
+        }
+    });
+}
+
 }  // namespace hirep
