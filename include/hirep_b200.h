@@ -113,8 +113,11 @@ int hirep_set_link_mode(hirep_geom *g, int mode); /* HIREP_LINKS_STORED | HIREP_
 int hirep_set_kernel_variant(hirep_geom *g, int variant);
 /* Measurement / test knobs of the persistent stencil kernels.  Results never depend on them.
  *   HIREP_TUNE_MAX_CTAS    cap on the number of persistent CTAs (0 = one per SM); a small cap makes every warp
- *                          walk many tiles, which the parity tests use on small lattices */
-enum { HIREP_TUNE_MAX_CTAS = 1 };
+ *                          walk many tiles, which the parity tests use on small lattices
+ *   HIREP_TUNE_SUM_ALGORITHM  accumulation of the reductions (this one does change the last bits of their results):
+ *                          2 = Neumaier, Algorithm 2 (default), 3 = second-order Neumaier, Algorithm 3 (L682),
+ *                          4 = double-double, Algorithm 4 (L706) */
+enum { HIREP_TUNE_MAX_CTAS = 1, HIREP_TUNE_SUM_ALGORITHM = 2 };
 int hirep_set_tuning(hirep_geom *g, int key, int value);
 /* number of kernels this library has launched on behalf of g since creation (bench.py's gpu_launches) */
 long hirep_launch_count(const hirep_geom *g);

@@ -20,7 +20,7 @@ struct hirep_geom {
     Geo geo;
     int N, rep, prec, dR, real;
     int mode, variant;
-    int tune_max_ctas;            // hirep_set_tuning
+    int tune_max_ctas, sum_alg;   // hirep_set_tuning
     cudaStream_t stream;
     void *ws_half, *ws_half2, *ws_full;   // workspace spinors (lazy)
     void *ws_red;                   // reduction partials + 4 result doubles (lazy)
@@ -83,7 +83,7 @@ extern "C" int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep
     g->geo.Nh = (int)(V / 2);
     g->geo.n_tiles = (g->geo.Nh + TILE - 1) / TILE;
     g->geo.bc[0] = -1; g->geo.bc[1] = g->geo.bc[2] = g->geo.bc[3] = 1;
-    g->tune_max_ctas = 0;
+    g->tune_max_ctas = 0; g->sum_alg = 2;
     g->N = N_g; g->rep = rep; g->prec = prec; g->dR = dR; g->real = (rep == HIREP_ADJ);
     const size_t w = prec == HIREP_F64 ? 8 : 4;
     g->bytes_spinor_half = (size_t)g->geo.n_tiles * 4 * dR * TILE * 2 * w;
@@ -145,6 +145,10 @@ extern "C" int hirep_set_kernel_variant(hirep_geom *g, int variant) {
 extern "C" int hirep_set_tuning(hirep_geom *g, int key, int value) {
     if (!g) return fail(HIREP_EINVAL, "hirep_set_tuning: NULL geometry");
     switch (key) {
+    case HIREP_TUNE_SUM_ALGORITHM:
+        if (value < 2 || value > 4) return fail(HIREP_EINVAL, "hirep_set_tuning: summation algorithm %d (2, 3 or 4)", value);
+        g->sum_alg = value;
+        return HIREP_OK;
     case HIREP_TUNE_MAX_CTAS:
         if (value < 0) return fail(HIREP_EINVAL, "hirep_set_tuning: max CTAs %d", value);
         g->tune_max_ctas = value;
@@ -354,7 +358,7 @@ static int reduce_prod(hirep_geom *g, int which, int mode, const void *xi, const
     if (which < 0 || which > 2) return fail(HIREP_EINVAL, "%s: parity_or_full=%d", what, which);
     int rc = red_workspace(g);
     if (rc) return rc;
-    rc = kern_result(g, k_prod(g->geo, g->prec, g->dR, which == HIREP_FULL ? 2 : 1, mode, xi, eta, g->ws_red, red_out(g), g->stream), what, 2);
+    rc = kern_result(g, k_prod(g->geo, g->prec, g->dR, which == HIREP_FULL ? 2 : 1, mode, g->sum_alg, xi, eta, g->ws_red, red_out(g), g->stream), what, 2);
     if (rc) return rc;
     return fetch_result(g, host, 2, what);
 }
@@ -411,7 +415,7 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
         if ((rc = reduce_prod(g, which, 0, g->cg_p, g->cg_Ap, res, what))) return rc;
         if (!(res[0] > 0.0)) return fail(HIREP_EINVAL, "%s: <p,Ap> = %g is not positive (operator not positive definite?)", what, res[0]);
         const double alpha = rr / res[0];
-        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, halves, alpha, x, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, red_out(g), g->stream), what, 2);
+        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, halves, g->sum_alg, alpha, x, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, red_out(g), g->stream), what, 2);
         if (rc) return rc;
         if ((rc = fetch_result(g, res, 2, what))) return rc;
         const double rr_new = res[0];

@@ -35,9 +35,9 @@ int k_hop(const Geo &g, int prec, int N, int rep, int mode, int variant, const H
 int k_reduce_workspace_bytes();
 int k_lincomb(int prec, long n, void *xi, const double c0[2], int use_xi, const void *eta, const double c1[2], const void *zeta,
               const double c2[2], int use_zeta, cudaStream_t s);
-int k_prod(const Geo &g, int prec, int dR, int halves, int mode, const void *xi, const void *eta, void *ws, double *out_dev, cudaStream_t s);
+int k_prod(const Geo &g, int prec, int dR, int halves, int mode, int alg, const void *xi, const void *eta, void *ws, double *out_dev, cudaStream_t s);
 int k_maxnorm(const Geo &g, int prec, int dR, int halves, const void *xi, void *ws, double *out_dev, cudaStream_t s);
-int k_cg_update(const Geo &g, int prec, int dR, int halves, double alpha, void *x, void *r, const void *p, const void *Ap, void *ws,
+int k_cg_update(const Geo &g, int prec, int dR, int halves, int alg, double alpha, void *x, void *r, const void *p, const void *Ap, void *ws,
                 double *out_dev, cudaStream_t s);
 int k_fma_peak(int prec, double *tflops, cudaStream_t s);   // fma_peak.cu: measured FP64/FP32 FMA throughput
 // number of distinct kernel launches k_hop issues for this configuration (for launch accounting): always 1.

@@ -4,7 +4,8 @@
 //                         coefficients (a real coefficient is a complex one with zero imaginary part), one fused
 //                         kernel -- "fusing together one or more linear algebra kernels" (L379)
 //   reductions            Eq 27 (L402) <xi,eta>, Eq 32 (L426) ||xi||^2, Eq 33 (L430) max norm, accumulated with
-//                         Neumaier's compensated sum, Algorithm 2 (L662) -- the paper's default -- per thread, and
+//                         Neumaier's compensated sum, Algorithm 2 (L662) -- the paper's default; Algorithms 3 and 4
+//                         (second-order Neumaier, double-double) selectable -- per thread, and
 //                         merged across lanes / warps / blocks with the branch-free two-sum (L654: "either variant
 //                         can be used"); fp32 fields are accumulated in fp64 (their products are exact in fp64)
 //   cg_update             the fused CG step  x += alpha p ; r -= alpha Ap ; ||r||^2  (one pass over four fields)
@@ -19,34 +20,64 @@ namespace {
 
 constexpr int RED_THREADS = 256;
 
-struct Acc {   // running compensated sum: value = s + c
-    double s, c;
+// running compensated sum.  ALG selects the paper's accumulation algorithm (L636: "different algorithms for the
+// accumulation are available"):  2 = Neumaier (Algorithm 2, the default): value = s + c
+//                                3 = second-order Neumaier (Algorithm 3):  value = s + (c + c2)
+//                                4 = double-double (Algorithm 4):          value = s, with (s, c) a normalised pair
+struct Acc {
+    double s, c, c2;
 };
 __device__ __forceinline__ void two_sum(double a, double b, double &s, double &e) {   // branch-free variant of Alg 1
     s = __dadd_rn(a, b);
     const double bb = __dsub_rn(s, a);
     e = __dadd_rn(__dsub_rn(a, __dsub_rn(s, bb)), __dsub_rn(b, bb));
 }
-__device__ __forceinline__ void acc_add(Acc &A, double x) {   // one step of Algorithm 2 (Neumaier)
+__device__ __forceinline__ void acc_add(Acc &A, double x, int alg) {   // one loop iteration of Algorithm 2 / 3 / 4
     double s, e;
     two_sum(A.s, x, s, e);
-    A.s = s;
-    A.c = __dadd_rn(A.c, e);
+    if (alg == 2) {
+        A.s = s;
+        A.c = __dadd_rn(A.c, e);
+    } else if (alg == 3) {
+        double c, e2;
+        two_sum(A.c, e, c, e2);
+        A.s = s;
+        A.c = c;
+        A.c2 = __dadd_rn(A.c2, e2);
+    } else {
+        two_sum(s, __dadd_rn(A.c, e), A.s, A.c);
+    }
 }
-__device__ __forceinline__ void acc_merge(Acc &A, const Acc &B) {
+// merge two partial sums of the same algorithm (lanes, warps, blocks): the partner's components enter as terms
+__device__ __forceinline__ void acc_merge(Acc &A, const Acc &B, int alg) {
     double s, e;
     two_sum(A.s, B.s, s, e);
-    A.s = s;
-    A.c = __dadd_rn(__dadd_rn(A.c, B.c), e);
+    if (alg == 2) {
+        A.s = s;
+        A.c = __dadd_rn(__dadd_rn(A.c, B.c), e);
+    } else if (alg == 3) {
+        double c, e2, c3, e3;
+        two_sum(A.c, B.c, c, e2);
+        two_sum(c, e, c3, e3);
+        A.s = s;
+        A.c = c3;
+        A.c2 = __dadd_rn(__dadd_rn(A.c2, B.c2), __dadd_rn(e2, e3));
+    } else {
+        two_sum(s, __dadd_rn(__dadd_rn(A.c, B.c), e), A.s, A.c);
+    }
+}
+__device__ __forceinline__ double acc_value(const Acc &A, int alg) {
+    return alg == 2 ? __dadd_rn(A.s, A.c) : alg == 3 ? __dadd_rn(A.s, __dadd_rn(A.c, A.c2)) : A.s;
 }
 __device__ __forceinline__ Acc acc_shfl_down(const Acc &A, int off) {
     Acc B;
     B.s = __shfl_down_sync(0xffffffffu, A.s, off);
     B.c = __shfl_down_sync(0xffffffffu, A.c, off);
+    B.c2 = __shfl_down_sync(0xffffffffu, A.c2, off);
     return B;
 }
 // block-wide merge of NV accumulators per thread; result valid in thread 0
-template <int NV> __device__ void block_merge(Acc (&a)[NV]) {
+template <int NV> __device__ void block_merge(Acc (&a)[NV], int alg) {
     __shared__ Acc sh[NV][RED_THREADS / 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
@@ -54,7 +85,7 @@ template <int NV> __device__ void block_merge(Acc (&a)[NV]) {
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
             const Acc b = acc_shfl_down(a[v], off);
-            acc_merge(a[v], b);
+            acc_merge(a[v], b, alg);
         }
         if (lane == 0) sh[v][warp] = a[v];
     }
@@ -62,11 +93,11 @@ template <int NV> __device__ void block_merge(Acc (&a)[NV]) {
     if (warp == 0) {
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
-            Acc x = lane < RED_THREADS / 32 ? sh[v][lane] : Acc{0.0, 0.0};
+            Acc x = lane < RED_THREADS / 32 ? sh[v][lane] : Acc{0.0, 0.0, 0.0};
 #pragma unroll
             for (int off = 16; off > 0; off >>= 1) {
                 const Acc b = acc_shfl_down(x, off);
-                acc_merge(x, b);
+                acc_merge(x, b, alg);
             }
             a[v] = x;
         }
@@ -111,35 +142,35 @@ __global__ void __launch_bounds__(256) lincomb_kernel(long n, cplx<T> *__restric
 // ---- partial reductions: one Acc pair (or quadruple) per block -------------------------------------------------
 // mode 0: <xi,eta> (re, im)   mode 1: ||xi||^2 (re only)
 template <typename T, int MODE>
-__global__ void __launch_bounds__(RED_THREADS) prod_partial_kernel(Pad P, long n, const cplx<T> *__restrict__ xi,
+__global__ void __launch_bounds__(RED_THREADS) prod_partial_kernel(Pad P, long n, int alg, const cplx<T> *__restrict__ xi,
                                                                    const cplx<T> *__restrict__ eta, Acc *__restrict__ partial) {
-    Acc a[2] = {{0.0, 0.0}, {0.0, 0.0}};
+    Acc a[2] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
         if (!is_site(P, i)) continue;
         const cplx<T> x = xi[i];
         const double xr = (double)x.x, xm = (double)x.y;
         if (MODE == 1) {
-            acc_add(a[0], __dmul_rn(xr, xr));
-            acc_add(a[0], __dmul_rn(xm, xm));
+            acc_add(a[0], __dmul_rn(xr, xr), alg);
+            acc_add(a[0], __dmul_rn(xm, xm), alg);
         } else {
             const cplx<T> e = eta[i];
             const double er = (double)e.x, em = (double)e.y;
-            acc_add(a[0], __dmul_rn(xr, er));
-            acc_add(a[0], __dmul_rn(xm, em));
-            acc_add(a[1], __dmul_rn(xr, em));
-            acc_add(a[1], -__dmul_rn(xm, er));
+            acc_add(a[0], __dmul_rn(xr, er), alg);
+            acc_add(a[0], __dmul_rn(xm, em), alg);
+            acc_add(a[1], __dmul_rn(xr, em), alg);
+            acc_add(a[1], -__dmul_rn(xm, er), alg);
         }
     }
-    block_merge<2>(a);
+    block_merge<2>(a, alg);
     if (threadIdx.x == 0) { partial[2 * blockIdx.x] = a[0]; partial[2 * blockIdx.x + 1] = a[1]; }
 }
 
 // fused CG step: x += alpha p ; r -= alpha Ap ; partial ||r||^2          (alpha real: A is Hermitian positive definite)
 template <typename T>
-__global__ void __launch_bounds__(RED_THREADS) cg_update_kernel(Pad P, long n, double alpha, cplx<T> *__restrict__ x,
+__global__ void __launch_bounds__(RED_THREADS) cg_update_kernel(Pad P, long n, int alg, double alpha, cplx<T> *__restrict__ x,
                                                                 cplx<T> *__restrict__ r, const cplx<T> *__restrict__ p,
                                                                 const cplx<T> *__restrict__ Ap, Acc *__restrict__ partial) {
-    Acc a[2] = {{0.0, 0.0}, {0.0, 0.0}};
+    Acc a[2] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
     const T al = (T)alpha;
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
         const cplx<T> pv = p[i], av = Ap[i];
@@ -149,23 +180,23 @@ __global__ void __launch_bounds__(RED_THREADS) cg_update_kernel(Pad P, long n, d
         x[i] = xv;
         r[i] = rv;
         if (is_site(P, i)) {
-            acc_add(a[0], __dmul_rn((double)rv.x, (double)rv.x));
-            acc_add(a[0], __dmul_rn((double)rv.y, (double)rv.y));
+            acc_add(a[0], __dmul_rn((double)rv.x, (double)rv.x), alg);
+            acc_add(a[0], __dmul_rn((double)rv.y, (double)rv.y), alg);
         }
     }
-    block_merge<2>(a);
+    block_merge<2>(a, alg);
     if (threadIdx.x == 0) { partial[2 * blockIdx.x] = a[0]; partial[2 * blockIdx.x + 1] = a[1]; }
 }
 
-// second stage: merge the per-block accumulators (fixed order: deterministic), out[v] = s + c  (last line of Alg 2)
-__global__ void __launch_bounds__(RED_THREADS) reduce_final_kernel(int nblocks, const Acc *__restrict__ partial, double *__restrict__ out) {
-    Acc a[2] = {{0.0, 0.0}, {0.0, 0.0}};
+// second stage: merge the per-block accumulators (fixed order: deterministic), out[v] = the algorithm's final value
+__global__ void __launch_bounds__(RED_THREADS) reduce_final_kernel(int nblocks, int alg, const Acc *__restrict__ partial, double *__restrict__ out) {
+    Acc a[2] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
     for (int b = threadIdx.x; b < nblocks; b += RED_THREADS) {
-        acc_merge(a[0], partial[2 * b]);
-        acc_merge(a[1], partial[2 * b + 1]);
+        acc_merge(a[0], partial[2 * b], alg);
+        acc_merge(a[1], partial[2 * b + 1], alg);
     }
-    block_merge<2>(a);
-    if (threadIdx.x == 0) { out[0] = __dadd_rn(a[0].s, a[0].c); out[1] = __dadd_rn(a[1].s, a[1].c); }
+    block_merge<2>(a, alg);
+    if (threadIdx.x == 0) { out[0] = acc_value(a[0], alg); out[1] = acc_value(a[1], alg); }
 }
 
 template <typename T>
@@ -233,20 +264,20 @@ int k_lincomb(int prec, long n, void *xi, const double c0[2], int use_xi, const 
 }
 
 // mode 0: <xi,eta> -> out_dev[0..1] ; mode 1: ||xi||^2 -> out_dev[0] ; ws = k_reduce_workspace_bytes() device bytes
-int k_prod(const Geo &g, int prec, int dR, int halves, int mode, const void *xi, const void *eta, void *ws, double *out_dev, cudaStream_t s) {
+int k_prod(const Geo &g, int prec, int dR, int halves, int mode, int alg, const void *xi, const void *eta, void *ws, double *out_dev, cudaStream_t s) {
     const int ncomp = 4 * dR;
     const long half_elems = (long)g.n_tiles * ncomp * TILE, n = half_elems * halves;
     const Pad P{(long)g.n_tiles * ncomp, ncomp, g.Nh % TILE == 0 ? TILE : g.Nh % TILE};
     const int nb = blocks_for(n);
     Acc *partial = (Acc *)ws;
     if (prec == 0) {
-        if (mode == 0) prod_partial_kernel<double, 0><<<nb, RED_THREADS, 0, s>>>(P, n, (const double2 *)xi, (const double2 *)eta, partial);
-        else prod_partial_kernel<double, 1><<<nb, RED_THREADS, 0, s>>>(P, n, (const double2 *)xi, (const double2 *)eta, partial);
+        if (mode == 0) prod_partial_kernel<double, 0><<<nb, RED_THREADS, 0, s>>>(P, n, alg, (const double2 *)xi, (const double2 *)eta, partial);
+        else prod_partial_kernel<double, 1><<<nb, RED_THREADS, 0, s>>>(P, n, alg, (const double2 *)xi, (const double2 *)eta, partial);
     } else {
-        if (mode == 0) prod_partial_kernel<float, 0><<<nb, RED_THREADS, 0, s>>>(P, n, (const float2 *)xi, (const float2 *)eta, partial);
-        else prod_partial_kernel<float, 1><<<nb, RED_THREADS, 0, s>>>(P, n, (const float2 *)xi, (const float2 *)eta, partial);
+        if (mode == 0) prod_partial_kernel<float, 0><<<nb, RED_THREADS, 0, s>>>(P, n, alg, (const float2 *)xi, (const float2 *)eta, partial);
+        else prod_partial_kernel<float, 1><<<nb, RED_THREADS, 0, s>>>(P, n, alg, (const float2 *)xi, (const float2 *)eta, partial);
     }
-    reduce_final_kernel<<<1, RED_THREADS, 0, s>>>(nb, partial, out_dev);
+    reduce_final_kernel<<<1, RED_THREADS, 0, s>>>(nb, alg, partial, out_dev);
     return (int)cudaGetLastError();
 }
 
@@ -261,16 +292,16 @@ int k_maxnorm(const Geo &g, int prec, int dR, int halves, const void *xi, void *
     return (int)cudaGetLastError();
 }
 
-int k_cg_update(const Geo &g, int prec, int dR, int halves, double alpha, void *x, void *r, const void *p, const void *Ap, void *ws,
+int k_cg_update(const Geo &g, int prec, int dR, int halves, int alg, double alpha, void *x, void *r, const void *p, const void *Ap, void *ws,
                 double *out_dev, cudaStream_t s) {
     const int ncomp = 4 * dR;
     const long half_elems = (long)g.n_tiles * ncomp * TILE, n = half_elems * halves;
     const Pad P{(long)g.n_tiles * ncomp, ncomp, g.Nh % TILE == 0 ? TILE : g.Nh % TILE};
     const int nb = blocks_for(n);
     Acc *partial = (Acc *)ws;
-    if (prec == 0) cg_update_kernel<double><<<nb, RED_THREADS, 0, s>>>(P, n, alpha, (double2 *)x, (double2 *)r, (const double2 *)p, (const double2 *)Ap, partial);
-    else cg_update_kernel<float><<<nb, RED_THREADS, 0, s>>>(P, n, alpha, (float2 *)x, (float2 *)r, (const float2 *)p, (const float2 *)Ap, partial);
-    reduce_final_kernel<<<1, RED_THREADS, 0, s>>>(nb, partial, out_dev);
+    if (prec == 0) cg_update_kernel<double><<<nb, RED_THREADS, 0, s>>>(P, n, alg, alpha, (double2 *)x, (double2 *)r, (const double2 *)p, (const double2 *)Ap, partial);
+    else cg_update_kernel<float><<<nb, RED_THREADS, 0, s>>>(P, n, alg, alpha, (float2 *)x, (float2 *)r, (const float2 *)p, (const float2 *)Ap, partial);
+    reduce_final_kernel<<<1, RED_THREADS, 0, s>>>(nb, alg, partial, out_dev);
     return (int)cudaGetLastError();
 }
 
