@@ -202,3 +202,43 @@ def test_eo_preconditioned_solve_on_gpu(env):
     x_ref, it_ref, _, _ = la.cg(lambda v: oracle.g5Dphi_hat_sq(T, L, d, m0, p.R, v, BC), rhs_np, 1e-12, 2000)
     assert abs(it - it_ref) <= 2
     assert oracle.rel_l2(p.to_numpy(x_e, hirep.EVEN), x_ref) < 1e-8
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_full_size_linalg_and_cg(env, prec):
+    """BASELINE configs[1] at full size (SU(3) fundamental, 32^4), the launch configuration bench.py times:
+    reductions against the correctly rounded sum of the downloaded field, a linear combination on sampled sites, and
+    the CG solution checked on sampled sites with the per-site oracle: (Q^2 x)(ix) = b(ix)."""
+    from tests.gpu_helpers import SampledOracle, sample_sites, torch_field_fetch
+    from tests.test_gpu_parity import full_size_problem
+    torch, hirep, oracle = env["torch"], env["hirep"], env["oracle"]
+    cfg, geom, links, psi, lr = full_size_problem(env, "C2", prec)
+    x = geom.spinor_import(psi, hirep.FULL)
+    host = psi.cpu().numpy().astype(np.complex128)
+    eps = 2.0 ** -52
+    ref = la.sqnorm(host)
+    assert abs(geom.sqnorm(hirep.FULL, x) - ref) <= 4 * eps * ref
+    assert geom.max_norm(hirep.FULL, x) == la.max_norm(host)
+    # y = 0.5 x - 1.5 i x on sampled rows (lc2 with xi = a copy of x)
+    y = geom.new_spinor(hirep.FULL)
+    y.copy_(x)
+    geom.lc2(hirep.FULL, y, 0.5, -1.5j, x)
+    yc = geom.spinor_export(y, hirep.FULL)
+    sites = sample_sites(cfg, 8, seed=5)
+    for ix in sites:
+        got = yc[ix].cpu().numpy().astype(np.complex128)
+        assert np.linalg.norm(got - (0.5 - 1.5j) * host[ix]) <= TOL[prec] * np.linalg.norm(host[ix])
+    prod = geom.prod(hirep.FULL, x, y)                       # <x, (0.5-1.5i) x> = (0.5-1.5i) ||x||^2
+    assert abs(prod - (0.5 - 1.5j) * ref) <= (1e-12 if prec == "f64" else 1e-6) * abs(ref)
+    # CG on Q^2 at a heavy mass (converges in a few tens of iterations)
+    m0 = 1.0
+    tol = 1e-9 if prec == "f64" else 2e-5
+    sol, it, res = geom.cg_g5Dphi_sq(m0, x, lr, tol, 500)
+    assert res <= tol and 5 < it < 500
+    so = SampledOracle(oracle, cfg, links)
+    fetch = torch_field_fetch(geom.spinor_export(sol, hirep.FULL))
+    bnorm = np.sqrt(ref / cfg.volume)                        # typical |b(ix)| per site
+    for ix in sites[:5]:
+        r = host[ix] - so.g5Dphi_sq(fetch, ix, m0)
+        assert np.linalg.norm(r) <= (1e-6 if prec == "f64" else 2e-3) * bnorm * np.sqrt(4 * cfg.d_R), (ix, np.linalg.norm(r))
+    geom.sync()
