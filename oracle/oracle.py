@@ -188,6 +188,32 @@ def g5Dphi_hat_sq(T, L, d_R, m0, Rlinks, psi_even, bc=DEFAULT_BC) -> np.ndarray:
     return g5Dphi_hat(T, L, d_R, m0, Rlinks, g5Dphi_hat(T, L, d_R, m0, Rlinks, psi_even, bc), bc)
 
 
+# ---- twisted mass (Eq 51) and the general Schur form it needs (Eq 43); SURVEY 8(f) NEXT-2 ---------------
+def g5_lc(c1, c2, eta) -> np.ndarray:
+    """xi = c1 eta + c2 gamma_5 eta (the gamma_5-fused linear combination, L447)."""
+    return complex(c1) * np.asarray(eta, dtype=np.complex128) + complex(c2) * g5(eta)
+
+
+def Dphi_tm(T, L, d_R, m0, mu, Rlinks, psi, bc=DEFAULT_BC) -> np.ndarray:
+    """Eq 51 for the tau^3 = +1 flavour: D^tm psi = D_m psi + i mu gamma_5 psi (the other flavour is mu -> -mu)."""
+    return Dphi(T, L, d_R, m0, Rlinks, psi, bc) + 1j * float(mu) * g5(psi)
+
+
+def Dphi_tm_hat(T, L, d_R, m0, mu, Rlinks, psi_even, bc=DEFAULT_BC) -> np.ndarray:
+    """Eq 43 literally, with D_ee = D_oo = (4+m) + i mu gamma_5 (site-diagonal, so its inverse is
+    ((4+m) - i mu gamma_5) / ((4+m)^2 + mu^2)):  D_hat psi_e = D_ee psi_e - D_eo D_oo^{-1} D_oe psi_e."""
+    a, mu = 4.0 + float(m0), float(mu)
+    t = Dphi_oe(T, L, d_R, Rlinks, psi_even, bc)
+    t = g5_lc(a / (a * a + mu * mu), -1j * mu / (a * a + mu * mu), t)
+    return g5_lc(a, 1j * mu, psi_even) - Dphi_eo(T, L, d_R, Rlinks, t, bc)
+
+
+def Dphi_tm_sq(T, L, d_R, m0, mu, Rlinks, psi, bc=DEFAULT_BC) -> np.ndarray:
+    """(D^tm)^dagger D^tm psi, with (D^tm(mu))^dagger = gamma_5 D^tm(-mu) gamma_5 (gamma_5-hermiticity of D_m, and
+    (i mu gamma_5)^dagger = -i mu gamma_5): the Hermitian positive-definite operator of the twisted-mass monomial."""
+    return g5(Dphi_tm(T, L, d_R, m0, -mu, Rlinks, g5(Dphi_tm(T, L, d_R, m0, mu, Rlinks, psi, bc)), bc))
+
+
 def rel_l2(a: np.ndarray, b: np.ndarray) -> float:
     """||a - b||_2 / ||b||_2 in fp64 with compensated (math.fsum) accumulation."""
     import math

@@ -233,3 +233,50 @@ def test_antiperiodic_bc_equals_link_sign_on_last_time_slice(oracle):
     R3 = R.reshape(T, L ** 3, 4, d, d).copy()
     R3[0, :, 0] *= -1
     assert oracle.rel_l2(oracle.Dphi(T, L, d, 0.2, R3.reshape(R.shape), psi, (1, 1, 1, 1)), out_bc) > 1e-3
+
+
+# ------------------------------------------------------------------ twisted mass (Eq 51) and Eq 43
+def test_twisted_mass_pins(oracle):
+    """Eq 51 / Eq 43 for the twisted-mass diagonal term: free-field symbol, the identity
+    (D^tm)^dagger D^tm = D^dagger D + mu^2, and the dense 4^4 matrix with its Schur complement."""
+    # (i) free field: D^tm psi = [M(p) + i sum gamma sin p + i mu gamma_5] psi
+    T, L, n, rep, m0, mu = 4, 2, 3, FUND, 0.37, 0.21
+    d, V = 3, 4 * 8
+    U = np.broadcast_to(np.eye(n, dtype=complex), (V, 4, n, n)).copy()
+    R = oracle.represent_field(n, rep, U)
+    g, g5 = oracle.gamma(), oracle.gamma5()
+    c = synth.site_coords(T, L)
+    p = np.array([3 * np.pi / T, 2 * np.pi / L, 0.0, 2 * np.pi / L])
+    rng = np.random.default_rng(4)
+    chi = rng.standard_normal((4, d)) + 1j * rng.standard_normal((4, d))
+    psi = np.exp(1j * (c @ p))[:, None, None] * chi[None]
+    symbol = (4 + m0 - np.cos(p).sum()) * np.eye(4) + 1j * sum(g[k] * np.sin(p[k]) for k in range(4)) + 1j * mu * g5
+    assert oracle.rel_l2(oracle.Dphi_tm(T, L, d, m0, mu, R, psi, BC), np.einsum("ab,xbi->xai", symbol, psi)) < 1e-13
+    # (ii) random links: (D^tm)^dag D^tm = Q^2 + mu^2 (the cross terms cancel by gamma_5-hermiticity), any sign of mu
+    cfg = synth.CONFIGS["C1"]
+    Uc, (b, phi) = synth.make_inputs(cfg, 2)
+    Rc = oracle.represent_field(cfg.n_g, cfg.rep, Uc)
+    T, L, d = cfg.T, cfg.L, cfg.d_R
+    for sgn in (+1, -1):
+        lhs = oracle.Dphi_tm_sq(T, L, d, m0, sgn * mu, Rc, b, BC)
+        rhs = oracle.g5Dphi_sq(T, L, d, m0, Rc, b, BC) + mu * mu * b
+        assert oracle.rel_l2(lhs, rhs) < 1e-13
+    # (iii) dense: D^tm = D + i mu G5; its dagger; the Schur complement of Eq 43
+    D = dense.dense_D(T, L, cfg.n_g, cfg.rep, Uc, m0, BC)
+    G5 = np.kron(np.eye(cfg.volume), np.kron(dense.gamma5(), np.eye(d)))
+    Dtm = D + 1j * mu * G5
+    out = oracle.Dphi_tm(T, L, d, m0, mu, Rc, b, BC)
+    assert np.linalg.norm(out.ravel() - Dtm @ b.ravel()) < 1e-13 * np.linalg.norm(out)
+    sq = oracle.Dphi_tm_sq(T, L, d, m0, mu, Rc, b, BC)
+    assert np.linalg.norm(sq.ravel() - Dtm.conj().T @ (Dtm @ b.ravel())) < 1e-13 * np.linalg.norm(sq)
+    e, o = dense.parity_index(T, L, d, 0), dense.parity_index(T, L, d, 1)
+    schur = Dtm[np.ix_(e, e)] - Dtm[np.ix_(e, o)] @ np.linalg.solve(Dtm[np.ix_(o, o)], Dtm[np.ix_(o, e)])
+    ev = synth.parity_sites(T, L, 0)
+    hat = oracle.Dphi_tm_hat(T, L, d, m0, mu, Rc, phi[ev], BC)
+    assert np.linalg.norm(hat.ravel() - schur @ phi[ev].ravel()) < 1e-13 * np.linalg.norm(hat)
+    # mu = 0 reduces to Eq 43 = Eq 44 / (4+m)
+    hat0 = oracle.Dphi_tm_hat(T, L, d, m0, 0.0, Rc, phi[ev], BC)
+    assert oracle.rel_l2((4 + m0) * hat0, oracle.Dphi_hat(T, L, d, m0, Rc, phi[ev], BC)) < 1e-13
+    # gamma_5 linear combination: hand values on one site
+    one = np.zeros((1, 4, 1), complex); one[0, :, 0] = [1, 2j, 3, -1]
+    assert np.array_equal(oracle.g5_lc(2.0, 1j, one)[0, :, 0], np.array([2 + 1j, 4j - 2, 6 - 3j, -2 + 1j]))
