@@ -369,6 +369,10 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
     out["cg_g5Dphi_hat_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gflops_operator": round(fl_it / ms_it / 1e6, 1),
                                "gbs": round(by_it / ms_it / 1e6, 1), "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3),
                                "launches_per_iteration": 9, "relres_after": res}
+    ms = timeit(lambda: geom.Dphi_tm_hat(m0, 0.3, x_e, lr, out=y_e), reps=10)
+    by = cm["ops"]["Dphi_hat"][1] + 2 * S * V / 2          # + the in-place gamma_5 combination on the odd field
+    out["Dphi_tm_hat"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3),
+                          "gflops": round(cm["ops"]["Dphi_hat"][0] / ms / 1e6, 1), "launches": 3}
     try:
         out["fma_peak_tflops"] = {"f64": round(hirep.hirep_fma_peak(hirep.F64), 2), "f32": round(hirep.hirep_fma_peak(hirep.F32), 2)}
     except Exception as e:   # measurement utility only

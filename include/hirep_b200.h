@@ -158,6 +158,16 @@ int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const void *b_ful
 int hirep_cg_g5Dphi_hat_sq(hirep_geom *g, double m0, void *x_even, const void *b_even, const void *links, double tol, int maxiter,
                            int *iters, double *relres);
 
+/* ---- twisted mass (Eq 51) and the general even-odd form it needs (Eq 43) ----
+ *   hirep_spinor_g5_lc  xi = c1 eta + c2 gamma_5 eta             (gamma_5-fused linear combination, L447; xi may alias eta)
+ *   hirep_Dphi_tm       out = D_m in + i mu gamma_5 in           (Eq 51 for the tau^3 = +1 flavour; -mu gives the other)
+ *   hirep_Dphi_tm_sq    out = (D^tm)^dagger D^tm in = gamma_5 D^tm(-mu) gamma_5 D^tm(mu) in   (Hermitian positive definite)
+ *   hirep_Dphi_tm_hat   out_even = D_ee in_even - D_eo D_oo^{-1} D_oe in_even, D_ee = D_oo = (4+m) + i mu gamma_5  (Eq 43) */
+int hirep_spinor_g5_lc(hirep_geom *g, int which, void *xi, const double c1[2], const double c2[2], const void *eta);
+int hirep_Dphi_tm(hirep_geom *g, double m0, double mu, void *out_full, const void *in_full, const void *links);
+int hirep_Dphi_tm_sq(hirep_geom *g, double m0, double mu, void *out_full, const void *in_full, const void *links);
+int hirep_Dphi_tm_hat(hirep_geom *g, double m0, double mu, void *out_even, const void *in_even, const void *links);
+
 /* Measurement utility: achieved TFLOP/s (2 flops per FMA) of a register-resident chain of
  * FMAs in the given precision on the current device, the ALU roofline the pipe utilisation is read against.
  * Synchronous; tflops is a host pointer. */

@@ -234,7 +234,7 @@ extern "C" int hirep_Dphi_oe(hirep_geom *g, void *out_odd, const void *in_even, 
     return offdiag(g, out_odd, in_even, links, 1, "hirep_Dphi_oe");
 }
 
-static int dphi_full(hirep_geom *g, double m0, void *out, const void *in, const void *links, int g5, const char *what) {
+static int dphi_full(hirep_geom *g, double m0, void *out, const void *in, const void *links, int g5, const char *what, double am = 0.0) {
     const size_t hb = g->bytes_spinor_half;
     const char *in_e = (const char *)in, *in_o = in_e + hb;
     char *out_e = (char *)out, *out_o = out_e + hb;
@@ -242,7 +242,7 @@ static int dphi_full(hirep_geom *g, double m0, void *out, const void *in, const 
     L.nsets = 2;
     L.set[0] = HopSet{in_o, out_e, in_e, links_parity(g, links, 0), 0};
     L.set[1] = HopSet{in_e, out_o, in_o, links_parity(g, links, 1), 1};
-    L.a = 4.0 + m0; L.b = -0.5; L.g5 = g5;
+    L.a = 4.0 + m0; L.b = -0.5; L.g5 = g5; L.am = am;
     return hop(g, L, what);
 }
 
@@ -297,6 +297,54 @@ extern "C" int hirep_g5Dphi_sq(hirep_geom *g, double m0, void *out_full, const v
     rc = dphi_full(g, m0, g->ws_full, in_full, links, 1, "hirep_g5Dphi_sq (first g5 D)");
     if (rc) return rc;
     return dphi_full(g, m0, out_full, g->ws_full, links, 1, "hirep_g5Dphi_sq (second g5 D)");
+}
+
+// ---- twisted mass (Eq 51) and its Schur form (Eq 43): SURVEY.md 8(f) NEXT-2, first part --------
+extern "C" int hirep_spinor_g5_lc(hirep_geom *g, int which, void *xi, const double c1[2], const double c2[2], const void *eta) {
+    CHECK_PTRS("hirep_spinor_g5_lc", xi, eta);
+    if (!c1 || !c2) return fail(HIREP_EINVAL, "hirep_spinor_g5_lc: NULL coefficient");
+    if (which < 0 || which > 2) return fail(HIREP_EINVAL, "hirep_spinor_g5_lc: parity_or_full=%d", which);
+    const long n = (long)g->geo.n_tiles * 4 * g->dR * TILE * (which == HIREP_FULL ? 2 : 1);
+    return kern_result(g, k_g5_lincomb(g->prec, n, g->dR, xi, c1, c2, eta, g->stream), "hirep_spinor_g5_lc");
+}
+
+extern "C" int hirep_Dphi_tm(hirep_geom *g, double m0, double mu, void *out_full, const void *in_full, const void *links) {
+    CHECK_PTRS("hirep_Dphi_tm", out_full, in_full, links);
+    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Dphi_tm: out aliases in");
+    return dphi_full(g, m0, out_full, in_full, links, 0, "hirep_Dphi_tm", mu);
+}
+
+// (D^tm)^dagger D^tm = gamma_5 D^tm(-mu) gamma_5 D^tm(mu): two full-lattice launches with the gamma_5 fused in the store
+extern "C" int hirep_Dphi_tm_sq(hirep_geom *g, double m0, double mu, void *out_full, const void *in_full, const void *links) {
+    CHECK_PTRS("hirep_Dphi_tm_sq", out_full, in_full, links);
+    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Dphi_tm_sq: out aliases in");
+    int rc = workspace(&g->ws_full, 2 * g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = dphi_full(g, m0, g->ws_full, in_full, links, 1, "hirep_Dphi_tm_sq (gamma_5 D^tm(mu))", mu);
+    if (rc) return rc;
+    return dphi_full(g, m0, out_full, g->ws_full, links, 1, "hirep_Dphi_tm_sq (gamma_5 D^tm(-mu))", -mu);
+}
+
+// Eq 43 with D_ee = D_oo = (4+m) + i mu gamma_5:  out_e = D_ee in_e - D_eo D_oo^{-1} D_oe in_e.
+// Three launches: D_oe pass; D_oo^{-1} = ((4+m) - i mu gamma_5)/((4+m)^2 + mu^2) as a gamma_5 linear combination in
+// place; D_eo pass with the diagonal term (a + i mu gamma_5) in_e fused in the epilogue.
+extern "C" int hirep_Dphi_tm_hat(hirep_geom *g, double m0, double mu, void *out_even, const void *in_even, const void *links) {
+    CHECK_PTRS("hirep_Dphi_tm_hat", out_even, in_even, links);
+    if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_Dphi_tm_hat: out aliases in");
+    int rc = workspace(&g->ws_half, g->bytes_spinor_half);
+    if (rc) return rc;
+    if ((rc = offdiag(g, g->ws_half, in_even, links, 1, "hirep_Dphi_tm_hat (D_oe pass)"))) return rc;
+    const double a = 4.0 + m0, den = a * a + mu * mu;
+    const double c1[2] = {a / den, 0.0}, c2[2] = {0.0, -mu / den};
+    if ((rc = hirep_spinor_g5_lc(g, HIREP_ODD, g->ws_half, c1, c2, g->ws_half))) return rc;
+    HopLaunch L{};
+    L.nsets = 1;
+    L.set[0] = HopSet{g->ws_half, out_even, in_even, links_parity(g, links, 0), 0};
+    L.a = a;
+    L.am = mu;
+    L.b = +0.5;   // - D_eo = -(-1/2) hop
+    L.g5 = 0;
+    return hop(g, L, "hirep_Dphi_tm_hat (D_eo pass)");
 }
 
 // ---- spinor linear algebra, reductions, CG ------------------------------------------

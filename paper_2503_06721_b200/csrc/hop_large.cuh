@@ -97,6 +97,7 @@ __global__ void __launch_bounds__(32 * ((DR + R - 1) / R)) hop_large_kernel(cons
 
     if (!active) return;
     const T a = (T)L.a, b = (T)L.b;
+    const T am = (T)L.am;
     const T g5s = L.g5 ? T(-1) : T(1);
     C *__restrict__ out = (C *)S.out + ((size_t)tile * NC) * TILE + lane;
     const C *__restrict__ self = (const C *)S.self + ((size_t)tile * NC) * TILE + lane;
@@ -114,6 +115,10 @@ __global__ void __launch_bounds__(32 * ((DR + R - 1) / R)) hop_large_kernel(cons
                 const C sl = self[(size_t)((2 + s) * DR + i) * TILE];
                 vu.x = fma(a, su.x, vu.x); vu.y = fma(a, su.y, vu.y);
                 vl.x = fma(a, sl.x, vl.x); vl.y = fma(a, sl.y, vl.y);
+                if (am != T(0)) {   // twisted mass: + i mu gamma_5 self (Eq 51)
+                    vu.x = fma(-am, su.y, vu.x); vu.y = fma(am, su.x, vu.y);
+                    vl.x = fma(am, sl.y, vl.x); vl.y = fma(-am, sl.x, vl.y);
+                }
             }
             out[(size_t)(s * DR + i) * TILE] = vu;
             out[(size_t)((2 + s) * DR + i) * TILE] = mk<T>(g5s * vl.x, g5s * vl.y);

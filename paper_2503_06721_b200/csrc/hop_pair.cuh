@@ -158,6 +158,7 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
     int q = 0, slot = 0;
     uint32_t phase = 0;
     const T a = (T)L.a, b = (T)L.b;
+    const T am = (T)L.am;
     const T g5s = L.g5 ? T(-1) : T(1);
 
     for (int k = 0; k < my_tiles; ++k) {
@@ -259,6 +260,10 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
                     const C sl = selfbuf[((2 + s) * DR + c) * TILE + lane];
                     vu.x = fma(a, su.x, vu.x); vu.y = fma(a, su.y, vu.y);
                     vl.x = fma(a, sl.x, vl.x); vl.y = fma(a, sl.y, vl.y);
+                    if (am != T(0)) {   // twisted mass: + i mu gamma_5 self (Eq 51)
+                        vu.x = fma(-am, su.y, vu.x); vu.y = fma(am, su.x, vu.y);
+                        vl.x = fma(am, sl.y, vl.x); vl.y = fma(-am, sl.x, vl.y);
+                    }
                 }
                 st_spinor(out + (size_t)(s * DR + c) * TILE, vu);
                 st_spinor(out + (size_t)((2 + s) * DR + c) * TILE, mk<T>(g5s * vl.x, g5s * vl.y));

@@ -20,6 +20,7 @@ struct HopLaunch {
     HopSet set[2];
     int nsets;          // 1 = half lattice, 2 = both parities in one launch
     double a, b;
+    double am;          // twisted mass mu: the diagonal term is (a + i am gamma_5) self (Eq 51); 0 = plain Wilson
     int g5;             // multiply the result by gamma_5 = diag(1,1,-1,-1)
     int max_ctas;       // cap on the persistent grid (0 = one CTA per SM); tests use it to force many tiles per warp
 };
@@ -35,6 +36,7 @@ int k_hop(const Geo &g, int prec, int N, int rep, int mode, int variant, const H
 int k_reduce_workspace_bytes();
 int k_lincomb(int prec, long n, void *xi, const double c0[2], int use_xi, const void *eta, const double c1[2], const void *zeta,
               const double c2[2], int use_zeta, cudaStream_t s);
+int k_g5_lincomb(int prec, long n, int dR, void *xi, const double c1[2], const double c2[2], const void *eta, cudaStream_t s);
 int k_prod(const Geo &g, int prec, int dR, int halves, int mode, int alg, const void *xi, const void *eta, void *ws, double *out_dev, cudaStream_t s);
 int k_maxnorm(const Geo &g, int prec, int dR, int halves, const void *xi, void *ws, double *out_dev, cudaStream_t s);
 int k_cg_update(const Geo &g, int prec, int dR, int halves, int alg, double alpha, void *x, void *r, const void *p, const void *Ap, void *ws,

@@ -139,6 +139,20 @@ __global__ void __launch_bounds__(256) lincomb_kernel(long n, cplx<T> *__restric
     }
 }
 
+// ---- xi = c1*eta + c2*gamma_5*eta: the factor is c1 + c2 on the upper two spin components, c1 - c2 on the lower two
+template <typename T>
+__global__ void __launch_bounds__(256) g5_lincomb_kernel(long n, int ncomp, cplx<T> *__restrict__ xi, const cplx<T> *__restrict__ eta,
+                                                         double2 cu, double2 cl) {
+    const T ux = (T)cu.x, uy = (T)cu.y, lx = (T)cl.x, ly = (T)cl.y;
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
+        const int comp = (int)((i >> 5) % ncomp);          // row = (half, tile, component)
+        const bool lower = 2 * comp >= ncomp;
+        const T cx = lower ? lx : ux, cy = lower ? ly : uy;
+        const cplx<T> e = eta[i];
+        xi[i] = mk<T>(cx * e.x - cy * e.y, cx * e.y + cy * e.x);
+    }
+}
+
 // ---- partial reductions: one Acc pair (or quadruple) per block -------------------------------------------------
 // mode 0: <xi,eta> (re, im)   mode 1: ||xi||^2 (re only)
 template <typename T, int MODE>
@@ -261,6 +275,14 @@ int k_lincomb(int prec, long n, void *xi, const double c0[2], int use_xi, const 
     const double2 a = make_double2(c0[0], c0[1]), b = make_double2(c1[0], c1[1]), c = make_double2(c2[0], c2[1]);
     return prec == 0 ? lincomb_t<double>(n, xi, a, use_xi, eta, b, zeta, c, use_zeta, s)
                      : lincomb_t<float>(n, xi, a, use_xi, eta, b, zeta, c, use_zeta, s);
+}
+
+int k_g5_lincomb(int prec, long n, int dR, void *xi, const double c1[2], const double c2[2], const void *eta, cudaStream_t s) {
+    const double2 cu = make_double2(c1[0] + c2[0], c1[1] + c2[1]), cl = make_double2(c1[0] - c2[0], c1[1] - c2[1]);
+    const int nb = blocks_for(n);
+    if (prec == 0) g5_lincomb_kernel<double><<<nb, 256, 0, s>>>(n, 4 * dR, (double2 *)xi, (const double2 *)eta, cu, cl);
+    else g5_lincomb_kernel<float><<<nb, 256, 0, s>>>(n, 4 * dR, (float2 *)xi, (const float2 *)eta, cu, cl);
+    return (int)cudaGetLastError();
 }
 
 // mode 0: <xi,eta> -> out_dev[0..1] ; mode 1: ||xi||^2 -> out_dev[0] ; ws = k_reduce_workspace_bytes() device bytes

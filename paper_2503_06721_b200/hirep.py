@@ -30,7 +30,8 @@ SYMBOLS = [
     "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_g5Dphi_hat", "hirep_g5Dphi_hat_sq", "hirep_cg_g5Dphi_hat_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_set_tuning", "hirep_launch_count",
     "hirep_apply_host", "hirep_spinor_lc", "hirep_spinor_clc", "hirep_spinor_lc_add_assign", "hirep_spinor_clc_add_assign",
     "hirep_spinor_lc1", "hirep_spinor_lc2", "hirep_spinor_lc3", "hirep_spinor_prod", "hirep_spinor_sqnorm",
-    "hirep_spinor_max_norm", "hirep_cg_g5Dphi_sq", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
+    "hirep_spinor_max_norm", "hirep_cg_g5Dphi_sq", "hirep_spinor_g5_lc", "hirep_Dphi_tm", "hirep_Dphi_tm_sq",
+    "hirep_Dphi_tm_hat", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
 ]
 
 
@@ -86,6 +87,9 @@ def load():
     lib.hirep_spinor_max_norm.argtypes = [vp, ci, vp, c2p]
     lib.hirep_cg_g5Dphi_sq.argtypes = [vp, cd, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_cg_g5Dphi_hat_sq.argtypes = [vp, cd, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
+    lib.hirep_spinor_g5_lc.argtypes = [vp, ci, vp, c2p, c2p, vp]
+    for n in ("hirep_Dphi_tm", "hirep_Dphi_tm_sq", "hirep_Dphi_tm_hat"):
+        getattr(lib, n).argtypes = [vp, cd, cd, vp, vp, vp]
     lib.hirep_fma_peak.argtypes = [ci, ctypes.POINTER(cd)]
     lib.hirep_sync.argtypes = [vp]
     lib.hirep_last_error.restype = ctypes.c_char_p
@@ -185,6 +189,12 @@ def hirep_cg_g5Dphi_sq(g, m0, x, b, links, tol, maxiter):
     it, res = ctypes.c_int(), (ctypes.c_double * 2)()
     _check(load().hirep_cg_g5Dphi_sq(g, m0, x, b, links, tol, maxiter, ctypes.byref(it), res))
     return it.value, res[0]
+
+
+def hirep_spinor_g5_lc(g, which, xi, c1, c2, eta): _check(load().hirep_spinor_g5_lc(g, which, xi, _c2(c1), _c2(c2), eta))
+def hirep_Dphi_tm(g, m0, mu, out, inp, links): _check(load().hirep_Dphi_tm(g, m0, mu, out, inp, links))
+def hirep_Dphi_tm_sq(g, m0, mu, out, inp, links): _check(load().hirep_Dphi_tm_sq(g, m0, mu, out, inp, links))
+def hirep_Dphi_tm_hat(g, m0, mu, out, inp, links): _check(load().hirep_Dphi_tm_hat(g, m0, mu, out, inp, links))
 
 
 def hirep_cg_g5Dphi_hat_sq(g, m0, x, b, links, tol, maxiter):
@@ -345,6 +355,23 @@ class Geometry:
         out = self.new_spinor(FULL) if out is None else out
         it, res = hirep_cg_g5Dphi_sq(self.handle, m0, out.data_ptr(), b.data_ptr(), links.data_ptr(), tol, maxiter)
         return out, it, res
+
+    def g5_lc(self, which, xi, c1, c2, eta): hirep_spinor_g5_lc(self.handle, which, xi.data_ptr(), c1, c2, eta.data_ptr())
+
+    def Dphi_tm(self, m0, mu, inp, links, out=None):
+        out = self.new_spinor(FULL) if out is None else out
+        hirep_Dphi_tm(self.handle, m0, mu, out.data_ptr(), inp.data_ptr(), links.data_ptr())
+        return out
+
+    def Dphi_tm_sq(self, m0, mu, inp, links, out=None):
+        out = self.new_spinor(FULL) if out is None else out
+        hirep_Dphi_tm_sq(self.handle, m0, mu, out.data_ptr(), inp.data_ptr(), links.data_ptr())
+        return out
+
+    def Dphi_tm_hat(self, m0, mu, inp_even, links, out=None):
+        out = self.new_spinor(EVEN) if out is None else out
+        hirep_Dphi_tm_hat(self.handle, m0, mu, out.data_ptr(), inp_even.data_ptr(), links.data_ptr())
+        return out
 
     def cg_g5Dphi_hat_sq(self, m0, b_even, links, tol, maxiter, out=None):
         out = self.new_spinor(EVEN) if out is None else out

@@ -1,0 +1,69 @@
+"""GPU parity of the twisted-mass operators (Eq 51) and their even-odd Schur form (Eq 43) -- the first part
+of SURVEY.md 8(f) NEXT-2 -- against oracle.Dphi_tm / Dphi_tm_hat / Dphi_tm_sq / g5_lc, through the C-ABI binding.
+Same tolerances as the Wilson operators: relative L2 <= 1e-13 (fp64) / 1e-5 (fp32)."""
+import numpy as np
+import pytest
+
+from paper_2503_06721_b200 import synth
+from tests.gpu_helpers import BC, TOL
+from tests.test_gpu_parity import Problem, env  # noqa: F401  (env is a fixture)
+
+pytestmark = pytest.mark.gpu
+
+# every kernel family: ring (C1, C2, C3), pair (C4), rows (C5); ragged tails and whole tiles
+CASES = [("C1", 4, 4), ("C2", 6, 6), ("C3", 4, 8), ("C4", 4, 6), ("C5", 2, 4)]
+
+
+@pytest.mark.parametrize("name,T,L", CASES)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("mu", [0.35, -1.2])
+def test_twisted_mass_operators(env, name, T, L, prec, mu):
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS[name].resized(T, L)
+    p = Problem(env, cfg, prec)
+    g, d, m0, tol = p.geom, cfg.d_R, cfg.m0, TOL[prec]
+    psi = p.spinors[0]
+    x = p.to_native(psi, hirep.FULL)
+    got = p.to_numpy(g.Dphi_tm(m0, mu, x, p.links_rep), hirep.FULL)
+    assert oracle.rel_l2(got, oracle.Dphi_tm(T, L, d, m0, mu, p.R, psi, BC)) < tol
+    got = p.to_numpy(g.Dphi_tm_sq(m0, mu, x, p.links_rep), hirep.FULL)
+    assert oracle.rel_l2(got, oracle.Dphi_tm_sq(T, L, d, m0, mu, p.R, psi, BC)) < tol
+    xe = p.to_native(psi[p.ev], hirep.EVEN)
+    got = p.to_numpy(g.Dphi_tm_hat(m0, mu, xe, p.links_rep), hirep.EVEN)
+    assert oracle.rel_l2(got, oracle.Dphi_tm_hat(T, L, d, m0, mu, p.R, psi[p.ev], BC)) < tol
+    # mu -> 0 leaves the Wilson results bit-for-bit (the twisted term is skipped, not multiplied by zero)
+    a = p.to_numpy(g.Dphi_tm(m0, 0.0, x, p.links_rep), hirep.FULL)
+    b = p.to_numpy(g.Dphi(m0, x, p.links_rep), hirep.FULL)
+    assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("which", ["full", "even", "odd"])
+def test_g5_linear_combination(env, prec, which):
+    hirep, oracle = env["hirep"], env["oracle"]
+    p = Problem(env, synth.CONFIGS["C4"].resized(2, 6), prec)
+    w = {"full": hirep.FULL, "even": hirep.EVEN, "odd": hirep.ODD}[which]
+    sel = {"full": slice(None), "even": p.ev, "odd": p.od}[which]
+    eta = p.spinors[0][sel]
+    c1, c2 = 0.75 - 0.5j, -1.25 + 2.0j
+    e = p.to_native(eta, w)
+    xi = p.geom.new_spinor(w)
+    p.geom.g5_lc(w, xi, c1, c2, e)
+    assert oracle.rel_l2(p.to_numpy(xi, w), oracle.g5_lc(c1, c2, eta)) < TOL[prec]
+    # in place, pure gamma_5: bit exact sign flips of the lower components
+    p.geom.g5_lc(w, e, 0.0, 1.0, e)
+    assert np.array_equal(p.to_numpy(e, w), oracle.g5(eta))
+
+
+def test_twisted_mass_rebuild_mode_and_persistent_grid(env):
+    """The twisted diagonal term through link mode REBUILD and a capped grid (many tiles per warp)."""
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS["C4"].resized(4, 8)
+    p = Problem(env, cfg, "f64")
+    p.geom.set_tuning(hirep.TUNE_MAX_CTAS, 2)
+    psi, mu = p.spinors[0], 0.4
+    ref = oracle.Dphi_tm_hat(cfg.T, cfg.L, cfg.d_R, cfg.m0, mu, p.R, psi[p.ev], BC)
+    xe = p.to_native(psi[p.ev], hirep.EVEN)
+    assert oracle.rel_l2(p.to_numpy(p.geom.Dphi_tm_hat(cfg.m0, mu, xe, p.links_rep), hirep.EVEN), ref) < 1e-13
+    p.geom.set_link_mode(hirep.LINKS_REBUILD)
+    assert oracle.rel_l2(p.to_numpy(p.geom.Dphi_tm_hat(cfg.m0, mu, xe, p.links_fund), hirep.EVEN), ref) < 1e-13
