@@ -1,0 +1,78 @@
+"""Robustness checks of the CUDA kernels that need no oracle (compute-sanitizer is not available on the GPU pool):
+  * determinism -- every operator gives bit-identical output when repeated (a shared-memory or mbarrier race in the
+    bulk-copy rings, the pair exchange or the row-group half-spinor buffers would show up as run-to-run differences);
+  * guard bands -- outputs are written into a slice of a larger buffer whose bytes before and after the slice keep
+    their fill pattern (no out-of-bounds store), and the padding lanes of the last tile keep theirs (stores of
+    inactive lanes are predicated)."""
+import numpy as np
+import pytest
+
+from paper_2503_06721_b200 import synth
+from tests.test_gpu_parity import Problem, env  # noqa: F401  (env is a fixture)
+
+pytestmark = pytest.mark.gpu
+
+GUARD = 4096
+CASES = [("C1", 4, 4, "f64"), ("C2", 6, 6, "f64"), ("C2", 6, 6, "f32"), ("C3", 4, 8, "f32"), ("C4", 6, 6, "f64"),
+         ("C4", 6, 6, "f32"), ("C5", 2, 6, "f64"), ("C5", 2, 6, "f32")]
+
+
+def guarded(torch, dev, nbytes):
+    big = torch.full((nbytes + 2 * GUARD,), 0xA5, dtype=torch.uint8, device=dev)
+    return big, big[GUARD:GUARD + nbytes]
+
+
+@pytest.mark.parametrize("name,T,L,prec", CASES)
+@pytest.mark.parametrize("max_ctas", [0, 2])
+def test_determinism_and_guard_bands(env, name, T, L, prec, max_ctas):
+    torch, hirep = env["torch"], env["hirep"]
+    cfg = synth.CONFIGS[name].resized(T, L)
+    p = Problem(env, cfg, prec)
+    g = p.geom
+    g.set_tuning(hirep.TUNE_MAX_CTAS, max_ctas)
+    x = p.to_native(p.spinors[0], hirep.FULL)
+    hb, fb = g.sizes["spinor_half"], g.sizes["spinor_full"]
+    ops = [
+        ("Dphi", fb, lambda out: g.Dphi(cfg.m0, x, p.links_rep, out=out)),
+        ("Dphi_eo", hb, lambda out: g.Dphi_eo(x[hb:], p.links_rep, out=out)),
+        ("Dphi_oe", hb, lambda out: g.Dphi_oe(x[:hb], p.links_rep, out=out)),
+        ("Dphi_hat", hb, lambda out: g.Dphi_hat(cfg.m0, x[:hb], p.links_rep, out=out)),
+        ("g5Dphi_sq", fb, lambda out: g.g5Dphi_sq(cfg.m0, x, p.links_rep, out=out)),
+        ("Dphi_tm_hat", hb, lambda out: g.Dphi_tm_hat(cfg.m0, 0.3, x[:hb], p.links_rep, out=out)),
+    ]
+    # lanes of the last tile beyond Nh are padding: [tile][comp][lane] -> mask of padding bytes of one half-lattice buffer
+    nh = cfg.volume // 2
+    valid = nh % 32 or 32
+    w = 16 if prec == "f64" else 8
+    ncomp = 4 * cfg.d_R
+    pad_mask = np.zeros(hb, dtype=bool)
+    if valid != 32:
+        last = (hb // (ncomp * 32 * w) - 1) * ncomp * 32 * w
+        m = pad_mask[last:].reshape(ncomp, 32, w)
+        m[:, valid:, :] = True
+    for nm, nbytes, run in ops:
+        results = []
+        for rep in range(3):
+            big, out = guarded(torch, env["dev"], nbytes)
+            run(out)
+            g.sync()
+            host = big.cpu().numpy()
+            assert (host[:GUARD] == 0xA5).all() and (host[GUARD + nbytes:] == 0xA5).all(), (nm, "guard band overwritten")
+            body = host[GUARD:GUARD + nbytes]
+            for h0 in range(0, nbytes, hb):
+                assert (body[h0:h0 + hb][pad_mask] == 0xA5).all(), (nm, "padding lanes written")
+            results.append(body.copy())
+        assert np.array_equal(results[0], results[1]) and np.array_equal(results[0], results[2]), (nm, "not deterministic")
+
+
+def test_reductions_and_cg_are_deterministic(env):
+    hirep = env["hirep"]
+    p = Problem(env, synth.CONFIGS["C2"].resized(6, 6), "f64")
+    x = p.to_native(p.spinors[0], hirep.FULL)
+    vals = {(p.geom.sqnorm(hirep.FULL, x), p.geom.prod(hirep.FULL, x, x)) for _ in range(5)}
+    assert len(vals) == 1
+    sols = []
+    for _ in range(2):
+        s, it, res = p.geom.cg_g5Dphi_sq(0.5, x, p.links_rep, 1e-10, 500)
+        sols.append((p.to_numpy(s, hirep.FULL), it, res))
+    assert sols[0][1:] == sols[1][1:] and np.array_equal(sols[0][0], sols[1][0])
