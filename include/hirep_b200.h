@@ -154,6 +154,9 @@ int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, double *out
  * *relres).  Full-lattice native spinors; iters / relres are host pointers (may be NULL).  x must not alias b. */
 int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const void *b_full, const void *links, double tol, int maxiter,
                        int *iters, double *relres);
+/* The same for (D^tm)^dagger D^tm x = b (hirep_Dphi_tm_sq), the twisted-mass monomial's operator. */
+int hirep_cg_Dphi_tm_sq(hirep_geom *g, double m0, double mu, void *x_full, const void *b_full, const void *links, double tol,
+                        int maxiter, int *iters, double *relres);
 /* The same for Q_hat^2 x = b on the even sites (hirep_g5Dphi_hat_sq): even-odd preconditioned CG. */
 int hirep_cg_g5Dphi_hat_sq(hirep_geom *g, double m0, void *x_even, const void *b_even, const void *links, double tol, int maxiter,
                            int *iters, double *relres);

@@ -440,7 +440,7 @@ extern "C" int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, 
 // beta = rr'/rr; p = r + beta p }.  Per iteration: the operator (2 or 4 stencil launches), <p,Ap> (2 launches), the
 // fused update + ||r||^2 (2), the p update (1).
 static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, const void *links, double tol, int maxiter, int *iters,
-                    double *relres, const char *what) {
+                    double *relres, const char *what, int twisted = 0, double mu = 0.0) {
     if (x == b) return fail(HIREP_EINVAL, "%s: x aliases b", what);
     if (!(tol > 0.0) || maxiter < 0) return fail(HIREP_EINVAL, "%s: tol=%g maxiter=%d", what, tol, maxiter);
     const int which = full ? HIREP_FULL : HIREP_EVEN, halves = full ? 2 : 1;
@@ -458,7 +458,8 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
     rr = bb;
     int it = 0;
     while (bb > 0.0 && it < maxiter && rr > tol * tol * bb) {
-        rc = full ? hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links) : hirep_g5Dphi_hat_sq(g, m0, g->cg_Ap, g->cg_p, links);
+        rc = twisted ? hirep_Dphi_tm_sq(g, m0, mu, g->cg_Ap, g->cg_p, links)
+                     : full ? hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links) : hirep_g5Dphi_hat_sq(g, m0, g->cg_Ap, g->cg_p, links);
         if (rc) return rc;
         if ((rc = reduce_prod(g, which, 0, g->cg_p, g->cg_Ap, res, what))) return rc;
         if (!(res[0] > 0.0)) return fail(HIREP_EINVAL, "%s: <p,Ap> = %g is not positive (operator not positive definite?)", what, res[0]);
@@ -481,6 +482,11 @@ extern "C" int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const 
                                   int maxiter, int *iters, double *relres) {
     CHECK_PTRS("hirep_cg_g5Dphi_sq", x_full, b_full, links);
     return cg_solve(g, 1, m0, x_full, b_full, links, tol, maxiter, iters, relres, "hirep_cg_g5Dphi_sq");
+}
+extern "C" int hirep_cg_Dphi_tm_sq(hirep_geom *g, double m0, double mu, void *x_full, const void *b_full, const void *links, double tol,
+                                   int maxiter, int *iters, double *relres) {
+    CHECK_PTRS("hirep_cg_Dphi_tm_sq", x_full, b_full, links);
+    return cg_solve(g, 1, m0, x_full, b_full, links, tol, maxiter, iters, relres, "hirep_cg_Dphi_tm_sq", 1, mu);
 }
 extern "C" int hirep_cg_g5Dphi_hat_sq(hirep_geom *g, double m0, void *x_even, const void *b_even, const void *links, double tol,
                                       int maxiter, int *iters, double *relres) {

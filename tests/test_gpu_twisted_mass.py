@@ -67,3 +67,23 @@ def test_twisted_mass_rebuild_mode_and_persistent_grid(env):
     assert oracle.rel_l2(p.to_numpy(p.geom.Dphi_tm_hat(cfg.m0, mu, xe, p.links_rep), hirep.EVEN), ref) < 1e-13
     p.geom.set_link_mode(hirep.LINKS_REBUILD)
     assert oracle.rel_l2(p.to_numpy(p.geom.Dphi_tm_hat(cfg.m0, mu, xe, p.links_fund), hirep.EVEN), ref) < 1e-13
+
+
+def test_twisted_mass_cg(env):
+    """CG on (D^tm)^dag D^tm: the twist lifts the spectrum by mu^2, so the solve needs fewer iterations than mu = 0;
+    solution against the oracle's CG and the true residual through the oracle operator."""
+    from oracle import linalg as la
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS["C2"].resized(4, 4)
+    p = Problem(env, cfg, "f64")
+    T, L, d, m0, mu = 4, 4, cfg.d_R, 0.2, 0.5
+    b = p.spinors[0]
+    A = lambda v: oracle.Dphi_tm_sq(T, L, d, m0, mu, p.R, v, BC)
+    x_ref, it_ref, _, _ = la.cg(A, b, 1e-10, 3000)
+    xs, it, res = p.geom.cg_Dphi_tm_sq(m0, mu, p.to_native(b, hirep.FULL), p.links_rep, 1e-10, 3000)
+    x = p.to_numpy(xs, hirep.FULL)
+    assert res <= 1e-10 and abs(it - it_ref) <= 2
+    assert oracle.rel_l2(x, x_ref) < 1e-7
+    assert np.linalg.norm((b - A(x)).ravel()) < 1e-9 * np.linalg.norm(b.ravel())
+    _, it0, _ = p.geom.cg_g5Dphi_sq(m0, p.to_native(b, hirep.FULL), p.links_rep, 1e-10, 3000)
+    assert it < it0
