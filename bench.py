@@ -167,6 +167,9 @@ def run_ours(args):
     hirep.load()
 
     cfg = synth.CONFIGS[args.config]
+    if args.custom:   # "N_g,rep,T,L": any other gauge group / representation / lattice (same recipe as C2: Haar links)
+        n_g, rep, T, L = [int(v) for v in args.custom.split(",")]
+        cfg = synth.Config("custom", T, L, n_g, rep, -0.2, "haar", 77, ("Dphi_eo", "Dphi_hat"))
     prec = args.prec
     rebuild = args.link_mode == "rebuild"
     cm = cost_model(cfg, prec, rebuild)
@@ -469,6 +472,7 @@ def main():
     ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--custom", default="", help="N_g,rep,T,L instead of --config (rep: 0 FUND, 1 ADJ, 2 SYM, 3 2AS); per-op table only")
     ap.add_argument("--link-mode", default="stored", choices=["stored", "rebuild"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the linear-algebra / CG measurements")

@@ -32,7 +32,8 @@ template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int
     return KERR_UNSUPPORTED;
 }
 
-// d_R >= 8: variant 0 = row-group kernel with bulk-copy rings (hop_rows.cuh; R rows per warp, TP tiles per CTA),
+// d_R >= 8: variant 0 = row-group kernel with bulk-copy rings (hop_rows.cuh; R rows per warp, TP tiles per CTA;
+// shapes from a sweep on 32x24^3, profiles/r01b_summary.md),
 // variant 1 = the direct-load row-group kernel of round 1 (hop_large.cuh), kept for comparison
 template <typename T, int DR, bool REAL, int R, int TP> int hop_large_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
     if (variant == 0) return launch_hop_rows<T, DR, REAL, R, TP>(g, L, s);
@@ -75,7 +76,7 @@ template <typename T> int hop_by_config(const Geo &g, int N, int rep, int mode, 
         case 4: return hop_small_variant<T, 4, false>(g, variant, L, s);
         case 5: return hop_small_variant<T, 5, false>(g, variant, L, s);
         case 6: return hop_small_variant<T, 6, false>(g, variant, L, s);
-        case 10: return hop_large_variant<T, 10, false, 5, 3>(g, variant, L, s);   // SU(4) SYM, SU(5) 2AS
+        case 10: return hop_large_variant<T, 10, false, 2, 2>(g, variant, L, s);   // SU(4) SYM, SU(5) 2AS
         case 15: return hop_large_variant<T, 15, false, 3, 2>(g, variant, L, s);   // SU(5) SYM, SU(6) 2AS
         case 21: return hop_large_variant<T, 21, false, 3, 1>(g, variant, L, s);   // SU(6) SYM
         }
@@ -83,7 +84,9 @@ template <typename T> int hop_by_config(const Geo &g, int N, int rep, int mode, 
         switch (dR) {
         case 3: return hop_small_variant<T, 3, true>(g, variant, L, s);
         case 8: return hop_large_variant<T, 8, true, 4, 4>(g, variant, L, s);      // SU(3) ADJ
-        case 15: return hop_large_variant<T, 15, true, 3, 2>(g, variant, L, s);    // SU(4) ADJ
+        case 15:                                                                   // SU(4) ADJ
+            if constexpr (sizeof(T) == 8) return hop_large_variant<T, 15, true, 3, 1>(g, variant, L, s);
+            else return hop_large_variant<T, 15, true, 3, 2>(g, variant, L, s);
         case 24: return hop_large_variant<T, 24, true, 4, 1>(g, variant, L, s);    // SU(5) ADJ
         case 35: return hop_large_variant<T, 35, true, 5, 1>(g, variant, L, s);    // SU(6) ADJ
         }
