@@ -19,7 +19,8 @@
 // Link mode REBUILD (NF > 0): the ring carries the FUNDAMENTAL gather block (N_g x N_g per direction) and each
 // row of R(W) is rebuilt in registers by RepMap (rep_maps.cuh) -- "rebuilding the represented field on the fly",
 // L343.  The boundary sign (Eq 61), which the stored represented field carries (L945), is applied to the
-// half spinor instead.  Both warps of the pair rebuild the rows they need (the rebuild is done twice per tile).
+// half spinor instead.  The pair rebuilds R(W) once per direction: each warp its half of the rows, into a shared-
+// memory buffer both then multiply from (two named barriers per direction); for FUND there is nothing to rebuild.
 #pragma once
 #include "hop_ring.cuh"
 #include "rep_maps.cuh"
@@ -46,16 +47,18 @@ template <int D> __device__ __forceinline__ int hop_sign_dir(const Geo &g, int p
     return (fwd ? (c == ext - 1) : (c == 0)) ? g.bc[mu] : 1;
 }
 
-template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF> struct PairCfg {
+template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF, int REP = 0> struct PairCfg {
     using E = link_elem<T, REAL>;                                   // element type of R
     static constexpr bool REBUILD = NF > 0;
+    static constexpr bool SHARED = REBUILD && REP != 0;             // the pair rebuilds R(W) once, into shared memory
     static constexpr int CPD = REBUILD ? 1 : DR / RPC;              // chunks per direction
     static constexpr uint32_t CHUNK = REBUILD ? NF * NF * TILE * sizeof(cplx<T>) : RPC * DR * TILE * sizeof(E);
     static_assert(REBUILD || DR % RPC == 0, "rows per chunk must divide d_R");
     static constexpr uint32_t SELF_BYTES = SELF ? 4 * DR * TILE * sizeof(cplx<T>) : 0;
     static constexpr uint32_t X_BYTES = 2 * DR * TILE * sizeof(cplx<T>);   // cross contributions of both warps
+    static constexpr uint32_t R_BYTES = SHARED ? DR * DR * TILE * sizeof(E) : 0;   // the rebuilt R(W) of one direction
     static constexpr uint32_t NBAR = 2 * STAGES + 2;                // full[S], empty[S], self full, self empty
-    static constexpr size_t PER_PAIR = (size_t)STAGES * CHUNK + SELF_BYTES + X_BYTES + NBAR * 8;
+    static constexpr size_t PER_PAIR = (size_t)STAGES * CHUNK + SELF_BYTES + X_BYTES + R_BYTES + NBAR * 8;
     static constexpr size_t SMEM = PER_PAIR * PAIRS;
     static_assert(CHUNK % 16 == 0 && PER_PAIR % 16 == 0, "bulk copies need 16-byte alignment");
     static_assert(SMEM <= 227 * 1024, "pair rings do not fit the 227 KB of shared memory of an sm_100 CTA");
@@ -65,8 +68,8 @@ template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SE
 __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, const HopLaunch L) {
     using C = cplx<T>;
     using E = link_elem<T, REAL>;
-    using Cfg = PairCfg<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF>;
-    constexpr bool REBUILD = NF > 0;
+    using Cfg = PairCfg<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF, REP>;
+    constexpr bool REBUILD = NF > 0, SHARED = Cfg::SHARED;
     constexpr int NC = 4 * DR, CPD = Cfg::CPD, CPT = 8 * CPD;
     constexpr int RPCE = REBUILD ? DR : RPC;                        // rows of R served by one chunk
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -78,7 +81,8 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
     const C *selfbuf = reinterpret_cast<const C *>(base + (size_t)STAGES * Cfg::CHUNK);
     C *xbuf = reinterpret_cast<C *>(base + (size_t)STAGES * Cfg::CHUNK + Cfg::SELF_BYTES);
     const uint32_t ring_s = smem_u32(ring), self_s = smem_u32(selfbuf);
-    const uint32_t full_s = smem_u32(base + (size_t)STAGES * Cfg::CHUNK + Cfg::SELF_BYTES + Cfg::X_BYTES);
+    E *rbuf = reinterpret_cast<E *>(base + (size_t)STAGES * Cfg::CHUNK + Cfg::SELF_BYTES + Cfg::X_BYTES);
+    const uint32_t full_s = smem_u32(base + (size_t)STAGES * Cfg::CHUNK + Cfg::SELF_BYTES + Cfg::X_BYTES + Cfg::R_BYTES);
     const uint32_t empty_s = full_s + 8 * STAGES;
     const uint32_t selffull_s = empty_s + 8 * STAGES, selfempty_s = selffull_s + 8;
     const bool producer = (s == 0) && (lane == 0);
@@ -200,6 +204,50 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
                     fetch(neighbour<dir_of<true>(0)>(g, p_out, t, x, y, zh), DirInfo<dir_of<true>(0)>::swap);
                 }
             }
+            if constexpr (SHARED) {
+                // (a1') REBUILD: the two warps rebuild R(W) ONCE -- each its half of the rows -- from the fundamental
+                // chunk into the pair's R buffer, then both multiply all rows from there
+                mbar_wait(full_s + 8 * slot, phase);
+                {
+                    const SmemMat<T> Wm{reinterpret_cast<const C *>(ring + (size_t)slot * Cfg::CHUNK) + lane};
+                    constexpr int H = (DR + 1) / 2;
+                    static_for<0, DR>([&](auto ic) {
+                        constexpr int i = decltype(ic)::value;
+                        if ((i < H) == (s == 0)) {
+                            E w[DR];
+                            RepMap<T, NF, REP>::template row<i>(Wm, w);
+#pragma unroll
+                            for (int j = 0; j < DR; ++j) rbuf[(i * DR + j) * TILE + lane] = w[j];
+                        }
+                    });
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty_s + 8 * slot);
+                if (producer && q + STAGES < my_chunks) {
+                    mbar_wait(empty_s + 8 * slot, phase);
+                    issue(slot);
+                }
+                ++q;
+                if (++slot == STAGES) { slot = 0; phase ^= 1; }
+                pair_sync(1 + pair);   // R(W) of this direction complete
+                static_for<0, DR>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    E w[DR];
+#pragma unroll
+                    for (int j = 0; j < DR; ++j) w[j] = rbuf[(i * DR + j) * TILE + lane];
+                    C chi = mk<T>(0, 0);
+#pragma unroll
+                    for (int j = 0; j < DR; ++j) mac<T>(chi, w[j], hs[j]);
+                    up[i].x += chi.x;
+                    up[i].y += chi.y;
+                    C add;   // sg conj(k_mu(s)) chi
+                    if (DI::imag) add = mk<T>(cs * chi.y, -cs * chi.x);
+                    else add = mk<T>(cs * chi.x, cs * chi.y);
+                    if (DI::swap) { lx[i].x += add.x; lx[i].y += add.y; }
+                    else { ls[i].x += add.x; ls[i].y += add.y; }
+                });
+                pair_sync(1 + pair);   // both warps are done with R before the next direction overwrites it
+            } else {
             // (a3) link rows from the pair's ring, (a4) reconstruct + accumulate
             static_for<0, DR>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
@@ -235,6 +283,7 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
                     if (++slot == STAGES) { slot = 0; phase ^= 1; }
                 }
             });
+            }
         });
 
         // exchange the cross contributions: lower component s += partner's lx
@@ -278,7 +327,7 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
 
 template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF, int REP>
 int launch_hop_pair_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
-    using Cfg = PairCfg<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF>;
+    using Cfg = PairCfg<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF, REP>;
     auto kern = hop_pair_kernel<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF, REP>;
     static int n_sm = 0;
     if (n_sm == 0) {
@@ -297,10 +346,11 @@ int launch_hop_pair_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
 
 // default shape of the pair kernel: PAIRS pairs per CTA; the chunk is the largest whole number of link rows that
 // divides d_R, stays <= 13 KB and leaves room for two stages; then as many stages (<= 4) as fit
-template <typename T, int DR, bool REAL, bool SELF, int NF> struct PairPick {
+template <typename T, int DR, bool REAL, bool SELF, int NF, int REP = 0> struct PairPick {
     using E = link_elem<T, REAL>;
     static constexpr int PAIRS = sizeof(T) == 4 ? 8 : 4;   // warps per SM sub-partition: 4 (fp32, <= 128 registers) or 2 (fp64, <= 255)
-    static constexpr size_t FIXED = (SELF ? 4 : 0) * DR * TILE * sizeof(cplx<T>) + 2 * DR * TILE * sizeof(cplx<T>) + 10 * 8;
+    static constexpr size_t FIXED = (SELF ? 4 : 0) * DR * TILE * sizeof(cplx<T>) + 2 * DR * TILE * sizeof(cplx<T>) +
+                                    ((NF > 0 && REP != 0) ? DR * DR * TILE * sizeof(E) : 0) + 10 * 8;
     static constexpr size_t chunk_of(int r) { return NF > 0 ? (size_t)NF * NF * TILE * sizeof(cplx<T>) : (size_t)r * DR * TILE * sizeof(E); }
     static constexpr int stages_of(int r) {
         const size_t per_pair = ((226 * 1024) / PAIRS) & ~(size_t)15;
@@ -323,10 +373,10 @@ template <typename T, int DR, bool REAL, bool SELF, int NF> struct PairPick {
 template <typename T, int DR, bool REAL, int NF = 0, int REP = 0> int launch_hop_pair(const Geo &g, const HopLaunch &L, cudaStream_t s) {
     const bool self = (L.a != 0.0) && L.set[0].self != nullptr;
     if (self) {
-        using P = PairPick<T, DR, REAL, true, NF>;
+        using P = PairPick<T, DR, REAL, true, NF, REP>;
         return launch_hop_pair_cfg<T, DR, REAL, P::PAIRS, P::STAGES, P::RPC, true, NF, REP>(g, L, s);
     }
-    using P = PairPick<T, DR, REAL, false, NF>;
+    using P = PairPick<T, DR, REAL, false, NF, REP>;
     return launch_hop_pair_cfg<T, DR, REAL, P::PAIRS, P::STAGES, P::RPC, false, NF, REP>(g, L, s);
 }
 
