@@ -59,6 +59,23 @@ def test_geom_create_validation_and_sizes(hirep):
     hirep.hirep_geom_destroy(g)
 
 
+def test_maximum_sizes(hirep):
+    """Largest lattices: byte counts are computed in size_t without overflow, and a lattice whose half-volume does not
+    fit 32-bit site indices is rejected (no partial handle)."""
+    g = hirep.hirep_geom_create(256, 128, 6, hirep.ADJ, hirep.F64)          # V = 2^29 sites, d_R = 35
+    sz = hirep.hirep_geom_sizes(g)
+    V = 256 * 128 ** 3
+    assert sz["spinor_full"] == V * 4 * 35 * 16                              # 1.2 TB: far beyond one GPU, still exact
+    assert sz["links_rep"] == 2 * (V // 2) * 8 * 35 * 35 * 8 and sz["links_fund"] == 2 * (V // 2) * 8 * 36 * 16
+    hirep.hirep_geom_destroy(g)
+    with pytest.raises(hirep.HirepError, match="too large"):
+        hirep.hirep_geom_create(4096, 128, 3, hirep.FUND, hirep.F64)         # V/2 = 2^32 sites
+    g = hirep.hirep_geom_create(2, 2, 2, hirep.FUND, hirep.F32)              # smallest lattice: 8 sites per parity, one padded tile
+    sz = hirep.hirep_geom_sizes(g)
+    assert sz["spinor_half"] == 1 * 8 * 32 * 8 and sz["links_fund"] == 2 * 1 * 8 * 4 * 32 * 8
+    hirep.hirep_geom_destroy(g)
+
+
 @pytest.mark.parametrize("n,rep,d", [(2, 0, 2), (3, 0, 3), (2, 1, 3), (4, 3, 6), (6, 1, 35), (3, 2, 6), (4, 2, 10), (6, 3, 15)])
 def test_rep_dimensions_table1(hirep, n, rep, d):
     g = hirep.hirep_geom_create(4, 4, n, rep, hirep.F64)

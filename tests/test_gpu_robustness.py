@@ -76,3 +76,39 @@ def test_reductions_and_cg_are_deterministic(env):
         s, it, res = p.geom.cg_g5Dphi_sq(0.5, x, p.links_rep, 1e-10, 500)
         sols.append((p.to_numpy(s, hirep.FULL), it, res))
     assert sols[0][1:] == sols[1][1:] and np.array_equal(sols[0][0], sols[1][0])
+
+
+def test_cuda_graph_capture_and_replay(env):
+    """The operator calls only enqueue kernels on the geometry's stream (no allocation or synchronisation once the
+    workspaces exist), so a whole step can be captured in a CUDA graph and replayed -- the launch-bound small-lattice
+    case of BASELINE configs[0] (4^4).  Replay must reproduce the eager result bit for bit."""
+    torch, hirep = env["torch"], env["hirep"]
+    cfg = synth.CONFIGS["C1"]
+    U, (psi,) = synth.make_inputs(cfg)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        g = hirep.Geometry(cfg.T, cfg.L, cfg.n_g, cfg.rep, "f64", device=env["dev"])
+        lf = g.links_import(torch.from_numpy(U).to(env["dev"]))
+        lr = g.links_to_rep(lf)
+        x = g.spinor_import(torch.from_numpy(psi).to(env["dev"]))
+        hb = g.sizes["spinor_half"]
+        ye, yf = g.new_spinor(hirep.EVEN), g.new_spinor(hirep.FULL)
+
+        def step():
+            g.links_to_rep(lf, out=lr)
+            g.Dphi_hat(cfg.m0, x[:hb], lr, out=ye)
+            g.g5Dphi_sq(cfg.m0, x, lr, out=yf)
+            g.Dphi_tm_hat(cfg.m0, 0.2, x[:hb], lr, out=ye)
+
+        for _ in range(2):
+            step()                       # warm-up: workspaces and kernel attributes are set up outside the capture
+        s.synchronize()
+        ref_e, ref_f = ye.clone(), yf.clone()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s):
+            step()
+        ye.zero_(); yf.zero_()
+        for _ in range(3):
+            graph.replay()
+        s.synchronize()
+        assert torch.equal(ye, ref_e) and torch.equal(yf, ref_f)
