@@ -351,7 +351,9 @@ template <typename T, int DR, bool REAL, bool SELF, int NF, int REP = 0> struct 
     // fp64 pure-hop passes run 3 pairs per CTA: fewer tiles in flight shorten the tile time (bytes per tile / the SM's
     // bandwidth share), which keeps the cross-tile spinor re-use inside what L2 retains (C4 fp64 Dphi_eo: 4 pairs 4.89 ms /
     // 30.4 GB read, 3 pairs 4.52 ms / 28.1 GB, 2 pairs 4.91 ms at 6.4 TB/s); passes with a diagonal term keep 4
-    static constexpr int PAIRS = sizeof(T) == 4 ? 8 : ((SELF || NF > 0) ? 4 : 3);   // warps per SM sub-partition: 4 (fp32, <= 128 registers) or 2 (fp64, <= 255)
+    // fp32: 8 pairs (4 warps per scheduler, <= 128 registers); REBUILD 6 pairs (168 registers: the rebuild no longer
+    // spills; C4 fp32 rebuilt Dphi_hat 5.05 -> 4.41 ms, below the 4.62 ms of stored links)
+    static constexpr int PAIRS = sizeof(T) == 4 ? (NF > 0 ? 6 : 8) : ((SELF || NF > 0) ? 4 : 3);   // warps per SM sub-partition: 4 (fp32, <= 128 registers) or 2 (fp64, <= 255)
     static constexpr size_t FIXED = (SELF ? 4 : 0) * DR * TILE * sizeof(cplx<T>) + 2 * DR * TILE * sizeof(cplx<T>) +
                                     ((NF > 0 && REP != 0) ? DR * DR * TILE * sizeof(E) : 0) + 10 * 8;
     static constexpr size_t chunk_of(int r) { return NF > 0 ? (size_t)NF * NF * TILE * sizeof(cplx<T>) : (size_t)r * DR * TILE * sizeof(E); }
