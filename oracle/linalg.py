@@ -174,3 +174,51 @@ def cg(apply_A, b, tol: float, maxiter: int, x0=None):
         p = r + beta * p
         rr = rr_new
     return x, it, math.sqrt(rr / bb), hist
+
+
+def cg_mshift(apply_A, b, shifts, tol: float, maxiter: int):
+    """Multi-shift conjugate gradient (L730: "the Multi-Shift Conjugate Gradient ... is necessary for simulations
+    with the RHMC"; Eq 39-40: the rational approximation needs (Q_m^2 + beta_k)^{-1} b for all k at once).
+
+    The paper prints no recurrence; the textbook one is used (reading A24 of DESIGN.md).  All shifted systems
+    (A + sigma_k) x_k = b share the Krylov space of A: their residuals are collinear with the residual r of the
+    unshifted recurrence, r_k = zeta_k r, with
+        zeta_k' = zeta_k zeta_k^- alpha^- / ( alpha beta^- (zeta_k^- - zeta_k) + zeta_k^- alpha^- (1 + sigma_k alpha) )
+        alpha_k = alpha zeta_k'/zeta_k ,  beta_k = beta (zeta_k'/zeta_k)^2
+        x_k += alpha_k p_k ,  p_k' = zeta_k' r' + beta_k p_k
+    where alpha, beta are the step and direction coefficients of plain CG on A (superscript - : previous iteration;
+    alpha^- = 1, beta^- = 0, zeta = zeta^- = 1 at the start).  Stops on the unshifted residual (the shifted ones are
+    smaller for sigma_k >= 0).  Returns ([x_k], iterations, relative residual of the unshifted recurrence)."""
+    b = np.asarray(b, dtype=np.complex128)
+    ns = len(shifts)
+    xs = [np.zeros_like(b) for _ in range(ns)]
+    ps = [b.copy() for _ in range(ns)]
+    r, p = b.copy(), b.copy()
+    bb = sqnorm(b)
+    rr = bb
+    zeta = [1.0] * ns
+    zeta_old = [1.0] * ns
+    alpha_old, beta_old = 1.0, 0.0
+    it = 0
+    if bb == 0.0:
+        return xs, 0, 0.0
+    while it < maxiter and rr > tol * tol * bb:
+        Ap = apply_A(p)
+        alpha = rr / prod_re(p, Ap)
+        zeta_new = []
+        for k in range(ns):
+            zn = zeta[k] * zeta_old[k] * alpha_old / (alpha * beta_old * (zeta_old[k] - zeta[k])
+                                                     + zeta_old[k] * alpha_old * (1.0 + float(shifts[k]) * alpha))
+            zeta_new.append(zn)
+            xs[k] = xs[k] + (alpha * zn / zeta[k]) * ps[k]
+        r = r - alpha * Ap
+        rr_new = sqnorm(r)
+        it += 1
+        beta = rr_new / rr
+        for k in range(ns):
+            ps[k] = zeta_new[k] * r + (beta * (zeta_new[k] / zeta[k]) ** 2) * ps[k]
+        p = r + beta * p
+        zeta_old, zeta = zeta, zeta_new
+        alpha_old, beta_old = alpha, beta
+        rr = rr_new
+    return xs, it, math.sqrt(rr / bb)

@@ -195,3 +195,37 @@ def test_cg_zero_rhs_and_initial_guess():
     b = np.array([1.0, 1.0j, -2.0])
     x, it, res, _ = la.cg(lambda v: A @ v, b, 1e-14, 10, x0=np.linalg.solve(A, b))
     assert it == 0
+
+
+def test_multishift_cg_against_direct_solves(oracle):
+    """Every shifted solution of the multi-shift CG equals the direct solve of (A + sigma_k) x = b -- on a random
+    Hermitian positive-definite matrix and on the dense (gamma_5 D)^2 of the 4^4 lattice -- and the zero shift
+    reproduces plain CG iterate for iterate."""
+    rng = np.random.default_rng(8)
+    n = 40
+    Q, _ = np.linalg.qr(rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n)))
+    A = (Q * rng.uniform(0.2, 5.0, size=n)) @ Q.conj().T
+    b = rng.normal(size=n) + 1j * rng.normal(size=n)
+    shifts = [0.0, 0.05, 0.7, 3.0]
+    xs, it, res = la.cg_mshift(lambda v: A @ v, b, shifts, 1e-13, 500)
+    assert res <= 1e-13
+    for sg, x in zip(shifts, xs):
+        ref = np.linalg.solve(A + sg * np.eye(n), b)
+        assert np.linalg.norm(x - ref) < 1e-11 * np.linalg.norm(ref), sg
+    x0, it0, _, _ = la.cg(lambda v: A @ v, b, 1e-13, 500)
+    assert it0 == it and np.linalg.norm(xs[0] - x0) < 1e-12 * np.linalg.norm(x0)
+    # the lattice operator
+    cfg = synth.CONFIGS["C1"]
+    U, (bl,) = synth.make_inputs(cfg)
+    R = oracle.represent_field(cfg.n_g, cfg.rep, U)
+    m0 = 0.6
+    D = dense.dense_D(cfg.T, cfg.L, cfg.n_g, cfg.rep, U, m0, BC)
+    G5 = np.kron(np.eye(cfg.volume), np.kron(dense.gamma5(), np.eye(cfg.d_R)))
+    Qsq = G5 @ D @ G5 @ D
+    shape = bl.shape
+    shifts = [0.01, 0.3, 2.0]
+    xs, it, res = la.cg_mshift(lambda v: oracle.g5Dphi_sq(cfg.T, cfg.L, cfg.d_R, m0, R, v.reshape(shape), BC), bl, shifts, 1e-12, 3000)
+    assert res <= 1e-12
+    for sg, x in zip(shifts, xs):
+        ref = np.linalg.solve(Qsq + sg * np.eye(Qsq.shape[0]), bl.ravel())
+        assert np.linalg.norm(x.ravel() - ref) < 1e-9 * np.linalg.norm(ref), sg
