@@ -154,6 +154,12 @@ int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, double *out
  * *relres).  Full-lattice native spinors; iters / relres are host pointers (may be NULL).  x must not alias b. */
 int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const void *b_full, const void *links, double tol, int maxiter,
                        int *iters, double *relres);
+/* Multi-shift CG (L730; Eq 39-40): (Q_m^2 + shifts[k]) x[k] = b for all k < nshift <= HIREP_MAX_SHIFTS in one
+ * Krylov space -- the inversion the RHMC's rational approximation needs.  shifts: host array, >= 0; x_full: host array of
+ * nshift device pointers (native full-lattice spinors, distinct from b).  Stops on the unshifted residual. */
+#define HIREP_MAX_SHIFTS 16
+int hirep_cg_mshift_g5Dphi_sq(hirep_geom *g, double m0, int nshift, const double *shifts, void *const *x_full, const void *b_full,
+                              const void *links, double tol, int maxiter, int *iters, double *relres);
 /* The same for (D^tm)^dagger D^tm x = b (hirep_Dphi_tm_sq), the twisted-mass monomial's operator. */
 int hirep_cg_Dphi_tm_sq(hirep_geom *g, double m0, double mu, void *x_full, const void *b_full, const void *links, double tol,
                         int maxiter, int *iters, double *relres);

@@ -25,6 +25,7 @@ struct hirep_geom {
     void *ws_half, *ws_half2, *ws_full;   // workspace spinors (lazy)
     void *ws_red;                   // reduction partials + 4 result doubles (lazy)
     void *cg_r, *cg_p, *cg_Ap;      // CG work fields (lazy)
+    void *ms_p[HIREP_MAX_SHIFTS];    // multi-shift CG direction fields (lazy)
     // hirep_apply_host staging (lazy)
     void *h_links_canon, *h_links_fund, *h_links_rep, *h_in_canon, *h_in_native, *h_out_native, *h_out_canon;
     int host_links_ready;
@@ -95,6 +96,8 @@ extern "C" int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep
 
 extern "C" int hirep_geom_destroy(hirep_geom *g) {
     if (!g) return HIREP_OK;
+    for (void *b : g->ms_p)
+        if (b) cudaFree(b);
     void *bufs[] = {g->ws_half, g->ws_half2, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
                     g->h_in_native, g->h_out_native, g->h_out_canon};
     for (void *b : bufs)
@@ -471,6 +474,72 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
         ++it;
         const double beta[2] = {rr_new / rr, 0.0};
         if ((rc = lincomb(g, which, g->cg_p, beta, 1, g->cg_r, ONE2, g->cg_r, ZERO2, 0, what))) return rc;
+        rr = rr_new;
+    }
+    if (iters) *iters = it;
+    if (relres) *relres = bb > 0.0 ? sqrt(rr / bb) : 0.0;
+    return hirep_sync(g);
+}
+
+// Multi-shift CG for (Q_m^2 + sigma_k) x_k = b, k < nshift (L730; Eq 39-40: what the RHMC's rational approximation
+// needs).  One Krylov space: the unshifted recurrence (r, p, alpha, beta) plus, per shift, zeta_k, x_k and p_k
+// (recurrence: DESIGN.md A24).  Per iteration: the operator, <p,Ap>, the residual update +
+// ||r||^2, the p update, and two fused linear combinations per shift.
+extern "C" int hirep_cg_mshift_g5Dphi_sq(hirep_geom *g, double m0, int nshift, const double *shifts, void *const *x_full, const void *b_full,
+                                         const void *links, double tol, int maxiter, int *iters, double *relres) {
+    CHECK_PTRS("hirep_cg_mshift_g5Dphi_sq", b_full, links);
+    const char *what = "hirep_cg_mshift_g5Dphi_sq";
+    if (!shifts || !x_full || nshift < 1 || nshift > HIREP_MAX_SHIFTS) return fail(HIREP_EINVAL, "%s: nshift=%d (1..%d), shifts/x must be given", what, nshift, HIREP_MAX_SHIFTS);
+    if (!(tol > 0.0) || maxiter < 0) return fail(HIREP_EINVAL, "%s: tol=%g maxiter=%d", what, tol, maxiter);
+    for (int k = 0; k < nshift; ++k) {
+        if (!x_full[k] || misaligned(x_full[k]) || x_full[k] == b_full) return fail(HIREP_EINVAL, "%s: bad solution pointer %d", what, k);
+        if (!(shifts[k] >= 0.0)) return fail(HIREP_EINVAL, "%s: shift %d = %g must be >= 0", what, k, shifts[k]);
+    }
+    const size_t fb = 2 * g->bytes_spinor_half;
+    int rc;
+    if ((rc = workspace(&g->cg_r, fb)) || (rc = workspace(&g->cg_p, fb)) || (rc = workspace(&g->cg_Ap, fb)) || (rc = red_workspace(g))) return rc;
+    cudaError_t e = cudaMemcpyAsync(g->cg_r, b_full, fb, cudaMemcpyDeviceToDevice, g->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(g->cg_p, b_full, fb, cudaMemcpyDeviceToDevice, g->stream);
+    for (int k = 0; k < nshift && e == cudaSuccess; ++k) {
+        if ((rc = workspace(&g->ms_p[k], fb))) return rc;
+        e = cudaMemsetAsync(x_full[k], 0, fb, g->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(g->ms_p[k], b_full, fb, cudaMemcpyDeviceToDevice, g->stream);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, what);
+    double bb, rr, res[2];
+    if ((rc = hirep_spinor_sqnorm(g, HIREP_FULL, b_full, &bb))) return rc;
+    rr = bb;
+    double zeta[HIREP_MAX_SHIFTS], zeta_old[HIREP_MAX_SHIFTS], zeta_new[HIREP_MAX_SHIFTS];
+    for (int k = 0; k < nshift; ++k) zeta[k] = zeta_old[k] = 1.0;
+    double alpha_old = 1.0, beta_old = 0.0;
+    int it = 0;
+    while (bb > 0.0 && it < maxiter && rr > tol * tol * bb) {
+        if ((rc = hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links))) return rc;
+        if ((rc = reduce_prod(g, HIREP_FULL, 0, g->cg_p, g->cg_Ap, res, what))) return rc;
+        if (!(res[0] > 0.0)) return fail(HIREP_EINVAL, "%s: <p,Ap> = %g is not positive", what, res[0]);
+        const double alpha = rr / res[0];
+        for (int k = 0; k < nshift; ++k) {
+            zeta_new[k] = zeta[k] * zeta_old[k] * alpha_old /
+                          (alpha * beta_old * (zeta_old[k] - zeta[k]) + zeta_old[k] * alpha_old * (1.0 + shifts[k] * alpha));
+            const double ak[2] = {alpha * zeta_new[k] / zeta[k], 0.0};
+            if ((rc = lincomb(g, HIREP_FULL, x_full[k], ONE2, 1, g->ms_p[k], ak, g->ms_p[k], ZERO2, 0, what))) return rc;   // x_k += alpha_k p_k
+        }
+        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, 2, g->sum_alg, alpha, nullptr, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, red_out(g), g->stream), what, 2);
+        if (rc) return rc;
+        if ((rc = fetch_result(g, res, 2, what))) return rc;
+        const double rr_new = res[0], beta = rr_new / rr;
+        ++it;
+        for (int k = 0; k < nshift; ++k) {
+            const double q = zeta_new[k] / zeta[k];
+            const double bk[2] = {beta * q * q, 0.0}, zk[2] = {zeta_new[k], 0.0};
+            if ((rc = lincomb(g, HIREP_FULL, g->ms_p[k], bk, 1, g->cg_r, zk, g->cg_r, ZERO2, 0, what))) return rc;   // p_k = zeta_k' r + beta_k p_k
+            zeta_old[k] = zeta[k];
+            zeta[k] = zeta_new[k];
+        }
+        const double b2[2] = {beta, 0.0};
+        if ((rc = lincomb(g, HIREP_FULL, g->cg_p, b2, 1, g->cg_r, ONE2, g->cg_r, ZERO2, 0, what))) return rc;
+        alpha_old = alpha;
+        beta_old = beta;
         rr = rr_new;
     }
     if (iters) *iters = it;

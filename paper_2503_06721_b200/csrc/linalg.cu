@@ -187,11 +187,15 @@ __global__ void __launch_bounds__(RED_THREADS) cg_update_kernel(Pad P, long n, i
     Acc a[2] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
     const T al = (T)alpha;
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
-        const cplx<T> pv = p[i], av = Ap[i];
-        cplx<T> xv = x[i], rv = r[i];
-        xv.x += al * pv.x; xv.y += al * pv.y;
+        const cplx<T> av = Ap[i];
+        cplx<T> rv = r[i];
+        if (x != nullptr) {   // null: only the residual is updated (multi-shift CG keeps its own x_k, p_k)
+            const cplx<T> pv = p[i];
+            cplx<T> xv = x[i];
+            xv.x += al * pv.x; xv.y += al * pv.y;
+            x[i] = xv;
+        }
         rv.x -= al * av.x; rv.y -= al * av.y;
-        x[i] = xv;
         r[i] = rv;
         if (is_site(P, i)) {
             acc_add(a[0], __dmul_rn((double)rv.x, (double)rv.x), alg);

@@ -242,3 +242,30 @@ def test_full_size_linalg_and_cg(env, prec):
         r = host[ix] - so.g5Dphi_sq(fetch, ix, m0)
         assert np.linalg.norm(r) <= (1e-6 if prec == "f64" else 2e-3) * bnorm * np.sqrt(4 * cfg.d_R), (ix, np.linalg.norm(r))
     geom.sync()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_multishift_cg(env, prec):
+    """Multi-shift CG on Q^2 (L730, Eq 39-40): every shifted solution against the oracle's multi-shift CG and, through
+    the oracle operator, the true residual of its own system; same iteration count as the oracle (+-2)."""
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS["C2"].resized(4, 4)
+    p = Problem(env, cfg, prec)
+    T, L, d, m0 = 4, 4, cfg.d_R, 0.3
+    b = p.spinors[0]
+    shifts = [0.0, 0.02, 0.5, 4.0]
+    tol = 1e-10 if prec == "f64" else 1e-5
+    A = lambda v: oracle.g5Dphi_sq(T, L, d, m0, p.R, v, BC)
+    xs_ref, it_ref, _ = la.cg_mshift(A, b, shifts, tol, 3000)
+    xs, it, res = p.geom.cg_mshift_g5Dphi_sq(m0, shifts, p.to_native(b, hirep.FULL), p.links_rep, tol, 3000)
+    assert res <= tol and abs(it - it_ref) <= max(2, it_ref // 20)
+    bn = np.linalg.norm(b.ravel())
+    for sg, xn, xr in zip(shifts, xs, xs_ref):
+        x = p.to_numpy(xn, hirep.FULL)
+        assert oracle.rel_l2(x, xr) < (1e-7 if prec == "f64" else 1e-3), sg
+        assert np.linalg.norm((b - A(x) - sg * x).ravel()) < (1e-9 if prec == "f64" else 1e-4) * bn, sg
+    # the zero shift is plain CG
+    x0, it0, _ = p.geom.cg_g5Dphi_sq(m0, p.to_native(b, hirep.FULL), p.links_rep, tol, 3000)
+    assert it0 == it and oracle.rel_l2(p.to_numpy(xs[0], hirep.FULL), p.to_numpy(x0, hirep.FULL)) < (1e-12 if prec == "f64" else 1e-5)
+    with pytest.raises(hirep.HirepError):
+        p.geom.cg_mshift_g5Dphi_sq(m0, [-1.0], p.to_native(b, hirep.FULL), p.links_rep, tol, 10)
