@@ -355,7 +355,7 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
     torch.cuda.synchronize()
     ms_it = (time.perf_counter() - t0) * 1e3 / max(it, 1)
     fl_it = cm["ops"]["g5Dphi_sq"][0]
-    by_it = cm["ops"]["g5Dphi_sq"][1] + (2 + 6 + 3) * S * V      # stencils + <p,Ap> + fused update + p update
+    by_it = cm["ops"]["g5Dphi_sq"][1] + (1 + 3 + 5) * S * V      # stencils + ||B p||^2 + (r update, ||r||^2) + (x, p update)
     out["cg_g5Dphi_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gflops_operator": round(fl_it / ms_it / 1e6, 1),
                            "gbs": round(by_it / ms_it / 1e6, 1), "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3),
                            "launches_per_iteration": 7, "relres_after": res}
@@ -368,7 +368,7 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
     torch.cuda.synchronize()
     ms_it = (time.perf_counter() - t0) * 1e3 / max(it, 1)
     fl_it = 2 * cm["ops"]["Dphi_hat"][0]
-    by_it = 2 * cm["ops"]["Dphi_hat"][1] + (2 + 6 + 3) * S * V / 2
+    by_it = 2 * cm["ops"]["Dphi_hat"][1] + (1 + 3 + 5) * S * V / 2
     out["cg_g5Dphi_hat_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gflops_operator": round(fl_it / ms_it / 1e6, 1),
                                "gbs": round(by_it / ms_it / 1e6, 1), "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3),
                                "launches_per_iteration": 9, "relres_after": res}

@@ -440,8 +440,8 @@ extern "C" int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, 
 // Conjugate gradient for A x = b with A = Q_m^2 = g5Dphi_sq (full lattice) or A = Q_hat^2 = g5Dphi_hat_sq (even
 // sites), both Hermitian positive definite (L772, L815).  Textbook recurrence (reading A19): x0 = 0; r = b;
 // p = r; repeat { Ap; alpha = rr/<p,Ap>; x += alpha p; r -= alpha Ap; rr' = <r,r>; stop if rr' <= tol^2 <b,b>;
-// beta = rr'/rr; p = r + beta p }.  Per iteration: the operator (2 or 4 stencil launches), <p,Ap> (2 launches), the
-// fused update + ||r||^2 (2), the p update (1).
+// beta = rr'/rr; p = r + beta p }.  Per iteration: the operator (2 or 4 stencil launches), <p,Ap> = ||B p||^2 (2 launches),
+// r -= alpha Ap fused with ||r||^2 (2), x += alpha p fused with the p update (1): 8 spinor passes of linear algebra.
 static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, const void *links, double tol, int maxiter, int *iters,
                     double *relres, const char *what, int twisted = 0, double mu = 0.0) {
     if (x == b) return fail(HIREP_EINVAL, "%s: x aliases b", what);
@@ -464,16 +464,18 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
         rc = twisted ? hirep_Dphi_tm_sq(g, m0, mu, g->cg_Ap, g->cg_p, links)
                      : full ? hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links) : hirep_g5Dphi_hat_sq(g, m0, g->cg_Ap, g->cg_p, links);
         if (rc) return rc;
-        if ((rc = reduce_prod(g, which, 0, g->cg_p, g->cg_Ap, res, what))) return rc;
+        // A = B^dagger B with B p left in the operator's workspace (gamma_5 D p, Q_hat p, gamma_5 D^tm p; gamma_5 is
+        // unitary), so <p, A p> = ||B p||^2: one field read instead of two
+        const void *Bp = (full || twisted) ? g->ws_full : g->ws_half2;
+        if ((rc = reduce_prod(g, which, 1, Bp, Bp, res, what))) return rc;
         if (!(res[0] > 0.0)) return fail(HIREP_EINVAL, "%s: <p,Ap> = %g is not positive (operator not positive definite?)", what, res[0]);
         const double alpha = rr / res[0];
-        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, halves, g->sum_alg, alpha, x, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, red_out(g), g->stream), what, 2);
+        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, halves, g->sum_alg, alpha, nullptr, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, red_out(g), g->stream), what, 2);
         if (rc) return rc;
         if ((rc = fetch_result(g, res, 2, what))) return rc;
         const double rr_new = res[0];
         ++it;
-        const double beta[2] = {rr_new / rr, 0.0};
-        if ((rc = lincomb(g, which, g->cg_p, beta, 1, g->cg_r, ONE2, g->cg_r, ZERO2, 0, what))) return rc;
+        if ((rc = kern_result(g, k_cg_xp(g->geo, g->prec, g->dR, halves, alpha, rr_new / rr, x, g->cg_p, g->cg_r, g->stream), what))) return rc;
         rr = rr_new;
     }
     if (iters) *iters = it;

@@ -41,6 +41,7 @@ int k_prod(const Geo &g, int prec, int dR, int halves, int mode, int alg, const 
 int k_maxnorm(const Geo &g, int prec, int dR, int halves, const void *xi, void *ws, double *out_dev, cudaStream_t s);
 int k_cg_update(const Geo &g, int prec, int dR, int halves, int alg, double alpha, void *x, void *r, const void *p, const void *Ap, void *ws,
                 double *out_dev, cudaStream_t s);
+int k_cg_xp(const Geo &g, int prec, int dR, int halves, double alpha, double beta, void *x, void *p, const void *r, cudaStream_t s);
 int k_fma_peak(int prec, double *tflops, cudaStream_t s);   // fma_peak.cu: measured FP64/FP32 FMA throughput
 // number of distinct kernel launches k_hop issues for this configuration (for launch accounting): always 1.
 

@@ -8,7 +8,8 @@
 //                         (second-order Neumaier, double-double) selectable -- per thread, and
 //                         merged across lanes / warps / blocks with the branch-free two-sum (L654: "either variant
 //                         can be used"); fp32 fields are accumulated in fp64 (their products are exact in fp64)
-//   cg_update             the fused CG step  x += alpha p ; r -= alpha Ap ; ||r||^2  (one pass over four fields)
+//   cg_update / cg_xp     the CG step in two fused passes:  r -= alpha Ap ; ||r||^2   and, once beta is known,
+//                         x += alpha p ; p = r + beta p   (8 spinor passes per iteration instead of 9)
 //
 // All kernels are HBM-bound streaming passes: 128-bit accesses, grid = 4 CTAs per SM, grid-stride loops.  The
 // padding lanes of the last tile (sites h >= Nh) are excluded from every reduction.
@@ -206,6 +207,20 @@ __global__ void __launch_bounds__(RED_THREADS) cg_update_kernel(Pad P, long n, i
     if (threadIdx.x == 0) { partial[2 * blockIdx.x] = a[0]; partial[2 * blockIdx.x + 1] = a[1]; }
 }
 
+// second half of the CG step, after beta is known:  x += alpha p ; p = r + beta p   (one pass: reads x, p, r; writes x, p)
+template <typename T>
+__global__ void __launch_bounds__(256) cg_xp_kernel(long n, double alpha, double beta, cplx<T> *__restrict__ x, cplx<T> *__restrict__ p,
+                                                    const cplx<T> *__restrict__ r) {
+    const T al = (T)alpha, be = (T)beta;
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
+        const cplx<T> pv = p[i], rv = r[i];
+        cplx<T> xv = x[i];
+        xv.x += al * pv.x; xv.y += al * pv.y;
+        x[i] = xv;
+        p[i] = mk<T>(rv.x + be * pv.x, rv.y + be * pv.y);
+    }
+}
+
 // second stage: merge the per-block accumulators (fixed order: deterministic), out[v] = the algorithm's final value
 __global__ void __launch_bounds__(RED_THREADS) reduce_final_kernel(int nblocks, int alg, const Acc *__restrict__ partial, double *__restrict__ out) {
     Acc a[2] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
@@ -315,6 +330,14 @@ int k_maxnorm(const Geo &g, int prec, int dR, int halves, const void *xi, void *
     if (prec == 0) maxnorm_partial_kernel<double><<<nb, RED_THREADS, 0, s>>>(P, n, (const double2 *)xi, (double *)ws);
     else maxnorm_partial_kernel<float><<<nb, RED_THREADS, 0, s>>>(P, n, (const float2 *)xi, (double *)ws);
     maxnorm_final_kernel<<<1, 1, 0, s>>>(nb, (const double *)ws, out_dev);
+    return (int)cudaGetLastError();
+}
+
+int k_cg_xp(const Geo &g, int prec, int dR, int halves, double alpha, double beta, void *x, void *p, const void *r, cudaStream_t s) {
+    const long n = (long)g.n_tiles * 4 * dR * TILE * halves;
+    const int nb = blocks_for(n);
+    if (prec == 0) cg_xp_kernel<double><<<nb, 256, 0, s>>>(n, alpha, beta, (double2 *)x, (double2 *)p, (const double2 *)r);
+    else cg_xp_kernel<float><<<nb, 256, 0, s>>>(n, alpha, beta, (float2 *)x, (float2 *)p, (const float2 *)r);
     return (int)cudaGetLastError();
 }
 
