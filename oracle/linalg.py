@@ -222,3 +222,46 @@ def cg_mshift(apply_A, b, shifts, tol: float, maxiter: int):
         alpha_old, beta_old = alpha, beta
         rr = rr_new
     return xs, it, math.sqrt(rr / bb)
+
+
+def bicgstab(apply_A, b, tol: float, maxiter: int):
+    """Stabilised bi-conjugate gradient (L730: "the stabilized Bi-Conjugate Gradient (BiCG)[35, 36] ... for
+    ill-conditioned systems often substantially faster") for a general (non-Hermitian) A x = b, e.g. A = D_m or
+    D_hat directly.  Textbook recurrence (van der Vorst), x0 = 0, shadow residual = b (reading A25 of DESIGN.md):
+        rho' = <rhat, r> ; beta = (rho'/rho)(alpha/omega) ; p = r + beta (p - omega v) ; v = A p
+        alpha = rho'/<rhat, v> ; s = r - alpha v ; t = A s ; omega = <t,s>/<t,t>
+        x += alpha p + omega s ; r = s - omega t
+    with <.,.> the product of Eq 27.  Stops when ||r|| <= tol ||b|| (checked on s as well, after the half step).
+    Returns (x, iterations, relative residual of the recurrence)."""
+    b = np.asarray(b, dtype=np.complex128)
+    x = np.zeros_like(b)
+    r = b.copy()
+    rhat = b.copy()
+    p = np.zeros_like(b)
+    v = np.zeros_like(b)
+    rho = alpha = omega = 1.0 + 0.0j
+    bb = sqnorm(b)
+    rr = bb
+    it = 0
+    if bb == 0.0:
+        return x, 0, 0.0
+    while it < maxiter and rr > tol * tol * bb:
+        rho_new = prod(rhat, r)
+        beta = (rho_new / rho) * (alpha / omega)
+        p = r + beta * (p - omega * v)
+        v = apply_A(p)
+        alpha = rho_new / prod(rhat, v)
+        s = r - alpha * v
+        it += 1
+        ss = sqnorm(s)
+        if ss <= tol * tol * bb:
+            x = x + alpha * p
+            rr = ss
+            break
+        t = apply_A(s)
+        omega = prod(t, s) / sqnorm(t)
+        x = x + alpha * p + omega * s
+        r = s - omega * t
+        rr = sqnorm(r)
+        rho = rho_new
+    return x, it, math.sqrt(rr / bb)

@@ -229,3 +229,33 @@ def test_multishift_cg_against_direct_solves(oracle):
     for sg, x in zip(shifts, xs):
         ref = np.linalg.solve(Qsq + sg * np.eye(Qsq.shape[0]), bl.ravel())
         assert np.linalg.norm(x.ravel() - ref) < 1e-9 * np.linalg.norm(ref), sg
+
+
+def test_bicgstab_against_direct_solves(oracle):
+    """BiCGstab on a random non-Hermitian matrix and on the dense D_m / D_hat of the 4^4 lattice equals numpy's direct
+    solve; it needs fewer operator applications than CG on the normal equations (the paper's remark, L730)."""
+    rng = np.random.default_rng(12)
+    n = 50
+    A = 3.0 * np.eye(n) + 0.3 * (rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n)))
+    b = rng.normal(size=n) + 1j * rng.normal(size=n)
+    x, it, res = la.bicgstab(lambda v: A @ v, b, 1e-13, 500)
+    assert res <= 1e-13 and np.linalg.norm(x - np.linalg.solve(A, b)) < 1e-11 * np.linalg.norm(x)
+    cfg = synth.CONFIGS["C1"]
+    U, (bl,) = synth.make_inputs(cfg)
+    R = oracle.represent_field(cfg.n_g, cfg.rep, U)
+    T, L, d, m0 = cfg.T, cfg.L, cfg.d_R, 0.3
+    D = dense.dense_D(T, L, cfg.n_g, cfg.rep, U, m0, BC)
+    shape = bl.shape
+    x, it, res = la.bicgstab(lambda v: oracle.Dphi(T, L, d, m0, R, v.reshape(shape), BC), bl, 1e-12, 2000)
+    ref = np.linalg.solve(D, bl.ravel())
+    assert res <= 1e-12 and np.linalg.norm(x.ravel() - ref) < 1e-9 * np.linalg.norm(ref)
+    _, it_cg, _, _ = la.cg(lambda v: oracle.g5Dphi_sq(T, L, d, m0, R, v.reshape(shape), BC), bl, 1e-12, 2000)
+    assert 2 * it < 2 * it_cg                      # operator applications: 2 per BiCGstab iteration, 2 per CG iteration on Q^2
+    # even-odd preconditioned operator
+    ev = synth.parity_sites(T, L, 0)
+    e, o = dense.parity_index(T, L, d, 0), dense.parity_index(T, L, d, 1)
+    a = 4.0 + m0
+    Dhat = a * a * np.eye(len(e)) - D[np.ix_(e, o)] @ D[np.ix_(o, e)]
+    xe, it, res = la.bicgstab(lambda v: oracle.Dphi_hat(T, L, d, m0, R, v, BC), bl[ev], 1e-12, 2000)
+    ref = np.linalg.solve(Dhat, bl[ev].ravel())
+    assert np.linalg.norm(xe.ravel() - ref) < 1e-9 * np.linalg.norm(ref)
