@@ -154,6 +154,10 @@ int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, double *out
  * *relres).  Full-lattice native spinors; iters / relres are host pointers (may be NULL).  x must not alias b. */
 int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const void *b_full, const void *links, double tol, int maxiter,
                        int *iters, double *relres);
+/* Stabilised bi-conjugate gradient (L730) for the non-Hermitian systems D_m x = b (op = HIREP_OP_DPHI, full-lattice
+ * spinors) or D_hat x = b (op = HIREP_OP_DPHI_HAT, even sites); x starts at 0; same stopping rule and outputs as the CG. */
+int hirep_bicgstab(hirep_geom *g, int op, double m0, void *x, const void *b, const void *links, double tol, int maxiter, int *iters,
+                   double *relres);
 /* Multi-shift CG (L730; Eq 39-40): (Q_m^2 + shifts[k]) x[k] = b for all k < nshift <= HIREP_MAX_SHIFTS in one
  * Krylov space -- the inversion the RHMC's rational approximation needs.  shifts: host array, >= 0; x_full: host array of
  * nshift device pointers (native full-lattice spinors, distinct from b).  Stops on the unshifted residual. */

@@ -26,6 +26,7 @@ struct hirep_geom {
     void *ws_red;                   // reduction partials + 4 result doubles (lazy)
     void *cg_r, *cg_p, *cg_Ap;      // CG work fields (lazy)
     void *ms_p[HIREP_MAX_SHIFTS];    // multi-shift CG direction fields (lazy)
+    void *bi_s, *bi_t;              // BiCGstab work fields (lazy)
     // hirep_apply_host staging (lazy)
     void *h_links_canon, *h_links_fund, *h_links_rep, *h_in_canon, *h_in_native, *h_out_native, *h_out_canon;
     int host_links_ready;
@@ -98,7 +99,7 @@ extern "C" int hirep_geom_destroy(hirep_geom *g) {
     if (!g) return HIREP_OK;
     for (void *b : g->ms_p)
         if (b) cudaFree(b);
-    void *bufs[] = {g->ws_half, g->ws_half2, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
+    void *bufs[] = {g->ws_half, g->ws_half2, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
                     g->h_in_native, g->h_out_native, g->h_out_canon};
     for (void *b : bufs)
         if (b) cudaFree(b);
@@ -543,6 +544,76 @@ extern "C" int hirep_cg_mshift_g5Dphi_sq(hirep_geom *g, double m0, int nshift, c
         alpha_old = alpha;
         beta_old = beta;
         rr = rr_new;
+    }
+    if (iters) *iters = it;
+    if (relres) *relres = bb > 0.0 ? sqrt(rr / bb) : 0.0;
+    return hirep_sync(g);
+}
+
+// BiCGstab (L730) for D_m x = b (op = HIREP_OP_DPHI, full lattice) or D_hat x = b (op = HIREP_OP_DPHI_HAT, even sites).
+// Textbook recurrence (A25), x0 = 0, shadow residual = b.  Work fields: r (cg_r), p (cg_p), v (cg_Ap), s and t
+// (bi_s, bi_t), rhat = b itself.  Per iteration: 2 operator applications, 4 products / norms, 4 fused linear combinations.
+extern "C" int hirep_bicgstab(hirep_geom *g, int op, double m0, void *x, const void *b, const void *links, double tol, int maxiter,
+                              int *iters, double *relres) {
+    CHECK_PTRS("hirep_bicgstab", x, b, links);
+    const char *what = "hirep_bicgstab";
+    if (op != HIREP_OP_DPHI && op != HIREP_OP_DPHI_HAT) return fail(HIREP_EINVAL, "%s: op %d (HIREP_OP_DPHI or HIREP_OP_DPHI_HAT)", what, op);
+    if (x == b) return fail(HIREP_EINVAL, "%s: x aliases b", what);
+    if (!(tol > 0.0) || maxiter < 0) return fail(HIREP_EINVAL, "%s: tol=%g maxiter=%d", what, tol, maxiter);
+    const int full = op == HIREP_OP_DPHI, which = full ? HIREP_FULL : HIREP_EVEN;
+    const size_t fb = (full ? 2 : 1) * g->bytes_spinor_half, wb = 2 * g->bytes_spinor_half;
+    int rc;
+    if ((rc = workspace(&g->cg_r, wb)) || (rc = workspace(&g->cg_p, wb)) || (rc = workspace(&g->cg_Ap, wb)) || (rc = workspace(&g->bi_s, wb)) ||
+        (rc = workspace(&g->bi_t, wb)) || (rc = red_workspace(g)))
+        return rc;
+    void *r = g->cg_r, *p = g->cg_p, *v = g->cg_Ap, *sv = g->bi_s, *t = g->bi_t;
+    cudaError_t e = cudaMemsetAsync(x, 0, fb, g->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(r, b, fb, cudaMemcpyDeviceToDevice, g->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(p, 0, fb, g->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(v, 0, fb, g->stream);
+    if (e != cudaSuccess) return cuda_fail(e, what);
+    auto apply = [&](void *out, const void *in) { return full ? hirep_Dphi(g, m0, out, in, links) : hirep_Dphi_hat(g, m0, out, in, links); };
+    auto cdiv = [](const double a[2], const double c[2], double out[2]) {
+        const double d = c[0] * c[0] + c[1] * c[1];
+        out[0] = (a[0] * c[0] + a[1] * c[1]) / d;
+        out[1] = (a[1] * c[0] - a[0] * c[1]) / d;
+    };
+    auto cmul2 = [](const double a[2], const double c[2], double out[2]) {
+        const double re = a[0] * c[0] - a[1] * c[1], im = a[0] * c[1] + a[1] * c[0];
+        out[0] = re; out[1] = im;
+    };
+    double bb, rr, rho[2] = {1, 0}, alpha[2] = {1, 0}, omega[2] = {1, 0};
+    if ((rc = hirep_spinor_sqnorm(g, which, b, &bb))) return rc;
+    rr = bb;
+    int it = 0;
+    while (bb > 0.0 && it < maxiter && rr > tol * tol * bb) {
+        double rho_new[2], q1[2], q2[2], beta[2], mbw[2], rv[2], ss, tt, ts[2];
+        if ((rc = reduce_prod(g, which, 0, b, r, rho_new, what))) return rc;                     // rho' = <rhat, r>
+        if (rho_new[0] == 0.0 && rho_new[1] == 0.0) return fail(HIREP_EINVAL, "%s: breakdown (rho = 0)", what);
+        cdiv(rho_new, rho, q1); cdiv(alpha, omega, q2); cmul2(q1, q2, beta);                      // beta = (rho'/rho)(alpha/omega)
+        cmul2(beta, omega, mbw); mbw[0] = -mbw[0]; mbw[1] = -mbw[1];
+        if ((rc = lincomb(g, which, p, beta, 1, r, ONE2, v, mbw, 1, what))) return rc;            // p = r + beta p - beta omega v
+        if ((rc = apply(v, p))) return rc;                                                        // v = A p
+        if ((rc = reduce_prod(g, which, 0, b, v, rv, what))) return rc;
+        cdiv(rho_new, rv, alpha);                                                                 // alpha = rho'/<rhat, v>
+        const double malpha[2] = {-alpha[0], -alpha[1]};
+        if ((rc = lincomb(g, which, sv, ZERO2, 0, r, ONE2, v, malpha, 1, what))) return rc;       // s = r - alpha v
+        ++it;
+        if ((rc = hirep_spinor_sqnorm(g, which, sv, &ss))) return rc;
+        if (ss <= tol * tol * bb) {
+            if ((rc = lincomb(g, which, x, ONE2, 1, p, alpha, p, ZERO2, 0, what))) return rc;     // x += alpha p
+            rr = ss;
+            break;
+        }
+        if ((rc = apply(t, sv))) return rc;                                                       // t = A s
+        if ((rc = reduce_prod(g, which, 0, t, sv, ts, what))) return rc;
+        if ((rc = hirep_spinor_sqnorm(g, which, t, &tt))) return rc;
+        omega[0] = ts[0] / tt; omega[1] = ts[1] / tt;                                             // omega = <t,s>/<t,t>
+        if ((rc = lincomb(g, which, x, ONE2, 1, p, alpha, sv, omega, 1, what))) return rc;        // x += alpha p + omega s
+        const double momega[2] = {-omega[0], -omega[1]};
+        if ((rc = lincomb(g, which, r, ZERO2, 0, sv, ONE2, t, momega, 1, what))) return rc;       // r = s - omega t
+        if ((rc = hirep_spinor_sqnorm(g, which, r, &rr))) return rc;
+        rho[0] = rho_new[0]; rho[1] = rho_new[1];
     }
     if (iters) *iters = it;
     if (relres) *relres = bb > 0.0 ? sqrt(rr / bb) : 0.0;

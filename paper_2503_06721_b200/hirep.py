@@ -31,7 +31,7 @@ SYMBOLS = [
     "hirep_apply_host", "hirep_spinor_lc", "hirep_spinor_clc", "hirep_spinor_lc_add_assign", "hirep_spinor_clc_add_assign",
     "hirep_spinor_lc1", "hirep_spinor_lc2", "hirep_spinor_lc3", "hirep_spinor_prod", "hirep_spinor_sqnorm",
     "hirep_spinor_max_norm", "hirep_cg_g5Dphi_sq", "hirep_spinor_g5_lc", "hirep_Dphi_tm", "hirep_Dphi_tm_sq",
-    "hirep_Dphi_tm_hat", "hirep_cg_Dphi_tm_sq", "hirep_cg_mshift_g5Dphi_sq", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
+    "hirep_Dphi_tm_hat", "hirep_cg_Dphi_tm_sq", "hirep_cg_mshift_g5Dphi_sq", "hirep_bicgstab", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
 ]
 
 
@@ -91,6 +91,7 @@ def load():
     for n in ("hirep_Dphi_tm", "hirep_Dphi_tm_sq", "hirep_Dphi_tm_hat"):
         getattr(lib, n).argtypes = [vp, cd, cd, vp, vp, vp]
     lib.hirep_cg_mshift_g5Dphi_sq.argtypes = [vp, cd, ci, c2p, ctypes.POINTER(vp), vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
+    lib.hirep_bicgstab.argtypes = [vp, ci, cd, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_cg_Dphi_tm_sq.argtypes = [vp, cd, cd, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_fma_peak.argtypes = [ci, ctypes.POINTER(cd)]
     lib.hirep_sync.argtypes = [vp]
@@ -205,6 +206,12 @@ def hirep_cg_mshift_g5Dphi_sq(g, m0, shifts, xs, b, links, tol, maxiter):
     xp = (ctypes.c_void_p * n)(*xs)
     it, res = ctypes.c_int(), (ctypes.c_double * 2)()
     _check(load().hirep_cg_mshift_g5Dphi_sq(g, m0, n, sh, xp, b, links, tol, maxiter, ctypes.byref(it), res))
+    return it.value, res[0]
+
+
+def hirep_bicgstab(g, op, m0, x, b, links, tol, maxiter):
+    it, res = ctypes.c_int(), (ctypes.c_double * 2)()
+    _check(load().hirep_bicgstab(g, op, m0, x, b, links, tol, maxiter, ctypes.byref(it), res))
     return it.value, res[0]
 
 
@@ -394,6 +401,11 @@ class Geometry:
         outs = [self.new_spinor(FULL) for _ in shifts]
         it, res = hirep_cg_mshift_g5Dphi_sq(self.handle, m0, shifts, [o.data_ptr() for o in outs], b.data_ptr(), links.data_ptr(), tol, maxiter)
         return outs, it, res
+
+    def bicgstab(self, op, m0, b, links, tol, maxiter, out=None):
+        out = self.new_spinor(FULL if op == OP_DPHI else EVEN) if out is None else out
+        it, res = hirep_bicgstab(self.handle, op, m0, out.data_ptr(), b.data_ptr(), links.data_ptr(), tol, maxiter)
+        return out, it, res
 
     def cg_Dphi_tm_sq(self, m0, mu, b, links, tol, maxiter, out=None):
         out = self.new_spinor(FULL) if out is None else out

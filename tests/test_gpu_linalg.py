@@ -269,3 +269,30 @@ def test_multishift_cg(env, prec):
     assert it0 == it and oracle.rel_l2(p.to_numpy(xs[0], hirep.FULL), p.to_numpy(x0, hirep.FULL)) < (1e-12 if prec == "f64" else 1e-5)
     with pytest.raises(hirep.HirepError):
         p.geom.cg_mshift_g5Dphi_sq(m0, [-1.0], p.to_native(b, hirep.FULL), p.links_rep, tol, 10)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("op", ["Dphi", "Dphi_hat"])
+def test_bicgstab(env, prec, op):
+    """BiCGstab (L730) on D_m (full lattice) and D_hat (even sites): solution against the oracle's BiCGstab and the true
+    residual through the oracle operator.  BiCGstab iterates are more sensitive to rounding than CG's (the products
+    rho, omega are not norms), so iteration counts may differ by a few."""
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS["C2"].resized(4, 4)
+    p = Problem(env, cfg, prec)
+    T, L, d, m0 = 4, 4, cfg.d_R, 0.3
+    tol = 1e-10 if prec == "f64" else 1e-5
+    if op == "Dphi":
+        b, w, code = p.spinors[0], hirep.FULL, hirep.OP_DPHI
+        A = lambda v: oracle.Dphi(T, L, d, m0, p.R, v, BC)
+    else:
+        b, w, code = p.spinors[0][p.ev], hirep.EVEN, hirep.OP_DPHI_HAT
+        A = lambda v: oracle.Dphi_hat(T, L, d, m0, p.R, v, BC)
+    x_ref, it_ref, _ = la.bicgstab(A, b, tol, 3000)
+    xn, it, res = p.geom.bicgstab(code, m0, p.to_native(b, w), p.links_rep, tol, 3000)
+    x = p.to_numpy(xn, w)
+    assert res <= tol and abs(it - it_ref) <= max(3, it_ref // 5), (it, it_ref)
+    assert oracle.rel_l2(x, x_ref) < (1e-7 if prec == "f64" else 1e-3)
+    assert np.linalg.norm((b - A(x)).ravel()) < (1e-9 if prec == "f64" else 1e-4) * np.linalg.norm(b.ravel())
+    with pytest.raises(hirep.HirepError):
+        p.geom.bicgstab(hirep.OP_G5DPHI_SQ, m0, p.to_native(b, w), p.links_rep, tol, 10)
