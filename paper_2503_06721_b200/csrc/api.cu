@@ -309,7 +309,16 @@ extern "C" int hirep_spinor_g5_lc(hirep_geom *g, int which, void *xi, const doub
     if (!c1 || !c2) return fail(HIREP_EINVAL, "hirep_spinor_g5_lc: NULL coefficient");
     if (which < 0 || which > 2) return fail(HIREP_EINVAL, "hirep_spinor_g5_lc: parity_or_full=%d", which);
     const long n = (long)g->geo.n_tiles * 4 * g->dR * TILE * (which == HIREP_FULL ? 2 : 1);
-    return kern_result(g, k_g5_lincomb(g->prec, n, g->dR, xi, c1, c2, eta, g->stream), "hirep_spinor_g5_lc");
+    static const double zero2[2] = {0.0, 0.0};
+    return kern_result(g, k_g5_lincomb(g->prec, n, g->dR, xi, zero2, 0, c1, c2, eta, g->stream), "hirep_spinor_g5_lc");
+}
+extern "C" int hirep_spinor_g5_lc_add_assign(hirep_geom *g, int which, void *xi, const double c0[2], const double c1[2], const double c2[2],
+                                             const void *eta) {
+    CHECK_PTRS("hirep_spinor_g5_lc_add_assign", xi, eta);
+    if (!c0 || !c1 || !c2) return fail(HIREP_EINVAL, "hirep_spinor_g5_lc_add_assign: NULL coefficient");
+    if (which < 0 || which > 2) return fail(HIREP_EINVAL, "hirep_spinor_g5_lc_add_assign: parity_or_full=%d", which);
+    const long n = (long)g->geo.n_tiles * 4 * g->dR * TILE * (which == HIREP_FULL ? 2 : 1);
+    return kern_result(g, k_g5_lincomb(g->prec, n, g->dR, xi, c0, 1, c1, c2, eta, g->stream), "hirep_spinor_g5_lc_add_assign");
 }
 
 extern "C" int hirep_Dphi_tm(hirep_geom *g, double m0, double mu, void *out_full, const void *in_full, const void *links) {
@@ -418,6 +427,11 @@ extern "C" int hirep_spinor_prod(hirep_geom *g, int which, const void *xi, const
     CHECK_PTRS("hirep_spinor_prod", xi, eta);
     if (!out) return fail(HIREP_EINVAL, "hirep_spinor_prod: NULL result pointer");
     return reduce_prod(g, which, 0, xi, eta, out, "hirep_spinor_prod");
+}
+extern "C" int hirep_spinor_g5_prod(hirep_geom *g, int which, const void *xi, const void *eta, double out[2]) {
+    CHECK_PTRS("hirep_spinor_g5_prod", xi, eta);
+    if (!out) return fail(HIREP_EINVAL, "hirep_spinor_g5_prod: NULL result pointer");
+    return reduce_prod(g, which, 2, xi, eta, out, "hirep_spinor_g5_prod");
 }
 extern "C" int hirep_spinor_sqnorm(hirep_geom *g, int which, const void *xi, double *out) {
     CHECK_PTRS("hirep_spinor_sqnorm", xi);

@@ -143,19 +143,25 @@ __global__ void __launch_bounds__(256) lincomb_kernel(long n, cplx<T> *__restric
 // ---- xi = c1*eta + c2*gamma_5*eta: the factor is c1 + c2 on the upper two spin components, c1 - c2 on the lower two
 template <typename T>
 __global__ void __launch_bounds__(256) g5_lincomb_kernel(long n, int ncomp, cplx<T> *__restrict__ xi, const cplx<T> *__restrict__ eta,
-                                                         double2 cu, double2 cl) {
-    const T ux = (T)cu.x, uy = (T)cu.y, lx = (T)cl.x, ly = (T)cl.y;
+                                                         double2 cu, double2 cl, double2 c0, int use_xi) {
+    const T ux = (T)cu.x, uy = (T)cu.y, lx = (T)cl.x, ly = (T)cl.y, c0x = (T)c0.x, c0y = (T)c0.y;
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
         const int comp = (int)((i >> 5) % ncomp);          // row = (half, tile, component)
         const bool lower = 2 * comp >= ncomp;
         const T cx = lower ? lx : ux, cy = lower ? ly : uy;
         const cplx<T> e = eta[i];
-        xi[i] = mk<T>(cx * e.x - cy * e.y, cx * e.y + cy * e.x);
+        T re = cx * e.x - cy * e.y, im = cx * e.y + cy * e.x;
+        if (use_xi) {   // add-(mul-)assign forms (L447): xi <- c0 xi + c1 eta + c2 gamma_5 eta
+            const cplx<T> x = xi[i];
+            re += c0x * x.x - c0y * x.y;
+            im += c0x * x.y + c0y * x.x;
+        }
+        xi[i] = mk<T>(re, im);
     }
 }
 
 // ---- partial reductions: one Acc pair (or quadruple) per block -------------------------------------------------
-// mode 0: <xi,eta> (re, im)   mode 1: ||xi||^2 (re only)
+// mode 0: <xi,eta> (re, im)   mode 1: ||xi||^2 (re only)   mode 2: <xi, gamma_5 eta> (the fused reduction of L447)
 template <typename T, int MODE>
 __global__ void __launch_bounds__(RED_THREADS) prod_partial_kernel(Pad P, long n, int alg, const cplx<T> *__restrict__ xi,
                                                                    const cplx<T> *__restrict__ eta, Acc *__restrict__ partial) {
@@ -169,7 +175,8 @@ __global__ void __launch_bounds__(RED_THREADS) prod_partial_kernel(Pad P, long n
             acc_add(a[0], __dmul_rn(xm, xm), alg);
         } else {
             const cplx<T> e = eta[i];
-            const double er = (double)e.x, em = (double)e.y;
+            double er = (double)e.x, em = (double)e.y;
+            if (MODE == 2 && 2 * (int)((i >> 5) % P.ncomp) >= P.ncomp) { er = -er; em = -em; }   // lower spin components
             acc_add(a[0], __dmul_rn(xr, er), alg);
             acc_add(a[0], __dmul_rn(xm, em), alg);
             acc_add(a[1], __dmul_rn(xr, em), alg);
@@ -296,11 +303,13 @@ int k_lincomb(int prec, long n, void *xi, const double c0[2], int use_xi, const 
                      : lincomb_t<float>(n, xi, a, use_xi, eta, b, zeta, c, use_zeta, s);
 }
 
-int k_g5_lincomb(int prec, long n, int dR, void *xi, const double c1[2], const double c2[2], const void *eta, cudaStream_t s) {
+int k_g5_lincomb(int prec, long n, int dR, void *xi, const double c0[2], int use_xi, const double c1[2], const double c2[2], const void *eta,
+                 cudaStream_t s) {
     const double2 cu = make_double2(c1[0] + c2[0], c1[1] + c2[1]), cl = make_double2(c1[0] - c2[0], c1[1] - c2[1]);
+    const double2 cx = make_double2(c0[0], c0[1]);
     const int nb = blocks_for(n);
-    if (prec == 0) g5_lincomb_kernel<double><<<nb, 256, 0, s>>>(n, 4 * dR, (double2 *)xi, (const double2 *)eta, cu, cl);
-    else g5_lincomb_kernel<float><<<nb, 256, 0, s>>>(n, 4 * dR, (float2 *)xi, (const float2 *)eta, cu, cl);
+    if (prec == 0) g5_lincomb_kernel<double><<<nb, 256, 0, s>>>(n, 4 * dR, (double2 *)xi, (const double2 *)eta, cu, cl, cx, use_xi);
+    else g5_lincomb_kernel<float><<<nb, 256, 0, s>>>(n, 4 * dR, (float2 *)xi, (const float2 *)eta, cu, cl, cx, use_xi);
     return (int)cudaGetLastError();
 }
 
@@ -313,9 +322,11 @@ int k_prod(const Geo &g, int prec, int dR, int halves, int mode, int alg, const 
     Acc *partial = (Acc *)ws;
     if (prec == 0) {
         if (mode == 0) prod_partial_kernel<double, 0><<<nb, RED_THREADS, 0, s>>>(P, n, alg, (const double2 *)xi, (const double2 *)eta, partial);
+        else if (mode == 2) prod_partial_kernel<double, 2><<<nb, RED_THREADS, 0, s>>>(P, n, alg, (const double2 *)xi, (const double2 *)eta, partial);
         else prod_partial_kernel<double, 1><<<nb, RED_THREADS, 0, s>>>(P, n, alg, (const double2 *)xi, (const double2 *)eta, partial);
     } else {
         if (mode == 0) prod_partial_kernel<float, 0><<<nb, RED_THREADS, 0, s>>>(P, n, alg, (const float2 *)xi, (const float2 *)eta, partial);
+        else if (mode == 2) prod_partial_kernel<float, 2><<<nb, RED_THREADS, 0, s>>>(P, n, alg, (const float2 *)xi, (const float2 *)eta, partial);
         else prod_partial_kernel<float, 1><<<nb, RED_THREADS, 0, s>>>(P, n, alg, (const float2 *)xi, (const float2 *)eta, partial);
     }
     reduce_final_kernel<<<1, RED_THREADS, 0, s>>>(nb, alg, partial, out_dev);

@@ -87,3 +87,24 @@ def test_twisted_mass_cg(env):
     assert np.linalg.norm((b - A(x)).ravel()) < 1e-9 * np.linalg.norm(b.ravel())
     _, it0, _ = p.geom.cg_g5Dphi_sq(m0, p.to_native(b, hirep.FULL), p.links_rep, 1e-10, 3000)
     assert it < it0
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_g5_fused_forms(env, prec):
+    """The gamma_5 add-mul-assign form and the fused reduction <xi, gamma_5 eta> against the oracle
+    composition g5() + lc / prod."""
+    from oracle import linalg as la
+    hirep, oracle = env["hirep"], env["oracle"]
+    p = Problem(env, synth.CONFIGS["C3"].resized(4, 6), prec, n_spinors=2)
+    xi0, eta0 = p.spinors
+    for w, sel in ((hirep.FULL, slice(None)), (hirep.ODD, p.od)):
+        a, b = xi0[sel], eta0[sel]
+        c0, c1, c2 = 0.5 + 0.25j, -1.5j, 2.0 - 1.0j
+        xi, e = p.to_native(a, w), p.to_native(b, w)
+        p.geom.g5_lc_add_assign(w, xi, c0, c1, c2, e)
+        assert oracle.rel_l2(p.to_numpy(xi, w), c0 * a + oracle.g5_lc(c1, c2, b)) < TOL[prec]
+        got = p.geom.g5_prod(w, p.to_native(a, w), e)
+        ref = la.prod(a, oracle.g5(b))
+        mag = float(np.sum(np.abs(a) * np.abs(b))) * 2
+        assert abs(got - ref) <= 8 * 2.0 ** -52 * mag
+        assert abs(got - ref) <= 1e-12 * mag
