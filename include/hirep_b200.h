@@ -177,6 +177,8 @@ int hirep_cg_g5Dphi_hat_sq(hirep_geom *g, double m0, void *x_even, const void *b
  *   hirep_Dphi_tm_sq    out = (D^tm)^dagger D^tm in = gamma_5 D^tm(-mu) gamma_5 D^tm(mu) in   (Hermitian positive definite)
  *   hirep_Dphi_tm_hat   out_even = D_ee in_even - D_eo D_oo^{-1} D_oe in_even, D_ee = D_oo = (4+m) + i mu gamma_5  (Eq 43) */
 int hirep_spinor_g5_lc(hirep_geom *g, int which, void *xi, const double c1[2], const double c2[2], const void *eta);
+/* gamma matrix application (Eq 34): xi = gamma_mu eta, mu = 0..3 in the basis of Eq 1-3, mu = 5 for gamma_5; xi != eta */
+int hirep_spinor_gamma(hirep_geom *g, int which, int mu, void *xi, const void *eta);
 /* the add-assign / add-mul-assign forms (L447): xi <- c0 xi + c1 eta + c2 gamma_5 eta */
 int hirep_spinor_g5_lc_add_assign(hirep_geom *g, int which, void *xi, const double c0[2], const double c1[2], const double c2[2], const void *eta);
 /* the fused reduction <xi, gamma_5 eta> (L447): out = {Re, Im}, host doubles, compensated like hirep_spinor_prod */

@@ -312,6 +312,13 @@ extern "C" int hirep_spinor_g5_lc(hirep_geom *g, int which, void *xi, const doub
     static const double zero2[2] = {0.0, 0.0};
     return kern_result(g, k_g5_lincomb(g->prec, n, g->dR, xi, zero2, 0, c1, c2, eta, g->stream), "hirep_spinor_g5_lc");
 }
+extern "C" int hirep_spinor_gamma(hirep_geom *g, int which, int mu, void *xi, const void *eta) {
+    CHECK_PTRS("hirep_spinor_gamma", xi, eta);
+    if (which < 0 || which > 2) return fail(HIREP_EINVAL, "hirep_spinor_gamma: parity_or_full=%d", which);
+    if (!((mu >= 0 && mu <= 3) || mu == 5)) return fail(HIREP_EINVAL, "hirep_spinor_gamma: mu=%d (0..3 or 5)", mu);
+    if (xi == eta) return fail(HIREP_EINVAL, "hirep_spinor_gamma: xi aliases eta");
+    return kern_result(g, k_gamma(g->geo, g->prec, g->dR, which == HIREP_FULL ? 2 : 1, mu, xi, eta, g->stream), "hirep_spinor_gamma");
+}
 extern "C" int hirep_spinor_g5_lc_add_assign(hirep_geom *g, int which, void *xi, const double c0[2], const double c1[2], const double c2[2],
                                              const void *eta) {
     CHECK_PTRS("hirep_spinor_g5_lc_add_assign", xi, eta);

@@ -36,6 +36,7 @@ int k_hop(const Geo &g, int prec, int N, int rep, int mode, int variant, const H
 int k_reduce_workspace_bytes();
 int k_lincomb(int prec, long n, void *xi, const double c0[2], int use_xi, const void *eta, const double c1[2], const void *zeta,
               const double c2[2], int use_zeta, cudaStream_t s);
+int k_gamma(const Geo &g, int prec, int dR, int halves, int mu, void *xi, const void *eta, cudaStream_t s);
 int k_g5_lincomb(int prec, long n, int dR, void *xi, const double c0[2], int use_xi, const double c1[2], const double c2[2], const void *eta,
                  cudaStream_t s);
 int k_prod(const Geo &g, int prec, int dR, int halves, int mode, int alg, const void *xi, const void *eta, void *ws, double *out_dev, cudaStream_t s);

@@ -160,6 +160,34 @@ __global__ void __launch_bounds__(256) g5_lincomb_kernel(long n, int ncomp, cplx
     }
 }
 
+// ---- xi = gamma_mu eta (Eq 34), gamma_mu = [[0, e_mu], [e_mu^dagger, 0]] in the basis of Eq 1-3 (L171-182):
+// e_0 = -1, e_k = -i sigma_k.  One thread per (site, colour): the four spin components of that colour.  mu = 5: gamma_5.
+template <typename T>
+__global__ void __launch_bounds__(256) gamma_kernel(long nrows32, int dR, int mu, cplx<T> *__restrict__ xi, const cplx<T> *__restrict__ eta) {
+    // element (tile-row block, colour c, lane): components at ((tile*4*dR) + s*dR + c)*32 + lane, s = 0..3
+    const long total = nrows32 * dR * TILE;   // nrows32 = number of tiles (halves included)
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
+        const int lane = (int)(i & (TILE - 1));
+        const long tc = i >> 5;
+        const int c = (int)(tc % dR);
+        const long tile = tc / dR;
+        const size_t base = ((size_t)tile * 4 * dR + c) * TILE + lane, st = (size_t)dR * TILE;
+        const cplx<T> a0 = eta[base], a1 = eta[base + st], a2 = eta[base + 2 * st], a3 = eta[base + 3 * st];
+        cplx<T> o0, o1, o2, o3;
+        auto neg = [](cplx<T> z) { return mk<T>(-z.x, -z.y); };
+        auto muli = [](cplx<T> z) { return mk<T>(-z.y, z.x); };      // i z
+        auto mulmi = [](cplx<T> z) { return mk<T>(z.y, -z.x); };     // -i z
+        switch (mu) {
+        case 0: o0 = neg(a2); o1 = neg(a3); o2 = neg(a0); o3 = neg(a1); break;                  // e_0 = -1
+        case 1: o0 = mulmi(a3); o1 = mulmi(a2); o2 = muli(a1); o3 = muli(a0); break;             // e_1 = -i sigma_1
+        case 2: o0 = neg(a3); o1 = a2; o2 = a1; o3 = neg(a0); break;                             // e_2 = -i sigma_2 = [[0,-1],[1,0]]
+        case 3: o0 = mulmi(a2); o1 = muli(a3); o2 = muli(a0); o3 = mulmi(a1); break;             // e_3 = -i sigma_3
+        default: o0 = a0; o1 = a1; o2 = neg(a2); o3 = neg(a3); break;                            // gamma_5
+        }
+        xi[base] = o0; xi[base + st] = o1; xi[base + 2 * st] = o2; xi[base + 3 * st] = o3;
+    }
+}
+
 // ---- partial reductions: one Acc pair (or quadruple) per block -------------------------------------------------
 // mode 0: <xi,eta> (re, im)   mode 1: ||xi||^2 (re only)   mode 2: <xi, gamma_5 eta> (the fused reduction of L447)
 template <typename T, int MODE>
@@ -301,6 +329,14 @@ int k_lincomb(int prec, long n, void *xi, const double c0[2], int use_xi, const 
     const double2 a = make_double2(c0[0], c0[1]), b = make_double2(c1[0], c1[1]), c = make_double2(c2[0], c2[1]);
     return prec == 0 ? lincomb_t<double>(n, xi, a, use_xi, eta, b, zeta, c, use_zeta, s)
                      : lincomb_t<float>(n, xi, a, use_xi, eta, b, zeta, c, use_zeta, s);
+}
+
+int k_gamma(const Geo &g, int prec, int dR, int halves, int mu, void *xi, const void *eta, cudaStream_t s) {
+    const long tiles = (long)g.n_tiles * halves;
+    const int nb = blocks_for(tiles * dR * TILE);
+    if (prec == 0) gamma_kernel<double><<<nb, 256, 0, s>>>(tiles, dR, mu, (double2 *)xi, (const double2 *)eta);
+    else gamma_kernel<float><<<nb, 256, 0, s>>>(tiles, dR, mu, (float2 *)xi, (const float2 *)eta);
+    return (int)cudaGetLastError();
 }
 
 int k_g5_lincomb(int prec, long n, int dR, void *xi, const double c0[2], int use_xi, const double c1[2], const double c2[2], const void *eta,

@@ -30,7 +30,7 @@ SYMBOLS = [
     "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_g5Dphi_hat", "hirep_g5Dphi_hat_sq", "hirep_cg_g5Dphi_hat_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_set_tuning", "hirep_launch_count",
     "hirep_apply_host", "hirep_spinor_lc", "hirep_spinor_clc", "hirep_spinor_lc_add_assign", "hirep_spinor_clc_add_assign",
     "hirep_spinor_lc1", "hirep_spinor_lc2", "hirep_spinor_lc3", "hirep_spinor_prod", "hirep_spinor_sqnorm",
-    "hirep_spinor_max_norm", "hirep_cg_g5Dphi_sq", "hirep_spinor_g5_lc", "hirep_spinor_g5_lc_add_assign", "hirep_spinor_g5_prod", "hirep_Dphi_tm", "hirep_Dphi_tm_sq",
+    "hirep_spinor_max_norm", "hirep_cg_g5Dphi_sq", "hirep_spinor_g5_lc", "hirep_spinor_gamma", "hirep_spinor_g5_lc_add_assign", "hirep_spinor_g5_prod", "hirep_Dphi_tm", "hirep_Dphi_tm_sq",
     "hirep_Dphi_tm_hat", "hirep_cg_Dphi_tm_sq", "hirep_cg_mshift_g5Dphi_sq", "hirep_bicgstab", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
 ]
 
@@ -88,6 +88,7 @@ def load():
     lib.hirep_cg_g5Dphi_sq.argtypes = [vp, cd, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_cg_g5Dphi_hat_sq.argtypes = [vp, cd, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_spinor_g5_lc.argtypes = [vp, ci, vp, c2p, c2p, vp]
+    lib.hirep_spinor_gamma.argtypes = [vp, ci, ci, vp, vp]
     lib.hirep_spinor_g5_lc_add_assign.argtypes = [vp, ci, vp, c2p, c2p, c2p, vp]
     lib.hirep_spinor_g5_prod.argtypes = [vp, ci, vp, vp, c2p]
     for n in ("hirep_Dphi_tm", "hirep_Dphi_tm_sq", "hirep_Dphi_tm_hat"):
@@ -197,6 +198,9 @@ def hirep_cg_g5Dphi_sq(g, m0, x, b, links, tol, maxiter):
 
 
 def hirep_spinor_g5_lc(g, which, xi, c1, c2, eta): _check(load().hirep_spinor_g5_lc(g, which, xi, _c2(c1), _c2(c2), eta))
+def hirep_spinor_gamma(g, which, mu, xi, eta): _check(load().hirep_spinor_gamma(g, which, mu, xi, eta))
+
+
 def hirep_spinor_g5_lc_add_assign(g, which, xi, c0, c1, c2, eta):
     _check(load().hirep_spinor_g5_lc_add_assign(g, which, xi, _c2(c0), _c2(c1), _c2(c2), eta))
 
@@ -395,6 +399,7 @@ class Geometry:
     def g5_lc(self, which, xi, c1, c2, eta): hirep_spinor_g5_lc(self.handle, which, xi.data_ptr(), c1, c2, eta.data_ptr())
 
     def g5_lc_add_assign(self, which, xi, c0, c1, c2, eta): hirep_spinor_g5_lc_add_assign(self.handle, which, xi.data_ptr(), c0, c1, c2, eta.data_ptr())
+    def gamma(self, which, mu, xi, eta): hirep_spinor_gamma(self.handle, which, mu, xi.data_ptr(), eta.data_ptr())
     def g5_prod(self, which, xi, eta): return hirep_spinor_g5_prod(self.handle, which, xi.data_ptr(), eta.data_ptr())
 
     def Dphi_tm(self, m0, mu, inp, links, out=None):

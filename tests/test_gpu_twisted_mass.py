@@ -108,3 +108,22 @@ def test_g5_fused_forms(env, prec):
         mag = float(np.sum(np.abs(a) * np.abs(b))) * 2
         assert abs(got - ref) <= 8 * 2.0 ** -52 * mag
         assert abs(got - ref) <= 1e-12 * mag
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_gamma_matrix_application(env, prec):
+    """Eq 34: xi = gamma_mu eta against the oracle's 4x4 gamma matrices (Eq 1-3); sign flips and factors of i only,
+    so the result is bit exact.  Ragged lattice, every extent selector."""
+    hirep, oracle = env["hirep"], env["oracle"]
+    p = Problem(env, synth.CONFIGS["C4"].resized(2, 6), prec)
+    gam = {mu: oracle.gamma()[mu] for mu in range(4)}
+    gam[5] = oracle.gamma5()
+    for w, sel in ((hirep.FULL, slice(None)), (hirep.EVEN, p.ev), (hirep.ODD, p.od)):
+        eta = p.spinors[0][sel]
+        e = p.to_native(eta, w)
+        for mu in (0, 1, 2, 3, 5):
+            xi = p.geom.new_spinor(w)
+            p.geom.gamma(w, mu, xi, e)
+            assert np.array_equal(p.to_numpy(xi, w), np.einsum("ab,xbi->xai", gam[mu], eta)), mu
+    with pytest.raises(hirep.HirepError):
+        p.geom.gamma(hirep.FULL, 4, p.geom.new_spinor(hirep.FULL), p.to_native(p.spinors[0], hirep.FULL))
