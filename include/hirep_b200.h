@@ -127,6 +127,10 @@ long hirep_launch_count(const hirep_geom *g);
  * links, applies `op` (HIREP_OP_*), exports and copies the result back to `out`; returns after the result is in
  * host memory.  Spinor extents follow the op (half lattice for EO/OE/HAT, full otherwise). */
 int hirep_apply_host(hirep_geom *g, int op, double m0, void *out_host, const void *in_host, const void *links_fund_host);
+/* The same without the final wait: returns once everything is enqueued; results are in host memory after hirep_sync.
+ * Consecutive calls pipeline: the device -> host copy of one call overlaps the host -> device copy and kernels of the
+ * next (pinned host buffers needed for the copies to be asynchronous; in_host must stay valid until hirep_sync). */
+int hirep_apply_host_async(hirep_geom *g, int op, double m0, void *out_host, const void *in_host, const void *links_fund_host);
 
 /* ---- spinor linear algebra, reductions and the CG inverter (Sect. 4.2 / 5.1; the consumer of the hot path) ----
  * Native spinor buffers (device pointers); `which` in {HIREP_EVEN, HIREP_ODD, HIREP_FULL} gives their extent.

@@ -28,7 +28,10 @@ struct hirep_geom {
     void *ms_p[HIREP_MAX_SHIFTS];    // multi-shift CG direction fields (lazy)
     void *bi_s, *bi_t;              // BiCGstab work fields (lazy)
     // hirep_apply_host staging (lazy)
-    void *h_links_canon, *h_links_fund, *h_links_rep, *h_in_canon, *h_in_native, *h_out_native, *h_out_canon;
+    void *h_links_canon, *h_links_fund, *h_links_rep, *h_in_canon, *h_in_native, *h_out_native, *h_out_canon, *h_out_canon2;
+    cudaStream_t copy_stream;       // device -> host copies of hirep_apply_host[_async] (lazy)
+    cudaEvent_t ev_done[2], ev_copied[2];
+    int host_slot, host_events;
     int host_links_ready;
     long launches;
     size_t bytes_spinor_half, bytes_links_fund, bytes_links_rep;
@@ -100,7 +103,11 @@ extern "C" int hirep_geom_destroy(hirep_geom *g) {
     for (void *b : g->ms_p)
         if (b) cudaFree(b);
     void *bufs[] = {g->ws_half, g->ws_half2, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
-                    g->h_in_native, g->h_out_native, g->h_out_canon};
+                    g->h_in_native, g->h_out_native, g->h_out_canon, g->h_out_canon2};
+    if (g->host_events) {
+        for (int i = 0; i < 2; ++i) { cudaEventDestroy(g->ev_done[i]); cudaEventDestroy(g->ev_copied[i]); }
+        cudaStreamDestroy(g->copy_stream);
+    }
     for (void *b : bufs)
         if (b) cudaFree(b);
     delete g;
@@ -668,6 +675,7 @@ extern "C" int hirep_fma_peak(int prec, double *tflops) {
 extern "C" int hirep_sync(hirep_geom *g) {
     if (!g) return fail(HIREP_EINVAL, "hirep_sync: NULL geometry");
     cudaError_t e = cudaStreamSynchronize(g->stream);
+    if (e == cudaSuccess && g->host_events) e = cudaStreamSynchronize(g->copy_stream);
     if (e != cudaSuccess) return cuda_fail(e, "hirep_sync");
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "hirep_sync (deferred)");
@@ -675,7 +683,7 @@ extern "C" int hirep_sync(hirep_geom *g) {
 }
 
 // ---- end-to-end host entry -------------------------------------------------------------------------
-extern "C" int hirep_apply_host(hirep_geom *g, int op, double m0, void *out_host, const void *in_host, const void *links_fund_host) {
+static int apply_host_impl(hirep_geom *g, int op, double m0, void *out_host, const void *in_host, const void *links_fund_host, bool async) {
     if (!g || !out_host || !in_host) return fail(HIREP_EINVAL, "hirep_apply_host: NULL argument");
     if (op < HIREP_OP_DPHI || op > HIREP_OP_G5DPHI_SQ) return fail(HIREP_EINVAL, "hirep_apply_host: unknown op %d", op);
     const bool full = (op == HIREP_OP_DPHI || op == HIREP_OP_G5DPHI_SQ);
@@ -689,6 +697,17 @@ extern "C" int hirep_apply_host(hirep_geom *g, int op, double m0, void *out_host
     if ((rc = workspace(&g->h_links_rep, g->bytes_links_rep))) return rc;
     if ((rc = workspace(&g->h_in_canon, V * 4 * g->dR * 2 * w))) return rc;
     if ((rc = workspace(&g->h_out_canon, V * 4 * g->dR * 2 * w))) return rc;
+    if ((rc = workspace(&g->h_out_canon2, V * 4 * g->dR * 2 * w))) return rc;
+    if (!g->host_events) {
+        cudaError_t ce = cudaStreamCreateWithFlags(&g->copy_stream, cudaStreamNonBlocking);
+        for (int i = 0; i < 2 && ce == cudaSuccess; ++i) {
+            ce = cudaEventCreateWithFlags(&g->ev_done[i], cudaEventDisableTiming);
+            if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&g->ev_copied[i], cudaEventDisableTiming);
+            if (ce == cudaSuccess) ce = cudaEventRecord(g->ev_copied[i], g->copy_stream);   // "slot free"
+        }
+        if (ce != cudaSuccess) return cuda_fail(ce, "hirep_apply_host: stream/event setup");
+        g->host_events = 1;
+    }
     if ((rc = workspace(&g->h_in_native, 2 * g->bytes_spinor_half))) return rc;
     if ((rc = workspace(&g->h_out_native, 2 * g->bytes_spinor_half))) return rc;
     cudaError_t e;
@@ -715,9 +734,27 @@ extern "C" int hirep_apply_host(hirep_geom *g, int op, double m0, void *out_host
     default: rc = hirep_g5Dphi_sq(g, m0, g->h_out_native, g->h_in_native, links); break;
     }
     if (rc) return rc;
-    if ((rc = hirep_spinor_export(g, g->h_out_canon, g->h_out_native, out_which))) return rc;
-    e = cudaMemcpyAsync(out_host, g->h_out_canon, canon_sp, cudaMemcpyDeviceToHost, g->stream);
+    // the result goes home on a second stream from one of two staging buffers, so that the device -> host copy of this
+    // call overlaps the host -> device copy and the kernels of the next one (PCIe is full duplex)
+    const int slot = g->host_slot;
+    g->host_slot ^= 1;
+    void *stage = slot ? g->h_out_canon2 : g->h_out_canon;
+    e = cudaStreamWaitEvent(g->stream, g->ev_copied[slot], 0);          // the buffer's previous copy has left
+    if (e != cudaSuccess) return cuda_fail(e, "hirep_apply_host: wait for staging buffer");
+    if ((rc = hirep_spinor_export(g, stage, g->h_out_native, out_which))) return rc;
+    e = cudaEventRecord(g->ev_done[slot], g->stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(g->copy_stream, g->ev_done[slot], 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out_host, stage, canon_sp, cudaMemcpyDeviceToHost, g->copy_stream);
+    if (e == cudaSuccess) e = cudaEventRecord(g->ev_copied[slot], g->copy_stream);
     if (e != cudaSuccess) return cuda_fail(e, "hirep_apply_host: result D2H");
     (void)native_sp;
+    if (async) return HIREP_OK;
     return hirep_sync(g);
+}
+
+extern "C" int hirep_apply_host(hirep_geom *g, int op, double m0, void *out_host, const void *in_host, const void *links_fund_host) {
+    return apply_host_impl(g, op, m0, out_host, in_host, links_fund_host, false);
+}
+extern "C" int hirep_apply_host_async(hirep_geom *g, int op, double m0, void *out_host, const void *in_host, const void *links_fund_host) {
+    return apply_host_impl(g, op, m0, out_host, in_host, links_fund_host, true);
 }

@@ -28,7 +28,7 @@ SYMBOLS = [
     "hirep_spinor_import", "hirep_spinor_export", "hirep_links_import", "hirep_links_rep_export",
     "hirep_links_rep_export_bwd", "hirep_links_to_rep", "hirep_Dphi", "hirep_Dphi_eo", "hirep_Dphi_oe",
     "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_g5Dphi_hat", "hirep_g5Dphi_hat_sq", "hirep_cg_g5Dphi_hat_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_set_tuning", "hirep_launch_count",
-    "hirep_apply_host", "hirep_spinor_lc", "hirep_spinor_clc", "hirep_spinor_lc_add_assign", "hirep_spinor_clc_add_assign",
+    "hirep_apply_host", "hirep_apply_host_async", "hirep_spinor_lc", "hirep_spinor_clc", "hirep_spinor_lc_add_assign", "hirep_spinor_clc_add_assign",
     "hirep_spinor_lc1", "hirep_spinor_lc2", "hirep_spinor_lc3", "hirep_spinor_prod", "hirep_spinor_sqnorm",
     "hirep_spinor_max_norm", "hirep_cg_g5Dphi_sq", "hirep_spinor_g5_lc", "hirep_spinor_gamma", "hirep_spinor_g5_lc_add_assign", "hirep_spinor_g5_prod", "hirep_Dphi_tm", "hirep_Dphi_tm_sq",
     "hirep_Dphi_tm_hat", "hirep_cg_Dphi_tm_sq", "hirep_cg_mshift_g5Dphi_sq", "hirep_bicgstab", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
@@ -75,6 +75,7 @@ def load():
     lib.hirep_launch_count.argtypes = [vp]
     lib.hirep_launch_count.restype = ctypes.c_long
     lib.hirep_apply_host.argtypes = [vp, ci, cd, vp, vp, vp]
+    lib.hirep_apply_host_async.argtypes = [vp, ci, cd, vp, vp, vp]
     c2p = ctypes.POINTER(cd)
     for n in ("hirep_spinor_lc", "hirep_spinor_lc_add_assign"):
         getattr(lib, n).argtypes = [vp, ci, vp, cd, vp, cd, vp]
@@ -254,6 +255,10 @@ def hirep_sync(g): _check(load().hirep_sync(g))
 
 def hirep_apply_host(g, op, m0, out_host_ptr, in_host_ptr, links_host_ptr):
     _check(load().hirep_apply_host(g, op, m0, out_host_ptr, in_host_ptr, links_host_ptr))
+
+
+def hirep_apply_host_async(g, op, m0, out_host_ptr, in_host_ptr, links_host_ptr):
+    _check(load().hirep_apply_host_async(g, op, m0, out_host_ptr, in_host_ptr, links_host_ptr))
 
 
 # ---- convenience wrapper ---------------------------------------------------------------------------------

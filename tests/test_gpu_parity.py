@@ -287,6 +287,28 @@ def test_apply_host_end_to_end(env):
     assert oracle.rel_l2(out.numpy(), oracle.Dphi(4, 4, 3, cfg.m0, p.R, psi, BC)) < 1e-13
 
 
+def test_apply_host_async_pipeline(env):
+    """hirep_apply_host_async: several calls in flight (results leave on a second stream from two staging buffers)
+    give, after hirep_sync, bit for bit what the synchronous entry gives."""
+    torch, hirep = env["torch"], env["hirep"]
+    cfg = synth.CONFIGS["C2"].resized(6, 6)
+    p = Problem(env, cfg, "f64")
+    U_h = torch.from_numpy(p.U).pin_memory()
+    psi = p.spinors[0]
+    ins = {"f": torch.from_numpy(psi).pin_memory(), "e": torch.from_numpy(np.ascontiguousarray(psi[p.ev])).pin_memory(),
+           "o": torch.from_numpy(np.ascontiguousarray(psi[p.od])).pin_memory()}
+    seq = [(hirep.OP_DPHI_EO, "o", "e"), (hirep.OP_DPHI_OE, "e", "o"), (hirep.OP_DPHI, "f", "f"), (hirep.OP_DPHI_HAT, "e", "e"),
+           (hirep.OP_G5DPHI_SQ, "f", "f"), (hirep.OP_DPHI_EO, "o", "e"), (hirep.OP_DPHI, "f", "f")]
+    ref = [p.geom.apply_host(op, cfg.m0, ins[i], U_h if k == 0 else None) for k, (op, i, o) in enumerate(seq)]
+    outs = [torch.empty_like(ins[o]).pin_memory() for (_, _, o) in seq]
+    for rep in range(2):
+        for k, (op, i, o) in enumerate(seq):
+            hirep.hirep_apply_host_async(p.geom.handle, op, cfg.m0, outs[k].data_ptr(), ins[i].data_ptr(), U_h.data_ptr() if k == 0 else None)
+        p.geom.sync()
+        for k in range(len(seq)):
+            assert torch.equal(outs[k], ref[k]), (rep, k)
+
+
 # --------------------------------------------------------- full BASELINE sizes, sampled outputs
 def full_size_problem(env, name, prec):
     torch, hirep = env["torch"], env["hirep"]
