@@ -139,6 +139,11 @@ int hirep_apply_host_async(hirep_geom *g, int op, double m0, void *out_host, con
  *   hirep_spinor_clc  xi = c1 eta + c2 zeta            (Eq 23)            hirep_spinor_lc2  xi <- c1 xi + c2 eta       (Eq 25)
  *   *_add_assign      xi <- xi + (the same)            (L387)             hirep_spinor_lc3  xi <- c1 eta + c2 zeta - xi (Eq 26) */
 int hirep_spinor_lc(hirep_geom *g, int which, void *xi, double r1, const void *eta, double r2, const void *zeta);
+/* elementary operations (L365-371): xi = 0 ; xi = eta ; xi = c eta (complex c) ; xi = -eta.  xi may alias eta. */
+int hirep_spinor_zero(hirep_geom *g, int which, void *xi);
+int hirep_spinor_copy(hirep_geom *g, int which, void *xi, const void *eta);
+int hirep_spinor_mul(hirep_geom *g, int which, void *xi, const double c[2], const void *eta);
+int hirep_spinor_minus(hirep_geom *g, int which, void *xi, const void *eta);
 int hirep_spinor_clc(hirep_geom *g, int which, void *xi, const double c1[2], const void *eta, const double c2[2], const void *zeta);
 int hirep_spinor_lc_add_assign(hirep_geom *g, int which, void *xi, double r1, const void *eta, double r2, const void *zeta);
 int hirep_spinor_clc_add_assign(hirep_geom *g, int which, void *xi, const double c1[2], const void *eta, const double c2[2], const void *zeta);

@@ -421,6 +421,29 @@ extern "C" int hirep_spinor_lc3(hirep_geom *g, int which, void *xi, const double
     return lincomb(g, which, xi, MINUS2, 1, eta, c1, zeta, c2, 1, "hirep_spinor_lc3");
 }
 
+// the elementary operations of L365-371: zero, copy, multiplication by a scalar, global minus sign (one streaming
+// kernel each, as the paper prefers over memset/memcpy)
+extern "C" int hirep_spinor_zero(hirep_geom *g, int which, void *xi) {
+    CHECK_PTRS("hirep_spinor_zero", xi);
+    if (which < 0 || which > 2) return fail(HIREP_EINVAL, "hirep_spinor_zero: parity_or_full=%d", which);
+    const cudaError_t e = cudaMemsetAsync(xi, 0, (which == HIREP_FULL ? 2 : 1) * g->bytes_spinor_half, g->stream);   // exact zeros, also over NaNs
+    return e == cudaSuccess ? HIREP_OK : cuda_fail(e, "hirep_spinor_zero");
+}
+extern "C" int hirep_spinor_copy(hirep_geom *g, int which, void *xi, const void *eta) {
+    CHECK_PTRS("hirep_spinor_copy", xi, eta);
+    if (xi == eta) return HIREP_OK;
+    return lincomb(g, which, xi, ZERO2, 0, eta, ONE2, eta, ZERO2, 0, "hirep_spinor_copy");
+}
+extern "C" int hirep_spinor_mul(hirep_geom *g, int which, void *xi, const double c[2], const void *eta) {
+    CHECK_PTRS("hirep_spinor_mul", xi, eta);
+    if (!c) return fail(HIREP_EINVAL, "hirep_spinor_mul: NULL coefficient");
+    return lincomb(g, which, xi, ZERO2, 0, eta, c, eta, ZERO2, 0, "hirep_spinor_mul");
+}
+extern "C" int hirep_spinor_minus(hirep_geom *g, int which, void *xi, const void *eta) {
+    CHECK_PTRS("hirep_spinor_minus", xi, eta);
+    return lincomb(g, which, xi, ZERO2, 0, eta, MINUS2, eta, ZERO2, 0, "hirep_spinor_minus");
+}
+
 static int red_workspace(hirep_geom *g) { return workspace(&g->ws_red, (size_t)k_reduce_workspace_bytes() + 64); }
 static double *red_out(hirep_geom *g) { return (double *)((char *)g->ws_red + k_reduce_workspace_bytes()); }
 static int fetch_result(hirep_geom *g, double *host, int n, const char *what) {

@@ -28,7 +28,8 @@ SYMBOLS = [
     "hirep_spinor_import", "hirep_spinor_export", "hirep_links_import", "hirep_links_rep_export",
     "hirep_links_rep_export_bwd", "hirep_links_to_rep", "hirep_Dphi", "hirep_Dphi_eo", "hirep_Dphi_oe",
     "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_g5Dphi_hat", "hirep_g5Dphi_hat_sq", "hirep_cg_g5Dphi_hat_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_set_tuning", "hirep_launch_count",
-    "hirep_apply_host", "hirep_apply_host_async", "hirep_spinor_lc", "hirep_spinor_clc", "hirep_spinor_lc_add_assign", "hirep_spinor_clc_add_assign",
+    "hirep_apply_host", "hirep_apply_host_async", "hirep_spinor_zero", "hirep_spinor_copy", "hirep_spinor_mul", "hirep_spinor_minus",
+    "hirep_spinor_lc", "hirep_spinor_clc", "hirep_spinor_lc_add_assign", "hirep_spinor_clc_add_assign",
     "hirep_spinor_lc1", "hirep_spinor_lc2", "hirep_spinor_lc3", "hirep_spinor_prod", "hirep_spinor_sqnorm",
     "hirep_spinor_max_norm", "hirep_cg_g5Dphi_sq", "hirep_spinor_g5_lc", "hirep_spinor_gamma", "hirep_spinor_g5_lc_add_assign", "hirep_spinor_g5_prod", "hirep_Dphi_tm", "hirep_Dphi_tm_sq",
     "hirep_Dphi_tm_hat", "hirep_cg_Dphi_tm_sq", "hirep_cg_mshift_g5Dphi_sq", "hirep_bicgstab", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
@@ -81,6 +82,10 @@ def load():
         getattr(lib, n).argtypes = [vp, ci, vp, cd, vp, cd, vp]
     for n in ("hirep_spinor_clc", "hirep_spinor_clc_add_assign", "hirep_spinor_lc3"):
         getattr(lib, n).argtypes = [vp, ci, vp, c2p, vp, c2p, vp]
+    lib.hirep_spinor_zero.argtypes = [vp, ci, vp]
+    lib.hirep_spinor_copy.argtypes = [vp, ci, vp, vp]
+    lib.hirep_spinor_minus.argtypes = [vp, ci, vp, vp]
+    lib.hirep_spinor_mul.argtypes = [vp, ci, vp, c2p, vp]
     lib.hirep_spinor_lc1.argtypes = [vp, ci, vp, c2p, vp]
     lib.hirep_spinor_lc2.argtypes = [vp, ci, vp, c2p, c2p, vp]
     lib.hirep_spinor_prod.argtypes = [vp, ci, vp, vp, c2p]
@@ -165,6 +170,10 @@ def _c2(z):
     return (ctypes.c_double * 2)(z.real, z.imag)
 
 
+def hirep_spinor_zero(g, which, xi): _check(load().hirep_spinor_zero(g, which, xi))
+def hirep_spinor_copy(g, which, xi, eta): _check(load().hirep_spinor_copy(g, which, xi, eta))
+def hirep_spinor_minus(g, which, xi, eta): _check(load().hirep_spinor_minus(g, which, xi, eta))
+def hirep_spinor_mul(g, which, xi, c, eta): _check(load().hirep_spinor_mul(g, which, xi, _c2(c), eta))
 def hirep_spinor_lc(g, which, xi, r1, eta, r2, zeta): _check(load().hirep_spinor_lc(g, which, xi, r1, eta, r2, zeta))
 def hirep_spinor_clc(g, which, xi, c1, eta, c2, zeta): _check(load().hirep_spinor_clc(g, which, xi, _c2(c1), eta, _c2(c2), zeta))
 def hirep_spinor_lc_add_assign(g, which, xi, r1, eta, r2, zeta): _check(load().hirep_spinor_lc_add_assign(g, which, xi, r1, eta, r2, zeta))

@@ -296,3 +296,24 @@ def test_bicgstab(env, prec, op):
     assert np.linalg.norm((b - A(x)).ravel()) < (1e-9 if prec == "f64" else 1e-4) * np.linalg.norm(b.ravel())
     with pytest.raises(hirep.HirepError):
         p.geom.bicgstab(hirep.OP_G5DPHI_SQ, m0, p.to_native(b, w), p.links_rep, tol, 10)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_elementary_operations(env, prec):
+    """zero / copy / multiplication by a scalar / minus on a ragged lattice, also in place."""
+    hirep, oracle = env["hirep"], env["oracle"]
+    p = Problem(env, synth.CONFIGS["C2"].resized(6, 6), prec)
+    h = p.geom.handle
+    for w, sel in ((hirep.FULL, slice(None)), (hirep.EVEN, p.ev)):
+        eta = p.spinors[0][sel]
+        e = p.to_native(eta, w)
+        xi = p.geom.new_spinor(w)
+        xi.fill_(0xFF)                                                  # NaN bit patterns
+        hirep.hirep_spinor_zero(h, w, xi.data_ptr())
+        assert not p.to_numpy(xi, w).any()
+        hirep.hirep_spinor_copy(h, w, xi.data_ptr(), e.data_ptr())
+        assert np.array_equal(p.to_numpy(xi, w), eta)
+        hirep.hirep_spinor_minus(h, w, xi.data_ptr(), xi.data_ptr())    # in place
+        assert np.array_equal(p.to_numpy(xi, w), -eta)
+        hirep.hirep_spinor_mul(h, w, xi.data_ptr(), 0.5 - 2.0j, e.data_ptr())
+        assert oracle.rel_l2(p.to_numpy(xi, w), (0.5 - 2.0j) * eta) < TOL[prec]
