@@ -21,7 +21,7 @@
 
 namespace hirep {
 
-template <typename T, int DR, bool REAL, int R, int TP, int JB, int STAGES> struct RowsCfg {
+template <typename T, int DR, bool REAL, int R, int TP, int JB, int STAGES, bool SELFBUF = false> struct RowsCfg {
     using E = link_elem<T, REAL>;
     static_assert(DR % R == 0 && DR % JB == 0, "row groups and column blocks must divide d_R");
     static constexpr int NG = DR / R, WARPS = NG * TP, NJB = DR / JB;
@@ -29,8 +29,10 @@ template <typename T, int DR, bool REAL, int R, int TP, int JB, int STAGES> stru
     static constexpr uint32_t CHUNK = R * SEG;
     static constexpr uint32_t HBUF = 2 * DR * TILE * sizeof(cplx<T>);  // one half-spinor buffer of one group
     static constexpr size_t RING_BYTES = (size_t)WARPS * STAGES * CHUNK;
-    static constexpr size_t H_OFF = RING_BYTES, BARS_OFF = H_OFF + (size_t)TP * 2 * HBUF;
-    static constexpr size_t SMEM = BARS_OFF + (size_t)WARPS * STAGES * 8;
+    static constexpr uint32_t SELF_BYTES = SELFBUF ? 4 * DR * TILE * sizeof(cplx<T>) : 0;   // the tile's own spinor, per group
+    static constexpr size_t H_OFF = RING_BYTES, SELF_OFF = H_OFF + (size_t)TP * 2 * HBUF;
+    static constexpr size_t BARS_OFF = SELF_OFF + (size_t)TP * SELF_BYTES;
+    static constexpr size_t SMEM = BARS_OFF + (size_t)WARPS * STAGES * 8 + (size_t)TP * 8;
     static_assert(SEG % 16 == 0, "bulk copies move multiples of 16 bytes");
     static_assert(WARPS <= 32 && TP <= 15, "CTA shape");
     static_assert(SMEM <= 227 * 1024, "rings do not fit the 227 KB of shared memory of an sm_100 CTA");
@@ -40,11 +42,11 @@ __device__ __forceinline__ void group_sync(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-template <typename T, int DR, bool REAL, int R, int TP, int JB, int STAGES>
+template <typename T, int DR, bool REAL, int R, int TP, int JB, int STAGES, bool SELFBUF>
 __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const Geo g, const HopLaunch L) {
     using C = cplx<T>;
     using E = link_elem<T, REAL>;
-    using Cfg = RowsCfg<T, DR, REAL, R, TP, JB, STAGES>;
+    using Cfg = RowsCfg<T, DR, REAL, R, TP, JB, STAGES, SELFBUF>;
     constexpr int NC = 4 * DR, NE = DR * DR, NG = Cfg::NG, NJB = Cfg::NJB;
     constexpr int CPT = 8 * NJB;                                       // chunks per tile (per warp)
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -55,11 +57,16 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
     C *hbuf = reinterpret_cast<C *>(smem_raw + Cfg::H_OFF + (size_t)grp * 2 * Cfg::HBUF);
     const uint32_t ring_s = smem_u32(ring);
     const uint32_t bars_s = smem_u32(smem_raw + Cfg::BARS_OFF) + warp * STAGES * 8;
+    const C *selfbuf = reinterpret_cast<const C *>(smem_raw + Cfg::SELF_OFF + (size_t)grp * Cfg::SELF_BYTES);
+    const uint32_t self_s = smem_u32(selfbuf);
+    const uint32_t selfbar_s = smem_u32(smem_raw + Cfg::BARS_OFF) + Cfg::WARPS * STAGES * 8 + grp * 8;
     if (lane == 0) {
         for (int s = 0; s < STAGES; ++s) mbar_init(bars_s + 8 * s, 1);
+        if (SELFBUF && wg == 0) mbar_init(selfbar_s, 1);
         fence_mbar_init();
     }
     __syncwarp();
+    if constexpr (SELFBUF) group_sync(1 + grp, NG * 32);   // the group's self barrier is initialised before anyone waits on it
 
     const bool two = L.nsets == 2;
     const int total_tiles = g.n_tiles * L.nsets;
@@ -158,6 +165,15 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
                 }
             }
             group_sync(1 + grp, NG * 32);   // h of step I complete; buffer (I&1) was last read at step I-2
+            if constexpr (SELFBUF && I == 0) {
+                // every warp of the group has passed the previous tile's epilogue: its self block may be overwritten.
+                // One bulk copy fetches this tile's own spinor (a contiguous block); it is consumed 7 steps later.
+                if (wg == 0 && lane == 0) {
+                    const C *sp = (const C *)(c_set ? L.set[1].self : L.set[0].self) + ((size_t)c_tile * NC) * TILE;
+                    mbar_expect_tx(selfbar_s, Cfg::SELF_BYTES);
+                    bulk_g2s_plain(self_s, sp, Cfg::SELF_BYTES, selfbar_s);
+                }
+            }
             // (a3) rows i0 .. i0+R-1 times both half-spinor components, column block by column block
             C chi[2][R];
 #pragma unroll
@@ -199,11 +215,12 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
             }
         });
 
+        if constexpr (SELFBUF) mbar_wait(selfbar_s, k & 1);
         if (c_active) {
             C *__restrict__ out = (C *)(c_set ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
             const C *self_base = (const C *)(c_set ? L.set[1].self : L.set[0].self);
-            const C *__restrict__ self = self_base + ((size_t)c_tile * NC) * TILE + lane;
-            const bool use_self = (self_base != nullptr) && (L.a != 0.0);
+            const C *__restrict__ self = SELFBUF ? selfbuf + lane : self_base + ((size_t)c_tile * NC) * TILE + lane;
+            const bool use_self = SELFBUF || ((self_base != nullptr) && (L.a != 0.0));
 #pragma unroll
             for (int s = 0; s < 2; ++s)
 #pragma unroll
@@ -230,12 +247,14 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
 
 // shape per instantiation: R rows per warp and TP groups per CTA are given; column block = the largest divisor of d_R
 // with a chunk of at most 13 KB; as many stages (2..4) as fit next to the half-spinor buffers
-template <typename T, int DR, bool REAL, int R, int TP> struct RowsPick {
+template <typename T, int DR, bool REAL, int R, int TP, bool SELFBUF = false> struct RowsPick {
     using E = link_elem<T, REAL>;
     static constexpr int WARPS = (DR / R) * TP;
     static constexpr size_t chunk_of(int c) { return (size_t)R * c * TILE * sizeof(E); }
     static constexpr int stages_of(int c) {
-        const size_t avail = 226 * 1024 - (size_t)TP * 2 * 2 * DR * TILE * sizeof(cplx<T>);
+        const size_t fixed = (size_t)TP * (2 * 2 + (SELFBUF ? 4 : 0)) * DR * TILE * sizeof(cplx<T>) + 8 * TP;
+        if (fixed >= 226 * 1024) return 0;
+        const size_t avail = 226 * 1024 - fixed;
         const int st = (int)(avail / (WARPS * (chunk_of(c) + 8)));
         return st > 4 ? 4 : st;
     }
@@ -247,14 +266,15 @@ template <typename T, int DR, bool REAL, int R, int TP> struct RowsPick {
     }
     static constexpr int JB = pick_jb();
     static constexpr int STAGES = stages_of(JB);
-    static_assert(STAGES >= 2, "row ring needs at least two stages");
+    static constexpr bool FITS = STAGES >= 2;
 };
 
-template <typename T, int DR, bool REAL, int R, int TP>
-int launch_hop_rows(const Geo &g, const HopLaunch &L, cudaStream_t s) {
-    using P = RowsPick<T, DR, REAL, R, TP>;
-    using Cfg = RowsCfg<T, DR, REAL, R, TP, P::JB, P::STAGES>;
-    auto kern = hop_rows_kernel<T, DR, REAL, R, TP, P::JB, P::STAGES>;
+template <typename T, int DR, bool REAL, int R, int TP, bool SELFBUF>
+int launch_hop_rows_cfg(const Geo &g, const HopLaunch &L, cudaStream_t s) {
+    using P = RowsPick<T, DR, REAL, R, TP, SELFBUF>;
+    static_assert(P::FITS, "row ring needs at least two stages");
+    using Cfg = RowsCfg<T, DR, REAL, R, TP, P::JB, P::STAGES, SELFBUF>;
+    auto kern = hop_rows_kernel<T, DR, REAL, R, TP, P::JB, P::STAGES, SELFBUF>;
     static int n_sm = 0;
     if (n_sm == 0) {
         int dev = 0, sms = 0;
@@ -267,6 +287,20 @@ int launch_hop_rows(const Geo &g, const HopLaunch &L, cudaStream_t s) {
     const int grid = ring_grid(n_sm, L.max_ctas, g.n_tiles * L.nsets, TP);
     kern<<<grid, Cfg::WARPS * 32, Cfg::SMEM, s>>>(g, L);
     return (int)cudaGetLastError();
+}
+
+// passes with a diagonal term stage the tile's own spinor through shared memory when it fits next to two ring stages
+// (the epilogue load is otherwise exposed latency -- 45 % of a tile at d_R = 8 in fp32); SU(6) adjoint fp64 does not fit
+// and its tiles are long enough (60 us) not to care
+template <typename T, int DR, bool REAL, int R, int TP>
+int launch_hop_rows(const Geo &g, const HopLaunch &L, cudaStream_t s) {
+    const bool self = (L.a != 0.0) && L.set[0].self != nullptr;
+    using PS = RowsPick<T, DR, REAL, R, TP, true>;
+    using PN = RowsPick<T, DR, REAL, R, TP, false>;
+    if constexpr (PS::FITS && PS::JB == PN::JB) {   // only if the ring keeps its chunk size (SU(6) adjoint fp64 would not)
+        if (self) return launch_hop_rows_cfg<T, DR, REAL, R, TP, true>(g, L, s);
+    }
+    return launch_hop_rows_cfg<T, DR, REAL, R, TP, false>(g, L, s);
 }
 
 }  // namespace hirep
