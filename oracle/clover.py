@@ -1,0 +1,111 @@
+"""Clover term of the Wilson-Dirac operator -- TEST ORACLE (plain numpy, fp64), not part of the product path.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / reference legs may import this module.
+
+What it follows:
+  * Eq 47 (L859):  D_ee,m + D_oo,m = (4+m) + c_sw (i/4) sum_{mu,nu} sigma_{mu nu} F_{mu nu}
+  * Eq 48 (L864):  C_{mu nu}(x) = sum of the four plaquettes that touch x in the (mu,nu) plane
+  * Eq 49 (L869):  F_{mu nu} = (1/8) (C_{mu nu} - C_{mu nu}^dagger)
+  * Eq 13 (L243):  P_{mu nu}(x) = U_mu(x) U_nu(x+mu) U_mu(x+nu)^dagger U_nu(x)^dagger
+  * Eq 3  (L182):  gamma_mu = [[0, e_mu], [e_mu^dagger, 0]]
+
+Readings (A26-A28):
+  A26  Eq 48 as printed adds plaquettes based at four different sites (not gauge covariant, and two of the four run
+       clockwise); it is read as the standard clover: the four plaquette loops in the (mu,nu) plane that pass
+       through x, each written as a closed path that starts and ends at x, all with the orientation of P_{mu nu}(x).
+  A27  Eq 49's second equality repeats Eq 48 and contradicts the first; the first is taken:
+       F = (C - C^dagger)/8, anti-Hermitian.
+  A28  sigma_{mu nu} is not defined in the paper; sigma_{mu nu} = (i/2) [gamma_mu, gamma_nu] (Hermitian) is taken, the
+       sum in Eq 47 runs over all ordered pairs (mu,nu), so the term is Hermitian and commutes with gamma_5.
+  The links are the represented links R(U_mu(x)); boundary signs +-1 cancel in every closed plaquette loop.
+
+Layout: Rlinks [V, 4, d, d] complex, V = T L^3 canonical sites ((t*L + x)*L + y)*L + z; spinors [V, 4, d].
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import dense
+
+
+def _field(T, L, Rlinks):
+    d = Rlinks.shape[-1]
+    return np.asarray(Rlinks, dtype=np.complex128).reshape(T, L, L, L, 4, d, d)
+
+
+def _shift(A, mu, s):
+    """A'(x) = A(x + s mu), periodic."""
+    return np.roll(A, -s, axis=mu)
+
+
+def _dag(A):
+    return np.conj(np.swapaxes(A, -1, -2))
+
+
+def clover_leaves(T, L, Rlinks, mu, nu):
+    """C_{mu nu}(x) (Eq 48, reading A26) as an array [T,L,L,L,d,d]."""
+    U = _field(T, L, Rlinks)
+    Um, Un = U[..., mu, :, :], U[..., nu, :, :]
+    mm = np.matmul
+    # leaf 1: x -> x+mu -> x+mu+nu -> x+nu -> x
+    l1 = mm(mm(Um, _shift(Un, mu, 1)), mm(_dag(_shift(Um, nu, 1)), _dag(Un)))
+    # leaf 2: x -> x+nu -> x-mu+nu -> x-mu -> x
+    Um_m = _shift(Um, mu, -1)                      # U_mu(x-mu)
+    l2 = mm(mm(Un, _dag(_shift(Um_m, nu, 1))), mm(_dag(_shift(Un, mu, -1)), Um_m))
+    # leaf 3: x -> x-mu -> x-mu-nu -> x-nu -> x
+    Un_n = _shift(Un, nu, -1)                      # U_nu(x-nu)
+    l3 = mm(mm(_dag(Um_m), _dag(_shift(Un_n, mu, -1))), mm(_shift(Um_m, nu, -1), Un_n))
+    # leaf 4: x -> x-nu -> x+mu-nu -> x+mu -> x
+    l4 = mm(mm(_dag(Un_n), _shift(Um, nu, -1)), mm(_shift(Un_n, mu, 1), _dag(Um)))
+    return l1 + l2 + l3 + l4
+
+
+def field_strength(T, L, Rlinks, mu, nu):
+    """F_{mu nu}(x) = (C - C^dagger)/8 (Eq 49, reading A27), [T,L,L,L,d,d]."""
+    C = clover_leaves(T, L, Rlinks, mu, nu)
+    return (C - _dag(C)) / 8.0
+
+
+def sigma(mu, nu):
+    """sigma_{mu nu} = (i/2)[gamma_mu, gamma_nu] (reading A28), 4x4."""
+    g = dense.gammas()
+    return 0.5j * (g[mu] @ g[nu] - g[nu] @ g[mu])
+
+
+def clover_term(T, L, Rlinks):
+    """(i/4) sum_{mu,nu} sigma_{mu nu} F_{mu nu}(x) as [V, 4, d, 4, d] (spin, colour, spin', colour')."""
+    d = Rlinks.shape[-1]
+    V = T * L ** 3
+    A = np.zeros((V, 4, d, 4, d), dtype=np.complex128)
+    for mu in range(4):
+        for nu in range(4):
+            if mu == nu:
+                continue
+            F = field_strength(T, L, Rlinks, mu, nu).reshape(V, d, d)
+            A += 0.25j * np.einsum("st,xab->xsatb", sigma(mu, nu), F)
+    return A
+
+
+def Cphi(T, L, m0, csw, Rlinks, psi):
+    """((4+m) + c_sw (i/4) sum sigma F) psi (Eq 47): the diagonal blocks D_ee,m + D_oo,m."""
+    A = clover_term(T, L, Rlinks)
+    psi = np.asarray(psi, dtype=np.complex128)
+    return (4.0 + m0) * psi + csw * np.einsum("xsatb,xtb->xsa", A, psi)
+
+
+def chiral_blocks(T, L, Rlinks):
+    """The two (2d x 2d) Hermitian blocks of the clover term (spin 0,1 and spin 2,3), [V, 2, 2d, 2d]; the
+    off-diagonal chirality blocks vanish because sigma_{mu nu} commutes with gamma_5 (checked in the tests)."""
+    A = clover_term(T, L, Rlinks)
+    V, _, d = A.shape[:3]
+    out = np.zeros((V, 2, 2 * d, 2 * d), dtype=np.complex128)
+    for c in range(2):
+        out[:, c] = A[:, 2 * c:2 * c + 2, :, 2 * c:2 * c + 2, :].reshape(V, 2 * d, 2 * d)
+    return out
+
+
+def Dphi_clover(T, L, m0, csw, Rlinks, psi, bc):
+    """Eq 8 with the diagonal term of Eq 47: hopping term (the C oracle's field loop) + Cphi."""
+    from . import oracle as _o
+    d = Rlinks.shape[-1]
+    return _o.hop_field(T, L, d, Rlinks, psi, bc) + Cphi(T, L, m0, csw, Rlinks, psi)
