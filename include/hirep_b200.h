@@ -196,6 +196,23 @@ int hirep_Dphi_tm(hirep_geom *g, double m0, double mu, void *out_full, const voi
 int hirep_Dphi_tm_sq(hirep_geom *g, double m0, double mu, void *out_full, const void *in_full, const void *links);
 int hirep_Dphi_tm_hat(hirep_geom *g, double m0, double mu, void *out_even, const void *in_even, const void *links);
 
+/* ---- clover term (Eq 47-49, second part) ----
+ *   D_ee,m + D_oo,m = (4+m) + c_sw (i/4) sum_{mu,nu} sigma_{mu nu} F_{mu nu},  F = (C - C^dagger)/8,  C = the four plaquette
+ *   loops through x in the (mu,nu) plane closed at x (readings A26-A28 in DESIGN.md; sigma_{mu nu} = (i/2)[gamma_mu,gamma_nu]).
+ *   The term is block diagonal in chirality; the library keeps per site and chirality c the d_R x d_R blocks H, B of
+ *   A_c = [[H, B], [B^dagger, -H]] in a caller-owned NATIVE buffer of hirep_clover_bytes() bytes (device, 16-byte aligned).
+ *   hirep_clover_field   clover <- from the STORED represented links of hirep_links_to_rep (boundary signs cancel in the
+ *                        closed loops); once per gauge update.  HIREP_EINVAL in HIREP_LINKS_REBUILD mode.
+ *   hirep_clover_export  canonical_out[V][2][2 d_R][2 d_R] complex (device; site index as the canonical spinor): A_0, A_1.
+ *   hirep_Cphi           out_full = ((4+m) + c_sw A) in_full           (the diagonal blocks of Eq 41 with Eq 47); out != in
+ *   hirep_Dphi_clover    out_full = D_m in_full with that diagonal term (Eq 8 + Eq 47): Cphi, then the hopping pass adds
+ *                        -1/2 hop(in) onto it in place; out != in; `links` as for hirep_Dphi (current link mode). */
+int hirep_clover_bytes(const hirep_geom *g, size_t *bytes);
+int hirep_clover_field(hirep_geom *g, void *clover, const void *links_rep);
+int hirep_clover_export(hirep_geom *g, void *canonical_out, const void *clover);
+int hirep_Cphi(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *clover);
+int hirep_Dphi_clover(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *links, const void *clover);
+
 /* Measurement utility: achieved TFLOP/s (2 flops per FMA) of a register-resident chain of
  * FMAs in the given precision on the current device, the ALU roofline the pipe utilisation is read against.
  * Synchronous; tflops is a host pointer. */

@@ -374,6 +374,47 @@ extern "C" int hirep_Dphi_tm_hat(hirep_geom *g, double m0, double mu, void *out_
     return hop(g, L, "hirep_Dphi_tm_hat (D_eo pass)");
 }
 
+// ---- clover term (Eq 47-49): SURVEY.md 8(f) NEXT-2, second part ----------------------------------------
+static size_t clover_bytes(const hirep_geom *g) {
+    return (size_t)2 * g->geo.n_tiles * 4 * g->dR * g->dR * TILE * 2 * (g->prec == HIREP_F64 ? 8 : 4);
+}
+extern "C" int hirep_clover_bytes(const hirep_geom *g, size_t *bytes) {
+    if (!g || !bytes) return fail(HIREP_EINVAL, "hirep_clover_bytes: NULL argument");
+    *bytes = clover_bytes(g);
+    return HIREP_OK;
+}
+extern "C" int hirep_clover_field(hirep_geom *g, void *clover, const void *links_rep) {
+    CHECK_PTRS("hirep_clover_field", clover, links_rep);
+    if (g->mode != HIREP_LINKS_STORED) return fail(HIREP_EINVAL, "hirep_clover_field: needs the stored represented links (HIREP_LINKS_STORED)");
+    const int nl = 1 + (g->geo.Nh % TILE ? 1 : 0);
+    return kern_result(g, k_clover_field(g->geo, g->prec, g->dR, g->real, clover, links_rep, g->stream), "hirep_clover_field", nl);
+}
+extern "C" int hirep_clover_export(hirep_geom *g, void *canonical_out, const void *clover) {
+    CHECK_PTRS("hirep_clover_export", canonical_out, clover);
+    return kern_result(g, k_clover_export(g->geo, g->prec, g->dR, canonical_out, clover, g->stream), "hirep_clover_export");
+}
+extern "C" int hirep_Cphi(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *clover) {
+    CHECK_PTRS("hirep_Cphi", out_full, in_full, clover);
+    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Cphi: out aliases in");
+    return kern_result(g, k_cphi(g->geo, g->prec, g->dR, 4.0 + m0, csw, clover, in_full, out_full, g->stream), "hirep_Cphi");
+}
+extern "C" int hirep_Dphi_clover(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *links, const void *clover) {
+    CHECK_PTRS("hirep_Dphi_clover", out_full, in_full, links, clover);
+    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Dphi_clover: out aliases in");
+    int rc = kern_result(g, k_cphi(g->geo, g->prec, g->dR, 4.0 + m0, csw, clover, in_full, out_full, g->stream), "hirep_Dphi_clover (diagonal term)");
+    if (rc) return rc;
+    // out = 1 * out - 1/2 hop(in): every site's own value is read before it is written, by the same tile
+    const size_t hb = g->bytes_spinor_half;
+    const char *in_e = (const char *)in_full, *in_o = in_e + hb;
+    char *out_e = (char *)out_full, *out_o = out_e + hb;
+    HopLaunch L{};
+    L.nsets = 2;
+    L.set[0] = HopSet{in_o, out_e, out_e, links_parity(g, links, 0), 0};
+    L.set[1] = HopSet{in_e, out_o, out_o, links_parity(g, links, 1), 1};
+    L.a = 1.0; L.b = -0.5; L.g5 = 0; L.am = 0.0;
+    return hop(g, L, "hirep_Dphi_clover (hopping term)");
+}
+
 // ---- spinor linear algebra, reductions, CG ------------------------------------------
 static long spinor_elems(const hirep_geom *g, int which) {   // complex elements of a native buffer, padding included
     return (long)g->geo.n_tiles * 4 * g->dR * TILE * (which == HIREP_FULL ? 2 : 1);

@@ -1,0 +1,233 @@
+// clover.cu -- clover term of the Wilson-Dirac operator (Eq 47-49).
+//
+//   D_ee,m + D_oo,m = (4+m) + c_sw (i/4) sum_{mu,nu} sigma_{mu nu} F_{mu nu}                       (Eq 47)
+//   C_{mu nu}(x) = the four plaquette loops through x in the (mu,nu) plane, each closed at x         (Eq 48; DESIGN A26)
+//   F_{mu nu} = (C_{mu nu} - C_{mu nu}^dagger)/8                                                    (Eq 49; DESIGN A27)
+//
+// With gamma_mu = [[0,e_mu],[e_mu^+,0]], e_0 = -1, e_k = -i sigma_k (Eq 2-3) and sigma_{mu nu} = (i/2)[gamma_mu,gamma_nu]
+// (DESIGN A28) the term is block diagonal in chirality, A = diag(A_0, A_1), A_c acting on spins (2c, 2c+1):
+//   sigma_01 = (s1,-s1)  sigma_02 = (s2,-s2)  sigma_03 = (s3,-s3)  sigma_12 = (-s3,-s3)  sigma_13 = (s2,s2)  sigma_23 = (-s1,-s1)
+//   A_c = s1 (x) K1 + s2 (x) K2 + s3 (x) K3 = [[H, B], [B^+, -H]],   H = K3,  B = K1 - i K2,   with (+ for c = 0, - for c = 1)
+//   K1 = (i/2)(+-F01 - F23),  K2 = (i/2)(+-F02 + F13),  K3 = (i/2)(+-F03 - F12)       (Hermitian, F being anti-Hermitian)
+//
+// Native clover field (caller-owned, hirep_clover_bytes): [parity][tile][c = 0,1][m = 0: H, 1: B][e = i*dR + j][lane]
+// complex<T>: 4 dR^2 complex per site, half the bytes of the eight represented links.
+//
+// Kernels: clover_field_kernel -- one CTA per site, the plaquette leaves as path products W_d1(x) W_d2(x+d1) ... out of
+// the gather-layout links (W_d = U_mu(x) / U_mu(x-mu)^dagger) in shared memory; runs once per gauge update like
+// links_to_rep.  cphi_kernel -- out = ((4+m) + c_sw A) in, one warp per (tile, output component), coalesced 32-lane rows.
+#include "kernels.h"
+
+namespace hirep {
+
+template <typename T> __device__ __forceinline__ cplx<T> cmul(cplx<T> a, cplx<T> b) { return mk<T>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+template <typename T> __device__ __forceinline__ void cfma(cplx<T> &acc, cplx<T> a, cplx<T> b) {
+    acc.x += a.x * b.x - a.y * b.y;
+    acc.y += a.x * b.y + a.y * b.x;
+}
+// acc += conj(a) * b
+template <typename T> __device__ __forceinline__ void cfma_conj(cplx<T> &acc, cplx<T> a, cplx<T> b) {
+    acc.x += a.x * b.x + a.y * b.y;
+    acc.y += a.x * b.y - a.y * b.x;
+}
+
+__host__ __device__ inline size_t clover_off(int n_tiles, int p, int tile, int c, int m, int e, int lane, int ne) {
+    return (((((size_t)p * n_tiles + tile) * 2 + c) * 2 + m) * ne + e) * TILE + lane;
+}
+
+__device__ inline int nbr_rt(const Geo &g, int p, int h, int d) {
+    int t, x, y, zh;
+    decode_site(g, h, t, x, y, zh);
+    switch (d) {
+    case 0: return neighbour<0>(g, p, t, x, y, zh);
+    case 1: return neighbour<1>(g, p, t, x, y, zh);
+    case 2: return neighbour<2>(g, p, t, x, y, zh);
+    case 3: return neighbour<3>(g, p, t, x, y, zh);
+    case 4: return neighbour<4>(g, p, t, x, y, zh);
+    case 5: return neighbour<5>(g, p, t, x, y, zh);
+    case 6: return neighbour<6>(g, p, t, x, y, zh);
+    default: return neighbour<7>(g, p, t, x, y, zh);
+    }
+}
+
+template <typename T, bool REAL> __device__ __forceinline__ cplx<T> ld_w(const link_elem<T, REAL> *links, size_t off) {
+    if constexpr (REAL) return mk<T>(links[off], T(0));
+    else return links[off];
+}
+
+// dynamic shared memory: P, Q, W, C (path product ping-pong, current link, leaf sum) and acc[4] = H0, B0, H1, B1
+template <typename T, bool REAL>
+__global__ void clover_field_kernel(Geo g, int dR, const link_elem<T, REAL> *__restrict__ links, cplx<T> *__restrict__ clover) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int ne = dR * dR;
+    cplx<T> *P = reinterpret_cast<cplx<T> *>(smem_raw), *Q = P + ne, *W = Q + ne, *C = W + ne, *acc = C + ne;
+    const int site = blockIdx.x;
+    const int p = site / g.Nh, h = site - p * g.Nh;
+    const int nt = blockDim.x, tid = threadIdx.x;
+    for (int e = tid; e < 4 * ne; e += nt) acc[e] = mk<T>(0, 0);
+    constexpr int PL[6][2] = {{0, 1}, {0, 2}, {0, 3}, {1, 2}, {1, 3}, {2, 3}};
+    for (int pl = 0; pl < 6; ++pl) {
+        const int mu = PL[pl][0], nu = PL[pl][1];
+        const int seq[4][4] = {{mu, nu, mu + 4, nu + 4}, {nu, mu + 4, nu + 4, mu}, {mu + 4, nu + 4, mu, nu}, {nu + 4, mu, nu, mu + 4}};
+        for (int e = tid; e < ne; e += nt) C[e] = mk<T>(0, 0);
+        for (int leaf = 0; leaf < 4; ++leaf) {
+            int cp = p, ch = h;
+            cplx<T> *A = P, *Bn = Q;
+            for (int k = 0; k < 4; ++k) {
+                const int d = seq[leaf][k];
+                const size_t base = link_off(g.n_tiles, cp, ch >> 5, d, 0, ch & 31, ne);
+                cplx<T> *dst = (k == 0) ? A : W;
+                for (int e = tid; e < ne; e += nt) dst[e] = ld_w<T, REAL>(links, base + (size_t)e * TILE);
+                __syncthreads();
+                if (k > 0) {
+                    for (int e = tid; e < ne; e += nt) {
+                        const int i = e / dR, j = e - i * dR;
+                        cplx<T> s = mk<T>(0, 0);
+                        for (int l = 0; l < dR; ++l) cfma<T>(s, A[i * dR + l], W[l * dR + j]);
+                        Bn[e] = s;
+                    }
+                    __syncthreads();
+                    cplx<T> *tmp = A; A = Bn; Bn = tmp;
+                }
+                ch = nbr_rt(g, cp, ch, d);
+                cp ^= 1;
+            }
+            for (int e = tid; e < ne; e += nt) { C[e].x += A[e].x; C[e].y += A[e].y; }
+            __syncthreads();
+        }
+        // F = (C - C^+)/8 ; contribution (i/2) F (and for K2, times -i) to H_c / B_c with the signs of the header table
+        for (int e = tid; e < ne; e += nt) {
+            const int i = e / dR, j = e - i * dR;
+            const cplx<T> a = C[e], b = C[j * dR + i];
+            const cplx<T> F = mk<T>((a.x - b.x) * T(0.125), (a.y + b.y) * T(0.125));
+            const cplx<T> iF = mk<T>(-T(0.5) * F.y, T(0.5) * F.x);    // (i/2) F
+            const cplx<T> hF = mk<T>(T(0.5) * F.x, T(0.5) * F.y);     // -i (i/2) F = F/2
+            cplx<T> *H0 = acc, *B0 = acc + ne, *H1 = acc + 2 * ne, *B1 = acc + 3 * ne;
+            switch (pl) {
+            case 0: B0[e].x += iF.x; B0[e].y += iF.y; B1[e].x -= iF.x; B1[e].y -= iF.y; break;   // K1 += +-(i/2) F01
+            case 5: B0[e].x -= iF.x; B0[e].y -= iF.y; B1[e].x -= iF.x; B1[e].y -= iF.y; break;   // K1 -= (i/2) F23
+            case 1: B0[e].x += hF.x; B0[e].y += hF.y; B1[e].x -= hF.x; B1[e].y -= hF.y; break;   // -i K2, K2 += +-(i/2) F02
+            case 4: B0[e].x += hF.x; B0[e].y += hF.y; B1[e].x += hF.x; B1[e].y += hF.y; break;   // -i K2, K2 += (i/2) F13
+            case 2: H0[e].x += iF.x; H0[e].y += iF.y; H1[e].x -= iF.x; H1[e].y -= iF.y; break;   // K3 += +-(i/2) F03
+            default: H0[e].x -= iF.x; H0[e].y -= iF.y; H1[e].x -= iF.x; H1[e].y -= iF.y; break;  // K3 -= (i/2) F12
+            }
+        }
+        __syncthreads();
+    }
+    const int tile = h >> 5, lane = h & 31;
+    for (int q = tid; q < 4 * ne; q += nt) {
+        const int cm = q / ne, e = q - cm * ne;
+        clover[clover_off(g.n_tiles, p, tile, cm >> 1, cm & 1, e, lane, ne)] = acc[q];
+    }
+}
+
+// padding lanes of the last tile of each parity
+template <typename T> __global__ void clover_pad_kernel(Geo g, int dR, cplx<T> *clover) {
+    const int ne = dR * dR, tile = g.n_tiles - 1;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= 4 * ne * TILE) return;
+    const int lane = idx % TILE, q = idx / TILE;
+    if (tile * TILE + lane < g.Nh) return;
+    for (int p = 0; p < 2; ++p) clover[clover_off(g.n_tiles, p, tile, q / (2 * ne), (q / ne) & 1, q % ne, lane, ne)] = mk<T>(0, 0);
+}
+
+// out = (a + csw A) in on `ntile_total` tiles (both parities are contiguous in every native buffer).
+// block = (32 lanes, WY warps); warp y of a block computes output components y, y + WY, ... of the block's tile.
+template <typename T>
+__global__ void cphi_kernel(int ntile_total, int dR, T a, T csw, const cplx<T> *__restrict__ clover, const cplx<T> *__restrict__ in,
+                            cplx<T> *__restrict__ out) {
+    const int ne = dR * dR, ncomp = 4 * dR, lane = threadIdx.x;
+    for (int tile = blockIdx.x; tile < ntile_total; tile += gridDim.x) {
+        const cplx<T> *psi = in + (size_t)tile * ncomp * TILE + lane;
+        const cplx<T> *cl = clover + (size_t)tile * 4 * ne * TILE + lane;
+        for (int comp = threadIdx.y; comp < ncomp; comp += blockDim.y) {
+            const int s = comp / dR, i = comp - s * dR, c = s >> 1, r = s & 1;
+            const cplx<T> *H = cl + (size_t)(2 * c) * ne * TILE, *B = H + (size_t)ne * TILE;
+            const cplx<T> *p0 = psi + (size_t)(2 * c) * dR * TILE, *p1 = p0 + (size_t)dR * TILE;
+            cplx<T> s0 = mk<T>(0, 0), s1 = mk<T>(0, 0);
+            if (r == 0) {
+#pragma unroll 4
+                for (int j = 0; j < dR; ++j) {
+                    cfma<T>(s0, __ldg(H + (size_t)(i * dR + j) * TILE), __ldg(p0 + (size_t)j * TILE));
+                    cfma<T>(s1, __ldg(B + (size_t)(i * dR + j) * TILE), __ldg(p1 + (size_t)j * TILE));
+                }
+                s0.x += s1.x; s0.y += s1.y;
+            } else {
+#pragma unroll 4
+                for (int j = 0; j < dR; ++j) {
+                    cfma_conj<T>(s0, __ldg(B + (size_t)(j * dR + i) * TILE), __ldg(p0 + (size_t)j * TILE));
+                    cfma<T>(s1, __ldg(H + (size_t)(i * dR + j) * TILE), __ldg(p1 + (size_t)j * TILE));
+                }
+                s0.x -= s1.x; s0.y -= s1.y;
+            }
+            const cplx<T> self = __ldg(psi + (size_t)comp * TILE);
+            __stcs(out + ((size_t)tile * ncomp + comp) * TILE + lane, mk<T>(a * self.x + csw * s0.x, a * self.y + csw * s0.y));
+        }
+    }
+}
+
+// canonical export: [V][c][2 dR][2 dR] complex, A_c = [[H, B], [B^+, -H]]; one thread per (site, c, row, column)
+template <typename T> __global__ void clover_export_kernel(Geo g, int dR, cplx<T> *__restrict__ canon, const cplx<T> *__restrict__ clover) {
+    const int n2 = 2 * dR, ne = dR * dR;
+    const long per_site = 2L * n2 * n2;
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= 2L * g.Nh * per_site) return;
+    const long site = idx / per_site;
+    int q = (int)(idx - site * per_site);
+    const int c = q / (n2 * n2);
+    q -= c * n2 * n2;
+    const int I = q / n2, J = q - I * n2;
+    const int p = (int)(site / g.Nh), h = (int)(site - (long)p * g.Nh);
+    const int tile = h >> 5, lane = h & 31;
+    const int bi = I / dR, i = I - bi * dR, bj = J / dR, j = J - bj * dR;
+    cplx<T> v;
+    if (bi == bj) {
+        v = clover[clover_off(g.n_tiles, p, tile, c, 0, i * dR + j, lane, ne)];
+        if (bi) { v.x = -v.x; v.y = -v.y; }
+    } else if (bi == 0) {
+        v = clover[clover_off(g.n_tiles, p, tile, c, 1, i * dR + j, lane, ne)];
+    } else {
+        v = clover[clover_off(g.n_tiles, p, tile, c, 1, j * dR + i, lane, ne)];
+        v.y = -v.y;
+    }
+    canon[(size_t)canonical_index(g, p, h) * per_site + (size_t)c * n2 * n2 + (size_t)I * n2 + J] = v;
+}
+
+template <typename T, bool REAL> static int clover_field_t(const Geo &g, int dR, void *clover, const void *links, cudaStream_t s) {
+    const int ne = dR * dR;
+    const size_t smem = (size_t)8 * ne * sizeof(cplx<T>);
+    auto kern = clover_field_kernel<T, REAL>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return (int)e;
+    const int nt = ne <= 32 ? 32 : ne <= 64 ? 64 : ne <= 128 ? 128 : 256;
+    kern<<<2 * g.Nh, nt, smem, s>>>(g, dR, (const link_elem<T, REAL> *)links, (cplx<T> *)clover);
+    if (g.Nh % TILE) clover_pad_kernel<T><<<(4 * ne * TILE + 255) / 256, 256, 0, s>>>(g, dR, (cplx<T> *)clover);
+    return (int)cudaGetLastError();
+}
+
+int k_clover_field(const Geo &g, int prec, int dR, int real, void *clover, const void *links_rep, cudaStream_t s) {
+    if (prec == 0) return real ? clover_field_t<double, true>(g, dR, clover, links_rep, s) : clover_field_t<double, false>(g, dR, clover, links_rep, s);
+    return real ? clover_field_t<float, true>(g, dR, clover, links_rep, s) : clover_field_t<float, false>(g, dR, clover, links_rep, s);
+}
+
+template <typename T> static int cphi_t(const Geo &g, int dR, double a, double csw, const void *clover, const void *in, void *out, cudaStream_t s) {
+    const int ntile = 2 * g.n_tiles;
+    const int wy = 4 * dR < 16 ? 4 * dR : 16;
+    int grid = ntile < 148 * 16 ? ntile : 148 * 16;
+    cphi_kernel<T><<<grid, dim3(TILE, wy), 0, s>>>(ntile, dR, (T)a, (T)csw, (const cplx<T> *)clover, (const cplx<T> *)in, (cplx<T> *)out);
+    return (int)cudaGetLastError();
+}
+int k_cphi(const Geo &g, int prec, int dR, double a, double csw, const void *clover, const void *in, void *out, cudaStream_t s) {
+    return prec == 0 ? cphi_t<double>(g, dR, a, csw, clover, in, out, s) : cphi_t<float>(g, dR, a, csw, clover, in, out, s);
+}
+
+template <typename T> static int clover_export_t(const Geo &g, int dR, void *canon, const void *clover, cudaStream_t s) {
+    const long n = 2L * g.Nh * 2 * (2 * dR) * (2 * dR);
+    clover_export_kernel<T><<<(unsigned)((n + 255) / 256), 256, 0, s>>>(g, dR, (cplx<T> *)canon, (const cplx<T> *)clover);
+    return (int)cudaGetLastError();
+}
+int k_clover_export(const Geo &g, int prec, int dR, void *canon, const void *clover, cudaStream_t s) {
+    return prec == 0 ? clover_export_t<double>(g, dR, canon, clover, s) : clover_export_t<float>(g, dR, canon, clover, s);
+}
+
+}  // namespace hirep

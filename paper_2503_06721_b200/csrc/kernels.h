@@ -45,6 +45,10 @@ int k_cg_update(const Geo &g, int prec, int dR, int halves, int alg, double alph
                 double *out_dev, cudaStream_t s);
 int k_cg_xp(const Geo &g, int prec, int dR, int halves, double alpha, double beta, void *x, void *p, const void *r, cudaStream_t s);
 int k_fma_peak(int prec, double *tflops, cudaStream_t s);   // fma_peak.cu: measured FP64/FP32 FMA throughput
+// clover.cu: clover term (Eq 47-49); native clover field = 4 dR^2 complex per site
+int k_clover_field(const Geo &g, int prec, int dR, int real, void *clover, const void *links_rep, cudaStream_t s);
+int k_clover_export(const Geo &g, int prec, int dR, void *canon, const void *clover, cudaStream_t s);
+int k_cphi(const Geo &g, int prec, int dR, double a, double csw, const void *clover, const void *in, void *out, cudaStream_t s);
 // number of distinct kernel launches k_hop issues for this configuration (for launch accounting): always 1.
 
 }  // namespace hirep

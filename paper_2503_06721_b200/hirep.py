@@ -33,6 +33,7 @@ SYMBOLS = [
     "hirep_spinor_lc1", "hirep_spinor_lc2", "hirep_spinor_lc3", "hirep_spinor_prod", "hirep_spinor_sqnorm",
     "hirep_spinor_max_norm", "hirep_cg_g5Dphi_sq", "hirep_spinor_g5_lc", "hirep_spinor_gamma", "hirep_spinor_g5_lc_add_assign", "hirep_spinor_g5_prod", "hirep_Dphi_tm", "hirep_Dphi_tm_sq",
     "hirep_Dphi_tm_hat", "hirep_cg_Dphi_tm_sq", "hirep_cg_mshift_g5Dphi_sq", "hirep_bicgstab", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
+    "hirep_clover_bytes", "hirep_clover_field", "hirep_clover_export", "hirep_Cphi", "hirep_Dphi_clover",
 ]
 
 
@@ -103,6 +104,11 @@ def load():
     lib.hirep_bicgstab.argtypes = [vp, ci, cd, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_cg_Dphi_tm_sq.argtypes = [vp, cd, cd, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_fma_peak.argtypes = [ci, ctypes.POINTER(cd)]
+    lib.hirep_clover_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t)]
+    lib.hirep_clover_field.argtypes = [vp, vp, vp]
+    lib.hirep_clover_export.argtypes = [vp, vp, vp]
+    lib.hirep_Cphi.argtypes = [vp, cd, cd, vp, vp, vp]
+    lib.hirep_Dphi_clover.argtypes = [vp, cd, cd, vp, vp, vp, vp]
     lib.hirep_sync.argtypes = [vp]
     lib.hirep_last_error.restype = ctypes.c_char_p
     for n in SYMBOLS:
@@ -223,6 +229,16 @@ def hirep_spinor_g5_prod(g, which, xi, eta):
 
 def hirep_Dphi_tm(g, m0, mu, out, inp, links): _check(load().hirep_Dphi_tm(g, m0, mu, out, inp, links))
 def hirep_Dphi_tm_sq(g, m0, mu, out, inp, links): _check(load().hirep_Dphi_tm_sq(g, m0, mu, out, inp, links))
+def hirep_clover_bytes(g) -> int:
+    n = ctypes.c_size_t(0)
+    _check(load().hirep_clover_bytes(g, ctypes.byref(n)))
+    return n.value
+
+
+def hirep_clover_field(g, clover, links_rep): _check(load().hirep_clover_field(g, clover, links_rep))
+def hirep_clover_export(g, canonical, clover): _check(load().hirep_clover_export(g, canonical, clover))
+def hirep_Cphi(g, m0, csw, out, inp, clover): _check(load().hirep_Cphi(g, m0, csw, out, inp, clover))
+def hirep_Dphi_clover(g, m0, csw, out, inp, links, clover): _check(load().hirep_Dphi_clover(g, m0, csw, out, inp, links, clover))
 def hirep_Dphi_tm_hat(g, m0, mu, out, inp, links): _check(load().hirep_Dphi_tm_hat(g, m0, mu, out, inp, links))
 
 
@@ -429,6 +445,28 @@ class Geometry:
     def Dphi_tm_hat(self, m0, mu, inp_even, links, out=None):
         out = self.new_spinor(EVEN) if out is None else out
         hirep_Dphi_tm_hat(self.handle, m0, mu, out.data_ptr(), inp_even.data_ptr(), links.data_ptr())
+        return out
+
+    # clover term (Eq 47-49)
+    def clover_field(self, links_rep, out=None):
+        if out is None:
+            out = self.torch.empty(hirep_clover_bytes(self.handle), dtype=self.torch.uint8, device=self.device)
+        hirep_clover_field(self.handle, out.data_ptr(), links_rep.data_ptr())
+        return out
+
+    def clover_export(self, clover):
+        canonical = self.torch.empty((self.V, 2, 2 * self.d_R, 2 * self.d_R), dtype=self.cdtype, device=self.device)
+        hirep_clover_export(self.handle, canonical.data_ptr(), clover.data_ptr())
+        return canonical
+
+    def Cphi(self, m0, csw, inp, clover, out=None):
+        out = self.new_spinor(FULL) if out is None else out
+        hirep_Cphi(self.handle, m0, csw, out.data_ptr(), inp.data_ptr(), clover.data_ptr())
+        return out
+
+    def Dphi_clover(self, m0, csw, inp, links, clover, out=None):
+        out = self.new_spinor(FULL) if out is None else out
+        hirep_Dphi_clover(self.handle, m0, csw, out.data_ptr(), inp.data_ptr(), links.data_ptr(), clover.data_ptr())
         return out
 
     def cg_mshift_g5Dphi_sq(self, m0, shifts, b, links, tol, maxiter):

@@ -1,0 +1,80 @@
+"""GPU parity of the clover term (Eq 47-49, second part) against oracle/clover.py,
+through the C-ABI binding: the clover field itself (both chirality blocks, element by element), Cphi and Dphi_clover.
+Tolerances as for the Wilson operators: relative L2 <= 1e-13 (fp64) / 1e-5 (fp32)."""
+import numpy as np
+import pytest
+
+from paper_2503_06721_b200 import synth
+from tests.gpu_helpers import BC, TOL
+from tests.test_gpu_parity import Problem, env  # noqa: F401  (env is a fixture)
+
+pytestmark = pytest.mark.gpu
+
+# ring (C1-C3), pair (C4) and row-group (C5) hopping kernels under the in-place second pass; ragged tails and whole tiles
+CASES = [("C1", 4, 4), ("C2", 6, 6), ("C3", 4, 8), ("C4", 4, 6), ("C5", 2, 4)]
+
+
+@pytest.mark.parametrize("name,T,L", CASES)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_clover_field_and_operators(env, name, T, L, prec):
+    from oracle import clover as oc
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS[name].resized(T, L)
+    p = Problem(env, cfg, prec)
+    g, m0, tol, csw = p.geom, cfg.m0, TOL[prec], 1.7
+    cl = g.clover_field(p.links_rep)
+    got = g.clover_export(cl).cpu().numpy().astype(np.complex128)
+    want = oc.chiral_blocks(T, L, p.R)
+    assert np.abs(want).max() > 0.05
+    assert oracle.rel_l2(got, want) < tol
+    assert np.abs(got - want).max() < 50 * tol * np.abs(want).max()
+    psi = p.spinors[0]
+    x = p.to_native(psi, hirep.FULL)
+    out = p.to_numpy(g.Cphi(m0, csw, x, cl), hirep.FULL)
+    assert oracle.rel_l2(out, oc.Cphi(T, L, m0, csw, p.R, psi)) < tol
+    out = p.to_numpy(g.Dphi_clover(m0, csw, x, p.links_rep, cl), hirep.FULL)
+    assert oracle.rel_l2(out, oc.Dphi_clover(T, L, m0, csw, p.R, psi, BC)) < tol
+    # c_sw = 0 is the unimproved operator
+    a = p.to_numpy(g.Dphi_clover(m0, 0.0, x, p.links_rep, cl), hirep.FULL)
+    assert oracle.rel_l2(a, oracle.Dphi(T, L, cfg.d_R, m0, p.R, psi, BC)) < tol
+
+
+@pytest.mark.parametrize("n,rep,T,L", [(2, 1, 2, 4), (3, 2, 4, 4), (4, 1, 2, 2), (6, 0, 2, 4), (3, 3, 4, 4)])
+def test_clover_other_representations(env, n, rep, T, L):
+    """SU(2) adjoint (real links), SU(3) symmetric, SU(4) adjoint (d_R = 15, real), SU(6) fundamental, SU(3) 2AS."""
+    from oracle import clover as oc
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.Config("t", T, L, n, rep, -0.1, "haar", 17, ())
+    p = Problem(env, cfg, "f64")
+    cl = p.geom.clover_field(p.links_rep)
+    assert oracle.rel_l2(p.geom.clover_export(cl).cpu().numpy(), oc.chiral_blocks(T, L, p.R)) < 1e-13
+    psi = p.spinors[0]
+    out = p.to_numpy(p.geom.Dphi_clover(cfg.m0, 0.9, p.to_native(psi, hirep.FULL), p.links_rep, cl), hirep.FULL)
+    assert oracle.rel_l2(out, oc.Dphi_clover(T, L, cfg.m0, 0.9, p.R, psi, BC)) < 1e-13
+
+
+def test_clover_periodic_bc_and_capped_grid(env):
+    """Boundary signs cancel in the closed loops: the clover field is the same for periodic and antiperiodic links;
+    Dphi_clover with a capped persistent grid (many tiles per warp in the in-place hopping pass)."""
+    from oracle import clover as oc
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS["C2"].resized(4, 6)
+    p = Problem(env, cfg, "f64")
+    cl = p.geom.clover_field(p.links_rep)
+    a = p.geom.clover_export(cl).cpu().numpy()
+    p.geom.set_tuning(hirep.TUNE_MAX_CTAS, 3)
+    psi = p.spinors[0]
+    out = p.to_numpy(p.geom.Dphi_clover(cfg.m0, 1.0, p.to_native(psi, hirep.FULL), p.links_rep, cl), hirep.FULL)
+    assert oracle.rel_l2(out, oc.Dphi_clover(cfg.T, cfg.L, cfg.m0, 1.0, p.R, psi, BC)) < 1e-13
+    p.geom.set_bc((1, 1, 1, 1))
+    links_rep = p.geom.links_to_rep(p.links_fund)
+    b = p.geom.clover_export(p.geom.clover_field(links_rep)).cpu().numpy()
+    assert np.array_equal(a, b)
+
+
+def test_clover_needs_stored_links(env):
+    hirep = env["hirep"]
+    p = Problem(env, synth.CONFIGS["C4"].resized(2, 4), "f64")
+    p.geom.set_link_mode(hirep.LINKS_REBUILD)
+    with pytest.raises(hirep.HirepError):
+        p.geom.clover_field(p.links_fund)
