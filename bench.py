@@ -381,6 +381,23 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
     by = cm["ops"]["Dphi_hat"][1] + 2 * S * V / 2          # + the in-place gamma_5 combination on the odd field
     out["Dphi_tm_hat"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3),
                           "gflops": round(cm["ops"]["Dphi_hat"][0] / ms / 1e6, 1), "launches": 3}
+    # NEXT-2, second part: clover term (Eq 47-49).  Algorithmic bytes per site: clover field 4 d^2 complex + spinor in/out.
+    d = cfg.d_R
+    cb = S * d                                          # clover bytes per site: 4 d^2 complex (S = 4 d complex)
+    if torch.cuda.mem_get_info()[0] < cb * V + (4 << 30):
+        out["clover"] = {"skipped": "clover field of %.1f GB does not fit beside the resident fields" % (cb * V / 1e9)}
+    else:
+        lbytes = geom.sizes["links_rep"] / V            # represented-link bytes per site
+        cl = geom.clover_field(lr)
+        ms = timeit(lambda: geom.clover_field(lr, out=cl), reps=3)
+        out["clover_field"] = {"ms": round(ms, 3), "note": "once per gauge update; 72 d_R^3 complex MACs per site out of the gather-layout links"}
+        ms = timeit(lambda: geom.Cphi(m0, 1.0, x_full, cl, out=y_full))
+        by = (cb + 2 * S) * V
+        out["Cphi"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3)}
+        ms = timeit(lambda: geom.Dphi_clover(m0, 1.0, x_full, lr, cl, out=y_full), reps=10)
+        by = (cb + 2 * S + lbytes + 3 * S) * V
+        out["Dphi_clover"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3), "launches": 2}
+        del cl
     try:
         out["fma_peak_tflops"] = {"f64": round(hirep.hirep_fma_peak(hirep.F64), 2), "f32": round(hirep.hirep_fma_peak(hirep.F32), 2)}
     except Exception as e:   # measurement utility only

@@ -13,9 +13,9 @@
 // Native clover field (caller-owned, hirep_clover_bytes): [parity][tile][c = 0,1][m = 0: H, 1: B][e = i*dR + j][lane]
 // complex<T>: 4 dR^2 complex per site, half the bytes of the eight represented links.
 //
-// Kernels: clover_field_kernel -- one CTA per site, the plaquette leaves as path products W_d1(x) W_d2(x+d1) ... out of
+// Kernels: clover_field_kernel -- a group of threads per site (several sites per CTA), the plaquette leaves as path products W_d1(x) W_d2(x+d1) ... out of
 // the gather-layout links (W_d = U_mu(x) / U_mu(x-mu)^dagger) in shared memory; runs once per gauge update like
-// links_to_rep.  cphi_kernel -- out = ((4+m) + c_sw A) in, one warp per (tile, output component), coalesced 32-lane rows.
+// links_to_rep.  cphi_site_kernel / cphi_kernel -- out = ((4+m) + c_sw A) in, coalesced 32-lane rows (see there).
 #include "kernels.h"
 
 namespace hirep {
@@ -60,8 +60,11 @@ template <typename T, bool REAL>
 __global__ void clover_field_kernel(Geo g, int dR, const link_elem<T, REAL> *__restrict__ links, cplx<T> *__restrict__ clover) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int ne = dR * dR;
-    cplx<T> *P = reinterpret_cast<cplx<T> *>(smem_raw), *Q = P + ne, *W = Q + ne, *C = W + ne, *acc = C + ne;
-    const int site = blockIdx.x;
+    cplx<T> *P = reinterpret_cast<cplx<T> *>(smem_raw) + (size_t)threadIdx.y * 8 * ne, *Q = P + ne, *W = Q + ne, *C = W + ne, *acc = C + ne;
+    // blockDim = (threads per site, sites per CTA); a CTA past the end recomputes the last site and does not store
+    const long want = (long)blockIdx.x * blockDim.y + threadIdx.y;
+    const bool live = want < 2L * g.Nh;
+    const int site = live ? (int)want : 2 * g.Nh - 1;
     const int p = site / g.Nh, h = site - p * g.Nh;
     const int nt = blockDim.x, tid = threadIdx.x;
     for (int e = tid; e < 4 * ne; e += nt) acc[e] = mk<T>(0, 0);
@@ -115,7 +118,7 @@ __global__ void clover_field_kernel(Geo g, int dR, const link_elem<T, REAL> *__r
         __syncthreads();
     }
     const int tile = h >> 5, lane = h & 31;
-    for (int q = tid; q < 4 * ne; q += nt) {
+    for (int q = tid; live && q < 4 * ne; q += nt) {
         const int cm = q / ne, e = q - cm * ne;
         clover[clover_off(g.n_tiles, p, tile, cm >> 1, cm & 1, e, lane, ne)] = acc[q];
     }
@@ -132,7 +135,52 @@ template <typename T> __global__ void clover_pad_kernel(Geo g, int dR, cplx<T> *
 }
 
 // out = (a + csw A) in on `ntile_total` tiles (both parities are contiguous in every native buffer).
-// block = (32 lanes, WY warps); warp y of a block computes output components y, y + WY, ... of the block's tile.
+// Small d_R (<= 6): one thread per site, one warp per tile, everything unrolled: per chirality the 2 d_R^2 block elements
+// stream through once (H serves both spin rows, B serves B psi_1 and B^+ psi_0), all loads independent.
+template <typename T, int DR>
+__global__ void __launch_bounds__(128) cphi_site_kernel(int ntile_total, T a, T csw, const cplx<T> *__restrict__ clover,
+                                                        const cplx<T> *__restrict__ in, cplx<T> *__restrict__ out) {
+    constexpr int NE = DR * DR, NCOMP = 4 * DR;
+    const int lane = threadIdx.x & 31;
+    const int wpb = blockDim.x >> 5;
+    for (int tile = blockIdx.x * wpb + (threadIdx.x >> 5); tile < ntile_total; tile += gridDim.x * wpb) {
+        const cplx<T> *psi = in + (size_t)tile * NCOMP * TILE + lane;
+        const cplx<T> *cl = clover + (size_t)tile * 4 * NE * TILE + lane;
+        cplx<T> *o = out + (size_t)tile * NCOMP * TILE + lane;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            const cplx<T> *H = cl + (size_t)(2 * c) * NE * TILE, *B = H + (size_t)NE * TILE;
+            cplx<T> p0[DR], p1[DR], o0[DR], o1[DR];
+#pragma unroll
+            for (int j = 0; j < DR; ++j) {
+                p0[j] = __ldg(psi + (size_t)((2 * c) * DR + j) * TILE);
+                p1[j] = __ldg(psi + (size_t)((2 * c + 1) * DR + j) * TILE);
+                o0[j] = mk<T>(0, 0);
+                o1[j] = mk<T>(0, 0);
+            }
+#pragma unroll
+            for (int i = 0; i < DR; ++i) {
+#pragma unroll
+                for (int j = 0; j < DR; ++j) {
+                    const cplx<T> h = __ldcs(H + (size_t)(i * DR + j) * TILE);
+                    const cplx<T> b = __ldcs(B + (size_t)(i * DR + j) * TILE);
+                    cfma<T>(o0[i], h, p0[j]);
+                    cfma<T>(o1[i], mk<T>(-h.x, -h.y), p1[j]);
+                    cfma<T>(o0[i], b, p1[j]);
+                    cfma_conj<T>(o1[j], b, p0[i]);
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < DR; ++i) {
+                __stcs(o + (size_t)((2 * c) * DR + i) * TILE, mk<T>(a * p0[i].x + csw * o0[i].x, a * p0[i].y + csw * o0[i].y));
+                __stcs(o + (size_t)((2 * c + 1) * DR + i) * TILE, mk<T>(a * p1[i].x + csw * o1[i].x, a * p1[i].y + csw * o1[i].y));
+            }
+        }
+    }
+}
+
+// Any d_R: block = (32 lanes, WY warps); warp y computes the output rows (2c, i) and (2c+1, i) for the pairs
+// (c, i) = y, y + WY, ... of the block's tile: row i of H once for both, row i and column i of B.
 template <typename T>
 __global__ void cphi_kernel(int ntile_total, int dR, T a, T csw, const cplx<T> *__restrict__ clover, const cplx<T> *__restrict__ in,
                             cplx<T> *__restrict__ out) {
@@ -140,28 +188,25 @@ __global__ void cphi_kernel(int ntile_total, int dR, T a, T csw, const cplx<T> *
     for (int tile = blockIdx.x; tile < ntile_total; tile += gridDim.x) {
         const cplx<T> *psi = in + (size_t)tile * ncomp * TILE + lane;
         const cplx<T> *cl = clover + (size_t)tile * 4 * ne * TILE + lane;
-        for (int comp = threadIdx.y; comp < ncomp; comp += blockDim.y) {
-            const int s = comp / dR, i = comp - s * dR, c = s >> 1, r = s & 1;
+        cplx<T> *o = out + (size_t)tile * ncomp * TILE + lane;
+        for (int q = threadIdx.y; q < 2 * dR; q += blockDim.y) {
+            const int c = q / dR, i = q - c * dR;
             const cplx<T> *H = cl + (size_t)(2 * c) * ne * TILE, *B = H + (size_t)ne * TILE;
             const cplx<T> *p0 = psi + (size_t)(2 * c) * dR * TILE, *p1 = p0 + (size_t)dR * TILE;
-            cplx<T> s0 = mk<T>(0, 0), s1 = mk<T>(0, 0);
-            if (r == 0) {
-#pragma unroll 4
-                for (int j = 0; j < dR; ++j) {
-                    cfma<T>(s0, __ldg(H + (size_t)(i * dR + j) * TILE), __ldg(p0 + (size_t)j * TILE));
-                    cfma<T>(s1, __ldg(B + (size_t)(i * dR + j) * TILE), __ldg(p1 + (size_t)j * TILE));
-                }
-                s0.x += s1.x; s0.y += s1.y;
-            } else {
-#pragma unroll 4
-                for (int j = 0; j < dR; ++j) {
-                    cfma_conj<T>(s0, __ldg(B + (size_t)(j * dR + i) * TILE), __ldg(p0 + (size_t)j * TILE));
-                    cfma<T>(s1, __ldg(H + (size_t)(i * dR + j) * TILE), __ldg(p1 + (size_t)j * TILE));
-                }
-                s0.x -= s1.x; s0.y -= s1.y;
+            cplx<T> s0 = mk<T>(0, 0), s1 = mk<T>(0, 0), s2 = mk<T>(0, 0), s3 = mk<T>(0, 0);
+#pragma unroll 5
+            for (int j = 0; j < dR; ++j) {
+                const cplx<T> h = __ldg(H + (size_t)(i * dR + j) * TILE), b = __ldg(B + (size_t)(i * dR + j) * TILE);
+                const cplx<T> bt = __ldg(B + (size_t)(j * dR + i) * TILE);
+                const cplx<T> x0 = __ldg(p0 + (size_t)j * TILE), x1 = __ldg(p1 + (size_t)j * TILE);
+                cfma<T>(s0, h, x0);
+                cfma<T>(s1, b, x1);
+                cfma_conj<T>(s2, bt, x0);
+                cfma<T>(s3, h, x1);
             }
-            const cplx<T> self = __ldg(psi + (size_t)comp * TILE);
-            __stcs(out + ((size_t)tile * ncomp + comp) * TILE + lane, mk<T>(a * self.x + csw * s0.x, a * self.y + csw * s0.y));
+            const cplx<T> e0 = __ldg(p0 + (size_t)i * TILE), e1 = __ldg(p1 + (size_t)i * TILE);
+            __stcs(o + (size_t)((2 * c) * dR + i) * TILE, mk<T>(a * e0.x + csw * (s0.x + s1.x), a * e0.y + csw * (s0.y + s1.y)));
+            __stcs(o + (size_t)((2 * c + 1) * dR + i) * TILE, mk<T>(a * e1.x + csw * (s2.x - s3.x), a * e1.y + csw * (s2.y - s3.y)));
         }
     }
 }
@@ -195,12 +240,15 @@ template <typename T> __global__ void clover_export_kernel(Geo g, int dR, cplx<T
 
 template <typename T, bool REAL> static int clover_field_t(const Geo &g, int dR, void *clover, const void *links, cudaStream_t s) {
     const int ne = dR * dR;
-    const size_t smem = (size_t)8 * ne * sizeof(cplx<T>);
+    int nt = 4;
+    while (nt < ne && nt < 256) nt *= 2;
+    const int sites = nt >= 128 ? 1 : 128 / nt;
+    const size_t smem = (size_t)sites * 8 * ne * sizeof(cplx<T>);
     auto kern = clover_field_kernel<T, REAL>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
-    const int nt = ne <= 32 ? 32 : ne <= 64 ? 64 : ne <= 128 ? 128 : 256;
-    kern<<<2 * g.Nh, nt, smem, s>>>(g, dR, (const link_elem<T, REAL> *)links, (cplx<T> *)clover);
+    const unsigned blocks = (unsigned)((2L * g.Nh + sites - 1) / sites);
+    kern<<<blocks, dim3(nt, sites), smem, s>>>(g, dR, (const link_elem<T, REAL> *)links, (cplx<T> *)clover);
     if (g.Nh % TILE) clover_pad_kernel<T><<<(4 * ne * TILE + 255) / 256, 256, 0, s>>>(g, dR, (cplx<T> *)clover);
     return (int)cudaGetLastError();
 }
@@ -210,9 +258,22 @@ int k_clover_field(const Geo &g, int prec, int dR, int real, void *clover, const
     return real ? clover_field_t<float, true>(g, dR, clover, links_rep, s) : clover_field_t<float, false>(g, dR, clover, links_rep, s);
 }
 
+template <typename T, int DR> static int cphi_site_t(int ntile, double a, double csw, const void *clover, const void *in, void *out, cudaStream_t s) {
+    const int blocks = (ntile + 3) / 4;
+    cphi_site_kernel<T, DR><<<blocks < 148 * 16 ? blocks : 148 * 16, 128, 0, s>>>(ntile, (T)a, (T)csw, (const cplx<T> *)clover, (const cplx<T> *)in,
+                                                                                 (cplx<T> *)out);
+    return (int)cudaGetLastError();
+}
 template <typename T> static int cphi_t(const Geo &g, int dR, double a, double csw, const void *clover, const void *in, void *out, cudaStream_t s) {
     const int ntile = 2 * g.n_tiles;
-    const int wy = 4 * dR < 16 ? 4 * dR : 16;
+    switch (dR) {
+    case 2: return cphi_site_t<T, 2>(ntile, a, csw, clover, in, out, s);
+    case 3: return cphi_site_t<T, 3>(ntile, a, csw, clover, in, out, s);
+    case 4: return cphi_site_t<T, 4>(ntile, a, csw, clover, in, out, s);
+    case 5: return cphi_site_t<T, 5>(ntile, a, csw, clover, in, out, s);
+    case 6: return cphi_site_t<T, 6>(ntile, a, csw, clover, in, out, s);
+    }
+    const int wy = 2 * dR < 16 ? 2 * dR : 16;
     int grid = ntile < 148 * 16 ? ntile : 148 * 16;
     cphi_kernel<T><<<grid, dim3(TILE, wy), 0, s>>>(ntile, dR, (T)a, (T)csw, (const cplx<T> *)clover, (const cplx<T> *)in, (cplx<T> *)out);
     return (int)cudaGetLastError();
