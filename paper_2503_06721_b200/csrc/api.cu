@@ -386,8 +386,7 @@ extern "C" int hirep_clover_bytes(const hirep_geom *g, size_t *bytes) {
 extern "C" int hirep_clover_field(hirep_geom *g, void *clover, const void *links_rep) {
     CHECK_PTRS("hirep_clover_field", clover, links_rep);
     if (g->mode != HIREP_LINKS_STORED) return fail(HIREP_EINVAL, "hirep_clover_field: needs the stored represented links (HIREP_LINKS_STORED)");
-    const int nl = 1 + (g->geo.Nh % TILE ? 1 : 0);
-    return kern_result(g, k_clover_field(g->geo, g->prec, g->dR, g->real, clover, links_rep, g->stream), "hirep_clover_field", nl);
+    return kern_result(g, k_clover_field(g->geo, g->prec, g->dR, g->real, clover, links_rep, g->stream), "hirep_clover_field");
 }
 extern "C" int hirep_clover_export(hirep_geom *g, void *canonical_out, const void *clover) {
     CHECK_PTRS("hirep_clover_export", canonical_out, clover);

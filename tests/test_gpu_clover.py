@@ -39,9 +39,10 @@ def test_clover_field_and_operators(env, name, T, L, prec):
     assert oracle.rel_l2(a, oracle.Dphi(T, L, cfg.d_R, m0, p.R, psi, BC)) < tol
 
 
-@pytest.mark.parametrize("n,rep,T,L", [(2, 1, 2, 4), (3, 2, 4, 4), (4, 1, 2, 2), (6, 0, 2, 4), (3, 3, 4, 4)])
+@pytest.mark.parametrize("n,rep,T,L", [(2, 1, 2, 4), (3, 2, 4, 4), (4, 1, 2, 2), (6, 0, 2, 4), (3, 3, 4, 4), (3, 1, 2, 4), (4, 2, 2, 4), (5, 0, 4, 2)])
 def test_clover_other_representations(env, n, rep, T, L):
-    """SU(2) adjoint (real links), SU(3) symmetric, SU(4) adjoint (d_R = 15, real), SU(6) fundamental, SU(3) 2AS."""
+    """SU(2) adjoint (real links), SU(3) symmetric, SU(4) adjoint (d_R = 15, real), SU(6) fundamental, SU(3) 2AS, SU(3) adjoint
+    (d_R = 8), SU(4) symmetric (d_R = 10), SU(5) fundamental: every Cphi / clover-field instantiation and the generic ones."""
     from oracle import clover as oc
     hirep, oracle = env["hirep"], env["oracle"]
     cfg = synth.Config("t", T, L, n, rep, -0.1, "haar", 17, ())
