@@ -19,6 +19,12 @@ Readings (A26-A28):
        sum in Eq 47 runs over all ordered pairs (mu,nu), so the term is Hermitian and commutes with gamma_5.
   The links are the represented links R(U_mu(x)); boundary signs +-1 cancel in every closed plaquette loop.
 
+Pins (tests/test_oracle_clover.py): sigma matrices typed from hand algebra, constant abelian background (closed form),
+random abelian background against a brute-force sum over the four base points Eq 48 prints, gauge covariance, pure
+gauge = 0, Hermiticity / tracelessness / chirality blocks, gamma_5-Hermiticity of the full operator, c_sw = 0.
+Parity unpinned in one respect: the overall sign convention of the c_sw term (A28) -- the paper prints nothing that
+fixes sigma_{mu nu} beyond the name.
+
 Layout: Rlinks [V, 4, d, d] complex, V = T L^3 canonical sites ((t*L + x)*L + y)*L + z; spinors [V, 4, d].
 """
 from __future__ import annotations
