@@ -222,7 +222,7 @@ __global__ void __launch_bounds__(128) cphi_site_kernel(int ntile_total, T a, T 
 // Any d_R: block = (32 lanes, WY warps); warp y computes the output rows (2c, i) and (2c+1, i) for the pairs
 // (c, i) = y, y + WY, ... of the block's tile: row i of H once for both, row i and column i of B.
 template <typename T>
-__global__ void cphi_kernel(int ntile_total, int dR, T a, T csw, const cplx<T> *__restrict__ clover, const cplx<T> *__restrict__ in,
+__global__ void __launch_bounds__(256, sizeof(T) == 8 ? 4 : 3) cphi_kernel(int ntile_total, int dR, T a, T csw, const cplx<T> *__restrict__ clover, const cplx<T> *__restrict__ in,
                             cplx<T> *__restrict__ out) {
     const int ne = dR * dR, ncomp = 4 * dR, lane = threadIdx.x;
     for (int tile = blockIdx.x; tile < ntile_total; tile += gridDim.x) {
@@ -318,7 +318,7 @@ template <typename T> static int cphi_t(const Geo &g, int dR, double a, double c
     case 8: return cphi_site_t<T, 8>(ntile, a, csw, clover, in, out, s);
     case 10: return cphi_site_t<T, 10>(ntile, a, csw, clover, in, out, s);
     }
-    const int wy = 2 * dR < 16 ? 2 * dR : 16;
+    const int wy = 2 * dR < 8 ? 2 * dR : 8;      // 8 warps per CTA, 3 CTAs per SM (one 16-warp CTA per SM was latency bound: 2.9 TB/s)
     int grid = ntile < 148 * 16 ? ntile : 148 * 16;   // (one CTA per SM measured slower: 4.7 vs 4.1 ms at d_R = 35 fp64)
     cphi_kernel<T><<<grid, dim3(TILE, wy), 0, s>>>(ntile, dR, (T)a, (T)csw, (const cplx<T> *)clover, (const cplx<T> *)in, (cplx<T> *)out);
     return (int)cudaGetLastError();
