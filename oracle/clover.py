@@ -115,3 +115,40 @@ def Dphi_clover(T, L, m0, csw, Rlinks, psi, bc):
     from . import oracle as _o
     d = Rlinks.shape[-1]
     return _o.hop_field(T, L, d, Rlinks, psi, bc) + Cphi(T, L, m0, csw, Rlinks, psi)
+
+
+def _parity_sites(T, L, parity):
+    t, x, y, z = np.meshgrid(np.arange(T), np.arange(L), np.arange(L), np.arange(L), indexing="ij")
+    return np.nonzero(((t + x + y + z) % 2).reshape(-1) == parity)[0]
+
+
+def diag_blocks(T, L, m0, csw, Rlinks):
+    """The site-diagonal blocks of D_ee,m / D_oo,m (Eq 47) per chirality: (4+m) 1 + c_sw A_c, [V, 2, 2d, 2d]."""
+    B = csw * chiral_blocks(T, L, Rlinks)
+    n = B.shape[-1]
+    return B + (4.0 + m0) * np.eye(n)
+
+
+def Cphi_inv(T, L, m0, csw, Rlinks, psi, sites=None):
+    """((4+m) + c_sw (i/4) sum sigma F)^{-1} psi, site by site (numpy's dense inverse of each 2d x 2d block);
+    psi [n, 4, d] on the canonical sites `sites` (all sites if None)."""
+    M = diag_blocks(T, L, m0, csw, Rlinks)
+    if sites is not None:
+        M = M[sites]
+    psi = np.asarray(psi, dtype=np.complex128)
+    n, _, d = psi.shape
+    v = psi.reshape(n, 2, 2 * d)
+    return np.einsum("xcij,xcj->xci", np.linalg.inv(M), v).reshape(n, 4, d)
+
+
+def Dphi_clover_hat(T, L, m0, csw, Rlinks, psi_even, bc):
+    """Eq 43 with the clover diagonal blocks of Eq 47: D_ee psi_e - D_eo D_oo^{-1} D_oe psi_e (even sites)."""
+    from . import oracle as _o
+    d = Rlinks.shape[-1]
+    ev, od = _parity_sites(T, L, 0), _parity_sites(T, L, 1)
+    psi_even = np.asarray(psi_even, dtype=np.complex128)
+    M = diag_blocks(T, L, m0, csw, Rlinks)
+    dee = np.einsum("xcij,xcj->xci", M[ev], psi_even.reshape(len(ev), 2, 2 * d)).reshape(len(ev), 4, d)
+    t = _o.Dphi_oe(T, L, d, Rlinks, psi_even, bc)
+    u = Cphi_inv(T, L, m0, csw, Rlinks, t, sites=od)
+    return dee - _o.Dphi_eo(T, L, d, Rlinks, u, bc)

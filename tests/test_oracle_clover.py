@@ -140,3 +140,34 @@ def test_g5_hermiticity_of_clover_operator(oracle):
     # c_sw = 0 reduces to the unimproved operator
     np.testing.assert_allclose(clover.Dphi_clover(T, L, -0.2, 0.0, R, psi, BC),
                                oracle.Dphi(T, L, 3, -0.2, R, psi, BC), atol=1e-13)
+
+
+def test_clover_schur_form_against_dense_matrix(oracle):
+    """Eq 43 for the clover operator: build the dense matrix of Dphi_clover column by column on 4x2^3, take the Schur
+    complement D_ee - D_eo D_oo^{-1} D_oe with numpy's dense solver on the full odd block, compare with the oracle's
+    site-by-site version; and det D = det D_oo det D_hat (Eq 42)."""
+    from oracle import dense
+    T, L, n, rep = 4, 2, 2, FUND
+    _, _, R, psi, _ = random_problem(oracle, T, L, n, rep, 8)
+    m0, csw = 0.3, 1.1
+    V, d = T * L ** 3, 2
+    N = V * 4 * d
+    D = np.zeros((N, N), dtype=complex)
+    for k in range(N):
+        e = np.zeros(N, dtype=complex)
+        e[k] = 1
+        D[:, k] = clover.Dphi_clover(T, L, m0, csw, R, e.reshape(V, 4, d), BC).reshape(-1)
+    ie, io = dense.parity_index(T, L, d, 0), dense.parity_index(T, L, d, 1)
+    Dee, Deo, Doe, Doo = D[np.ix_(ie, ie)], D[np.ix_(ie, io)], D[np.ix_(io, ie)], D[np.ix_(io, io)]
+    S = Dee - Deo @ np.linalg.solve(Doo, Doe)
+    ev = synth.parity_sites(T, L, 0)
+    got = clover.Dphi_clover_hat(T, L, m0, csw, R, psi[ev], BC).reshape(-1)
+    want = S @ psi[ev].reshape(-1)
+    assert np.linalg.norm(got - want) < 1e-12 * np.linalg.norm(want)
+    s1, l1 = np.linalg.slogdet(D)
+    s2, l2 = np.linalg.slogdet(Doo)
+    s3, l3 = np.linalg.slogdet(S)
+    assert abs(l1 - l2 - l3) < 1e-9 and abs(s1 - s2 * s3) < 1e-9
+    # the inverse of the diagonal blocks undoes Cphi
+    back = clover.Cphi_inv(T, L, m0, csw, R, clover.Cphi(T, L, m0, csw, R, psi))
+    np.testing.assert_allclose(back, psi, atol=1e-12)
