@@ -212,6 +212,19 @@ int hirep_clover_field(hirep_geom *g, void *clover, const void *links_rep);
 int hirep_clover_export(hirep_geom *g, void *canonical_out, const void *clover);
 int hirep_Cphi(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *clover);
 int hirep_Dphi_clover(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *links, const void *clover);
+/* The even-odd form Eq 43 (L803) with the clover blocks of Eq 47: D_hat = D_ee - D_eo D_oo^{-1} D_oe on the even sites.
+ *   hirep_clover_inv_field  inv <- ((4+m) + c_sw A_c)^{-1} for every site of ONE parity and both chiralities: the full
+ *                           (2 d_R) x (2 d_R) blocks, native, caller-owned buffer of hirep_clover_inv_bytes() bytes.  In-place
+ *                           Gauss-Jordan without pivoting: the blocks must be positive definite ((4+m) dominating c_sw |A|, the
+ *                           regime the operator is used in); depends on m0 and c_sw, so once per gauge update AND mass.
+ *   hirep_Cphi_inv          out_half = that block inverse applied to in_half (spinors of the parity `inv` was built for)
+ *   hirep_Dphi_clover_hat   out_even = D_ee in_even - D_eo D_oo^{-1} D_oe in_even; inv_odd = hirep_clover_inv_field(.., HIREP_ODD, ..)
+ *                           for the same m0, csw; four launches (D_oe, D_oo^{-1}, D_ee, D_eo accumulated in place); out != in. */
+int hirep_clover_inv_bytes(const hirep_geom *g, size_t *bytes);
+int hirep_clover_inv_field(hirep_geom *g, double m0, double csw, int parity, void *inv, const void *clover);
+int hirep_Cphi_inv(hirep_geom *g, void *out_half, const void *in_half, const void *inv);
+int hirep_Dphi_clover_hat(hirep_geom *g, double m0, double csw, void *out_even, const void *in_even, const void *links,
+                          const void *clover, const void *inv_odd);
 
 /* Measurement utility: achieved TFLOP/s (2 flops per FMA) of a register-resident chain of
  * FMAs in the given precision on the current device, the ALU roofline the pipe utilisation is read against.

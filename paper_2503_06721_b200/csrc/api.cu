@@ -395,12 +395,12 @@ extern "C" int hirep_clover_export(hirep_geom *g, void *canonical_out, const voi
 extern "C" int hirep_Cphi(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *clover) {
     CHECK_PTRS("hirep_Cphi", out_full, in_full, clover);
     if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Cphi: out aliases in");
-    return kern_result(g, k_cphi(g->geo, g->prec, g->dR, 4.0 + m0, csw, clover, in_full, out_full, g->stream), "hirep_Cphi");
+    return kern_result(g, k_cphi(g->prec, g->dR, 2 * g->geo.n_tiles, 4.0 + m0, csw, clover, in_full, out_full, g->stream), "hirep_Cphi");
 }
 extern "C" int hirep_Dphi_clover(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *links, const void *clover) {
     CHECK_PTRS("hirep_Dphi_clover", out_full, in_full, links, clover);
     if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Dphi_clover: out aliases in");
-    int rc = kern_result(g, k_cphi(g->geo, g->prec, g->dR, 4.0 + m0, csw, clover, in_full, out_full, g->stream), "hirep_Dphi_clover (diagonal term)");
+    int rc = kern_result(g, k_cphi(g->prec, g->dR, 2 * g->geo.n_tiles, 4.0 + m0, csw, clover, in_full, out_full, g->stream), "hirep_Dphi_clover (diagonal term)");
     if (rc) return rc;
     // out = 1 * out - 1/2 hop(in): every site's own value is read before it is written, by the same tile
     const size_t hb = g->bytes_spinor_half;
@@ -415,6 +415,46 @@ extern "C" int hirep_Dphi_clover(hirep_geom *g, double m0, double csw, void *out
 }
 
 // ---- spinor linear algebra, reductions, CG ------------------------------------------
+// the Schur form Eq 43 with the clover blocks: out_e = D_ee in_e - D_eo D_oo^{-1} D_oe in_e
+extern "C" int hirep_clover_inv_bytes(const hirep_geom *g, size_t *bytes) {
+    if (!g || !bytes) return fail(HIREP_EINVAL, "hirep_clover_inv_bytes: NULL argument");
+    *bytes = clover_bytes(g);   // one parity, (2 d_R)^2 = 4 d_R^2 per chirality: the same count as the H,B field of both parities
+    return HIREP_OK;
+}
+extern "C" int hirep_clover_inv_field(hirep_geom *g, double m0, double csw, int parity, void *inv, const void *clover) {
+    CHECK_PTRS("hirep_clover_inv_field", inv, clover);
+    if (parity != HIREP_EVEN && parity != HIREP_ODD) return fail(HIREP_EINVAL, "hirep_clover_inv_field: parity=%d", parity);
+    if (inv == clover) return fail(HIREP_EINVAL, "hirep_clover_inv_field: inv aliases clover");
+    return kern_result(g, k_clover_inv(g->geo, g->prec, g->dR, parity, 4.0 + m0, csw, clover, inv, g->stream), "hirep_clover_inv_field");
+}
+extern "C" int hirep_Cphi_inv(hirep_geom *g, void *out_half, const void *in_half, const void *inv) {
+    CHECK_PTRS("hirep_Cphi_inv", out_half, in_half, inv);
+    if (out_half == in_half) return fail(HIREP_EINVAL, "hirep_Cphi_inv: out aliases in");
+    return kern_result(g, k_cblock(g->prec, g->dR, g->geo.n_tiles, inv, in_half, out_half, g->stream), "hirep_Cphi_inv");
+}
+extern "C" int hirep_Dphi_clover_hat(hirep_geom *g, double m0, double csw, void *out_even, const void *in_even, const void *links,
+                                     const void *clover, const void *inv_odd) {
+    CHECK_PTRS("hirep_Dphi_clover_hat", out_even, in_even, links, clover, inv_odd);
+    if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_Dphi_clover_hat: out aliases in");
+    int rc = workspace(&g->ws_half, g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = workspace(&g->ws_half2, g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = offdiag(g, g->ws_half, in_even, links, 1, "hirep_Dphi_clover_hat (D_oe pass)");
+    if (rc) return rc;
+    rc = kern_result(g, k_cblock(g->prec, g->dR, g->geo.n_tiles, inv_odd, g->ws_half, g->ws_half2, g->stream), "hirep_Dphi_clover_hat (D_oo^-1)");
+    if (rc) return rc;
+    rc = kern_result(g, k_cphi(g->prec, g->dR, g->geo.n_tiles, 4.0 + m0, csw, clover, in_even, out_even, g->stream), "hirep_Dphi_clover_hat (D_ee)");
+    if (rc) return rc;
+    HopLaunch L{};
+    L.nsets = 1;
+    L.set[0] = HopSet{g->ws_half2, out_even, out_even, links_parity(g, links, 0), 0};
+    L.a = 1.0;
+    L.b = +0.5;   // - D_eo = -(-1/2) hop
+    L.g5 = 0;
+    return hop(g, L, "hirep_Dphi_clover_hat (D_eo pass)");
+}
+
 static long spinor_elems(const hirep_geom *g, int which) {   // complex elements of a native buffer, padding included
     return (long)g->geo.n_tiles * 4 * g->dR * TILE * (which == HIREP_FULL ? 2 : 1);
 }

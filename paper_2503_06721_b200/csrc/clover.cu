@@ -307,8 +307,7 @@ template <typename T, int DR> static int cphi_site_t(int ntile, double a, double
                                                                                  (cplx<T> *)out);
     return (int)cudaGetLastError();
 }
-template <typename T> static int cphi_t(const Geo &g, int dR, double a, double csw, const void *clover, const void *in, void *out, cudaStream_t s) {
-    const int ntile = 2 * g.n_tiles;
+template <typename T> static int cphi_t(int ntile, int dR, double a, double csw, const void *clover, const void *in, void *out, cudaStream_t s) {
     switch (dR) {
     case 2: return cphi_site_t<T, 2>(ntile, a, csw, clover, in, out, s);
     case 3: return cphi_site_t<T, 3>(ntile, a, csw, clover, in, out, s);
@@ -318,13 +317,146 @@ template <typename T> static int cphi_t(const Geo &g, int dR, double a, double c
     case 8: return cphi_site_t<T, 8>(ntile, a, csw, clover, in, out, s);
     case 10: return cphi_site_t<T, 10>(ntile, a, csw, clover, in, out, s);
     }
-    const int wy = 2 * dR < 8 ? 2 * dR : 8;      // 8 warps per CTA, 3 CTAs per SM (one 16-warp CTA per SM was latency bound: 2.9 TB/s)
+    const int wy = 2 * dR < 8 ? 2 * dR : 8;      // 8 warps per CTA, 3-4 CTAs per SM (one 16-warp CTA per SM was latency bound: 2.9 TB/s)
     int grid = ntile < 148 * 16 ? ntile : 148 * 16;   // (one CTA per SM measured slower: 4.7 vs 4.1 ms at d_R = 35 fp64)
     cphi_kernel<T><<<grid, dim3(TILE, wy), 0, s>>>(ntile, dR, (T)a, (T)csw, (const cplx<T> *)clover, (const cplx<T> *)in, (cplx<T> *)out);
     return (int)cudaGetLastError();
 }
-int k_cphi(const Geo &g, int prec, int dR, double a, double csw, const void *clover, const void *in, void *out, cudaStream_t s) {
-    return prec == 0 ? cphi_t<double>(g, dR, a, csw, clover, in, out, s) : cphi_t<float>(g, dR, a, csw, clover, in, out, s);
+// ntile tiles starting at the given pointers (2 n_tiles = full lattice; n_tiles with the parity's offsets = one half)
+int k_cphi(int prec, int dR, int ntile, double a, double csw, const void *clover, const void *in, void *out, cudaStream_t s) {
+    return prec == 0 ? cphi_t<double>(ntile, dR, a, csw, clover, in, out, s) : cphi_t<float>(ntile, dR, a, csw, clover, in, out, s);
+}
+
+// ---- inverse of the diagonal blocks, for the Schur form Eq 43 (L803) with the clover term ---------------------------
+// inv field of ONE parity: [tile][c][E = I*2dR + J][lane] complex<T>, the full (2 dR)^2 block of ((4+m) + c_sw A_c)^{-1}.
+// One thread per site and chirality: the block is written to the thread's own column of the output buffer (coalesced
+// across lanes) and inverted there in place by Gauss-Jordan elimination without pivoting -- the blocks are Hermitian and,
+// for the parameters the operator is used with ((4+m) dominates c_sw |A|), positive definite.  Once per gauge update.
+template <typename T>
+__global__ void clover_inv_kernel(Geo g, int dR, int parity, T a, T csw, const cplx<T> *__restrict__ clover, cplx<T> *inv) {
+    const int n = 2 * dR, ne = dR * dR;
+    const int slot = blockIdx.x * blockDim.x + threadIdx.x;      // padded site slot of the parity
+    const int c = blockIdx.y;
+    if (slot >= g.n_tiles * TILE) return;
+    const int tile = slot >> 5, lane = slot & 31;
+    cplx<T> *M = inv + ((size_t)(tile * 2 + c) * n * n) * TILE + lane;
+    const bool live = slot < g.Nh;
+    for (int I = 0; I < n; ++I)
+        for (int J = 0; J < n; ++J) {
+            const int bi = I / dR, i = I - bi * dR, bj = J / dR, j = J - bj * dR;
+            cplx<T> v;
+            if (bi == bj) {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 0, i * dR + j, lane, ne)];
+                if (bi) { v.x = -v.x; v.y = -v.y; }
+            } else if (bi == 0) {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 1, i * dR + j, lane, ne)];
+            } else {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 1, j * dR + i, lane, ne)];
+                v.y = -v.y;
+            }
+            v.x *= csw; v.y *= csw;
+            if (I == J) v.x += a;
+            if (!live) v = mk<T>(I == J ? T(1) : T(0), T(0));    // padding lanes: identity, inverted harmlessly, zeroed below
+            M[(size_t)(I * n + J) * TILE] = v;
+        }
+    for (int k = 0; k < n; ++k) {
+        const cplx<T> d = M[(size_t)(k * n + k) * TILE];
+        const T r = T(1) / (d.x * d.x + d.y * d.y);
+        const cplx<T> p = mk<T>(d.x * r, -d.y * r);
+        M[(size_t)(k * n + k) * TILE] = mk<T>(1, 0);
+        for (int J = 0; J < n; ++J) M[(size_t)(k * n + J) * TILE] = cmul<T>(M[(size_t)(k * n + J) * TILE], p);
+        for (int I = 0; I < n; ++I) {
+            if (I == k) continue;
+            const cplx<T> f = M[(size_t)(I * n + k) * TILE];
+            M[(size_t)(I * n + k) * TILE] = mk<T>(0, 0);
+            for (int J = 0; J < n; ++J) {
+                const cplx<T> x = M[(size_t)(k * n + J) * TILE];
+                cplx<T> y = M[(size_t)(I * n + J) * TILE];
+                y.x -= f.x * x.x - f.y * x.y;
+                y.y -= f.x * x.y + f.y * x.x;
+                M[(size_t)(I * n + J) * TILE] = y;
+            }
+        }
+    }
+    if (!live)
+        for (int E = 0; E < n * n; ++E) M[(size_t)E * TILE] = mk<T>(0, 0);
+}
+
+// out = block * in per chirality with the full (2 dR)^2 blocks of one parity (n_tiles tiles).
+template <typename T, int DR>
+__global__ void __launch_bounds__(128) cblock_site_kernel(int ntile, const cplx<T> *__restrict__ blk, const cplx<T> *__restrict__ in,
+                                                          cplx<T> *__restrict__ out) {
+    constexpr int N = 2 * DR, NCOMP = 4 * DR;
+    const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+    for (int tile = blockIdx.x * wpb + (threadIdx.x >> 5); tile < ntile; tile += gridDim.x * wpb) {
+        const cplx<T> *psi = in + (size_t)tile * NCOMP * TILE + lane;
+        cplx<T> *o = out + (size_t)tile * NCOMP * TILE + lane;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            const cplx<T> *M = blk + (size_t)(tile * 2 + c) * N * N * TILE + lane;
+            cplx<T> v[N];
+#pragma unroll
+            for (int J = 0; J < N; ++J) v[J] = __ldg(psi + (size_t)(c * N + J) * TILE);
+#pragma unroll
+            for (int I = 0; I < N; ++I) {
+                cplx<T> s = mk<T>(0, 0);
+#pragma unroll
+                for (int J = 0; J < N; ++J) cfma<T>(s, __ldcs(M + (size_t)(I * N + J) * TILE), v[J]);
+                __stcs(o + (size_t)(c * N + I) * TILE, s);
+            }
+        }
+    }
+}
+// any d_R: warp y of block (32, WY) computes rows (c, I) = y, y + WY, ... of the block's tile
+template <typename T>
+__global__ void __launch_bounds__(256, sizeof(T) == 8 ? 4 : 3) cblock_kernel(int ntile, int dR, const cplx<T> *__restrict__ blk,
+                                                                             const cplx<T> *__restrict__ in, cplx<T> *__restrict__ out) {
+    const int n = 2 * dR, ncomp = 4 * dR, lane = threadIdx.x;
+    for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
+        const cplx<T> *psi = in + (size_t)tile * ncomp * TILE + lane;
+        cplx<T> *o = out + (size_t)tile * ncomp * TILE + lane;
+        for (int q = threadIdx.y; q < 2 * n; q += blockDim.y) {
+            const int c = q / n, I = q - c * n;
+            const cplx<T> *M = blk + ((size_t)(tile * 2 + c) * n * n + (size_t)I * n) * TILE + lane;
+            const cplx<T> *v = psi + (size_t)c * n * TILE;
+            cplx<T> s0 = mk<T>(0, 0), s1 = mk<T>(0, 0);
+            int J = 0;
+#pragma unroll 4
+            for (; J + 1 < n; J += 2) {
+                cfma<T>(s0, __ldg(M + (size_t)J * TILE), __ldg(v + (size_t)J * TILE));
+                cfma<T>(s1, __ldg(M + (size_t)(J + 1) * TILE), __ldg(v + (size_t)(J + 1) * TILE));
+            }
+            __stcs(o + (size_t)(c * n + I) * TILE, mk<T>(s0.x + s1.x, s0.y + s1.y));
+        }
+    }
+}
+
+template <typename T, int DR> static int cblock_site_t(int ntile, const void *blk, const void *in, void *out, cudaStream_t s) {
+    const int blocks = (ntile + 3) / 4;
+    cblock_site_kernel<T, DR><<<blocks < 148 * 16 ? blocks : 148 * 16, 128, 0, s>>>(ntile, (const cplx<T> *)blk, (const cplx<T> *)in, (cplx<T> *)out);
+    return (int)cudaGetLastError();
+}
+template <typename T> static int cblock_t(int ntile, int dR, const void *blk, const void *in, void *out, cudaStream_t s) {
+    switch (dR) {
+    case 2: return cblock_site_t<T, 2>(ntile, blk, in, out, s);
+    case 3: return cblock_site_t<T, 3>(ntile, blk, in, out, s);
+    case 4: return cblock_site_t<T, 4>(ntile, blk, in, out, s);
+    case 5: return cblock_site_t<T, 5>(ntile, blk, in, out, s);
+    case 6: return cblock_site_t<T, 6>(ntile, blk, in, out, s);
+    }
+    const int wy = 4 * dR < 8 ? 4 * dR : 8;
+    cblock_kernel<T><<<ntile < 148 * 16 ? ntile : 148 * 16, dim3(TILE, wy), 0, s>>>(ntile, dR, (const cplx<T> *)blk, (const cplx<T> *)in, (cplx<T> *)out);
+    return (int)cudaGetLastError();
+}
+int k_cblock(int prec, int dR, int ntile, const void *blk, const void *in, void *out, cudaStream_t s) {
+    return prec == 0 ? cblock_t<double>(ntile, dR, blk, in, out, s) : cblock_t<float>(ntile, dR, blk, in, out, s);
+}
+template <typename T> static int clover_inv_t(const Geo &g, int dR, int parity, double a, double csw, const void *clover, void *inv, cudaStream_t s) {
+    clover_inv_kernel<T><<<dim3((g.n_tiles * TILE + 63) / 64, 2), 64, 0, s>>>(g, dR, parity, (T)a, (T)csw, (const cplx<T> *)clover, (cplx<T> *)inv);
+    return (int)cudaGetLastError();
+}
+int k_clover_inv(const Geo &g, int prec, int dR, int parity, double a, double csw, const void *clover, void *inv, cudaStream_t s) {
+    return prec == 0 ? clover_inv_t<double>(g, dR, parity, a, csw, clover, inv, s) : clover_inv_t<float>(g, dR, parity, a, csw, clover, inv, s);
 }
 
 template <typename T> static int clover_export_t(const Geo &g, int dR, void *canon, const void *clover, cudaStream_t s) {

@@ -48,7 +48,10 @@ int k_fma_peak(int prec, double *tflops, cudaStream_t s);   // fma_peak.cu: meas
 // clover.cu: clover term (Eq 47-49); native clover field = 4 dR^2 complex per site
 int k_clover_field(const Geo &g, int prec, int dR, int real, void *clover, const void *links_rep, cudaStream_t s);
 int k_clover_export(const Geo &g, int prec, int dR, void *canon, const void *clover, cudaStream_t s);
-int k_cphi(const Geo &g, int prec, int dR, double a, double csw, const void *clover, const void *in, void *out, cudaStream_t s);
+int k_cphi(int prec, int dR, int ntile, double a, double csw, const void *clover, const void *in, void *out, cudaStream_t s);
+// inverse diagonal blocks of one parity ((2 dR)^2 complex per site and chirality) and their application
+int k_clover_inv(const Geo &g, int prec, int dR, int parity, double a, double csw, const void *clover, void *inv, cudaStream_t s);
+int k_cblock(int prec, int dR, int ntile, const void *blk, const void *in, void *out, cudaStream_t s);
 // number of distinct kernel launches k_hop issues for this configuration (for launch accounting): always 1.
 
 }  // namespace hirep

@@ -34,6 +34,7 @@ SYMBOLS = [
     "hirep_spinor_max_norm", "hirep_cg_g5Dphi_sq", "hirep_spinor_g5_lc", "hirep_spinor_gamma", "hirep_spinor_g5_lc_add_assign", "hirep_spinor_g5_prod", "hirep_Dphi_tm", "hirep_Dphi_tm_sq",
     "hirep_Dphi_tm_hat", "hirep_cg_Dphi_tm_sq", "hirep_cg_mshift_g5Dphi_sq", "hirep_bicgstab", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
     "hirep_clover_bytes", "hirep_clover_field", "hirep_clover_export", "hirep_Cphi", "hirep_Dphi_clover",
+    "hirep_clover_inv_bytes", "hirep_clover_inv_field", "hirep_Cphi_inv", "hirep_Dphi_clover_hat",
 ]
 
 
@@ -109,6 +110,10 @@ def load():
     lib.hirep_clover_export.argtypes = [vp, vp, vp]
     lib.hirep_Cphi.argtypes = [vp, cd, cd, vp, vp, vp]
     lib.hirep_Dphi_clover.argtypes = [vp, cd, cd, vp, vp, vp, vp]
+    lib.hirep_clover_inv_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t)]
+    lib.hirep_clover_inv_field.argtypes = [vp, cd, cd, ci, vp, vp]
+    lib.hirep_Cphi_inv.argtypes = [vp, vp, vp, vp]
+    lib.hirep_Dphi_clover_hat.argtypes = [vp, cd, cd, vp, vp, vp, vp, vp]
     lib.hirep_sync.argtypes = [vp]
     lib.hirep_last_error.restype = ctypes.c_char_p
     for n in SYMBOLS:
@@ -239,6 +244,15 @@ def hirep_clover_field(g, clover, links_rep): _check(load().hirep_clover_field(g
 def hirep_clover_export(g, canonical, clover): _check(load().hirep_clover_export(g, canonical, clover))
 def hirep_Cphi(g, m0, csw, out, inp, clover): _check(load().hirep_Cphi(g, m0, csw, out, inp, clover))
 def hirep_Dphi_clover(g, m0, csw, out, inp, links, clover): _check(load().hirep_Dphi_clover(g, m0, csw, out, inp, links, clover))
+def hirep_clover_inv_bytes(g) -> int:
+    n = ctypes.c_size_t(0)
+    _check(load().hirep_clover_inv_bytes(g, ctypes.byref(n)))
+    return n.value
+
+
+def hirep_clover_inv_field(g, m0, csw, parity, inv, clover): _check(load().hirep_clover_inv_field(g, m0, csw, parity, inv, clover))
+def hirep_Cphi_inv(g, out, inp, inv): _check(load().hirep_Cphi_inv(g, out, inp, inv))
+def hirep_Dphi_clover_hat(g, m0, csw, out, inp, links, clover, inv_odd): _check(load().hirep_Dphi_clover_hat(g, m0, csw, out, inp, links, clover, inv_odd))
 def hirep_Dphi_tm_hat(g, m0, mu, out, inp, links): _check(load().hirep_Dphi_tm_hat(g, m0, mu, out, inp, links))
 
 
@@ -467,6 +481,22 @@ class Geometry:
     def Dphi_clover(self, m0, csw, inp, links, clover, out=None):
         out = self.new_spinor(FULL) if out is None else out
         hirep_Dphi_clover(self.handle, m0, csw, out.data_ptr(), inp.data_ptr(), links.data_ptr(), clover.data_ptr())
+        return out
+
+    def clover_inv_field(self, m0, csw, parity, clover, out=None):
+        if out is None:
+            out = self.torch.empty(hirep_clover_inv_bytes(self.handle), dtype=self.torch.uint8, device=self.device)
+        hirep_clover_inv_field(self.handle, m0, csw, parity, out.data_ptr(), clover.data_ptr())
+        return out
+
+    def Cphi_inv(self, parity, inp_half, inv, out=None):
+        out = self.new_spinor(parity) if out is None else out
+        hirep_Cphi_inv(self.handle, out.data_ptr(), inp_half.data_ptr(), inv.data_ptr())
+        return out
+
+    def Dphi_clover_hat(self, m0, csw, inp_even, links, clover, inv_odd, out=None):
+        out = self.new_spinor(EVEN) if out is None else out
+        hirep_Dphi_clover_hat(self.handle, m0, csw, out.data_ptr(), inp_even.data_ptr(), links.data_ptr(), clover.data_ptr(), inv_odd.data_ptr())
         return out
 
     def cg_mshift_g5Dphi_sq(self, m0, shifts, b, links, tol, maxiter):

@@ -79,3 +79,44 @@ def test_clover_needs_stored_links(env):
     p.geom.set_link_mode(hirep.LINKS_REBUILD)
     with pytest.raises(hirep.HirepError):
         p.geom.clover_field(p.links_fund)
+
+
+@pytest.mark.parametrize("name,T,L", CASES)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_clover_schur_form(env, name, T, L, prec):
+    """Eq 43 with the clover blocks: the block inverse (D_oo^{-1} and D_ee^{-1}) and Dphi_clover_hat against the oracle.
+    c_sw = 0.5 keeps the blocks positive definite on Haar-random links ((4+m) >= 3.5 against c_sw |A| <= 1.5)."""
+    from oracle import clover as oc
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS[name].resized(T, L)
+    p = Problem(env, cfg, prec)
+    g, m0, tol, csw = p.geom, cfg.m0, TOL[prec], 0.5
+    cl = g.clover_field(p.links_rep)
+    psi = p.spinors[0]
+    for parity, sites in ((hirep.ODD, p.od), (hirep.EVEN, p.ev)):
+        inv = g.clover_inv_field(m0, csw, parity, cl)
+        got = p.to_numpy(g.Cphi_inv(parity, p.to_native(psi[sites], parity), inv), parity)
+        assert oracle.rel_l2(got, oc.Cphi_inv(T, L, m0, csw, p.R, psi[sites], sites=sites)) < tol
+    inv_odd = g.clover_inv_field(m0, csw, hirep.ODD, cl)
+    xe = p.to_native(psi[p.ev], hirep.EVEN)
+    got = p.to_numpy(g.Dphi_clover_hat(m0, csw, xe, p.links_rep, cl, inv_odd), hirep.EVEN)
+    assert oracle.rel_l2(got, oc.Dphi_clover_hat(T, L, m0, csw, p.R, psi[p.ev], BC)) < tol
+
+
+def test_clover_schur_form_other_representations(env):
+    """d_R = 8 and 10 (generic block kernel) and c_sw = 0: (4+m) D_hat_clover = the Wilson Dphi_hat of Eq 44."""
+    from oracle import clover as oc
+    hirep, oracle = env["hirep"], env["oracle"]
+    for n, rep, T, L in [(3, 1, 2, 4), (4, 2, 2, 4)]:
+        cfg = synth.Config("t", T, L, n, rep, -0.1, "haar", 23, ())
+        p = Problem(env, cfg, "f64")
+        cl = p.geom.clover_field(p.links_rep)
+        psi = p.spinors[0]
+        xe = p.to_native(psi[p.ev], hirep.EVEN)
+        inv = p.geom.clover_inv_field(cfg.m0, 0.4, hirep.ODD, cl)
+        got = p.to_numpy(p.geom.Dphi_clover_hat(cfg.m0, 0.4, xe, p.links_rep, cl, inv), hirep.EVEN)
+        assert oracle.rel_l2(got, oc.Dphi_clover_hat(T, L, cfg.m0, 0.4, p.R, psi[p.ev], BC)) < 1e-13
+        inv0 = p.geom.clover_inv_field(cfg.m0, 0.0, hirep.ODD, cl)
+        a = p.to_numpy(p.geom.Dphi_clover_hat(cfg.m0, 0.0, xe, p.links_rep, cl, inv0), hirep.EVEN)
+        b = oracle.Dphi_hat(T, L, cfg.d_R, cfg.m0, p.R, psi[p.ev], BC)
+        assert oracle.rel_l2((4.0 + cfg.m0) * a, b) < 1e-13
