@@ -384,7 +384,7 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
     # NEXT-2, second part: clover term (Eq 47-49).  Algorithmic bytes per site: clover field 4 d^2 complex + spinor in/out.
     d = cfg.d_R
     cb = S * d                                          # clover bytes per site: 4 d^2 complex (S = 4 d complex)
-    if torch.cuda.mem_get_info()[0] < cb * V + (4 << 30):
+    if torch.cuda.mem_get_info()[0] < 2 * cb * V + (4 << 30):
         out["clover"] = {"skipped": "clover field of %.1f GB does not fit beside the resident fields" % (cb * V / 1e9)}
     else:
         lbytes = geom.sizes["links_rep"] / V            # represented-link bytes per site
@@ -397,7 +397,19 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
         ms = timeit(lambda: geom.Dphi_clover(m0, 1.0, x_full, lr, cl, out=y_full), reps=10)
         by = (cb + 2 * S + lbytes + 3 * S) * V
         out["Dphi_clover"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3), "launches": 2}
-        del cl
+        # the Schur form Eq 43 with these blocks: block inverse (once per gauge update and mass), its application, D_hat
+        hb = geom.sizes["spinor_half"]
+        x_e, y_e = x_full[:hb], y_full[:hb]
+        inv = geom.clover_inv_field(m0, 0.5, hirep.ODD, cl)
+        ms = timeit(lambda: geom.clover_inv_field(m0, 0.5, hirep.ODD, cl, out=inv), reps=3)
+        out["clover_inv_field"] = {"ms": round(ms, 3), "note": "in-place Gauss-Jordan of the 2 d_R x 2 d_R blocks of the odd sites"}
+        ms = timeit(lambda: geom.Cphi_inv(hirep.ODD, x_e, inv, out=y_e))
+        by = (2 * cb + 2 * S) * V / 2                    # full blocks: 8 d^2 complex per site, one parity
+        out["Cphi_inv"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3)}
+        ms = timeit(lambda: geom.Dphi_clover_hat(m0, 0.5, x_e, lr, cl, inv, out=y_e), reps=10)
+        by = cm["ops"]["Dphi_eo"][1] * 2 + S * V / 2 + (2 * cb + 2 * S) * V / 2 + (cb + 2 * S) * V / 2
+        out["Dphi_clover_hat"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3), "launches": 4}
+        del cl, inv
     try:
         out["fma_peak_tflops"] = {"f64": round(hirep.hirep_fma_peak(hirep.F64), 2), "f32": round(hirep.hirep_fma_peak(hirep.F32), 2)}
     except Exception as e:   # measurement utility only
