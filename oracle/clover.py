@@ -152,3 +152,39 @@ def Dphi_clover_hat(T, L, m0, csw, Rlinks, psi_even, bc):
     t = _o.Dphi_oe(T, L, d, Rlinks, psi_even, bc)
     u = Cphi_inv(T, L, m0, csw, Rlinks, t, sites=od)
     return dee - _o.Dphi_eo(T, L, d, Rlinks, u, bc)
+
+
+def exp_blocks(T, L, m0, csw, Rlinks, inverse=False):
+    """Exponential clover (Eq 50): the site-diagonal blocks (4+m0) exp(c_sw/(4+m0) A_c), [V, 2, 2d, 2d], through the
+    Hermitian eigendecomposition A_c = V diag(lambda) V^+ (exp of a Hermitian matrix by its definition on the spectrum);
+    inverse=True gives their inverses exp(-c_sw/(4+m0) A_c)/(4+m0)."""
+    A = chiral_blocks(T, L, Rlinks)
+    lam, vec = np.linalg.eigh(A)
+    x = csw / (4.0 + m0) * lam
+    f = np.exp(-x) / (4.0 + m0) if inverse else (4.0 + m0) * np.exp(x)
+    return np.einsum("xcik,xck,xcjk->xcij", vec, f, np.conj(vec))
+
+
+def apply_blocks(blocks, psi):
+    """Site-diagonal chirality blocks [n, 2, 2d, 2d] applied to spinors [n, 4, d]."""
+    psi = np.asarray(psi, dtype=np.complex128)
+    n, _, d = psi.shape
+    return np.einsum("xcij,xcj->xci", blocks, psi.reshape(n, 2, 2 * d)).reshape(n, 4, d)
+
+
+def Dphi_expclover(T, L, m0, csw, Rlinks, psi, bc):
+    """Eq 8 with the diagonal term of Eq 50."""
+    from . import oracle as _o
+    d = Rlinks.shape[-1]
+    return _o.hop_field(T, L, d, Rlinks, psi, bc) + apply_blocks(exp_blocks(T, L, m0, csw, Rlinks), psi)
+
+
+def Dphi_expclover_hat(T, L, m0, csw, Rlinks, psi_even, bc):
+    """Eq 43 with the blocks of Eq 50: D_ee psi_e - D_eo D_oo^{-1} D_oe psi_e."""
+    from . import oracle as _o
+    d = Rlinks.shape[-1]
+    ev, od = _parity_sites(T, L, 0), _parity_sites(T, L, 1)
+    E = exp_blocks(T, L, m0, csw, Rlinks)
+    Einv = exp_blocks(T, L, m0, csw, Rlinks, inverse=True)
+    t = _o.Dphi_oe(T, L, d, Rlinks, psi_even, bc)
+    return apply_blocks(E[ev], psi_even) - _o.Dphi_eo(T, L, d, Rlinks, apply_blocks(Einv[od], t), bc)

@@ -171,3 +171,56 @@ def test_clover_schur_form_against_dense_matrix(oracle):
     # the inverse of the diagonal blocks undoes Cphi
     back = clover.Cphi_inv(T, L, m0, csw, R, clover.Cphi(T, L, m0, csw, R, psi))
     np.testing.assert_allclose(back, psi, atol=1e-12)
+
+
+def test_exponential_clover_blocks(oracle):
+    """Eq 50: closed forms and expansions.  det = (4+m)^(2d) (A traceless), E(c_sw) E^{-1}(c_sw) = 1, c_sw = 0 gives (4+m),
+    the expansion to second order in c_sw agrees with (4+m) + c_sw A + c_sw^2 A^2 / (2(4+m)) up to O(c_sw^3), an
+    independent Taylor series of the exponential (40 terms, plain matrix products), and the constant abelian background
+    where exp(-x sigma_01) = cosh x - sigma_01 sinh x."""
+    T, L, n, rep = 4, 2, 3, FUND
+    _, _, R, psi, _ = random_problem(oracle, T, L, n, rep, 12)
+    m0, csw = -0.2, 1.3
+    A = clover.chiral_blocks(T, L, R)
+    E = clover.exp_blocks(T, L, m0, csw, R)
+    Ei = clover.exp_blocks(T, L, m0, csw, R, inverse=True)
+    nn = A.shape[-1]
+    eye = np.eye(nn)
+    np.testing.assert_allclose(np.linalg.det(E), (4 + m0) ** nn * np.ones(E.shape[:2]), rtol=1e-12)
+    np.testing.assert_allclose(E @ Ei, np.broadcast_to(eye, E.shape), atol=1e-13)
+    np.testing.assert_allclose(clover.exp_blocks(T, L, m0, 0.0, R), np.broadcast_to((4 + m0) * eye, E.shape), atol=1e-14)
+    eps = 1e-3
+    E2 = (4 + m0) * eye + eps * A + eps ** 2 * (A @ A) / (2 * (4 + m0))
+    assert np.abs(clover.exp_blocks(T, L, m0, eps, R) - E2).max() < 10 * eps ** 3
+    X = csw / (4 + m0) * A
+    term, ser = np.broadcast_to(eye, A.shape).astype(complex), np.broadcast_to(eye, A.shape).astype(complex)
+    for k in range(1, 40):
+        term = term @ X / k
+        ser = ser + term
+    np.testing.assert_allclose(E, (4 + m0) * ser, atol=1e-12)
+    # constant abelian background in the (0,1) plane: A = -(1/2) sin(phi) sigma_01, sigma_01^2 = 1
+    Ta, La = 6, 4
+    phi = 2 * np.pi / Ta
+    c = synth.site_coords(Ta, La)
+    theta = np.zeros((Ta * La ** 3, 4))
+    theta[:, 1] = phi * c[:, 0]
+    Eab = clover.exp_blocks(Ta, La, m0, csw, abelian_links(theta))
+    x = csw / (4 + m0) * 0.5 * np.sin(phi)
+    for cblk, s in ((0, S1), (1, -S1)):
+        want = (4 + m0) * (np.cosh(x) * np.eye(2) - np.sinh(x) * s)
+        np.testing.assert_allclose(Eab[:, cblk], np.broadcast_to(want, Eab[:, cblk].shape), atol=1e-13)
+    # operator level: gamma_5-Hermiticity of the full operator and the Schur form against its definition
+    g5 = np.array([1, 1, -1, -1])[None, :, None]
+    _, _, _, psi, phi_s = random_problem(oracle, T, L, n, rep, 12)
+    D = lambda v: clover.Dphi_expclover(T, L, m0, csw, R, v, BC)
+    lhs, rhs = np.vdot(phi_s, g5 * D(psi)), np.vdot(g5 * D(phi_s), psi)
+    assert abs(lhs - rhs) < 1e-11 * abs(lhs)
+    ev, od = synth.parity_sites(T, L, 0), synth.parity_sites(T, L, 1)
+    # solve D (x_e, x_o) = (b, 0) blockwise: D_hat x_e = b with x_o = -D_oo^{-1} D_oe x_e
+    xe = psi[ev]
+    xo = -clover.apply_blocks(Ei[od], oracle.Dphi_oe(T, L, 3, R, xe, BC))
+    full = np.zeros_like(psi)
+    full[ev], full[od] = xe, xo
+    out = D(full)
+    assert np.abs(out[od]).max() < 1e-12
+    np.testing.assert_allclose(out[ev], clover.Dphi_expclover_hat(T, L, m0, csw, R, xe, BC), atol=1e-12)
