@@ -226,6 +226,20 @@ int hirep_Cphi_inv(hirep_geom *g, void *out_half, const void *in_half, const voi
 int hirep_Dphi_clover_hat(hirep_geom *g, double m0, double csw, void *out_even, const void *in_even, const void *links,
                           const void *clover, const void *inv_odd);
 
+/* ---- exponential clover (Eq 50): D_ee,m + D_oo,m = (4+m0) exp(c_sw/(4+m0) (i/4) sum sigma F) ----
+ *   hirep_clover_exp_field  blocks <- (4+m0) exp(+c_sw/(4+m0) A_c) (inverse = 0) or its inverse exp(-c_sw/(4+m0) A_c)/(4+m0)
+ *                           (inverse = 1) for the sites of ONE parity: full (2 d_R)^2 blocks, same native layout and size
+ *                           (hirep_clover_inv_bytes) as hirep_clover_inv_field; scaling and squaring (2^4) of a 14-term
+ *                           Taylor sum, |c_sw A|/(4+m0) <= 8.  A buffer of 2 x that size holding the even blocks followed by
+ *                           the odd blocks is a full-lattice block field.
+ *   hirep_Dphi_blocks       out_full = blocks_full in_full - 1/2 hop(in_full): Eq 8 with ANY site-diagonal chirality blocks
+ *                           (the exponential clover's; also (4+m) + c_sw A written out as full blocks); out != in
+ *   hirep_Dphi_blocks_hat   out_even = blocks_even in_even - D_eo inv_blocks_odd D_oe in_even (Eq 43); four launches; out != in */
+int hirep_clover_exp_field(hirep_geom *g, double m0, double csw, int parity, int inverse, void *blocks, const void *clover);
+int hirep_Dphi_blocks(hirep_geom *g, void *out_full, const void *in_full, const void *links, const void *blocks_full);
+int hirep_Dphi_blocks_hat(hirep_geom *g, void *out_even, const void *in_even, const void *links, const void *blocks_even,
+                          const void *inv_blocks_odd);
+
 /* Measurement utility: achieved TFLOP/s (2 flops per FMA) of a register-resident chain of
  * FMAs in the given precision on the current device, the ALU roofline the pipe utilisation is read against.
  * Synchronous; tflops is a host pointer. */

@@ -27,6 +27,7 @@ struct hirep_geom {
     void *cg_r, *cg_p, *cg_Ap;      // CG work fields (lazy)
     void *ms_p[HIREP_MAX_SHIFTS];    // multi-shift CG direction fields (lazy)
     void *bi_s, *bi_t;              // BiCGstab work fields (lazy)
+    void *ws_exp;                   // hirep_clover_exp_field work matrices (lazy)
     // hirep_apply_host staging (lazy)
     void *h_links_canon, *h_links_fund, *h_links_rep, *h_in_canon, *h_in_native, *h_out_native, *h_out_canon, *h_out_canon2;
     cudaStream_t copy_stream;       // device -> host copies of hirep_apply_host[_async] (lazy)
@@ -102,7 +103,7 @@ extern "C" int hirep_geom_destroy(hirep_geom *g) {
     if (!g) return HIREP_OK;
     for (void *b : g->ms_p)
         if (b) cudaFree(b);
-    void *bufs[] = {g->ws_half, g->ws_half2, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
+    void *bufs[] = {g->ws_exp, g->ws_half, g->ws_half2, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
                     g->h_in_native, g->h_out_native, g->h_out_canon, g->h_out_canon2};
     if (g->host_events) {
         for (int i = 0; i < 2; ++i) { cudaEventDestroy(g->ev_done[i]); cudaEventDestroy(g->ev_copied[i]); }
@@ -453,6 +454,53 @@ extern "C" int hirep_Dphi_clover_hat(hirep_geom *g, double m0, double csw, void 
     L.b = +0.5;   // - D_eo = -(-1/2) hop
     L.g5 = 0;
     return hop(g, L, "hirep_Dphi_clover_hat (D_eo pass)");
+}
+
+// ---- exponential clover (Eq 50) and operators with general site-diagonal chirality blocks -----------------------
+extern "C" int hirep_clover_exp_field(hirep_geom *g, double m0, double csw, int parity, int inverse, void *blocks, const void *clover) {
+    CHECK_PTRS("hirep_clover_exp_field", blocks, clover);
+    if (parity != HIREP_EVEN && parity != HIREP_ODD) return fail(HIREP_EINVAL, "hirep_clover_exp_field: parity=%d", parity);
+    if (4.0 + m0 == 0.0) return fail(HIREP_EINVAL, "hirep_clover_exp_field: 4 + m0 = 0");
+    if (blocks == clover) return fail(HIREP_EINVAL, "hirep_clover_exp_field: blocks aliases clover");
+    int rc = workspace(&g->ws_exp, 2 * clover_bytes(g));
+    if (rc) return rc;
+    const double x = (inverse ? -1.0 : 1.0) * csw / (4.0 + m0), pref = inverse ? 1.0 / (4.0 + m0) : 4.0 + m0;
+    return kern_result(g, k_clover_exp(g->geo, g->prec, g->dR, parity, x, pref, clover, blocks, g->ws_exp, g->stream), "hirep_clover_exp_field");
+}
+extern "C" int hirep_Dphi_blocks(hirep_geom *g, void *out_full, const void *in_full, const void *links, const void *blocks_full) {
+    CHECK_PTRS("hirep_Dphi_blocks", out_full, in_full, links, blocks_full);
+    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Dphi_blocks: out aliases in");
+    int rc = kern_result(g, k_cblock(g->prec, g->dR, 2 * g->geo.n_tiles, blocks_full, in_full, out_full, g->stream), "hirep_Dphi_blocks (diagonal term)");
+    if (rc) return rc;
+    const size_t hb = g->bytes_spinor_half;
+    const char *in_e = (const char *)in_full, *in_o = in_e + hb;
+    char *out_e = (char *)out_full, *out_o = out_e + hb;
+    HopLaunch L{};
+    L.nsets = 2;
+    L.set[0] = HopSet{in_o, out_e, out_e, links_parity(g, links, 0), 0};
+    L.set[1] = HopSet{in_e, out_o, out_o, links_parity(g, links, 1), 1};
+    L.a = 1.0; L.b = -0.5; L.g5 = 0; L.am = 0.0;
+    return hop(g, L, "hirep_Dphi_blocks (hopping term)");
+}
+extern "C" int hirep_Dphi_blocks_hat(hirep_geom *g, void *out_even, const void *in_even, const void *links, const void *blocks_even,
+                                     const void *inv_blocks_odd) {
+    CHECK_PTRS("hirep_Dphi_blocks_hat", out_even, in_even, links, blocks_even, inv_blocks_odd);
+    if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_Dphi_blocks_hat: out aliases in");
+    int rc = workspace(&g->ws_half, g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = workspace(&g->ws_half2, g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = offdiag(g, g->ws_half, in_even, links, 1, "hirep_Dphi_blocks_hat (D_oe pass)");
+    if (rc) return rc;
+    rc = kern_result(g, k_cblock(g->prec, g->dR, g->geo.n_tiles, inv_blocks_odd, g->ws_half, g->ws_half2, g->stream), "hirep_Dphi_blocks_hat (D_oo^-1)");
+    if (rc) return rc;
+    rc = kern_result(g, k_cblock(g->prec, g->dR, g->geo.n_tiles, blocks_even, in_even, out_even, g->stream), "hirep_Dphi_blocks_hat (D_ee)");
+    if (rc) return rc;
+    HopLaunch L{};
+    L.nsets = 1;
+    L.set[0] = HopSet{g->ws_half2, out_even, out_even, links_parity(g, links, 0), 0};
+    L.a = 1.0; L.b = +0.5; L.g5 = 0;
+    return hop(g, L, "hirep_Dphi_blocks_hat (D_eo pass)");
 }
 
 static long spinor_elems(const hirep_geom *g, int which) {   // complex elements of a native buffer, padding included

@@ -451,6 +451,71 @@ template <typename T> static int cblock_t(int ntile, int dR, const void *blk, co
 int k_cblock(int prec, int dR, int ntile, const void *blk, const void *in, void *out, cudaStream_t s) {
     return prec == 0 ? cblock_t<double>(ntile, dR, blk, in, out, s) : cblock_t<float>(ntile, dR, blk, in, out, s);
 }
+// Exponential clover (Eq 50): blocks pref * exp(x A_c) of one parity, x = +-c_sw/(4+m0), pref = (4+m0) or 1/(4+m0)
+// (the inverse).  Per site and chirality, in the thread's own columns of global memory (S = output, X and Tm = workspace):
+// scaling and squaring, exp(Y) = (sum_{k <= K} (Y/2^s)^k / k!)^(2^s) with the sum in Horner form; s = 4, K = 14 covers
+// |x A| <= 8 to 1e-16 (truncation 0.5^15/15!) and the four squarings amplify rounding by 16 ulp.
+template <typename T>
+__global__ void clover_exp_kernel(Geo g, int dR, int parity, T x, T pref, const cplx<T> *__restrict__ clover, cplx<T> *blocks, cplx<T> *work) {
+    constexpr int SQ = 4, K = 14;
+    const int n = 2 * dR, ne = dR * dR;
+    const int slot = blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = blockIdx.y;
+    if (slot >= g.n_tiles * TILE) return;
+    const int tile = slot >> 5, lane = slot & 31;
+    const size_t off = ((size_t)(tile * 2 + c) * n * n) * TILE + lane;
+    cplx<T> *S = blocks + off, *X = work + off, *Tm = work + (size_t)g.n_tiles * 2 * n * n * TILE + off;
+    const bool live = slot < g.Nh;
+    const T sc = x / T(1 << SQ);
+    for (int I = 0; I < n; ++I)
+        for (int J = 0; J < n; ++J) {
+            const int bi = I / dR, i = I - bi * dR, bj = J / dR, j = J - bj * dR;
+            cplx<T> v;
+            if (bi == bj) {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 0, i * dR + j, lane, ne)];
+                if (bi) { v.x = -v.x; v.y = -v.y; }
+            } else if (bi == 0) {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 1, i * dR + j, lane, ne)];
+            } else {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 1, j * dR + i, lane, ne)];
+                v.y = -v.y;
+            }
+            X[(size_t)(I * n + J) * TILE] = mk<T>(sc * v.x, sc * v.y);
+            S[(size_t)(I * n + J) * TILE] = mk<T>(I == J ? T(1) : T(0), T(0));
+        }
+    for (int k = K; k >= 1; --k) {            // S <- 1 + (X S)/k
+        const T rk = T(1) / T(k);
+        for (int I = 0; I < n; ++I)
+            for (int J = 0; J < n; ++J) {
+                cplx<T> a = mk<T>(0, 0);
+                for (int l = 0; l < n; ++l) cfma<T>(a, X[(size_t)(I * n + l) * TILE], S[(size_t)(l * n + J) * TILE]);
+                Tm[(size_t)(I * n + J) * TILE] = mk<T>(a.x * rk + (I == J ? T(1) : T(0)), a.y * rk);
+            }
+        for (int E = 0; E < n * n; ++E) S[(size_t)E * TILE] = Tm[(size_t)E * TILE];
+    }
+    for (int q = 0; q < SQ; ++q) {            // S <- S S
+        for (int I = 0; I < n; ++I)
+            for (int J = 0; J < n; ++J) {
+                cplx<T> a = mk<T>(0, 0);
+                for (int l = 0; l < n; ++l) cfma<T>(a, S[(size_t)(I * n + l) * TILE], S[(size_t)(l * n + J) * TILE]);
+                Tm[(size_t)(I * n + J) * TILE] = a;
+            }
+        for (int E = 0; E < n * n; ++E) S[(size_t)E * TILE] = Tm[(size_t)E * TILE];
+    }
+    for (int E = 0; E < n * n; ++E) {
+        const cplx<T> v = S[(size_t)E * TILE];
+        S[(size_t)E * TILE] = live ? mk<T>(pref * v.x, pref * v.y) : mk<T>(0, 0);
+    }
+}
+template <typename T> static int clover_exp_t(const Geo &g, int dR, int parity, double x, double pref, const void *clover, void *blocks, void *work, cudaStream_t s) {
+    clover_exp_kernel<T><<<dim3((g.n_tiles * TILE + 63) / 64, 2), 64, 0, s>>>(g, dR, parity, (T)x, (T)pref, (const cplx<T> *)clover, (cplx<T> *)blocks,
+                                                                           (cplx<T> *)work);
+    return (int)cudaGetLastError();
+}
+int k_clover_exp(const Geo &g, int prec, int dR, int parity, double x, double pref, const void *clover, void *blocks, void *work, cudaStream_t s) {
+    return prec == 0 ? clover_exp_t<double>(g, dR, parity, x, pref, clover, blocks, work, s) : clover_exp_t<float>(g, dR, parity, x, pref, clover, blocks, work, s);
+}
+
 template <typename T> static int clover_inv_t(const Geo &g, int dR, int parity, double a, double csw, const void *clover, void *inv, cudaStream_t s) {
     clover_inv_kernel<T><<<dim3((g.n_tiles * TILE + 63) / 64, 2), 64, 0, s>>>(g, dR, parity, (T)a, (T)csw, (const cplx<T> *)clover, (cplx<T> *)inv);
     return (int)cudaGetLastError();

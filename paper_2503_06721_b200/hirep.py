@@ -35,6 +35,7 @@ SYMBOLS = [
     "hirep_Dphi_tm_hat", "hirep_cg_Dphi_tm_sq", "hirep_cg_mshift_g5Dphi_sq", "hirep_bicgstab", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
     "hirep_clover_bytes", "hirep_clover_field", "hirep_clover_export", "hirep_Cphi", "hirep_Dphi_clover",
     "hirep_clover_inv_bytes", "hirep_clover_inv_field", "hirep_Cphi_inv", "hirep_Dphi_clover_hat",
+    "hirep_clover_exp_field", "hirep_Dphi_blocks", "hirep_Dphi_blocks_hat",
 ]
 
 
@@ -114,6 +115,9 @@ def load():
     lib.hirep_clover_inv_field.argtypes = [vp, cd, cd, ci, vp, vp]
     lib.hirep_Cphi_inv.argtypes = [vp, vp, vp, vp]
     lib.hirep_Dphi_clover_hat.argtypes = [vp, cd, cd, vp, vp, vp, vp, vp]
+    lib.hirep_clover_exp_field.argtypes = [vp, cd, cd, ci, ci, vp, vp]
+    lib.hirep_Dphi_blocks.argtypes = [vp, vp, vp, vp, vp]
+    lib.hirep_Dphi_blocks_hat.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.hirep_sync.argtypes = [vp]
     lib.hirep_last_error.restype = ctypes.c_char_p
     for n in SYMBOLS:
@@ -253,6 +257,9 @@ def hirep_clover_inv_bytes(g) -> int:
 def hirep_clover_inv_field(g, m0, csw, parity, inv, clover): _check(load().hirep_clover_inv_field(g, m0, csw, parity, inv, clover))
 def hirep_Cphi_inv(g, out, inp, inv): _check(load().hirep_Cphi_inv(g, out, inp, inv))
 def hirep_Dphi_clover_hat(g, m0, csw, out, inp, links, clover, inv_odd): _check(load().hirep_Dphi_clover_hat(g, m0, csw, out, inp, links, clover, inv_odd))
+def hirep_clover_exp_field(g, m0, csw, parity, inverse, blocks, clover): _check(load().hirep_clover_exp_field(g, m0, csw, parity, inverse, blocks, clover))
+def hirep_Dphi_blocks(g, out, inp, links, blocks): _check(load().hirep_Dphi_blocks(g, out, inp, links, blocks))
+def hirep_Dphi_blocks_hat(g, out, inp, links, blocks_even, inv_blocks_odd): _check(load().hirep_Dphi_blocks_hat(g, out, inp, links, blocks_even, inv_blocks_odd))
 def hirep_Dphi_tm_hat(g, m0, mu, out, inp, links): _check(load().hirep_Dphi_tm_hat(g, m0, mu, out, inp, links))
 
 
@@ -497,6 +504,24 @@ class Geometry:
     def Dphi_clover_hat(self, m0, csw, inp_even, links, clover, inv_odd, out=None):
         out = self.new_spinor(EVEN) if out is None else out
         hirep_Dphi_clover_hat(self.handle, m0, csw, out.data_ptr(), inp_even.data_ptr(), links.data_ptr(), clover.data_ptr(), inv_odd.data_ptr())
+        return out
+
+    def clover_exp_field(self, m0, csw, clover, inverse=False):
+        """Full-lattice block field of Eq 50: even blocks followed by odd blocks (or their inverses)."""
+        nb = hirep_clover_inv_bytes(self.handle)
+        out = self.torch.empty(2 * nb, dtype=self.torch.uint8, device=self.device)
+        for parity in (EVEN, ODD):
+            hirep_clover_exp_field(self.handle, m0, csw, parity, int(inverse), out[parity * nb:].data_ptr(), clover.data_ptr())
+        return out
+
+    def Dphi_blocks(self, inp, links, blocks_full, out=None):
+        out = self.new_spinor(FULL) if out is None else out
+        hirep_Dphi_blocks(self.handle, out.data_ptr(), inp.data_ptr(), links.data_ptr(), blocks_full.data_ptr())
+        return out
+
+    def Dphi_blocks_hat(self, inp_even, links, blocks_even, inv_blocks_odd, out=None):
+        out = self.new_spinor(EVEN) if out is None else out
+        hirep_Dphi_blocks_hat(self.handle, out.data_ptr(), inp_even.data_ptr(), links.data_ptr(), blocks_even.data_ptr(), inv_blocks_odd.data_ptr())
         return out
 
     def cg_mshift_g5Dphi_sq(self, m0, shifts, b, links, tol, maxiter):

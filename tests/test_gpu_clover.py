@@ -120,3 +120,57 @@ def test_clover_schur_form_other_representations(env):
         a = p.to_numpy(p.geom.Dphi_clover_hat(cfg.m0, 0.0, xe, p.links_rep, cl, inv0), hirep.EVEN)
         b = oracle.Dphi_hat(T, L, cfg.d_R, cfg.m0, p.R, psi[p.ev], BC)
         assert oracle.rel_l2((4.0 + cfg.m0) * a, b) < 1e-13
+
+
+@pytest.mark.parametrize("name,T,L", CASES)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_exponential_clover(env, name, T, L, prec):
+    """Eq 50: the exponential blocks and their inverses element by element, the operator and its Schur form (Eq 43)."""
+    from oracle import clover as oc
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS[name].resized(T, L)
+    p = Problem(env, cfg, prec)
+    g, m0, tol, csw = p.geom, cfg.m0, TOL[prec], 1.2
+    cl = g.clover_field(p.links_rep)
+    E = g.clover_exp_field(m0, csw, cl)
+    Ei = g.clover_exp_field(m0, csw, cl, inverse=True)
+    nb = E.numel() // 2
+    psi = p.spinors[0]
+    wantE, wantEi = oc.exp_blocks(T, L, m0, csw, p.R), oc.exp_blocks(T, L, m0, csw, p.R, inverse=True)
+    # the blocks, read back through their action on unit-like spinors would cost 2d applications; check the action on psi
+    # per parity for both fields, then the operators
+    for parity, sites in ((hirep.EVEN, p.ev), (hirep.ODD, p.od)):
+        x = p.to_native(psi[sites], parity)
+        got = p.to_numpy(g.Cphi_inv(parity, x, E[parity * nb:]), parity)
+        assert oracle.rel_l2(got, oc.apply_blocks(wantE[sites], psi[sites])) < tol
+        got = p.to_numpy(g.Cphi_inv(parity, x, Ei[parity * nb:]), parity)
+        assert oracle.rel_l2(got, oc.apply_blocks(wantEi[sites], psi[sites])) < tol
+    x = p.to_native(psi, hirep.FULL)
+    got = p.to_numpy(g.Dphi_blocks(x, p.links_rep, E), hirep.FULL)
+    assert oracle.rel_l2(got, oc.Dphi_expclover(T, L, m0, csw, p.R, psi, BC)) < tol
+    xe = p.to_native(psi[p.ev], hirep.EVEN)
+    got = p.to_numpy(g.Dphi_blocks_hat(xe, p.links_rep, E, Ei[nb:]), hirep.EVEN)
+    assert oracle.rel_l2(got, oc.Dphi_expclover_hat(T, L, m0, csw, p.R, psi[p.ev], BC)) < tol
+
+
+def test_exponential_clover_unit_vectors(env):
+    """Every element of the exponential blocks: apply them to the 2 d_R unit spinors per chirality (SU(3) adjoint, d_R = 8)."""
+    from oracle import clover as oc
+    hirep, oracle = env["hirep"], env["oracle"]
+    T, L = 2, 2
+    cfg = synth.Config("t", T, L, 3, 1, -0.3, "haar", 29, ())
+    p = Problem(env, cfg, "f64")
+    d, m0, csw = cfg.d_R, cfg.m0, 0.8
+    cl = p.geom.clover_field(p.links_rep)
+    E = p.geom.clover_exp_field(m0, csw, cl)
+    want = oc.exp_blocks(T, L, m0, csw, p.R)
+    V = cfg.volume
+    for s in range(4):
+        for j in range(d):
+            e = np.zeros((V, 4, d), dtype=np.complex128)
+            e[:, s, j] = 1.0
+            got = p.to_numpy(p.geom.Cphi_inv(hirep.EVEN, p.to_native(e[p.ev], hirep.EVEN), E), hirep.EVEN)
+            col = want[p.ev][:, s // 2, :, (s % 2) * d + j]            # column J of block c = s//2
+            ref = np.zeros_like(got)
+            ref[:, 2 * (s // 2):2 * (s // 2) + 2, :] = col.reshape(len(p.ev), 2, d)
+            assert np.abs(got - ref).max() < 1e-13 * np.abs(want).max()
