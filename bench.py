@@ -409,7 +409,22 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
         ms = timeit(lambda: geom.Dphi_clover_hat(m0, 0.5, x_e, lr, cl, inv, out=y_e), reps=10)
         by = cm["ops"]["Dphi_eo"][1] * 2 + S * V / 2 + (2 * cb + 2 * S) * V / 2 + (cb + 2 * S) * V / 2
         out["Dphi_clover_hat"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3), "launches": 4}
-        del cl, inv
+        del inv
+        # exponential clover (Eq 50): full 2 d_R x 2 d_R blocks on both parities (8 d^2 complex per site)
+        if d <= 10 and torch.cuda.mem_get_info()[0] > 6 * cb * V + (4 << 30):
+            nb = hirep.hirep_clover_inv_bytes(geom.handle)
+            E = geom.clover_exp_field(m0, 1.0, cl)
+            ms = timeit(lambda: hirep.hirep_clover_exp_field(geom.handle, m0, 1.0, hirep.ODD, 0, E[nb:].data_ptr(), cl.data_ptr()), reps=3)
+            out["clover_exp_field"] = {"ms": round(ms, 3), "note": "one parity; scaling and squaring, 18 block products per site and chirality"}
+            Ei = geom.clover_exp_field(m0, 1.0, cl, inverse=True)
+            ms = timeit(lambda: geom.Dphi_blocks(x_full, lr, E, out=y_full), reps=10)
+            by = (2 * cb + 2 * S + lbytes + 3 * S) * V
+            out["Dphi_expclover"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3), "launches": 2}
+            ms = timeit(lambda: geom.Dphi_blocks_hat(x_e, lr, E, Ei[nb:], out=y_e), reps=10)
+            by = cm["ops"]["Dphi_eo"][1] * 2 + S * V / 2 + 2 * (2 * cb + 2 * S) * V / 2
+            out["Dphi_expclover_hat"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3), "launches": 4}
+            del E, Ei
+        del cl
     try:
         out["fma_peak_tflops"] = {"f64": round(hirep.hirep_fma_peak(hirep.F64), 2), "f32": round(hirep.hirep_fma_peak(hirep.F32), 2)}
     except Exception as e:   # measurement utility only
