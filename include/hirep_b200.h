@@ -212,6 +212,10 @@ int hirep_clover_field(hirep_geom *g, void *clover, const void *links_rep);
 int hirep_clover_export(hirep_geom *g, void *canonical_out, const void *clover);
 int hirep_Cphi(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *clover);
 int hirep_Dphi_clover(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *links, const void *clover);
+/* (gamma_5 D_clover)^2 (two passes of the above with gamma_5 fused in the store) and the CG on it (as hirep_cg_g5Dphi_sq). */
+int hirep_g5Dphi_clover_sq(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *links, const void *clover);
+int hirep_cg_g5Dphi_clover_sq(hirep_geom *g, double m0, double csw, void *x_full, const void *b_full, const void *links,
+                              const void *clover, double tol, int maxiter, int *iters, double *relres);
 /* The even-odd form Eq 43 (L803) with the clover blocks of Eq 47: D_hat = D_ee - D_eo D_oo^{-1} D_oe on the even sites.
  *   hirep_clover_inv_field  inv <- ((4+m) + c_sw A_c)^{-1} for every site of ONE parity and both chiralities: the full
  *                           (2 d_R) x (2 d_R) blocks, native, caller-owned buffer of hirep_clover_inv_bytes() bytes.  In-place

@@ -398,12 +398,12 @@ extern "C" int hirep_Cphi(hirep_geom *g, double m0, double csw, void *out_full, 
     if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Cphi: out aliases in");
     return kern_result(g, k_cphi(g->prec, g->dR, 2 * g->geo.n_tiles, 4.0 + m0, csw, clover, in_full, out_full, g->stream), "hirep_Cphi");
 }
-extern "C" int hirep_Dphi_clover(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *links, const void *clover) {
-    CHECK_PTRS("hirep_Dphi_clover", out_full, in_full, links, clover);
-    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Dphi_clover: out aliases in");
-    int rc = kern_result(g, k_cphi(g->prec, g->dR, 2 * g->geo.n_tiles, 4.0 + m0, csw, clover, in_full, out_full, g->stream), "hirep_Dphi_clover (diagonal term)");
+// out = [gamma_5] (Cphi in - 1/2 hop(in)): Cphi writes out, the hopping pass accumulates onto it in place (every site's own
+// value is read before it is written, by the same tile); gamma_5 commutes with the diagonal blocks
+static int dphi_clover(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *links, const void *clover, int g5,
+                       const char *what) {
+    int rc = kern_result(g, k_cphi(g->prec, g->dR, 2 * g->geo.n_tiles, 4.0 + m0, csw, clover, in_full, out_full, g->stream), what);
     if (rc) return rc;
-    // out = 1 * out - 1/2 hop(in): every site's own value is read before it is written, by the same tile
     const size_t hb = g->bytes_spinor_half;
     const char *in_e = (const char *)in_full, *in_o = in_e + hb;
     char *out_e = (char *)out_full, *out_o = out_e + hb;
@@ -411,11 +411,25 @@ extern "C" int hirep_Dphi_clover(hirep_geom *g, double m0, double csw, void *out
     L.nsets = 2;
     L.set[0] = HopSet{in_o, out_e, out_e, links_parity(g, links, 0), 0};
     L.set[1] = HopSet{in_e, out_o, out_o, links_parity(g, links, 1), 1};
-    L.a = 1.0; L.b = -0.5; L.g5 = 0; L.am = 0.0;
-    return hop(g, L, "hirep_Dphi_clover (hopping term)");
+    L.a = 1.0; L.b = -0.5; L.g5 = g5; L.am = 0.0;
+    return hop(g, L, what);
 }
-
-// ---- spinor linear algebra, reductions, CG ------------------------------------------
+extern "C" int hirep_Dphi_clover(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *links, const void *clover) {
+    CHECK_PTRS("hirep_Dphi_clover", out_full, in_full, links, clover);
+    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Dphi_clover: out aliases in");
+    return dphi_clover(g, m0, csw, out_full, in_full, links, clover, 0, "hirep_Dphi_clover");
+}
+// (gamma_5 D_clover)^2, Hermitian positive definite: the operator of the CG with the clover term (L772)
+extern "C" int hirep_g5Dphi_clover_sq(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *links,
+                                      const void *clover) {
+    CHECK_PTRS("hirep_g5Dphi_clover_sq", out_full, in_full, links, clover);
+    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_g5Dphi_clover_sq: out aliases in");
+    int rc = workspace(&g->ws_full, 2 * g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = dphi_clover(g, m0, csw, g->ws_full, in_full, links, clover, 1, "hirep_g5Dphi_clover_sq (first g5 D)");
+    if (rc) return rc;
+    return dphi_clover(g, m0, csw, out_full, g->ws_full, links, clover, 1, "hirep_g5Dphi_clover_sq (second g5 D)");
+}
 // the Schur form Eq 43 with the clover blocks: out_e = D_ee in_e - D_eo D_oo^{-1} D_oe in_e
 extern "C" int hirep_clover_inv_bytes(const hirep_geom *g, size_t *bytes) {
     if (!g || !bytes) return fail(HIREP_EINVAL, "hirep_clover_inv_bytes: NULL argument");
@@ -623,7 +637,7 @@ extern "C" int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, 
 // beta = rr'/rr; p = r + beta p }.  Per iteration: the operator (2 or 4 stencil launches), <p,Ap> = ||B p||^2 (2 launches),
 // r -= alpha Ap fused with ||r||^2 (2), x += alpha p fused with the p update (1): 8 spinor passes of linear algebra.
 static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, const void *links, double tol, int maxiter, int *iters,
-                    double *relres, const char *what, int twisted = 0, double mu = 0.0) {
+                    double *relres, const char *what, int twisted = 0, double mu = 0.0, const void *clover = nullptr, double csw = 0.0) {
     if (x == b) return fail(HIREP_EINVAL, "%s: x aliases b", what);
     if (!(tol > 0.0) || maxiter < 0) return fail(HIREP_EINVAL, "%s: tol=%g maxiter=%d", what, tol, maxiter);
     const int which = full ? HIREP_FULL : HIREP_EVEN, halves = full ? 2 : 1;
@@ -641,7 +655,8 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
     rr = bb;
     int it = 0;
     while (bb > 0.0 && it < maxiter && rr > tol * tol * bb) {
-        rc = twisted ? hirep_Dphi_tm_sq(g, m0, mu, g->cg_Ap, g->cg_p, links)
+        rc = clover ? hirep_g5Dphi_clover_sq(g, m0, csw, g->cg_Ap, g->cg_p, links, clover)
+           : twisted ? hirep_Dphi_tm_sq(g, m0, mu, g->cg_Ap, g->cg_p, links)
                      : full ? hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links) : hirep_g5Dphi_hat_sq(g, m0, g->cg_Ap, g->cg_p, links);
         if (rc) return rc;
         // A = B^dagger B with B p left in the operator's workspace (gamma_5 D p, Q_hat p, gamma_5 D^tm p; gamma_5 is
@@ -803,6 +818,11 @@ extern "C" int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const 
                                   int maxiter, int *iters, double *relres) {
     CHECK_PTRS("hirep_cg_g5Dphi_sq", x_full, b_full, links);
     return cg_solve(g, 1, m0, x_full, b_full, links, tol, maxiter, iters, relres, "hirep_cg_g5Dphi_sq");
+}
+extern "C" int hirep_cg_g5Dphi_clover_sq(hirep_geom *g, double m0, double csw, void *x_full, const void *b_full, const void *links,
+                                         const void *clover, double tol, int maxiter, int *iters, double *relres) {
+    CHECK_PTRS("hirep_cg_g5Dphi_clover_sq", x_full, b_full, links, clover);
+    return cg_solve(g, 1, m0, x_full, b_full, links, tol, maxiter, iters, relres, "hirep_cg_g5Dphi_clover_sq", 0, 0.0, clover, csw);
 }
 extern "C" int hirep_cg_Dphi_tm_sq(hirep_geom *g, double m0, double mu, void *x_full, const void *b_full, const void *links, double tol,
                                    int maxiter, int *iters, double *relres) {

@@ -35,7 +35,7 @@ SYMBOLS = [
     "hirep_Dphi_tm_hat", "hirep_cg_Dphi_tm_sq", "hirep_cg_mshift_g5Dphi_sq", "hirep_bicgstab", "hirep_fma_peak", "hirep_sync", "hirep_last_error",
     "hirep_clover_bytes", "hirep_clover_field", "hirep_clover_export", "hirep_Cphi", "hirep_Dphi_clover",
     "hirep_clover_inv_bytes", "hirep_clover_inv_field", "hirep_Cphi_inv", "hirep_Dphi_clover_hat",
-    "hirep_clover_exp_field", "hirep_Dphi_blocks", "hirep_Dphi_blocks_hat",
+    "hirep_clover_exp_field", "hirep_Dphi_blocks", "hirep_Dphi_blocks_hat", "hirep_g5Dphi_clover_sq", "hirep_cg_g5Dphi_clover_sq",
 ]
 
 
@@ -116,6 +116,8 @@ def load():
     lib.hirep_Cphi_inv.argtypes = [vp, vp, vp, vp]
     lib.hirep_Dphi_clover_hat.argtypes = [vp, cd, cd, vp, vp, vp, vp, vp]
     lib.hirep_clover_exp_field.argtypes = [vp, cd, cd, ci, ci, vp, vp]
+    lib.hirep_g5Dphi_clover_sq.argtypes = [vp, cd, cd, vp, vp, vp, vp]
+    lib.hirep_cg_g5Dphi_clover_sq.argtypes = [vp, cd, cd, vp, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_Dphi_blocks.argtypes = [vp, vp, vp, vp, vp]
     lib.hirep_Dphi_blocks_hat.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.hirep_sync.argtypes = [vp]
@@ -281,6 +283,15 @@ def hirep_bicgstab(g, op, m0, x, b, links, tol, maxiter):
 def hirep_cg_Dphi_tm_sq(g, m0, mu, x, b, links, tol, maxiter):
     it, res = ctypes.c_int(), (ctypes.c_double * 2)()
     _check(load().hirep_cg_Dphi_tm_sq(g, m0, mu, x, b, links, tol, maxiter, ctypes.byref(it), res))
+    return it.value, res[0]
+
+
+def hirep_g5Dphi_clover_sq(g, m0, csw, out, inp, links, clover): _check(load().hirep_g5Dphi_clover_sq(g, m0, csw, out, inp, links, clover))
+
+
+def hirep_cg_g5Dphi_clover_sq(g, m0, csw, x, b, links, clover, tol, maxiter):
+    it, res = ctypes.c_int(), (ctypes.c_double * 2)()
+    _check(load().hirep_cg_g5Dphi_clover_sq(g, m0, csw, x, b, links, clover, tol, maxiter, ctypes.byref(it), res))
     return it.value, res[0]
 
 
@@ -537,6 +548,16 @@ class Geometry:
     def cg_Dphi_tm_sq(self, m0, mu, b, links, tol, maxiter, out=None):
         out = self.new_spinor(FULL) if out is None else out
         it, res = hirep_cg_Dphi_tm_sq(self.handle, m0, mu, out.data_ptr(), b.data_ptr(), links.data_ptr(), tol, maxiter)
+        return out, it, res
+
+    def g5Dphi_clover_sq(self, m0, csw, inp, links, clover, out=None):
+        out = self.new_spinor(FULL) if out is None else out
+        hirep_g5Dphi_clover_sq(self.handle, m0, csw, out.data_ptr(), inp.data_ptr(), links.data_ptr(), clover.data_ptr())
+        return out
+
+    def cg_g5Dphi_clover_sq(self, m0, csw, b, links, clover, tol, maxiter, out=None):
+        out = self.new_spinor(FULL) if out is None else out
+        it, res = hirep_cg_g5Dphi_clover_sq(self.handle, m0, csw, out.data_ptr(), b.data_ptr(), links.data_ptr(), clover.data_ptr(), tol, maxiter)
         return out, it, res
 
     def cg_g5Dphi_hat_sq(self, m0, b_even, links, tol, maxiter, out=None):
