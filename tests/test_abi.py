@@ -127,6 +127,32 @@ def test_new_entry_points_argument_errors_without_gpu(hirep):
     hirep.hirep_geom_destroy(g)
 
 
+def test_clover_entry_points_argument_errors_without_gpu(hirep):
+    g = hirep.hirep_geom_create(4, 4, 3, hirep.FUND, hirep.F64)
+    # 4 d_R^2 complex per site, 256 sites (= 8 tiles of 32 lanes), 16 bytes per complex: both fields are the same size
+    assert hirep.hirep_clover_bytes(g) == 256 * 4 * 9 * 16
+    assert hirep.hirep_clover_inv_bytes(g) == 128 * 2 * 36 * 16
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_clover_field(g, None, 4096)
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_Cphi(g, 0.1, 1.0, 4096, 4096, 8192)                    # out aliases in
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_Dphi_clover(g, 0.1, 1.0, 4096, 8192, 12288 + 8, 16384)  # misaligned links
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_clover_inv_field(g, 0.1, 1.0, hirep.FULL, 4096, 8192)  # parity must be EVEN or ODD
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_clover_exp_field(g, -4.0, 1.0, hirep.ODD, 0, 4096, 8192)   # 4 + m0 = 0
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_Dphi_blocks_hat(g, 4096, 4096, 8192, 12288, 16384)
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_cg_g5Dphi_clover_sq(g, 0.1, 1.0, 4096, 4096, 8192, 12288, 1e-8, 10)   # x aliases b
+    hirep.hirep_set_link_mode(g, hirep.LINKS_REBUILD)
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_clover_field(g, 4096, 8192)                            # needs the stored represented links
+    assert hirep.hirep_launch_count(g) == 0
+    hirep.hirep_geom_destroy(g)
+
+
 def test_compute_without_device_is_an_error_not_a_fallback(hirep):
     """On a box without a GPU every compute entry point reports HIREP_ECUDA (-3); nothing is computed on the CPU."""
     import torch
