@@ -278,7 +278,104 @@ template <typename T> __global__ void clover_export_kernel(Geo g, int dR, cplx<T
     canon[(size_t)canonical_index(g, p, h) * per_site + (size_t)c * n2 * n2 + (size_t)I * n2 + J] = v;
 }
 
+// d_R <= 3: one thread per site, every matrix in registers (P, Q path products, C leaf sum, two accumulators).  Planes
+// and leaves are run-time loops around ONE unrolled leaf body (a fully unrolled walk would be ~170 KB of code and
+// instruction-fetch bound); the direction of step k of leaf l in plane (mu,nu) is s[(l+k)&3] with s = (mu, nu, -mu, -nu),
+// the walk keeps the four coordinates in scalar registers.  Plane order 03,12 -> H_c ; 01,23,02,13 -> B_c.
+template <typename T, bool REAL, int DR>
+__global__ void __launch_bounds__(128) clover_field_site_kernel(Geo g, const link_elem<T, REAL> *__restrict__ links, cplx<T> *__restrict__ clover) {
+    constexpr int NE = DR * DR;
+    const long slot = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int slots_half = g.n_tiles * TILE;
+    if (slot >= 2L * slots_half) return;
+    const int p = (int)(slot / slots_half), hp = (int)(slot - (long)p * slots_half);
+    const bool live = hp < g.Nh;
+    const int h = live ? hp : g.Nh - 1;
+    int t0, x0, y0, zh0;
+    decode_site(g, h, t0, x0, y0, zh0);
+    const int z0 = 2 * zh0 + ((t0 + x0 + y0 + p) & 1);
+    cplx<T> acc0[NE], acc1[NE];
+    cplx<T> *dst = clover + clover_off(g.n_tiles, p, hp >> 5, 0, 0, 0, hp & 31, NE);
+    for (int q = 0; q < 6; ++q) {
+        const int pl = (0x415032 >> (4 * q)) & 7;                  // plane order 2,3,0,5,1,4  (03,12 | 01,23 | 02,13)
+        const int mu = (0x211000 >> (4 * pl)) & 3, nu = (0x332321 >> (4 * pl)) & 3;
+        if (q == 0 || q == 2) {
+#pragma unroll
+            for (int e = 0; e < NE; ++e) acc0[e] = acc1[e] = mk<T>(0, 0);
+        }
+        cplx<T> C[NE];
+#pragma unroll
+        for (int e = 0; e < NE; ++e) C[e] = mk<T>(0, 0);
+        for (int leaf = 0; leaf < 4; ++leaf) {
+            int t = t0, x = x0, y = y0, z = z0, cp = p, ch = h;
+            cplx<T> P[NE], Q[NE];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int sq = (leaf + k) & 3;
+                const int dmu = (sq & 1) ? nu : mu, d = dmu + ((sq & 2) ? 4 : 0);
+                const link_elem<T, REAL> *W = links + link_off(g.n_tiles, cp, ch >> 5, d, 0, ch & 31, NE);
+                if (k == 0) {
+#pragma unroll
+                    for (int e = 0; e < NE; ++e) P[e] = ld_w<T, REAL>(W, (size_t)e * TILE);
+                } else {
+#pragma unroll
+                    for (int e = 0; e < NE; ++e) Q[e] = mk<T>(0, 0);
+#pragma unroll
+                    for (int l = 0; l < DR; ++l)
+#pragma unroll
+                        for (int j = 0; j < DR; ++j) {
+                            const cplx<T> w = ld_w<T, REAL>(W, (size_t)(l * DR + j) * TILE);
+#pragma unroll
+                            for (int i = 0; i < DR; ++i) cfma<T>(Q[i * DR + j], P[i * DR + l], w);
+                        }
+#pragma unroll
+                    for (int e = 0; e < NE; ++e) P[e] = Q[e];
+                }
+                const int dl = (sq & 2) ? -1 : 1;
+                t += dmu == 0 ? dl : 0; x += dmu == 1 ? dl : 0; y += dmu == 2 ? dl : 0; z += dmu == 3 ? dl : 0;
+                t = t == g.T ? 0 : (t < 0 ? g.T - 1 : t);
+                x = x == g.L ? 0 : (x < 0 ? g.L - 1 : x);
+                y = y == g.L ? 0 : (y < 0 ? g.L - 1 : y);
+                z = z == g.L ? 0 : (z < 0 ? g.L - 1 : z);
+                ch = encode_site(g, t, x, y, z >> 1);
+                cp ^= 1;
+            }
+#pragma unroll
+            for (int e = 0; e < NE; ++e) { C[e].x += P[e].x; C[e].y += P[e].y; }
+        }
+        // F = (C - C^+)/8; (i/2) F -> K1 (planes 01, 23) or K3 (03, 12); F/2 = -i (i/2) F -> -i K2 (02, 13)
+        const T s0 = (pl == 3 || pl == 5) ? T(-1) : T(1);          // c = 0: +F01 -F23 | +F02 +F13 | +F03 -F12
+        const T s1 = (pl == 4) ? T(1) : T(-1);                     // c = 1: -F01 -F23 | -F02 +F13 | -F03 -F12
+        const bool half = (pl == 1 || pl == 4);
+#pragma unroll
+        for (int i = 0; i < DR; ++i)
+#pragma unroll
+            for (int j = 0; j < DR; ++j) {
+                const cplx<T> a = C[i * DR + j], b = C[j * DR + i];
+                const cplx<T> F = mk<T>((a.x - b.x) * T(0.125), (a.y + b.y) * T(0.125));
+                const cplx<T> v = half ? mk<T>(T(0.5) * F.x, T(0.5) * F.y) : mk<T>(-T(0.5) * F.y, T(0.5) * F.x);
+                acc0[i * DR + j].x += s0 * v.x; acc0[i * DR + j].y += s0 * v.y;
+                acc1[i * DR + j].x += s1 * v.x; acc1[i * DR + j].y += s1 * v.y;
+            }
+        if (q == 1 || q == 5) {                                     // H (m = 0) after 03,12; B (m = 1) after all four
+            const int m = q == 1 ? 0 : 1;
+#pragma unroll
+            for (int e = 0; e < NE; ++e) {
+                dst[(size_t)((0 * 2 + m) * NE + e) * TILE] = live ? acc0[e] : mk<T>(0, 0);
+                dst[(size_t)((1 * 2 + m) * NE + e) * TILE] = live ? acc1[e] : mk<T>(0, 0);
+            }
+        }
+    }
+}
+template <typename T, bool REAL, int DR> static int clover_field_site_t(const Geo &g, void *clover, const void *links, cudaStream_t s) {
+    const long slots = 2L * g.n_tiles * TILE;
+    clover_field_site_kernel<T, REAL, DR><<<(unsigned)((slots + 127) / 128), 128, 0, s>>>(g, (const link_elem<T, REAL> *)links, (cplx<T> *)clover);
+    return (int)cudaGetLastError();
+}
+
 template <typename T, bool REAL> static int clover_field_t(const Geo &g, int dR, void *clover, const void *links, cudaStream_t s) {
+    if (dR == 2) return clover_field_site_t<T, REAL, 2>(g, clover, links, s);
+    if (dR == 3) return clover_field_site_t<T, REAL, 3>(g, clover, links, s);
     constexpr int LP = 1;
     const int ne = dR * dR;
     const size_t per_site = (size_t)(6 * LP + 5) * ne * sizeof(cplx<T>);
