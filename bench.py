@@ -409,6 +409,18 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
         ms = timeit(lambda: geom.Dphi_clover_hat(m0, 0.5, x_e, lr, cl, inv, out=y_e), reps=10)
         by = cm["ops"]["Dphi_eo"][1] * 2 + S * V / 2 + (2 * cb + 2 * S) * V / 2 + (cb + 2 * S) * V / 2
         out["Dphi_clover_hat"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3), "launches": 4}
+        try:    # even-odd preconditioned CG with the clover term: Q_hat^2 = 2 x (the four launches above), then the CG's linear algebra
+            geom.cg_g5Dphi_clover_hat_sq(m0, 0.5, x_e, lr, cl, inv, 1e-30, 2, out=y_e)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            _, it, res = geom.cg_g5Dphi_clover_hat_sq(m0, 0.5, x_e, lr, cl, inv, 1e-30, iters, out=y_e)
+            torch.cuda.synchronize()
+            ms_it = (time.perf_counter() - t0) * 1e3 / max(it, 1)
+            by_it = 2 * by + (1 + 3 + 5) * S * V / 2
+            out["cg_g5Dphi_clover_hat_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gbs": round(by_it / ms_it / 1e6, 1),
+                                              "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3), "launches_per_iteration": 13, "relres_after": res}
+        except Exception as e:
+            out["cg_g5Dphi_clover_hat_sq"] = {"error": str(e)}
         del inv
         # exponential clover (Eq 50): full 2 d_R x 2 d_R blocks on both parities (8 d^2 complex per site)
         if d <= 10 and torch.cuda.mem_get_info()[0] > 6 * cb * V + (4 << 30):

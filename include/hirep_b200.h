@@ -244,6 +244,21 @@ int hirep_Dphi_blocks(hirep_geom *g, void *out_full, const void *in_full, const 
 int hirep_Dphi_blocks_hat(hirep_geom *g, void *out_even, const void *in_even, const void *links, const void *blocks_even,
                           const void *inv_blocks_odd);
 
+/* Even-odd preconditioned CG with a site-diagonal term (L803, L815): Q_hat = gamma_5 D_hat with D_hat of Eq 43 is Hermitian
+ * when the blocks are (gamma_5 commutes with them and gamma_5 D_eo gamma_5 = D_oe^dagger), so Q_hat^2 is Hermitian positive
+ * definite.  Arguments as hirep_Dphi_clover_hat / hirep_Dphi_blocks_hat; eight launches per application; out != in.
+ *   hirep_g5Dphi_clover_hat_sq / hirep_g5Dphi_blocks_hat_sq     out_even = Q_hat^2 in_even
+ *   hirep_cg_g5Dphi_clover_hat_sq / hirep_cg_g5Dphi_blocks_hat_sq   Q_hat^2 x_even = b_even; recurrence, stopping rule, iters
+ *                           and relres (host pointers, may be NULL) as hirep_cg_g5Dphi_hat_sq; x != b. */
+int hirep_g5Dphi_clover_hat_sq(hirep_geom *g, double m0, double csw, void *out_even, const void *in_even, const void *links,
+                               const void *clover, const void *inv_odd);
+int hirep_g5Dphi_blocks_hat_sq(hirep_geom *g, void *out_even, const void *in_even, const void *links, const void *blocks_even,
+                               const void *inv_blocks_odd);
+int hirep_cg_g5Dphi_clover_hat_sq(hirep_geom *g, double m0, double csw, void *x_even, const void *b_even, const void *links,
+                                  const void *clover, const void *inv_odd, double tol, int maxiter, int *iters, double *relres);
+int hirep_cg_g5Dphi_blocks_hat_sq(hirep_geom *g, void *x_even, const void *b_even, const void *links, const void *blocks_even,
+                                  const void *inv_blocks_odd, double tol, int maxiter, int *iters, double *relres);
+
 /* Measurement utility: achieved TFLOP/s (2 flops per FMA) of a register-resident chain of
  * FMAs in the given precision on the current device, the ALU roofline the pipe utilisation is read against.
  * Synchronous; tflops is a host pointer. */

@@ -22,7 +22,7 @@ struct hirep_geom {
     int mode, variant;
     int tune_max_ctas, sum_alg;   // hirep_set_tuning
     cudaStream_t stream;
-    void *ws_half, *ws_half2, *ws_full;   // workspace spinors (lazy)
+    void *ws_half, *ws_half2, *ws_half3, *ws_full;   // workspace spinors (lazy)
     void *ws_red;                   // reduction partials + 4 result doubles (lazy)
     void *cg_r, *cg_p, *cg_Ap;      // CG work fields (lazy)
     void *ms_p[HIREP_MAX_SHIFTS];    // multi-shift CG direction fields (lazy)
@@ -103,7 +103,7 @@ extern "C" int hirep_geom_destroy(hirep_geom *g) {
     if (!g) return HIREP_OK;
     for (void *b : g->ms_p)
         if (b) cudaFree(b);
-    void *bufs[] = {g->ws_exp, g->ws_half, g->ws_half2, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
+    void *bufs[] = {g->ws_exp, g->ws_half, g->ws_half2, g->ws_half3, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
                     g->h_in_native, g->h_out_native, g->h_out_canon, g->h_out_canon2};
     if (g->host_events) {
         for (int i = 0; i < 2; ++i) { cudaEventDestroy(g->ev_done[i]); cudaEventDestroy(g->ev_copied[i]); }
@@ -517,6 +517,51 @@ extern "C" int hirep_Dphi_blocks_hat(hirep_geom *g, void *out_even, const void *
     return hop(g, L, "hirep_Dphi_blocks_hat (D_eo pass)");
 }
 
+// [gamma_5] D_hat for site-diagonal blocks (Eq 43): D_ee is either Cphi from the clover field (clover != NULL) or the
+// given even blocks; gamma_5 commutes with the blocks, so it is applied once in the last stencil epilogue
+static int blocks_hat(hirep_geom *g, double m0, double csw, void *out_even, const void *in_even, const void *links, const void *clover,
+                      const void *blocks_even, const void *inv_odd, int g5, const char *what) {
+    int rc = workspace(&g->ws_half, g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = workspace(&g->ws_half2, g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = offdiag(g, g->ws_half, in_even, links, 1, what);
+    if (rc) return rc;
+    rc = kern_result(g, k_cblock(g->prec, g->dR, g->geo.n_tiles, inv_odd, g->ws_half, g->ws_half2, g->stream), what);
+    if (rc) return rc;
+    rc = clover ? kern_result(g, k_cphi(g->prec, g->dR, g->geo.n_tiles, 4.0 + m0, csw, clover, in_even, out_even, g->stream), what)
+                : kern_result(g, k_cblock(g->prec, g->dR, g->geo.n_tiles, blocks_even, in_even, out_even, g->stream), what);
+    if (rc) return rc;
+    HopLaunch L{};
+    L.nsets = 1;
+    L.set[0] = HopSet{g->ws_half2, out_even, out_even, links_parity(g, links, 0), 0};
+    L.a = 1.0; L.b = +0.5; L.g5 = g5;
+    return hop(g, L, what);
+}
+// Q_hat^2 = (gamma_5 D_hat)^2 with D_hat of Eq 43: gamma_5 D_hat is Hermitian when the blocks are (gamma_5 D_ee gamma_5 =
+// D_ee^dagger, gamma_5 D_eo gamma_5 = D_oe^dagger), so this is Hermitian positive definite: the even-odd preconditioned
+// CG operator with a clover or exponential clover term (L803, L815).  Q_hat in is left in ws_half3 for the CG.
+static int blocks_hat_sq(hirep_geom *g, double m0, double csw, void *out_even, const void *in_even, const void *links, const void *clover,
+                         const void *blocks_even, const void *inv_odd, const char *what) {
+    int rc = workspace(&g->ws_half3, g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = blocks_hat(g, m0, csw, g->ws_half3, in_even, links, clover, blocks_even, inv_odd, 1, what);
+    if (rc) return rc;
+    return blocks_hat(g, m0, csw, out_even, g->ws_half3, links, clover, blocks_even, inv_odd, 1, what);
+}
+extern "C" int hirep_g5Dphi_clover_hat_sq(hirep_geom *g, double m0, double csw, void *out_even, const void *in_even, const void *links,
+                                          const void *clover, const void *inv_odd) {
+    CHECK_PTRS("hirep_g5Dphi_clover_hat_sq", out_even, in_even, links, clover, inv_odd);
+    if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_g5Dphi_clover_hat_sq: out aliases in");
+    return blocks_hat_sq(g, m0, csw, out_even, in_even, links, clover, nullptr, inv_odd, "hirep_g5Dphi_clover_hat_sq");
+}
+extern "C" int hirep_g5Dphi_blocks_hat_sq(hirep_geom *g, void *out_even, const void *in_even, const void *links, const void *blocks_even,
+                                          const void *inv_blocks_odd) {
+    CHECK_PTRS("hirep_g5Dphi_blocks_hat_sq", out_even, in_even, links, blocks_even, inv_blocks_odd);
+    if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_g5Dphi_blocks_hat_sq: out aliases in");
+    return blocks_hat_sq(g, 0.0, 0.0, out_even, in_even, links, nullptr, blocks_even, inv_blocks_odd, "hirep_g5Dphi_blocks_hat_sq");
+}
+
 static long spinor_elems(const hirep_geom *g, int which) {   // complex elements of a native buffer, padding included
     return (long)g->geo.n_tiles * 4 * g->dR * TILE * (which == HIREP_FULL ? 2 : 1);
 }
@@ -637,7 +682,8 @@ extern "C" int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, 
 // beta = rr'/rr; p = r + beta p }.  Per iteration: the operator (2 or 4 stencil launches), <p,Ap> = ||B p||^2 (2 launches),
 // r -= alpha Ap fused with ||r||^2 (2), x += alpha p fused with the p update (1): 8 spinor passes of linear algebra.
 static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, const void *links, double tol, int maxiter, int *iters,
-                    double *relres, const char *what, int twisted = 0, double mu = 0.0, const void *clover = nullptr, double csw = 0.0) {
+                    double *relres, const char *what, int twisted = 0, double mu = 0.0, const void *clover = nullptr, double csw = 0.0,
+                    const void *blocks_even = nullptr, const void *inv_odd = nullptr) {
     if (x == b) return fail(HIREP_EINVAL, "%s: x aliases b", what);
     if (!(tol > 0.0) || maxiter < 0) return fail(HIREP_EINVAL, "%s: tol=%g maxiter=%d", what, tol, maxiter);
     const int which = full ? HIREP_FULL : HIREP_EVEN, halves = full ? 2 : 1;
@@ -655,13 +701,14 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
     rr = bb;
     int it = 0;
     while (bb > 0.0 && it < maxiter && rr > tol * tol * bb) {
-        rc = clover ? hirep_g5Dphi_clover_sq(g, m0, csw, g->cg_Ap, g->cg_p, links, clover)
+        rc = inv_odd ? blocks_hat_sq(g, m0, csw, g->cg_Ap, g->cg_p, links, clover, blocks_even, inv_odd, what)
+           : clover ? hirep_g5Dphi_clover_sq(g, m0, csw, g->cg_Ap, g->cg_p, links, clover)
            : twisted ? hirep_Dphi_tm_sq(g, m0, mu, g->cg_Ap, g->cg_p, links)
                      : full ? hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links) : hirep_g5Dphi_hat_sq(g, m0, g->cg_Ap, g->cg_p, links);
         if (rc) return rc;
         // A = B^dagger B with B p left in the operator's workspace (gamma_5 D p, Q_hat p, gamma_5 D^tm p; gamma_5 is
         // unitary), so <p, A p> = ||B p||^2: one field read instead of two
-        const void *Bp = (full || twisted) ? g->ws_full : g->ws_half2;
+        const void *Bp = inv_odd ? g->ws_half3 : (full || twisted) ? g->ws_full : g->ws_half2;
         if ((rc = reduce_prod(g, which, 1, Bp, Bp, res, what))) return rc;
         if (!(res[0] > 0.0)) return fail(HIREP_EINVAL, "%s: <p,Ap> = %g is not positive (operator not positive definite?)", what, res[0]);
         const double alpha = rr / res[0];
@@ -833,6 +880,21 @@ extern "C" int hirep_cg_g5Dphi_hat_sq(hirep_geom *g, double m0, void *x_even, co
                                       int maxiter, int *iters, double *relres) {
     CHECK_PTRS("hirep_cg_g5Dphi_hat_sq", x_even, b_even, links);
     return cg_solve(g, 0, m0, x_even, b_even, links, tol, maxiter, iters, relres, "hirep_cg_g5Dphi_hat_sq");
+}
+
+// CG on the even-odd preconditioned operator with site-diagonal blocks, A = (gamma_5 D_hat)^2 with D_hat of Eq 43 (L803, L815):
+// the clover term (D_ee from the clover field, D_oo^{-1} from hirep_clover_inv_field) or any Hermitian blocks (exponential
+// clover: hirep_clover_exp_field and its inverse)
+extern "C" int hirep_cg_g5Dphi_clover_hat_sq(hirep_geom *g, double m0, double csw, void *x_even, const void *b_even, const void *links,
+                                             const void *clover, const void *inv_odd, double tol, int maxiter, int *iters, double *relres) {
+    CHECK_PTRS("hirep_cg_g5Dphi_clover_hat_sq", x_even, b_even, links, clover, inv_odd);
+    return cg_solve(g, 0, m0, x_even, b_even, links, tol, maxiter, iters, relres, "hirep_cg_g5Dphi_clover_hat_sq", 0, 0.0, clover, csw, nullptr, inv_odd);
+}
+extern "C" int hirep_cg_g5Dphi_blocks_hat_sq(hirep_geom *g, void *x_even, const void *b_even, const void *links, const void *blocks_even,
+                                             const void *inv_blocks_odd, double tol, int maxiter, int *iters, double *relres) {
+    CHECK_PTRS("hirep_cg_g5Dphi_blocks_hat_sq", x_even, b_even, links, blocks_even, inv_blocks_odd);
+    return cg_solve(g, 0, 0.0, x_even, b_even, links, tol, maxiter, iters, relres, "hirep_cg_g5Dphi_blocks_hat_sq", 0, 0.0, nullptr, 0.0, blocks_even,
+                    inv_blocks_odd);
 }
 
 extern "C" int hirep_fma_peak(int prec, double *tflops) {

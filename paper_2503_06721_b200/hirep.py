@@ -36,6 +36,7 @@ SYMBOLS = [
     "hirep_clover_bytes", "hirep_clover_field", "hirep_clover_export", "hirep_Cphi", "hirep_Dphi_clover",
     "hirep_clover_inv_bytes", "hirep_clover_inv_field", "hirep_Cphi_inv", "hirep_Dphi_clover_hat",
     "hirep_clover_exp_field", "hirep_Dphi_blocks", "hirep_Dphi_blocks_hat", "hirep_g5Dphi_clover_sq", "hirep_cg_g5Dphi_clover_sq",
+    "hirep_g5Dphi_clover_hat_sq", "hirep_g5Dphi_blocks_hat_sq", "hirep_cg_g5Dphi_clover_hat_sq", "hirep_cg_g5Dphi_blocks_hat_sq",
 ]
 
 
@@ -120,6 +121,10 @@ def load():
     lib.hirep_cg_g5Dphi_clover_sq.argtypes = [vp, cd, cd, vp, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_Dphi_blocks.argtypes = [vp, vp, vp, vp, vp]
     lib.hirep_Dphi_blocks_hat.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.hirep_g5Dphi_clover_hat_sq.argtypes = [vp, cd, cd, vp, vp, vp, vp, vp]
+    lib.hirep_g5Dphi_blocks_hat_sq.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.hirep_cg_g5Dphi_clover_hat_sq.argtypes = [vp, cd, cd, vp, vp, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
+    lib.hirep_cg_g5Dphi_blocks_hat_sq.argtypes = [vp, vp, vp, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_sync.argtypes = [vp]
     lib.hirep_last_error.restype = ctypes.c_char_p
     for n in SYMBOLS:
@@ -292,6 +297,26 @@ def hirep_g5Dphi_clover_sq(g, m0, csw, out, inp, links, clover): _check(load().h
 def hirep_cg_g5Dphi_clover_sq(g, m0, csw, x, b, links, clover, tol, maxiter):
     it, res = ctypes.c_int(), (ctypes.c_double * 2)()
     _check(load().hirep_cg_g5Dphi_clover_sq(g, m0, csw, x, b, links, clover, tol, maxiter, ctypes.byref(it), res))
+    return it.value, res[0]
+
+
+def hirep_g5Dphi_clover_hat_sq(g, m0, csw, out, inp, links, clover, inv_odd):
+    _check(load().hirep_g5Dphi_clover_hat_sq(g, m0, csw, out, inp, links, clover, inv_odd))
+
+
+def hirep_g5Dphi_blocks_hat_sq(g, out, inp, links, blocks_even, inv_blocks_odd):
+    _check(load().hirep_g5Dphi_blocks_hat_sq(g, out, inp, links, blocks_even, inv_blocks_odd))
+
+
+def hirep_cg_g5Dphi_clover_hat_sq(g, m0, csw, x, b, links, clover, inv_odd, tol, maxiter):
+    it, res = ctypes.c_int(), (ctypes.c_double * 2)()
+    _check(load().hirep_cg_g5Dphi_clover_hat_sq(g, m0, csw, x, b, links, clover, inv_odd, tol, maxiter, ctypes.byref(it), res))
+    return it.value, res[0]
+
+
+def hirep_cg_g5Dphi_blocks_hat_sq(g, x, b, links, blocks_even, inv_blocks_odd, tol, maxiter):
+    it, res = ctypes.c_int(), (ctypes.c_double * 2)()
+    _check(load().hirep_cg_g5Dphi_blocks_hat_sq(g, x, b, links, blocks_even, inv_blocks_odd, tol, maxiter, ctypes.byref(it), res))
     return it.value, res[0]
 
 
@@ -558,6 +583,28 @@ class Geometry:
     def cg_g5Dphi_clover_sq(self, m0, csw, b, links, clover, tol, maxiter, out=None):
         out = self.new_spinor(FULL) if out is None else out
         it, res = hirep_cg_g5Dphi_clover_sq(self.handle, m0, csw, out.data_ptr(), b.data_ptr(), links.data_ptr(), clover.data_ptr(), tol, maxiter)
+        return out, it, res
+
+    def g5Dphi_clover_hat_sq(self, m0, csw, inp_even, links, clover, inv_odd, out=None):
+        out = self.new_spinor(EVEN) if out is None else out
+        hirep_g5Dphi_clover_hat_sq(self.handle, m0, csw, out.data_ptr(), inp_even.data_ptr(), links.data_ptr(), clover.data_ptr(), inv_odd.data_ptr())
+        return out
+
+    def g5Dphi_blocks_hat_sq(self, inp_even, links, blocks_even, inv_blocks_odd, out=None):
+        out = self.new_spinor(EVEN) if out is None else out
+        hirep_g5Dphi_blocks_hat_sq(self.handle, out.data_ptr(), inp_even.data_ptr(), links.data_ptr(), blocks_even.data_ptr(), inv_blocks_odd.data_ptr())
+        return out
+
+    def cg_g5Dphi_clover_hat_sq(self, m0, csw, b_even, links, clover, inv_odd, tol, maxiter, out=None):
+        out = self.new_spinor(EVEN) if out is None else out
+        it, res = hirep_cg_g5Dphi_clover_hat_sq(self.handle, m0, csw, out.data_ptr(), b_even.data_ptr(), links.data_ptr(), clover.data_ptr(),
+                                                inv_odd.data_ptr(), tol, maxiter)
+        return out, it, res
+
+    def cg_g5Dphi_blocks_hat_sq(self, b_even, links, blocks_even, inv_blocks_odd, tol, maxiter, out=None):
+        out = self.new_spinor(EVEN) if out is None else out
+        it, res = hirep_cg_g5Dphi_blocks_hat_sq(self.handle, out.data_ptr(), b_even.data_ptr(), links.data_ptr(), blocks_even.data_ptr(),
+                                                inv_blocks_odd.data_ptr(), tol, maxiter)
         return out, it, res
 
     def cg_g5Dphi_hat_sq(self, m0, b_even, links, tol, maxiter, out=None):

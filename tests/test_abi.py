@@ -146,6 +146,14 @@ def test_clover_entry_points_argument_errors_without_gpu(hirep):
         hirep.hirep_Dphi_blocks_hat(g, 4096, 4096, 8192, 12288, 16384)
     with pytest.raises(hirep.HirepError):
         hirep.hirep_cg_g5Dphi_clover_sq(g, 0.1, 1.0, 4096, 4096, 8192, 12288, 1e-8, 10)   # x aliases b
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_g5Dphi_clover_hat_sq(g, 0.1, 1.0, 4096, 4096, 8192, 12288, 16384)      # out aliases in
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_g5Dphi_blocks_hat_sq(g, 4096, 8192, 12288, None, 16384)                # NULL blocks
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_cg_g5Dphi_clover_hat_sq(g, 0.1, 1.0, 4096, 4096, 8192, 12288, 16384, 1e-8, 10)   # x aliases b
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_cg_g5Dphi_blocks_hat_sq(g, 4096, 8192, 12288, 16384, 20480, -1.0, 10)  # tol <= 0
     hirep.hirep_set_link_mode(g, hirep.LINKS_REBUILD)
     with pytest.raises(hirep.HirepError):
         hirep.hirep_clover_field(g, 4096, 8192)                            # needs the stored represented links

@@ -202,3 +202,44 @@ def test_clover_cg_and_rebuild_mode(env):
     p.geom.set_link_mode(hirep.LINKS_REBUILD)
     got = p.to_numpy(p.geom.Dphi_clover(m0, csw, xb, p.links_fund, cl), hirep.FULL)
     assert oracle.rel_l2(got, oc.Dphi_clover(T, L, m0, csw, p.R, b, BC)) < 1e-13
+
+
+@pytest.mark.parametrize("kind", ["clover", "expclover"])
+def test_schur_form_cg(env, kind):
+    """Even-odd preconditioned CG with a site-diagonal term (L803, L815): Q_hat^2 = (gamma_5 D_hat)^2 with D_hat of Eq 43
+    against the oracle's Schur operator, then the CG against the oracle's CG and the true residual through the oracle."""
+    from oracle import clover as oc
+    from oracle import linalg as la
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS["C2"].resized(4, 4)
+    p = Problem(env, cfg, "f64")
+    T, L, m0, csw = 4, 4, 0.2, 1.0
+    g = p.geom
+    b = p.spinors[0][p.ev]
+    g5 = np.array([1, 1, -1, -1])[None, :, None]
+    Dhat = oc.Dphi_clover_hat if kind == "clover" else oc.Dphi_expclover_hat
+    Q = lambda v: g5 * Dhat(T, L, m0, csw, p.R, v, BC)
+    A = lambda v: Q(Q(v))
+    cl = g.clover_field(p.links_rep)
+    xb = p.to_native(b, hirep.EVEN)
+    if kind == "clover":
+        inv_odd = g.clover_inv_field(m0, csw, hirep.ODD, cl)
+        op = lambda x: g.g5Dphi_clover_hat_sq(m0, csw, x, p.links_rep, cl, inv_odd)
+        cg = lambda x: g.cg_g5Dphi_clover_hat_sq(m0, csw, x, p.links_rep, cl, inv_odd, 1e-10, 2000)
+    else:
+        E = g.clover_exp_field(m0, csw, cl)
+        Ei = g.clover_exp_field(m0, csw, cl, inverse=True)
+        nb = E.numel() // 2
+        op = lambda x: g.g5Dphi_blocks_hat_sq(x, p.links_rep, E, Ei[nb:])
+        cg = lambda x: g.cg_g5Dphi_blocks_hat_sq(x, p.links_rep, E, Ei[nb:], 1e-10, 2000)
+    got = p.to_numpy(op(xb), hirep.EVEN)
+    want = A(b)
+    assert oracle.rel_l2(got, want) < 1e-13
+    # Hermitian positive definite on the device: <b, A b> real and positive
+    assert abs(np.vdot(b, got).imag) < 1e-12 * abs(np.vdot(b, got).real) and np.vdot(b, got).real > 0
+    x_ref, it_ref, _, _ = la.cg(A, b, 1e-10, 2000)
+    xs, it, res = cg(xb)
+    x = p.to_numpy(xs, hirep.EVEN)
+    assert res <= 1e-10 and abs(it - it_ref) <= 2
+    assert oracle.rel_l2(x, x_ref) < 1e-7
+    assert np.linalg.norm((b - A(x)).ravel()) < 1e-9 * np.linalg.norm(b.ravel())
