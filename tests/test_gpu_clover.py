@@ -243,3 +243,49 @@ def test_schur_form_cg(env, kind):
     assert res <= 1e-10 and abs(it - it_ref) <= 2
     assert oracle.rel_l2(x, x_ref) < 1e-7
     assert np.linalg.norm((b - A(x)).ravel()) < 1e-9 * np.linalg.norm(b.ravel())
+
+
+@pytest.mark.parametrize("name,prec", [("C2", "f64"), ("C2", "f32"), ("C3", "f64"), ("C3", "f32"), ("C4", "f32"), ("C5", "f64"), ("C5", "f32")])
+def test_full_size_clover_sampled(env, name, prec):
+    """BASELINE lattice sizes in the launch configuration bench.py times: the clover blocks, Cphi and Dphi_clover at sampled
+    sites (lattice corners included).  The clover term at x only involves links inside the 3^4 neighbourhood of x, so the
+    oracle, as it stands, is run on that neighbourhood cut out as a 3 x 3^3 lattice (its periodic wraps are never reached from
+    the centre site) and read at the centre; the hopping term comes from the sampled oracle of the Wilson tests."""
+    import itertools
+    from oracle import clover as oc
+    from tests.gpu_helpers import SampledOracle, coords_of, index_of, sample_sites, torch_field_fetch
+    from tests.test_gpu_parity import full_size_problem
+    torch, hirep, oracle = env["torch"], env["hirep"], env["oracle"]
+    cfg, geom, links, psi, lr = full_size_problem(env, name, prec)
+    so = SampledOracle(oracle, cfg, links)
+    fetch = torch_field_fetch(psi)
+    tol, m0, csw, d = TOL[prec], cfg.m0, 1.3, cfg.d_R
+    ext = np.array([cfg.T, cfg.L, cfg.L, cfg.L])
+    cl = geom.clover_field(lr)
+    x = geom.spinor_import(psi, hirep.FULL)
+    out_c = geom.spinor_export(geom.Cphi(m0, csw, x, cl), hirep.FULL)
+    out_d = geom.spinor_export(geom.Dphi_clover(m0, csw, x, lr, cl), hirep.FULL)
+    blocks = geom.clover_export(cl)
+    centre = index_of((1, 1, 1, 1), 3)
+    num = den = 0.0
+    for ix in sample_sites(cfg, 3 if d > 8 else 8, seed=5):
+        c = coords_of(ix, cfg.T, cfg.L)
+        idx = [index_of((c + np.array(off) - 1) % ext, cfg.L) for off in itertools.product(range(3), repeat=4)]
+        Up = links[torch.tensor(idx, device=links.device)].cpu().numpy().astype(np.complex128)          # [81,4,N,N]
+        Rp = np.array([[oracle.rep_matrix(cfg.n_g, cfg.rep, Up[s, mu]) for mu in range(4)] for s in range(81)])
+        want_blocks = oc.chiral_blocks(3, 3, Rp)[centre]
+        got_blocks = blocks[ix].cpu().numpy().astype(np.complex128)
+        assert np.abs(got_blocks - want_blocks).max() <= 50 * tol * max(np.abs(want_blocks).max(), 1e-3), (name, prec, ix)
+        pp = np.zeros((81, 4, d), dtype=np.complex128)
+        pp[centre] = fetch(ix)
+        want_c = oc.Cphi(3, 3, m0, csw, Rp, pp)[centre]
+        want_d = want_c + so.hop(fetch, ix)
+        for got, want in ((out_c[ix], want_c), (out_d[ix], want_d)):
+            got = got.cpu().numpy().astype(np.complex128)
+            assert np.linalg.norm(got - want) <= 10 * tol * np.linalg.norm(want), (name, prec, ix)
+            num += float(np.sum(np.abs(got - want) ** 2)); den += float(np.sum(np.abs(want) ** 2))
+    assert np.sqrt(num / den) < tol
+    geom.sync()
+    del cl, x, out_c, out_d, blocks, lr, links, psi
+    torch.cuda.empty_cache()
+
