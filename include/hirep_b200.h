@@ -250,6 +250,11 @@ int hirep_Dphi_blocks_hat(hirep_geom *g, void *out_even, const void *in_even, co
  *   hirep_g5Dphi_clover_hat_sq / hirep_g5Dphi_blocks_hat_sq     out_even = Q_hat^2 in_even
  *   hirep_cg_g5Dphi_clover_hat_sq / hirep_cg_g5Dphi_blocks_hat_sq   Q_hat^2 x_even = b_even; recurrence, stopping rule, iters
  *                           and relres (host pointers, may be NULL) as hirep_cg_g5Dphi_hat_sq; x != b. */
+/* The same on the full lattice with general Hermitian blocks (exponential clover): (gamma_5 D)^2 with D = hirep_Dphi_blocks, and
+ * the CG on it (as hirep_cg_g5Dphi_clover_sq). */
+int hirep_g5Dphi_blocks_sq(hirep_geom *g, void *out_full, const void *in_full, const void *links, const void *blocks_full);
+int hirep_cg_g5Dphi_blocks_sq(hirep_geom *g, void *x_full, const void *b_full, const void *links, const void *blocks_full, double tol,
+                              int maxiter, int *iters, double *relres);
 int hirep_g5Dphi_clover_hat_sq(hirep_geom *g, double m0, double csw, void *out_even, const void *in_even, const void *links,
                                const void *clover, const void *inv_odd);
 int hirep_g5Dphi_blocks_hat_sq(hirep_geom *g, void *out_even, const void *in_even, const void *links, const void *blocks_even,

@@ -481,10 +481,9 @@ extern "C" int hirep_clover_exp_field(hirep_geom *g, double m0, double csw, int 
     const double x = (inverse ? -1.0 : 1.0) * csw / (4.0 + m0), pref = inverse ? 1.0 / (4.0 + m0) : 4.0 + m0;
     return kern_result(g, k_clover_exp(g->geo, g->prec, g->dR, parity, x, pref, clover, blocks, g->ws_exp, g->stream), "hirep_clover_exp_field");
 }
-extern "C" int hirep_Dphi_blocks(hirep_geom *g, void *out_full, const void *in_full, const void *links, const void *blocks_full) {
-    CHECK_PTRS("hirep_Dphi_blocks", out_full, in_full, links, blocks_full);
-    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Dphi_blocks: out aliases in");
-    int rc = kern_result(g, k_cblock(g->prec, g->dR, 2 * g->geo.n_tiles, blocks_full, in_full, out_full, g->stream), "hirep_Dphi_blocks (diagonal term)");
+// out = [gamma_5] (blocks in - 1/2 hop(in)); gamma_5 commutes with the chirality blocks
+static int dphi_blocks(hirep_geom *g, void *out_full, const void *in_full, const void *links, const void *blocks_full, int g5, const char *what) {
+    int rc = kern_result(g, k_cblock(g->prec, g->dR, 2 * g->geo.n_tiles, blocks_full, in_full, out_full, g->stream), what);
     if (rc) return rc;
     const size_t hb = g->bytes_spinor_half;
     const char *in_e = (const char *)in_full, *in_o = in_e + hb;
@@ -493,8 +492,24 @@ extern "C" int hirep_Dphi_blocks(hirep_geom *g, void *out_full, const void *in_f
     L.nsets = 2;
     L.set[0] = HopSet{in_o, out_e, out_e, links_parity(g, links, 0), 0};
     L.set[1] = HopSet{in_e, out_o, out_o, links_parity(g, links, 1), 1};
-    L.a = 1.0; L.b = -0.5; L.g5 = 0; L.am = 0.0;
-    return hop(g, L, "hirep_Dphi_blocks (hopping term)");
+    L.a = 1.0; L.b = -0.5; L.g5 = g5; L.am = 0.0;
+    return hop(g, L, what);
+}
+extern "C" int hirep_Dphi_blocks(hirep_geom *g, void *out_full, const void *in_full, const void *links, const void *blocks_full) {
+    CHECK_PTRS("hirep_Dphi_blocks", out_full, in_full, links, blocks_full);
+    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Dphi_blocks: out aliases in");
+    return dphi_blocks(g, out_full, in_full, links, blocks_full, 0, "hirep_Dphi_blocks");
+}
+// (gamma_5 D)^2 with Hermitian site-diagonal blocks (the exponential clover's): Hermitian positive definite; gamma_5 D in is
+// left in ws_full for the CG
+extern "C" int hirep_g5Dphi_blocks_sq(hirep_geom *g, void *out_full, const void *in_full, const void *links, const void *blocks_full) {
+    CHECK_PTRS("hirep_g5Dphi_blocks_sq", out_full, in_full, links, blocks_full);
+    if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_g5Dphi_blocks_sq: out aliases in");
+    int rc = workspace(&g->ws_full, 2 * g->bytes_spinor_half);
+    if (rc) return rc;
+    rc = dphi_blocks(g, g->ws_full, in_full, links, blocks_full, 1, "hirep_g5Dphi_blocks_sq (first g5 D)");
+    if (rc) return rc;
+    return dphi_blocks(g, out_full, g->ws_full, links, blocks_full, 1, "hirep_g5Dphi_blocks_sq (second g5 D)");
 }
 extern "C" int hirep_Dphi_blocks_hat(hirep_geom *g, void *out_even, const void *in_even, const void *links, const void *blocks_even,
                                      const void *inv_blocks_odd) {
@@ -702,6 +717,7 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
     int it = 0;
     while (bb > 0.0 && it < maxiter && rr > tol * tol * bb) {
         rc = inv_odd ? blocks_hat_sq(g, m0, csw, g->cg_Ap, g->cg_p, links, clover, blocks_even, inv_odd, what)
+           : blocks_even ? hirep_g5Dphi_blocks_sq(g, g->cg_Ap, g->cg_p, links, blocks_even)
            : clover ? hirep_g5Dphi_clover_sq(g, m0, csw, g->cg_Ap, g->cg_p, links, clover)
            : twisted ? hirep_Dphi_tm_sq(g, m0, mu, g->cg_Ap, g->cg_p, links)
                      : full ? hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links) : hirep_g5Dphi_hat_sq(g, m0, g->cg_Ap, g->cg_p, links);
@@ -889,6 +905,11 @@ extern "C" int hirep_cg_g5Dphi_clover_hat_sq(hirep_geom *g, double m0, double cs
                                              const void *clover, const void *inv_odd, double tol, int maxiter, int *iters, double *relres) {
     CHECK_PTRS("hirep_cg_g5Dphi_clover_hat_sq", x_even, b_even, links, clover, inv_odd);
     return cg_solve(g, 0, m0, x_even, b_even, links, tol, maxiter, iters, relres, "hirep_cg_g5Dphi_clover_hat_sq", 0, 0.0, clover, csw, nullptr, inv_odd);
+}
+extern "C" int hirep_cg_g5Dphi_blocks_sq(hirep_geom *g, void *x_full, const void *b_full, const void *links, const void *blocks_full, double tol,
+                                         int maxiter, int *iters, double *relres) {
+    CHECK_PTRS("hirep_cg_g5Dphi_blocks_sq", x_full, b_full, links, blocks_full);
+    return cg_solve(g, 1, 0.0, x_full, b_full, links, tol, maxiter, iters, relres, "hirep_cg_g5Dphi_blocks_sq", 0, 0.0, nullptr, 0.0, blocks_full, nullptr);
 }
 extern "C" int hirep_cg_g5Dphi_blocks_hat_sq(hirep_geom *g, void *x_even, const void *b_even, const void *links, const void *blocks_even,
                                              const void *inv_blocks_odd, double tol, int maxiter, int *iters, double *relres) {

@@ -37,6 +37,7 @@ SYMBOLS = [
     "hirep_clover_inv_bytes", "hirep_clover_inv_field", "hirep_Cphi_inv", "hirep_Dphi_clover_hat",
     "hirep_clover_exp_field", "hirep_Dphi_blocks", "hirep_Dphi_blocks_hat", "hirep_g5Dphi_clover_sq", "hirep_cg_g5Dphi_clover_sq",
     "hirep_g5Dphi_clover_hat_sq", "hirep_g5Dphi_blocks_hat_sq", "hirep_cg_g5Dphi_clover_hat_sq", "hirep_cg_g5Dphi_blocks_hat_sq",
+    "hirep_g5Dphi_blocks_sq", "hirep_cg_g5Dphi_blocks_sq",
 ]
 
 
@@ -121,6 +122,8 @@ def load():
     lib.hirep_cg_g5Dphi_clover_sq.argtypes = [vp, cd, cd, vp, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_Dphi_blocks.argtypes = [vp, vp, vp, vp, vp]
     lib.hirep_Dphi_blocks_hat.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.hirep_g5Dphi_blocks_sq.argtypes = [vp, vp, vp, vp, vp]
+    lib.hirep_cg_g5Dphi_blocks_sq.argtypes = [vp, vp, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_g5Dphi_clover_hat_sq.argtypes = [vp, cd, cd, vp, vp, vp, vp, vp]
     lib.hirep_g5Dphi_blocks_hat_sq.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.hirep_cg_g5Dphi_clover_hat_sq.argtypes = [vp, cd, cd, vp, vp, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
@@ -297,6 +300,15 @@ def hirep_g5Dphi_clover_sq(g, m0, csw, out, inp, links, clover): _check(load().h
 def hirep_cg_g5Dphi_clover_sq(g, m0, csw, x, b, links, clover, tol, maxiter):
     it, res = ctypes.c_int(), (ctypes.c_double * 2)()
     _check(load().hirep_cg_g5Dphi_clover_sq(g, m0, csw, x, b, links, clover, tol, maxiter, ctypes.byref(it), res))
+    return it.value, res[0]
+
+
+def hirep_g5Dphi_blocks_sq(g, out, inp, links, blocks_full): _check(load().hirep_g5Dphi_blocks_sq(g, out, inp, links, blocks_full))
+
+
+def hirep_cg_g5Dphi_blocks_sq(g, x, b, links, blocks_full, tol, maxiter):
+    it, res = ctypes.c_int(), (ctypes.c_double * 2)()
+    _check(load().hirep_cg_g5Dphi_blocks_sq(g, x, b, links, blocks_full, tol, maxiter, ctypes.byref(it), res))
     return it.value, res[0]
 
 
@@ -583,6 +595,16 @@ class Geometry:
     def cg_g5Dphi_clover_sq(self, m0, csw, b, links, clover, tol, maxiter, out=None):
         out = self.new_spinor(FULL) if out is None else out
         it, res = hirep_cg_g5Dphi_clover_sq(self.handle, m0, csw, out.data_ptr(), b.data_ptr(), links.data_ptr(), clover.data_ptr(), tol, maxiter)
+        return out, it, res
+
+    def g5Dphi_blocks_sq(self, inp, links, blocks_full, out=None):
+        out = self.new_spinor(FULL) if out is None else out
+        hirep_g5Dphi_blocks_sq(self.handle, out.data_ptr(), inp.data_ptr(), links.data_ptr(), blocks_full.data_ptr())
+        return out
+
+    def cg_g5Dphi_blocks_sq(self, b, links, blocks_full, tol, maxiter, out=None):
+        out = self.new_spinor(FULL) if out is None else out
+        it, res = hirep_cg_g5Dphi_blocks_sq(self.handle, out.data_ptr(), b.data_ptr(), links.data_ptr(), blocks_full.data_ptr(), tol, maxiter)
         return out, it, res
 
     def g5Dphi_clover_hat_sq(self, m0, csw, inp_even, links, clover, inv_odd, out=None):

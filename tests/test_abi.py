@@ -149,6 +149,10 @@ def test_clover_entry_points_argument_errors_without_gpu(hirep):
     with pytest.raises(hirep.HirepError):
         hirep.hirep_g5Dphi_clover_hat_sq(g, 0.1, 1.0, 4096, 4096, 8192, 12288, 16384)      # out aliases in
     with pytest.raises(hirep.HirepError):
+        hirep.hirep_g5Dphi_blocks_sq(g, 4096, 4096, 8192, 12288)                           # out aliases in
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_cg_g5Dphi_blocks_sq(g, 4096, 8192, 12288, 16384, 1e-8, -1)             # maxiter < 0
+    with pytest.raises(hirep.HirepError):
         hirep.hirep_g5Dphi_blocks_hat_sq(g, 4096, 8192, 12288, None, 16384)                # NULL blocks
     with pytest.raises(hirep.HirepError):
         hirep.hirep_cg_g5Dphi_clover_hat_sq(g, 0.1, 1.0, 4096, 4096, 8192, 12288, 16384, 1e-8, 10)   # x aliases b

@@ -289,3 +289,29 @@ def test_full_size_clover_sampled(env, name, prec):
     del cl, x, out_c, out_d, blocks, lr, links, psi
     torch.cuda.empty_cache()
 
+
+
+def test_exponential_clover_cg_full_lattice(env):
+    """(gamma_5 D)^2 with the exponential clover blocks (Eq 50) on the full lattice and the CG on it."""
+    from oracle import clover as oc
+    from oracle import linalg as la
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.CONFIGS["C3"].resized(4, 4)
+    p = Problem(env, cfg, "f64")
+    T, L, m0, csw = 4, 4, 0.25, 0.9
+    g = p.geom
+    b = p.spinors[0]
+    g5 = np.array([1, 1, -1, -1])[None, :, None]
+    Q = lambda v: g5 * oc.Dphi_expclover(T, L, m0, csw, p.R, v, BC)
+    A = lambda v: Q(Q(v))
+    cl = g.clover_field(p.links_rep)
+    E = g.clover_exp_field(m0, csw, cl)
+    xb = p.to_native(b, hirep.FULL)
+    got = p.to_numpy(g.g5Dphi_blocks_sq(xb, p.links_rep, E), hirep.FULL)
+    assert oracle.rel_l2(got, A(b)) < 1e-13
+    x_ref, it_ref, _, _ = la.cg(A, b, 1e-10, 2000)
+    xs, it, res = g.cg_g5Dphi_blocks_sq(xb, p.links_rep, E, 1e-10, 2000)
+    x = p.to_numpy(xs, hirep.FULL)
+    assert res <= 1e-10 and abs(it - it_ref) <= 2
+    assert oracle.rel_l2(x, x_ref) < 1e-7
+    assert np.linalg.norm((b - A(x)).ravel()) < 1e-9 * np.linalg.norm(b.ravel())
