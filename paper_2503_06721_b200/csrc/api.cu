@@ -34,6 +34,8 @@ struct hirep_geom {
     cudaEvent_t ev_done[2], ev_copied[2];
     int host_slot, host_events;
     int host_links_ready;
+    double *h_scal;                 // pinned: the CG's scalars read back without blocking the launches behind them (lazy)
+    cudaEvent_t ev_scal;
     long launches;
     size_t bytes_spinor_half, bytes_links_fund, bytes_links_rep;
 };
@@ -111,6 +113,7 @@ extern "C" int hirep_geom_destroy(hirep_geom *g) {
     }
     for (void *b : bufs)
         if (b) cudaFree(b);
+    if (g->h_scal) { cudaFreeHost(g->h_scal); cudaEventDestroy(g->ev_scal); }
     delete g;
     return HIREP_OK;
 }
@@ -696,6 +699,7 @@ extern "C" int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, 
 // p = r; repeat { Ap; alpha = rr/<p,Ap>; x += alpha p; r -= alpha Ap; rr' = <r,r>; stop if rr' <= tol^2 <b,b>;
 // beta = rr'/rr; p = r + beta p }.  Per iteration: the operator (2 or 4 stencil launches), <p,Ap> = ||B p||^2 (2 launches),
 // r -= alpha Ap fused with ||r||^2 (2), x += alpha p fused with the p update (1): 8 spinor passes of linear algebra.
+// alpha, beta never leave the device and the next operator application is queued before the host reads ||r||^2 (see below).
 static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, const void *links, double tol, int maxiter, int *iters,
                     double *relres, const char *what, int twisted = 0, double mu = 0.0, const void *clover = nullptr, double csw = 0.0,
                     const void *blocks_even = nullptr, const void *inv_odd = nullptr) {
@@ -711,30 +715,53 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
     if (e == cudaSuccess) e = cudaMemcpyAsync(g->cg_r, b, fb, cudaMemcpyDeviceToDevice, g->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(g->cg_p, b, fb, cudaMemcpyDeviceToDevice, g->stream);
     if (e != cudaSuccess) return cuda_fail(e, what);
-    double bb, rr, res[2];
+    if (!g->h_scal) {
+        if ((e = cudaHostAlloc((void **)&g->h_scal, 8 * sizeof(double), cudaHostAllocDefault)) != cudaSuccess) return cuda_fail(e, what);
+        if ((e = cudaEventCreateWithFlags(&g->ev_scal, cudaEventDisableTiming)) != cudaSuccess) {
+            cudaFreeHost(g->h_scal); g->h_scal = nullptr;
+            return cuda_fail(e, what);
+        }
+    }
+    double bb, rr;
     if ((rc = hirep_spinor_sqnorm(g, which, b, &bb))) return rc;
     rr = bb;
-    int it = 0;
-    while (bb > 0.0 && it < maxiter && rr > tol * tol * bb) {
-        rc = inv_odd ? blocks_hat_sq(g, m0, csw, g->cg_Ap, g->cg_p, links, clover, blocks_even, inv_odd, what)
-           : blocks_even ? hirep_g5Dphi_blocks_sq(g, g->cg_Ap, g->cg_p, links, blocks_even)
-           : clover ? hirep_g5Dphi_clover_sq(g, m0, csw, g->cg_Ap, g->cg_p, links, clover)
-           : twisted ? hirep_Dphi_tm_sq(g, m0, mu, g->cg_Ap, g->cg_p, links)
-                     : full ? hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links) : hirep_g5Dphi_hat_sq(g, m0, g->cg_Ap, g->cg_p, links);
-        if (rc) return rc;
+    // The scalars stay on the device: d[0..1] = <p,Ap>, d[2..3] / d[4..5] = ||r||^2 of the even / odd iterations; alpha and beta
+    // are formed in the update kernels by the same IEEE divisions the host would do.  The host only reads ||r||^2 (and <p,Ap>,
+    // to report a non-positive value) for the stopping rule, and it does so AFTER it has queued the next operator application, so
+    // the GPU never idles on the round trip; a solve that stops on the tolerance has queued one operator application too many
+    // (it writes only Ap and the operator's workspaces).
+    double *d = red_out(g);
+    if ((e = cudaMemcpyAsync(d + 2, d, sizeof(double), cudaMemcpyDeviceToDevice, g->stream)) != cudaSuccess) return cuda_fail(e, what);
+    auto apply_op = [&]() -> int {
+        int rc2 = inv_odd ? blocks_hat_sq(g, m0, csw, g->cg_Ap, g->cg_p, links, clover, blocks_even, inv_odd, what)
+                : blocks_even ? hirep_g5Dphi_blocks_sq(g, g->cg_Ap, g->cg_p, links, blocks_even)
+                : clover ? hirep_g5Dphi_clover_sq(g, m0, csw, g->cg_Ap, g->cg_p, links, clover)
+                : twisted ? hirep_Dphi_tm_sq(g, m0, mu, g->cg_Ap, g->cg_p, links)
+                          : full ? hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links) : hirep_g5Dphi_hat_sq(g, m0, g->cg_Ap, g->cg_p, links);
+        if (rc2) return rc2;
         // A = B^dagger B with B p left in the operator's workspace (gamma_5 D p, Q_hat p, gamma_5 D^tm p; gamma_5 is
         // unitary), so <p, A p> = ||B p||^2: one field read instead of two
         const void *Bp = inv_odd ? g->ws_half3 : (full || twisted) ? g->ws_full : g->ws_half2;
-        if ((rc = reduce_prod(g, which, 1, Bp, Bp, res, what))) return rc;
-        if (!(res[0] > 0.0)) return fail(HIREP_EINVAL, "%s: <p,Ap> = %g is not positive (operator not positive definite?)", what, res[0]);
-        const double alpha = rr / res[0];
-        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, halves, g->sum_alg, alpha, nullptr, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, red_out(g), g->stream), what, 2);
+        return kern_result(g, k_prod(g->geo, g->prec, g->dR, halves, 1, g->sum_alg, Bp, Bp, g->ws_red, d, g->stream), what, 2);
+    };
+    int it = 0;
+    bool more = bb > 0.0 && it < maxiter && rr > tol * tol * bb;
+    if (more && (rc = apply_op())) return rc;
+    while (more) {
+        double *rr_old = d + 2 + 2 * (it & 1), *rr_new_d = d + 2 + 2 * ((it + 1) & 1);
+        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, halves, g->sum_alg, 0.0, rr_old, d, nullptr, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, rr_new_d, g->stream), what, 2);
         if (rc) return rc;
-        if ((rc = fetch_result(g, res, 2, what))) return rc;
-        const double rr_new = res[0];
+        if ((rc = kern_result(g, k_cg_xp(g->geo, g->prec, g->dR, halves, 0.0, 0.0, rr_old, d, rr_new_d, x, g->cg_p, g->cg_r, g->stream), what))) return rc;
+        if ((e = cudaMemcpyAsync(g->h_scal, d, sizeof(double), cudaMemcpyDeviceToHost, g->stream)) != cudaSuccess) return cuda_fail(e, what);
+        if ((e = cudaMemcpyAsync(g->h_scal + 1, rr_new_d, sizeof(double), cudaMemcpyDeviceToHost, g->stream)) != cudaSuccess) return cuda_fail(e, what);
+        if ((e = cudaEventRecord(g->ev_scal, g->stream)) != cudaSuccess) return cuda_fail(e, what);
         ++it;
-        if ((rc = kern_result(g, k_cg_xp(g->geo, g->prec, g->dR, halves, alpha, rr_new / rr, x, g->cg_p, g->cg_r, g->stream), what))) return rc;
-        rr = rr_new;
+        if (it < maxiter && (rc = apply_op())) return rc;   // queued before the host looks at ||r||^2
+        if ((e = cudaEventSynchronize(g->ev_scal)) != cudaSuccess) return cuda_fail(e, what);
+        const double pAp = g->h_scal[0];
+        if (!(pAp > 0.0)) return fail(HIREP_EINVAL, "%s: <p,Ap> = %g is not positive (operator not positive definite?)", what, pAp);
+        rr = g->h_scal[1];
+        more = it < maxiter && rr > tol * tol * bb;
     }
     if (iters) *iters = it;
     if (relres) *relres = bb > 0.0 ? sqrt(rr / bb) : 0.0;
@@ -784,7 +811,7 @@ extern "C" int hirep_cg_mshift_g5Dphi_sq(hirep_geom *g, double m0, int nshift, c
             const double ak[2] = {alpha * zeta_new[k] / zeta[k], 0.0};
             if ((rc = lincomb(g, HIREP_FULL, x_full[k], ONE2, 1, g->ms_p[k], ak, g->ms_p[k], ZERO2, 0, what))) return rc;   // x_k += alpha_k p_k
         }
-        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, 2, g->sum_alg, alpha, nullptr, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, red_out(g), g->stream), what, 2);
+        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, 2, g->sum_alg, alpha, nullptr, nullptr, nullptr, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, red_out(g), g->stream), what, 2);
         if (rc) return rc;
         if ((rc = fetch_result(g, res, 2, what))) return rc;
         const double rr_new = res[0], beta = rr_new / rr;

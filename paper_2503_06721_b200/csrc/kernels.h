@@ -41,9 +41,12 @@ int k_g5_lincomb(int prec, long n, int dR, void *xi, const double c0[2], int use
                  cudaStream_t s);
 int k_prod(const Geo &g, int prec, int dR, int halves, int mode, int alg, const void *xi, const void *eta, void *ws, double *out_dev, cudaStream_t s);
 int k_maxnorm(const Geo &g, int prec, int dR, int halves, const void *xi, void *ws, double *out_dev, cudaStream_t s);
-int k_cg_update(const Geo &g, int prec, int dR, int halves, int alg, double alpha, void *x, void *r, const void *p, const void *Ap, void *ws,
-                double *out_dev, cudaStream_t s);
-int k_cg_xp(const Geo &g, int prec, int dR, int halves, double alpha, double beta, void *x, void *p, const void *r, cudaStream_t s);
+// num/den, rr_old/pAp/rr_new: device-resident scalars (alpha = num/den; alpha = rr_old/pAp, beta = rr_new/rr_old) used instead of
+// the by-value alpha, beta when non-null: the pipelined CG never waits for the host between the operator and the updates
+int k_cg_update(const Geo &g, int prec, int dR, int halves, int alg, double alpha, const double *num, const double *den, void *x, void *r,
+                const void *p, const void *Ap, void *ws, double *out_dev, cudaStream_t s);
+int k_cg_xp(const Geo &g, int prec, int dR, int halves, double alpha, double beta, const double *rr_old, const double *pAp, const double *rr_new,
+            void *x, void *p, const void *r, cudaStream_t s);
 int k_fma_peak(int prec, double *tflops, cudaStream_t s);   // fma_peak.cu: measured FP64/FP32 FMA throughput
 // clover.cu: clover term (Eq 47-49); native clover field = 4 dR^2 complex per site
 int k_clover_field(const Geo &g, int prec, int dR, int real, void *clover, const void *links_rep, cudaStream_t s);

@@ -217,10 +217,12 @@ __global__ void __launch_bounds__(RED_THREADS) prod_partial_kernel(Pad P, long n
 
 // fused CG step: x += alpha p ; r -= alpha Ap ; partial ||r||^2          (alpha real: A is Hermitian positive definite)
 template <typename T>
-__global__ void __launch_bounds__(RED_THREADS) cg_update_kernel(Pad P, long n, int alg, double alpha, cplx<T> *__restrict__ x,
+__global__ void __launch_bounds__(RED_THREADS) cg_update_kernel(Pad P, long n, int alg, double alpha, const double *__restrict__ num,
+                                                                const double *__restrict__ den, cplx<T> *__restrict__ x,
                                                                 cplx<T> *__restrict__ r, const cplx<T> *__restrict__ p,
                                                                 const cplx<T> *__restrict__ Ap, Acc *__restrict__ partial) {
     Acc a[2] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
+    if (num != nullptr) alpha = __ddiv_rn(num[0], den[0]);   // device-resident scalars: the same IEEE division the host would do
     const T al = (T)alpha;
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
         const cplx<T> av = Ap[i];
@@ -244,8 +246,10 @@ __global__ void __launch_bounds__(RED_THREADS) cg_update_kernel(Pad P, long n, i
 
 // second half of the CG step, after beta is known:  x += alpha p ; p = r + beta p   (one pass: reads x, p, r; writes x, p)
 template <typename T>
-__global__ void __launch_bounds__(256) cg_xp_kernel(long n, double alpha, double beta, cplx<T> *__restrict__ x, cplx<T> *__restrict__ p,
-                                                    const cplx<T> *__restrict__ r) {
+__global__ void __launch_bounds__(256) cg_xp_kernel(long n, double alpha, double beta, const double *__restrict__ rr_old,
+                                                    const double *__restrict__ pAp, const double *__restrict__ rr_new, cplx<T> *__restrict__ x,
+                                                    cplx<T> *__restrict__ p, const cplx<T> *__restrict__ r) {
+    if (rr_old != nullptr) { alpha = __ddiv_rn(rr_old[0], pAp[0]); beta = __ddiv_rn(rr_new[0], rr_old[0]); }
     const T al = (T)alpha, be = (T)beta;
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
         const cplx<T> pv = p[i], rv = r[i];
@@ -380,23 +384,24 @@ int k_maxnorm(const Geo &g, int prec, int dR, int halves, const void *xi, void *
     return (int)cudaGetLastError();
 }
 
-int k_cg_xp(const Geo &g, int prec, int dR, int halves, double alpha, double beta, void *x, void *p, const void *r, cudaStream_t s) {
+int k_cg_xp(const Geo &g, int prec, int dR, int halves, double alpha, double beta, const double *rr_old, const double *pAp, const double *rr_new,
+            void *x, void *p, const void *r, cudaStream_t s) {
     const long n = (long)g.n_tiles * 4 * dR * TILE * halves;
     const int nb = blocks_for(n);
-    if (prec == 0) cg_xp_kernel<double><<<nb, 256, 0, s>>>(n, alpha, beta, (double2 *)x, (double2 *)p, (const double2 *)r);
-    else cg_xp_kernel<float><<<nb, 256, 0, s>>>(n, alpha, beta, (float2 *)x, (float2 *)p, (const float2 *)r);
+    if (prec == 0) cg_xp_kernel<double><<<nb, 256, 0, s>>>(n, alpha, beta, rr_old, pAp, rr_new, (double2 *)x, (double2 *)p, (const double2 *)r);
+    else cg_xp_kernel<float><<<nb, 256, 0, s>>>(n, alpha, beta, rr_old, pAp, rr_new, (float2 *)x, (float2 *)p, (const float2 *)r);
     return (int)cudaGetLastError();
 }
 
-int k_cg_update(const Geo &g, int prec, int dR, int halves, int alg, double alpha, void *x, void *r, const void *p, const void *Ap, void *ws,
-                double *out_dev, cudaStream_t s) {
+int k_cg_update(const Geo &g, int prec, int dR, int halves, int alg, double alpha, const double *num, const double *den, void *x, void *r,
+                const void *p, const void *Ap, void *ws, double *out_dev, cudaStream_t s) {
     const int ncomp = 4 * dR;
     const long half_elems = (long)g.n_tiles * ncomp * TILE, n = half_elems * halves;
     const Pad P{(long)g.n_tiles * ncomp, ncomp, g.Nh % TILE == 0 ? TILE : g.Nh % TILE};
     const int nb = blocks_for(n);
     Acc *partial = (Acc *)ws;
-    if (prec == 0) cg_update_kernel<double><<<nb, RED_THREADS, 0, s>>>(P, n, alg, alpha, (double2 *)x, (double2 *)r, (const double2 *)p, (const double2 *)Ap, partial);
-    else cg_update_kernel<float><<<nb, RED_THREADS, 0, s>>>(P, n, alg, alpha, (float2 *)x, (float2 *)r, (const float2 *)p, (const float2 *)Ap, partial);
+    if (prec == 0) cg_update_kernel<double><<<nb, RED_THREADS, 0, s>>>(P, n, alg, alpha, num, den, (double2 *)x, (double2 *)r, (const double2 *)p, (const double2 *)Ap, partial);
+    else cg_update_kernel<float><<<nb, RED_THREADS, 0, s>>>(P, n, alg, alpha, num, den, (float2 *)x, (float2 *)r, (const float2 *)p, (const float2 *)Ap, partial);
     reduce_final_kernel<<<1, RED_THREADS, 0, s>>>(nb, alg, partial, out_dev);
     return (int)cudaGetLastError();
 }
