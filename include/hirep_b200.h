@@ -160,7 +160,10 @@ int hirep_spinor_sqnorm(hirep_geom *g, int which, const void *xi, double *out);
 int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, double *out);
 /* Conjugate gradient (L730) for Q_m^2 x = b with Q_m^2 = g5Dphi_sq, Hermitian positive definite (L772); x starts at 0.
  * Stops when ||r||_2 <= tol ||b||_2 (r the recurrence residual) or after maxiter iterations (not an error: check
- * *relres).  Full-lattice native spinors; iters / relres are host pointers (may be NULL).  x must not alias b. */
+ * *relres).  Full-lattice native spinors; iters / relres are host pointers (may be NULL).  x must not alias b.
+ * alpha and beta stay on the device; the host reads ||r||^2 once per iteration AFTER queueing the next operator application, so a
+ * solve that stops on the tolerance has launched one operator application more than it needed (it touches only the
+ * library's own work fields); a non-positive <p,Ap> is reported (HIREP_EINVAL) after that iteration's update.  Synchronous on return. */
 int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const void *b_full, const void *links, double tol, int maxiter,
                        int *iters, double *relres);
 /* Stabilised bi-conjugate gradient (L730) for the non-Hermitian systems D_m x = b (op = HIREP_OP_DPHI, full-lattice
