@@ -57,11 +57,16 @@ enum {
     HIREP_EINVAL = -1,       /* bad argument: null/misaligned pointer, odd or <2 extent, unknown enum, out aliases in */
     HIREP_EUNSUPPORTED = -2, /* (N_g, rep, prec, mode) combination not instantiated                               */
     HIREP_ECUDA = -3,        /* CUDA runtime error (no device, launch or execution failure)                        */
-    HIREP_ENOMEM = -4        /* workspace allocation failed                                                        */
+    HIREP_ENOMEM = -4,       /* workspace allocation failed                                                        */
+    HIREP_EBREAKDOWN = -5    /* an iterative solver met a non-finite or degenerate scalar (NaN/inf in b or in a field,
+                                <p,Ap> <= 0, rho = 0, <rhat,v> = 0, <t,t> = 0, omega = 0); the stream has been drained
+                                and the solution field is UNDEFINED                                                  */
 };
 
 /* Lattice T x L^3 (both even, >= 2), gauge group SU(N_g) (2 <= N_g <= 6), representation, precision.
- * Default boundary conditions: antiperiodic in time, periodic in space ({-1,+1,+1,+1}); link mode STORED. */
+ * Default boundary conditions: antiperiodic in time, periodic in space ({-1,+1,+1,+1}); link mode STORED.
+ * The handle is bound to the CUDA device that is current at creation: its workspaces are allocated there and every
+ * compute call made while another device is current returns HIREP_EINVAL. */
 int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep_geom **out);
 int hirep_geom_destroy(hirep_geom *g); /* frees the handle and its workspace; NULL is a no-op */
 
@@ -163,7 +168,8 @@ int hirep_spinor_max_norm(hirep_geom *g, int which, const void *eta, double *out
  * *relres).  Full-lattice native spinors; iters / relres are host pointers (may be NULL).  x must not alias b.
  * alpha and beta stay on the device; the host reads ||r||^2 once per iteration AFTER queueing the next operator application, so a
  * solve that stops on the tolerance has launched one operator application more than it needed (it touches only the
- * library's own work fields); a non-positive <p,Ap> is reported (HIREP_EINVAL) after that iteration's update.  Synchronous on return. */
+ * library's own work fields); a non-positive or non-finite <p,Ap>, <b,b> or ||r||^2 returns HIREP_EBREAKDOWN after that iteration's
+ * update (x is then undefined; the stream is synchronised first).  Synchronous on return.  All solvers below follow the same rule. */
 int hirep_cg_g5Dphi_sq(hirep_geom *g, double m0, void *x_full, const void *b_full, const void *links, double tol, int maxiter,
                        int *iters, double *relres);
 /* Stabilised bi-conjugate gradient (L730) for the non-Hermitian systems D_m x = b (op = HIREP_OP_DPHI, full-lattice

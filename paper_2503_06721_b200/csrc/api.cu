@@ -37,6 +37,7 @@ struct hirep_geom {
     double *h_scal;                 // pinned: the CG's scalars read back without blocking the launches behind them (lazy)
     cudaEvent_t ev_scal;
     long launches;
+    int device;                     // CUDA device current at hirep_geom_create (-1: none); compute calls check it
     size_t bytes_spinor_half, bytes_links_fund, bytes_links_rep;
 };
 
@@ -60,6 +61,16 @@ static int kern_result(hirep_geom *g, int rc, const char *what, int nlaunch = 1)
     return cuda_fail((cudaError_t)rc, what);
 }
 static bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+// a solver stopped on a non-finite or degenerate scalar: drain the stream (kernels may be queued ahead), then report.
+// The solution field is undefined after a breakdown (include/hirep_b200.h).
+static int breakdown(hirep_geom *g, const char *fmt, ...) {
+    cudaStreamSynchronize(g->stream);
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return HIREP_EBREAKDOWN;
+}
 
 extern "C" const char *hirep_last_error(void) { return g_err; }
 
@@ -83,7 +94,6 @@ extern "C" int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep
     const long long V = (long long)T * L * L * L;
     if (V / 2 + 32 >= (1LL << 31)) return fail(HIREP_EINVAL, "hirep_geom_create: lattice too large for 32-bit site indices");
     const int dR = rep_dim(N_g, rep);
-    if (dR < 2) return fail(HIREP_EUNSUPPORTED, "hirep_geom_create: d_R=%d is not supported", dR);
     hirep_geom *g = new (std::nothrow) hirep_geom;
     if (!g) return fail(HIREP_ENOMEM, "hirep_geom_create: out of host memory");
     memset(g, 0, sizeof(*g));
@@ -97,6 +107,7 @@ extern "C" int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep
     g->bytes_spinor_half = (size_t)g->geo.n_tiles * 4 * dR * TILE * 2 * w;
     g->bytes_links_fund = (size_t)2 * g->geo.n_tiles * 8 * N_g * N_g * TILE * 2 * w;
     g->bytes_links_rep = (size_t)2 * g->geo.n_tiles * 8 * dR * dR * TILE * (g->real ? 1 : 2) * w;
+    if (cudaGetDevice(&g->device) != cudaSuccess) { g->device = -1; cudaGetLastError(); }
     *out = g;
     return HIREP_OK;
 }
@@ -173,9 +184,16 @@ extern "C" int hirep_set_tuning(hirep_geom *g, int key, int value) {
 }
 extern "C" long hirep_launch_count(const hirep_geom *g) { return g ? g->launches : 0; }
 
+// a geometry belongs to the device that was current when it was created (its workspaces live there)
+static bool wrong_device(const hirep_geom *g) {
+    int dev = -1;
+    if (g->device < 0 || cudaGetDevice(&dev) != cudaSuccess) return false;   // no device: the launch itself reports HIREP_ECUDA
+    return dev != g->device;
+}
 #define CHECK_PTRS(name, ...)                                                                                      \
     do {                                                                                                           \
         if (!g) return fail(HIREP_EINVAL, name ": NULL geometry");                                                 \
+        if (wrong_device(g)) return fail(HIREP_EINVAL, name ": the geometry was created on CUDA device %d, which is not the current device", g->device); \
         const void *ptrs_[] = {__VA_ARGS__};                                                                       \
         for (const void *p_ : ptrs_) {                                                                             \
             if (!p_) return fail(HIREP_EINVAL, name ": NULL pointer argument");                                    \
@@ -725,6 +743,7 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
     double bb, rr;
     if ((rc = hirep_spinor_sqnorm(g, which, b, &bb))) return rc;
     rr = bb;
+    if (!std::isfinite(bb)) return breakdown(g, "%s: <b,b> = %g is not finite", what, bb);
     // The scalars stay on the device: d[0..1] = <p,Ap>, d[2..3] / d[4..5] = ||r||^2 of the even / odd iterations; alpha and beta
     // are formed in the update kernels by the same IEEE divisions the host would do.  The host only reads ||r||^2 (and <p,Ap>,
     // to report a non-positive value) for the stopping rule, and it does so AFTER it has queued the next operator application, so
@@ -745,7 +764,7 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
         return kern_result(g, k_prod(g->geo, g->prec, g->dR, halves, 1, g->sum_alg, Bp, Bp, g->ws_red, d, g->stream), what, 2);
     };
     int it = 0;
-    bool more = bb > 0.0 && it < maxiter && rr > tol * tol * bb;
+    bool more = bb > 0.0 && it < maxiter && !(rr <= tol * tol * bb);
     if (more && (rc = apply_op())) return rc;
     while (more) {
         double *rr_old = d + 2 + 2 * (it & 1), *rr_new_d = d + 2 + 2 * ((it + 1) & 1);
@@ -759,9 +778,11 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
         if (it < maxiter && (rc = apply_op())) return rc;   // queued before the host looks at ||r||^2
         if ((e = cudaEventSynchronize(g->ev_scal)) != cudaSuccess) return cuda_fail(e, what);
         const double pAp = g->h_scal[0];
-        if (!(pAp > 0.0)) return fail(HIREP_EINVAL, "%s: <p,Ap> = %g is not positive (operator not positive definite?)", what, pAp);
+        if (!(pAp > 0.0) || !std::isfinite(pAp))
+            return breakdown(g, "%s: <p,Ap> = %g is not positive and finite (operator not positive definite?); x is undefined", what, pAp);
         rr = g->h_scal[1];
-        more = it < maxiter && rr > tol * tol * bb;
+        if (!std::isfinite(rr)) return breakdown(g, "%s: ||r||^2 = %g is not finite; x is undefined", what, rr);
+        more = it < maxiter && !(rr <= tol * tol * bb);
     }
     if (iters) *iters = it;
     if (relres) *relres = bb > 0.0 ? sqrt(rr / bb) : 0.0;
@@ -796,14 +817,15 @@ extern "C" int hirep_cg_mshift_g5Dphi_sq(hirep_geom *g, double m0, int nshift, c
     double bb, rr, res[2];
     if ((rc = hirep_spinor_sqnorm(g, HIREP_FULL, b_full, &bb))) return rc;
     rr = bb;
+    if (!std::isfinite(bb)) return breakdown(g, "%s: <b,b> = %g is not finite", what, bb);
     double zeta[HIREP_MAX_SHIFTS], zeta_old[HIREP_MAX_SHIFTS], zeta_new[HIREP_MAX_SHIFTS];
     for (int k = 0; k < nshift; ++k) zeta[k] = zeta_old[k] = 1.0;
     double alpha_old = 1.0, beta_old = 0.0;
     int it = 0;
-    while (bb > 0.0 && it < maxiter && rr > tol * tol * bb) {
+    while (bb > 0.0 && it < maxiter && !(rr <= tol * tol * bb)) {
         if ((rc = hirep_g5Dphi_sq(g, m0, g->cg_Ap, g->cg_p, links))) return rc;
         if ((rc = reduce_prod(g, HIREP_FULL, 0, g->cg_p, g->cg_Ap, res, what))) return rc;
-        if (!(res[0] > 0.0)) return fail(HIREP_EINVAL, "%s: <p,Ap> = %g is not positive", what, res[0]);
+        if (!(res[0] > 0.0) || !std::isfinite(res[0])) return breakdown(g, "%s: <p,Ap> = %g is not positive and finite; x is undefined", what, res[0]);
         const double alpha = rr / res[0];
         for (int k = 0; k < nshift; ++k) {
             zeta_new[k] = zeta[k] * zeta_old[k] * alpha_old /
@@ -815,6 +837,7 @@ extern "C" int hirep_cg_mshift_g5Dphi_sq(hirep_geom *g, double m0, int nshift, c
         if (rc) return rc;
         if ((rc = fetch_result(g, res, 2, what))) return rc;
         const double rr_new = res[0], beta = rr_new / rr;
+        if (!std::isfinite(rr_new)) return breakdown(g, "%s: ||r||^2 = %g is not finite; x is undefined", what, rr_new);
         ++it;
         for (int k = 0; k < nshift; ++k) {
             const double q = zeta_new[k] / zeta[k];
@@ -869,21 +892,25 @@ extern "C" int hirep_bicgstab(hirep_geom *g, int op, double m0, void *x, const v
     double bb, rr, rho[2] = {1, 0}, alpha[2] = {1, 0}, omega[2] = {1, 0};
     if ((rc = hirep_spinor_sqnorm(g, which, b, &bb))) return rc;
     rr = bb;
+    if (!std::isfinite(bb)) return breakdown(g, "%s: <b,b> = %g is not finite", what, bb);
+    auto zero_or_nan = [](const double c[2]) { return !std::isfinite(c[0]) || !std::isfinite(c[1]) || (c[0] == 0.0 && c[1] == 0.0); };
     int it = 0;
-    while (bb > 0.0 && it < maxiter && rr > tol * tol * bb) {
+    while (bb > 0.0 && it < maxiter && !(rr <= tol * tol * bb)) {
         double rho_new[2], q1[2], q2[2], beta[2], mbw[2], rv[2], ss, tt, ts[2];
         if ((rc = reduce_prod(g, which, 0, b, r, rho_new, what))) return rc;                     // rho' = <rhat, r>
-        if (rho_new[0] == 0.0 && rho_new[1] == 0.0) return fail(HIREP_EINVAL, "%s: breakdown (rho = 0)", what);
+        if (zero_or_nan(rho_new)) return breakdown(g, "%s: breakdown (rho = <rhat,r> = %g%+gi); x is undefined", what, rho_new[0], rho_new[1]);
         cdiv(rho_new, rho, q1); cdiv(alpha, omega, q2); cmul2(q1, q2, beta);                      // beta = (rho'/rho)(alpha/omega)
         cmul2(beta, omega, mbw); mbw[0] = -mbw[0]; mbw[1] = -mbw[1];
         if ((rc = lincomb(g, which, p, beta, 1, r, ONE2, v, mbw, 1, what))) return rc;            // p = r + beta p - beta omega v
         if ((rc = apply(v, p))) return rc;                                                        // v = A p
         if ((rc = reduce_prod(g, which, 0, b, v, rv, what))) return rc;
+        if (zero_or_nan(rv)) return breakdown(g, "%s: breakdown (<rhat,v> = %g%+gi); x is undefined", what, rv[0], rv[1]);
         cdiv(rho_new, rv, alpha);                                                                 // alpha = rho'/<rhat, v>
         const double malpha[2] = {-alpha[0], -alpha[1]};
         if ((rc = lincomb(g, which, sv, ZERO2, 0, r, ONE2, v, malpha, 1, what))) return rc;       // s = r - alpha v
         ++it;
         if ((rc = hirep_spinor_sqnorm(g, which, sv, &ss))) return rc;
+        if (!std::isfinite(ss)) return breakdown(g, "%s: ||s||^2 = %g is not finite; x is undefined", what, ss);
         if (ss <= tol * tol * bb) {
             if ((rc = lincomb(g, which, x, ONE2, 1, p, alpha, p, ZERO2, 0, what))) return rc;     // x += alpha p
             rr = ss;
@@ -892,11 +919,14 @@ extern "C" int hirep_bicgstab(hirep_geom *g, int op, double m0, void *x, const v
         if ((rc = apply(t, sv))) return rc;                                                       // t = A s
         if ((rc = reduce_prod(g, which, 0, t, sv, ts, what))) return rc;
         if ((rc = hirep_spinor_sqnorm(g, which, t, &tt))) return rc;
+        if (!(tt > 0.0) || !std::isfinite(tt)) return breakdown(g, "%s: breakdown (<t,t> = %g); x is undefined", what, tt);
+        if (zero_or_nan(ts)) return breakdown(g, "%s: breakdown (omega = <t,s>/<t,t> = 0 or not finite); x is undefined", what);
         omega[0] = ts[0] / tt; omega[1] = ts[1] / tt;                                             // omega = <t,s>/<t,t>
         if ((rc = lincomb(g, which, x, ONE2, 1, p, alpha, sv, omega, 1, what))) return rc;        // x += alpha p + omega s
         const double momega[2] = {-omega[0], -omega[1]};
         if ((rc = lincomb(g, which, r, ZERO2, 0, sv, ONE2, t, momega, 1, what))) return rc;       // r = s - omega t
         if ((rc = hirep_spinor_sqnorm(g, which, r, &rr))) return rc;
+        if (!std::isfinite(rr)) return breakdown(g, "%s: ||r||^2 = %g is not finite; x is undefined", what, rr);
         rho[0] = rho_new[0]; rho[1] = rho_new[1];
     }
     if (iters) *iters = it;

@@ -58,7 +58,8 @@ template <typename T> int hop_rebuild_by_config(const Geo &g, int N, int rep, in
     case 12: return hop_rebuild<T, 2, 1>(g, variant, L, s);   // ADJ SU(2), d_R = 3
     case 22: return hop_rebuild<T, 2, 2>(g, variant, L, s);   // SYM SU(2), SU(3): d_R = 3, 6
     case 23: return hop_rebuild<T, 3, 2>(g, variant, L, s);
-    case 33: return hop_rebuild<T, 3, 3>(g, variant, L, s);   // 2AS SU(3), SU(4): d_R = 3, 6
+    case 32: return hop_rebuild<T, 2, 3>(g, variant, L, s);   // 2AS SU(2), SU(3), SU(4): d_R = 1, 3, 6
+    case 33: return hop_rebuild<T, 3, 3>(g, variant, L, s);
     case 34: return hop_rebuild<T, 4, 3>(g, variant, L, s);
     }
     return KERR_UNSUPPORTED;
@@ -71,6 +72,7 @@ template <typename T> int hop_by_config(const Geo &g, int N, int rep, int mode, 
     const bool real = (rep == 1);
     if (!real) {
         switch (dR) {
+        case 1: return hop_small_variant<T, 1, false>(g, variant, L, s);   // SU(2) 2AS: R = det U (allowed)
         case 2: return hop_small_variant<T, 2, false>(g, variant, L, s);
         case 3: return hop_small_variant<T, 3, false>(g, variant, L, s);
         case 4: return hop_small_variant<T, 4, false>(g, variant, L, s);

@@ -99,8 +99,8 @@ __global__ void __launch_bounds__(32 * ((DR + R - 1) / R)) hop_large_kernel(cons
     const T a = (T)L.a, b = (T)L.b;
     const T am = (T)L.am;
     const T g5s = L.g5 ? T(-1) : T(1);
-    C *__restrict__ out = (C *)S.out + ((size_t)tile * NC) * TILE + lane;
-    const C *__restrict__ self = (const C *)S.self + ((size_t)tile * NC) * TILE + lane;
+    C *out = (C *)S.out + ((size_t)tile * NC) * TILE + lane;
+    const C *self = (const C *)S.self + ((size_t)tile * NC) * TILE + lane;
     const bool use_self = (S.self != nullptr) && (L.a != 0.0);
 #pragma unroll
     for (int s = 0; s < 2; ++s)

@@ -299,7 +299,7 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
         }
         if constexpr (SELF) mbar_wait(selffull_s, k & 1);
         if (c_active) {
-            C *__restrict__ out = (C *)(c_set ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
+            C *out = (C *)(c_set ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
 #pragma unroll
             for (int c = 0; c < DR; ++c) {
                 C vu = mk<T>(b * up[c].x, b * up[c].y);
@@ -329,15 +329,9 @@ template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SE
 int launch_hop_pair_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
     using Cfg = PairCfg<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF, REP>;
     auto kern = hop_pair_kernel<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF, REP>;
-    static int n_sm = 0;
-    if (n_sm == 0) {
-        int dev = 0, sms = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-        if (e != cudaSuccess) return (int)e;
-        n_sm = sms;
-    }
+    static DevCache cache{};
+    int n_sm = 0;
+    if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
     const HopLaunch &L = L0;
     const int grid = ring_grid(n_sm, L.max_ctas, g.n_tiles * L.nsets, PAIRS);
     kern<<<grid, PAIRS * 64, Cfg::SMEM, s>>>(g, L);

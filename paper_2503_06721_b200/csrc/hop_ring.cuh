@@ -268,7 +268,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
 
         if constexpr (SELF) mbar_wait(selfbar_s, k & 1);
         if (c_active) {
-            C *__restrict__ out = (C *)(c_set ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
+            C *out = (C *)(c_set ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
 #pragma unroll
             for (int s = 0; s < 2; ++s)
 #pragma unroll
@@ -292,6 +292,25 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
     }
 }
 
+// Per-device launch preparation, cached per kernel instantiation AND per device: the opt-in shared-memory size is a
+// per-device function attribute and the persistent grid follows the SM count of the device the launch goes to.
+struct DevCache { int sms[64]; };
+template <typename K> inline int prepare_launch(K kern, size_t smem, DevCache &c, int &n_sm) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return (int)e;
+    if (dev < 0 || dev >= 64) return (int)cudaErrorInvalidDevice;
+    if (c.sms[dev] == 0) {
+        int sms = 0;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess && smem > 0) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return (int)e;
+        c.sms[dev] = sms;
+    }
+    n_sm = c.sms[dev];
+    return 0;
+}
+
 inline int ring_grid(int n_sm, int max_ctas, int total_tiles, int tiles_per_cta) {
     int grid = (total_tiles + tiles_per_cta - 1) / tiles_per_cta;
     if (grid > n_sm) grid = n_sm;
@@ -303,15 +322,9 @@ template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC, bool SE
 int launch_hop_ring_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
     using Cfg = RingCfg<T, DR, REAL, WARPS, STAGES, RPC, SELF>;
     auto kern = hop_ring_kernel<T, DR, REAL, WARPS, STAGES, RPC, SELF>;
-    static int n_sm = 0;
-    if (n_sm == 0) {
-        int dev = 0, sms = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-        if (e != cudaSuccess) return (int)e;
-        n_sm = sms;
-    }
+    static DevCache cache{};
+    int n_sm = 0;
+    if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
     const HopLaunch &L = L0;
     const int grid = ring_grid(n_sm, L.max_ctas, g.n_tiles * L.nsets, WARPS);
     kern<<<grid, WARPS * 32, Cfg::SMEM, s>>>(g, L);

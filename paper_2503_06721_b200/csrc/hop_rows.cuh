@@ -217,9 +217,9 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
 
         if constexpr (SELFBUF) mbar_wait(selfbar_s, k & 1);
         if (c_active) {
-            C *__restrict__ out = (C *)(c_set ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
+            C *out = (C *)(c_set ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
             const C *self_base = (const C *)(c_set ? L.set[1].self : L.set[0].self);
-            const C *__restrict__ self = SELFBUF ? selfbuf + lane : self_base + ((size_t)c_tile * NC) * TILE + lane;
+            const C *self = SELFBUF ? selfbuf + lane : self_base + ((size_t)c_tile * NC) * TILE + lane;
             const bool use_self = SELFBUF || ((self_base != nullptr) && (L.a != 0.0));
 #pragma unroll
             for (int s = 0; s < 2; ++s)
@@ -275,15 +275,9 @@ int launch_hop_rows_cfg(const Geo &g, const HopLaunch &L, cudaStream_t s) {
     static_assert(P::FITS, "row ring needs at least two stages");
     using Cfg = RowsCfg<T, DR, REAL, R, TP, P::JB, P::STAGES, SELFBUF>;
     auto kern = hop_rows_kernel<T, DR, REAL, R, TP, P::JB, P::STAGES, SELFBUF>;
-    static int n_sm = 0;
-    if (n_sm == 0) {
-        int dev = 0, sms = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-        if (e != cudaSuccess) return (int)e;
-        n_sm = sms;
-    }
+    static DevCache cache{};
+    int n_sm = 0;
+    if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
     const int grid = ring_grid(n_sm, L.max_ctas, g.n_tiles * L.nsets, TP);
     kern<<<grid, Cfg::WARPS * 32, Cfg::SMEM, s>>>(g, L);
     return (int)cudaGetLastError();

@@ -120,8 +120,8 @@ __device__ __forceinline__ bool is_site(const Pad &P, long i) {
 
 // ---- xi = c0*xi + c1*eta + c2*zeta --------------------------------------------------------------------------
 template <typename T, bool USE_XI, bool USE_ZETA>
-__global__ void __launch_bounds__(256) lincomb_kernel(long n, cplx<T> *__restrict__ xi, double2 c0, const cplx<T> *__restrict__ eta,
-                                                      double2 c1, const cplx<T> *__restrict__ zeta, double2 c2) {
+__global__ void __launch_bounds__(256) lincomb_kernel(long n, cplx<T> *xi, double2 c0, const cplx<T> *eta,
+                                                      double2 c1, const cplx<T> *zeta, double2 c2) {
     const T c0x = (T)c0.x, c0y = (T)c0.y, c1x = (T)c1.x, c1y = (T)c1.y, c2x = (T)c2.x, c2y = (T)c2.y;
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
         const cplx<T> e = eta[i];
@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(256) lincomb_kernel(long n, cplx<T> *__restric
 
 // ---- xi = c1*eta + c2*gamma_5*eta: the factor is c1 + c2 on the upper two spin components, c1 - c2 on the lower two
 template <typename T>
-__global__ void __launch_bounds__(256) g5_lincomb_kernel(long n, int ncomp, cplx<T> *__restrict__ xi, const cplx<T> *__restrict__ eta,
+__global__ void __launch_bounds__(256) g5_lincomb_kernel(long n, int ncomp, cplx<T> *xi, const cplx<T> *eta,
                                                          double2 cu, double2 cl, double2 c0, int use_xi) {
     const T ux = (T)cu.x, uy = (T)cu.y, lx = (T)cl.x, ly = (T)cl.y, c0x = (T)c0.x, c0y = (T)c0.y;
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
@@ -295,15 +295,9 @@ __global__ void maxnorm_final_kernel(int nblocks, const double *__restrict__ par
     out[0] = m;
 }
 
-int red_blocks() {
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0, sms = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 148;
-        n = 4 * sms;
-    }
-    return n;
-}
+// partial-sum blocks of the reductions: a constant (4 CTAs per SM of the 148-SM B200 this library is written for), so that the
+// workspace size and the summation order do not depend on which device of a process asks first
+int red_blocks() { return 4 * 148; }
 int blocks_for(long n) {
     const long need = (n + RED_THREADS - 1) / RED_THREADS;
     const int cap = red_blocks();

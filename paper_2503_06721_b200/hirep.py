@@ -21,6 +21,7 @@ EVEN, ODD, FULL = 0, 1, 2
 LINKS_STORED, LINKS_REBUILD = 0, 1
 OP_DPHI, OP_DPHI_EO, OP_DPHI_OE, OP_DPHI_HAT, OP_G5DPHI_SQ = 0, 1, 2, 3, 4
 TUNE_MAX_CTAS, TUNE_SUM_ALGORITHM = 1, 2
+OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM, EBREAKDOWN = 0, -1, -2, -3, -4, -5
 
 # every symbol include/hirep_b200.h declares
 SYMBOLS = [
@@ -42,7 +43,9 @@ SYMBOLS = [
 
 
 class HirepError(RuntimeError):
-    pass
+    def __init__(self, msg, rc=None):
+        super().__init__(msg)
+        self.rc = rc
 
 
 _lib = None
@@ -143,7 +146,7 @@ def hirep_last_error() -> str:
 
 def _check(rc: int):
     if rc != 0:
-        raise HirepError("hirep error %d: %s" % (rc, hirep_last_error()))
+        raise HirepError("hirep error %d: %s" % (rc, hirep_last_error()), rc)
 
 
 # ---- same-name module-level functions (raw handles / pointers) -----------------------------------------

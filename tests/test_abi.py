@@ -38,8 +38,9 @@ def test_geom_create_validation_and_sizes(hirep):
         with pytest.raises(hirep.HirepError):
             hirep.hirep_geom_create(*bad)
     assert "N_g" in hirep.hirep_last_error() or "precision" in hirep.hirep_last_error()
-    with pytest.raises(hirep.HirepError):
-        hirep.hirep_geom_create(4, 4, 2, hirep.ASY, 0)       # d_R = 1: unsupported
+    g = hirep.hirep_geom_create(4, 4, 2, hirep.ASY, 0)       # SU(2) 2AS, d_R = 1 (R = det U = 1): allowed
+    assert hirep.hirep_geom_sizes(g)["d_R"] == 1
+    hirep.hirep_geom_destroy(g)
     # sizes: SU(3) FUND 32^4 fp64 (BASELINE configs[1]) -- SURVEY.md 8(a) table: 201 MB spinor, 604 MB links (x2 gather copies)
     g = hirep.hirep_geom_create(32, 32, 3, hirep.FUND, hirep.F64)
     sz = hirep.hirep_geom_sizes(g)

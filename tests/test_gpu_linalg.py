@@ -317,3 +317,39 @@ def test_elementary_operations(env, prec):
         assert np.array_equal(p.to_numpy(xi, w), -eta)
         hirep.hirep_spinor_mul(h, w, xi.data_ptr(), 0.5 - 2.0j, e.data_ptr())
         assert oracle.rel_l2(p.to_numpy(xi, w), (0.5 - 2.0j) * eta) < TOL[prec]
+
+
+def test_solver_breakdown_is_reported(env):
+    """a NaN right-hand side, a NaN residual or an indefinite operator must return HIREP_EBREAKDOWN (stream
+    drained, x undefined) and never HIREP_OK with relres = 0."""
+    hirep, torch = env["hirep"], env["torch"]
+    cfg = synth.CONFIGS["C2"].resized(4, 4)
+    p = Problem(env, cfg, "f64")
+    b = p.spinors[0].copy()
+    b[5, 1, 2] = np.nan
+    bn = p.to_native(b, hirep.FULL)
+    for call in (lambda: p.geom.cg_g5Dphi_sq(0.3, bn, p.links_rep, 1e-10, 50),
+                 lambda: p.geom.cg_mshift_g5Dphi_sq(0.3, [0.0, 0.5], bn, p.links_rep, 1e-10, 50),
+                 lambda: p.geom.bicgstab(hirep.OP_DPHI, 0.3, bn, p.links_rep, 1e-10, 50)):
+        with pytest.raises(hirep.HirepError) as ei:
+            call()
+        assert ei.value.rc == hirep.EBREAKDOWN, ei.value
+    be = p.to_native(b[p.ev], hirep.EVEN)
+    with pytest.raises(hirep.HirepError) as ei:
+        p.geom.cg_g5Dphi_hat_sq(0.3, be, p.links_rep, 1e-10, 50)
+    assert ei.value.rc == hirep.EBREAKDOWN
+    # site-diagonal blocks that contain NaN: <p,Ap> = ||B p||^2 is NaN in the first iteration
+    good = p.to_native(p.spinors[0], hirep.FULL)
+    nb = hirep.hirep_clover_inv_bytes(p.geom.handle)
+    blocks = torch.zeros(2 * nb, dtype=torch.uint8, device=env["dev"])
+    blocks.view(torch.float64)[::7] = float("nan")
+    with pytest.raises(hirep.HirepError) as ei:
+        p.geom.cg_g5Dphi_blocks_sq(good, p.links_rep, blocks, 1e-10, 20)
+    assert ei.value.rc == hirep.EBREAKDOWN
+    # the geometry is still usable afterwards (stream drained, no sticky error)
+    x, it, res = p.geom.cg_g5Dphi_sq(0.3, good, p.links_rep, 1e-10, 500)
+    assert res <= 1e-10 and it > 0
+    # zero right-hand side: x = 0 after zero iterations, not an error
+    z = torch.zeros_like(good)
+    x, it, res = p.geom.cg_g5Dphi_sq(0.3, z, p.links_rep, 1e-10, 50)
+    assert it == 0 and res == 0.0 and not bool(x.any())

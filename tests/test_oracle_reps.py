@@ -142,7 +142,7 @@ def test_su2_adjoint_is_textbook_rotation(oracle):
         assert np.allclose(R, ref, atol=1e-14)
 
 
-@pytest.mark.parametrize("n", [3, 4, 6])
+@pytest.mark.parametrize("n", [2, 3, 4, 6])
 def test_2as_is_2x2_minors(oracle, n):
     U = rand_su(n, 1, seed=77 + n)[0]
     R = oracle.rep_matrix(n, ASY, U)
@@ -150,6 +150,14 @@ def test_2as_is_2x2_minors(oracle, n):
     for A, (i, j) in enumerate(pairs):
         for B, (k, l) in enumerate(pairs):
             assert abs(R[A, B] - (U[i, k] * U[j, l] - U[i, l] * U[j, k])) < 1e-14
+
+
+def test_su2_2as_is_the_trivial_representation(oracle):
+    """SU(2) 2AS: d_R = N(N-1)/2 = 1 (Tbl 1, L213-220) and R(U) = det U = 1 -- the singlet.  With unit represented links the
+    operator is the free one, whatever the gauge field."""
+    for U in rand_su(2, 4, seed=5):
+        R = oracle.rep_matrix(2, ASY, U)
+        assert R.shape == (1, 1) and abs(R[0, 0] - 1.0) < 1e-14
 
 
 @pytest.mark.parametrize("n", [2, 3, 4])
