@@ -151,7 +151,8 @@ class ClockSampler:
 # -------------------------------------------------------------------------------------------- our arm
 def run_ours(args):
     import torch
-    from paper_2503_06721_b200 import hirep, synth
+    from harness import synth
+    from paper_2503_06721_b200 import hirep
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -446,7 +447,7 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
 
 # ------------------------------------------------------------------------------- oracle arm / cpu baseline
 def prepare_sample(config, prec, T, L):
-    from paper_2503_06721_b200 import synth
+    from harness import synth
     cfg = synth.CONFIGS[config].resized(T, L)
     U, (psi,) = synth.make_inputs(cfg)
     U, psi = synth.round_to_precision(U, prec), synth.round_to_precision(psi, prec)
@@ -503,7 +504,7 @@ def run_reference(args):
     if rank != 0:
         return
     from oracle import oracle as orc
-    from paper_2503_06721_b200 import synth
+    from harness import synth
     prep, (T, L) = pick_sample(args.config, args.prec, args.steps + min(args.warmup, 1), 150.0)
     for _ in range(min(args.warmup, 1)):
         oracle_step(prep)

@@ -8,7 +8,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from paper_2503_06721_b200 import synth
+from harness import synth
 
 BC = (-1, 1, 1, 1)
 TOL = {"f64": 1e-13, "f32": 1e-5}          # BASELINE.json north_star: relative L2
@@ -74,9 +74,9 @@ class SampledOracle:
         return (4.0 + m0) ** 2 * field_even(ix) - self.hop(inner, ix)
 
     def g5Dphi_sq(self, field, ix, m0):
-        g5 = np.array([1, 1, -1, -1])[:, None]
-        inner = lambda iy: g5 * self.Dphi(field, iy, m0)
-        return g5 * self.Dphi(inner, ix, m0)
+        G5 = self.o.gamma5()                                  # the oracle's own gamma_5 (4 x 4), pinned in test_oracle_dirac.py
+        inner = lambda iy: G5 @ self.Dphi(field, iy, m0)
+        return G5 @ self.Dphi(inner, ix, m0)
 
 
 def torch_field_fetch(canon):

@@ -6,7 +6,7 @@ import socket
 import pytest
 
 import bench
-from paper_2503_06721_b200 import synth
+from harness import synth
 
 
 def test_cost_model_textbook_numbers():

@@ -4,7 +4,7 @@ Tolerances as for the Wilson operators: relative L2 <= 1e-13 (fp64) / 1e-5 (fp32
 import numpy as np
 import pytest
 
-from paper_2503_06721_b200 import synth
+from harness import synth
 from tests.gpu_helpers import BC, TOL
 from tests.test_gpu_parity import Problem, env  # noqa: F401  (env is a fixture)
 

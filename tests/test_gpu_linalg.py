@@ -12,7 +12,7 @@ import numpy as np
 import pytest
 
 from oracle import linalg as la
-from paper_2503_06721_b200 import synth
+from harness import synth
 from tests.gpu_helpers import BC
 from tests.test_gpu_parity import Problem, env, np_c  # noqa: F401  (env is a fixture)
 

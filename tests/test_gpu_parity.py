@@ -8,7 +8,7 @@ on sampled output sites (tests/gpu_helpers.py) in the launch configuration bench
 import numpy as np
 import pytest
 
-from paper_2503_06721_b200 import synth
+from harness import synth
 from tests.gpu_helpers import BC, TOL, SampledOracle, half_rank, sample_sites, torch_field_fetch
 
 pytestmark = pytest.mark.gpu

@@ -7,7 +7,7 @@
 import numpy as np
 import pytest
 
-from paper_2503_06721_b200 import synth
+from harness import synth
 from tests.test_gpu_parity import Problem, env  # noqa: F401  (env is a fixture)
 
 pytestmark = pytest.mark.gpu

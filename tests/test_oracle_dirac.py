@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 from oracle import dense
-from paper_2503_06721_b200 import synth
+from harness import synth
 
 FUND, ADJ, SYM, ASY = 0, 1, 2, 3
 BC = (-1, 1, 1, 1)

@@ -12,7 +12,7 @@ import pytest
 
 from oracle import dense
 from oracle import linalg as la
-from paper_2503_06721_b200 import synth
+from harness import synth
 
 BC = (-1, 1, 1, 1)
 

@@ -9,7 +9,7 @@ import os
 import numpy as np
 import pytest
 
-from paper_2503_06721_b200 import synth
+from harness import synth
 
 FUND, ADJ, SYM, ASY = 0, 1, 2, 3
 REP_ID = {"FUND": FUND, "ADJ": ADJ, "SYM": SYM, "2AS": ASY}
