@@ -11,6 +11,10 @@ Default workload: BASELINE.json configs[1] -- SU(3) fundamental, 32^4, fp64 (the
 CUDA-event duration, against the measured copy bandwidth of MEASURED_PEAKS.json.
 `e2e` = the same step through hirep_apply_host with pinned HOST buffers (H2D of links+spinors, D2H of results, timed).
 `cpu_baseline` = the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+`per_config` = after the headline step, the same six operators on EVERY BASELINE configuration C2..C5 in fp64 and fp32 (C4 also
+in link mode REBUILD), timed the way SURVEY.md 8(d) prescribes: >= 10 warm-ups, then n back-to-back launches (n = 100, fewer
+for multi-millisecond kernels so that a repeat stays near 0.25 s; never < 10) over 4 rotating spinor buffer sets, median of 5
+repeats -- next to the single-launch-inside-a-step number, so launch gaps are visible instead of folded into a fraction.
 `--impl reference` times the oracle alone (this tier's reference arm).  N > 1: independent replicas.
 """
 from __future__ import annotations
@@ -148,6 +152,119 @@ class ClockSampler:
         return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": self.smax, "reasons": reasons, "samples": len(sm)}
 
 
+
+# ------------------------------------------------------------------- all configurations (SURVEY.md 8(d) timing)
+SWEEP = [("C2", "f64", False), ("C2", "f32", False), ("C3", "f64", False), ("C3", "f32", False), ("C4", "f64", False),
+         ("C4", "f32", False), ("C4", "f64", True), ("C4", "f32", True), ("C5", "f64", False), ("C5", "f32", False)]
+NSETS = 4          # rotating spinor buffer sets (C2 fp32 half spinors are 50 MB < L2: one set would be timed out of L2)
+
+
+class Fields:
+    """Device-resident native fields of one configuration: links (stored represented or fundamental for REBUILD) and NSETS
+    independent input / output spinor sets."""
+
+    def __init__(self, torch, hirep, synth, cfg, prec, rebuild, dev, variant=0, nsets=NSETS):
+        cdt = torch.complex128 if prec == "f64" else torch.complex64
+        links_c, (psi_c,) = synth.make_inputs_torch(cfg, dev, cdt, n_spinors=1)
+        self.cfg, self.prec, self.rebuild = cfg, prec, rebuild
+        self.geom = g = hirep.Geometry(cfg.T, cfg.L, cfg.n_g, cfg.rep, prec, device=dev)
+        g.set_kernel_variant(variant)
+        self.lf = g.links_import(links_c)
+        self.links_c, self.psi_c = links_c, psi_c      # canonical tensors (the e2e leg copies them to the host); drop() frees them
+        if rebuild:
+            g.set_link_mode(hirep.LINKS_REBUILD)
+            self.lr = self.lf
+        else:
+            self.lr = g.new_links_rep()
+            g.links_to_rep(self.lf, out=self.lr)
+        hb = g.sizes["spinor_half"]
+        x0 = g.spinor_import(psi_c, hirep.FULL)
+        self.x = [x0] + [x0.clone() for _ in range(nsets - 1)]
+        self.y = [g.new_spinor(hirep.FULL) for _ in range(nsets)]
+        self.hb = hb
+
+    def drop_canonical(self):
+        self.links_c = self.psi_c = None
+
+    def op(self, name, k=0):
+        """closure launching operator `name` on spinor set k"""
+        g, m0, hb = self.geom, self.cfg.m0, self.hb
+        x, y, lr, lf = self.x[k % len(self.x)], self.y[k % len(self.y)], self.lr, self.lf
+        if name == "links_to_rep":
+            return lambda: g.links_to_rep(lf, out=lr)
+        if name == "Dphi_eo":
+            return lambda: g.Dphi_eo(x[hb:], lr, out=y[:hb])
+        if name == "Dphi_oe":
+            return lambda: g.Dphi_oe(x[:hb], lr, out=y[hb:])
+        if name == "Dphi":
+            return lambda: g.Dphi(m0, x, lr, out=y)
+        if name == "Dphi_hat":
+            return lambda: g.Dphi_hat(m0, x[:hb], lr, out=y[:hb])
+        if name == "g5Dphi_sq":
+            return lambda: g.g5Dphi_sq(m0, x, lr, out=y)
+        raise KeyError(name)
+
+
+def op_row(cm, name, ms, peak):
+    fl, by, by_ideal = cm["ops"][name]
+    return {"ms": round(ms, 4), "gflops": round(fl / ms / 1e6, 1), "gbs": round(by / ms / 1e6, 1),
+            "frac_hbm": round(by / ms / 1e6 / peak, 4), "frac_8TBs_nominal": round(by / ms / 1e6 / 8000.0, 4),
+            "gbs_survey_bytes": round(by_ideal / ms / 1e6, 1), "frac_survey_bytes": round(by_ideal / ms / 1e6 / peak, 4)}
+
+
+def time_back_to_back(torch, fields, name, target_s=0.25, repeats=5, warm=10, nmax=100, nmin=10):
+    """warm-ups, then `repeats` x n back-to-back launches rotating over the spinor sets; median ms per launch."""
+    fns = [fields.op(name, k) for k in range(NSETS)]
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for i in range(warm):
+        fns[i % NSETS]()
+    b.record()
+    torch.cuda.synchronize()
+    est = max(a.elapsed_time(b) / warm, 1e-3)
+    n = int(max(nmin, min(nmax, target_s * 1e3 / est)))
+    times = []
+    for _ in range(repeats):
+        a.record()
+        for i in range(n):
+            fns[i % NSETS]()
+        b.record()
+        torch.cuda.synchronize()
+        times.append(a.elapsed_time(b) / n)
+    times.sort()
+    return times[len(times) // 2], n
+
+
+def sweep_config(torch, hirep, synth, dev, name, prec, rebuild, peak, variant=0, fields=None):
+    cfg = synth.CONFIGS[name]
+    cm = cost_model(cfg, prec, rebuild)
+    own = fields is None
+    if own:
+        fields = Fields(torch, hirep, synth, cfg, prec, rebuild, dev, variant)
+        fields.drop_canonical()
+        torch.cuda.empty_cache()
+    ops = [k for k in OP_ORDER if not (rebuild and k == "links_to_rep")]
+    # (i) single launches inside whole steps (what the headline's per_op reports): 3 steps, one event pair per launch
+    in_step = {k: [] for k in ops}
+    for it in range(2 + 3):
+        for k in ops:
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fields.op(k, it)(); b.record()
+            if it >= 2:
+                in_step[k].append((a, b))
+    torch.cuda.synchronize()
+    out = {"d_R": cfg.d_R, "lattice": "%dx%d^3" % (cfg.T, cfg.L), "links": "rebuild" if rebuild else "stored", "ops": {}}
+    for k in ops:
+        ms, n = time_back_to_back(torch, fields, k)
+        row = op_row(cm, k, ms, peak)
+        row["launches_per_repeat"] = n
+        row["ms_in_step"] = round(sum(a.elapsed_time(b) for a, b in in_step[k]) / len(in_step[k]), 4)
+        out["ops"][k] = row
+    if own:
+        del fields
+        torch.cuda.empty_cache()
+    return out
+
 # -------------------------------------------------------------------------------------------- our arm
 def run_ours(args):
     import torch
@@ -175,47 +292,27 @@ def run_ours(args):
     rebuild = args.link_mode == "rebuild"
     cm = cost_model(cfg, prec, rebuild)
     ops_run = [k for k in OP_ORDER if not (rebuild and k == "links_to_rep")]
-    cdt = torch.complex128 if prec == "f64" else torch.complex64
-    links_c, (psi_c,) = synth.make_inputs_torch(cfg, dev, cdt, n_spinors=1)
-    geom = hirep.Geometry(cfg.T, cfg.L, cfg.n_g, cfg.rep, prec, device=dev)
-    geom.set_kernel_variant(args.variant)
-    lf = geom.links_import(links_c)
-    if rebuild:
-        geom.set_link_mode(hirep.LINKS_REBUILD)
-        lr = lf                                    # the operators read the fundamental field
-    else:
-        lr = geom.new_links_rep()
-    x_full = geom.spinor_import(psi_c, hirep.FULL)
-    hb = geom.sizes["spinor_half"]
-    x_e, x_o = x_full[:hb], x_full[hb:]
-    y_full, y_e, y_o = geom.new_spinor(hirep.FULL), geom.new_spinor(hirep.EVEN), geom.new_spinor(hirep.ODD)
-    m0 = cfg.m0
+    F = Fields(torch, hirep, synth, cfg, prec, rebuild, dev, args.variant)
+    geom, m0 = F.geom, cfg.m0
     ev = {k: [] for k in OP_ORDER}
 
-    def timed(name, fn, record):
-        if record:
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(); fn(); b.record()
-            ev[name].append((a, b))
-        else:
-            fn()
-
-    def step(record=False):
-        if not rebuild:
-            timed("links_to_rep", lambda: geom.links_to_rep(lf, out=lr), record)
-        timed("Dphi_eo", lambda: geom.Dphi_eo(x_o, lr, out=y_e), record)
-        timed("Dphi_oe", lambda: geom.Dphi_oe(x_e, lr, out=y_o), record)
-        timed("Dphi", lambda: geom.Dphi(m0, x_full, lr, out=y_full), record)
-        timed("Dphi_hat", lambda: geom.Dphi_hat(m0, x_e, lr, out=y_e), record)
-        timed("g5Dphi_sq", lambda: geom.g5Dphi_sq(m0, x_full, lr, out=y_full), record)
+    def step(it, record=False):
+        for k in ops_run:
+            fn = F.op(k, it)
+            if record:
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); fn(); b.record()
+                ev[k].append((a, b))
+            else:
+                fn()
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        step()
+    for it in range(args.warmup):
+        step(it)
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
@@ -224,8 +321,8 @@ def run_ours(args):
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     t0.record()
-    for _ in range(args.steps):
-        step(record=True)
+    for it in range(args.steps):
+        step(it, record=True)
     t1.record()
     barrier()
     clocks = sampler.stop() if rank == 0 else None
@@ -240,20 +337,20 @@ def run_ours(args):
     per_op = {}
     for k in ops_run:
         ms = sum(a.elapsed_time(b) for a, b in ev[k]) / len(ev[k])
-        fl, by, by_ideal = cm["ops"][k]
-        per_op[k] = {"ms": round(ms, 4), "gflops": round(fl / ms / 1e6, 1), "gbs": round(by / ms / 1e6, 1),
-                     "frac_hbm": round(by / ms / 1e6 / peak, 4), "gbs_paper_ideal_bytes": round(by_ideal / ms / 1e6, 1)}
+        per_op[k] = op_row(cm, k, ms, peak)
     eo = per_op["Dphi_eo"]
     traffic = ncu_traffic(args.config, prec, "Dphi_eo") if not rebuild else None
     roofline = {"bound": "hbm", "kernel": "hop stencil (Dphi_eo pass)", "achieved": eo["gbs"], "peak": peak,
                 "unit": "GB/s", "frac": round(eo["gbs"] / peak, 4), "traffic": traffic, "peak_source": peak_src,
-                "algorithmic_bytes": cm["ops"]["Dphi_eo"][1], "frac_of_8TBs_nominal": round(eo["gbs"] / 8000.0, 4)}
+                "algorithmic_bytes": cm["ops"]["Dphi_eo"][1], "frac_of_8TBs_nominal": round(eo["gbs"] / 8000.0, 4),
+                "timing": "one CUDA-event pair around the single launch inside each timed step (launch gap and pipeline fill included); "
+                          "per_config has the back-to-back figure"}
 
     # ---- e2e: same step through hirep_apply_host with pinned host buffers
     e2e = None
     if not args.no_e2e and not rebuild:
-        links_h = links_c.cpu().pin_memory()
-        psi_h = psi_c.cpu().pin_memory()
+        links_h = F.links_c.cpu().pin_memory()
+        psi_h = F.psi_c.cpu().pin_memory()
         idx = torch.arange(cfg.volume)
         par = ((idx // cfg.L ** 3) + (idx // cfg.L ** 2) % cfg.L + (idx // cfg.L) % cfg.L + idx % cfg.L) % 2
         psi_e_h = psi_h[par == 0].contiguous().pin_memory()
@@ -291,17 +388,48 @@ def run_ours(args):
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": ksteps,
                "api": "hirep_apply_host_async x5 + hirep_sync (pinned host canonical buffers; links copied once per step)"}
         del links_h, psi_h
+    F.drop_canonical()
+    torch.cuda.empty_cache()
 
     # ---- NEXT-1 row: linear algebra, reductions and CG on the same fields; outside the timed step
     extras = None
     if not args.no_extras and not rebuild:
-        extras = measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, peak)
+        extras = measure_extras(torch, hirep, geom, cfg, prec, cm, m0, F.x[0], F.y[0], F.lr, peak)
+
+    # ---- every BASELINE configuration x precision (+ C4 REBUILD), SURVEY 8(d) timing; rank 0 of a 1-GPU run only
+    per_config, sweep_s = None, None
+    if world == 1 and args.sweep != "none" and not args.custom:
+        ts = time.perf_counter()
+        per_config = {}
+        wanted = SWEEP if args.sweep == "all" else [c for c in SWEEP if c[0] in args.sweep.split(",")]
+        for name, pr, rb in wanted:
+            key = "%s_%s%s" % (name, pr, "_rebuild" if rb else "")
+            same = (name == args.config and pr == prec and rb == rebuild and not args.custom)
+            if not same:
+                need = sweep_bytes(synth.CONFIGS[name], pr, rb)
+                if F is not None and torch.cuda.mem_get_info()[0] < need:
+                    del geom
+                    F = None            # the headline's fields make room for the big configurations
+                    torch.cuda.empty_cache()
+            try:
+                per_config[key] = sweep_config(torch, hirep, synth, dev, name, pr, rb, peak, args.variant, F if same else None)
+            except Exception as e:      # one configuration must not take the headline line down with it
+                per_config[key] = {"error": "%s: %s" % (type(e).__name__, e)}
+                torch.cuda.empty_cache()
+        sweep_s = round(time.perf_counter() - ts, 1)
 
     cpu = None
     if rank == 0 and not args.no_cpu_baseline:
         cpu = cpu_baseline(args.config, prec)
 
     if rank == 0:
+        roofline_c4 = None
+        c4 = (per_config or {}).get("C4_f64", {}).get("ops", {}).get("Dphi_hat")
+        if c4:
+            roofline_c4 = {"bound": "hbm", "kernel": "C4 fp64 Dphi_hat (two hop stencil passes, d_R = 6)", "achieved": c4["gbs"], "peak": peak,
+                           "unit": "GB/s", "frac": c4["frac_hbm"], "traffic": ncu_traffic("C4", "f64", "Dphi_hat"), "peak_source": peak_src,
+                           "algorithmic_bytes": cost_model(synth.CONFIGS["C4"], "f64")["ops"]["Dphi_hat"][1],
+                           "frac_of_8TBs_nominal": c4["frac_8TBs_nominal"], "timing": "back-to-back launches, median of 5 repeats"}
         out = {
             "metric": METRIC, "value": round(value, 1), "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": True, "scaling": "weak",
@@ -310,13 +438,16 @@ def run_ours(args):
                                    % (cfg.name, cfg.n_g, synth.REP_NAMES[cfg.rep], cfg.d_R, cfg.T, cfg.L, prec),
                        "links": ("fundamental links, R rebuilt in registers (link mode REBUILD; no links_to_rep in the step)" if rebuild
                                  else "stored represented links (gather layout)"), "kernel_variant": args.variant,
-                       "l2": "inputs larger than L2: each step streams %.2f GB of links and spinors (L2 = 126 MB)"
-                             % (sum(cm["ops"][k][1] for k in ops_run) / 1e9),
+                       "l2": "inputs larger than L2: each step streams %.2f GB of links and spinors (L2 = 126 MB) and rotates over %d spinor sets"
+                             % (sum(cm["ops"][k][1] for k in ops_run) / 1e9, NSETS),
                        "parallelism": "replicas x%d (no sharding; DESIGN.md)" % world},
             "gpu_launches": launches,
             "per_op": per_op,
             "roofline": roofline,
+            "roofline_C4_f64_Dphi_hat": roofline_c4,
             "e2e": e2e,
+            "per_config": per_config,
+            "per_config_seconds": sweep_s,
             "next1_linalg_cg": extras,
             "cpu_baseline": cpu,
             "clocks": clocks,
@@ -324,6 +455,17 @@ def run_ours(args):
         print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def sweep_bytes(cfg, prec, rebuild):
+    """device memory one configuration of the sweep needs: links (fundamental + represented), canonical inputs while they
+    are imported, 2 x NSETS full spinors, work space of the two-pass operators"""
+    w = 8 if prec == "f64" else 4
+    V, d, N = cfg.volume, cfg.d_R, cfg.n_g
+    S = 8 * d * w
+    K = d * d * (1 if cfg.rep == 1 else 2) * w
+    KF = 2 * N * N * w
+    return V * (8 * KF + (0 if rebuild else 8 * K) + 4 * KF + (2 * NSETS + 3) * S) + (2 << 30)
 
 
 def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, peak):
@@ -536,6 +678,7 @@ def main():
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--custom", default="", help="N_g,rep,T,L instead of --config (rep: 0 FUND, 1 ADJ, 2 SYM, 3 2AS); per-op table only")
     ap.add_argument("--link-mode", default="stored", choices=["stored", "rebuild"])
+    ap.add_argument("--sweep", default="all", help="per_config sweep after the headline: all | none | comma list of C2..C5")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the linear-algebra / CG measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -91,11 +91,14 @@ def torch_field_fetch(canon):
 
 
 def sample_sites(cfg, n, parity=None, seed=0):
-    """Canonical indices: the lattice corners/edges (boundary wraps) plus random interior sites."""
+    """Canonical indices: the lattice corners/edges (boundary wraps), sites of the last tile of the kernels' grid rounds,
+    plus random interior sites."""
     T, L = cfg.T, cfg.L
     rng = np.random.default_rng(seed)
     picks = [0, cfg.volume - 1, index_of((T - 1, 0, L - 1, 0), L), index_of((0, L - 1, 0, L - 1), L),
              index_of((T // 2, L // 2, 1, L - 1), L), index_of((T - 1, L - 1, L - 1, L - 2), L)]
+    if n >= 16:
+        picks += round_end_sites(cfg, parity, n // 2, seed)
     picks += list(rng.integers(0, cfg.volume, size=4 * n))
     out = []
     for ix in picks:
@@ -107,6 +110,40 @@ def sample_sites(cfg, n, parity=None, seed=0):
         if len(out) == n:
             break
     return out
+
+
+def native_to_canonical(cfg, parity, h):
+    """Canonical index of the site with half index h of `parity` in the library's documented site order (DESIGN.md 4:
+    h = ((t L + x) L + y) L/2 + zh, z = 2 zh + ((t+x+y+parity) & 1)).  Used only to AIM samples at particular tiles."""
+    L, Lh = cfg.L, cfg.L // 2
+    zh = h % Lh; r = h // Lh
+    y = r % L; r //= L
+    x = r % L; t = r // L
+    z = 2 * zh + ((t + x + y + parity) & 1)
+    return index_of((t, x, y, z), L)
+
+
+def round_end_sites(cfg, parity, n, seed=0):
+    """Sites in the LAST tile of a grid round of the persistent kernels (a round = all warps / pairs / groups of the grid
+    take one tile each), for every plausible round size, spread over the lattice, plus the ragged last tile."""
+    rng = np.random.default_rng(seed)
+    nh = cfg.volume // 2
+    n_tiles = (nh + 31) // 32
+    tiles = {n_tiles - 1}
+    for per_sm in (1, 2, 3, 4, 6, 8, 12, 16):          # tiles in flight per SM: groups, pairs or warps per CTA
+        R = 148 * per_sm
+        for k in (1, 2, 3, max(1, n_tiles // (2 * R)), max(1, n_tiles // R)):
+            for full_lattice in (1, 2):                # full-lattice launches interleave the parities: half the tiles per round
+                tl = k * R // full_lattice - 1
+                if 0 <= tl < n_tiles:
+                    tiles.add(tl)
+    tiles = sorted(tiles)
+    picks = []
+    for tl in tiles:
+        h = min(tl * 32 + int(rng.integers(0, 32)), nh - 1)
+        picks.append(native_to_canonical(cfg, parity if parity is not None else int(rng.integers(0, 2)), h))
+    rng.shuffle(picks)
+    return [int(v) for v in picks[:n]]
 
 
 def half_rank(ix):

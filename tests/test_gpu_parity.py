@@ -310,64 +310,113 @@ def test_apply_host_async_pipeline(env):
 
 
 # --------------------------------------------------------- full BASELINE sizes, sampled outputs
-def full_size_problem(env, name, prec):
+def full_size_problem(env, name, prec, rebuild=False):
     torch, hirep = env["torch"], env["hirep"]
     cfg = synth.CONFIGS[name]
     cdt = torch.complex128 if prec == "f64" else torch.complex64
     links, (psi,) = synth.make_inputs_torch(cfg, env["dev"], cdt, n_spinors=1)
     geom = hirep.Geometry(cfg.T, cfg.L, cfg.n_g, cfg.rep, prec, device=env["dev"])
     lf = geom.links_import(links)
+    if rebuild:
+        geom.set_link_mode(hirep.LINKS_REBUILD)   # the operators read the fundamental field
+        return cfg, geom, links, psi, lf
     lr = geom.links_to_rep(lf)
     del lf
     torch.cuda.empty_cache()
     return cfg, geom, links, psi, lr
 
 
+def half_canon(env, cfg, psi, parity):
+    """canonical half-lattice spinor = rows of that parity in increasing ix; row of ix is ix >> 1"""
+    torch = env["torch"]
+    idx = torch.arange(cfg.volume, device=env["dev"])
+    c = (idx // cfg.L ** 3) + (idx // cfg.L ** 2) % cfg.L + (idx // cfg.L) % cfg.L + idx % cfg.L
+    return psi[(c % 2) == parity].contiguous()
+
+
+def compare_sampled(out_canon, sites, ref_fn, row_of, tol, tag):
+    num = den = 0.0
+    for ix in sites:
+        ref = ref_fn(ix)
+        got = out_canon[row_of(ix)].cpu().numpy().astype(np.complex128)
+        num += float(np.sum(np.abs(got - ref) ** 2)); den += float(np.sum(np.abs(ref) ** 2))
+        assert np.linalg.norm(got - ref) <= 10 * tol * np.linalg.norm(ref), (tag, ix)
+    assert np.sqrt(num / den) < tol, tag
+
+
+NSAMP = 64      # sampled sites per operator: corners, the last tile of the kernels' grid rounds, random interior sites
+
 FULL = [("C2", "f64"), ("C2", "f32"), ("C3", "f64"), ("C3", "f32"), ("C4", "f64"), ("C4", "f32"), ("C5", "f64"), ("C5", "f32")]
+
+
+def run_sampled(env, name, prec, rebuild):
+    torch, hirep, oracle = env["torch"], env["hirep"], env["oracle"]
+    cfg, geom, links, psi, lk = full_size_problem(env, name, prec, rebuild)
+    so = SampledOracle(oracle, cfg, links)
+    fetch = torch_field_fetch(psi)
+    tol = TOL[prec]
+    tag = (name, prec, "rebuild" if rebuild else "stored")
+    if "Dphi_eo" in cfg.ops:
+        x = geom.spinor_import(half_canon(env, cfg, psi, 1), hirep.ODD)
+        out = geom.spinor_export(geom.Dphi_eo(x, lk), hirep.EVEN)
+        compare_sampled(out, sample_sites(cfg, NSAMP, parity=0, seed=1), lambda ix: so.hop(fetch, ix), half_rank, tol, tag + ("Dphi_eo",))
+        del x, out
+    if "Dphi_hat" in cfg.ops:
+        x = geom.spinor_import(half_canon(env, cfg, psi, 0), hirep.EVEN)
+        out = geom.spinor_export(geom.Dphi_hat(cfg.m0, x, lk), hirep.EVEN)
+        compare_sampled(out, sample_sites(cfg, NSAMP, parity=0, seed=2), lambda ix: so.Dphi_hat(fetch, ix, cfg.m0), half_rank, tol, tag + ("Dphi_hat",))
+        del x, out
+    if "g5Dphi_sq" in cfg.ops:
+        x = geom.spinor_import(psi, hirep.FULL)
+        out = geom.spinor_export(geom.g5Dphi_sq(cfg.m0, x, lk), hirep.FULL)
+        compare_sampled(out, sample_sites(cfg, NSAMP, seed=3), lambda ix: so.g5Dphi_sq(fetch, ix, cfg.m0), lambda ix: ix, tol, tag + ("g5Dphi_sq",))
+        del x, out
+    geom.sync()
+    del lk, links, psi
+    torch.cuda.empty_cache()
 
 
 @pytest.mark.parametrize("name,prec", FULL)
 def test_full_size_sampled(env, name, prec):
-    """BASELINE lattice sizes, default launch configuration (the one bench.py times); outputs compared with the
-    oracle on sampled sites including the lattice corners (all boundary wraps)."""
+    """BASELINE lattice sizes, default launch configuration (the one bench.py times); outputs compared with the oracle on
+    64 sampled sites per operator: the lattice corners (all boundary wraps), a site from the last tile of every grid
+    round of the persistent kernels, random interior sites."""
+    run_sampled(env, name, prec, rebuild=False)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_full_size_sampled_rebuild_C4(env, prec):
+    """Link mode REBUILD (R rebuilt in the kernel from the fundamental links) at the full C4 size bench.py times it on."""
+    run_sampled(env, "C4", prec, rebuild=True)
+
+
+# ------------------------------------------------ full BASELINE sizes, the WHOLE output field (C2: all ops; C3: Dphi_eo)
+@pytest.mark.parametrize("name,prec", [("C2", "f64"), ("C2", "f32"), ("C3", "f64"), ("C3", "f32")])
+def test_full_size_whole_field(env, name, prec):
+    """Every output element of the bench launch configuration against the oracle at the BASELINE size: the oracle runs a
+    32^4 step in ~2 s, so C2 (all five operators) and C3 (Dphi_eo) are compared over the whole field, not on samples."""
     torch, hirep, oracle = env["torch"], env["hirep"], env["oracle"]
-    cfg, geom, links, psi, lr = full_size_problem(env, name, prec)
-    so = SampledOracle(oracle, cfg, links)
-    fetch = torch_field_fetch(psi)
+    cfg, geom, links, psi, lr = full_size_problem(env, name, prec, rebuild=False)
+    T, L, d, m0 = cfg.T, cfg.L, cfg.d_R, cfg.m0
     tol = TOL[prec]
-    nsamp = 6 if cfg.d_R > 8 else 12
-
-    def half_canon(parity):
-        # canonical half-lattice spinor = rows of that parity in increasing ix; row of ix is ix>>1
-        idx = torch.arange(cfg.volume, device=env["dev"])
-        c = (idx // cfg.L ** 3) + (idx // cfg.L ** 2) % cfg.L + (idx // cfg.L) % cfg.L + idx % cfg.L
-        return psi[(c % 2) == parity].contiguous()
-
-    def compare(out_canon, sites, ref_fn, row_of):
-        num = den = 0.0
-        for ix in sites:
-            ref = ref_fn(ix)
-            got = out_canon[row_of(ix)].cpu().numpy().astype(np.complex128)
-            num += float(np.sum(np.abs(got - ref) ** 2)); den += float(np.sum(np.abs(ref) ** 2))
-            assert np.linalg.norm(got - ref) <= 10 * tol * np.linalg.norm(ref), (name, prec, ix)
-        assert np.sqrt(num / den) < tol
-
-    if "Dphi_eo" in cfg.ops:
-        x = geom.spinor_import(half_canon(1), hirep.ODD)
-        out = geom.spinor_export(geom.Dphi_eo(x, lr), hirep.EVEN)
-        odd_only = lambda iy: fetch(iy)
-        compare(out, sample_sites(cfg, nsamp, parity=0, seed=1), lambda ix: so.hop(odd_only, ix), half_rank)
-        del x, out
-    if "Dphi_hat" in cfg.ops:
-        x = geom.spinor_import(half_canon(0), hirep.EVEN)
-        out = geom.spinor_export(geom.Dphi_hat(cfg.m0, x, lr), hirep.EVEN)
-        compare(out, sample_sites(cfg, max(4, nsamp // 3), parity=0, seed=2), lambda ix: so.Dphi_hat(fetch, ix, cfg.m0), half_rank)
-        del x, out
-    if "g5Dphi_sq" in cfg.ops:
-        x = geom.spinor_import(psi, hirep.FULL)
-        out = geom.spinor_export(geom.g5Dphi_sq(cfg.m0, x, lr), hirep.FULL)
-        compare(out, sample_sites(cfg, max(4, nsamp // 3), seed=3), lambda ix: so.g5Dphi_sq(fetch, ix, cfg.m0), lambda ix: ix)
-        del x, out
+    U = links.cpu().numpy().astype(np.complex128)
+    psi_h = psi.cpu().numpy().astype(np.complex128)
+    R = oracle.represent_field(cfg.n_g, cfg.rep, U)
+    del U
+    ev, od = synth.parity_sites(T, L, 0), synth.parity_sites(T, L, 1)
+    imp = lambda a, w: geom.spinor_import(torch.from_numpy(np.ascontiguousarray(a)).to(env["dev"]), w)
+    exp = lambda n, w: geom.spinor_export(n, w).cpu().numpy().astype(np.complex128)
+    errs = {}
+    errs["Dphi_eo"] = oracle.rel_l2(exp(geom.Dphi_eo(imp(psi_h[od], hirep.ODD), lr), hirep.EVEN), oracle.Dphi_eo(T, L, d, R, psi_h[od], BC))
+    if name == "C2":
+        errs["Dphi_oe"] = oracle.rel_l2(exp(geom.Dphi_oe(imp(psi_h[ev], hirep.EVEN), lr), hirep.ODD), oracle.Dphi_oe(T, L, d, R, psi_h[ev], BC))
+        errs["Dphi_hat"] = oracle.rel_l2(exp(geom.Dphi_hat(m0, imp(psi_h[ev], hirep.EVEN), lr), hirep.EVEN), oracle.Dphi_hat(T, L, d, m0, R, psi_h[ev], BC))
+        xf = imp(psi_h, hirep.FULL)
+        errs["Dphi"] = oracle.rel_l2(exp(geom.Dphi(m0, xf, lr), hirep.FULL), oracle.Dphi(T, L, d, m0, R, psi_h, BC))
+        errs["g5Dphi_sq"] = oracle.rel_l2(exp(geom.g5Dphi_sq(m0, xf, lr), hirep.FULL), oracle.g5Dphi_sq(T, L, d, m0, R, psi_h, BC))
     geom.sync()
-    del lr, links, psi
+    print(name, prec, {k: "%.2e" % v for k, v in errs.items()})
+    for k, v in errs.items():
+        assert v < tol, (name, prec, k, v)
+    del lr, links, psi, R
     torch.cuda.empty_cache()
