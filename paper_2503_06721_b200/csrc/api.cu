@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -233,6 +234,8 @@ extern "C" int hirep_links_to_rep(hirep_geom *g, void *native_rep, const void *n
 // ---- operators ------------------------------------------------------------------------------------
 static int hop(hirep_geom *g, HopLaunch L, const char *what) {
     L.max_ctas = g->tune_max_ctas;
+    static const int dbg = getenv("HIREP_DBG") ? atoi(getenv("HIREP_DBG")) : 0;
+    L.dbg = dbg;
     const int rc = g->prec == HIREP_F64 ? k_hop_f64(g->geo, g->N, g->rep, g->mode, g->variant, L, g->stream)
                                         : k_hop_f32(g->geo, g->N, g->rep, g->mode, g->variant, L, g->stream);
     return kern_result(g, rc, what);

@@ -6,6 +6,8 @@
 //   2 = direct-load kernel, two lanes per site           (hop_small.cuh, P = 2)
 //   3 = persistent kernel, link stream through a per-warp bulk-copy (TMA) ring in shared memory (hop_ring.cuh)
 //   4 = the same with two warps per tile, one per half-spinor component (hop_pair.cuh)
+//   5 = (= 0) full-lattice launches by the tile-pair kernel that stages every forward link once for both of its uses
+//       (hop_full.cuh); variants 1-4 force the gather-layout kernels on full-lattice launches too
 // Default for d_R <= 6: variant 3, except at d_R >= 5 in fp64 (one thread per site spills) and for the fp32 passes
 // with a diagonal term: variant 4 (measured on B200, profiles/).  Link mode REBUILD always runs variant 4.  Large d_R (>= 8) always uses the row-group
 // kernel of hop_large.cuh.
@@ -13,10 +15,16 @@
 #include "hop_large.cuh"
 #include "hop_rows.cuh"
 #include "hop_pair.cuh"
+#include "hop_full.cuh"
 
 namespace hirep {
 
 template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
+    // full-lattice launches whose diagonal term is the other parity's input: every link crosses the SM once (hop_full.cuh)
+    // Default where it wins on B200 (profiles/r02_hop_full.md): fp64 at d_R <= 3 (C1-C3: 0.26 -> 0.22 ms at C2 in bursts, on par under
+    // a sustained power-capped load).  In fp32 and at d_R >= 4 the gather-layout kernels are faster; variant 5 forces it anywhere.
+    if (hop_full_eligible(L) && (variant == 5 || (variant == 0 && sizeof(T) == 8 && DR <= 3))) return launch_hop_full<T, DR, REAL>(g, L, s);
+    if (variant == 5) variant = 0;
     if (variant == 0) {
         // one thread per site spills in fp64 from d_R = 5 on; in fp32 at d_R >= 5 only the passes with a diagonal
         // term (self block in shared memory, fewer ring stages) run better with two warps per tile (profiles/)

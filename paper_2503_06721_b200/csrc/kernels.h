@@ -23,6 +23,8 @@ struct HopLaunch {
     double am;          // twisted mass mu: the diagonal term is (a + i am gamma_5) self (Eq 51); 0 = plain Wilson
     int g5;             // multiply the result by gamma_5 = diag(1,1,-1,-1)
     int max_ctas;       // cap on the persistent grid (0 = one CTA per SM); tests use it to force many tiles per warp
+    int dbg;            // HIREP_DBG (development only, results become wrong): bit mu skips the backward-link gather of direction mu,
+                        // bit 4+mu the neighbour-spinor gathers of +-mu in hop_full.cuh -- traffic attribution under ncu
 };
 
 int k_spinor_import(const Geo &g, int prec, int dR, void *native, const void *canon, int which, cudaStream_t s);

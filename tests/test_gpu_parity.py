@@ -156,14 +156,16 @@ def test_operators_vs_oracle_reduced(env, name, T, L, prec):
 
 @pytest.mark.parametrize("name,T,L", [("C1", 4, 4), ("C2", 6, 6), ("C3", 2, 6), ("C4", 4, 6)])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("variant", [1, 2, 3, 4])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5])
 def test_kernel_variants(env, name, T, L, prec, variant):
     p = Problem(env, synth.CONFIGS[name].resized(T, L), prec)
     check_all_ops(env, p, variant)
 
 
 @pytest.mark.parametrize("name,prec,variant", [("C2", "f64", 3), ("C2", "f32", 3), ("C3", "f64", 3), ("C4", "f32", 3),
-                                               ("C4", "f64", 4), ("C2", "f64", 4), ("C3", "f32", 4)])
+                                               ("C4", "f64", 4), ("C2", "f64", 4), ("C3", "f32", 4),
+                                               ("C1", "f64", 5), ("C2", "f64", 5), ("C2", "f32", 5), ("C3", "f64", 5), ("C3", "f32", 5),
+                                               ("C4", "f64", 5), ("C4", "f32", 5)])
 @pytest.mark.parametrize("max_ctas", [1, 3])
 def test_persistent_loop(env, name, prec, variant, max_ctas):
     """Persistent kernels with MANY tiles per warp (grid capped at 1-3 CTAs: the bulk-copy ring wraps across tile
