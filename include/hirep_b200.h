@@ -273,6 +273,21 @@ int hirep_cg_g5Dphi_clover_hat_sq(hirep_geom *g, double m0, double csw, void *x_
 int hirep_cg_g5Dphi_blocks_hat_sq(hirep_geom *g, void *x_even, const void *b_even, const void *links, const void *blocks_even,
                                   const void *inv_blocks_odd, double tol, int maxiter, int *iters, double *relres);
 
+/* ---- fermion force of the hopping term (Sect. 2.5) ----
+ * With eta = (Q_m^2)^-1 psi and xi = Q_m eta (native full-lattice spinors the caller has computed, e.g. by hirep_cg_g5Dphi_sq
+ * and gamma_5 hirep_Dphi):
+ *   T_mu(x)   = tr_spin[ gamma_5 (1 - gamma_mu) { eta(x+mu) (x) xi^dagger(x) + xi(x+mu) (x) eta^dagger(x) } ]          (Eq 20)
+ *   F^a_mu(x) = -(1/T_FUND) Re tr[ i T_R^a U^R_mu(x) T_mu(x) ],  a = 0 .. N_g^2 - 2, T_FUND = 1/2                      (Eq 21)
+ * The printed Eq 21 has lost the generator; with i T_R^a (as in Eq 19) this is -(1/T_FUND) dS_f/d omega^a for
+ * U_mu(x) -> exp(i omega^a T^a) U_mu(x), S_f = psi^dagger (Q_m^2)^-1 psi (reading A32).  T_R^a = -i dR/d omega^a are the
+ * generators of the representation in the basis of reading A10/A11 (fundamental T^a = generalised Gell-Mann / 2).
+ * force_canonical: device buffer of hirep_force_bytes bytes, REAL numbers of the working precision in CANONICAL order
+ * [ix][mu][a] (ix = ((t L + x) L + y) L + z); overwritten.  links_rep: the stored represented field (boundary signs included: a
+ * hop across the edge contributes with bc_mu, Eq 61).  HIREP_EINVAL in HIREP_LINKS_REBUILD mode.  The first call builds the
+ * generator table (one small kernel + a host round trip; not capturable in a CUDA graph), later calls only enqueue one kernel. */
+int hirep_force_bytes(const hirep_geom *g, size_t *bytes, int *n_generators);
+int hirep_force_hopping(hirep_geom *g, void *force_canonical, const void *eta_full, const void *xi_full, const void *links_rep);
+
 /* Measurement utility: achieved TFLOP/s (2 flops per FMA) of a register-resident chain of
  * FMAs in the given precision on the current device, the ALU roofline the pipe utilisation is read against.
  * Synchronous; tflops is a host pointer. */

@@ -11,6 +11,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "../../include/hirep_b200.h"
 #include "hop_dispatch.cuh"
@@ -37,6 +38,8 @@ struct hirep_geom {
     int host_links_ready;
     double *h_scal;                 // pinned: the CG's scalars read back without blocking the launches behind them (lazy)
     cudaEvent_t ev_scal;
+    int *force_rowptr, *force_jk;   // sparse represented generators T_R^a for hirep_force_hopping (lazy)
+    void *force_val;
     long launches;
     int device;                     // CUDA device current at hirep_geom_create (-1: none); compute calls check it
     size_t bytes_spinor_half, bytes_links_fund, bytes_links_rep;
@@ -117,7 +120,7 @@ extern "C" int hirep_geom_destroy(hirep_geom *g) {
     if (!g) return HIREP_OK;
     for (void *b : g->ms_p)
         if (b) cudaFree(b);
-    void *bufs[] = {g->ws_exp, g->ws_half, g->ws_half2, g->ws_half3, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
+    void *bufs[] = {g->force_rowptr, g->force_jk, g->force_val, g->ws_exp, g->ws_half, g->ws_half2, g->ws_half3, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
                     g->h_in_native, g->h_out_native, g->h_out_canon, g->h_out_canon2};
     if (g->host_events) {
         for (int i = 0; i < 2; ++i) { cudaEventDestroy(g->ev_done[i]); cudaEventDestroy(g->ev_copied[i]); }
@@ -976,6 +979,63 @@ extern "C" int hirep_cg_g5Dphi_blocks_hat_sq(hirep_geom *g, void *x_even, const 
     CHECK_PTRS("hirep_cg_g5Dphi_blocks_hat_sq", x_even, b_even, links, blocks_even, inv_blocks_odd);
     return cg_solve(g, 0, 0.0, x_even, b_even, links, tol, maxiter, iters, relres, "hirep_cg_g5Dphi_blocks_hat_sq", 0, 0.0, nullptr, 0.0, blocks_even,
                     inv_blocks_odd);
+}
+
+// ---- fermion force of the hopping term (Eq 20-21): SURVEY.md 8(f) NEXT-4 --------------------------------------------
+static int force_table(hirep_geom *g) {
+    if (g->force_rowptr) return HIREP_OK;
+    const int NA = g->N * g->N - 1, d = g->dR;
+    const size_t n = (size_t)NA * d * d;
+    double2 *dense = nullptr;
+    cudaError_t e = cudaMalloc((void **)&dense, n * sizeof(double2));
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(HIREP_ENOMEM, "hirep_force_hopping: generator table: %s", cudaGetErrorString(e)); }
+    int rc = k_rep_generators(g->N, g->rep, dense, g->stream);
+    if (rc) { cudaFree(dense); return kern_result(g, rc, "hirep_force_hopping (generator table)"); }
+    std::vector<double2> h(n);
+    e = cudaMemcpyAsync(h.data(), dense, n * sizeof(double2), cudaMemcpyDeviceToHost, g->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
+    cudaFree(dense);
+    if (e != cudaSuccess) return cuda_fail(e, "hirep_force_hopping (generator table)");
+    g->launches += 1;
+    std::vector<int> rowptr(NA + 1, 0), jk;
+    std::vector<double2> val;
+    for (int a = 0; a < NA; ++a) {
+        for (int j = 0; j < d; ++j)
+            for (int k = 0; k < d; ++k) {
+                const double2 v = h[((size_t)a * d + j) * d + k];
+                if (fabs(v.x) > 1e-14 || fabs(v.y) > 1e-14) { jk.push_back(j * d + k); val.push_back(v); }
+            }
+        rowptr[a + 1] = (int)jk.size();
+    }
+    if (jk.empty()) { jk.push_back(0); val.push_back(make_double2(0, 0)); }   // SU(2) 2AS: the trivial representation has T_R = 0
+    void *p0 = nullptr, *p1 = nullptr, *p2 = nullptr;
+    e = cudaMalloc(&p0, rowptr.size() * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&p1, jk.size() * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&p2, val.size() * sizeof(double2));
+    if (e == cudaSuccess) e = cudaMemcpy(p0, rowptr.data(), rowptr.size() * sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(p1, jk.data(), jk.size() * sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(p2, val.data(), val.size() * sizeof(double2), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        cudaFree(p0); cudaFree(p1); cudaFree(p2); cudaGetLastError();
+        return fail(HIREP_ENOMEM, "hirep_force_hopping: generator table upload: %s", cudaGetErrorString(e));
+    }
+    g->force_rowptr = (int *)p0; g->force_jk = (int *)p1; g->force_val = p2;
+    return HIREP_OK;
+}
+extern "C" int hirep_force_bytes(const hirep_geom *g, size_t *bytes, int *n_generators) {
+    if (!g) return fail(HIREP_EINVAL, "hirep_force_bytes: NULL geometry");
+    const int NA = g->N * g->N - 1;
+    if (bytes) *bytes = (size_t)2 * g->geo.Nh * 4 * NA * (g->prec == HIREP_F64 ? 8 : 4);
+    if (n_generators) *n_generators = NA;
+    return HIREP_OK;
+}
+extern "C" int hirep_force_hopping(hirep_geom *g, void *force_canonical, const void *eta_full, const void *xi_full, const void *links_rep) {
+    CHECK_PTRS("hirep_force_hopping", force_canonical, eta_full, xi_full, links_rep);
+    if (g->mode != HIREP_LINKS_STORED) return fail(HIREP_EINVAL, "hirep_force_hopping: needs the stored represented links (HIREP_LINKS_STORED)");
+    int rc = force_table(g);
+    if (rc) return rc;
+    return kern_result(g, k_force_hopping(g->geo, g->prec, g->dR, g->real, eta_full, xi_full, links_rep, g->force_rowptr, g->force_jk, g->force_val,
+                                          g->N * g->N - 1, force_canonical, g->stream), "hirep_force_hopping");
 }
 
 extern "C" int hirep_fma_peak(int prec, double *tflops) {

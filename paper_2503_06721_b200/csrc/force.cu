@@ -1,0 +1,218 @@
+// force.cu -- fermion force of the hopping term (Eq 20-21).
+//
+//   T_mu(x)   = tr_spin[ gamma_5 (1 - gamma_mu) { eta(x+mu) (x) xi^dagger(x) + xi(x+mu) (x) eta^dagger(x) } ]        (Eq 20)
+//   F^a_mu(x) = -(1/T_FUND) Re tr[ i T_R^a U^R_mu(x) T_mu(x) ] = 2 Im tr[ T_R^a M ],   M = U^R_mu(x) T_mu(x)         (Eq 21, A32)
+//
+// The same neighbour gather, spin projection and link matvec as the stencil (steps a2-a3), followed by an outer product
+// in colour space that is never formed: with the rank-2 structure of gamma_5 (1 - gamma_mu),
+//   h^psi_s = psi_up(x+mu) - e_mu psi_low(x+mu)   (the forward projection of the stencil),
+//   k^psi_s = psi_up(x)    + e_mu psi_low(x)      (the (1 + gamma_mu) projection of the site's own spinor),
+//   M_kj = sum_s [ (U h^eta_s)_k conj(k^xi_s)_j + (U h^xi_s)_k conj(k^eta_s)_j ],
+// and the projection onto the algebra runs over the NON-ZERO entries of the represented generators T_R^a only (a sparse
+// table built once per geometry: T_R^a = -i dR/d omega^a, taken exactly as the odd part of the polynomial map R, A33).
+// One warp per (parity, tile, mu), lane = site; the eight vectors live in shared memory [vector][component][lane]
+// (conflict free), all loops run over run-time d_R, so one kernel serves every representation.
+#include <vector>
+
+#include "hop_small.cuh"
+#include "rep_maps.cuh"
+
+namespace hirep {
+namespace {
+
+// ---- generator table ------------------------------------------------------------------------------------------------
+// dense [a][A][B] double2, a < N^2-1, A,B < d_R:  T_R^a = (R(1 + iT^a) - R(1 - iT^a)) / (2i)
+template <int N> __device__ void fund_generator(int a, double sgn, cplx<double> *W) {   // W = 1 + sgn * i * T^a
+    for (int e = 0; e < N * N; ++e) W[e] = mk<double>(0, 0);
+    for (int i = 0; i < N; ++i) W[i * N + i].x = 1.0;
+    const GenIdx ga = gen_decode(a);
+    if (ga.kind == 0) {            // S_ij = (E_ij + E_ji)/2
+        W[ga.i * N + ga.j].y += sgn * 0.5;
+        W[ga.j * N + ga.i].y += sgn * 0.5;
+    } else if (ga.kind == 1) {     // A_ij = -i (E_ij - E_ji)/2  ->  i A_ij = (E_ij - E_ji)/2
+        W[ga.i * N + ga.j].x += sgn * 0.5;
+        W[ga.j * N + ga.i].x -= sgn * 0.5;
+    } else {                       // D_j = diag(1,..,1 (j times), -j, 0,..) / sqrt(2 j (j+1))
+        const double nrm = diag_norm(ga.j);
+        for (int r = 0; r < ga.j; ++r) W[r * N + r].y += sgn * nrm;
+        W[ga.j * N + ga.j].y -= sgn * nrm * ga.j;
+    }
+}
+
+struct LocalMat {
+    const cplx<double> *p;
+    __device__ __forceinline__ cplx<double> operator[](int e) const { return p[e]; }
+};
+
+template <int N, int REP> __global__ void rep_generators_kernel(double2 *table) {
+    using Map = RepMap<double, N, REP>;
+    constexpr int DR = Map::DR, NA = N * N - 1;
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= NA) return;
+    cplx<double> Wp[N * N], Wm[N * N];
+    fund_generator<N>(a, +1.0, Wp);
+    fund_generator<N>(a, -1.0, Wm);
+    const LocalMat P{Wp}, M{Wm};
+    double2 *out = table + (size_t)a * DR * DR;
+    if constexpr (REP == 1) {      // real rows; run-time row index keeps the code small for the large adjoints
+#pragma unroll 1
+        for (int A = 0; A < DR; ++A) {
+            double rp[DR], rm[DR];
+            adj_row_runtime<double, N>(P, A, rp);
+            adj_row_runtime<double, N>(M, A, rm);
+            for (int B = 0; B < DR; ++B) out[A * DR + B] = make_double2(0.0, -0.5 * (rp[B] - rm[B]));   // (r+ - r-)/(2i)
+        }
+    } else {
+        static_for<0, DR>([&](auto ac) {
+            constexpr int A = decltype(ac)::value;
+            cplx<double> rp[DR], rm[DR];
+            Map::template row<A>(P, rp);
+            Map::template row<A>(M, rm);
+            for (int B = 0; B < DR; ++B) {
+                const double dx = rp[B].x - rm[B].x, dy = rp[B].y - rm[B].y;
+                out[A * DR + B] = make_double2(0.5 * dy, -0.5 * dx);                                    // (dx + i dy)/(2i)
+            }
+        });
+    }
+}
+
+template <int N> int gen_by_rep(int rep, double2 *table, cudaStream_t s) {
+    constexpr int NA = N * N - 1;
+    const int nb = (NA + 31) / 32;
+    switch (rep) {
+    case 0: rep_generators_kernel<N, 0><<<nb, 32, 0, s>>>(table); break;
+    case 1: rep_generators_kernel<N, 1><<<nb, 32, 0, s>>>(table); break;
+    case 2: rep_generators_kernel<N, 2><<<nb, 32, 0, s>>>(table); break;
+    case 3: rep_generators_kernel<N, 3><<<nb, 32, 0, s>>>(table); break;
+    default: return KERR_UNSUPPORTED;
+    }
+    return (int)cudaGetLastError();
+}
+
+// ---- the force kernel -------------------------------------------------------------------------------------------------
+struct ForceTab {
+    const int *rowptr;      // [NA + 1] entries of generator a: rowptr[a] .. rowptr[a+1]
+    const int *jk;          // packed j * d_R + k of entry T^a_jk
+    const double2 *val;     // T^a_jk
+    int NA;
+};
+
+// psi_up + cs * (i?) psi_low  with the conventions of hop_small.cuh: (e_mu v)_s = k_mu(s) v_{q_mu(s)}
+template <typename T> __device__ __forceinline__ cplx<T> proj(const cplx<T> &u, const cplx<T> &v, T cs, bool imag) {
+    return imag ? mk<T>(fma(-cs, v.y, u.x), fma(cs, v.x, u.y)) : mk<T>(fma(cs, v.x, u.x), fma(cs, v.y, u.y));
+}
+
+template <typename T, bool REAL>
+__global__ void __launch_bounds__(256) force_hopping_kernel(const Geo g, int dR, const cplx<T> *eta, const cplx<T> *xi, const void *links_v,
+                                                           ForceTab tab, T *force, long n_units, size_t warp_smem) {
+    using C = cplx<T>;
+    using E = link_elem<T, REAL>;
+    extern __shared__ __align__(16) unsigned char smem_force[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const long unit = (long)blockIdx.x * (blockDim.x >> 5) + wib;          // (parity, tile, mu)
+    if (unit >= n_units) return;
+    const int mu = (int)(unit & 3);
+    const long pt = unit >> 2;
+    const int tile = (int)(pt % g.n_tiles), p = (int)(pt / g.n_tiles);
+    int h = tile * TILE + lane;
+    const bool active = h < g.Nh;
+    if (!active) h = g.Nh - 1;
+    int t, x, y, zh;
+    decode_site(g, h, t, x, y, zh);
+    const int hn = mu == 0 ? neighbour<0>(g, p, t, x, y, zh) : mu == 1 ? neighbour<1>(g, p, t, x, y, zh)
+                 : mu == 2 ? neighbour<2>(g, p, t, x, y, zh) : neighbour<3>(g, p, t, x, y, zh);
+    const int NC = 4 * dR;
+    const size_t half = (size_t)g.n_tiles * NC * TILE;                     // complex elements of a half-lattice spinor
+    // vectors [v][s][c][lane]: v = 0 h^eta, 1 h^xi, 2 k^eta, 3 k^xi, 4 chi^eta = U h^eta, 5 chi^xi
+    C *vec = reinterpret_cast<C *>(smem_force + (size_t)wib * warp_smem) + lane;
+    auto V = [&](int v, int s, int c) -> C & { return vec[(size_t)((v * 2 + s) * dR + c) * TILE]; };
+    const bool imag = (mu & 1), swap = (mu == 1 || mu == 2);
+    for (int f = 0; f < 2; ++f) {
+        const C *field = f ? xi : eta;
+        const C *own = field + (size_t)p * half + ((size_t)tile * NC) * TILE + lane;
+        const C *nb = field + (size_t)(1 - p) * half + ((size_t)(hn >> 5) * NC) * TILE + (hn & 31);
+        for (int s = 0; s < 2; ++s) {
+            const int qq = swap ? 1 - s : s;
+            const T sig = (mu < 2) ? T(-1) : (s ? T(1) : T(-1));           // DirInfo::sigma(s)
+            for (int c = 0; c < dR; ++c) {
+                V(f, s, c) = proj<T>(nb[(size_t)(s * dR + c) * TILE], nb[(size_t)((2 + qq) * dR + c) * TILE], -sig, imag);       // sg = -1
+                V(2 + f, s, c) = proj<T>(own[(size_t)(s * dR + c) * TILE], own[(size_t)((2 + qq) * dR + c) * TILE], sig, imag);  // sg = +1
+            }
+        }
+    }
+    // chi = U_mu(x) h: the forward matrix of the gather block (carries the boundary sign, L945)
+    const E *W = (const E *)links_v + ((((size_t)p * g.n_tiles + tile) * 8 + mu) * (size_t)dR * dR) * TILE + lane;
+    for (int i = 0; i < dR; ++i) {
+        C a0 = mk<T>(0, 0), a1 = a0, b0 = a0, b1 = a0;
+        for (int j = 0; j < dR; ++j) {
+            const E w = W[(size_t)(i * dR + j) * TILE];
+            mac<T>(a0, w, V(0, 0, j));
+            mac<T>(a1, w, V(0, 1, j));
+            mac<T>(b0, w, V(1, 0, j));
+            mac<T>(b1, w, V(1, 1, j));
+        }
+        V(4, 0, i) = a0; V(4, 1, i) = a1; V(5, 0, i) = b0; V(5, 1, i) = b1;
+    }
+    // F^a = 2 Im sum_{jk} T^a_jk M_kj,  M_kj = sum_s chi^eta_s[k] conj(k^xi_s[j]) + chi^xi_s[k] conj(k^eta_s[j])
+    const long ix = canonical_index(g, p, h);
+    T *out = force + ((size_t)ix * 4 + mu) * tab.NA;
+    for (int a = 0; a < tab.NA; ++a) {
+        T acc = 0;
+        for (int e = tab.rowptr[a]; e < tab.rowptr[a + 1]; ++e) {
+            const int jk = tab.jk[e], j = jk / dR, k = jk - j * dR;
+            const double2 tv = tab.val[e];
+            T mx = 0, my = 0;
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                const C ce = V(4, s, k), kx = V(3, s, j), cx = V(5, s, k), ke = V(2, s, j);
+                mx += ce.x * kx.x + ce.y * kx.y + cx.x * ke.x + cx.y * ke.y;       // Re(chi conj(k))
+                my += ce.y * kx.x - ce.x * kx.y + cx.y * ke.x - cx.x * ke.y;       // Im(chi conj(k))
+            }
+            acc += (T)tv.x * my + (T)tv.y * mx;                                   // Im(tv * M_kj)
+        }
+        if (active) out[a] = 2 * acc;
+    }
+}
+
+}  // namespace
+
+// dense generator table -> device (double2 [NA][dR][dR]); the caller converts it to the sparse form once
+int k_rep_generators(int N, int rep, void *table_dev, cudaStream_t s) {
+    double2 *t = (double2 *)table_dev;
+    switch (N) {
+    case 2: return gen_by_rep<2>(rep, t, s);
+    case 3: return gen_by_rep<3>(rep, t, s);
+    case 4: return gen_by_rep<4>(rep, t, s);
+    case 5: return gen_by_rep<5>(rep, t, s);
+    case 6: return gen_by_rep<6>(rep, t, s);
+    }
+    return KERR_UNSUPPORTED;
+}
+
+int k_force_hopping(const Geo &g, int prec, int dR, int real, const void *eta, const void *xi, const void *links, const int *rowptr,
+                    const int *jk, const void *val, int NA, void *force, cudaStream_t s) {
+    const size_t w = prec == 0 ? 16 : 8;
+    const size_t warp_smem = (size_t)6 * 2 * dR * TILE * w;
+    int wpc = (int)((200 * 1024) / warp_smem);
+    if (wpc < 1) wpc = 1;
+    if (wpc > 8) wpc = 8;
+    const long n_units = (long)2 * g.n_tiles * 4;
+    const unsigned grid = (unsigned)((n_units + wpc - 1) / wpc);
+    const size_t smem = warp_smem * wpc;
+    ForceTab tab{rowptr, jk, (const double2 *)val, NA};
+    cudaError_t e = cudaSuccess;
+#define LAUNCH(TT, RR)                                                                                                              \
+    do {                                                                                                                            \
+        auto kern = force_hopping_kernel<TT, RR>;                                                                                   \
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                                     \
+        if (e == cudaSuccess)                                                                                                       \
+            kern<<<grid, wpc * 32, smem, s>>>(g, dR, (const cplx<TT> *)eta, (const cplx<TT> *)xi, links, tab, (TT *)force, n_units, warp_smem); \
+    } while (0)
+    if (prec == 0) { if (real) LAUNCH(double, true); else LAUNCH(double, false); }
+    else { if (real) LAUNCH(float, true); else LAUNCH(float, false); }
+#undef LAUNCH
+    if (e != cudaSuccess) return (int)e;
+    return (int)cudaGetLastError();
+}
+
+}  // namespace hirep

@@ -38,7 +38,7 @@ SYMBOLS = [
     "hirep_clover_inv_bytes", "hirep_clover_inv_field", "hirep_Cphi_inv", "hirep_Dphi_clover_hat",
     "hirep_clover_exp_field", "hirep_Dphi_blocks", "hirep_Dphi_blocks_hat", "hirep_g5Dphi_clover_sq", "hirep_cg_g5Dphi_clover_sq",
     "hirep_g5Dphi_clover_hat_sq", "hirep_g5Dphi_blocks_hat_sq", "hirep_cg_g5Dphi_clover_hat_sq", "hirep_cg_g5Dphi_blocks_hat_sq",
-    "hirep_g5Dphi_blocks_sq", "hirep_cg_g5Dphi_blocks_sq",
+    "hirep_g5Dphi_blocks_sq", "hirep_cg_g5Dphi_blocks_sq", "hirep_force_bytes", "hirep_force_hopping",
 ]
 
 
@@ -125,6 +125,8 @@ def load():
     lib.hirep_cg_g5Dphi_clover_sq.argtypes = [vp, cd, cd, vp, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_Dphi_blocks.argtypes = [vp, vp, vp, vp, vp]
     lib.hirep_Dphi_blocks_hat.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.hirep_force_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t), ctypes.POINTER(ci)]
+    lib.hirep_force_hopping.argtypes = [vp, vp, vp, vp, vp]
     lib.hirep_g5Dphi_blocks_sq.argtypes = [vp, vp, vp, vp, vp]
     lib.hirep_cg_g5Dphi_blocks_sq.argtypes = [vp, vp, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_g5Dphi_clover_hat_sq.argtypes = [vp, cd, cd, vp, vp, vp, vp, vp]
@@ -304,6 +306,15 @@ def hirep_cg_g5Dphi_clover_sq(g, m0, csw, x, b, links, clover, tol, maxiter):
     it, res = ctypes.c_int(), (ctypes.c_double * 2)()
     _check(load().hirep_cg_g5Dphi_clover_sq(g, m0, csw, x, b, links, clover, tol, maxiter, ctypes.byref(it), res))
     return it.value, res[0]
+
+
+def hirep_force_bytes(g):
+    nb, na = ctypes.c_size_t(), ctypes.c_int()
+    _check(load().hirep_force_bytes(g, ctypes.byref(nb), ctypes.byref(na)))
+    return nb.value, na.value
+
+
+def hirep_force_hopping(g, force, eta, xi, links): _check(load().hirep_force_hopping(g, force, eta, xi, links))
 
 
 def hirep_g5Dphi_blocks_sq(g, out, inp, links, blocks_full): _check(load().hirep_g5Dphi_blocks_sq(g, out, inp, links, blocks_full))
@@ -599,6 +610,13 @@ class Geometry:
         out = self.new_spinor(FULL) if out is None else out
         it, res = hirep_cg_g5Dphi_clover_sq(self.handle, m0, csw, out.data_ptr(), b.data_ptr(), links.data_ptr(), clover.data_ptr(), tol, maxiter)
         return out, it, res
+
+    def force_hopping(self, eta, xi, links, out=None):
+        """F^a_mu(x) of Eq 20-21 as a real tensor [V, 4, N_g^2 - 1] in canonical site order."""
+        nb, na = hirep_force_bytes(self.handle)
+        out = out if out is not None else self.torch.empty((self.V, 4, na), dtype=self.rdtype, device=self.device)
+        hirep_force_hopping(self.handle, out.data_ptr(), eta.data_ptr(), xi.data_ptr(), links.data_ptr())
+        return out
 
     def g5Dphi_blocks_sq(self, inp, links, blocks_full, out=None):
         out = self.new_spinor(FULL) if out is None else out
