@@ -155,7 +155,8 @@ class ClockSampler:
 
 # ------------------------------------------------------------------- all configurations (SURVEY.md 8(d) timing)
 SWEEP = [("C2", "f64", False), ("C2", "f32", False), ("C3", "f64", False), ("C3", "f32", False), ("C4", "f64", False),
-         ("C4", "f32", False), ("C4", "f64", True), ("C4", "f32", True), ("C5", "f64", False), ("C5", "f32", False)]
+         ("C4", "f32", False), ("C4", "f64", True), ("C4", "f32", True), ("C5", "f64", False), ("C5", "f32", False),
+         ("C5", "f64", True), ("C5", "f32", True)]
 NSETS = 4          # rotating spinor buffer sets (C2 fp32 half spinors are 50 MB < L2: one set would be timed out of L2)
 
 

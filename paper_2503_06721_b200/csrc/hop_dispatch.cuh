@@ -16,6 +16,7 @@
 #include "hop_rows.cuh"
 #include "hop_pair.cuh"
 #include "hop_full.cuh"
+#include "hop_adjmf.cuh"
 
 namespace hirep {
 
@@ -50,7 +51,7 @@ template <typename T, int DR, bool REAL, int R, int TP> int hop_large_variant(co
 }
 
 // link mode REBUILD: the pair kernel with the fundamental block in the ring and R rebuilt row by row (rep_maps.cuh).
-// Instantiated for every (N_g, rep) with d_R <= 6.
+// Instantiated for every (N_g, rep) with d_R <= 6; the adjoint of SU(3..6) has its own matrix-free kernel.
 template <typename T, int N, int REP> int hop_rebuild(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
     using M = RepMap<T, N, REP>;
     if (variant != 0 && variant != 4) return KERR_UNSUPPORTED;
@@ -64,6 +65,11 @@ template <typename T> int hop_rebuild_by_config(const Geo &g, int N, int rep, in
     case 5: return hop_rebuild<T, 5, 0>(g, variant, L, s);
     case 6: return hop_rebuild<T, 6, 0>(g, variant, L, s);
     case 12: return hop_rebuild<T, 2, 1>(g, variant, L, s);   // ADJ SU(2), d_R = 3
+    // ADJ SU(3..6), d_R = 8..35: matrix-free, psi^a T^a -> W (psi^a T^a) W^dagger on the fundamental link (hop_adjmf.cuh)
+    case 13: return variant == 0 ? launch_hop_adjmf<T, 3>(g, L, s) : KERR_UNSUPPORTED;
+    case 14: return variant == 0 ? launch_hop_adjmf<T, 4>(g, L, s) : KERR_UNSUPPORTED;
+    case 15: return variant == 0 ? launch_hop_adjmf<T, 5>(g, L, s) : KERR_UNSUPPORTED;
+    case 16: return variant == 0 ? launch_hop_adjmf<T, 6>(g, L, s) : KERR_UNSUPPORTED;
     case 22: return hop_rebuild<T, 2, 2>(g, variant, L, s);   // SYM SU(2), SU(3): d_R = 3, 6
     case 23: return hop_rebuild<T, 3, 2>(g, variant, L, s);
     case 32: return hop_rebuild<T, 2, 3>(g, variant, L, s);   // 2AS SU(2), SU(3), SU(4): d_R = 1, 3, 6

@@ -196,15 +196,16 @@ def test_large_dR_kernels(env, n, rep, max_ctas, variant):
     check_all_ops(env, p, variant)
 
 
-REBUILD = [(2, FUND), (3, FUND), (4, FUND), (5, FUND), (6, FUND), (2, ADJ), (2, SYM), (3, SYM), (2, ASY), (3, ASY), (4, ASY)]
+REBUILD = [(2, FUND), (3, FUND), (4, FUND), (5, FUND), (6, FUND), (2, ADJ), (2, SYM), (3, SYM), (2, ASY), (3, ASY), (4, ASY),
+           (3, ADJ), (4, ADJ), (5, ADJ), (6, ADJ)]        # the last four: matrix-free adjoint (hop_adjmf.cuh)
 
 
 @pytest.mark.parametrize("n,rep", REBUILD)
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 def test_rebuild_mode(env, n, rep, prec):
     """Link mode REBUILD (`links` = the fundamental field, R rebuilt in registers, boundary sign applied to the
-    half spinor) against the oracle, every (N_g, rep) with d_R <= 6; non-trivial signs in two directions and a
-    ragged tail."""
+    half spinor) against the oracle, every (N_g, rep) with d_R <= 6 and the matrix-free adjoint of SU(3..6); non-trivial
+    signs in two directions and a ragged tail."""
     cfg = synth.Config("t", 6, 6, n, rep, -0.3, "haar", 700 + 10 * n + rep, ())
     check_all_ops(env, Problem(env, cfg, prec, bc=(-1, 1, -1, 1)), rebuild=True)
 
@@ -220,8 +221,8 @@ def test_rebuild_mode_persistent_and_unsupported(env):
     p.geom.set_link_mode(hirep.LINKS_STORED)
     b = p.to_numpy(p.geom.Dphi_hat(-0.3, x, p.links_rep), hirep.EVEN)
     assert env["oracle"].rel_l2(a, b) < 1e-14
-    # d_R > 6 has no rebuild kernel: loud error, no fallback
-    q = Problem(env, synth.CONFIGS["C5"].resized(2, 2), "f64")
+    # 2-index representations with d_R > 6 have no rebuild kernel: loud error, no fallback
+    q = Problem(env, synth.Config("t", 2, 2, 4, SYM, -0.4, "haar", 5, ()), "f64")
     q.geom.set_link_mode(hirep.LINKS_REBUILD)
     with pytest.raises(hirep.HirepError, match="no kernel instantiated"):
         q.geom.Dphi_eo(q.to_native(q.spinors[0][q.od], hirep.ODD), q.links_fund)
@@ -386,10 +387,21 @@ def test_full_size_sampled(env, name, prec):
     run_sampled(env, name, prec, rebuild=False)
 
 
+@pytest.mark.parametrize("name", ["C4", "C5"])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-def test_full_size_sampled_rebuild_C4(env, prec):
-    """Link mode REBUILD (R rebuilt in the kernel from the fundamental links) at the full C4 size bench.py times it on."""
-    run_sampled(env, "C4", prec, rebuild=True)
+def test_full_size_sampled_rebuild(env, name, prec):
+    """Link mode REBUILD (R rebuilt in the kernel from the fundamental links; C5: the matrix-free adjoint) at the full sizes
+    bench.py times it on."""
+    run_sampled(env, name, prec, rebuild=True)
+
+
+def test_adjoint_matrix_free_capped_grid(env):
+    """hop_adjmf.cuh with many site groups per warp (grid capped), SU(3) and SU(6), all operators."""
+    hirep = env["hirep"]
+    for n in (3, 6):
+        p = Problem(env, synth.Config("t", 4, 6, n, ADJ, -0.4, "haar", 910 + n, ()), "f64")
+        p.geom.set_tuning(hirep.TUNE_MAX_CTAS, 2)
+        check_all_ops(env, p, rebuild=True)
 
 
 # ------------------------------------------------ full BASELINE sizes, the WHOLE output field (C2: all ops; C3: Dphi_eo)
