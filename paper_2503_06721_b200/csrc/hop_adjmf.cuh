@@ -34,7 +34,7 @@ template <typename T, int N> struct AdjMfCfg {
     static constexpr int SPW = 32 / N;                       // sites per warp
     static constexpr int NCL = (DR + N - 1) / N;             // colours per lane (a = r + N m)
     static constexpr int NLD = (NC + N - 1) / N;             // neighbour components per lane (c = r + N m)
-    static constexpr uint32_t RAW = NC * SPW * sizeof(C);    // staged neighbour spinor [c][site]
+    static constexpr uint32_t RAW = 4 * NN * SPW * sizeof(C); // staged neighbour spinor [c][site] (4 d_R rows); reused for the 4 result matrices
     static constexpr uint32_t MAT = NN * SPW * sizeof(C);    // one N x N matrix per site [e][site]
     static constexpr uint32_t PER_WARP = RAW + 2 * MAT /* Psi_0, Psi_1 (then chi_0, chi_1) */ + 2 * MAT /* W double buffer */;
     static constexpr int WARPS = sizeof(T) == 8 ? 8 : 12;
@@ -80,10 +80,23 @@ __global__ void __launch_bounds__(AdjMfCfg<T, N>::WARPS * 32, 1) hop_adjmf_kerne
         const C *in = (const C *)(set ? L.set[1].in : L.set[0].in);
         const C *lk = (const C *)(set ? L.set[1].links : L.set[0].links) + ((size_t)tile * 8 * NN) * TILE + hl;   // fundamental gather block
 
-        // stage direction D: the neighbour spinor (lane r copies components r, r+N, ...) and row r of W_D
-        auto stage = [&](auto dc) {
-            constexpr int D = decltype(dc)::value;
-            const int hn = neighbour<D>(g, p_out, t, x, y, zh);
+        // the 8 hops run in a RUN-TIME loop: unrolled over the directions the kernel is ~8x the code and stalls on instruction
+        // fetch (ncu: 3.7 "no instruction" stalls per issued instruction).  Direction constants of hop_small.cuh at run time:
+        auto nbr = [&](int d) {
+            switch (d) {
+            case 0: return neighbour<0>(g, p_out, t, x, y, zh);
+            case 1: return neighbour<1>(g, p_out, t, x, y, zh);
+            case 2: return neighbour<2>(g, p_out, t, x, y, zh);
+            case 3: return neighbour<3>(g, p_out, t, x, y, zh);
+            case 4: return neighbour<4>(g, p_out, t, x, y, zh);
+            case 5: return neighbour<5>(g, p_out, t, x, y, zh);
+            case 6: return neighbour<6>(g, p_out, t, x, y, zh);
+            default: return neighbour<7>(g, p_out, t, x, y, zh);
+            }
+        };
+        // stage direction d: the neighbour spinor (lane r copies components r, r+N, ...) and row r of W_d
+        auto stage = [&](int d) {
+            const int hn = nbr(d);
             const C *src = in + ((size_t)(hn >> 5) * NC) * TILE + (hn & 31);
             if (lane_on) {
 #pragma unroll
@@ -91,37 +104,50 @@ __global__ void __launch_bounds__(AdjMfCfg<T, N>::WARPS * 32, 1) hop_adjmf_kerne
                     const int c = r + N * m;
                     if (c < NC) cp_async<sizeof(C)>(raw_s + (uint32_t)((c * SPW + sl) * sizeof(C)), src + (size_t)c * TILE);
                 }
-                const uint32_t wb = wsm_s + (D & 1) * Cfg::MAT;
+                const uint32_t wb = wsm_s + (d & 1) * Cfg::MAT;
 #pragma unroll
                 for (int k = 0; k < N; ++k)
-                    cp_async<sizeof(C)>(wb + (uint32_t)(((r * N + k) * SPW + sl) * sizeof(C)), lk + (size_t)(D * NN + r * N + k) * TILE);
+                    cp_async<sizeof(C)>(wb + (uint32_t)(((r * N + k) * SPW + sl) * sizeof(C)), lk + (size_t)(d * NN + r * N + k) * TILE);
             }
         };
 
-        C acc[4][NCL];
+        // the hop sum is accumulated in the MATRIX basis (row r of the four spin components' N x N matrices): the projection back
+        // onto the generators, chi^a = 2 tr(T^a chi), is linear and commutes with the sum over directions and with the spin
+        // reconstruction, so it is done once per site instead of once per direction
+        C acc[4][N];
 #pragma unroll
         for (int sp = 0; sp < 4; ++sp)
 #pragma unroll
-            for (int m = 0; m < NCL; ++m) acc[sp][m] = mk<T>(0, 0);
+            for (int k = 0; k < N; ++k) acc[sp][k] = mk<T>(0, 0);
 
         __syncwarp();                                         // the previous group's last reads of the staging area are done
-        stage(IntC<0>{});
-        static_for<0, 8>([&](auto dc) {
-            constexpr int D = decltype(dc)::value;
-            using DI = DirInfo<D>;
+        stage(0);
+#pragma unroll 1
+        for (int d = 0; d < 8; ++d) {
+            const int mu = d & 3;
+            const bool fwd = d < 4, imag = (mu & 1) != 0, swap = (mu == 1 || mu == 2);
+            const T sg = fwd ? T(-1) : T(1);
             cp_async_wait_all();
             __syncwarp();
-            const T sgn = (T)hop_sign_dir<D>(g, p_out, t, x, y, zh);
+            // boundary factor of the hop (Eq 61), applied to the half spinor
+            const int crd = mu == 0 ? t : mu == 1 ? x : mu == 2 ? y : 2 * zh + ((t + x + y + p_out) & 1);
+            const int ext = mu == 0 ? g.T : g.L;
+            const T sgn = (T)((fwd ? (crd == ext - 1) : (crd == 0)) ? g.bc[mu] : 1);
             const C *rw = raw + ssl;
-            // (a2) on-the-fly projection h_s^a = sgn (psi_s^a + cs psi_low^a) and row r of Psi_s = h_s^a T^a
+            // (a2) on-the-fly projection h_s^a = sgn (psi_s^a + k psi_low^a), k = cs or i cs, and row r of Psi_s = h_s^a T^a.
+            // (Projecting every colour once into shared memory and assembling from there -- each h^a is needed by two rows, the
+            // diagonal ones by all N -- was measured slower: two more warp barriers per direction, 0.64 -> 0.68 ms at C5 fp64.)
             C P[2][N];
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
-                const int qq = DI::swap ? 1 - s : s;
-                const T cs = (T)(DI::sg * DI::sigma(s)) * sgn;
+                const int qq = swap ? 1 - s : s;
+                const T sig = (mu < 2) ? T(-1) : (s ? T(1) : T(-1));
+                const T cs = sg * sig * sgn;
+                const T kr = imag ? T(0) : cs, ki = imag ? cs : T(0);
+                const C *pu = rw + (size_t)(s * DR) * SPW, *pl = rw + (size_t)((2 + qq) * DR) * SPW;
                 auto hval = [&](int aa) {
-                    const C u = rw[(s * DR + aa) * SPW], v = rw[((2 + qq) * DR + aa) * SPW];
-                    return DI::imag ? mk<T>(fma(-cs, v.y, sgn * u.x), fma(cs, v.x, sgn * u.y)) : mk<T>(fma(cs, v.x, sgn * u.x), fma(cs, v.y, sgn * u.y));
+                    const C u = pu[aa * SPW], v = pl[aa * SPW];
+                    return mk<T>(fma(kr, v.x, fma(-ki, v.y, sgn * u.x)), fma(kr, v.y, fma(ki, v.x, sgn * u.y)));
                 };
                 C dg = mk<T>(0, 0);                           // diagonal entry Psi_rr = sum_j h^{D_j} nrm_j (r < j: 1, r = j: -j)
 #pragma unroll
@@ -133,24 +159,25 @@ __global__ void __launch_bounds__(AdjMfCfg<T, N>::WARPS * 32, 1) hop_adjmf_kerne
                 }
 #pragma unroll
                 for (int k = 0; k < N; ++k) {
-                    if (k == r) { P[s][k] = dg; continue; }
-                    const int i = k < r ? k : r, j = k < r ? r : k;           // pair (i < j)
-                    const C hS = hval(gen_base(j) + 2 * i), hA = hval(gen_base(j) + 2 * i + 1);
+                    const int i = k < r ? k : r, j = k < r ? r : k;           // pair (i < j); k = r: unused
+                    const int as_ = k == r ? 0 : gen_base(j) + 2 * i;
+                    const C hS = hval(as_), hA = hval(as_ + 1);
                     // k > r: Psi_ij = (h^S - i h^A)/2 ;  k < r: Psi_ji = (h^S + i h^A)/2
                     const T sg2 = k > r ? T(1) : T(-1);
-                    P[s][k] = mk<T>(T(0.5) * (hS.x + sg2 * hA.y), T(0.5) * (hS.y - sg2 * hA.x));
+                    const C off = mk<T>(T(0.5) * (hS.x + sg2 * hA.y), T(0.5) * (hS.y - sg2 * hA.x));
+                    P[s][k] = k == r ? dg : off;
                 }
                 if (lane_on) {
 #pragma unroll
                     for (int k = 0; k < N; ++k) psi[(size_t)((s * NN + r * N + k) * SPW + sl)] = P[s][k];
                 }
             }
-            const C *wm = wsm + (size_t)(D & 1) * NN * SPW + ssl;
+            const C *wm = wsm + (size_t)(d & 1) * NN * SPW + ssl;
             C wr[N];
 #pragma unroll
             for (int k = 0; k < N; ++k) wr[k] = wm[(r * N + k) * SPW];
             __syncwarp();                                     // Psi complete; the staged spinor has been consumed
-            if constexpr (D < 7) stage(IntC<(D < 7 ? D + 1 : 7)>{});
+            if (d < 7) stage(d + 1);
             // (a3) A_s = W Psi_s, chi_s = A_s W^dagger
             C chi[2][N];
 #pragma unroll
@@ -175,46 +202,57 @@ __global__ void __launch_bounds__(AdjMfCfg<T, N>::WARPS * 32, 1) hop_adjmf_kerne
                     chi[s][k] = c_;
                 }
             }
-            __syncwarp();                                     // every row has finished reading Psi
-            if (lane_on) {
+            // (a4) reconstruct + accumulate, entry by entry: lower component q(s) += sg conj(k_mu(s)) chi, i.e. times cl or -i cl
 #pragma unroll
-                for (int s = 0; s < 2; ++s)
+            for (int s = 0; s < 2; ++s) {
+                const T sig = (mu < 2) ? T(-1) : (s ? T(1) : T(-1));
+                const T cl = sg * sig;
+                const bool to0 = (swap ? 1 - s : s) == 0;   // lower component 0 or 1, selected without dynamic register indexing
 #pragma unroll
-                    for (int k = 0; k < N; ++k) psi[(size_t)((s * NN + r * N + k) * SPW + sl)] = chi[s][k];
-            }
-            __syncwarp();
-            // chi^a = 2 tr(T^a chi) for this lane's colours a = r + N m, then (a4) reconstruct + accumulate
-#pragma unroll
-            for (int m = 0; m < NCL; ++m) {
-                const int aa = r + N * m;
-                if (aa < DR) {
-                    const GenIdx ga = gen_decode(aa);
-#pragma unroll
-                    for (int s = 0; s < 2; ++s) {
-                        const C *cs_ = psi + (size_t)(s * NN) * SPW + ssl;
-                        C v;
-                        if (ga.kind == 2) {
-                            C sum = mk<T>(0, 0);
-                            for (int q = 0; q < ga.j; ++q) { const C d_ = cs_[(q * N + q) * SPW]; sum.x += d_.x; sum.y += d_.y; }
-                            const C dj = cs_[(ga.j * N + ga.j) * SPW];
-                            const T f = (T)(2.0 * diag_norm(ga.j));
-                            v = mk<T>(f * (sum.x - ga.j * dj.x), f * (sum.y - ga.j * dj.y));
-                        } else {
-                            const C cij = cs_[(ga.i * N + ga.j) * SPW], cji = cs_[(ga.j * N + ga.i) * SPW];
-                            if (ga.kind == 0) v = mk<T>(cij.x + cji.x, cij.y + cji.y);              // chi_ij + chi_ji
-                            else v = mk<T>(cji.y - cij.y, cij.x - cji.x);                           // -i (chi_ji - chi_ij)
-                        }
-                        acc[s][m].x += v.x;
-                        acc[s][m].y += v.y;
-                        const T cl = (T)(DI::sg * DI::sigma(s));
-                        const int qq = DI::swap ? 1 - s : s;
-                        if (DI::imag) { acc[2 + qq][m].x += cl * v.y; acc[2 + qq][m].y -= cl * v.x; }
-                        else { acc[2 + qq][m].x += cl * v.x; acc[2 + qq][m].y += cl * v.y; }
-                    }
+                for (int k = 0; k < N; ++k) {
+                    const C v = chi[s][k];
+                    const C add = imag ? mk<T>(cl * v.y, -cl * v.x) : mk<T>(cl * v.x, cl * v.y);
+                    acc[s][k].x += v.x;
+                    acc[s][k].y += v.y;
+                    acc[2][k].x += to0 ? add.x : T(0); acc[2][k].y += to0 ? add.y : T(0);
+                    acc[3][k].x += to0 ? T(0) : add.x; acc[3][k].y += to0 ? T(0) : add.y;
                 }
             }
-            __syncwarp();                                     // chi consumed before the next direction overwrites the area
-        });
+            __syncwarp();                                     // every row has finished reading Psi and W before they are overwritten
+        }
+
+        // the four accumulated matrices -> shared memory (the staging area is free), then each lane projects its colours
+        // a = r + N m: out^a = 2 tr(T^a acc)
+        if (lane_on) {
+#pragma unroll
+            for (int sp = 0; sp < 4; ++sp)
+#pragma unroll
+                for (int k = 0; k < N; ++k) raw[(size_t)((sp * NN + r * N + k) * SPW + sl)] = acc[sp][k];
+        }
+        __syncwarp();
+        C res[4][NCL];
+#pragma unroll
+        for (int m = 0; m < NCL; ++m) {
+            const int aa = r + N * m;
+            const GenIdx ga = gen_decode(aa < DR ? aa : 0);
+#pragma unroll
+            for (int sp = 0; sp < 4; ++sp) {
+                const C *cs_ = raw + (size_t)(sp * NN) * SPW + ssl;
+                C v;
+                if (ga.kind == 2) {
+                    C sum = mk<T>(0, 0);
+                    for (int q = 0; q < ga.j; ++q) { const C d_ = cs_[(q * N + q) * SPW]; sum.x += d_.x; sum.y += d_.y; }
+                    const C dj = cs_[(ga.j * N + ga.j) * SPW];
+                    const T f = (T)(2.0 * diag_norm(ga.j));
+                    v = mk<T>(f * (sum.x - ga.j * dj.x), f * (sum.y - ga.j * dj.y));
+                } else {
+                    const C cij = cs_[(ga.i * N + ga.j) * SPW], cji = cs_[(ga.j * N + ga.i) * SPW];
+                    if (ga.kind == 0) v = mk<T>(cij.x + cji.x, cij.y + cji.y);              // chi_ij + chi_ji
+                    else v = mk<T>(cji.y - cij.y, cij.x - cji.x);                           // -i (chi_ji - chi_ij)
+                }
+                res[sp][m] = v;
+            }
+        }
 
         if (active) {
             C *out = (C *)(set ? L.set[1].out : L.set[0].out) + ((size_t)tile * NC) * TILE + hl;
@@ -227,7 +265,7 @@ __global__ void __launch_bounds__(AdjMfCfg<T, N>::WARPS * 32, 1) hop_adjmf_kerne
                 for (int m = 0; m < NCL; ++m) {
                     const int aa = r + N * m;
                     if (aa < DR) {
-                        C v = mk<T>(b * acc[sp][m].x, b * acc[sp][m].y);
+                        C v = mk<T>(b * res[sp][m].x, b * res[sp][m].y);
                         if (use_self) {
                             const C sv = self[(size_t)(sp * DR + aa) * TILE];
                             const T tm = sp < 2 ? am : -am;                                        // + i mu gamma_5 self (Eq 51)
