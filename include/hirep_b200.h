@@ -70,6 +70,33 @@ enum {
 int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep_geom **out);
 int hirep_geom_destroy(hirep_geom *g); /* frees the handle and its workspace; NULL is a no-op */
 
+/* ---- sharded operator: slab of a lattice block-partitioned in t over ranks (Fig 1; Sect. 4.8) ----
+ * One rank owns the global time slices [t_start, t_start + T_loc) of a T_glob x L^3 lattice.  Its geometry is a LOCAL lattice of
+ * T_loc + 2 slices: local slice 0 and T_loc + 1 are GHOST slices (global slices t_start - 1 and t_start + T_loc, mod T_glob), local
+ * slices 1 .. T_loc are owned.  Every buffer (spinors, links) has the local lattice's native size.  t_start, T_loc, T_glob even,
+ * so local parity = global parity XOR 1 on every rank (local slice t is global slice t_start - 1 + t).  The boundary factor bc_0
+ * sits where the GLOBAL lattice closes: hirep_links_to_rep puts it on the links of global slice T_glob - 1, so only the owning
+ * rank carries it (L945).  Links: import the fundamental field of the local lattice (owned slices plus the ghost slice BEFORE them,
+ * whose t-links the first owned slice's backward hop uses; the other ghost links are not read by owned sites).
+ * Spinors: per application the caller (a) packs the two faces of the input -- PROJECTED half spinors, 2 d_R complex per face site
+ * (L624) -- (b) ships them to the neighbour ranks (peer copy / NCCL send-recv; not this library's business), (c) unpacks what it
+ * received into the ghost slices, (d) applies the operator.  With hirep_set_region the interior can run while the faces are in
+ * flight and the two boundary slabs afterwards (the paper's inner/boundary split, Fig 1):
+ *     region OWNED (default for a slab) | INTERIOR (tiles whose hops reach no ghost slice) | BOUNDARY (the rest of OWNED) | ALL.
+ * Regions are honoured by hirep_Dphi, hirep_Dphi_eo, hirep_Dphi_oe and the other single-pass stencil calls (persistent kernels,
+ * link mode STORED or the d_R <= 6 REBUILD kernels); two-pass operators return HIREP_EUNSUPPORTED on a slab (a halo exchange belongs
+ * between their passes), reductions and linear algebra see the whole local buffers including ghosts.
+ * face: 0 = first owned slice, projected with (1 - gamma_0): goes to the PREVIOUS rank, which unpacks it (face 0) into its last
+ * ghost slice; 1 = last owned slice, (1 + gamma_0): goes to the NEXT rank, unpacked (face 1) into its ghost slice 0.  buf: device
+ * buffer of hirep_halo_bytes bytes; spinor_half: native half-lattice spinor of the local lattice (either parity).  unpack stores
+ * the ghost spinor (h, 0), whose projection inside the stencil is h again, so halo sites need no second code path. */
+enum { HIREP_REGION_ALL = 0, HIREP_REGION_OWNED = 1, HIREP_REGION_INTERIOR = 2, HIREP_REGION_BOUNDARY = 3 };
+int hirep_geom_create_slab(int T_glob, int L, int N_g, int rep, int prec, int t_start, int T_loc, hirep_geom **out);
+int hirep_set_region(hirep_geom *g, int region);
+int hirep_halo_bytes(const hirep_geom *g, size_t *bytes);
+int hirep_halo_pack(hirep_geom *g, int face, void *buf, const void *spinor_half);
+int hirep_halo_unpack(hirep_geom *g, int face, void *spinor_half, const void *buf);
+
 /* bc_mu = +-1 per direction (Eq 58-63).  The signs are baked into the represented links by
  * hirep_links_to_rep (the paper's implementation, L945), so call it again after changing them. */
 int hirep_geom_set_bc(hirep_geom *g, const int sign[4]);

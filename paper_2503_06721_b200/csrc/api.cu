@@ -23,6 +23,7 @@ struct hirep_geom {
     int N, rep, prec, dR, real;
     int mode, variant;
     int tune_max_ctas, sum_alg;   // hirep_set_tuning
+    int slab, region;             // hirep_geom_create_slab / hirep_set_region
     cudaStream_t stream;
     void *ws_half, *ws_half2, *ws_half3, *ws_full;   // workspace spinors (lazy)
     void *ws_red;                   // reduction partials + 4 result doubles (lazy)
@@ -105,6 +106,7 @@ extern "C" int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep
     g->geo.Nh = (int)(V / 2);
     g->geo.n_tiles = (g->geo.Nh + TILE - 1) / TILE;
     g->geo.bc[0] = -1; g->geo.bc[1] = g->geo.bc[2] = g->geo.bc[3] = 1;
+    g->geo.t0 = 0; g->geo.Tg = T;
     g->tune_max_ctas = 0; g->sum_alg = 2;
     g->N = N_g; g->rep = rep; g->prec = prec; g->dR = dR; g->real = (rep == HIREP_ADJ);
     const size_t w = prec == HIREP_F64 ? 8 : 4;
@@ -113,6 +115,36 @@ extern "C" int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep
     g->bytes_links_rep = (size_t)2 * g->geo.n_tiles * 8 * dR * dR * TILE * (g->real ? 1 : 2) * w;
     if (cudaGetDevice(&g->device) != cudaSuccess) { g->device = -1; cudaGetLastError(); }
     *out = g;
+    return HIREP_OK;
+}
+
+// ---- slab of a lattice block-partitioned in t (Fig 1) ---------------------------------
+extern "C" int hirep_geom_create_slab(int T_glob, int L, int N_g, int rep, int prec, int t_start, int T_loc, hirep_geom **out) {
+    if (!out) return fail(HIREP_EINVAL, "hirep_geom_create_slab: out is NULL");
+    *out = nullptr;
+    if (T_glob < 2 || (T_glob & 1) || T_loc < 2 || (T_loc & 1) || t_start < 0 || (t_start & 1) || t_start + T_loc > T_glob)
+        return fail(HIREP_EINVAL, "hirep_geom_create_slab: T_glob=%d t_start=%d T_loc=%d (all even, T_loc >= 2, t_start + T_loc <= T_glob)", T_glob, t_start, T_loc);
+    const int rc = hirep_geom_create(T_loc + 2, L, N_g, rep, prec, out);
+    if (rc) return rc;
+    (*out)->geo.t0 = (t_start - 1 + T_glob) % T_glob;   // local slice 0 is the ghost slice before the first owned one
+    (*out)->geo.Tg = T_glob;
+    (*out)->slab = 1;
+    (*out)->region = HIREP_REGION_OWNED;
+    return HIREP_OK;
+}
+extern "C" int hirep_set_region(hirep_geom *g, int region) {
+    if (!g) return fail(HIREP_EINVAL, "hirep_set_region: NULL geometry");
+    if (region < HIREP_REGION_ALL || region > HIREP_REGION_BOUNDARY) return fail(HIREP_EINVAL, "hirep_set_region: unknown region %d", region);
+    if (!g->slab && region != HIREP_REGION_ALL) return fail(HIREP_EINVAL, "hirep_set_region: only a slab geometry has owned / interior / boundary regions");
+    g->region = region;
+    return HIREP_OK;
+}
+static size_t halo_bytes(const hirep_geom *g) {
+    return (size_t)g->geo.L * g->geo.L * g->geo.Lh * 2 * g->dR * 2 * (g->prec == HIREP_F64 ? 8 : 4);
+}
+extern "C" int hirep_halo_bytes(const hirep_geom *g, size_t *bytes) {
+    if (!g || !bytes) return fail(HIREP_EINVAL, "hirep_halo_bytes: NULL argument");
+    *bytes = halo_bytes(g);
     return HIREP_OK;
 }
 
@@ -235,13 +267,45 @@ extern "C" int hirep_links_to_rep(hirep_geom *g, void *native_rep, const void *n
 }
 
 // ---- operators ------------------------------------------------------------------------------------
+static int hop_range(hirep_geom *g, HopLaunch L, int tb, int te, const char *what) {
+    L.tile_begin = tb; L.tile_end = te;
+    const int rc = g->prec == HIREP_F64 ? k_hop_f64(g->geo, g->N, g->rep, g->mode, g->variant, L, g->stream)
+                                        : k_hop_f32(g->geo, g->N, g->rep, g->mode, g->variant, L, g->stream);
+    return kern_result(g, rc, what);
+}
+// Regions of a slab in tiles of each parity (slice t = half indices [t S, (t+1) S), S = L^3/2; local slices 0 and T-1 are ghosts):
+//   OWNED    = slices 1 .. T-2;  INTERIOR = the tiles that lie entirely in slices 2 .. T-3 (no hop reaches a ghost slice);
+//   BOUNDARY = the rest of OWNED, i.e. the tiles touching slice 1 and those touching slice T-2 (two launches, one if they meet).
+// Tiles that straddle a slice boundary also compute a few sites of the neighbouring slice (ghost outputs are scratch).
 static int hop(hirep_geom *g, HopLaunch L, const char *what) {
     L.max_ctas = g->tune_max_ctas;
     static const int dbg = getenv("HIREP_DBG") ? atoi(getenv("HIREP_DBG")) : 0;
     L.dbg = dbg;
-    const int rc = g->prec == HIREP_F64 ? k_hop_f64(g->geo, g->N, g->rep, g->mode, g->variant, L, g->stream)
-                                        : k_hop_f32(g->geo, g->N, g->rep, g->mode, g->variant, L, g->stream);
-    return kern_result(g, rc, what);
+    if (!g->slab || g->region == HIREP_REGION_ALL) return hop_range(g, L, 0, 0, what);
+    const long S = (long)g->geo.L * g->geo.L * g->geo.Lh;
+    const int T = g->geo.T;
+    const int own_b = (int)(S / TILE), own_e = (int)(((T - 1) * S + TILE - 1) / TILE);
+    int int_b = (int)((2 * S + TILE - 1) / TILE), int_e = (int)(((T - 2) * S) / TILE);
+    if (int_e < int_b) int_e = int_b = (own_b + own_e) / 2 > own_b ? (own_b + own_e) / 2 : own_b;   // no interior: split point only
+    if (int_b < own_b) int_b = own_b;
+    if (int_e > own_e) int_e = own_e;
+    if (g->region == HIREP_REGION_OWNED) return hop_range(g, L, own_b, own_e, what);
+    if (g->region == HIREP_REGION_INTERIOR) return int_e > int_b ? hop_range(g, L, int_b, int_e, what) : HIREP_OK;
+    int rc = int_b > own_b ? hop_range(g, L, own_b, int_b, what) : HIREP_OK;
+    if (rc) return rc;
+    return own_e > int_e ? hop_range(g, L, int_e, own_e, what) : HIREP_OK;
+}
+extern "C" int hirep_halo_pack(hirep_geom *g, int face, void *buf, const void *spinor_half) {
+    CHECK_PTRS("hirep_halo_pack", buf, spinor_half);
+    if (!g->slab) return fail(HIREP_EINVAL, "hirep_halo_pack: not a slab geometry");
+    if (face != 0 && face != 1) return fail(HIREP_EINVAL, "hirep_halo_pack: face=%d (0 first owned slice, 1 last owned slice)", face);
+    return kern_result(g, k_halo_pack(g->geo, g->prec, g->dR, 0, face, buf, spinor_half, g->stream), "hirep_halo_pack");
+}
+extern "C" int hirep_halo_unpack(hirep_geom *g, int face, void *spinor_half, const void *buf) {
+    CHECK_PTRS("hirep_halo_unpack", spinor_half, buf);
+    if (!g->slab) return fail(HIREP_EINVAL, "hirep_halo_unpack: not a slab geometry");
+    if (face != 0 && face != 1) return fail(HIREP_EINVAL, "hirep_halo_unpack: face=%d", face);
+    return kern_result(g, k_halo_unpack(g->geo, g->prec, g->dR, 0, face, spinor_half, buf, g->stream), "hirep_halo_unpack");
 }
 static const char *links_parity(const hirep_geom *g, const void *links, int p) {
     const size_t total = g->mode == HIREP_LINKS_STORED ? g->bytes_links_rep : g->bytes_links_fund;
@@ -293,6 +357,7 @@ extern "C" int hirep_Dphi(hirep_geom *g, double m0, void *out_full, const void *
 
 // out_even = [gamma_5] ((4+m)^2 in_even - D_eo D_oe in_even): two half-lattice passes through the odd workspace
 static int dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links, int g5, const char *what) {
+    if (g->slab) return fail(HIREP_EUNSUPPORTED, "%s: on a slab compose the two passes yourself (Dphi_oe, halo exchange, Dphi_eo)", what);
     int rc = workspace(&g->ws_half, g->bytes_spinor_half);
     if (rc) return rc;
     rc = offdiag(g, g->ws_half, in_even, links, 1, what);
@@ -331,6 +396,7 @@ extern "C" int hirep_g5Dphi_hat_sq(hirep_geom *g, double m0, void *out_even, con
 extern "C" int hirep_g5Dphi_sq(hirep_geom *g, double m0, void *out_full, const void *in_full, const void *links) {
     CHECK_PTRS("hirep_g5Dphi_sq", out_full, in_full, links);
     if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_g5Dphi_sq: out aliases in");
+    if (g->slab) return fail(HIREP_EUNSUPPORTED, "hirep_g5Dphi_sq: on a slab compose the two applications yourself with a halo exchange in between");
     int rc = workspace(&g->ws_full, 2 * g->bytes_spinor_half);
     if (rc) return rc;
     rc = dphi_full(g, m0, g->ws_full, in_full, links, 1, "hirep_g5Dphi_sq (first g5 D)");

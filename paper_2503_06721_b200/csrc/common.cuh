@@ -24,7 +24,18 @@ struct Geo {
     int Nh;         // sites per parity
     int n_tiles;    // ceil(Nh / 32)
     int bc[4];      // +-1 per direction (Eq 58-63)
+    // Slab of a lattice that is block-partitioned in t over several GPUs (Fig 1): local slice t holds global slice
+    // (t + t0) mod Tg.  The boundary factor of direction 0 sits where the GLOBAL lattice closes (only the ranks owning global
+    // slices Tg-1 / 0 see it); the local wrap in t is never used by an owned site (ghost slices at both ends).  Undivided
+    // lattice: t0 = 0, Tg = T.
+    int t0, Tg;
 };
+// does the hop from local slice t in direction 0 cross the edge of the GLOBAL lattice?
+__host__ __device__ inline bool t_edge(const Geo &g, int t, bool fwd) {
+    int tg = t + g.t0;
+    if (tg >= g.Tg) tg -= g.Tg;
+    return fwd ? (tg == g.Tg - 1) : (tg == 0);
+}
 
 template <typename T> struct CplxOf;
 template <> struct CplxOf<double> { using type = double2; };
@@ -102,9 +113,9 @@ __host__ __device__ inline int hop_sign(const Geo &g, int p, int t, int x, int y
     const int mu = d & 3;
     const bool fwd = d < 4;
     const int z = 2 * zh + ((t + x + y + p) & 1);
-    const int c = (mu == 0) ? t : (mu == 1) ? x : (mu == 2) ? y : z;
-    const int ext = (mu == 0) ? g.T : g.L;
-    const bool cross = fwd ? (c == ext - 1) : (c == 0);
+    if (mu == 0) return t_edge(g, t, fwd) ? g.bc[0] : 1;
+    const int c = (mu == 1) ? x : (mu == 2) ? y : z;
+    const bool cross = fwd ? (c == g.L - 1) : (c == 0);
     return cross ? g.bc[mu] : 1;
 }
 

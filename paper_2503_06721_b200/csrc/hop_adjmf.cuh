@@ -132,7 +132,8 @@ __global__ void __launch_bounds__(AdjMfCfg<T, N>::WARPS * 32, 1) hop_adjmf_kerne
             // boundary factor of the hop (Eq 61), applied to the half spinor
             const int crd = mu == 0 ? t : mu == 1 ? x : mu == 2 ? y : 2 * zh + ((t + x + y + p_out) & 1);
             const int ext = mu == 0 ? g.T : g.L;
-            const T sgn = (T)((fwd ? (crd == ext - 1) : (crd == 0)) ? g.bc[mu] : 1);
+            const bool edge = mu == 0 ? t_edge(g, t, fwd) : (fwd ? (crd == ext - 1) : (crd == 0));
+            const T sgn = (T)(edge ? g.bc[mu] : 1);
             const C *rw = raw + ssl;
             // (a2) on-the-fly projection h_s^a = sgn (psi_s^a + k psi_low^a), k = cs or i cs, and row r of Psi_s = h_s^a T^a.
             // (Projecting every colour once into shared memory and assembling from there -- each h^a is needed by two rows, the

@@ -32,6 +32,7 @@ template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int
         const bool self = (L.a != 0.0) && L.set[0].self != nullptr;
         variant = (DR >= 5 && (sizeof(T) == 8 || self)) ? 4 : 3;
     }
+    if (L.tile_end > 0 && variant < 3) return KERR_UNSUPPORTED;   // slab regions: persistent kernels only
     switch (variant) {
     case 1: return launch_hop_small<T, DR, REAL, 1, 128>(g, L, s);
     case 2: return launch_hop_small<T, DR, REAL, 2, 128>(g, L, s);
@@ -46,7 +47,7 @@ template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int
 // variant 1 = the direct-load row-group kernel of round 1 (hop_large.cuh), kept for comparison
 template <typename T, int DR, bool REAL, int R, int TP> int hop_large_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
     if (variant == 0) return launch_hop_rows<T, DR, REAL, R, TP>(g, L, s);
-    if (variant == 1) return launch_hop_large<T, DR, REAL, R>(g, L, s);
+    if (variant == 1 && L.tile_end == 0) return launch_hop_large<T, DR, REAL, R>(g, L, s);
     return KERR_UNSUPPORTED;
 }
 
@@ -66,10 +67,10 @@ template <typename T> int hop_rebuild_by_config(const Geo &g, int N, int rep, in
     case 6: return hop_rebuild<T, 6, 0>(g, variant, L, s);
     case 12: return hop_rebuild<T, 2, 1>(g, variant, L, s);   // ADJ SU(2), d_R = 3
     // ADJ SU(3..6), d_R = 8..35: matrix-free, psi^a T^a -> W (psi^a T^a) W^dagger on the fundamental link (hop_adjmf.cuh)
-    case 13: return variant == 0 ? launch_hop_adjmf<T, 3>(g, L, s) : KERR_UNSUPPORTED;
-    case 14: return variant == 0 ? launch_hop_adjmf<T, 4>(g, L, s) : KERR_UNSUPPORTED;
-    case 15: return variant == 0 ? launch_hop_adjmf<T, 5>(g, L, s) : KERR_UNSUPPORTED;
-    case 16: return variant == 0 ? launch_hop_adjmf<T, 6>(g, L, s) : KERR_UNSUPPORTED;
+    case 13: return (variant == 0 && L.tile_end == 0) ? launch_hop_adjmf<T, 3>(g, L, s) : KERR_UNSUPPORTED;
+    case 14: return (variant == 0 && L.tile_end == 0) ? launch_hop_adjmf<T, 4>(g, L, s) : KERR_UNSUPPORTED;
+    case 15: return (variant == 0 && L.tile_end == 0) ? launch_hop_adjmf<T, 5>(g, L, s) : KERR_UNSUPPORTED;
+    case 16: return (variant == 0 && L.tile_end == 0) ? launch_hop_adjmf<T, 6>(g, L, s) : KERR_UNSUPPORTED;
     case 22: return hop_rebuild<T, 2, 2>(g, variant, L, s);   // SYM SU(2), SU(3): d_R = 3, 6
     case 23: return hop_rebuild<T, 3, 2>(g, variant, L, s);
     case 32: return hop_rebuild<T, 2, 3>(g, variant, L, s);   // 2AS SU(2), SU(3), SU(4): d_R = 1, 3, 6

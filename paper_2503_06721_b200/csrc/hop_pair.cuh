@@ -42,9 +42,9 @@ template <typename T> struct SmemMat {
 template <int D> __device__ __forceinline__ int hop_sign_dir(const Geo &g, int p, int t, int x, int y, int zh) {
     constexpr int mu = D & 3;
     constexpr bool fwd = D < 4;
-    const int c = (mu == 0) ? t : (mu == 1) ? x : (mu == 2) ? y : 2 * zh + ((t + x + y + p) & 1);
-    const int ext = (mu == 0) ? g.T : g.L;
-    return (fwd ? (c == ext - 1) : (c == 0)) ? g.bc[mu] : 1;
+    if (mu == 0) return t_edge(g, t, fwd) ? g.bc[0] : 1;
+    const int c = (mu == 1) ? x : (mu == 2) ? y : 2 * zh + ((t + x + y + p) & 1);
+    return (fwd ? (c == g.L - 1) : (c == 0)) ? g.bc[mu] : 1;
 }
 
 template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF, int REP = 0> struct PairCfg {
@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
     pair_sync(1 + pair);
 
     const bool two = L.nsets == 2;
-    const int total_tiles = g.n_tiles * L.nsets;
+    const int total_tiles = launch_tiles(g, L) * L.nsets;
     const int gp = blockIdx.x * PAIRS + pair, np = gridDim.x * PAIRS;
     if (gp >= total_tiles) return;
     const int my_tiles = (total_tiles - gp + np - 1) / np;
@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
         const int gt = gp + k * np;
         set_ = two ? (gt & 1) : 0;
         int sq = two ? (gt >> 1) : gt;
-        tile_ = sq;
+        tile_ = sq + L.tile_begin;
     };
 
     // producer state: the next chunk to issue is chunk iq_c of the pair's iq_k-th tile
@@ -333,7 +333,7 @@ int launch_hop_pair_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
     int n_sm = 0;
     if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
     const HopLaunch &L = L0;
-    const int grid = ring_grid(n_sm, L.max_ctas, g.n_tiles * L.nsets, PAIRS);
+    const int grid = ring_grid(n_sm, L.max_ctas, launch_tiles(g, L) * L.nsets, PAIRS);
     kern<<<grid, PAIRS * 64, Cfg::SMEM, s>>>(g, L);
     return (int)cudaGetLastError();
 }

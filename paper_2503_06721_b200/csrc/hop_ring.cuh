@@ -132,7 +132,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
     // full-lattice launches (nsets = 2) interleave the two parities tile by tile: the `self` spinor of an even tile is
     // the neighbour data of the odd tiles processed at the same time, so it is served by L2
     const bool two = L.nsets == 2;
-    const int total_tiles = g.n_tiles * L.nsets;
+    const int total_tiles = launch_tiles(g, L) * L.nsets;
     const int gw = blockIdx.x * WARPS + warp, nw = gridDim.x * WARPS;
     if (gw >= total_tiles) return;
     const int my_tiles = (total_tiles - gw + nw - 1) / nw;
@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
         const int gt = gw + k * nw;
         set_ = two ? (gt & 1) : 0;
         int sq = two ? (gt >> 1) : gt;
-        tile_ = sq;
+        tile_ = sq + L.tile_begin;
     };
 
     // chunk qi of this warp = chunk qi % CPT of its (qi / CPT)-th tile; a tile's chunks are consecutive in memory
@@ -326,7 +326,7 @@ int launch_hop_ring_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
     int n_sm = 0;
     if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
     const HopLaunch &L = L0;
-    const int grid = ring_grid(n_sm, L.max_ctas, g.n_tiles * L.nsets, WARPS);
+    const int grid = ring_grid(n_sm, L.max_ctas, launch_tiles(g, L) * L.nsets, WARPS);
     kern<<<grid, WARPS * 32, Cfg::SMEM, s>>>(g, L);
     return (int)cudaGetLastError();
 }

@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
     if constexpr (SELFBUF) group_sync(1 + grp, NG * 32);   // the group's self barrier is initialised before anyone waits on it
 
     const bool two = L.nsets == 2;
-    const int total_tiles = g.n_tiles * L.nsets;
+    const int total_tiles = launch_tiles(g, L) * L.nsets;
     const int gg = blockIdx.x * TP + grp, ngr = gridDim.x * TP;
     if (gg >= total_tiles) return;                                     // whole group leaves together
     const int my_tiles = (total_tiles - gg + ngr - 1) / ngr;
@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
     auto locate = [&](int k, int &set_, int &tile_) {
         const int gt = gg + k * ngr;
         set_ = two ? (gt & 1) : 0;
-        tile_ = two ? (gt >> 1) : gt;
+        tile_ = (two ? (gt >> 1) : gt) + L.tile_begin;
     };
     // chunk qi of this warp: tile qi / CPT, direction (qi % CPT) / NJB, column block qi % NJB; R row segments
     auto issue = [&](int qi, int slot) {
@@ -278,7 +278,7 @@ int launch_hop_rows_cfg(const Geo &g, const HopLaunch &L, cudaStream_t s) {
     static DevCache cache{};
     int n_sm = 0;
     if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
-    const int grid = ring_grid(n_sm, L.max_ctas, g.n_tiles * L.nsets, TP);
+    const int grid = ring_grid(n_sm, L.max_ctas, launch_tiles(g, L) * L.nsets, TP);
     kern<<<grid, Cfg::WARPS * 32, Cfg::SMEM, s>>>(g, L);
     return (int)cudaGetLastError();
 }

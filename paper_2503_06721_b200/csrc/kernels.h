@@ -23,10 +23,17 @@ struct HopLaunch {
     double am;          // twisted mass mu: the diagonal term is (a + i am gamma_5) self (Eq 51); 0 = plain Wilson
     int g5;             // multiply the result by gamma_5 = diag(1,1,-1,-1)
     int max_ctas;       // cap on the persistent grid (0 = one CTA per SM); tests use it to force many tiles per warp
+    int tile_begin, tile_end;   // tiles [begin, end) of each parity to compute (slab regions: interior / boundary); end = 0: all
     int dbg;            // HIREP_DBG (development only, results become wrong): bit mu skips the backward-link gather of direction mu,
                         // bit 4+mu the neighbour-spinor gathers of +-mu in hop_full.cuh -- traffic attribution under ncu
 };
 
+inline __host__ __device__ int launch_tiles(const Geo &g, const HopLaunch &L) { return L.tile_end > 0 ? L.tile_end - L.tile_begin : g.n_tiles; }
+
+// slab halo (half-spinor faces, L624): face = 0 first owned slice (projected with 1-gamma_0, for the previous rank's forward hop),
+// face = 1 last owned slice (1+gamma_0, for the next rank's backward hop); unpack writes ghost slice T-1 (face 0 data) or 0 (face 1 data)
+int k_halo_pack(const Geo &g, int prec, int dR, int parity, int face, void *buf, const void *spinor_half, cudaStream_t s);
+int k_halo_unpack(const Geo &g, int prec, int dR, int parity, int face, void *spinor_half, const void *buf, cudaStream_t s);
 int k_spinor_import(const Geo &g, int prec, int dR, void *native, const void *canon, int which, cudaStream_t s);
 int k_spinor_export(const Geo &g, int prec, int dR, void *canon, const void *native, int which, cudaStream_t s);
 int k_links_import(const Geo &g, int prec, int N, void *native_fund, const void *canon, cudaStream_t s);

@@ -118,4 +118,46 @@ int k_links_rep_export(const Geo &g, int prec, int dR, int real, void *canon, co
     return (int)cudaGetLastError();
 }
 
+// ---- slab halo: projected half-spinor faces (L624: "send only the projected half spinors") ---------------------------
+// The face of a slab = one time slice of one parity = the contiguous half-index range [t_f S, (t_f + 1) S), S = L^3/2.
+// face 0: first owned slice (t_f = 1), h = psi_up - e_0 psi_low = psi_up + psi_low : what (1 - gamma_0) needs at the previous rank
+// face 1: last owned slice (t_f = T-2), h = psi_up + e_0 psi_low = psi_up - psi_low : what (1 + gamma_0) needs at the next rank
+// Message layout [s * d_R + c][site of the slice]: 2 d_R complex per face site.  unpack writes the ghost spinor (h, 0): the
+// stencil's own projection of it returns h, so the kernels need no second code path for halo sites.
+template <typename T> __global__ void halo_pack_kernel(Geo g, int dR, int face, cplx<T> *buf, const cplx<T> *sp) {
+    const int S = g.L * g.L * g.Lh;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= S) return;
+    const int h = (face ? g.T - 2 : 1) * S + i, ncomp = 4 * dR;
+    const T sg = face ? T(-1) : T(1);
+    for (int c = 0; c < 2 * dR; ++c) {
+        const cplx<T> u = sp[spinor_off(h >> 5, c, h & 31, ncomp)], v = sp[spinor_off(h >> 5, 2 * dR + c, h & 31, ncomp)];
+        buf[(size_t)c * S + i] = mk<T>(u.x + sg * v.x, u.y + sg * v.y);
+    }
+}
+template <typename T> __global__ void halo_unpack_kernel(Geo g, int dR, int face, cplx<T> *sp, const cplx<T> *buf) {
+    const int S = g.L * g.L * g.Lh;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= S) return;
+    const int h = (face ? 0 : g.T - 1) * S + i, ncomp = 4 * dR;   // face-0 data (next rank's first slice) -> ghost slice T-1
+    for (int c = 0; c < 2 * dR; ++c) {
+        sp[spinor_off(h >> 5, c, h & 31, ncomp)] = buf[(size_t)c * S + i];
+        sp[spinor_off(h >> 5, 2 * dR + c, h & 31, ncomp)] = mk<T>(0, 0);
+    }
+}
+int k_halo_pack(const Geo &g, int prec, int dR, int parity, int face, void *buf, const void *spinor_half, cudaStream_t s) {
+    (void)parity;
+    const int S = g.L * g.L * g.Lh, nb = (S + 127) / 128;
+    if (prec == 0) halo_pack_kernel<double><<<nb, 128, 0, s>>>(g, dR, face, (cplx<double> *)buf, (const cplx<double> *)spinor_half);
+    else halo_pack_kernel<float><<<nb, 128, 0, s>>>(g, dR, face, (cplx<float> *)buf, (const cplx<float> *)spinor_half);
+    return (int)cudaGetLastError();
+}
+int k_halo_unpack(const Geo &g, int prec, int dR, int parity, int face, void *spinor_half, const void *buf, cudaStream_t s) {
+    (void)parity;
+    const int S = g.L * g.L * g.Lh, nb = (S + 127) / 128;
+    if (prec == 0) halo_unpack_kernel<double><<<nb, 128, 0, s>>>(g, dR, face, (cplx<double> *)spinor_half, (const cplx<double> *)buf);
+    else halo_unpack_kernel<float><<<nb, 128, 0, s>>>(g, dR, face, (cplx<float> *)spinor_half, (const cplx<float> *)buf);
+    return (int)cudaGetLastError();
+}
+
 }  // namespace hirep

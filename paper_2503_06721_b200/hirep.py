@@ -21,6 +21,7 @@ EVEN, ODD, FULL = 0, 1, 2
 LINKS_STORED, LINKS_REBUILD = 0, 1
 OP_DPHI, OP_DPHI_EO, OP_DPHI_OE, OP_DPHI_HAT, OP_G5DPHI_SQ = 0, 1, 2, 3, 4
 TUNE_MAX_CTAS, TUNE_SUM_ALGORITHM = 1, 2
+REGION_ALL, REGION_OWNED, REGION_INTERIOR, REGION_BOUNDARY = 0, 1, 2, 3
 OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM, EBREAKDOWN = 0, -1, -2, -3, -4, -5
 
 # every symbol include/hirep_b200.h declares
@@ -39,6 +40,7 @@ SYMBOLS = [
     "hirep_clover_exp_field", "hirep_Dphi_blocks", "hirep_Dphi_blocks_hat", "hirep_g5Dphi_clover_sq", "hirep_cg_g5Dphi_clover_sq",
     "hirep_g5Dphi_clover_hat_sq", "hirep_g5Dphi_blocks_hat_sq", "hirep_cg_g5Dphi_clover_hat_sq", "hirep_cg_g5Dphi_blocks_hat_sq",
     "hirep_g5Dphi_blocks_sq", "hirep_cg_g5Dphi_blocks_sq", "hirep_force_bytes", "hirep_force_hopping",
+    "hirep_geom_create_slab", "hirep_set_region", "hirep_halo_bytes", "hirep_halo_pack", "hirep_halo_unpack",
 ]
 
 
@@ -125,6 +127,11 @@ def load():
     lib.hirep_cg_g5Dphi_clover_sq.argtypes = [vp, cd, cd, vp, vp, vp, vp, cd, ci, ctypes.POINTER(ci), c2p]
     lib.hirep_Dphi_blocks.argtypes = [vp, vp, vp, vp, vp]
     lib.hirep_Dphi_blocks_hat.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.hirep_geom_create_slab.argtypes = [ci, ci, ci, ci, ci, ci, ci, ctypes.POINTER(vp)]
+    lib.hirep_set_region.argtypes = [vp, ci]
+    lib.hirep_halo_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t)]
+    lib.hirep_halo_pack.argtypes = [vp, ci, vp, vp]
+    lib.hirep_halo_unpack.argtypes = [vp, ci, vp, vp]
     lib.hirep_force_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t), ctypes.POINTER(ci)]
     lib.hirep_force_hopping.argtypes = [vp, vp, vp, vp, vp]
     lib.hirep_g5Dphi_blocks_sq.argtypes = [vp, vp, vp, vp, vp]
@@ -308,6 +315,25 @@ def hirep_cg_g5Dphi_clover_sq(g, m0, csw, x, b, links, clover, tol, maxiter):
     return it.value, res[0]
 
 
+def hirep_geom_create_slab(T_glob, L, N_g, rep, prec, t_start, T_loc):
+    h = ctypes.c_void_p()
+    _check(load().hirep_geom_create_slab(T_glob, L, N_g, rep, prec, t_start, T_loc, ctypes.byref(h)))
+    return h
+
+
+def hirep_set_region(g, region): _check(load().hirep_set_region(g, region))
+
+
+def hirep_halo_bytes(g):
+    nb = ctypes.c_size_t()
+    _check(load().hirep_halo_bytes(g, ctypes.byref(nb)))
+    return nb.value
+
+
+def hirep_halo_pack(g, face, buf, spinor_half): _check(load().hirep_halo_pack(g, face, buf, spinor_half))
+def hirep_halo_unpack(g, face, spinor_half, buf): _check(load().hirep_halo_unpack(g, face, spinor_half, buf))
+
+
 def hirep_force_bytes(g):
     nb, na = ctypes.c_size_t(), ctypes.c_int()
     _check(load().hirep_force_bytes(g, ctypes.byref(nb), ctypes.byref(na)))
@@ -373,13 +399,18 @@ def hirep_apply_host_async(g, op, m0, out_host_ptr, in_host_ptr, links_host_ptr)
 class Geometry:
     """Owns a hirep_geom handle; allocates native buffers as uint8 torch tensors on `device`."""
 
-    def __init__(self, T, L, N_g, rep, prec="f64", device=None, bc=None):
+    def __init__(self, T, L, N_g, rep, prec="f64", device=None, bc=None, slab=None):
+        """slab = (T_glob, t_start): T is then the number of OWNED slices and the local lattice has T + 2 (two ghost slices)."""
         import torch
         self.torch = torch
-        self.T, self.L, self.N_g, self.rep = T, L, N_g, rep
         self.prec = {"f64": F64, "f32": F32}[prec] if isinstance(prec, str) else prec
         self.device = torch.device(device if device is not None else "cuda:0")
-        self.handle = hirep_geom_create(T, L, N_g, rep, self.prec)
+        if slab is not None:
+            self.handle = hirep_geom_create_slab(slab[0], L, N_g, rep, self.prec, slab[1], T)
+            T = T + 2
+        else:
+            self.handle = hirep_geom_create(T, L, N_g, rep, self.prec)
+        self.T, self.L, self.N_g, self.rep = T, L, N_g, rep
         self.sizes = hirep_geom_sizes(self.handle)
         self.d_R = self.sizes["d_R"]
         self.cdtype = torch.complex128 if self.prec == F64 else torch.complex64
@@ -610,6 +641,15 @@ class Geometry:
         out = self.new_spinor(FULL) if out is None else out
         it, res = hirep_cg_g5Dphi_clover_sq(self.handle, m0, csw, out.data_ptr(), b.data_ptr(), links.data_ptr(), clover.data_ptr(), tol, maxiter)
         return out, it, res
+
+    def set_region(self, region): hirep_set_region(self.handle, region)
+
+    def halo_pack(self, face, spinor_half):
+        buf = self._buf(hirep_halo_bytes(self.handle))
+        hirep_halo_pack(self.handle, face, buf.data_ptr(), spinor_half.data_ptr())
+        return buf
+
+    def halo_unpack(self, face, spinor_half, buf): hirep_halo_unpack(self.handle, face, spinor_half.data_ptr(), buf.data_ptr())
 
     def force_hopping(self, eta, xi, links, out=None):
         """F^a_mu(x) of Eq 20-21 as a real tensor [V, 4, N_g^2 - 1] in canonical site order."""
