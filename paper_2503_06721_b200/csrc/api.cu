@@ -315,6 +315,10 @@ static int workspace(void **slot, size_t bytes) {
     if (*slot) return HIREP_OK;
     cudaError_t e = cudaMalloc(slot, bytes);
     if (e != cudaSuccess) { *slot = nullptr; cudaGetLastError(); return fail(HIREP_ENOMEM, "workspace allocation of %zu bytes failed: %s", bytes, cudaGetErrorString(e)); }
+    // once, at allocation: padding lanes of the library's own work fields hold zeros, never stale memory (they are excluded from every
+    // reduction, but kernels that copy whole tiles would otherwise carry garbage into the caller's padding)
+    e = cudaMemset(*slot, 0, bytes);
+    if (e != cudaSuccess) return cuda_fail(e, "workspace initialisation");
     return HIREP_OK;
 }
 

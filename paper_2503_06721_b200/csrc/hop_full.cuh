@@ -159,6 +159,8 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
         fence_mbar_init();
     }
     group_sync(1 + grp, GW * 32);
+    pdl_launch_dependents();
+    pdl_wait();
 
     const int gg = blockIdx.x * GROUPS + grp, ng = gridDim.x * GROUPS;
     if (gg >= g.n_tiles) return;                        // the whole group leaves together
@@ -309,6 +311,7 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
                 if (k + 1 < my_tiles) {
                     if (producer) {
                         mbar_wait(spempty_s, k & 1);            // ... and by every warp of the group
+                        fence_proxy_async();
                         issue_sp(gg + (k + 1) * ng);
                     }
                     enter_tile(k + 1);
@@ -353,6 +356,7 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
                 if (lane == 0) mbar_arrive(empty_s + 8 * slot);
                 if (q + STAGES < my_chunks) {
                     mbar_wait(empty_s + 8 * slot, phase);
+                    if (producer) fence_proxy_async();
                     issue_chunk(slot);
                 }
                 ++q;
@@ -446,8 +450,7 @@ template <typename T, int DR, bool REAL, bool SPLIT, int GROUPS, int STAGES, int
     int n_sm = 0;
     if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
     const int grid = ring_grid(n_sm, L.max_ctas, g.n_tiles, GROUPS);
-    kern<<<grid, GROUPS * Cfg::GW * 32, Cfg::SMEM, s>>>(g, L);
-    return (int)cudaGetLastError();
+    return launch_pdl(kern, grid, GROUPS * Cfg::GW * 32, Cfg::SMEM, s, g, L);
 }
 
 template <typename T, int DR, bool REAL> int launch_hop_full(const Geo &g, const HopLaunch &L, cudaStream_t s) {

@@ -93,6 +93,8 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
         fence_mbar_init();
     }
     pair_sync(1 + pair);
+    pdl_launch_dependents();
+    pdl_wait();
 
     const bool two = L.nsets == 2;
     const int total_tiles = launch_tiles(g, L) * L.nsets;
@@ -170,7 +172,7 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
         const bool c_active = active;
         if constexpr (SELF) {
             if (producer) {
-                if (k > 0) mbar_wait(selfempty_s, (k - 1) & 1);   // both warps have read the previous tile's block
+                if (k > 0) { mbar_wait(selfempty_s, (k - 1) & 1); fence_proxy_async(); }   // both warps have read the previous tile's block
                 const C *sp = (const C *)(c_set ? L.set[1].self : L.set[0].self) + ((size_t)c_tile * NC) * TILE;
                 mbar_expect_tx(selffull_s, Cfg::SELF_BYTES);
                 bulk_g2s_plain(self_s, sp, Cfg::SELF_BYTES, selffull_s);
@@ -225,6 +227,7 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
                 if (lane == 0) mbar_arrive(empty_s + 8 * slot);
                 if (producer && q + STAGES < my_chunks) {
                     mbar_wait(empty_s + 8 * slot, phase);
+                    fence_proxy_async();
                     issue(slot);
                 }
                 ++q;
@@ -277,6 +280,7 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
                     if (lane == 0) mbar_arrive(empty_s + 8 * slot);
                     if (producer && q + STAGES < my_chunks) {
                         mbar_wait(empty_s + 8 * slot, phase);
+                        fence_proxy_async();
                         issue(slot);
                     }
                     ++q;
@@ -334,8 +338,7 @@ int launch_hop_pair_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
     if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
     const HopLaunch &L = L0;
     const int grid = ring_grid(n_sm, L.max_ctas, launch_tiles(g, L) * L.nsets, PAIRS);
-    kern<<<grid, PAIRS * 64, Cfg::SMEM, s>>>(g, L);
-    return (int)cudaGetLastError();
+    return launch_pdl(kern, grid, PAIRS * 64, Cfg::SMEM, s, g, L);
 }
 
 // default shape of the pair kernel: PAIRS pairs per CTA; the chunk is the largest whole number of link rows that

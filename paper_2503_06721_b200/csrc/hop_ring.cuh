@@ -65,6 +65,31 @@ __device__ __forceinline__ void bulk_g2s_plain(uint32_t dst, const void *src, ui
                  : "memory");
 }
 
+// cross-proxy hand-off: shared-memory reads through the generic proxy (the consumers' ld.shared, ordered before this point by
+// __syncwarp / an mbarrier) must be ordered before the async-proxy write of the bulk copy that refills the same bytes
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// Programmatic dependent launch (PTX griddepcontrol): every stencil launch carries the programmatic-stream-serialization attribute,
+// so its CTAs may be scheduled while the previous kernel of the stream drains; pdl_wait() -- before the first global read -- blocks
+// until that kernel has completed and flushed, pdl_launch_dependents() lets the NEXT launch start its prologue early.  What is
+// overlapped is the launch latency, the barrier set-up and the pipeline fill of back-to-back passes (Dphi_hat, g5Dphi_sq, CG).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename K> inline int launch_pdl(K kern, int grid, int block, size_t smem, cudaStream_t s, const Geo &g, const HopLaunch &L) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return (int)cudaLaunchKernelEx(&cfg, kern, g, L);
+}
+
 // ring geometry for one instantiation; CHUNK = RPC rows of the link block of one direction of one tile
 template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC, bool SELF> struct RingCfg {
     using E = link_elem<T, REAL>;
@@ -128,6 +153,8 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
         fence_mbar_init();
     }
     __syncwarp();
+    pdl_launch_dependents();
+    pdl_wait();   // everything below reads global memory the previous kernel of the stream may have written
 
     // full-lattice launches (nsets = 2) interleave the two parities tile by tile: the `self` spinor of an even tile is
     // the neighbour data of the odd tiles processed at the same time, so it is served by L2
@@ -199,6 +226,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
             // the tile's own spinor: one contiguous block -> one bulk copy, consumed in the epilogue
             __syncwarp();   // every lane has finished reading the buffer in the previous epilogue
             if (lane == 0) {
+                fence_proxy_async();
                 const C *sp = (const C *)(c_set ? L.set[1].self : L.set[0].self) + ((size_t)c_tile * NC) * TILE;
                 mbar_expect_tx(selfbar_s, Cfg::SELF_BYTES);
                 bulk_g2s_plain(self_s, sp, Cfg::SELF_BYTES, selfbar_s);
@@ -259,7 +287,10 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
                 if (i % RPC == RPC - 1) {
                     // slot consumed by every lane -> refill it with the chunk STAGES ahead
                     __syncwarp();
-                    if (lane == 0 && q + STAGES < my_chunks) issue(q + STAGES, slot);
+                    if (lane == 0 && q + STAGES < my_chunks) {
+                        fence_proxy_async();
+                        issue(q + STAGES, slot);
+                    }
                     ++q;
                     if (++slot == STAGES) { slot = 0; phase ^= 1; }
                 }
@@ -327,8 +358,7 @@ int launch_hop_ring_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
     if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
     const HopLaunch &L = L0;
     const int grid = ring_grid(n_sm, L.max_ctas, launch_tiles(g, L) * L.nsets, WARPS);
-    kern<<<grid, WARPS * 32, Cfg::SMEM, s>>>(g, L);
-    return (int)cudaGetLastError();
+    return launch_pdl(kern, grid, WARPS * 32, Cfg::SMEM, s, g, L);
 }
 
 // a pass with a diagonal term (a != 0 and a self spinor) uses the SELF instantiation, a pure hop the plain one

@@ -67,6 +67,8 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
     }
     __syncwarp();
     if constexpr (SELFBUF) group_sync(1 + grp, NG * 32);   // the group's self barrier is initialised before anyone waits on it
+    pdl_launch_dependents();
+    pdl_wait();
 
     const bool two = L.nsets == 2;
     const int total_tiles = launch_tiles(g, L) * L.nsets;
@@ -169,6 +171,7 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
                 // every warp of the group has passed the previous tile's epilogue: its self block may be overwritten.
                 // One bulk copy fetches this tile's own spinor (a contiguous block); it is consumed 7 steps later.
                 if (wg == 0 && lane == 0) {
+                    fence_proxy_async();
                     const C *sp = (const C *)(c_set ? L.set[1].self : L.set[0].self) + ((size_t)c_tile * NC) * TILE;
                     mbar_expect_tx(selfbar_s, Cfg::SELF_BYTES);
                     bulk_g2s_plain(self_s, sp, Cfg::SELF_BYTES, selfbar_s);
@@ -196,7 +199,10 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
                     }
                 }
                 __syncwarp();
-                if (lane == 0 && q + STAGES < my_chunks) issue(q + STAGES, slot);
+                if (lane == 0 && q + STAGES < my_chunks) {
+                    fence_proxy_async();
+                    issue(q + STAGES, slot);
+                }
                 ++q;
                 if (++slot == STAGES) { slot = 0; phase ^= 1; }
             }
@@ -279,8 +285,7 @@ int launch_hop_rows_cfg(const Geo &g, const HopLaunch &L, cudaStream_t s) {
     int n_sm = 0;
     if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
     const int grid = ring_grid(n_sm, L.max_ctas, launch_tiles(g, L) * L.nsets, TP);
-    kern<<<grid, Cfg::WARPS * 32, Cfg::SMEM, s>>>(g, L);
-    return (int)cudaGetLastError();
+    return launch_pdl(kern, grid, Cfg::WARPS * 32, Cfg::SMEM, s, g, L);
 }
 
 // passes with a diagonal term stage the tile's own spinor through shared memory when it fits next to two ring stages
