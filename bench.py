@@ -61,9 +61,11 @@ OP_ORDER = ["links_to_rep", "Dphi_eo", "Dphi_oe", "Dphi", "Dphi_hat", "g5Dphi_sq
 
 
 def ncu_traffic(config, prec, op):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `op`, from the committed ncu capture
-    (profiles/r01b_traffic.csv; the command that made it is in profiles/r01b_summary.md)."""
-    path = os.path.join(ROOT, "profiles", "r01b_traffic.csv")
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `op`, from the committed ncu captures
+    (profiles/r02_traffic.csv, else profiles/r01b_traffic.csv; the commands that made them are in the .md beside them)."""
+    path = os.path.join(ROOT, "profiles", "r02_traffic.csv")
+    if not os.path.exists(path):
+        path = os.path.join(ROOT, "profiles", "r01b_traffic.csv")
     if not os.path.exists(path):
         return None
     import csv
@@ -207,10 +209,12 @@ class Fields:
 
 
 def op_row(cm, name, ms, peak):
-    fl, by, by_ideal = cm["ops"][name]
+    """Fractions are on SURVEY.md 8(d)'s COMPULSORY bytes (every datum crosses HBM once: Dphi (2S+4K)V, links_to_rep 4V(K_F+K)); the
+    bytes the gather layout actually streams (every link stored twice) are reported beside them as `*_as_executed`."""
+    fl, by_exec, by = cm["ops"][name]
     return {"ms": round(ms, 4), "gflops": round(fl / ms / 1e6, 1), "gbs": round(by / ms / 1e6, 1),
             "frac_hbm": round(by / ms / 1e6 / peak, 4), "frac_8TBs_nominal": round(by / ms / 1e6 / 8000.0, 4),
-            "gbs_survey_bytes": round(by_ideal / ms / 1e6, 1), "frac_survey_bytes": round(by_ideal / ms / 1e6 / peak, 4)}
+            "gbs_as_executed": round(by_exec / ms / 1e6, 1), "frac_as_executed": round(by_exec / ms / 1e6 / peak, 4)}
 
 
 def time_back_to_back(torch, fields, name, target_s=0.25, repeats=5, warm=10, nmax=100, nmin=10):
@@ -255,12 +259,16 @@ def sweep_config(torch, hirep, synth, dev, name, prec, rebuild, peak, variant=0,
                 in_step[k].append((a, b))
     torch.cuda.synchronize()
     out = {"d_R": cfg.d_R, "lattice": "%dx%d^3" % (cfg.T, cfg.L), "links": "rebuild" if rebuild else "stored", "ops": {}}
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
     for k in ops:
         ms, n = time_back_to_back(torch, fields, k)
         row = op_row(cm, k, ms, peak)
         row["launches_per_repeat"] = n
         row["ms_in_step"] = round(sum(a.elapsed_time(b) for a, b in in_step[k]) / len(in_step[k]), 4)
         out["ops"][k] = row
+    ck = sampler.stop()
+    out["clocks"] = {"sm_mhz": ck.get("sm_mhz"), "reasons": ck.get("reasons")}   # sustained back-to-back load: the power cap shows here
     if own:
         del fields
         torch.cuda.empty_cache()
@@ -431,6 +439,9 @@ def run_ours(args):
                            "unit": "GB/s", "frac": c4["frac_hbm"], "traffic": ncu_traffic("C4", "f64", "Dphi_hat"), "peak_source": peak_src,
                            "algorithmic_bytes": cost_model(synth.CONFIGS["C4"], "f64")["ops"]["Dphi_hat"][1],
                            "frac_of_8TBs_nominal": c4["frac_8TBs_nominal"], "timing": "back-to-back launches, median of 5 repeats"}
+        b2b = (per_config or {}).get("%s_%s%s" % (args.config, prec, "_rebuild" if rebuild else ""), {}).get("ops", {}).get("Dphi_eo")
+        if b2b:
+            roofline["back_to_back"] = {"ms": b2b["ms"], "achieved": b2b["gbs"], "frac": b2b["frac_hbm"]}
         out = {
             "metric": METRIC, "value": round(value, 1), "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": True, "scaling": "weak",
@@ -581,6 +592,18 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
             out["Dphi_expclover_hat"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3), "launches": 4}
             del E, Ei
         del cl
+    # NEXT-4: fermion force of the hopping term (Eq 20-21): both fields and the forward links once, N^2-1 reals per link out
+    try:
+        na = cfg.n_g ** 2 - 1
+        w = 8 if prec == "f64" else 4
+        fbuf = geom.force_hopping(x_full, z_full, lr)
+        ms = timeit(lambda: geom.force_hopping(x_full, z_full, lr, out=fbuf), reps=10)
+        by = (2 * S + 4 * cm["K"] + 4 * na * w) * V
+        out["force_hopping"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3),
+                                "note": "compulsory bytes (2S + 4K + 4(N^2-1)w) per site; one warp per (tile, mu), vectors in shared memory"}
+        del fbuf
+    except Exception as e:
+        out["force_hopping"] = {"error": str(e)}
     try:
         out["fma_peak_tflops"] = {"f64": round(hirep.hirep_fma_peak(hirep.F64), 2), "f32": round(hirep.hirep_fma_peak(hirep.F32), 2)}
     except Exception as e:   # measurement utility only
