@@ -4,10 +4,10 @@
 //
 // Why another kernel.  The half-lattice kernels (hop_ring / hop_pair) read the gather block of a tile: 8 matrices per
 // site, U_mu(x) and U_mu(x-mu)^dagger.  On the full lattice every U_mu(x) is needed twice -- forward by x, daggered
-// backward by x+mu -- so that scheme moves 8K per site where (2S+4K) is compulsory, and it asks L2 for
-// (10S+8K) per site: at SU(3) fp64 that is 3072 B x 1M sites / 0.26 ms = 12 TB/s, the measured throughput cap of the L2
-// slices (B300_MICROARCH.md: ~6300 B/clk).  The full-lattice operator was bound by L2 REQUESTS, not by HBM, so serving
-// the second use of a link out of L2 would not have helped: the bytes have to stay on the SM.
+// backward by x+mu -- so that scheme moves 8K per site where (2S+4K) is compulsory: 1.58x (SU(3), 32^4) to 2.0x the
+// compulsory DRAM traffic, 0.59 of the roofline.  It also asks L2 for (10S+8K) per site, 3.2 GB per launch at SU(3) fp64 -- 12 TB/s
+// at 0.26 ms, the order of what the L2 slices deliver (B300_MICROARCH.md) -- so the second use of a link is served ON THE SM here
+// rather than from L2.
 //
 // Scheme.  A GROUP of warps owns the tile PAIR (even tile k, odd tile k): the 64 sites (t,x,y,z) with the same half
 // index h in both parities.  Those sites are each other's z neighbours (and, for the rows inside the tile, y
