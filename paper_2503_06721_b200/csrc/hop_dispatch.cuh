@@ -22,9 +22,10 @@ namespace hirep {
 
 template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
     // full-lattice launches whose diagonal term is the other parity's input: every link crosses the SM once (hop_full.cuh)
-    // Default where it wins on B200 (profiles/r02_hop_full.md): fp64 at d_R <= 3 (C1-C3: 0.26 -> 0.22 ms at C2 in bursts, on par under
-    // a sustained power-capped load).  In fp32 and at d_R >= 4 the gather-layout kernels are faster; variant 5 forces it anywhere.
-    if (hop_full_eligible(L) && (variant == 5 || (variant == 0 && sizeof(T) == 8 && DR <= 3))) return launch_hop_full<T, DR, REAL>(g, L, s);
+    // Default where it wins on B200 (profiles/r02_summary.md): complex links at d_R <= 3 in both precisions (C1, C2: 0.26 -> 0.20 ms at C2 fp64,
+    // 0.130 -> 0.119 ms in fp32, in bursts; on par under a sustained power-capped load) and the real SU(2) adjoint in fp64 (C3: 0.98 -> 0.89 ms).
+    // Elsewhere the gather-layout kernels are faster; variant 5 forces it anywhere.
+    if (hop_full_eligible(L) && (variant == 5 || (variant == 0 && DR <= 3 && (sizeof(T) == 8 || !REAL)))) return launch_hop_full<T, DR, REAL>(g, L, s);
     if (variant == 5) variant = 0;
     if (variant == 0) {
         // one thread per site spills in fp64 from d_R = 5 on; in fp32 at d_R >= 5 only the passes with a diagonal

@@ -52,7 +52,7 @@ template <typename T> __device__ __forceinline__ void macc(cplx<T> &acc, const T
     acc.y = fma(w, h.y, acc.y);
 }
 
-template <typename T, int DR, bool REAL, bool SPLIT, int GROUPS, int STAGES, int RPC> struct FullCfg {
+template <typename T, int DR, bool REAL, bool SPLIT, int GROUPS, int STAGES, int RPC, bool NBREG = false> struct FullCfg {
     using E = link_elem<T, REAL>;
     using C = cplx<T>;
     static_assert(DR % RPC == 0, "rows per chunk must divide d_R");
@@ -62,7 +62,10 @@ template <typename T, int DR, bool REAL, bool SPLIT, int GROUPS, int STAGES, int
     static constexpr uint32_t SLOT = 4 * CH;                           // forward rows even | odd | gathered rows even | odd
     static constexpr uint32_t SB = 4 * DR * TILE * sizeof(C);          // one spinor tile
     static constexpr int NBC = SPLIT ? 2 * DR : 4 * DR;                // neighbour components a warp stages per direction
-    static constexpr uint32_t NBD = NBC * TILE * sizeof(C);            // one direction of a warp's neighbour buffer
+    // NBREG: the out-of-pair neighbour spinors travel through registers (read-only loads issued half a direction pair ahead)
+    // instead of a per-warp shared-memory buffer: 2 x 4 d_R x 512 B per warp go to the ring (one more stage or one more group)
+    static_assert(!NBREG || (!SPLIT && RPC == DR), "register neighbours: one thread per site, one chunk per direction pair");
+    static constexpr uint32_t NBD = NBREG ? 0 : NBC * TILE * sizeof(C);   // one direction of a warp's neighbour buffer
     static constexpr uint32_t XB = SPLIT ? 2 * 2 * DR * TILE * sizeof(C) : 0;   // cross contributions [parity][s][d_R][32]
     static constexpr size_t SP_OFF = (size_t)STAGES * SLOT, NB_OFF = SP_OFF + 2 * SB, X_OFF = NB_OFF + (size_t)GW * 2 * NBD;
     static constexpr size_t BAR_OFF = X_OFF + XB;
@@ -105,6 +108,24 @@ __device__ __forceinline__ void project_half(const cplx<T> *spo, const cplx<T> *
     }
 }
 
+// the same with the out-of-pair neighbour in registers (NBREG)
+template <typename T, int DR, typename DI>
+__device__ __forceinline__ void project_regs(const cplx<T> *spo, const cplx<T> (&nb)[4 * DR], bool in_tile, int ln, cplx<T> (&h)[2][DR]) {
+    using C = cplx<T>;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+        const int qq = DI::swap ? 1 - s : s;
+        const T cs = (T)(DI::sg * DI::sigma(s));
+#pragma unroll
+        for (int c = 0; c < DR; ++c) {
+            C u = nb[s * DR + c], v = nb[(2 + qq) * DR + c];
+            if (in_tile) { u = spo[(size_t)(s * DR + c) * TILE + ln]; v = spo[(size_t)((2 + qq) * DR + c) * TILE + ln]; }
+            if (DI::imag) h[s][c] = mk<T>(fma(-cs, v.y, u.x), fma(cs, v.x, u.y));
+            else h[s][c] = mk<T>(fma(cs, v.x, u.x), fma(cs, v.y, u.y));
+        }
+    }
+}
+
 // (a4) reconstruct + accumulate chi = W h of direction DI, row i, component s
 template <typename T, int DR, bool SPLIT, typename DI>
 __device__ __forceinline__ void accumulate(const cplx<T> &chi, int kk, int s, int i, cplx<T> (&up)[SPLIT ? 1 : 2][DR],
@@ -125,11 +146,11 @@ __device__ __forceinline__ void accumulate(const cplx<T> &chi, int kk, int s, in
     }
 }
 
-template <typename T, int DR, bool REAL, bool SPLIT, int GROUPS, int STAGES, int RPC>
+template <typename T, int DR, bool REAL, bool SPLIT, int GROUPS, int STAGES, int RPC, bool NBREG>
 __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_kernel(const Geo g, const HopLaunch L) {
     using C = cplx<T>;
     using E = link_elem<T, REAL>;
-    using Cfg = FullCfg<T, DR, REAL, SPLIT, GROUPS, STAGES, RPC>;
+    using Cfg = FullCfg<T, DR, REAL, SPLIT, GROUPS, STAGES, RPC, NBREG>;
     constexpr int GW = Cfg::GW, NC = 4 * DR, NE = DR * DR, CPD = Cfg::CPD, CPT = Cfg::CPT, NSC = SPLIT ? 1 : 2;
     constexpr uint32_t CH = Cfg::CH, SLOT = Cfg::SLOT, SB = Cfg::SB, NBD = Cfg::NBD;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -250,6 +271,17 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
         cp_async_arrive_noinc(nbfull_s);
     };
 
+    C nb[NBREG ? 4 * DR : 1];
+    auto fetch = [&](int hn, int mu_) {   // NBREG: the out-of-pair neighbour's 4 d_R components (in-pair ones are read from the staged tiles)
+        if constexpr (NBREG) {
+            if ((hn >> 5) != tile && !((L.dbg >> (4 + mu_)) & 1)) {
+                const C *src = in_nb + ((size_t)(hn >> 5) * NC) * TILE + (hn & 31);
+#pragma unroll
+                for (int c = 0; c < NC; ++c) nb[c] = ld_spinor<T>(src + (size_t)c * TILE);
+            }
+        }
+    };
+
     // ---- prologue
     iq_enter();
     {
@@ -258,7 +290,8 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
     }
     if (producer) issue_sp(gg);
     enter_tile(0);
-    stage_nb(IntC<0>{});
+    if constexpr (NBREG) fetch(neighbour<0>(g, par, t, x, y, zh), 0);
+    else stage_nb(IntC<0>{});
     int q = 0, slot = 0;
     uint32_t phase = 0, nbphase = 0;
     const T b = (T)L.b, ab = (T)(L.a / L.b), amb = (T)(L.am / L.b);
@@ -293,6 +326,74 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
             const int hnf = neighbour<MU>(g, par, t, x, y, zh), hnb = neighbour<4 + MU>(g, par, t, x, y, zh);
             const bool inf = (hnf >> 5) == c_tile, inb = (hnb >> 5) == c_tile;
             const int lnb = hnb & 31;
+            if constexpr (NBREG) {
+                // one chunk per direction pair: forward hop while the -mu neighbour is in flight, backward hop while the next +mu one is
+                const C *spo = sp + (size_t)(1 - par) * NC * TILE;
+                C hh[2][DR];
+                project_regs<T, DR, DF>(spo, nb, inf, hnf & 31, hh);
+                fetch(hnb, MU);
+                C chib[NSC][DR];
+#pragma unroll
+                for (int kk = 0; kk < NSC; ++kk)
+#pragma unroll
+                    for (int c = 0; c < DR; ++c) chib[kk][c] = mk<T>(0, 0);
+                mbar_wait(full_s + 8 * slot, phase);
+                const unsigned char *sl_ = ring + (size_t)slot * SLOT;
+                const E *Wo = reinterpret_cast<const E *>(sl_ + par * CH) + lane;
+                const E *Wb = inb ? reinterpret_cast<const E *>(sl_ + (1 - par) * CH) + lnb : reinterpret_cast<const E *>(sl_ + (2 + par) * CH) + lane;
+#pragma unroll
+                for (int i = 0; i < DR; ++i) {
+                    E w[DR];
+#pragma unroll
+                    for (int j = 0; j < DR; ++j) w[j] = Wo[(i * DR + j) * TILE];
+#pragma unroll
+                    for (int kk = 0; kk < 2; ++kk) {
+                        C chi = mk<T>(0, 0);
+#pragma unroll
+                        for (int j = 0; j < DR; ++j) mac<T>(chi, w[j], hh[kk][j]);
+                        accumulate<T, DR, SPLIT, DF>(chi, kk, kk, i, up, lo, lx);
+                    }
+                }
+                project_regs<T, DR, DB>(spo, nb, inb, lnb, hh);
+                if constexpr (MU < 3) {
+                    fetch(neighbour<MU + 1>(g, par, t, x, y, zh), MU + 1);
+                } else {
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(spempty_s);          // last read of the staged tiles by this warp
+                    if (k + 1 < my_tiles) {
+                        if (producer) {
+                            mbar_wait(spempty_s, k & 1);
+                            fence_proxy_async();
+                            issue_sp(gg + (k + 1) * ng);
+                        }
+                        enter_tile(k + 1);
+                        fetch(neighbour<0>(g, par, t, x, y, zh), 0);
+                    }
+                }
+#pragma unroll
+                for (int i = 0; i < DR; ++i) {
+                    E w[DR];
+#pragma unroll
+                    for (int j = 0; j < DR; ++j) w[j] = Wb[(i * DR + j) * TILE];   // row i of U_mu(x-mu)
+#pragma unroll
+                    for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+                        for (int j = 0; j < DR; ++j) macc<T>(chib[kk][j], w[j], hh[kk][i]);   // chi_j += conj(U_ij) h_i
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty_s + 8 * slot);
+                if (q + STAGES < my_chunks) {
+                    mbar_wait(empty_s + 8 * slot, phase);
+                    if (producer) fence_proxy_async();
+                    issue_chunk(slot);
+                }
+                ++q;
+                if (++slot == STAGES) { slot = 0; phase ^= 1; }
+#pragma unroll
+                for (int kk = 0; kk < NSC; ++kk)
+#pragma unroll
+                    for (int c = 0; c < DR; ++c) accumulate<T, DR, SPLIT, DB>(chib[kk][c], kk, kk, c, up, lo, lx);
+            } else {
             // (a2) both half spinors of this direction pair
             mbar_wait(nbfull_s, nbphase);
             nbphase ^= 1;
@@ -367,6 +468,7 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
             for (int kk = 0; kk < NSC; ++kk)
 #pragma unroll
                 for (int c = 0; c < DR; ++c) accumulate<T, DR, SPLIT, DB>(chib[kk][c], kk, SPLIT ? s_rt : kk, c, up, lo, lx);
+            }
         });
 
         if constexpr (SPLIT) {
@@ -399,22 +501,28 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
     }
 }
 
-// shape per instantiation: SPLIT in fp64 from d_R = 4 on (one thread per site would hold 2 x 4 d_R accumulators, two
-// half spinors and the column accumulators: > 255 registers); rows per chunk = the largest divisor of d_R whose slot
-// (4 parts) stays <= 19 KB; as many groups per CTA as leave room for two stages; then up to 4 stages
+// shape per instantiation (B200 sweeps, profiles/r02_summary.md): SPLIT in fp64 from d_R = 4 on (one thread per site would hold
+// 2 x 4 d_R accumulators, two half spinors and the column accumulators: > 255 registers).  NBREG (out-of-pair neighbours through
+// registers, whole matrices per slot) for complex links at d_R <= 3: the shared memory the neighbour buffers would take buys a fourth
+// group per SM (fp64: 8 warps; fp32: 8 groups = 16 warps) -- C2 fp64 0.224 -> 0.204 ms, fp32 0.144 -> 0.119 ms.  For the real SU(2)
+// adjoint on 48^4 (few in-pair neighbours, L/2 = 24 does not divide the tile) the buffered version measured faster and is kept.
+// Rows per chunk = the largest divisor of d_R whose slot (4 parts) stays <= 19 KB; as many groups per CTA as leave room for two stages;
+// then up to 4 stages.
 template <typename T, int DR, bool REAL> struct FullPick {
     using E = link_elem<T, REAL>;
     static constexpr bool SPLIT = sizeof(T) == 8 && DR >= 4;
+    static constexpr bool NBREG = !SPLIT && !REAL && DR <= 3;
     static constexpr int GW = SPLIT ? 4 : 2;
     static constexpr size_t ch_of(int r) { return (size_t)r * DR * TILE * sizeof(E); }
     static constexpr int pick_rpc() {
+        if (NBREG) return DR;
         int best = 1;
         for (int r = 1; r <= DR; ++r)
             if (DR % r == 0 && 4 * ch_of(r) <= 19 * 1024) best = r;
         return best;
     }
     static constexpr int RPC = pick_rpc();
-    static constexpr size_t FIXED = 2 * (size_t)4 * DR * TILE * sizeof(cplx<T>) + (size_t)GW * 2 * (SPLIT ? 2 : 4) * DR * TILE * sizeof(cplx<T>) +
+    static constexpr size_t FIXED = 2 * (size_t)4 * DR * TILE * sizeof(cplx<T>) + (NBREG ? 0 : (size_t)GW * 2 * (SPLIT ? 2 : 4) * DR * TILE * sizeof(cplx<T>)) +
                                     (SPLIT ? (size_t)4 * DR * TILE * sizeof(cplx<T>) : 0) + 16 * 8 + 128;
     static constexpr int stages_of(int groups) {
         const size_t per = ((226 * 1024) / groups) & ~(size_t)127;
@@ -424,7 +532,7 @@ template <typename T, int DR, bool REAL> struct FullPick {
         if (st > cpt) st = cpt;
         return st > 4 ? 4 : st;
     }
-    static constexpr int GMAX = sizeof(T) == 8 ? (SPLIT ? 2 : 4) : 6;
+    static constexpr int GMAX = sizeof(T) == 8 ? (SPLIT ? 2 : 4) : (NBREG ? 8 : 6);
     static constexpr int pick_groups() {
         for (int gr = GMAX; gr >= 1; --gr)
             if (stages_of(gr) >= 2) return gr;
@@ -443,9 +551,9 @@ inline bool hop_full_eligible(const HopLaunch &L) {
            L.b != 0.0 && L.tile_end == 0;
 }
 
-template <typename T, int DR, bool REAL, bool SPLIT, int GROUPS, int STAGES, int RPC> int launch_hop_full_cfg(const Geo &g, const HopLaunch &L, cudaStream_t s) {
-    using Cfg = FullCfg<T, DR, REAL, SPLIT, GROUPS, STAGES, RPC>;
-    auto kern = hop_full_kernel<T, DR, REAL, SPLIT, GROUPS, STAGES, RPC>;
+template <typename T, int DR, bool REAL, bool SPLIT, int GROUPS, int STAGES, int RPC, bool NBREG = false> int launch_hop_full_cfg(const Geo &g, const HopLaunch &L, cudaStream_t s) {
+    using Cfg = FullCfg<T, DR, REAL, SPLIT, GROUPS, STAGES, RPC, NBREG>;
+    auto kern = hop_full_kernel<T, DR, REAL, SPLIT, GROUPS, STAGES, RPC, NBREG>;
     static DevCache cache{};
     int n_sm = 0;
     if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
@@ -455,21 +563,40 @@ template <typename T, int DR, bool REAL, bool SPLIT, int GROUPS, int STAGES, int
 
 template <typename T, int DR, bool REAL> int launch_hop_full(const Geo &g, const HopLaunch &L, cudaStream_t s) {
 #ifdef HIREP_FULL_SWEEP   // development: shapes selected by HIREP_DBG bits 8..11 (d_R = 3 only)
-    if constexpr (DR == 3 && !REAL) {
-        switch ((L.dbg >> 8) & 15) {
-        case 1: return launch_hop_full_cfg<T, DR, REAL, true, 2, 3, 3>(g, L, s);
-        case 2: return launch_hop_full_cfg<T, DR, REAL, true, 2, 2, 3>(g, L, s);
-        case 3: return launch_hop_full_cfg<T, DR, REAL, false, 2, 4, 3>(g, L, s);
-        case 4: return launch_hop_full_cfg<T, DR, REAL, false, 3, 4, 1>(g, L, s);
-        case 5: return launch_hop_full_cfg<T, DR, REAL, true, 3, 4, 1>(g, L, s);
-        case 6: return launch_hop_full_cfg<T, DR, REAL, true, 3, 2, 1>(g, L, s);
-        case 7: return launch_hop_full_cfg<T, DR, REAL, false, 4, 3, 1>(g, L, s);
+    if constexpr (DR == 3) {
+        const int sel = (L.dbg >> 8) & 15;
+        if constexpr (sizeof(T) == 8 && !REAL) {
+            switch (sel) {
+            case 1: return launch_hop_full_cfg<T, DR, REAL, true, 2, 3, 3>(g, L, s);
+            case 3: return launch_hop_full_cfg<T, DR, REAL, false, 2, 4, 3>(g, L, s);
+            case 8: return launch_hop_full_cfg<T, DR, REAL, false, 3, 3, 3, true>(g, L, s);
+            case 9: return launch_hop_full_cfg<T, DR, REAL, false, 4, 2, 3, true>(g, L, s);
+            }
+        } else if constexpr (sizeof(T) == 8 && REAL) {
+            switch (sel) {
+            case 9: return launch_hop_full_cfg<T, DR, REAL, false, 4, 2, 3, true>(g, L, s);
+            case 11: return launch_hop_full_cfg<T, DR, REAL, false, 4, 4, 3, true>(g, L, s);
+            case 12: return launch_hop_full_cfg<T, DR, REAL, false, 5, 3, 3, true>(g, L, s);
+            case 13: return launch_hop_full_cfg<T, DR, REAL, false, 6, 2, 3, true>(g, L, s);
+            }
+        } else if constexpr (!REAL) {
+            switch (sel) {
+            case 9: return launch_hop_full_cfg<T, DR, REAL, false, 4, 2, 3, true>(g, L, s);
+            case 11: return launch_hop_full_cfg<T, DR, REAL, false, 6, 3, 3, true>(g, L, s);
+            case 12: return launch_hop_full_cfg<T, DR, REAL, false, 8, 2, 3, true>(g, L, s);
+            case 13: return launch_hop_full_cfg<T, DR, REAL, false, 4, 4, 3, true>(g, L, s);
+            }
+        } else {
+            switch (sel) {
+            case 11: return launch_hop_full_cfg<T, DR, REAL, false, 6, 4, 3, true>(g, L, s);
+            case 12: return launch_hop_full_cfg<T, DR, REAL, false, 8, 3, 3, true>(g, L, s);
+            }
         }
     }
 #endif
     using P = FullPick<T, DR, REAL>;
-    using Cfg = FullCfg<T, DR, REAL, P::SPLIT, P::GROUPS, P::STAGES, P::RPC>;
-    auto kern = hop_full_kernel<T, DR, REAL, P::SPLIT, P::GROUPS, P::STAGES, P::RPC>;
+    using Cfg = FullCfg<T, DR, REAL, P::SPLIT, P::GROUPS, P::STAGES, P::RPC, P::NBREG>;
+    auto kern = hop_full_kernel<T, DR, REAL, P::SPLIT, P::GROUPS, P::STAGES, P::RPC, P::NBREG>;
     static DevCache cache{};
     int n_sm = 0;
     if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
