@@ -40,7 +40,7 @@ struct hirep_geom {
     double *h_scal;                 // pinned: the CG's scalars read back without blocking the launches behind them (lazy)
     cudaEvent_t ev_scal;
     int *force_rowptr, *force_jk;   // sparse represented generators T_R^a for hirep_force_hopping (lazy)
-    void *force_val;
+    void *force_val, *force_dense;  // ... and the dense table [a][j][k] (double2)
     long launches;
     int device;                     // CUDA device current at hirep_geom_create (-1: none); compute calls check it
     size_t bytes_spinor_half, bytes_links_fund, bytes_links_rep;
@@ -152,7 +152,7 @@ extern "C" int hirep_geom_destroy(hirep_geom *g) {
     if (!g) return HIREP_OK;
     for (void *b : g->ms_p)
         if (b) cudaFree(b);
-    void *bufs[] = {g->force_rowptr, g->force_jk, g->force_val, g->ws_exp, g->ws_half, g->ws_half2, g->ws_half3, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
+    void *bufs[] = {g->force_rowptr, g->force_jk, g->force_val, g->force_dense, g->ws_exp, g->ws_half, g->ws_half2, g->ws_half3, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
                     g->h_in_native, g->h_out_native, g->h_out_canon, g->h_out_canon2};
     if (g->host_events) {
         for (int i = 0; i < 2; ++i) { cudaEventDestroy(g->ev_done[i]); cudaEventDestroy(g->ev_copied[i]); }
@@ -1064,8 +1064,7 @@ static int force_table(hirep_geom *g) {
     std::vector<double2> h(n);
     e = cudaMemcpyAsync(h.data(), dense, n * sizeof(double2), cudaMemcpyDeviceToHost, g->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
-    cudaFree(dense);
-    if (e != cudaSuccess) return cuda_fail(e, "hirep_force_hopping (generator table)");
+    if (e != cudaSuccess) { cudaFree(dense); return cuda_fail(e, "hirep_force_hopping (generator table)"); }
     g->launches += 1;
     std::vector<int> rowptr(NA + 1, 0), jk;
     std::vector<double2> val;
@@ -1086,10 +1085,10 @@ static int force_table(hirep_geom *g) {
     if (e == cudaSuccess) e = cudaMemcpy(p1, jk.data(), jk.size() * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(p2, val.data(), val.size() * sizeof(double2), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
-        cudaFree(p0); cudaFree(p1); cudaFree(p2); cudaGetLastError();
+        cudaFree(p0); cudaFree(p1); cudaFree(p2); cudaFree(dense); cudaGetLastError();
         return fail(HIREP_ENOMEM, "hirep_force_hopping: generator table upload: %s", cudaGetErrorString(e));
     }
-    g->force_rowptr = (int *)p0; g->force_jk = (int *)p1; g->force_val = p2;
+    g->force_rowptr = (int *)p0; g->force_jk = (int *)p1; g->force_val = p2; g->force_dense = dense;
     return HIREP_OK;
 }
 extern "C" int hirep_force_bytes(const hirep_geom *g, size_t *bytes, int *n_generators) {
@@ -1105,7 +1104,7 @@ extern "C" int hirep_force_hopping(hirep_geom *g, void *force_canonical, const v
     int rc = force_table(g);
     if (rc) return rc;
     return kern_result(g, k_force_hopping(g->geo, g->prec, g->dR, g->real, eta_full, xi_full, links_rep, g->force_rowptr, g->force_jk, g->force_val,
-                                          g->N * g->N - 1, force_canonical, g->stream), "hirep_force_hopping");
+                                          g->force_dense, g->N * g->N - 1, force_canonical, g->stream), "hirep_force_hopping");
 }
 
 extern "C" int hirep_fma_peak(int prec, double *tflops) {

@@ -174,6 +174,101 @@ __global__ void __launch_bounds__(256) force_hopping_kernel(const Geo g, int dR,
     }
 }
 
+// ---- small d_R: everything in registers, one thread per (site, mu), dense generator table read uniformly -----------------------
+// M_kj (d_R^2 complex) is accumulated in registers from the two outer products, then F^a = 2 sum_jk Im(T^a_jk M_kj) with T^a_jk
+// loaded at the same address by every lane (a broadcast).  Same arithmetic as the kernel above, without the shared-memory staging
+// that limits it to 8 warps per SM.
+template <typename T, int DR, bool REAL>
+__global__ void __launch_bounds__(128) force_site_kernel(const Geo g, const cplx<T> *eta, const cplx<T> *xi, const void *links_v,
+                                                         const double2 *dense, int NA, T *force, long n_units) {
+    using C = cplx<T>;
+    using E = link_elem<T, REAL>;
+    constexpr int NC = 4 * DR;
+    const int lane = threadIdx.x & 31;
+    const long unit = (long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);   // (parity, tile, mu)
+    if (unit >= n_units) return;
+    const int mu = (int)(unit & 3);
+    const long pt = unit >> 2;
+    const int tile = (int)(pt % g.n_tiles), p = (int)(pt / g.n_tiles);
+    int h = tile * TILE + lane;
+    const bool active = h < g.Nh;
+    if (!active) h = g.Nh - 1;
+    int t, x, y, zh;
+    decode_site(g, h, t, x, y, zh);
+    const int hn = mu == 0 ? neighbour<0>(g, p, t, x, y, zh) : mu == 1 ? neighbour<1>(g, p, t, x, y, zh)
+                 : mu == 2 ? neighbour<2>(g, p, t, x, y, zh) : neighbour<3>(g, p, t, x, y, zh);
+    const size_t half = (size_t)g.n_tiles * NC * TILE;
+    const bool imag = (mu & 1), swap = (mu == 1 || mu == 2);
+    const E *W = (const E *)links_v + ((((size_t)p * g.n_tiles + tile) * 8 + mu) * (size_t)DR * DR) * TILE + lane;
+    C M[DR][DR];
+#pragma unroll
+    for (int k = 0; k < DR; ++k)
+#pragma unroll
+        for (int j = 0; j < DR; ++j) M[k][j] = mk<T>(0, 0);
+    // M += (U h^A) (x) (k^B)^dagger for (A, B) = (eta, xi) and (xi, eta)
+#pragma unroll
+    for (int f = 0; f < 2; ++f) {
+        const C *fa = f ? xi : eta, *fb = f ? eta : xi;
+        const C *nb = fa + (size_t)(1 - p) * half + ((size_t)(hn >> 5) * NC) * TILE + (hn & 31);
+        const C *own = fb + (size_t)p * half + ((size_t)tile * NC) * TILE + lane;
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            const int qq = swap ? 1 - s : s;
+            const T sig = (mu < 2) ? T(-1) : (s ? T(1) : T(-1));
+            C hv[DR], kv[DR];
+#pragma unroll
+            for (int c = 0; c < DR; ++c) {
+                hv[c] = proj<T>(__ldg(nb + (size_t)(s * DR + c) * TILE), __ldg(nb + (size_t)((2 + qq) * DR + c) * TILE), -sig, imag);
+                kv[c] = proj<T>(__ldg(own + (size_t)(s * DR + c) * TILE), __ldg(own + (size_t)((2 + qq) * DR + c) * TILE), sig, imag);
+            }
+#pragma unroll
+            for (int k = 0; k < DR; ++k) {
+                C chi = mk<T>(0, 0);
+#pragma unroll
+                for (int j = 0; j < DR; ++j) mac<T>(chi, W[(size_t)(k * DR + j) * TILE], hv[j]);
+#pragma unroll
+                for (int j = 0; j < DR; ++j) {     // M_kj += chi_k conj(k_j)
+                    M[k][j].x += chi.x * kv[j].x + chi.y * kv[j].y;
+                    M[k][j].y += chi.y * kv[j].x - chi.x * kv[j].y;
+                }
+            }
+        }
+    }
+    if (!active) return;
+    const long ix = canonical_index(g, p, h);
+    T *out = force + ((size_t)ix * 4 + mu) * NA;
+    for (int a = 0; a < NA; ++a) {
+        const double2 *ta = dense + (size_t)a * DR * DR;
+        T acc = 0;
+#pragma unroll
+        for (int j = 0; j < DR; ++j)
+#pragma unroll
+            for (int k = 0; k < DR; ++k) {
+                const double2 tv = __ldg(ta + j * DR + k);          // T^a_jk, the same address in every lane
+                acc += (T)tv.x * M[k][j].y + (T)tv.y * M[k][j].x;   // Im(T^a_jk M_kj)
+            }
+        out[a] = 2 * acc;
+    }
+}
+
+template <typename T, bool REAL>
+int force_site_dispatch(const Geo &g, int dR, const void *eta, const void *xi, const void *links, const void *dense, int NA, void *force, cudaStream_t s) {
+    const long n_units = (long)2 * g.n_tiles * 4;
+    const unsigned grid = (unsigned)((n_units + 3) / 4);
+#define FS(D) force_site_kernel<T, D, REAL><<<grid, 128, 0, s>>>(g, (const cplx<T> *)eta, (const cplx<T> *)xi, links, (const double2 *)dense, NA, (T *)force, n_units)
+    switch (dR) {
+    case 1: FS(1); break;
+    case 2: FS(2); break;
+    case 3: FS(3); break;
+    case 4: FS(4); break;
+    case 5: if constexpr (sizeof(T) == 4) { FS(5); break; } else return KERR_UNSUPPORTED;
+    case 6: if constexpr (sizeof(T) == 4) { FS(6); break; } else return KERR_UNSUPPORTED;
+    default: return KERR_UNSUPPORTED;
+    }
+#undef FS
+    return (int)cudaGetLastError();
+}
+
 }  // namespace
 
 // dense generator table -> device (double2 [NA][dR][dR]); the caller converts it to the sparse form once
@@ -190,7 +285,14 @@ int k_rep_generators(int N, int rep, void *table_dev, cudaStream_t s) {
 }
 
 int k_force_hopping(const Geo &g, int prec, int dR, int real, const void *eta, const void *xi, const void *links, const int *rowptr,
-                    const int *jk, const void *val, int NA, void *force, cudaStream_t s) {
+                    const int *jk, const void *val, const void *dense, int NA, void *force, cudaStream_t s) {
+    if (dense) {   // d_R <= 4 (fp32: <= 6): the register kernel
+        const int rc = prec == 0 ? (real ? force_site_dispatch<double, true>(g, dR, eta, xi, links, dense, NA, force, s)
+                                         : force_site_dispatch<double, false>(g, dR, eta, xi, links, dense, NA, force, s))
+                                 : (real ? force_site_dispatch<float, true>(g, dR, eta, xi, links, dense, NA, force, s)
+                                         : force_site_dispatch<float, false>(g, dR, eta, xi, links, dense, NA, force, s));
+        if (rc != KERR_UNSUPPORTED) return rc;
+    }
     const size_t w = prec == 0 ? 16 : 8;
     const size_t warp_smem = (size_t)6 * 2 * dR * TILE * w;
     int wpc = (int)((200 * 1024) / warp_smem);

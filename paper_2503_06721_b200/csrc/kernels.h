@@ -68,9 +68,10 @@ int k_clover_exp(const Geo &g, int prec, int dR, int parity, double x, double pr
 int k_cblock(int prec, int dR, int ntile, const void *blk, const void *in, void *out, cudaStream_t s);
 // force.cu: fermion force of the hopping term (Eq 20-21).  k_rep_generators fills a dense double2 table [N^2-1][dR][dR] of the
 // represented generators; k_force_hopping takes them as a sparse list (entries of generator a: rowptr[a]..rowptr[a+1], jk = j*dR+k)
+// and, for the register kernel at small d_R, the dense table itself
 int k_rep_generators(int N, int rep, void *table_dev, cudaStream_t s);
 int k_force_hopping(const Geo &g, int prec, int dR, int real, const void *eta, const void *xi, const void *links, const int *rowptr,
-                    const int *jk, const void *val, int NA, void *force, cudaStream_t s);
+                    const int *jk, const void *val, const void *dense, int NA, void *force, cudaStream_t s);
 // number of distinct kernel launches k_hop issues for this configuration (for launch accounting): always 1.
 
 }  // namespace hirep
