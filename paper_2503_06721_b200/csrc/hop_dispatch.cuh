@@ -23,9 +23,11 @@ namespace hirep {
 template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
     // full-lattice launches whose diagonal term is the other parity's input: every link crosses the SM once (hop_full.cuh)
     // Default where it wins on B200 (profiles/r02_summary.md): complex links at d_R <= 3 in both precisions (C1, C2: 0.26 -> 0.20 ms at C2 fp64,
-    // 0.130 -> 0.119 ms in fp32, in bursts; on par under a sustained power-capped load) and the real SU(2) adjoint in fp64 (C3: 0.98 -> 0.89 ms).
-    // Elsewhere the gather-layout kernels are faster; variant 5 forces it anywhere.
-    if (hop_full_eligible(L) && (variant == 5 || (variant == 0 && DR <= 3 && (sizeof(T) == 8 || !REAL)))) return launch_hop_full<T, DR, REAL>(g, L, s);
+    // 0.130 -> 0.119 ms in fp32, in bursts; on par under a sustained power-capped load), the real SU(2) adjoint in fp64 (C3: 0.98 -> 0.89 ms) and
+    // complex links at d_R = 4, 6 in fp32 (C4: 4.91 -> 4.47 ms; SU(3) SYM 32^4 0.47 -> 0.34 ms; d_R = 5 has only one-row chunks and loses).  In fp64 at d_R >= 4 (half-spinor split over 4 warps: C4 10.7 vs 10.3 ms) and for real
+    // links in fp32 the gather-layout kernels are faster; variant 5 forces it anywhere.
+    if (hop_full_eligible(L) && (variant == 5 || (variant == 0 && ((DR <= 3 && (sizeof(T) == 8 || !REAL)) || (sizeof(T) == 4 && !REAL && DR != 5)))))
+        return launch_hop_full<T, DR, REAL>(g, L, s);
     if (variant == 5) variant = 0;
     if (variant == 0) {
         // one thread per site spills in fp64 from d_R = 5 on; in fp32 at d_R >= 5 only the passes with a diagonal

@@ -64,7 +64,7 @@ template <typename T, int DR, bool REAL, bool SPLIT, int GROUPS, int STAGES, int
     static constexpr int NBC = SPLIT ? 2 * DR : 4 * DR;                // neighbour components a warp stages per direction
     // NBREG: the out-of-pair neighbour spinors travel through registers (read-only loads issued half a direction pair ahead)
     // instead of a per-warp shared-memory buffer: 2 x 4 d_R x 512 B per warp go to the ring (one more stage or one more group)
-    static_assert(!NBREG || (!SPLIT && RPC == DR), "register neighbours: one thread per site, one chunk per direction pair");
+
     static constexpr uint32_t NBD = NBREG ? 0 : NBC * TILE * sizeof(C);   // one direction of a warp's neighbour buffer
     static constexpr uint32_t XB = SPLIT ? 2 * 2 * DR * TILE * sizeof(C) : 0;   // cross contributions [parity][s][d_R][32]
     static constexpr size_t SP_OFF = (size_t)STAGES * SLOT, NB_OFF = SP_OFF + 2 * SB, X_OFF = NB_OFF + (size_t)GW * 2 * NBD;
@@ -108,20 +108,25 @@ __device__ __forceinline__ void project_half(const cplx<T> *spo, const cplx<T> *
     }
 }
 
-// the same with the out-of-pair neighbour in registers (NBREG)
-template <typename T, int DR, typename DI>
-__device__ __forceinline__ void project_regs(const cplx<T> *spo, const cplx<T> (&nb)[4 * DR], bool in_tile, int ln, cplx<T> (&h)[2][DR]) {
+// the same with the out-of-pair neighbour in registers (NBREG).  nb holds the components this warp needs: all 4 d_R (one
+// thread per site) or [upper s | lower q(s)] (SPLIT)
+template <typename T, int DR, bool SPLIT, typename DI>
+__device__ __forceinline__ void project_regs(const cplx<T> *spo, const cplx<T> (&nb)[(SPLIT ? 2 : 4) * DR], bool in_tile, int ln, int s_rt,
+                                             cplx<T> (&h)[SPLIT ? 1 : 2][DR]) {
     using C = cplx<T>;
+    constexpr int NSC = SPLIT ? 1 : 2;
 #pragma unroll
-    for (int s = 0; s < 2; ++s) {
+    for (int kk = 0; kk < NSC; ++kk) {
+        const int s = SPLIT ? s_rt : kk;
         const int qq = DI::swap ? 1 - s : s;
         const T cs = (T)(DI::sg * DI::sigma(s));
 #pragma unroll
         for (int c = 0; c < DR; ++c) {
-            C u = nb[s * DR + c], v = nb[(2 + qq) * DR + c];
+            C u = SPLIT ? nb[c] : nb[kk * DR + c];
+            C v = SPLIT ? nb[DR + c] : nb[(2 + (DI::swap ? 1 - kk : kk)) * DR + c];
             if (in_tile) { u = spo[(size_t)(s * DR + c) * TILE + ln]; v = spo[(size_t)((2 + qq) * DR + c) * TILE + ln]; }
-            if (DI::imag) h[s][c] = mk<T>(fma(-cs, v.y, u.x), fma(cs, v.x, u.y));
-            else h[s][c] = mk<T>(fma(cs, v.x, u.x), fma(cs, v.y, u.y));
+            if (DI::imag) h[kk][c] = mk<T>(fma(-cs, v.y, u.x), fma(cs, v.x, u.y));
+            else h[kk][c] = mk<T>(fma(cs, v.x, u.x), fma(cs, v.y, u.y));
         }
     }
 }
@@ -271,13 +276,22 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
         cp_async_arrive_noinc(nbfull_s);
     };
 
-    C nb[NBREG ? 4 * DR : 1];
-    auto fetch = [&](int hn, int mu_) {   // NBREG: the out-of-pair neighbour's 4 d_R components (in-pair ones are read from the staged tiles)
+    C nb[NBREG ? Cfg::NBC : 1];
+    auto fetch = [&](int hn, int mu_, bool swap) {   // NBREG: the out-of-pair neighbour's components (in-pair ones are read from the staged tiles)
         if constexpr (NBREG) {
             if ((hn >> 5) != tile && !((L.dbg >> (4 + mu_)) & 1)) {
                 const C *src = in_nb + ((size_t)(hn >> 5) * NC) * TILE + (hn & 31);
+                if constexpr (SPLIT) {
+                    const int ql = swap ? 1 - s_rt : s_rt;
 #pragma unroll
-                for (int c = 0; c < NC; ++c) nb[c] = ld_spinor<T>(src + (size_t)c * TILE);
+                    for (int c = 0; c < DR; ++c) {
+                        nb[c] = ld_spinor<T>(src + (size_t)(s_rt * DR + c) * TILE);
+                        nb[DR + c] = ld_spinor<T>(src + (size_t)((2 + ql) * DR + c) * TILE);
+                    }
+                } else {
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) nb[c] = ld_spinor<T>(src + (size_t)c * TILE);
+                }
             }
         }
     };
@@ -290,7 +304,7 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
     }
     if (producer) issue_sp(gg);
     enter_tile(0);
-    if constexpr (NBREG) fetch(neighbour<0>(g, par, t, x, y, zh), 0);
+    if constexpr (NBREG) fetch(neighbour<0>(g, par, t, x, y, zh), 0, DirInfo<0>::swap);
     else stage_nb(IntC<0>{});
     int q = 0, slot = 0;
     uint32_t phase = 0, nbphase = 0;
@@ -327,72 +341,79 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
             const bool inf = (hnf >> 5) == c_tile, inb = (hnb >> 5) == c_tile;
             const int lnb = hnb & 31;
             if constexpr (NBREG) {
-                // one chunk per direction pair: forward hop while the -mu neighbour is in flight, backward hop while the next +mu one is
+                // forward hop of the first chunk while the -mu neighbour is in flight, backward hops while the next +mu one is
                 const C *spo = sp + (size_t)(1 - par) * NC * TILE;
-                C hh[2][DR];
-                project_regs<T, DR, DF>(spo, nb, inf, hnf & 31, hh);
-                fetch(hnb, MU);
+                C hp[NSC][DR], hm[NSC][DR];
+                project_regs<T, DR, SPLIT, DF>(spo, nb, inf, hnf & 31, s_rt, hp);
+                fetch(hnb, MU, DB::swap);
                 C chib[NSC][DR];
 #pragma unroll
                 for (int kk = 0; kk < NSC; ++kk)
 #pragma unroll
                     for (int c = 0; c < DR; ++c) chib[kk][c] = mk<T>(0, 0);
-                mbar_wait(full_s + 8 * slot, phase);
-                const unsigned char *sl_ = ring + (size_t)slot * SLOT;
-                const E *Wo = reinterpret_cast<const E *>(sl_ + par * CH) + lane;
-                const E *Wb = inb ? reinterpret_cast<const E *>(sl_ + (1 - par) * CH) + lnb : reinterpret_cast<const E *>(sl_ + (2 + par) * CH) + lane;
+                static_for<0, CPD>([&](auto rcc) {
+                    constexpr int RC = decltype(rcc)::value;
+                    mbar_wait(full_s + 8 * slot, phase);
+                    const unsigned char *sl_ = ring + (size_t)slot * SLOT;
+                    const E *Wo = reinterpret_cast<const E *>(sl_ + par * CH) + lane;
+                    const E *Wb = inb ? reinterpret_cast<const E *>(sl_ + (1 - par) * CH) + lnb : reinterpret_cast<const E *>(sl_ + (2 + par) * CH) + lane;
 #pragma unroll
-                for (int i = 0; i < DR; ++i) {
-                    E w[DR];
+                    for (int r = 0; r < RPC; ++r) {
+                        const int i = RC * RPC + r;
+                        E w[DR];
 #pragma unroll
-                    for (int j = 0; j < DR; ++j) w[j] = Wo[(i * DR + j) * TILE];
+                        for (int j = 0; j < DR; ++j) w[j] = Wo[(r * DR + j) * TILE];
 #pragma unroll
-                    for (int kk = 0; kk < 2; ++kk) {
-                        C chi = mk<T>(0, 0);
+                        for (int kk = 0; kk < NSC; ++kk) {
+                            C chi = mk<T>(0, 0);
 #pragma unroll
-                        for (int j = 0; j < DR; ++j) mac<T>(chi, w[j], hh[kk][j]);
-                        accumulate<T, DR, SPLIT, DF>(chi, kk, kk, i, up, lo, lx);
-                    }
-                }
-                project_regs<T, DR, DB>(spo, nb, inb, lnb, hh);
-                if constexpr (MU < 3) {
-                    fetch(neighbour<MU + 1>(g, par, t, x, y, zh), MU + 1);
-                } else {
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(spempty_s);          // last read of the staged tiles by this warp
-                    if (k + 1 < my_tiles) {
-                        if (producer) {
-                            mbar_wait(spempty_s, k & 1);
-                            fence_proxy_async();
-                            issue_sp(gg + (k + 1) * ng);
+                            for (int j = 0; j < DR; ++j) mac<T>(chi, w[j], hp[kk][j]);
+                            accumulate<T, DR, SPLIT, DF>(chi, kk, SPLIT ? s_rt : kk, i, up, lo, lx);
                         }
-                        enter_tile(k + 1);
-                        fetch(neighbour<0>(g, par, t, x, y, zh), 0);
                     }
-                }
+                    if constexpr (RC == 0) {
+                        project_regs<T, DR, SPLIT, DB>(spo, nb, inb, lnb, s_rt, hm);
+                        if constexpr (MU < 3) {
+                            fetch(neighbour<MU + 1>(g, par, t, x, y, zh), MU + 1, DirInfo<MU + 1>::swap);
+                        } else {
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(spempty_s);          // last read of the staged tiles by this warp
+                            if (k + 1 < my_tiles) {
+                                if (producer) {
+                                    mbar_wait(spempty_s, k & 1);
+                                    fence_proxy_async();
+                                    issue_sp(gg + (k + 1) * ng);
+                                }
+                                enter_tile(k + 1);
+                                fetch(neighbour<0>(g, par, t, x, y, zh), 0, DirInfo<0>::swap);
+                            }
+                        }
+                    }
 #pragma unroll
-                for (int i = 0; i < DR; ++i) {
-                    E w[DR];
+                    for (int r = 0; r < RPC; ++r) {
+                        const int i = RC * RPC + r;
+                        E w[DR];
 #pragma unroll
-                    for (int j = 0; j < DR; ++j) w[j] = Wb[(i * DR + j) * TILE];   // row i of U_mu(x-mu)
+                        for (int j = 0; j < DR; ++j) w[j] = Wb[(r * DR + j) * TILE];   // row i of U_mu(x-mu)
 #pragma unroll
-                    for (int kk = 0; kk < 2; ++kk)
+                        for (int kk = 0; kk < NSC; ++kk)
 #pragma unroll
-                        for (int j = 0; j < DR; ++j) macc<T>(chib[kk][j], w[j], hh[kk][i]);   // chi_j += conj(U_ij) h_i
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(empty_s + 8 * slot);
-                if (q + STAGES < my_chunks) {
-                    mbar_wait(empty_s + 8 * slot, phase);
-                    if (producer) fence_proxy_async();
-                    issue_chunk(slot);
-                }
-                ++q;
-                if (++slot == STAGES) { slot = 0; phase ^= 1; }
+                            for (int j = 0; j < DR; ++j) macc<T>(chib[kk][j], w[j], hm[kk][i]);   // chi_j += conj(U_ij) h_i
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(empty_s + 8 * slot);
+                    if (q + STAGES < my_chunks) {
+                        mbar_wait(empty_s + 8 * slot, phase);
+                        if (producer) fence_proxy_async();
+                        issue_chunk(slot);
+                    }
+                    ++q;
+                    if (++slot == STAGES) { slot = 0; phase ^= 1; }
+                });
 #pragma unroll
                 for (int kk = 0; kk < NSC; ++kk)
 #pragma unroll
-                    for (int c = 0; c < DR; ++c) accumulate<T, DR, SPLIT, DB>(chib[kk][c], kk, kk, c, up, lo, lx);
+                    for (int c = 0; c < DR; ++c) accumulate<T, DR, SPLIT, DB>(chib[kk][c], kk, SPLIT ? s_rt : kk, c, up, lo, lx);
             } else {
             // (a2) both half spinors of this direction pair
             mbar_wait(nbfull_s, nbphase);
@@ -503,22 +524,22 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
 
 // shape per instantiation (B200 sweeps, profiles/r02_summary.md): SPLIT in fp64 from d_R = 4 on (one thread per site would hold
 // 2 x 4 d_R accumulators, two half spinors and the column accumulators: > 255 registers).  NBREG (out-of-pair neighbours through
-// registers, whole matrices per slot) for complex links at d_R <= 3: the shared memory the neighbour buffers would take buys a fourth
-// group per SM (fp64: 8 warps; fp32: 8 groups = 16 warps) -- C2 fp64 0.224 -> 0.204 ms, fp32 0.144 -> 0.119 ms.  For the real SU(2)
-// adjoint on 48^4 (few in-pair neighbours, L/2 = 24 does not divide the tile) the buffered version measured faster and is kept.
-// Rows per chunk = the largest divisor of d_R whose slot (4 parts) stays <= 19 KB; as many groups per CTA as leave room for two stages;
-// then up to 4 stages.
+// registers) for complex links: the shared memory the neighbour buffers would take buys more groups per SM (d_R = 3: fp64 4 groups =
+// 8 warps, fp32 8 groups = 16 warps; C2 fp64 0.224 -> 0.204 ms, fp32 0.144 -> 0.119 ms; d_R = 6 fp32 4 groups: C4 Dphi 5.97 -> 4.47 ms,
+// gather-layout kernel 4.91).  For the real SU(2) adjoint on 48^4 (few in-pair neighbours, L/2 = 24 does not divide the tile) the
+// buffered version measured faster and is kept.  Rows per chunk = the largest divisor of d_R whose slot (4 parts) stays <= 19 KB
+// (SPLIT: 37 KB; NBREG at d_R <= 3: the whole matrix); as many groups per CTA as leave room for two stages; then up to 4 stages.
 template <typename T, int DR, bool REAL> struct FullPick {
     using E = link_elem<T, REAL>;
     static constexpr bool SPLIT = sizeof(T) == 8 && DR >= 4;
-    static constexpr bool NBREG = !SPLIT && !REAL && DR <= 3;
+    static constexpr bool NBREG = !REAL;
     static constexpr int GW = SPLIT ? 4 : 2;
     static constexpr size_t ch_of(int r) { return (size_t)r * DR * TILE * sizeof(E); }
     static constexpr int pick_rpc() {
-        if (NBREG) return DR;
+        if (NBREG && DR <= 3) return DR;
         int best = 1;
         for (int r = 1; r <= DR; ++r)
-            if (DR % r == 0 && 4 * ch_of(r) <= 19 * 1024) best = r;
+            if (DR % r == 0 && 4 * ch_of(r) <= (NBREG && SPLIT ? 37 : 19) * 1024) best = r;
         return best;
     }
     static constexpr int RPC = pick_rpc();
@@ -532,7 +553,7 @@ template <typename T, int DR, bool REAL> struct FullPick {
         if (st > cpt) st = cpt;
         return st > 4 ? 4 : st;
     }
-    static constexpr int GMAX = sizeof(T) == 8 ? (SPLIT ? 2 : 4) : (NBREG ? 8 : 6);
+    static constexpr int GMAX = sizeof(T) == 8 ? (SPLIT ? 2 : 4) : (NBREG ? (DR <= 3 ? 8 : 4) : 6);
     static constexpr int pick_groups() {
         for (int gr = GMAX; gr >= 1; --gr)
             if (stages_of(gr) >= 2) return gr;
@@ -562,7 +583,24 @@ template <typename T, int DR, bool REAL, bool SPLIT, int GROUPS, int STAGES, int
 }
 
 template <typename T, int DR, bool REAL> int launch_hop_full(const Geo &g, const HopLaunch &L, cudaStream_t s) {
-#ifdef HIREP_FULL_SWEEP   // development: shapes selected by HIREP_DBG bits 8..11 (d_R = 3 only)
+#ifdef HIREP_FULL_SWEEP   // development: shapes selected by HIREP_DBG bits 8..11
+    if constexpr (DR == 6 && !REAL) {
+        const int sel = (L.dbg >> 8) & 15;
+        if constexpr (sizeof(T) == 8) {
+            switch (sel) {
+            case 1: return launch_hop_full_cfg<T, DR, REAL, true, 2, 2, 3, true>(g, L, s);
+            case 2: return launch_hop_full_cfg<T, DR, REAL, true, 2, 3, 2, true>(g, L, s);
+            case 3: return launch_hop_full_cfg<T, DR, REAL, true, 2, 4, 1, true>(g, L, s);
+            }
+        } else {
+            switch (sel) {
+            case 1: return launch_hop_full_cfg<T, DR, REAL, false, 4, 2, 3, true>(g, L, s);
+            case 2: return launch_hop_full_cfg<T, DR, REAL, false, 4, 3, 2, true>(g, L, s);
+            case 3: return launch_hop_full_cfg<T, DR, REAL, false, 2, 2, 6, true>(g, L, s);
+            case 4: return launch_hop_full_cfg<T, DR, REAL, true, 4, 2, 3, true>(g, L, s);
+            }
+        }
+    }
     if constexpr (DR == 3) {
         const int sel = (L.dbg >> 8) & 15;
         if constexpr (sizeof(T) == 8 && !REAL) {
