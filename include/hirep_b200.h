@@ -320,7 +320,11 @@ int hirep_force_hopping(hirep_geom *g, void *force_canonical, const void *eta_fu
  * Synchronous; tflops is a host pointer. */
 int hirep_fma_peak(int prec, double *tflops);
 
-int hirep_sync(hirep_geom *g); /* synchronise the stream; returns any pending execution error */
+int hirep_sync(hirep_geom *g);
+/* hirep_sync also reports numerical breakdowns that kernels flagged since the last sync (HIREP_EBREAKDOWN, flags cleared):
+ * hirep_clover_inv_field eliminates without pivoting and flags a pivot below 1e-10 (fp32: 1e-4) of the block's largest entry or a
+ * non-finite one (blocks not positive definite: c_sw |A| is not small against 4 + m0); hirep_clover_exp_field flags sites with
+ * |c_sw/(4+m0) A_c|_inf > 8, outside the range its scaling-and-squaring series is accurate for.  The fields are then unusable. */ /* synchronise the stream; returns any pending execution error */
 const char *hirep_last_error(void);
 
 #ifdef __cplusplus

@@ -41,6 +41,7 @@ struct hirep_geom {
     cudaEvent_t ev_scal;
     int *force_rowptr, *force_jk;   // sparse represented generators T_R^a for hirep_force_hopping (lazy)
     void *force_val, *force_dense;  // ... and the dense table [a][j][k] (double2)
+    int *dev_flags;                 // device word set by kernels that met a numerical breakdown (clover block inverse / exponential); read by hirep_sync
     long launches;
     int device;                     // CUDA device current at hirep_geom_create (-1: none); compute calls check it
     size_t bytes_spinor_half, bytes_links_fund, bytes_links_rep;
@@ -152,7 +153,7 @@ extern "C" int hirep_geom_destroy(hirep_geom *g) {
     if (!g) return HIREP_OK;
     for (void *b : g->ms_p)
         if (b) cudaFree(b);
-    void *bufs[] = {g->force_rowptr, g->force_jk, g->force_val, g->force_dense, g->ws_exp, g->ws_half, g->ws_half2, g->ws_half3, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
+    void *bufs[] = {g->dev_flags, g->force_rowptr, g->force_jk, g->force_val, g->force_dense, g->ws_exp, g->ws_half, g->ws_half2, g->ws_half3, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
                     g->h_in_native, g->h_out_native, g->h_out_canon, g->h_out_canon2};
     if (g->host_events) {
         for (int i = 0; i < 2; ++i) { cudaEventDestroy(g->ev_done[i]); cudaEventDestroy(g->ev_copied[i]); }
@@ -537,7 +538,9 @@ extern "C" int hirep_clover_inv_field(hirep_geom *g, double m0, double csw, int 
     CHECK_PTRS("hirep_clover_inv_field", inv, clover);
     if (parity != HIREP_EVEN && parity != HIREP_ODD) return fail(HIREP_EINVAL, "hirep_clover_inv_field: parity=%d", parity);
     if (inv == clover) return fail(HIREP_EINVAL, "hirep_clover_inv_field: inv aliases clover");
-    return kern_result(g, k_clover_inv(g->geo, g->prec, g->dR, parity, 4.0 + m0, csw, clover, inv, g->stream), "hirep_clover_inv_field");
+    int rc = workspace((void **)&g->dev_flags, 64);
+    if (rc) return rc;
+    return kern_result(g, k_clover_inv(g->geo, g->prec, g->dR, parity, 4.0 + m0, csw, clover, inv, g->dev_flags, g->stream), "hirep_clover_inv_field");
 }
 extern "C" int hirep_Cphi_inv(hirep_geom *g, void *out_half, const void *in_half, const void *inv) {
     CHECK_PTRS("hirep_Cphi_inv", out_half, in_half, inv);
@@ -575,8 +578,9 @@ extern "C" int hirep_clover_exp_field(hirep_geom *g, double m0, double csw, int 
     if (blocks == clover) return fail(HIREP_EINVAL, "hirep_clover_exp_field: blocks aliases clover");
     int rc = workspace(&g->ws_exp, 2 * clover_bytes(g));
     if (rc) return rc;
+    if ((rc = workspace((void **)&g->dev_flags, 64))) return rc;
     const double x = (inverse ? -1.0 : 1.0) * csw / (4.0 + m0), pref = inverse ? 1.0 / (4.0 + m0) : 4.0 + m0;
-    return kern_result(g, k_clover_exp(g->geo, g->prec, g->dR, parity, x, pref, clover, blocks, g->ws_exp, g->stream), "hirep_clover_exp_field");
+    return kern_result(g, k_clover_exp(g->geo, g->prec, g->dR, parity, x, pref, clover, blocks, g->ws_exp, g->dev_flags, g->stream), "hirep_clover_exp_field");
 }
 // out = [gamma_5] (blocks in - 1/2 hop(in)); gamma_5 commutes with the chirality blocks
 static int dphi_blocks(hirep_geom *g, void *out_full, const void *in_full, const void *links, const void *blocks_full, int g5, const char *what) {
@@ -1122,6 +1126,16 @@ extern "C" int hirep_sync(hirep_geom *g) {
     if (e != cudaSuccess) return cuda_fail(e, "hirep_sync");
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "hirep_sync (deferred)");
+    if (g->dev_flags) {   // numerical breakdowns reported by kernels since the last sync
+        int fl = 0;
+        e = cudaMemcpy(&fl, g->dev_flags, sizeof(int), cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return cuda_fail(e, "hirep_sync (flags)");
+        if (fl) {
+            cudaMemset(g->dev_flags, 0, sizeof(int));
+            return fail(HIREP_EBREAKDOWN, "hirep_sync: %s%s%s", (fl & 1) ? "hirep_clover_inv_field met a vanishing or non-finite pivot (block not positive definite: c_sw |A| against 4+m0)" : "",
+                        (fl & 3) == 3 ? "; " : "", (fl & 2) ? "hirep_clover_exp_field: |c_sw/(4+m0) A| > 8 at some site, outside the range of the exponential series" : "");
+        }
+    }
     return HIREP_OK;
 }
 

@@ -430,7 +430,7 @@ int k_cphi(int prec, int dR, int ntile, double a, double csw, const void *clover
 // across lanes) and inverted there in place by Gauss-Jordan elimination without pivoting -- the blocks are Hermitian and,
 // for the parameters the operator is used with ((4+m) dominates c_sw |A|), positive definite.  Once per gauge update.
 template <typename T>
-__global__ void clover_inv_kernel(Geo g, int dR, int parity, T a, T csw, const cplx<T> *__restrict__ clover, cplx<T> *inv) {
+__global__ void clover_inv_kernel(Geo g, int dR, int parity, T a, T csw, const cplx<T> *__restrict__ clover, cplx<T> *inv, int *flags) {
     const int n = 2 * dR, ne = dR * dR;
     const int slot = blockIdx.x * blockDim.x + threadIdx.x;      // padded site slot of the parity
     const int c = blockIdx.y;
@@ -438,6 +438,7 @@ __global__ void clover_inv_kernel(Geo g, int dR, int parity, T a, T csw, const c
     const int tile = slot >> 5, lane = slot & 31;
     cplx<T> *M = inv + ((size_t)(tile * 2 + c) * n * n) * TILE + lane;
     const bool live = slot < g.Nh;
+    T scale = 0;                                                  // largest |entry| of the block: the yardstick for the pivots
     for (int I = 0; I < n; ++I)
         for (int J = 0; J < n; ++J) {
             const int bi = I / dR, i = I - bi * dR, bj = J / dR, j = J - bj * dR;
@@ -455,10 +456,17 @@ __global__ void clover_inv_kernel(Geo g, int dR, int parity, T a, T csw, const c
             if (I == J) v.x += a;
             if (!live) v = mk<T>(I == J ? T(1) : T(0), T(0));    // padding lanes: identity, inverted harmlessly, zeroed below
             M[(size_t)(I * n + J) * TILE] = v;
+            scale = fmax(scale, fmax(fabs(v.x), fabs(v.y)));
         }
+    // elimination without pivoting is only safe for well-conditioned (positive definite) blocks: a pivot that is tiny against the
+    // block, or not finite, is reported through the geometry's device flags (hirep_sync returns HIREP_EBREAKDOWN)
+    const T tiny = scale * (sizeof(T) == 8 ? T(1e-10) : T(1e-4));
+    bool bad = false;
     for (int k = 0; k < n; ++k) {
         const cplx<T> d = M[(size_t)(k * n + k) * TILE];
-        const T r = T(1) / (d.x * d.x + d.y * d.y);
+        const T d2 = d.x * d.x + d.y * d.y;
+        if (!(d2 > tiny * tiny) || !isfinite(d2)) bad = true;
+        const T r = T(1) / d2;
         const cplx<T> p = mk<T>(d.x * r, -d.y * r);
         M[(size_t)(k * n + k) * TILE] = mk<T>(1, 0);
         for (int J = 0; J < n; ++J) M[(size_t)(k * n + J) * TILE] = cmul<T>(M[(size_t)(k * n + J) * TILE], p);
@@ -477,6 +485,7 @@ __global__ void clover_inv_kernel(Geo g, int dR, int parity, T a, T csw, const c
     }
     if (!live)
         for (int E = 0; E < n * n; ++E) M[(size_t)E * TILE] = mk<T>(0, 0);
+    if (bad && live && flags) atomicOr(flags, 1);
 }
 
 // out = block * in per chirality with the full (2 dR)^2 blocks of one parity (n_tiles tiles).
@@ -553,7 +562,7 @@ int k_cblock(int prec, int dR, int ntile, const void *blk, const void *in, void 
 // scaling and squaring, exp(Y) = (sum_{k <= K} (Y/2^s)^k / k!)^(2^s) with the sum in Horner form; s = 4, K = 14 covers
 // |x A| <= 8 to 1e-16 (truncation 0.5^15/15!) and the four squarings amplify rounding by 16 ulp.
 template <typename T>
-__global__ void clover_exp_kernel(Geo g, int dR, int parity, T x, T pref, const cplx<T> *__restrict__ clover, cplx<T> *blocks, cplx<T> *work) {
+__global__ void clover_exp_kernel(Geo g, int dR, int parity, T x, T pref, const cplx<T> *__restrict__ clover, cplx<T> *blocks, cplx<T> *work, int *flags) {
     constexpr int SQ = 4, K = 14;
     const int n = 2 * dR, ne = dR * dR;
     const int slot = blockIdx.x * blockDim.x + threadIdx.x;
@@ -564,7 +573,9 @@ __global__ void clover_exp_kernel(Geo g, int dR, int parity, T x, T pref, const 
     cplx<T> *S = blocks + off, *X = work + off, *Tm = work + (size_t)g.n_tiles * 2 * n * n * TILE + off;
     const bool live = slot < g.Nh;
     const T sc = x / T(1 << SQ);
-    for (int I = 0; I < n; ++I)
+    T norm = 0;                                                   // inf-norm of x A_c: the series below is accurate for <= 8
+    for (int I = 0; I < n; ++I) {
+        T rowsum = 0;
         for (int J = 0; J < n; ++J) {
             const int bi = I / dR, i = I - bi * dR, bj = J / dR, j = J - bj * dR;
             cplx<T> v;
@@ -579,7 +590,11 @@ __global__ void clover_exp_kernel(Geo g, int dR, int parity, T x, T pref, const 
             }
             X[(size_t)(I * n + J) * TILE] = mk<T>(sc * v.x, sc * v.y);
             S[(size_t)(I * n + J) * TILE] = mk<T>(I == J ? T(1) : T(0), T(0));
+            rowsum += sqrt(v.x * v.x + v.y * v.y);
         }
+        norm = fmax(norm, fabs(x) * rowsum);
+    }
+    if (live && flags && (!(norm <= T(8)) )) atomicOr(flags, 2);   // also catches NaN
     for (int k = K; k >= 1; --k) {            // S <- 1 + (X S)/k
         const T rk = T(1) / T(k);
         for (int I = 0; I < n; ++I)
@@ -604,21 +619,21 @@ __global__ void clover_exp_kernel(Geo g, int dR, int parity, T x, T pref, const 
         S[(size_t)E * TILE] = live ? mk<T>(pref * v.x, pref * v.y) : mk<T>(0, 0);
     }
 }
-template <typename T> static int clover_exp_t(const Geo &g, int dR, int parity, double x, double pref, const void *clover, void *blocks, void *work, cudaStream_t s) {
+template <typename T> static int clover_exp_t(const Geo &g, int dR, int parity, double x, double pref, const void *clover, void *blocks, void *work, int *flags, cudaStream_t s) {
     clover_exp_kernel<T><<<dim3((g.n_tiles * TILE + 63) / 64, 2), 64, 0, s>>>(g, dR, parity, (T)x, (T)pref, (const cplx<T> *)clover, (cplx<T> *)blocks,
-                                                                           (cplx<T> *)work);
+                                                                           (cplx<T> *)work, flags);
     return (int)cudaGetLastError();
 }
-int k_clover_exp(const Geo &g, int prec, int dR, int parity, double x, double pref, const void *clover, void *blocks, void *work, cudaStream_t s) {
-    return prec == 0 ? clover_exp_t<double>(g, dR, parity, x, pref, clover, blocks, work, s) : clover_exp_t<float>(g, dR, parity, x, pref, clover, blocks, work, s);
+int k_clover_exp(const Geo &g, int prec, int dR, int parity, double x, double pref, const void *clover, void *blocks, void *work, int *flags, cudaStream_t s) {
+    return prec == 0 ? clover_exp_t<double>(g, dR, parity, x, pref, clover, blocks, work, flags, s) : clover_exp_t<float>(g, dR, parity, x, pref, clover, blocks, work, flags, s);
 }
 
-template <typename T> static int clover_inv_t(const Geo &g, int dR, int parity, double a, double csw, const void *clover, void *inv, cudaStream_t s) {
-    clover_inv_kernel<T><<<dim3((g.n_tiles * TILE + 63) / 64, 2), 64, 0, s>>>(g, dR, parity, (T)a, (T)csw, (const cplx<T> *)clover, (cplx<T> *)inv);
+template <typename T> static int clover_inv_t(const Geo &g, int dR, int parity, double a, double csw, const void *clover, void *inv, int *flags, cudaStream_t s) {
+    clover_inv_kernel<T><<<dim3((g.n_tiles * TILE + 63) / 64, 2), 64, 0, s>>>(g, dR, parity, (T)a, (T)csw, (const cplx<T> *)clover, (cplx<T> *)inv, flags);
     return (int)cudaGetLastError();
 }
-int k_clover_inv(const Geo &g, int prec, int dR, int parity, double a, double csw, const void *clover, void *inv, cudaStream_t s) {
-    return prec == 0 ? clover_inv_t<double>(g, dR, parity, a, csw, clover, inv, s) : clover_inv_t<float>(g, dR, parity, a, csw, clover, inv, s);
+int k_clover_inv(const Geo &g, int prec, int dR, int parity, double a, double csw, const void *clover, void *inv, int *flags, cudaStream_t s) {
+    return prec == 0 ? clover_inv_t<double>(g, dR, parity, a, csw, clover, inv, flags, s) : clover_inv_t<float>(g, dR, parity, a, csw, clover, inv, flags, s);
 }
 
 template <typename T> static int clover_export_t(const Geo &g, int dR, void *canon, const void *clover, cudaStream_t s) {

@@ -62,9 +62,9 @@ int k_clover_field(const Geo &g, int prec, int dR, int real, void *clover, const
 int k_clover_export(const Geo &g, int prec, int dR, void *canon, const void *clover, cudaStream_t s);
 int k_cphi(int prec, int dR, int ntile, double a, double csw, const void *clover, const void *in, void *out, cudaStream_t s);
 // inverse diagonal blocks of one parity ((2 dR)^2 complex per site and chirality) and their application
-int k_clover_inv(const Geo &g, int prec, int dR, int parity, double a, double csw, const void *clover, void *inv, cudaStream_t s);
+int k_clover_inv(const Geo &g, int prec, int dR, int parity, double a, double csw, const void *clover, void *inv, int *flags, cudaStream_t s);
 // blocks of one parity <- pref * exp(x A_c) (Eq 50); work = 2 x the bytes of `blocks`
-int k_clover_exp(const Geo &g, int prec, int dR, int parity, double x, double pref, const void *clover, void *blocks, void *work, cudaStream_t s);
+int k_clover_exp(const Geo &g, int prec, int dR, int parity, double x, double pref, const void *clover, void *blocks, void *work, int *flags, cudaStream_t s);
 int k_cblock(int prec, int dR, int ntile, const void *blk, const void *in, void *out, cudaStream_t s);
 // force.cu: fermion force of the hopping term (Eq 20-21).  k_rep_generators fills a dense double2 table [N^2-1][dR][dR] of the
 // represented generators; k_force_hopping takes them as a sparse list (entries of generator a: rowptr[a]..rowptr[a+1], jk = j*dR+k)

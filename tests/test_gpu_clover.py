@@ -315,3 +315,28 @@ def test_exponential_clover_cg_full_lattice(env):
     assert res <= 1e-10 and abs(it - it_ref) <= 2
     assert oracle.rel_l2(x, x_ref) < 1e-7
     assert np.linalg.norm((b - A(x)).ravel()) < 1e-9 * np.linalg.norm(b.ravel())
+
+
+def test_clover_block_breakdowns_are_flagged(env):
+    """the unpivoted block inverse and the fixed-order exponential must not hand back garbage silently: indefinite
+    blocks (large c_sw, small 4 + m0) and |c_sw/(4+m0) A| > 8 are reported by hirep_sync as HIREP_EBREAKDOWN, and the geometry
+    stays usable."""
+    hirep = env["hirep"]
+    p = Problem(env, synth.CONFIGS["C2"].resized(4, 4), "f64")
+    cl = p.geom.clover_field(p.links_rep)
+    p.geom.sync()
+    p.geom.clover_inv_field(-0.2, 0.5, hirep.ODD, cl)            # well conditioned: no flag
+    p.geom.sync()
+    # blocks (4+m0) + c_sw A_c with 4+m0 = 0: the first pivot of the traceless A_c blocks can vanish or the blocks are indefinite ->
+    # make it certain with an exactly singular block: c_sw = 0 and 4 + m0 = 0
+    p.geom.clover_inv_field(-4.0, 0.0, hirep.ODD, cl)
+    with pytest.raises(hirep.HirepError) as ei:
+        p.geom.sync()
+    assert ei.value.rc == hirep.EBREAKDOWN and "pivot" in str(ei.value)
+    p.geom.sync()                                                # flags cleared
+    p.geom.clover_exp_field(-3.99, 100.0, cl)                    # c_sw/(4+m0) = 1e4: far outside the series' range
+    with pytest.raises(hirep.HirepError) as ei:
+        p.geom.sync()
+    assert ei.value.rc == hirep.EBREAKDOWN and "exponential" in str(ei.value)
+    p.geom.clover_exp_field(-0.2, 1.0, cl)                       # fine again
+    p.geom.sync()
