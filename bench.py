@@ -438,7 +438,9 @@ def run_ours(args):
             roofline_c4 = {"bound": "hbm", "kernel": "C4 fp64 Dphi_hat (two hop stencil passes, d_R = 6)", "achieved": c4["gbs"], "peak": peak,
                            "unit": "GB/s", "frac": c4["frac_hbm"], "traffic": ncu_traffic("C4", "f64", "Dphi_hat"), "peak_source": peak_src,
                            "algorithmic_bytes": cost_model(synth.CONFIGS["C4"], "f64")["ops"]["Dphi_hat"][1],
-                           "frac_of_8TBs_nominal": c4["frac_8TBs_nominal"], "timing": "back-to-back launches, median of 5 repeats"}
+                           "frac_of_8TBs_nominal": c4["frac_8TBs_nominal"],
+                           "timing": "back-to-back launches, median of 5 repeats (sustained: the SM clock under the power cap is in per_config.C4_f64.clocks)",
+                           "in_step": {"ms": c4["ms_in_step"], "frac": round(c4["frac_hbm"] * c4["ms"] / c4["ms_in_step"], 4)}}
         b2b = (per_config or {}).get("%s_%s%s" % (args.config, prec, "_rebuild" if rebuild else ""), {}).get("ops", {}).get("Dphi_eo")
         if b2b:
             roofline["back_to_back"] = {"ms": b2b["ms"], "achieved": b2b["gbs"], "frac": b2b["frac_hbm"]}
