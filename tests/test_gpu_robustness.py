@@ -65,6 +65,46 @@ def test_determinism_and_guard_bands(env, name, T, L, prec, max_ctas):
         assert np.array_equal(results[0], results[1]) and np.array_equal(results[0], results[2]), (nm, "not deterministic")
 
 
+NEW_KERNELS = [  # (N, rep, T, L, prec, variant, rebuild): hop_full in all its shapes (variant 5) and the matrix-free adjoint (REBUILD)
+    (3, 0, 8, 8, "f64", 5, False), (3, 0, 8, 8, "f32", 5, False), (2, 1, 4, 12, "f64", 5, False), (2, 1, 4, 12, "f32", 5, False),
+    (4, 3, 4, 12, "f64", 5, False), (4, 3, 4, 12, "f32", 5, False), (5, 0, 4, 6, "f64", 5, False), (4, 0, 6, 6, "f32", 5, False),
+    (3, 1, 4, 8, "f64", 0, True), (6, 1, 4, 6, "f64", 0, True), (6, 1, 4, 6, "f32", 0, True), (4, 1, 6, 6, "f32", 0, True)]
+
+
+@pytest.mark.parametrize("n,rep,T,L,prec,variant,rebuild", NEW_KERNELS)
+@pytest.mark.parametrize("max_ctas", [0, 3])
+def test_determinism_of_the_round2_kernels(env, n, rep, T, L, prec, variant, rebuild, max_ctas):
+    """compute-sanitizer is closed on the GPU pool, so races in the tile-pair staging (mbarrier slots shared by bulk copies and
+    per-lane cp.async gathers, register neighbours, staged input tiles refilled during the last direction) and in the per-warp
+    areas of the matrix-free adjoint are hunted the other way: six repetitions must agree bit for bit, with guard bands around the
+    output and L^3/2 not a multiple of the tile (ragged rows, in-pair and out-of-pair neighbours mixed within a warp)."""
+    torch, hirep = env["torch"], env["hirep"]
+    cfg = synth.Config("t", T, L, n, rep, -0.3, "haar", 321, ())
+    p = Problem(env, cfg, prec)
+    g = p.geom
+    g.set_kernel_variant(variant)
+    g.set_tuning(hirep.TUNE_MAX_CTAS, max_ctas)
+    links = p.links_rep
+    if rebuild:
+        g.set_link_mode(hirep.LINKS_REBUILD)
+        links = p.links_fund
+    x = p.to_native(p.spinors[0], hirep.FULL)
+    fb = g.sizes["spinor_full"]
+    for nm, run in [("Dphi", lambda out: g.Dphi(cfg.m0, x, links, out=out)), ("g5Dphi_sq", lambda out: g.g5Dphi_sq(cfg.m0, x, links, out=out)),
+                    ("Dphi_tm", lambda out: g.Dphi_tm(cfg.m0, 0.25, x, links, out=out))]:
+        first = None
+        for rep_ in range(6):
+            big, out = guarded(torch, env["dev"], fb)
+            run(out)
+            g.sync()
+            host = big.cpu().numpy()
+            assert (host[:GUARD] == 0xA5).all() and (host[GUARD + fb:] == 0xA5).all(), (nm, "guard band overwritten")
+            body = host[GUARD:GUARD + fb].copy()
+            if first is None:
+                first = body
+            assert np.array_equal(first, body), (nm, rep_, "not deterministic")
+
+
 def test_reductions_and_cg_are_deterministic(env):
     hirep = env["hirep"]
     p = Problem(env, synth.CONFIGS["C2"].resized(6, 6), "f64")
