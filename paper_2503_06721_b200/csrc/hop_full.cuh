@@ -22,7 +22,8 @@
 //   * what is not in the tile pair -- the +-t, +-x (and half of the +-y) neighbours: spinors, and the links of the
 //     backward hops -- is GATHERED per lane with cp.async (16/8/4-byte asynchronous copies, no registers) into
 //     shared memory: link rows into the gather part of the ring slot they are consumed with (same mbarrier as the
-//     bulk part), neighbour spinors into a per-warp buffer one direction ahead.
+//     bulk part), neighbour spinors into a per-warp buffer one direction ahead -- or (NBREG, complex links) through
+//     registers by read-only loads issued half a direction pair ahead, which leaves the shared memory to more groups.
 // Requests to L2 per site drop from 10S+8K to about 7S+6.5K (L = 32), DRAM traffic from 2S+8K towards 2S+4K (the
 // backward t links of a tile pair were streamed by another group of the same or the previous grid round).
 // Optionally (SPLIT) the two half-spinor components are split over two warps as in hop_pair.cuh (fp64, d_R >= 4).
