@@ -148,8 +148,12 @@ int hirep_set_kernel_variant(hirep_geom *g, int variant);
  *                          walk many tiles, which the parity tests use on small lattices
  *   HIREP_TUNE_SUM_ALGORITHM  accumulation of the reductions (this one does change the last bits of their results):
  *                          2 = Neumaier, Algorithm 2 (default), 3 = second-order Neumaier, Algorithm 3 (L682),
- *                          4 = double-double, Algorithm 4 (L706) */
-enum { HIREP_TUNE_MAX_CTAS = 1, HIREP_TUNE_SUM_ALGORITHM = 2 };
+ *                          4 = double-double, Algorithm 4 (L706)
+ *   HIREP_TUNE_PACE_WINDOW W > 0: full-lattice launches of the tile-pair kernel throttle their leading warp groups -- a group starts
+ *                          its round k only when the grid has completed k - W rounds' worth of tile pairs -- so that link blocks and
+ *                          spinor tiles gathered from other tile pairs are still in L2 (C4: DRAM reads -16..-26 %; time +-5 %, so
+ *                          off by default: 0).  Needs all CTAs of the launch co-resident (the library's grids are <= one CTA per SM). */
+enum { HIREP_TUNE_MAX_CTAS = 1, HIREP_TUNE_SUM_ALGORITHM = 2, HIREP_TUNE_PACE_WINDOW = 3 };
 int hirep_set_tuning(hirep_geom *g, int key, int value);
 /* number of kernels this library has launched on behalf of g since creation (bench.py's gpu_launches) */
 long hirep_launch_count(const hirep_geom *g);

@@ -22,7 +22,7 @@ struct hirep_geom {
     Geo geo;
     int N, rep, prec, dR, real;
     int mode, variant;
-    int tune_max_ctas, sum_alg;   // hirep_set_tuning
+    int tune_max_ctas, sum_alg, tune_pace;   // hirep_set_tuning
     int slab, region;             // hirep_geom_create_slab / hirep_set_region
     cudaStream_t stream;
     void *ws_half, *ws_half2, *ws_half3, *ws_full;   // workspace spinors (lazy)
@@ -216,6 +216,10 @@ extern "C" int hirep_set_tuning(hirep_geom *g, int key, int value) {
         if (value < 0) return fail(HIREP_EINVAL, "hirep_set_tuning: max CTAs %d", value);
         g->tune_max_ctas = value;
         return HIREP_OK;
+    case HIREP_TUNE_PACE_WINDOW:
+        if (value < 0 || value > 64) return fail(HIREP_EINVAL, "hirep_set_tuning: pace window %d (0 = off, 1..64 rounds)", value);
+        g->tune_pace = value;
+        return HIREP_OK;
     }
     return fail(HIREP_EINVAL, "hirep_set_tuning: unknown key %d", key);
 }
@@ -268,6 +272,7 @@ extern "C" int hirep_links_to_rep(hirep_geom *g, void *native_rep, const void *n
 }
 
 // ---- operators ------------------------------------------------------------------------------------
+static int workspace(void **slot, size_t bytes);
 static int hop_range(hirep_geom *g, HopLaunch L, int tb, int te, const char *what) {
     L.tile_begin = tb; L.tile_end = te;
     const int rc = g->prec == HIREP_F64 ? k_hop_f64(g->geo, g->N, g->rep, g->mode, g->variant, L, g->stream)
@@ -282,6 +287,14 @@ static int hop(hirep_geom *g, HopLaunch L, const char *what) {
     L.max_ctas = g->tune_max_ctas;
     static const int dbg = getenv("HIREP_DBG") ? atoi(getenv("HIREP_DBG")) : 0;
     L.dbg = dbg;
+    if (g->tune_pace > 0 && L.nsets == 2) {   // hirep_set_tuning(HIREP_TUNE_PACE_WINDOW): round pacing of the tile-pair kernel
+        int rc0 = workspace((void **)&g->dev_flags, 64);
+        if (rc0) return rc0;
+        L.pace = (unsigned *)g->dev_flags + 4;
+        L.pace_every = g->tune_pace;
+        const cudaError_t pe = cudaMemsetAsync(L.pace, 0, sizeof(unsigned), g->stream);
+        if (pe != cudaSuccess) return cuda_fail(pe, what);
+    }
     if (!g->slab || g->region == HIREP_REGION_ALL) return hop_range(g, L, 0, 0, what);
     const long S = (long)g->geo.L * g->geo.L * g->geo.Lh;
     const int T = g->geo.T;

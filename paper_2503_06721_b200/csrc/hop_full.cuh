@@ -313,6 +313,17 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
     const T g5s = L.g5 ? T(-1) : T(1);
 
     for (int k = 0; k < my_tiles; ++k) {
+        // Round pacing: without it the groups of the grid drift apart (no global synchronisation in a persistent kernel), and a
+        // link block or spinor tile gathered from another tile pair has left L2 when the two groups are more than ~20 us apart
+        // (6 TB/s turn the 126 MB over that fast).  Leaders are throttled, laggards never wait: a group may start its round k only
+        // when the grid as a whole has completed (k - W) rounds' worth of tile pairs (one counter, one poll per group and round).
+        if (L.pace_every > 0 && k >= L.pace_every) {
+            if (wg == 0 && lane == 0) {
+                const unsigned target = (unsigned)(k - L.pace_every) * (unsigned)ng;
+                while (*((volatile unsigned *)L.pace) < target) __nanosleep(200);
+            }
+            group_sync(1 + grp, GW * 32);
+        }
         const int c_tile = tile;
         const bool c_active = active;
         // the diagonal term goes into the accumulators first: out = b * ((a/b) self + i (am/b) gamma_5 self + hop), so that the
@@ -520,6 +531,7 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
                 }
             }
         }
+        if (L.pace_every > 0 && wg == 0 && lane == 0) atomicAdd(L.pace, 1u);
     }
 }
 

@@ -24,6 +24,8 @@ struct HopLaunch {
     int g5;             // multiply the result by gamma_5 = diag(1,1,-1,-1)
     int max_ctas;       // cap on the persistent grid (0 = one CTA per SM); tests use it to force many tiles per warp
     int tile_begin, tile_end;   // tiles [begin, end) of each parity to compute (slab regions: interior / boundary); end = 0: all
+    unsigned *pace;     // hop_full.cuh: device counter of the round pacing (NULL / pace_every = 0: off)
+    int pace_every;     // grid-wide rendezvous every pace_every tile rounds
     int dbg;            // HIREP_DBG (development only, results become wrong): bit mu skips the backward-link gather of direction mu,
                         // bit 4+mu the neighbour-spinor gathers of +-mu in hop_full.cuh -- traffic attribution under ncu
 };

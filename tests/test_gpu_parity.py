@@ -434,3 +434,22 @@ def test_full_size_whole_field(env, name, prec):
         assert v < tol, (name, prec, k, v)
     del lr, links, psi, R
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("name,prec,variant", [("C2", "f64", 0), ("C4", "f32", 0), ("C4", "f64", 5), ("C3", "f64", 0)])
+def test_round_pacing_is_result_neutral(env, name, prec, variant):
+    """HIREP_TUNE_PACE_WINDOW throttles leading warp groups of the tile-pair kernel; results are bit-identical with and without it
+    (many rounds: 8x8^3 lattice on a capped grid, window 1 and 3)."""
+    hirep = env["hirep"]
+    p = Problem(env, synth.CONFIGS[name].resized(8, 8), prec)
+    g = p.geom
+    g.set_kernel_variant(variant)
+    x = p.to_native(p.spinors[0], hirep.FULL)
+    ref = g.Dphi(p.cfg.m0, x, p.links_rep).clone()
+    for cap in (0, 5):
+        g.set_tuning(hirep.TUNE_MAX_CTAS, cap)
+        for w in (1, 3):
+            g.set_tuning(hirep.TUNE_PACE_WINDOW, w)
+            assert env["torch"].equal(g.Dphi(p.cfg.m0, x, p.links_rep), ref), (cap, w)
+    g.set_tuning(hirep.TUNE_PACE_WINDOW, 0)
+    check_all_ops(env, p, variant)
