@@ -314,7 +314,9 @@ int hirep_cg_g5Dphi_blocks_hat_sq(hirep_geom *g, void *x_even, const void *b_eve
  * generators of the representation in the basis of reading A10/A11 (fundamental T^a = generalised Gell-Mann / 2).
  * force_canonical: device buffer of hirep_force_bytes bytes, REAL numbers of the working precision in CANONICAL order
  * [ix][mu][a] (ix = ((t L + x) L + y) L + z); overwritten.  links_rep: the stored represented field (boundary signs included: a
- * hop across the edge contributes with bc_mu, Eq 61).  HIREP_EINVAL in HIREP_LINKS_REBUILD mode.  The first call builds the
+ * hop across the edge contributes with bc_mu, Eq 61).  In HIREP_LINKS_REBUILD mode `links_rep` is the FUNDAMENTAL field and only the
+ * adjoint representation is served (matrix-free: (T^a_adj)_bc = -i f^abc turns the projection into -4 Im tr(T^a C) with C a sum of
+ * commutators [K^dagger, W H W^dagger] of N x N matrices); every other representation returns HIREP_EINVAL there.  The first call builds the
  * generator table (one small kernel + a host round trip; not capturable in a CUDA graph), later calls only enqueue one kernel. */
 int hirep_force_bytes(const hirep_geom *g, size_t *bytes, int *n_generators);
 int hirep_force_hopping(hirep_geom *g, void *force_canonical, const void *eta_full, const void *xi_full, const void *links_rep);

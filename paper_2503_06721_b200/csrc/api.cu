@@ -1117,7 +1117,9 @@ extern "C" int hirep_force_bytes(const hirep_geom *g, size_t *bytes, int *n_gene
 }
 extern "C" int hirep_force_hopping(hirep_geom *g, void *force_canonical, const void *eta_full, const void *xi_full, const void *links_rep) {
     CHECK_PTRS("hirep_force_hopping", force_canonical, eta_full, xi_full, links_rep);
-    if (g->mode != HIREP_LINKS_STORED) return fail(HIREP_EINVAL, "hirep_force_hopping: needs the stored represented links (HIREP_LINKS_STORED)");
+    if (g->mode == HIREP_LINKS_REBUILD && g->rep == HIREP_ADJ)   // `links` is the fundamental field: matrix-free commutator form
+        return kern_result(g, k_force_hopping_adj(g->geo, g->prec, g->N, eta_full, xi_full, links_rep, force_canonical, g->stream), "hirep_force_hopping (adjoint, matrix-free)");
+    if (g->mode != HIREP_LINKS_STORED) return fail(HIREP_EINVAL, "hirep_force_hopping: needs the stored represented links (HIREP_LINKS_STORED), or the adjoint representation in HIREP_LINKS_REBUILD mode");
     int rc = force_table(g);
     if (rc) return rc;
     return kern_result(g, k_force_hopping(g->geo, g->prec, g->dR, g->real, eta_full, xi_full, links_rep, g->force_rowptr, g->force_jk, g->force_val,

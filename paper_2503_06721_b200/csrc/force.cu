@@ -14,8 +14,7 @@
 // (conflict free), all loops run over run-time d_R, so one kernel serves every representation.
 #include <vector>
 
-#include "hop_small.cuh"
-#include "rep_maps.cuh"
+#include "hop_adjmf.cuh"
 
 namespace hirep {
 namespace {
@@ -269,6 +268,212 @@ int force_site_dispatch(const Geo &g, int dR, const void *eta, const void *xi, c
     return (int)cudaGetLastError();
 }
 
+// ---- adjoint representation, matrix-free (link mode REBUILD): the force as a commutator of N x N matrices -----------------------
+// (T^a_adj)_bc = -i f^abc, so  k^dagger T^a_adj chi = -2 tr( T^a [K^dagger, X] )  with K = k_b T^b, X = chi_c T^c, and chi = R(W) h means
+// X = W H W^dagger (hop_adjmf.cuh).  Hence
+//   F^a_mu(x) = -4 Im tr( T^a C ),  C = sum_s [K^xi_s^dagger, W H^eta_s W^dagger] + [K^eta_s^dagger, W H^xi_s W^dagger],
+// four N x N products per (field pair, s) on the FUNDAMENTAL link instead of d_R x d_R work per generator: the SU(6) adjoint force
+// drops from 50 ms (sparse-generator kernel, one warp per SM) to the cost of a few stencil applications.  Same lane mapping as
+// hop_adjmf.cuh: N lanes per site (lane = matrix row), matrices exchanged through a per-warp shared-memory area [entry][site].
+template <typename T, int N> struct ForceAdjCfg {
+    using C = cplx<T>;
+    static constexpr int DR = N * N - 1, NC = 4 * DR, NN = N * N, SPW = 32 / N;
+    static constexpr int NCL = (DR + N - 1) / N, NLD = (NC + N - 1) / N;
+    static constexpr uint32_t RAW = NC * SPW * sizeof(C), MAT = NN * SPW * sizeof(C);
+    static constexpr uint32_t PER_WARP = 2 * RAW + 3 * MAT;        // neighbour spinor, own spinor | X (then C), K, W
+    static constexpr int WARPS = (int)((200 * 1024) / PER_WARP) > 8 ? 8 : (int)((200 * 1024) / PER_WARP);
+    static constexpr size_t SMEM = (size_t)PER_WARP * WARPS;
+};
+
+template <typename T, int N>
+__global__ void __launch_bounds__(ForceAdjCfg<T, N>::WARPS * 32) force_adjmf_kernel(const Geo g, const cplx<T> *eta, const cplx<T> *xi, const cplx<T> *links_fund,
+                                                                                  T *force, long n_units) {
+    using C = cplx<T>;
+    using Cfg = ForceAdjCfg<T, N>;
+    constexpr int DR = Cfg::DR, NC = Cfg::NC, NN = Cfg::NN, SPW = Cfg::SPW, NCL = Cfg::NCL, NLD = Cfg::NLD;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int sl = lane / N, r = lane - sl * N;
+    const bool lane_on = sl < SPW;
+    const int ssl = lane_on ? sl : 0;
+    unsigned char *base = smem_raw + (size_t)warp * Cfg::PER_WARP;
+    C *rawA = reinterpret_cast<C *>(base), *rawB = reinterpret_cast<C *>(base + Cfg::RAW);
+    C *mX = reinterpret_cast<C *>(base + 2 * Cfg::RAW), *mK = mX + NN * SPW, *mW = mK + NN * SPW;
+    const uint32_t rawA_s = smem_u32(rawA), rawB_s = smem_u32(rawB), mW_s = smem_u32(mW);
+    const long n_groups_par = (g.Nh + SPW - 1) / SPW;
+    const size_t half = (size_t)g.n_tiles * NC * TILE;
+
+    for (long unit = (long)blockIdx.x * Cfg::WARPS + warp; unit < n_units; unit += (long)gridDim.x * Cfg::WARPS) {
+        const int mu = (int)(unit & 3);
+        const long gp = unit >> 2;
+        const int p = (int)(gp / n_groups_par);
+        int h = (int)((gp - p * n_groups_par) * SPW) + ssl;
+        const bool active = lane_on && h < g.Nh;
+        if (h >= g.Nh) h = g.Nh - 1;
+        const int tile = h >> 5, hl = h & 31;
+        int t, x, y, zh;
+        decode_site(g, h, t, x, y, zh);
+        const int hn = mu == 0 ? neighbour<0>(g, p, t, x, y, zh) : mu == 1 ? neighbour<1>(g, p, t, x, y, zh)
+                     : mu == 2 ? neighbour<2>(g, p, t, x, y, zh) : neighbour<3>(g, p, t, x, y, zh);
+        const bool imag = (mu & 1) != 0, swap = (mu == 1 || mu == 2);
+        const int crd = mu == 0 ? t : mu == 1 ? x : mu == 2 ? y : 2 * zh + ((t + x + y + p) & 1);
+        const bool edge = mu == 0 ? t_edge(g, t, true) : (crd == g.L - 1);
+        const T sgn = (T)(edge ? g.bc[mu] : 1);                  // boundary factor of the forward hop (Eq 61)
+        const C *lk = links_fund + ((((size_t)p * g.n_tiles + tile) * 8 + mu) * NN) * TILE + hl;   // U_mu(x), forward matrix of the gather block
+
+        // row r of  sum_a h^a T^a  with h^a = psi_s^a + k psi_low^a  (k = cs or i cs)  from a staged spinor [c][site]
+        auto assemble = [&](const C *rw, int s, T sgp, C (&P)[N]) {
+            const int qq = swap ? 1 - s : s;
+            const T cs = sgp * ((mu < 2) ? T(-1) : (s ? T(1) : T(-1)));
+            const T kr = imag ? T(0) : cs, ki = imag ? cs : T(0);
+            const C *pu = rw + (size_t)(s * DR) * SPW, *pl = rw + (size_t)((2 + qq) * DR) * SPW;
+            auto hval = [&](int aa) {
+                const C u = pu[aa * SPW], v = pl[aa * SPW];
+                return mk<T>(fma(kr, v.x, fma(-ki, v.y, u.x)), fma(kr, v.y, fma(ki, v.x, u.y)));
+            };
+            C dg = mk<T>(0, 0);
+#pragma unroll
+            for (int j = 1; j < N; ++j) {
+                const C hd = hval(gen_base(j) + 2 * j);
+                const T f = (T)diag_norm(j) * (r < j ? T(1) : (r == j ? T(-j) : T(0)));
+                dg.x = fma(f, hd.x, dg.x);
+                dg.y = fma(f, hd.y, dg.y);
+            }
+#pragma unroll
+            for (int k = 0; k < N; ++k) {
+                const int i = k < r ? k : r, j = k < r ? r : k;
+                const int as_ = k == r ? 0 : gen_base(j) + 2 * i;
+                const C hS = hval(as_), hA = hval(as_ + 1);
+                const T sg2 = k > r ? T(1) : T(-1);
+                const C off = mk<T>(T(0.5) * (hS.x + sg2 * hA.y), T(0.5) * (hS.y - sg2 * hA.x));
+                P[k] = k == r ? dg : off;
+            }
+        };
+
+        C Cr[N];                                                 // row r of C
+#pragma unroll
+        for (int k = 0; k < N; ++k) Cr[k] = mk<T>(0, 0);
+        __syncwarp();
+        if (lane_on) {
+#pragma unroll
+            for (int k = 0; k < N; ++k) cp_async<sizeof(C)>(mW_s + (uint32_t)(((r * N + k) * SPW + sl) * sizeof(C)), lk + (size_t)(r * N + k) * TILE);
+        }
+#pragma unroll 1
+        for (int f = 0; f < 2; ++f) {                            // (neighbour field, own field) = (eta, xi), (xi, eta)
+            const C *fa = f ? xi : eta, *fb = f ? eta : xi;
+            const C *srcA = fa + (size_t)(1 - p) * half + ((size_t)(hn >> 5) * NC) * TILE + (hn & 31);
+            const C *srcB = fb + (size_t)p * half + ((size_t)tile * NC) * TILE + hl;
+            __syncwarp();                                        // previous readers of the staging areas are done
+            if (lane_on) {
+#pragma unroll
+                for (int m = 0; m < NLD; ++m) {
+                    const int c = r + N * m;
+                    if (c < NC) {
+                        cp_async<sizeof(C)>(rawA_s + (uint32_t)((c * SPW + sl) * sizeof(C)), srcA + (size_t)c * TILE);
+                        cp_async<sizeof(C)>(rawB_s + (uint32_t)((c * SPW + sl) * sizeof(C)), srcB + (size_t)c * TILE);
+                    }
+                }
+            }
+            cp_async_wait_all();
+            __syncwarp();
+            C wr[N];
+#pragma unroll
+            for (int k = 0; k < N; ++k) wr[k] = mW[((r * N + k) * SPW) + ssl];
+#pragma unroll 1
+            for (int s = 0; s < 2; ++s) {
+                C P[N], Kr[N];
+                assemble(rawA + ssl, s, T(-1), P);               // H_s: forward projection (1 - gamma_mu) of the neighbour
+                assemble(rawB + ssl, s, T(1), Kr);               // K_s: (1 + gamma_mu) projection of the site's own spinor
+                __syncwarp();                                    // the previous s has finished reading mX, mK
+                if (lane_on) {
+#pragma unroll
+                    for (int k = 0; k < N; ++k) { mX[((r * N + k) * SPW) + sl] = P[k]; mK[((r * N + k) * SPW) + sl] = Kr[k]; }
+                }
+                __syncwarp();
+                C A[N], X[N];
+#pragma unroll
+                for (int k = 0; k < N; ++k) A[k] = mk<T>(0, 0);
+#pragma unroll
+                for (int j = 0; j < N; ++j)
+#pragma unroll
+                    for (int k = 0; k < N; ++k) mac<T>(A[k], wr[j], mX[((j * N + k) * SPW) + ssl]);          // A = W H
+#pragma unroll
+                for (int k = 0; k < N; ++k) {
+                    C c_ = mk<T>(0, 0);
+#pragma unroll
+                    for (int j = 0; j < N; ++j) {                                                           // X = A W^dagger
+                        const C w = mW[((k * N + j) * SPW) + ssl];
+                        c_.x = fma(A[j].x, w.x, c_.x); c_.x = fma(A[j].y, w.y, c_.x);
+                        c_.y = fma(A[j].y, w.x, c_.y); c_.y = fma(-A[j].x, w.y, c_.y);
+                    }
+                    X[k] = c_;
+                }
+                __syncwarp();                                    // every row has read H
+                if (lane_on) {
+#pragma unroll
+                    for (int k = 0; k < N; ++k) mX[((r * N + k) * SPW) + sl] = X[k];
+                }
+                __syncwarp();
+                // C_r. += (K^dagger X)_r. - (X K^dagger)_r.,   K^dagger_ab = conj(K_ba)
+#pragma unroll
+                for (int j = 0; j < N; ++j) {
+                    const C kjr = mK[((j * N + r) * SPW) + ssl];                                             // K_jr -> K^dagger_rj = conj
+#pragma unroll
+                    for (int k = 0; k < N; ++k) {
+                        const C xv = mX[((j * N + k) * SPW) + ssl];
+                        Cr[k].x += kjr.x * xv.x + kjr.y * xv.y;                                              // conj(K_jr) X_jk
+                        Cr[k].y += kjr.x * xv.y - kjr.y * xv.x;
+                        const C kkj = mK[((k * N + j) * SPW) + ssl];                                         // K^dagger_jk = conj(K_kj)
+                        Cr[k].x -= X[j].x * kkj.x + X[j].y * kkj.y;                                          // X_rj conj(K_kj)
+                        Cr[k].y -= X[j].y * kkj.x - X[j].x * kkj.y;
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (lane_on) {
+#pragma unroll
+            for (int k = 0; k < N; ++k) mX[((r * N + k) * SPW) + sl] = Cr[k];
+        }
+        __syncwarp();
+        if (active) {
+            const long ix = canonical_index(g, p, h);
+            T *out = force + ((size_t)ix * 4 + mu) * DR;
+            const C *cm = mX + ssl;
+#pragma unroll
+            for (int m = 0; m < NCL; ++m) {
+                const int aa = r + N * m;
+                if (aa < DR) {
+                    const GenIdx ga = gen_decode(aa);
+                    T v;
+                    if (ga.kind == 2) {
+                        T sum = 0;
+                        for (int q = 0; q < ga.j; ++q) sum += cm[(q * N + q) * SPW].y;
+                        v = T(-4) * (T)diag_norm(ga.j) * (sum - ga.j * cm[(ga.j * N + ga.j) * SPW].y);
+                    } else {
+                        const C cij = cm[(ga.i * N + ga.j) * SPW], cji = cm[(ga.j * N + ga.i) * SPW];
+                        v = ga.kind == 0 ? T(-2) * (cij.y + cji.y) : T(2) * (cji.x - cij.x);
+                    }
+                    out[aa] = sgn * v;
+                }
+            }
+        }
+    }
+}
+
+template <typename T, int N> int launch_force_adjmf(const Geo &g, const void *eta, const void *xi, const void *links_fund, void *force, cudaStream_t s) {
+    using Cfg = ForceAdjCfg<T, N>;
+    auto kern = force_adjmf_kernel<T, N>;
+    static DevCache cache{};
+    int n_sm = 0;
+    if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
+    const long n_units = (long)2 * ((g.Nh + Cfg::SPW - 1) / Cfg::SPW) * 4;
+    long grid = (n_units + Cfg::WARPS - 1) / Cfg::WARPS;
+    if (grid > 4L * n_sm) grid = 4L * n_sm;
+    kern<<<(unsigned)grid, Cfg::WARPS * 32, Cfg::SMEM, s>>>(g, (const cplx<T> *)eta, (const cplx<T> *)xi, (const cplx<T> *)links_fund, (T *)force, n_units);
+    return (int)cudaGetLastError();
+}
+
 }  // namespace
 
 // dense generator table -> device (double2 [NA][dR][dR]); the caller converts it to the sparse form once
@@ -281,6 +486,20 @@ int k_rep_generators(int N, int rep, void *table_dev, cudaStream_t s) {
     case 5: return gen_by_rep<5>(rep, t, s);
     case 6: return gen_by_rep<6>(rep, t, s);
     }
+    return KERR_UNSUPPORTED;
+}
+
+// adjoint representation from the FUNDAMENTAL links (link mode REBUILD)
+int k_force_hopping_adj(const Geo &g, int prec, int N, const void *eta, const void *xi, const void *links_fund, void *force, cudaStream_t s) {
+#define FA(NN_) (prec == 0 ? launch_force_adjmf<double, NN_>(g, eta, xi, links_fund, force, s) : launch_force_adjmf<float, NN_>(g, eta, xi, links_fund, force, s))
+    switch (N) {
+    case 2: return FA(2);
+    case 3: return FA(3);
+    case 4: return FA(4);
+    case 5: return FA(5);
+    case 6: return FA(6);
+    }
+#undef FA
     return KERR_UNSUPPORTED;
 }
 

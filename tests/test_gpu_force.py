@@ -42,6 +42,24 @@ def test_force_baseline_configs_reduced(env, name, T, L, prec):
     check_force(env, Problem(env, synth.CONFIGS[name].resized(T, L), prec, n_spinors=2))
 
 
+@pytest.mark.parametrize("n", [2, 3, 4, 5, 6])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_force_adjoint_matrix_free(env, n, prec):
+    """Link mode REBUILD, adjoint representation: the commutator form on the FUNDAMENTAL links against the same oracle (and so against
+    the sparse-generator kernel on the stored adjoint links); 6x4^3 with a ragged site-group tail, antiperiodic t and y."""
+    hirep, oracle = env["hirep"], env["oracle"]
+    cfg = synth.Config("t", 6, 4, n, ADJ, 0.0, "haar", 6100 + n, ())
+    p = Problem(env, cfg, prec, bc=(-1, 1, -1, 1), n_spinors=2)
+    eta, xi = p.spinors
+    p.geom.set_link_mode(hirep.LINKS_REBUILD)
+    F = p.geom.force_hopping(p.to_native(eta, hirep.FULL), p.to_native(xi, hirep.FULL), p.links_fund).cpu().numpy().astype(np.float64)
+    ref = of.force_hopping(cfg.T, cfg.L, n, ADJ, p.R, eta, xi, p.bc)
+    assert oracle.rel_l2(F, ref) < TOL[prec], (n, prec, oracle.rel_l2(F, ref))
+    p.geom.set_link_mode(hirep.LINKS_STORED)
+    G = p.geom.force_hopping(p.to_native(eta, hirep.FULL), p.to_native(xi, hirep.FULL), p.links_rep).cpu().numpy().astype(np.float64)
+    assert oracle.rel_l2(F, G) < 10 * TOL[prec]
+
+
 def test_force_degenerate_and_errors(env):
     hirep = env["hirep"]
     for T, L in [(2, 2), (4, 2)]:
