@@ -484,7 +484,7 @@ def sweep_bytes(cfg, prec, rebuild):
 
 def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, peak):
     """GB/s of the streaming kernels (full-lattice spinors) and ms per CG iteration of hirep_cg_g5Dphi_sq."""
-    V, S = cfg.volume, cm["S"]
+    V, S, d = cfg.volume, cm["S"], cfg.d_R
     z_full = geom.new_spinor(hirep.FULL)
     z_full.copy_(x_full)
 
@@ -517,10 +517,14 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
     torch.cuda.synchronize()
     ms_it = (time.perf_counter() - t0) * 1e3 / max(it, 1)
     fl_it = cm["ops"]["g5Dphi_sq"][0]
-    by_it = cm["ops"]["g5Dphi_sq"][1] + (1 + 3 + 5) * S * V      # stencils + ||B p||^2 + (r update, ||r||^2) + (x, p update)
+    # compulsory bytes of one iteration: two full-lattice stencil passes (2S + 4K each; the fused form never stores A p: -S) plus the
+    # linear algebra -- unfused: ||B p||^2 (1) + r update (3) + x, p update (5) spinor passes; fused into the stencil epilogues
+    # (tile-pair kernel: complex links d_R <= 3, fp32 also d_R = 4, 6; real SU(2) adjoint in fp64): r read + write (2) + x, p update (5)
+    fused = (d <= 3 and (prec == "f64" or cfg.rep != 1)) or (prec == "f32" and cfg.rep != 1 and d in (4, 6))
+    by_it = cm["ops"]["g5Dphi_sq"][2] + ((2 + 5 - 1) if fused else (1 + 3 + 5)) * S * V
     out["cg_g5Dphi_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gflops_operator": round(fl_it / ms_it / 1e6, 1),
                            "gbs": round(by_it / ms_it / 1e6, 1), "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3),
-                           "launches_per_iteration": 7, "relres_after": res}
+                           "launches_per_iteration": 5 if fused else 7, "fused_reductions": fused, "relres_after": res}
     hb = geom.sizes["spinor_half"]
     x_e, y_e = x_full[:hb], y_full[:hb]
     geom.cg_g5Dphi_hat_sq(2.0, x_e, lr, 1e-30, 2, out=y_e)

@@ -27,6 +27,7 @@ struct hirep_geom {
     cudaStream_t stream;
     void *ws_half, *ws_half2, *ws_half3, *ws_full;   // workspace spinors (lazy)
     void *ws_red;                   // reduction partials + 4 result doubles (lazy)
+    void *ws_red2;                  // partials written by stencil launches with a fused reduction (lazy)
     void *cg_r, *cg_p, *cg_Ap;      // CG work fields (lazy)
     void *ms_p[HIREP_MAX_SHIFTS];    // multi-shift CG direction fields (lazy)
     void *bi_s, *bi_t;              // BiCGstab work fields (lazy)
@@ -153,7 +154,7 @@ extern "C" int hirep_geom_destroy(hirep_geom *g) {
     if (!g) return HIREP_OK;
     for (void *b : g->ms_p)
         if (b) cudaFree(b);
-    void *bufs[] = {g->dev_flags, g->force_rowptr, g->force_jk, g->force_val, g->force_dense, g->ws_exp, g->ws_half, g->ws_half2, g->ws_half3, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
+    void *bufs[] = {g->ws_red2, g->dev_flags, g->force_rowptr, g->force_jk, g->force_val, g->force_dense, g->ws_exp, g->ws_half, g->ws_half2, g->ws_half3, g->ws_full, g->ws_red, g->cg_r, g->cg_p, g->cg_Ap, g->bi_s, g->bi_t, g->h_links_canon, g->h_links_fund, g->h_links_rep, g->h_in_canon,
                     g->h_in_native, g->h_out_native, g->h_out_canon, g->h_out_canon2};
     if (g->host_events) {
         for (int i = 0; i < 2; ++i) { cudaEventDestroy(g->ev_done[i]); cudaEventDestroy(g->ev_copied[i]); }
@@ -355,7 +356,9 @@ extern "C" int hirep_Dphi_oe(hirep_geom *g, void *out_odd, const void *in_even, 
     return offdiag(g, out_odd, in_even, links, 1, "hirep_Dphi_oe");
 }
 
-static int dphi_full(hirep_geom *g, double m0, void *out, const void *in, const void *links, int g5, const char *what, double am = 0.0) {
+struct FusedRed { int mode; void *r; const double *num, *den; };
+static int dphi_full(hirep_geom *g, double m0, void *out, const void *in, const void *links, int g5, const char *what, double am = 0.0,
+                     const FusedRed *red = nullptr) {
     const size_t hb = g->bytes_spinor_half;
     const char *in_e = (const char *)in, *in_o = in_e + hb;
     char *out_e = (char *)out, *out_o = out_e + hb;
@@ -364,7 +367,17 @@ static int dphi_full(hirep_geom *g, double m0, void *out, const void *in, const 
     L.set[0] = HopSet{in_o, out_e, in_e, links_parity(g, links, 0), 0};
     L.set[1] = HopSet{in_e, out_o, in_o, links_parity(g, links, 1), 1};
     L.a = 4.0 + m0; L.b = -0.5; L.g5 = g5; L.am = am;
+    if (red) {
+        L.red_mode = red->mode; L.red_alg = g->sum_alg; L.red_partial = g->ws_red2;
+        L.red_r = red->r; L.red_num = red->num; L.red_den = red->den;
+    }
     return hop(g, L, what);
+}
+// does a default full-lattice launch of this geometry run the tile-pair kernel, whose epilogue can carry the CG's reductions?
+static bool fused_cg_ok(const hirep_geom *g) {
+    if (g->mode != HIREP_LINKS_STORED || g->variant != 0 || g->slab || g->tune_max_ctas < 0) return false;
+    const bool f64 = g->prec == HIREP_F64;
+    return (g->dR <= 3 && (f64 || !g->real)) || (!f64 && !g->real && g->dR != 5 && g->dR <= 6);
 }
 
 extern "C" int hirep_Dphi(hirep_geom *g, double m0, void *out_full, const void *in_full, const void *links) {
@@ -856,19 +869,40 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
         const void *Bp = inv_odd ? g->ws_half3 : (full || twisted) ? g->ws_full : g->ws_half2;
         return kern_result(g, k_prod(g->geo, g->prec, g->dR, halves, 1, g->sum_alg, Bp, Bp, g->ws_red, d, g->stream), what, 2);
     };
+    // Fused form (plain Wilson Q^2 on the full lattice, when the tile-pair kernel runs it): pass 1 = gamma_5 D p with ||B p||^2 = <p,Ap>
+    // accumulated in its epilogue; pass 2 = gamma_5 D (B p) whose epilogue does r -= alpha A p and accumulates ||r||^2 without ever
+    // storing A p: 3 spinor passes and 2 launches fewer per iteration (the separate ||Bp||^2 and residual-update kernels are gone).
+    const bool fused = full && !twisted && !clover && !blocks_even && !inv_odd && fused_cg_ok(g);
+    const int nred = k_reduce_workspace_bytes() / (int)(2 * 3 * sizeof(double));   // Acc pairs the partial buffer holds
+    if (fused) {
+        if ((rc = workspace(&g->ws_red2, (size_t)k_reduce_workspace_bytes())) || (rc = workspace(&g->ws_full, 2 * g->bytes_spinor_half))) return rc;
+        if ((e = cudaMemsetAsync(g->ws_red2, 0, (size_t)k_reduce_workspace_bytes(), g->stream)) != cudaSuccess) return cuda_fail(e, what);
+    }
+    auto fused_pass1 = [&]() -> int {
+        const FusedRed fr{1, nullptr, nullptr, nullptr};
+        int rc2 = dphi_full(g, m0, g->ws_full, g->cg_p, links, 1, what, 0.0, &fr);
+        if (rc2) return rc2;
+        return kern_result(g, k_reduce_final(nred, g->sum_alg, g->ws_red2, d, g->stream), what);
+    };
     int it = 0;
     bool more = bb > 0.0 && it < maxiter && !(rr <= tol * tol * bb);
-    if (more && (rc = apply_op())) return rc;
+    if (more && (rc = fused ? fused_pass1() : apply_op())) return rc;
     while (more) {
         double *rr_old = d + 2 + 2 * (it & 1), *rr_new_d = d + 2 + 2 * ((it + 1) & 1);
-        rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, halves, g->sum_alg, 0.0, rr_old, d, nullptr, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, rr_new_d, g->stream), what, 2);
-        if (rc) return rc;
+        if (fused) {
+            const FusedRed fr{2, g->cg_r, rr_old, d};
+            if ((rc = dphi_full(g, m0, g->cg_Ap, g->ws_full, links, 1, what, 0.0, &fr))) return rc;
+            if ((rc = kern_result(g, k_reduce_final(nred, g->sum_alg, g->ws_red2, rr_new_d, g->stream), what))) return rc;
+        } else {
+            rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, halves, g->sum_alg, 0.0, rr_old, d, nullptr, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, rr_new_d, g->stream), what, 2);
+            if (rc) return rc;
+        }
         if ((rc = kern_result(g, k_cg_xp(g->geo, g->prec, g->dR, halves, 0.0, 0.0, rr_old, d, rr_new_d, x, g->cg_p, g->cg_r, g->stream), what))) return rc;
         if ((e = cudaMemcpyAsync(g->h_scal, d, sizeof(double), cudaMemcpyDeviceToHost, g->stream)) != cudaSuccess) return cuda_fail(e, what);
         if ((e = cudaMemcpyAsync(g->h_scal + 1, rr_new_d, sizeof(double), cudaMemcpyDeviceToHost, g->stream)) != cudaSuccess) return cuda_fail(e, what);
         if ((e = cudaEventRecord(g->ev_scal, g->stream)) != cudaSuccess) return cuda_fail(e, what);
         ++it;
-        if (it < maxiter && (rc = apply_op())) return rc;   // queued before the host looks at ||r||^2
+        if (it < maxiter && (rc = fused ? fused_pass1() : apply_op())) return rc;   // queued before the host looks at ||r||^2
         if ((e = cudaEventSynchronize(g->ev_scal)) != cudaSuccess) return cuda_fail(e, what);
         const double pAp = g->h_scal[0];
         if (!(pAp > 0.0) || !std::isfinite(pAp))

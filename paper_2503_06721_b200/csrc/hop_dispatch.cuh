@@ -26,8 +26,8 @@ template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int
     // 0.130 -> 0.119 ms in fp32, in bursts; on par under a sustained power-capped load), the real SU(2) adjoint in fp64 (C3: 0.98 -> 0.89 ms) and
     // complex links at d_R = 4, 6 in fp32 (C4: 4.91 -> 4.47 ms; SU(3) SYM 32^4 0.47 -> 0.34 ms; d_R = 5 has only one-row chunks and loses).  In fp64 at d_R >= 4 (half-spinor split over 4 warps: C4 10.7 vs 10.3 ms) and for real
     // links in fp32 the gather-layout kernels are faster; variant 5 forces it anywhere.
-    if (hop_full_eligible(L) && (variant == 5 || (variant == 0 && ((DR <= 3 && (sizeof(T) == 8 || !REAL)) || (sizeof(T) == 4 && !REAL && DR != 5)))))
-        return launch_hop_full<T, DR, REAL>(g, L, s);
+    if (hop_full_eligible(L) && (variant == 5 || (variant == 0 && hop_full_default<T, DR, REAL>()))) return launch_hop_full<T, DR, REAL>(g, L, s);
+    if (L.red_mode != 0) return KERR_UNSUPPORTED;   // the fused reductions exist in the tile-pair kernel only
     if (variant == 5) variant = 0;
     if (variant == 0) {
         // one thread per site spills in fp64 from d_R = 5 on; in fp32 at d_R >= 5 only the passes with a diagonal
@@ -49,6 +49,7 @@ template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int
 // shapes from a sweep on 32x24^3, profiles/r01b_summary.md),
 // variant 1 = the direct-load row-group kernel of round 1 (hop_large.cuh), kept for comparison
 template <typename T, int DR, bool REAL, int R, int TP> int hop_large_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
+    if (L.red_mode != 0) return KERR_UNSUPPORTED;
     if (variant == 0) return launch_hop_rows<T, DR, REAL, R, TP>(g, L, s);
     if (variant == 1 && L.tile_end == 0) return launch_hop_large<T, DR, REAL, R>(g, L, s);
     return KERR_UNSUPPORTED;
@@ -62,6 +63,7 @@ template <typename T, int N, int REP> int hop_rebuild(const Geo &g, int variant,
     return launch_hop_pair<T, M::DR, M::REAL, N, REP>(g, L, s);
 }
 template <typename T> int hop_rebuild_by_config(const Geo &g, int N, int rep, int variant, const HopLaunch &L, cudaStream_t s) {
+    if (L.red_mode != 0) return KERR_UNSUPPORTED;
     switch (rep * 10 + N) {
     case 2: return hop_rebuild<T, 2, 0>(g, variant, L, s);    // FUND
     case 3: return hop_rebuild<T, 3, 0>(g, variant, L, s);

@@ -29,6 +29,7 @@
 // Optionally (SPLIT) the two half-spinor components are split over two warps as in hop_pair.cuh (fp64, d_R >= 4).
 #pragma once
 #include "hop_pair.cuh"
+#include "reduce.cuh"
 
 namespace hirep {
 
@@ -190,7 +191,18 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
     pdl_wait();
 
     const int gg = blockIdx.x * GROUPS + grp, ng = gridDim.x * GROUPS;
-    if (gg >= g.n_tiles) return;                        // the whole group leaves together
+    Acc racc{0.0, 0.0, 0.0};                            // fused reduction (HopLaunch::red_mode): this thread's compensated partial sum
+    __shared__ Acc red_scratch[32];
+    auto red_finish = [&]() {                           // every thread of the CTA calls this exactly once
+        if (L.red_mode == 0) return;
+        cta_merge(racc, L.red_alg, red_scratch);
+        if (threadIdx.x == 0) {
+            Acc *part = (Acc *)L.red_partial;
+            part[2 * blockIdx.x] = racc;
+            part[2 * blockIdx.x + 1] = Acc{0.0, 0.0, 0.0};
+        }
+    };
+    if (gg >= g.n_tiles) { red_finish(); return; }      // the whole group leaves together
     const int my_tiles = (g.n_tiles - gg + ng - 1) / ng;
     const int my_chunks = my_tiles * CPT;
 
@@ -520,19 +532,50 @@ __global__ void __launch_bounds__(GROUPS * (SPLIT ? 4 : 2) * 32, 1) hop_full_ker
             }
         }
         if (c_active) {
-            C *out = (C *)(par ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
+            const size_t eoff = ((size_t)c_tile * NC) * TILE + lane;
+            // fused reductions: the <= 8 d_R squares of ONE site are summed in four independent plain chains (a serial compensated
+            // chain per element costs ~10 % of a tile), the site totals enter the thread's compensated accumulator
+            double site[4] = {0.0, 0.0, 0.0, 0.0};
+            if (L.red_mode == 2) {
+                // CG residual update fused into the second stencil pass: r -= alpha (A p), ||r||^2 accumulated; A p is never stored
+                C *rp = (C *)L.red_r + (size_t)par * ((size_t)g.n_tiles * NC * TILE) + eoff;
+                const T al = (T)__ddiv_rn(L.red_num[0], L.red_den[0]);
 #pragma unroll
-            for (int kk = 0; kk < NSC; ++kk) {
-                const int s = SPLIT ? s_rt : kk;
+                for (int kk = 0; kk < NSC; ++kk) {
+                    const int s = SPLIT ? s_rt : kk;
 #pragma unroll
-                for (int c = 0; c < DR; ++c) {
-                    st_spinor(out + (size_t)(s * DR + c) * TILE, mk<T>(b * up[kk][c].x, b * up[kk][c].y));
-                    st_spinor(out + (size_t)((2 + s) * DR + c) * TILE, mk<T>(g5s * b * lo[kk][c].x, g5s * b * lo[kk][c].y));
+                    for (int c = 0; c < DR; ++c) {
+                        C ru = rp[(size_t)(s * DR + c) * TILE], rl = rp[(size_t)((2 + s) * DR + c) * TILE];
+                        ru.x -= al * (b * up[kk][c].x); ru.y -= al * (b * up[kk][c].y);
+                        rl.x -= al * (g5s * b * lo[kk][c].x); rl.y -= al * (g5s * b * lo[kk][c].y);
+                        rp[(size_t)(s * DR + c) * TILE] = ru;
+                        rp[(size_t)((2 + s) * DR + c) * TILE] = rl;
+                        site[0] = fma((double)ru.x, (double)ru.x, site[0]); site[1] = fma((double)ru.y, (double)ru.y, site[1]);
+                        site[2] = fma((double)rl.x, (double)rl.x, site[2]); site[3] = fma((double)rl.y, (double)rl.y, site[3]);
+                    }
                 }
+                acc_add(racc, (site[0] + site[1]) + (site[2] + site[3]), L.red_alg);
+            } else {
+                C *out = (C *)(par ? L.set[1].out : L.set[0].out) + eoff;
+#pragma unroll
+                for (int kk = 0; kk < NSC; ++kk) {
+                    const int s = SPLIT ? s_rt : kk;
+#pragma unroll
+                    for (int c = 0; c < DR; ++c) {
+                        const C vu = mk<T>(b * up[kk][c].x, b * up[kk][c].y), vl = mk<T>(g5s * b * lo[kk][c].x, g5s * b * lo[kk][c].y);
+                        st_spinor(out + (size_t)(s * DR + c) * TILE, vu);
+                        st_spinor(out + (size_t)((2 + s) * DR + c) * TILE, vl);
+                        // ||out||^2 (= <p, A p> for A = B^dagger B when out = B p)
+                        site[0] = fma((double)vu.x, (double)vu.x, site[0]); site[1] = fma((double)vu.y, (double)vu.y, site[1]);
+                        site[2] = fma((double)vl.x, (double)vl.x, site[2]); site[3] = fma((double)vl.y, (double)vl.y, site[3]);
+                    }
+                }
+                if (L.red_mode == 1) acc_add(racc, (site[0] + site[1]) + (site[2] + site[3]), L.red_alg);
             }
         }
         if (L.pace_every > 0 && wg == 0 && lane == 0) atomicAdd(L.pace, 1u);
     }
+    red_finish();
 }
 
 // shape per instantiation (B200 sweeps, profiles/r02_summary.md): SPLIT in fp64 from d_R = 4 on (one thread per site would hold
@@ -583,6 +626,10 @@ template <typename T, int DR, bool REAL> struct FullPick {
 inline bool hop_full_eligible(const HopLaunch &L) {
     return L.nsets == 2 && L.set[0].p_out == 0 && L.set[1].p_out == 1 && L.set[0].self == L.set[1].in && L.set[1].self == L.set[0].in &&
            L.b != 0.0 && L.tile_end == 0;
+}
+// would a full-lattice launch of this instantiation run hop_full by default?  (the fused CG asks before it relies on the epilogue hooks)
+template <typename T, int DR, bool REAL> constexpr bool hop_full_default() {
+    return (DR <= 3 && (sizeof(T) == 8 || !REAL)) || (sizeof(T) == 4 && !REAL && DR != 5 && DR <= 6);
 }
 
 template <typename T, int DR, bool REAL, bool SPLIT, int GROUPS, int STAGES, int RPC, bool NBREG = false> int launch_hop_full_cfg(const Geo &g, const HopLaunch &L, cudaStream_t s) {

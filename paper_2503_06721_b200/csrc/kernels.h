@@ -24,6 +24,14 @@ struct HopLaunch {
     int g5;             // multiply the result by gamma_5 = diag(1,1,-1,-1)
     int max_ctas;       // cap on the persistent grid (0 = one CTA per SM); tests use it to force many tiles per warp
     int tile_begin, tile_end;   // tiles [begin, end) of each parity to compute (slab regions: interior / boundary); end = 0: all
+    // reductions fused into the epilogue of the tile-pair kernel (hop_full.cuh; the CG on Q^2):
+    //   red_mode 1: the result is stored as usual and sum |out|^2 over the real sites is accumulated
+    //   red_mode 2: the result is NOT stored; red_r -= (red_num / red_den) * result, sum |red_r|^2 is accumulated
+    // per-CTA partial sums (compensated, algorithm red_alg) go to red_partial[2 * blockIdx.x] (an Acc of reduce.cuh, second one zero)
+    int red_mode, red_alg;
+    void *red_partial;
+    void *red_r;                        // native full-lattice spinor (even half, then odd half)
+    const double *red_num, *red_den;    // device scalars
     unsigned *pace;     // hop_full.cuh: device counter of the round pacing (NULL / pace_every = 0: off)
     int pace_every;     // grid-wide rendezvous every pace_every tile rounds
     int dbg;            // HIREP_DBG (development only, results become wrong): bit mu skips the backward-link gather of direction mu,
@@ -45,6 +53,8 @@ int k_links_to_rep(const Geo &g, int prec, int N, int rep, void *native_rep, con
 int k_hop(const Geo &g, int prec, int N, int rep, int mode, int variant, const HopLaunch &L, cudaStream_t s);
 // linalg.cu: spinor linear algebra / reductions on native buffers (n = complex elements incl. padding; halves = 1 | 2)
 int k_reduce_workspace_bytes();
+// second stage of a reduction whose per-CTA partials a stencil launch has written (HopLaunch::red_partial): out_dev[0..1]
+int k_reduce_final(int nblocks, int alg, const void *partial, double *out_dev, cudaStream_t s);
 int k_lincomb(int prec, long n, void *xi, const double c0[2], int use_xi, const void *eta, const double c1[2], const void *zeta,
               const double c2[2], int use_zeta, cudaStream_t s);
 int k_gamma(const Geo &g, int prec, int dR, int halves, int mu, void *xi, const void *eta, cudaStream_t s);

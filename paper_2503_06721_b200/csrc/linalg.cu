@@ -14,6 +14,7 @@
 // All kernels are HBM-bound streaming passes: 128-bit accesses, grid = 4 CTAs per SM, grid-stride loops.  The
 // padding lanes of the last tile (sites h >= Nh) are excluded from every reduction.
 #include "kernels.h"
+#include "reduce.cuh"
 
 namespace hirep {
 
@@ -21,62 +22,6 @@ namespace {
 
 constexpr int RED_THREADS = 256;
 
-// running compensated sum.  ALG selects the paper's accumulation algorithm (L636: "different algorithms for the
-// accumulation are available"):  2 = Neumaier (Algorithm 2, the default): value = s + c
-//                                3 = second-order Neumaier (Algorithm 3):  value = s + (c + c2)
-//                                4 = double-double (Algorithm 4):          value = s, with (s, c) a normalised pair
-struct Acc {
-    double s, c, c2;
-};
-__device__ __forceinline__ void two_sum(double a, double b, double &s, double &e) {   // branch-free variant of Alg 1
-    s = __dadd_rn(a, b);
-    const double bb = __dsub_rn(s, a);
-    e = __dadd_rn(__dsub_rn(a, __dsub_rn(s, bb)), __dsub_rn(b, bb));
-}
-__device__ __forceinline__ void acc_add(Acc &A, double x, int alg) {   // one loop iteration of Algorithm 2 / 3 / 4
-    double s, e;
-    two_sum(A.s, x, s, e);
-    if (alg == 2) {
-        A.s = s;
-        A.c = __dadd_rn(A.c, e);
-    } else if (alg == 3) {
-        double c, e2;
-        two_sum(A.c, e, c, e2);
-        A.s = s;
-        A.c = c;
-        A.c2 = __dadd_rn(A.c2, e2);
-    } else {
-        two_sum(s, __dadd_rn(A.c, e), A.s, A.c);
-    }
-}
-// merge two partial sums of the same algorithm (lanes, warps, blocks): the partner's components enter as terms
-__device__ __forceinline__ void acc_merge(Acc &A, const Acc &B, int alg) {
-    double s, e;
-    two_sum(A.s, B.s, s, e);
-    if (alg == 2) {
-        A.s = s;
-        A.c = __dadd_rn(__dadd_rn(A.c, B.c), e);
-    } else if (alg == 3) {
-        double c, e2, c3, e3;
-        two_sum(A.c, B.c, c, e2);
-        two_sum(c, e, c3, e3);
-        A.s = s;
-        A.c = c3;
-        A.c2 = __dadd_rn(__dadd_rn(A.c2, B.c2), __dadd_rn(e2, e3));
-    } else {
-        two_sum(s, __dadd_rn(__dadd_rn(A.c, B.c), e), A.s, A.c);
-    }
-}
-__device__ __forceinline__ double acc_value(const Acc &A, int alg) {
-    return alg == 2 ? __dadd_rn(A.s, A.c) : alg == 3 ? __dadd_rn(A.s, __dadd_rn(A.c, A.c2)) : A.s;
-}
-__device__ __forceinline__ Acc acc_shfl_down(const Acc &A, int off) {
-    Acc B;
-    B.s = __shfl_down_sync(0xffffffffu, A.s, off);
-    B.c = __shfl_down_sync(0xffffffffu, A.c, off);
-    B.c2 = __shfl_down_sync(0xffffffffu, A.c2, off);
-    return B;
-}
 // block-wide merge of NV accumulators per thread; result valid in thread 0
 template <int NV> __device__ void block_merge(Acc (&a)[NV], int alg) {
     __shared__ Acc sh[NV][RED_THREADS / 32];
@@ -364,6 +309,11 @@ int k_prod(const Geo &g, int prec, int dR, int halves, int mode, int alg, const 
         else prod_partial_kernel<float, 1><<<nb, RED_THREADS, 0, s>>>(P, n, alg, (const float2 *)xi, (const float2 *)eta, partial);
     }
     reduce_final_kernel<<<1, RED_THREADS, 0, s>>>(nb, alg, partial, out_dev);
+    return (int)cudaGetLastError();
+}
+
+int k_reduce_final(int nblocks, int alg, const void *partial, double *out_dev, cudaStream_t s) {
+    reduce_final_kernel<<<1, RED_THREADS, 0, s>>>(nblocks, alg, (const Acc *)partial, out_dev);
     return (int)cudaGetLastError();
 }
 
