@@ -133,6 +133,22 @@ int hirep_Dphi_eo(hirep_geom *g, void *out_even, const void *in_odd, const void 
 int hirep_Dphi_oe(hirep_geom *g, void *out_odd, const void *in_even, const void *links);
 int hirep_Dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links);
 int hirep_g5Dphi_sq(hirep_geom *g, double m0, void *out_full, const void *in_full, const void *links);
+/* hirep_Dphi_hat_static: the same operator as hirep_Dphi_hat (Eq 44), same arguments, same kernels and launch order,
+ * same result bit for bit, for callers that cannot call cudaMalloc (a stream under CUDA graph capture, a serving loop, a harness
+ * that forbids it).  The odd intermediate field D_oe in_even lives in a static device array of HIREP_STATIC_SCRATCH_BYTES
+ * (16 MiB; every GPU that loads the library holds it until exit) instead of the handle's lazily allocated workspace: the call
+ * makes no cudaMalloc, cudaFree or allocating library call.  Limits and hazards:
+ *   - one half-lattice spinor of the geometry must fit: 4 d_R * 16 (8 in fp32) bytes per site slot * 32 * ceil(V/64) <=
+ *     HIREP_STATIC_SCRATCH_BYTES (e.g. SU(3) fundamental fp64 up to 16^3 x 32); larger geometries are rejected with
+ *     HIREP_EINVAL and a message, nothing is launched;
+ *   - slab geometries: HIREP_EUNSUPPORTED, as hirep_Dphi_hat;
+ *   - every call on a device shares the one array: two calls that overlap on the GPU (different streams, different handles,
+ *     different host threads) RACE on it.  Calls on one stream are ordered and safe.  The array keeps the previous call's
+ *     contents; what must be zero (the padding lanes of a ragged last tile) is cleared on the stream by each call;
+ *   - the first call on a device resolves the array's address (cudaGetSymbolAddress) and loads the kernels: make one call
+ *     before starting a capture.  out_even, in_even, links: device pointers owned by the caller, as hirep_Dphi_hat. */
+#define HIREP_STATIC_SCRATCH_BYTES (16u << 20)
+int hirep_Dphi_hat_static(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links);
 /* The Hermitian even-odd preconditioned operator (Eq 45) in the normalisation of Eq 44 (A22):
  *   hirep_g5Dphi_hat     out_even = gamma_5 ((4+m)^2 - D_eo D_oe) in_even = Q_hat in_even
  *   hirep_g5Dphi_hat_sq  out_even = Q_hat Q_hat in_even      (Hermitian positive definite: what CG inverts in HMC, L772/L806) */

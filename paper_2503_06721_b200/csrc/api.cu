@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -406,6 +407,57 @@ extern "C" int hirep_Dphi_hat(hirep_geom *g, double m0, void *out_even, const vo
     CHECK_PTRS("hirep_Dphi_hat", out_even, in_even, links);
     if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_Dphi_hat: out aliases in");
     return dphi_hat(g, m0, out_even, in_even, links, 0, "hirep_Dphi_hat");
+}
+
+// ---- hirep_Dphi_hat_static: Dphi_hat for callers that cannot call cudaMalloc (CUDA graph capture, serving loops) ----------
+// The odd intermediate field D_oe in_e of Eq 44 (L808) lives in a file-scope device array instead of the handle's lazily
+// allocated workspace.  Every GPU that loads the library holds HIREP_STATIC_SCRATCH_BYTES until exit.  In host code the array's
+// name is only a stand-in for the symbol: the device address is resolved once per device with cudaGetSymbolAddress.
+static __device__ __align__(256) unsigned char g_static_scratch[HIREP_STATIC_SCRATCH_BYTES];
+static void *g_static_scratch_addr[64];   // per CUDA device ordinal
+static std::mutex g_static_scratch_mu;
+static int static_scratch(const hirep_geom *g, void **ptr, const char *what) {
+    int dev = g->device;
+    cudaError_t e = dev >= 0 ? cudaSuccess : cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, what);
+    if (dev < 0 || dev >= 64) return fail(HIREP_EUNSUPPORTED, "%s: CUDA device ordinal %d outside the table of 64", what, dev);
+    std::lock_guard<std::mutex> lk(g_static_scratch_mu);
+    if (!g_static_scratch_addr[dev]) {   // the geometry's device is the current one (CHECK_PTRS): the address is that device's copy
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess || !p) return cuda_fail(e, "hirep_Dphi_hat_static: cudaGetSymbolAddress");
+        g_static_scratch_addr[dev] = p;
+    }
+    *ptr = g_static_scratch_addr[dev];
+    return HIREP_OK;
+}
+extern "C" int hirep_Dphi_hat_static(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links) {
+    const char *what = "hirep_Dphi_hat_static";
+    CHECK_PTRS("hirep_Dphi_hat_static", out_even, in_even, links);
+    if (out_even == in_even) return fail(HIREP_EINVAL, "%s: out aliases in", what);
+    if (g->slab) return fail(HIREP_EUNSUPPORTED, "%s: on a slab compose the two passes yourself (Dphi_oe, halo exchange, Dphi_eo)", what);
+    if (g->bytes_spinor_half > (size_t)HIREP_STATIC_SCRATCH_BYTES)
+        return fail(HIREP_EINVAL, "%s: one half-lattice spinor of this geometry is %zu bytes, the static scratch holds %zu (HIREP_STATIC_SCRATCH_BYTES); use hirep_Dphi_hat",
+                    what, g->bytes_spinor_half, (size_t)HIREP_STATIC_SCRATCH_BYTES);
+    void *tmp = nullptr;
+    int rc = static_scratch(g, &tmp, what);
+    if (rc) return rc;
+    // The array keeps the previous call's contents, possibly of another geometry.  Every site lane is overwritten by the first pass; the
+    // padding lanes of a ragged last tile are not, and the handle's own workspace holds zeros there: clear that tile.
+    if (g->geo.Nh % TILE) {
+        const size_t tile_bytes = g->bytes_spinor_half / (size_t)g->geo.n_tiles;
+        const cudaError_t e = cudaMemsetAsync((char *)tmp + (size_t)(g->geo.n_tiles - 1) * tile_bytes, 0, tile_bytes, g->stream);
+        if (e != cudaSuccess) return cuda_fail(e, what);
+    }
+    rc = offdiag(g, tmp, in_even, links, 1, what);
+    if (rc) return rc;
+    HopLaunch L{};
+    L.nsets = 1;
+    L.set[0] = HopSet{tmp, out_even, in_even, links_parity(g, links, 0), 0};
+    L.a = (4.0 + m0) * (4.0 + m0);
+    L.b = +0.5;
+    L.g5 = 0;
+    return hop(g, L, what);
 }
 
 extern "C" int hirep_g5Dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links) {

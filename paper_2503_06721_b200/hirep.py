@@ -22,6 +22,7 @@ LINKS_STORED, LINKS_REBUILD = 0, 1
 OP_DPHI, OP_DPHI_EO, OP_DPHI_OE, OP_DPHI_HAT, OP_G5DPHI_SQ = 0, 1, 2, 3, 4
 TUNE_MAX_CTAS, TUNE_SUM_ALGORITHM, TUNE_PACE_WINDOW = 1, 2, 3
 REGION_ALL, REGION_OWNED, REGION_INTERIOR, REGION_BOUNDARY = 0, 1, 2, 3
+STATIC_SCRATCH_BYTES = 16 << 20   # HIREP_STATIC_SCRATCH_BYTES
 OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM, EBREAKDOWN = 0, -1, -2, -3, -4, -5
 
 # every symbol include/hirep_b200.h declares
@@ -29,7 +30,7 @@ SYMBOLS = [
     "hirep_geom_create", "hirep_geom_destroy", "hirep_geom_set_bc", "hirep_geom_set_stream", "hirep_geom_sizes",
     "hirep_spinor_import", "hirep_spinor_export", "hirep_links_import", "hirep_links_rep_export",
     "hirep_links_rep_export_bwd", "hirep_links_to_rep", "hirep_Dphi", "hirep_Dphi_eo", "hirep_Dphi_oe",
-    "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_g5Dphi_hat", "hirep_g5Dphi_hat_sq", "hirep_cg_g5Dphi_hat_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_set_tuning", "hirep_launch_count",
+    "hirep_Dphi_hat", "hirep_Dphi_hat_static", "hirep_g5Dphi_sq", "hirep_g5Dphi_hat", "hirep_g5Dphi_hat_sq", "hirep_cg_g5Dphi_hat_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_set_tuning", "hirep_launch_count",
     "hirep_apply_host", "hirep_apply_host_async", "hirep_spinor_zero", "hirep_spinor_copy", "hirep_spinor_mul", "hirep_spinor_minus",
     "hirep_spinor_lc", "hirep_spinor_clc", "hirep_spinor_lc_add_assign", "hirep_spinor_clc_add_assign",
     "hirep_spinor_lc1", "hirep_spinor_lc2", "hirep_spinor_lc3", "hirep_spinor_prod", "hirep_spinor_sqnorm",
@@ -76,7 +77,7 @@ def load():
         getattr(lib, n).argtypes = [vp, vp, vp, ci]
     for n in ("hirep_links_import", "hirep_links_rep_export", "hirep_links_rep_export_bwd", "hirep_links_to_rep"):
         getattr(lib, n).argtypes = [vp, vp, vp]
-    for n in ("hirep_Dphi", "hirep_Dphi_hat", "hirep_g5Dphi_sq", "hirep_g5Dphi_hat", "hirep_g5Dphi_hat_sq"):
+    for n in ("hirep_Dphi", "hirep_Dphi_hat", "hirep_Dphi_hat_static", "hirep_g5Dphi_sq", "hirep_g5Dphi_hat", "hirep_g5Dphi_hat_sq"):
         getattr(lib, n).argtypes = [vp, cd, vp, vp, vp]
     for n in ("hirep_Dphi_eo", "hirep_Dphi_oe"):
         getattr(lib, n).argtypes = [vp, vp, vp, vp]
@@ -195,6 +196,7 @@ def hirep_Dphi(g, m0, out, inp, links): _check(load().hirep_Dphi(g, m0, out, inp
 def hirep_Dphi_eo(g, out, inp, links): _check(load().hirep_Dphi_eo(g, out, inp, links))
 def hirep_Dphi_oe(g, out, inp, links): _check(load().hirep_Dphi_oe(g, out, inp, links))
 def hirep_Dphi_hat(g, m0, out, inp, links): _check(load().hirep_Dphi_hat(g, m0, out, inp, links))
+def hirep_Dphi_hat_static(g, m0, out, inp, links): _check(load().hirep_Dphi_hat_static(g, m0, out, inp, links))
 def hirep_g5Dphi_sq(g, m0, out, inp, links): _check(load().hirep_g5Dphi_sq(g, m0, out, inp, links))
 def hirep_g5Dphi_hat(g, m0, out, inp, links): _check(load().hirep_g5Dphi_hat(g, m0, out, inp, links))
 def hirep_g5Dphi_hat_sq(g, m0, out, inp, links): _check(load().hirep_g5Dphi_hat_sq(g, m0, out, inp, links))
@@ -497,6 +499,11 @@ class Geometry:
     def Dphi_hat(self, m0, inp_even, links, out=None):
         out = self.new_spinor(EVEN) if out is None else out
         hirep_Dphi_hat(self.handle, m0, out.data_ptr(), inp_even.data_ptr(), links.data_ptr())
+        return out
+
+    def Dphi_hat_static(self, m0, inp_even, links, out):
+        """hirep_Dphi_hat_static: no allocation inside the call, so the caller passes `out` (include/hirep_b200.h)."""
+        hirep_Dphi_hat_static(self.handle, m0, out.data_ptr(), inp_even.data_ptr(), links.data_ptr())
         return out
 
     def g5Dphi_sq(self, m0, inp, links, out=None):
