@@ -534,10 +534,13 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
     torch.cuda.synchronize()
     ms_it = (time.perf_counter() - t0) * 1e3 / max(it, 1)
     fl_it = 2 * cm["ops"]["Dphi_hat"][0]
-    by_it = 2 * cm["ops"]["Dphi_hat"][1] + (1 + 3 + 5) * S * V / 2
+    # same accounting on the even sites; the ring / pair kernels (d_R <= 6, stored links) carry the reductions in the epilogue of the
+    # second pass of each Q_hat: ||Q_hat p||^2 with the first, r -= alpha A p and ||r||^2 (A p never stored) with the second
+    fused_eo = d <= 6
+    by_it = 2 * cm["ops"]["Dphi_hat"][1] + ((2 + 5 - 1) if fused_eo else (1 + 3 + 5)) * S * V / 2
     out["cg_g5Dphi_hat_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gflops_operator": round(fl_it / ms_it / 1e6, 1),
                                "gbs": round(by_it / ms_it / 1e6, 1), "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3),
-                               "launches_per_iteration": 9, "relres_after": res}
+                               "launches_per_iteration": 7 if fused_eo else 9, "fused_reductions": fused_eo, "relres_after": res}
     ms = timeit(lambda: geom.Dphi_tm_hat(m0, 0.3, x_e, lr, out=y_e), reps=10)
     by = cm["ops"]["Dphi_hat"][1] + 2 * S * V / 2          # + the in-place gamma_5 combination on the odd field
     out["Dphi_tm_hat"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3),

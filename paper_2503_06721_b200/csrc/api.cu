@@ -388,7 +388,9 @@ extern "C" int hirep_Dphi(hirep_geom *g, double m0, void *out_full, const void *
 }
 
 // out_even = [gamma_5] ((4+m)^2 in_even - D_eo D_oe in_even): two half-lattice passes through the odd workspace
-static int dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links, int g5, const char *what) {
+// `red` (CG only): the reduction fused into the epilogue of the SECOND pass, which writes the result (FusedRed, above)
+static int dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links, int g5, const char *what,
+                    const FusedRed *red = nullptr) {
     if (g->slab) return fail(HIREP_EUNSUPPORTED, "%s: on a slab compose the two passes yourself (Dphi_oe, halo exchange, Dphi_eo)", what);
     int rc = workspace(&g->ws_half, g->bytes_spinor_half);
     if (rc) return rc;
@@ -400,7 +402,15 @@ static int dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_eve
     L.a = (4.0 + m0) * (4.0 + m0);
     L.b = +0.5;   // - D_eo = -(-1/2) hop
     L.g5 = g5;
+    if (red) {
+        L.red_mode = red->mode; L.red_alg = g->sum_alg; L.red_partial = g->ws_red2;
+        L.red_r = red->r; L.red_num = red->num; L.red_den = red->den;
+    }
     return hop(g, L, what);
+}
+// does a default half-lattice launch of this geometry run the ring / pair kernels, whose epilogues can carry the CG's reductions?
+static bool fused_cg_eo_ok(const hirep_geom *g) {
+    return g->mode == HIREP_LINKS_STORED && g->variant == 0 && !g->slab && g->tune_max_ctas >= 0 && g->dR <= 6;
 }
 
 extern "C" int hirep_Dphi_hat(hirep_geom *g, double m0, void *out_even, const void *in_even, const void *links) {
@@ -924,15 +934,19 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
     // Fused form (plain Wilson Q^2 on the full lattice, when the tile-pair kernel runs it): pass 1 = gamma_5 D p with ||B p||^2 = <p,Ap>
     // accumulated in its epilogue; pass 2 = gamma_5 D (B p) whose epilogue does r -= alpha A p and accumulates ||r||^2 without ever
     // storing A p: 3 spinor passes and 2 launches fewer per iteration (the separate ||Bp||^2 and residual-update kernels are gone).
-    const bool fused = full && !twisted && !clover && !blocks_even && !inv_odd && fused_cg_ok(g);
+    // Even-odd form (Q_hat^2, ring / pair kernels): the same two reductions ride on the second pass of each Q_hat application.
+    const bool plain = !twisted && !clover && !blocks_even && !inv_odd;
+    const bool fused = plain && (full ? fused_cg_ok(g) : fused_cg_eo_ok(g));
     const int nred = k_reduce_workspace_bytes() / (int)(2 * 3 * sizeof(double));   // Acc pairs the partial buffer holds
     if (fused) {
-        if ((rc = workspace(&g->ws_red2, (size_t)k_reduce_workspace_bytes())) || (rc = workspace(&g->ws_full, 2 * g->bytes_spinor_half))) return rc;
+        if ((rc = workspace(&g->ws_red2, (size_t)k_reduce_workspace_bytes())) ||
+            (rc = full ? workspace(&g->ws_full, 2 * g->bytes_spinor_half) : workspace(&g->ws_half2, g->bytes_spinor_half))) return rc;
         if ((e = cudaMemsetAsync(g->ws_red2, 0, (size_t)k_reduce_workspace_bytes(), g->stream)) != cudaSuccess) return cuda_fail(e, what);
     }
     auto fused_pass1 = [&]() -> int {
         const FusedRed fr{1, nullptr, nullptr, nullptr};
-        int rc2 = dphi_full(g, m0, g->ws_full, g->cg_p, links, 1, what, 0.0, &fr);
+        int rc2 = full ? dphi_full(g, m0, g->ws_full, g->cg_p, links, 1, what, 0.0, &fr)
+                       : dphi_hat(g, m0, g->ws_half2, g->cg_p, links, 1, what, &fr);
         if (rc2) return rc2;
         return kern_result(g, k_reduce_final(nred, g->sum_alg, g->ws_red2, d, g->stream), what);
     };
@@ -943,7 +957,8 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
         double *rr_old = d + 2 + 2 * (it & 1), *rr_new_d = d + 2 + 2 * ((it + 1) & 1);
         if (fused) {
             const FusedRed fr{2, g->cg_r, rr_old, d};
-            if ((rc = dphi_full(g, m0, g->cg_Ap, g->ws_full, links, 1, what, 0.0, &fr))) return rc;
+            if ((rc = full ? dphi_full(g, m0, g->cg_Ap, g->ws_full, links, 1, what, 0.0, &fr)
+                           : dphi_hat(g, m0, g->cg_Ap, g->ws_half2, links, 1, what, &fr))) return rc;
             if ((rc = kern_result(g, k_reduce_final(nred, g->sum_alg, g->ws_red2, rr_new_d, g->stream), what))) return rc;
         } else {
             rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, halves, g->sum_alg, 0.0, rr_old, d, nullptr, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, rr_new_d, g->stream), what, 2);

@@ -27,7 +27,8 @@ template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int
     // complex links at d_R = 4, 6 in fp32 (C4: 4.91 -> 4.47 ms; SU(3) SYM 32^4 0.47 -> 0.34 ms; d_R = 5 has only one-row chunks and loses).  In fp64 at d_R >= 4 (half-spinor split over 4 warps: C4 10.7 vs 10.3 ms) and for real
     // links in fp32 the gather-layout kernels are faster; variant 5 forces it anywhere.
     if (hop_full_eligible(L) && (variant == 5 || (variant == 0 && hop_full_default<T, DR, REAL>()))) return launch_hop_full<T, DR, REAL>(g, L, s);
-    if (L.red_mode != 0) return KERR_UNSUPPORTED;   // the fused reductions exist in the tile-pair kernel only
+    // the fused reductions exist in the tile-pair kernel and in the persistent ring / pair kernels (variants 0, 3, 4)
+    if (L.red_mode != 0 && variant != 0 && variant != 3 && variant != 4) return KERR_UNSUPPORTED;
     if (variant == 5) variant = 0;
     if (variant == 0) {
         // one thread per site spills in fp64 from d_R = 5 on; in fp32 at d_R >= 5 only the passes with a diagonal

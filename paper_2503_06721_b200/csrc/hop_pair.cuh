@@ -99,7 +99,9 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
     const bool two = L.nsets == 2;
     const int total_tiles = launch_tiles(g, L) * L.nsets;
     const int gp = blockIdx.x * PAIRS + pair, np = gridDim.x * PAIRS;
-    if (gp >= total_tiles) return;
+    Acc racc{0.0, 0.0, 0.0};                            // fused reduction (HopLaunch::red_mode): this thread's compensated partial sum
+    __shared__ Acc red_scratch[32];
+    if (gp >= total_tiles) { red_finish_cta(L.red_mode, L.red_alg, racc, L.red_partial, red_scratch); return; }
     const int my_tiles = (total_tiles - gp + np - 1) / np;
     const int my_chunks = my_tiles * CPT;
     const uint64_t pol = l2_policy_evict_first();
@@ -303,7 +305,12 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
         }
         if constexpr (SELF) mbar_wait(selffull_s, k & 1);
         if (c_active) {
-            C *out = (C *)(c_set ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
+            const size_t eoff = ((size_t)c_tile * NC) * TILE + lane;
+            C *out = (C *)(c_set ? L.set[1].out : L.set[0].out) + eoff;
+            // fused CG reductions (reduce.cuh): mode 2 updates the residual in place of storing the result
+            C *rp = L.red_mode == 2 ? (C *)L.red_r + (size_t)c_set * ((size_t)g.n_tiles * NC * TILE) + eoff : out;
+            const T al = L.red_mode == 2 ? (T)__ddiv_rn(L.red_num[0], L.red_den[0]) : T(0);
+            double site[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
             for (int c = 0; c < DR; ++c) {
                 C vu = mk<T>(b * up[c].x, b * up[c].y);
@@ -318,15 +325,18 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
                         vl.x = fma(am, sl.y, vl.x); vl.y = fma(-am, sl.x, vl.y);
                     }
                 }
-                st_spinor(out + (size_t)(s * DR + c) * TILE, vu);
-                st_spinor(out + (size_t)((2 + s) * DR + c) * TILE, mk<T>(g5s * vl.x, g5s * vl.y));
+                red_store(L.red_mode, out + (size_t)(s * DR + c) * TILE, rp + (size_t)(s * DR + c) * TILE, al, vu, site[0], site[1]);
+                red_store(L.red_mode, out + (size_t)((2 + s) * DR + c) * TILE, rp + (size_t)((2 + s) * DR + c) * TILE, al,
+                          mk<T>(g5s * vl.x, g5s * vl.y), site[2], site[3]);
             }
+            if (L.red_mode != 0) acc_add(racc, (site[0] + site[1]) + (site[2] + site[3]), L.red_alg);
         }
         if constexpr (SELF) {
             __syncwarp();
             if (lane == 0) mbar_arrive(selfempty_s);
         }
     }
+    red_finish_cta(L.red_mode, L.red_alg, racc, L.red_partial, red_scratch);
 }
 
 template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF, int REP>

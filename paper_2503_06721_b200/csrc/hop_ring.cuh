@@ -22,6 +22,7 @@
 // No CTA-wide barrier anywhere: every warp is its own producer/consumer pipeline (lane 0 issues the bulk copies).
 #pragma once
 #include "hop_small.cuh"
+#include "reduce.cuh"
 
 namespace hirep {
 
@@ -161,7 +162,9 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
     const bool two = L.nsets == 2;
     const int total_tiles = launch_tiles(g, L) * L.nsets;
     const int gw = blockIdx.x * WARPS + warp, nw = gridDim.x * WARPS;
-    if (gw >= total_tiles) return;
+    Acc racc{0.0, 0.0, 0.0};                            // fused reduction (HopLaunch::red_mode): this thread's compensated partial sum
+    __shared__ Acc red_scratch[32];
+    if (gw >= total_tiles) { red_finish_cta(L.red_mode, L.red_alg, racc, L.red_partial, red_scratch); return; }
     const int my_tiles = (total_tiles - gw + nw - 1) / nw;
     const int my_chunks = my_tiles * CPT;
     const uint64_t pol = l2_policy_evict_first();
@@ -299,7 +302,12 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
 
         if constexpr (SELF) mbar_wait(selfbar_s, k & 1);
         if (c_active) {
-            C *out = (C *)(c_set ? L.set[1].out : L.set[0].out) + ((size_t)c_tile * NC) * TILE + lane;
+            const size_t eoff = ((size_t)c_tile * NC) * TILE + lane;
+            C *out = (C *)(c_set ? L.set[1].out : L.set[0].out) + eoff;
+            // fused CG reductions (reduce.cuh): mode 2 updates the residual in place of storing the result
+            C *rp = L.red_mode == 2 ? (C *)L.red_r + (size_t)c_set * ((size_t)g.n_tiles * NC * TILE) + eoff : out;
+            const T al = L.red_mode == 2 ? (T)__ddiv_rn(L.red_num[0], L.red_den[0]) : T(0);
+            double site[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
             for (int s = 0; s < 2; ++s)
 #pragma unroll
@@ -316,11 +324,14 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
                             vl.x = fma(am, sl.y, vl.x); vl.y = fma(-am, sl.x, vl.y);
                         }
                     }
-                    st_spinor(out + (size_t)(s * DR + c) * TILE, vu);
-                    st_spinor(out + (size_t)((2 + s) * DR + c) * TILE, mk<T>(g5s * vl.x, g5s * vl.y));
+                    red_store(L.red_mode, out + (size_t)(s * DR + c) * TILE, rp + (size_t)(s * DR + c) * TILE, al, vu, site[0], site[1]);
+                    red_store(L.red_mode, out + (size_t)((2 + s) * DR + c) * TILE, rp + (size_t)((2 + s) * DR + c) * TILE, al,
+                              mk<T>(g5s * vl.x, g5s * vl.y), site[2], site[3]);
                 }
+            if (L.red_mode != 0) acc_add(racc, (site[0] + site[1]) + (site[2] + site[3]), L.red_alg);
         }
     }
+    red_finish_cta(L.red_mode, L.red_alg, racc, L.red_partial, red_scratch);
 }
 
 // Per-device launch preparation, cached per kernel instantiation AND per device: the opt-in shared-memory size is a

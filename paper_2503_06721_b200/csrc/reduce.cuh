@@ -77,4 +77,32 @@ __device__ inline void cta_merge(Acc &a, int alg, Acc *scratch) {
         for (int w = 1; w < nwarp; ++w) acc_merge(a, scratch[w], alg);
 }
 
+
+// Reductions fused into a stencil epilogue (HopLaunch::red_mode), shared by hop_ring.cuh and hop_pair.cuh; one output element v:
+//   mode 0: out = v                                 mode 1: out = v, (s0, s1) += (re v)^2, (im v)^2
+//   mode 2: r -= alpha v, (s0, s1) += (re r)^2, (im r)^2; v itself is not stored (the CG's A p)
+// s0, s1 are PLAIN per-site chains (<= 8 d_R terms); the site total enters the thread's compensated accumulator once.
+template <typename C, typename T>
+__device__ __forceinline__ void red_store(int mode, C *out, C *rp, T alpha, const C &v, double &s0, double &s1) {
+    if (mode == 2) {
+        C r = *rp;
+        r.x -= alpha * v.x; r.y -= alpha * v.y;
+        *rp = r;
+        s0 = fma((double)r.x, (double)r.x, s0); s1 = fma((double)r.y, (double)r.y, s1);
+    } else {
+        __stcs(out, v);
+        if (mode == 1) { s0 = fma((double)v.x, (double)v.x, s0); s1 = fma((double)v.y, (double)v.y, s1); }
+    }
+}
+// end of a kernel with a fused reduction: EVERY thread of the CTA calls this exactly once (also the ones that leave early)
+__device__ inline void red_finish_cta(int mode, int alg, Acc &a, void *partial, Acc *scratch) {
+    if (mode == 0) return;
+    cta_merge(a, alg, scratch);
+    if (threadIdx.x == 0) {
+        Acc *part = (Acc *)partial;
+        part[2 * blockIdx.x] = a;
+        part[2 * blockIdx.x + 1] = Acc{0.0, 0.0, 0.0};
+    }
+}
+
 }  // namespace hirep
