@@ -558,9 +558,23 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
         ms = timeit(lambda: geom.Cphi(m0, 1.0, x_full, cl, out=y_full))
         by = (cb + 2 * S) * V
         out["Cphi"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3)}
-        ms = timeit(lambda: geom.Dphi_clover(m0, 1.0, x_full, lr, cl, out=y_full), reps=10)
-        by = (cb + 2 * S + lbytes + 3 * S) * V
-        out["Dphi_clover"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3), "launches": 2}
+        # Site-diagonal matrices inside the stencil epilogues ("fused into the second pass") where the ring kernel carries
+        # them (stored links, d_R <= 4 in fp64, <= 6 in fp32), else separate block-apply launches.  Fractions are on the compulsory bytes
+        # of the fused form (every field once); the composed form moves 2S more per block application and is timed beside it.
+        fused_diag = cfg.rep != 1 and d <= (4 if prec == "f64" else 6) or (cfg.rep == 1 and d == 3)
+
+        def both_forms(fn, by, nl_fused, nl_composed):
+            ms = timeit(fn, reps=10)
+            r = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3),
+                 "launches": nl_fused if fused_diag else nl_composed, "fused_epilogue": bool(fused_diag)}
+            if fused_diag:
+                geom.set_tuning(hirep.TUNE_FUSE_DIAG, 0)
+                r["ms_composed"] = round(timeit(fn, reps=10), 4)
+                r["launches_composed"] = nl_composed
+                geom.set_tuning(hirep.TUNE_FUSE_DIAG, 1)
+            return r
+
+        out["Dphi_clover"] = both_forms(lambda: geom.Dphi_clover(m0, 1.0, x_full, lr, cl, out=y_full), (cb + lbytes + 2 * S) * V, 1, 2)   # in is both neighbour data and self term: 2S
         # the Schur form Eq 43 with these blocks: block inverse (once per gauge update and mass), its application, D_hat
         hb = geom.sizes["spinor_half"]
         x_e, y_e = x_full[:hb], y_full[:hb]
@@ -570,10 +584,10 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
         ms = timeit(lambda: geom.Cphi_inv(hirep.ODD, x_e, inv, out=y_e))
         by = (2 * cb + 2 * S) * V / 2                    # full blocks: 8 d^2 complex per site, one parity
         out["Cphi_inv"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3)}
-        ms = timeit(lambda: geom.Dphi_clover_hat(m0, 0.5, x_e, lr, cl, inv, out=y_e), reps=10)
-        by = cm["ops"]["Dphi_eo"][1] * 2 + S * V / 2 + (2 * cb + 2 * S) * V / 2 + (cb + 2 * S) * V / 2
-        out["Dphi_clover_hat"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3), "launches": 4}
-        try:    # even-odd preconditioned CG with the clover term: Q_hat^2 = 2 x (the four launches above), then the CG's linear algebra
+        # two stencil passes (2S + 8K each) + the even input once more as the self term + inverse blocks (2 cb) + clover H, B (cb)
+        by = cm["ops"]["Dphi_eo"][1] * 2 + S * V / 2 + 3 * cb * V / 2
+        out["Dphi_clover_hat"] = both_forms(lambda: geom.Dphi_clover_hat(m0, 0.5, x_e, lr, cl, inv, out=y_e), by, 2, 4)
+        try:    # even-odd preconditioned CG with the clover term: Q_hat^2 = 2 x (the launches above), then the CG's linear algebra
             geom.cg_g5Dphi_clover_hat_sq(m0, 0.5, x_e, lr, cl, inv, 1e-30, 2, out=y_e)
             torch.cuda.synchronize()
             t0 = time.perf_counter()
@@ -582,7 +596,8 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
             ms_it = (time.perf_counter() - t0) * 1e3 / max(it, 1)
             by_it = 2 * by + (1 + 3 + 5) * S * V / 2
             out["cg_g5Dphi_clover_hat_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gbs": round(by_it / ms_it / 1e6, 1),
-                                              "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3), "launches_per_iteration": 13, "relres_after": res}
+                                              "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3), "launches_per_iteration": 9 if fused_diag else 13,
+                                              "relres_after": res}
         except Exception as e:
             out["cg_g5Dphi_clover_hat_sq"] = {"error": str(e)}
         del inv
@@ -593,12 +608,9 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
             ms = timeit(lambda: hirep.hirep_clover_exp_field(geom.handle, m0, 1.0, hirep.ODD, 0, E[nb:].data_ptr(), cl.data_ptr()), reps=3)
             out["clover_exp_field"] = {"ms": round(ms, 3), "note": "one parity; scaling and squaring, 18 block products per site and chirality"}
             Ei = geom.clover_exp_field(m0, 1.0, cl, inverse=True)
-            ms = timeit(lambda: geom.Dphi_blocks(x_full, lr, E, out=y_full), reps=10)
-            by = (2 * cb + 2 * S + lbytes + 3 * S) * V
-            out["Dphi_expclover"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3), "launches": 2}
-            ms = timeit(lambda: geom.Dphi_blocks_hat(x_e, lr, E, Ei[nb:], out=y_e), reps=10)
-            by = cm["ops"]["Dphi_eo"][1] * 2 + S * V / 2 + 2 * (2 * cb + 2 * S) * V / 2
-            out["Dphi_expclover_hat"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3), "launches": 4}
+            out["Dphi_expclover"] = both_forms(lambda: geom.Dphi_blocks(x_full, lr, E, out=y_full), (2 * cb + lbytes + 2 * S) * V, 1, 2)
+            by = cm["ops"]["Dphi_eo"][1] * 2 + S * V / 2 + 4 * cb * V / 2
+            out["Dphi_expclover_hat"] = both_forms(lambda: geom.Dphi_blocks_hat(x_e, lr, E, Ei[nb:], out=y_e), by, 2, 4)
             del E, Ei
         del cl
     # NEXT-4: fermion force of the hopping term (Eq 20-21): both fields and the forward links once, N^2-1 reals per link out

@@ -168,8 +168,12 @@ int hirep_set_kernel_variant(hirep_geom *g, int variant);
  *   HIREP_TUNE_PACE_WINDOW W > 0: full-lattice launches of the tile-pair kernel throttle their leading warp groups -- a group starts
  *                          its round k only when the grid has completed k - W rounds' worth of tile pairs -- so that link blocks and
  *                          spinor tiles gathered from other tile pairs are still in L2 (C4: DRAM reads -16..-26 %; time +-5 %, so
- *                          off by default: 0).  Needs all CTAs of the launch co-resident (the library's grids are <= one CTA per SM). */
-enum { HIREP_TUNE_MAX_CTAS = 1, HIREP_TUNE_SUM_ALGORITHM = 2, HIREP_TUNE_PACE_WINDOW = 3 };
+ *                          off by default: 0).  Needs all CTAs of the launch co-resident (the library's grids are <= one CTA per SM).
+ *   HIREP_TUNE_FUSE_DIAG   1 (default): the operators with site-diagonal matrices (clover, exponential clover, general blocks; Eq 43,
+ *                          47, 50) apply them inside the stencil epilogues wherever that kernel is instantiated (stored links,
+ *                          d_R <= 4 in fp64, d_R <= 6 in fp32): Dphi_clover / Dphi_blocks 1 launch, the Schur forms 2; 0: separate
+ *                          block-apply launches (2 resp. 4).  The two forms sum in different orders: results agree to rounding. */
+enum { HIREP_TUNE_MAX_CTAS = 1, HIREP_TUNE_SUM_ALGORITHM = 2, HIREP_TUNE_PACE_WINDOW = 3, HIREP_TUNE_FUSE_DIAG = 4 };
 int hirep_set_tuning(hirep_geom *g, int key, int value);
 /* number of kernels this library has launched on behalf of g since creation (bench.py's gpu_launches) */
 long hirep_launch_count(const hirep_geom *g);

@@ -23,7 +23,7 @@ struct hirep_geom {
     Geo geo;
     int N, rep, prec, dR, real;
     int mode, variant;
-    int tune_max_ctas, sum_alg, tune_pace;   // hirep_set_tuning
+    int tune_max_ctas, sum_alg, tune_pace, tune_fuse_diag;   // hirep_set_tuning
     int slab, region;             // hirep_geom_create_slab / hirep_set_region
     cudaStream_t stream;
     void *ws_half, *ws_half2, *ws_half3, *ws_full;   // workspace spinors (lazy)
@@ -110,7 +110,7 @@ extern "C" int hirep_geom_create(int T, int L, int N_g, int rep, int prec, hirep
     g->geo.n_tiles = (g->geo.Nh + TILE - 1) / TILE;
     g->geo.bc[0] = -1; g->geo.bc[1] = g->geo.bc[2] = g->geo.bc[3] = 1;
     g->geo.t0 = 0; g->geo.Tg = T;
-    g->tune_max_ctas = 0; g->sum_alg = 2;
+    g->tune_max_ctas = 0; g->sum_alg = 2; g->tune_fuse_diag = 1;
     g->N = N_g; g->rep = rep; g->prec = prec; g->dR = dR; g->real = (rep == HIREP_ADJ);
     const size_t w = prec == HIREP_F64 ? 8 : 4;
     g->bytes_spinor_half = (size_t)g->geo.n_tiles * 4 * dR * TILE * 2 * w;
@@ -221,6 +221,10 @@ extern "C" int hirep_set_tuning(hirep_geom *g, int key, int value) {
     case HIREP_TUNE_PACE_WINDOW:
         if (value < 0 || value > 64) return fail(HIREP_EINVAL, "hirep_set_tuning: pace window %d (0 = off, 1..64 rounds)", value);
         g->tune_pace = value;
+        return HIREP_OK;
+    case HIREP_TUNE_FUSE_DIAG:
+        if (value != 0 && value != 1) return fail(HIREP_EINVAL, "hirep_set_tuning: fuse-diagonal switch %d (0 or 1)", value);
+        g->tune_fuse_diag = value;
         return HIREP_OK;
     }
     return fail(HIREP_EINVAL, "hirep_set_tuning: unknown key %d", key);
@@ -584,10 +588,40 @@ extern "C" int hirep_Cphi(hirep_geom *g, double m0, double csw, void *out_full, 
     if (out_full == in_full) return fail(HIREP_EINVAL, "hirep_Cphi: out aliases in");
     return kern_result(g, k_cphi(g->prec, g->dR, 2 * g->geo.n_tiles, 4.0 + m0, csw, clover, in_full, out_full, g->stream), "hirep_Cphi");
 }
-// out = [gamma_5] (Cphi in - 1/2 hop(in)): Cphi writes out, the hopping pass accumulates onto it in place (every site's own
+// Are the site-diagonal matrices applied inside the stencil epilogue (one launch per stencil pass, "fused into the second pass",
+// SURVEY 8(f) row 2) or by separate block-apply launches?  Fused where the thread-per-site ring kernel is instantiated
+// (k_hop_diag_supported) unless hirep_set_tuning(HIREP_TUNE_FUSE_DIAG, 0); slab geometries keep the composed form.
+static bool fuse_diag(const hirep_geom *g) {
+    return g->tune_fuse_diag && !g->slab && k_hop_diag_supported(g->prec == HIREP_F64 ? 0 : 1, g->dR, g->real, g->mode, g->variant);
+}
+// one stencil pass over parity p_out with the diagonal matrices `diag` of that parity in its epilogue (kernels.h DIAG_*)
+static int hop_diag_half(hirep_geom *g, int diag_mode, double a, double csw, double b, int g5, void *out, const void *in, const void *self,
+                         const void *links, const void *diag, int p_out, const char *what) {
+    HopLaunch L{};
+    L.nsets = 1;
+    L.set[0] = HopSet{in, out, self, links_parity(g, links, p_out), p_out, diag};
+    L.a = a; L.b = b; L.g5 = g5; L.diag_mode = diag_mode; L.diag_csw = csw;
+    return hop(g, L, what);
+}
+// the same over both parities in one launch: out = [gamma_5] (Diag in + b hop(in)); diag_full = both parities, even first
+static int hop_diag_full(hirep_geom *g, int diag_mode, double a, double csw, int g5, void *out_full, const void *in_full, const void *links,
+                         const void *diag_full, size_t diag_parity_bytes, const char *what) {
+    const size_t hb = g->bytes_spinor_half;
+    const char *in_e = (const char *)in_full, *in_o = in_e + hb;
+    char *out_e = (char *)out_full, *out_o = out_e + hb;
+    HopLaunch L{};
+    L.nsets = 2;
+    L.set[0] = HopSet{in_o, out_e, in_e, links_parity(g, links, 0), 0, diag_full};
+    L.set[1] = HopSet{in_e, out_o, in_o, links_parity(g, links, 1), 1, (const char *)diag_full + diag_parity_bytes};
+    L.a = a; L.b = -0.5; L.g5 = g5; L.diag_mode = diag_mode; L.diag_csw = csw;
+    return hop(g, L, what);
+}
+// out = [gamma_5] (Cphi in - 1/2 hop(in)).  Fused: one stencil launch whose epilogue applies (4+m) + c_sw A to the site's own
+// input.  Composed: Cphi writes out, the hopping pass accumulates onto it in place (every site's own
 // value is read before it is written, by the same tile); gamma_5 commutes with the diagonal blocks
 static int dphi_clover(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *links, const void *clover, int g5,
                        const char *what) {
+    if (fuse_diag(g)) return hop_diag_full(g, DIAG_HB, 4.0 + m0, csw, g5, out_full, in_full, links, clover, clover_bytes(g) / 2, what);
     int rc = kern_result(g, k_cphi(g->prec, g->dR, 2 * g->geo.n_tiles, 4.0 + m0, csw, clover, in_full, out_full, g->stream), what);
     if (rc) return rc;
     const size_t hb = g->bytes_spinor_half;
@@ -641,6 +675,11 @@ extern "C" int hirep_Dphi_clover_hat(hirep_geom *g, double m0, double csw, void 
     if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_Dphi_clover_hat: out aliases in");
     int rc = workspace(&g->ws_half, g->bytes_spinor_half);
     if (rc) return rc;
+    if (fuse_diag(g)) {   // two launches: D_oo^-1 in the epilogue of the D_oe pass, D_ee in the epilogue of the D_eo pass
+        rc = hop_diag_half(g, DIAG_POST, 0.0, 0.0, -0.5, 0, g->ws_half, in_even, nullptr, links, inv_odd, 1, "hirep_Dphi_clover_hat (D_oo^-1 D_oe pass)");
+        if (rc) return rc;
+        return hop_diag_half(g, DIAG_HB, 4.0 + m0, csw, +0.5, 0, out_even, g->ws_half, in_even, links, clover, 0, "hirep_Dphi_clover_hat (D_ee - D_eo pass)");
+    }
     rc = workspace(&g->ws_half2, g->bytes_spinor_half);
     if (rc) return rc;
     rc = offdiag(g, g->ws_half, in_even, links, 1, "hirep_Dphi_clover_hat (D_oe pass)");
@@ -672,6 +711,7 @@ extern "C" int hirep_clover_exp_field(hirep_geom *g, double m0, double csw, int 
 }
 // out = [gamma_5] (blocks in - 1/2 hop(in)); gamma_5 commutes with the chirality blocks
 static int dphi_blocks(hirep_geom *g, void *out_full, const void *in_full, const void *links, const void *blocks_full, int g5, const char *what) {
+    if (fuse_diag(g)) return hop_diag_full(g, DIAG_PRE, 0.0, 0.0, g5, out_full, in_full, links, blocks_full, clover_bytes(g), what);
     int rc = kern_result(g, k_cblock(g->prec, g->dR, 2 * g->geo.n_tiles, blocks_full, in_full, out_full, g->stream), what);
     if (rc) return rc;
     const size_t hb = g->bytes_spinor_half;
@@ -706,6 +746,11 @@ extern "C" int hirep_Dphi_blocks_hat(hirep_geom *g, void *out_even, const void *
     if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_Dphi_blocks_hat: out aliases in");
     int rc = workspace(&g->ws_half, g->bytes_spinor_half);
     if (rc) return rc;
+    if (fuse_diag(g)) {
+        rc = hop_diag_half(g, DIAG_POST, 0.0, 0.0, -0.5, 0, g->ws_half, in_even, nullptr, links, inv_blocks_odd, 1, "hirep_Dphi_blocks_hat (D_oo^-1 D_oe pass)");
+        if (rc) return rc;
+        return hop_diag_half(g, DIAG_PRE, 0.0, 0.0, +0.5, 0, out_even, g->ws_half, in_even, links, blocks_even, 0, "hirep_Dphi_blocks_hat (D_ee - D_eo pass)");
+    }
     rc = workspace(&g->ws_half2, g->bytes_spinor_half);
     if (rc) return rc;
     rc = offdiag(g, g->ws_half, in_even, links, 1, "hirep_Dphi_blocks_hat (D_oe pass)");
@@ -727,6 +772,12 @@ static int blocks_hat(hirep_geom *g, double m0, double csw, void *out_even, cons
                       const void *blocks_even, const void *inv_odd, int g5, const char *what) {
     int rc = workspace(&g->ws_half, g->bytes_spinor_half);
     if (rc) return rc;
+    if (fuse_diag(g)) {
+        rc = hop_diag_half(g, DIAG_POST, 0.0, 0.0, -0.5, 0, g->ws_half, in_even, nullptr, links, inv_odd, 1, what);
+        if (rc) return rc;
+        return clover ? hop_diag_half(g, DIAG_HB, 4.0 + m0, csw, +0.5, g5, out_even, g->ws_half, in_even, links, clover, 0, what)
+                      : hop_diag_half(g, DIAG_PRE, 0.0, 0.0, +0.5, g5, out_even, g->ws_half, in_even, links, blocks_even, 0, what);
+    }
     rc = workspace(&g->ws_half2, g->bytes_spinor_half);
     if (rc) return rc;
     rc = offdiag(g, g->ws_half, in_even, links, 1, what);

@@ -20,7 +20,18 @@
 
 namespace hirep {
 
+// Launches with a site-diagonal matrix term in the epilogue (HopLaunch::diag_mode): the thread-per-site ring kernel, where one
+// thread holds the whole spinor of its site -- d_R <= 4 in fp64, d_R <= 6 in fp32 (beyond: the caller applies the blocks in
+// separate launches).  k_hop_diag_supported (hop_f64.cu) states the same rule to api.cu.
+template <typename T, int DR> constexpr bool hop_diag_ring() { return sizeof(T) == 8 ? DR <= 4 : DR <= 6; }
+
 template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
+    if (L.diag_mode != DIAG_NONE) {
+        if constexpr (hop_diag_ring<T, DR>()) {
+            if (variant == 0 || variant == 3) return launch_hop_ring<T, DR, REAL>(g, L, s);
+        }
+        return KERR_UNSUPPORTED;
+    }
     // full-lattice launches whose diagonal term is the other parity's input: every link crosses the SM once (hop_full.cuh)
     // Default where it wins on B200 (profiles/r02_summary.md): complex links at d_R <= 3 in both precisions (C1, C2: 0.26 -> 0.20 ms at C2 fp64,
     // 0.130 -> 0.119 ms in fp32, in bursts; on par under a sustained power-capped load), the real SU(2) adjoint in fp64 (C3: 0.98 -> 0.89 ms) and
@@ -50,7 +61,7 @@ template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int
 // shapes from a sweep on 32x24^3, profiles/r01b_summary.md),
 // variant 1 = the direct-load row-group kernel of round 1 (hop_large.cuh), kept for comparison
 template <typename T, int DR, bool REAL, int R, int TP> int hop_large_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
-    if (L.red_mode != 0) return KERR_UNSUPPORTED;
+    if (L.red_mode != 0 || L.diag_mode != DIAG_NONE) return KERR_UNSUPPORTED;
     if (variant == 0) return launch_hop_rows<T, DR, REAL, R, TP>(g, L, s);
     if (variant == 1 && L.tile_end == 0) return launch_hop_large<T, DR, REAL, R>(g, L, s);
     return KERR_UNSUPPORTED;
@@ -64,7 +75,7 @@ template <typename T, int N, int REP> int hop_rebuild(const Geo &g, int variant,
     return launch_hop_pair<T, M::DR, M::REAL, N, REP>(g, L, s);
 }
 template <typename T> int hop_rebuild_by_config(const Geo &g, int N, int rep, int variant, const HopLaunch &L, cudaStream_t s) {
-    if (L.red_mode != 0) return KERR_UNSUPPORTED;
+    if (L.red_mode != 0 || L.diag_mode != DIAG_NONE) return KERR_UNSUPPORTED;
     switch (rep * 10 + N) {
     case 2: return hop_rebuild<T, 2, 0>(g, variant, L, s);    // FUND
     case 3: return hop_rebuild<T, 3, 0>(g, variant, L, s);

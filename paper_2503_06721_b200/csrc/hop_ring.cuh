@@ -92,12 +92,20 @@ template <typename K> inline int launch_pdl(K kern, int grid, int block, size_t 
 }
 
 // ring geometry for one instantiation; CHUNK = RPC rows of the link block of one direction of one tile
-template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC, bool SELF> struct RingCfg {
+template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC, bool SELF, int DIAG = DIAG_NONE> struct RingCfg {
     using E = link_elem<T, REAL>;
     static constexpr int NE = DR * DR;
     static constexpr int CPD = DR / RPC;                            // chunks per direction
     static constexpr uint32_t CHUNK = RPC * DR * TILE * sizeof(E);  // RPC rows of one link matrix, 32 lanes
     static_assert(DR % RPC == 0, "rows per chunk must divide d_R");
+    // site-diagonal matrices (kernels.h DIAG_*): NENT complex entries per site, [entry][lane], streamed through the ring slots
+    // after the eight directions of the tile in pieces of DE entries (the whole entries that fit a slot), NDC pieces per tile
+    static constexpr int NENT = DIAG == DIAG_NONE ? 0 : DIAG == DIAG_HB ? 4 * NE : 8 * NE;
+    static constexpr int DE = (int)(CHUNK / (TILE * sizeof(cplx<T>)));
+    static constexpr int NDC = DIAG == DIAG_NONE ? 0 : (NENT + DE - 1) / DE;
+    static_assert(DIAG == DIAG_NONE || DE >= 1, "a ring slot must hold at least one entry of the diagonal matrices");
+    static_assert(DIAG == DIAG_NONE || DIAG == DIAG_POST || SELF, "DIAG_HB / DIAG_PRE act on the self spinor");
+    static_assert(DIAG != DIAG_POST || !SELF, "DIAG_POST has no self term");
     static constexpr uint32_t SELF_BYTES = SELF ? 4 * DR * TILE * sizeof(cplx<T>) : 0;   // one tile of the spinor
     static constexpr size_t RING_BYTES = (size_t)WARPS * STAGES * CHUNK;
     static constexpr size_t BARS_OFF = RING_BYTES + (size_t)WARPS * SELF_BYTES;
@@ -132,12 +140,13 @@ template <typename T, int DR, bool REAL, bool SELF> struct RingPick {
     static_assert(STAGES >= 2, "ring needs at least two stages");
 };
 
-template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC, bool SELF>
+template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC, bool SELF, int DIAG = DIAG_NONE>
 __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, const HopLaunch L) {
     using C = cplx<T>;
     using E = link_elem<T, REAL>;
-    using Cfg = RingCfg<T, DR, REAL, WARPS, STAGES, RPC, SELF>;
-    constexpr int NC = 4 * DR, CPD = Cfg::CPD, CPT = 8 * CPD;   // chunks per direction / per tile
+    using Cfg = RingCfg<T, DR, REAL, WARPS, STAGES, RPC, SELF, DIAG>;
+    constexpr int NC = 4 * DR, CPD = Cfg::CPD, CPT = 8 * CPD + Cfg::NDC;   // chunks per direction / per tile (links, then diagonal matrices)
+    constexpr int NENT = Cfg::NENT, DE = Cfg::DE;
     constexpr int CE = RPC * DR * TILE;                         // link elements per chunk
     constexpr bool IL = !(sizeof(T) == 4 && DR >= 5);           // hop order (common.cuh): the 168-register fp32 kernels
                                                                 // at d_R = 5, 6 lose 13 % with the interleaved walk
@@ -183,8 +192,19 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
         int set_, tile_;
         locate(kq, set_, tile_);
         // chunk c of the tile = step c / CPD of the walk -> direction dir_of<IL>(step) of the gather block
-        const int c = qi - kq * CPT, step = c / CPD, chunk = dir_of<IL>(step) * CPD + (c - step * CPD);
-        const E *src = (const E *)(set_ ? L.set[1].links : L.set[0].links) + ((size_t)tile_ * CPT + chunk) * CE;
+        const int c = qi - kq * CPT;
+        if constexpr (DIAG != DIAG_NONE) {
+            if (c >= 8 * CPD) {   // piece c - 8 CPD of the tile's diagonal matrices: DE entries (the last piece: what is left)
+                const int e0 = (c - 8 * CPD) * DE;
+                const uint32_t bytes = (uint32_t)((NENT - e0 < DE ? NENT - e0 : DE) * TILE * sizeof(C));
+                const C *src = (const C *)(set_ ? L.set[1].diag : L.set[0].diag) + ((size_t)tile_ * NENT + e0) * TILE;
+                mbar_expect_tx(bars_s + 8 * slot, bytes);
+                bulk_g2s(ring_s + slot * Cfg::CHUNK, src, bytes, bars_s + 8 * slot, pol);
+                return;
+            }
+        }
+        const int step = c / CPD, chunk = dir_of<IL>(step) * CPD + (c - step * CPD);
+        const E *src = (const E *)(set_ ? L.set[1].links : L.set[0].links) + ((size_t)tile_ * (8 * CPD) + chunk) * CE;
         mbar_expect_tx(bars_s + 8 * slot, Cfg::CHUNK);
         bulk_g2s(ring_s + slot * Cfg::CHUNK, src, Cfg::CHUNK, bars_s + 8 * slot, pol);
     };
@@ -301,6 +321,70 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
         });
 
         if constexpr (SELF) mbar_wait(selfbar_s, k & 1);
+        if constexpr (DIAG != DIAG_NONE) {
+            // Site-diagonal term (kernels.h DIAG_*), chirality by chirality: c = 0 is spin 0, 1 (the `up` accumulators), c = 1 is spin
+            // 2, 3 (`lo`).  v = the vector the matrix multiplies (self, or the scaled hop sum), o = the result rows; the matrix
+            // entries arrive through the ring in storage order, every lane reads its own site's column of the slot.
+            const T csw = (T)L.diag_csw;
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+                C v[2 * DR], o[2 * DR];
+#pragma unroll
+                for (int s = 0; s < 2; ++s)
+#pragma unroll
+                    for (int j = 0; j < DR; ++j) {
+                        const C h = c == 0 ? up[s][j] : lo[s][j];
+                        const C bh = mk<T>(b * h.x, b * h.y);
+                        if constexpr (DIAG == DIAG_POST) {
+                            v[s * DR + j] = bh;
+                            o[s * DR + j] = mk<T>(0, 0);
+                        } else {
+                            const C sv = selfbuf[((2 * c + s) * DR + j) * TILE + lane];
+                            if constexpr (DIAG == DIAG_HB) {   // (a + csw A) self: the unit term now, A on csw * self below
+                                o[s * DR + j] = mk<T>(fma(a, sv.x, bh.x), fma(a, sv.y, bh.y));
+                                v[s * DR + j] = mk<T>(csw * sv.x, csw * sv.y);
+                            } else {
+                                o[s * DR + j] = bh;
+                                v[s * DR + j] = sv;
+                            }
+                        }
+                    }
+#pragma unroll
+                for (int e = 0; e < NENT / 2; ++e) {
+                    const int ge = c * (NENT / 2) + e;   // entry of the site's matrices, storage order
+                    if (ge % DE == 0) mbar_wait(bars_s + 8 * slot, phase);
+                    const C m = reinterpret_cast<const C *>(smem_raw + (size_t)warp * STAGES * Cfg::CHUNK + (size_t)slot * Cfg::CHUNK)[(ge % DE) * TILE + lane];
+                    if constexpr (DIAG == DIAG_HB) {
+                        const int i = (e % (DR * DR)) / DR, j = e % DR;
+                        if (e < DR * DR) {   // H: +H on the upper spin row, -H on the lower
+                            mac<T>(o[i], m, v[j]);
+                            mac<T>(o[DR + i], mk<T>(-m.x, -m.y), v[DR + j]);
+                        } else {             // B: B psi_1 into row i of spin 0, B^+ psi_0 into row j of spin 1
+                            mac<T>(o[i], m, v[DR + j]);
+                            mac<T>(o[DR + j], mk<T>(m.x, -m.y), v[i]);
+                        }
+                    } else {
+                        mac<T>(o[e / (2 * DR)], m, v[e % (2 * DR)]);
+                    }
+                    if (ge % DE == DE - 1 || ge == NENT - 1) {
+                        __syncwarp();
+                        if (lane == 0 && q + STAGES < my_chunks) {
+                            fence_proxy_async();
+                            issue(q + STAGES, slot);
+                        }
+                        ++q;
+                        if (++slot == STAGES) { slot = 0; phase ^= 1; }
+                    }
+                }
+#pragma unroll
+                for (int s = 0; s < 2; ++s)
+#pragma unroll
+                    for (int j = 0; j < DR; ++j) {
+                        if (c == 0) up[s][j] = o[s * DR + j];
+                        else lo[s][j] = o[s * DR + j];
+                    }
+            }
+        }
         if (c_active) {
             const size_t eoff = ((size_t)c_tile * NC) * TILE + lane;
             C *out = (C *)(c_set ? L.set[1].out : L.set[0].out) + eoff;
@@ -312,9 +396,10 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
             for (int s = 0; s < 2; ++s)
 #pragma unroll
                 for (int c = 0; c < DR; ++c) {
-                    C vu = mk<T>(b * up[s][c].x, b * up[s][c].y);
-                    C vl = mk<T>(b * lo[s][c].x, b * lo[s][c].y);
-                    if constexpr (SELF) {
+                    C vu, vl;
+                    if constexpr (DIAG != DIAG_NONE) { vu = up[s][c]; vl = lo[s][c]; }
+                    else { vu = mk<T>(b * up[s][c].x, b * up[s][c].y); vl = mk<T>(b * lo[s][c].x, b * lo[s][c].y); }
+                    if constexpr (SELF && DIAG == DIAG_NONE) {
                         const C su = selfbuf[(s * DR + c) * TILE + lane];
                         const C sl = selfbuf[((2 + s) * DR + c) * TILE + lane];
                         vu.x = fma(a, su.x, vu.x); vu.y = fma(a, su.y, vu.y);
@@ -360,10 +445,10 @@ inline int ring_grid(int n_sm, int max_ctas, int total_tiles, int tiles_per_cta)
     return grid;
 }
 
-template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC, bool SELF>
+template <typename T, int DR, bool REAL, int WARPS, int STAGES, int RPC, bool SELF, int DIAG = DIAG_NONE>
 int launch_hop_ring_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
-    using Cfg = RingCfg<T, DR, REAL, WARPS, STAGES, RPC, SELF>;
-    auto kern = hop_ring_kernel<T, DR, REAL, WARPS, STAGES, RPC, SELF>;
+    using Cfg = RingCfg<T, DR, REAL, WARPS, STAGES, RPC, SELF, DIAG>;
+    auto kern = hop_ring_kernel<T, DR, REAL, WARPS, STAGES, RPC, SELF, DIAG>;
     static DevCache cache{};
     int n_sm = 0;
     if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
@@ -375,6 +460,18 @@ int launch_hop_ring_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
 // a pass with a diagonal term (a != 0 and a self spinor) uses the SELF instantiation, a pure hop the plain one
 template <typename T, int DR, bool REAL> int launch_hop_ring(const Geo &g, const HopLaunch &L, cudaStream_t s) {
     const bool self = (L.a != 0.0) && L.set[0].self != nullptr;
+    if (L.diag_mode != DIAG_NONE) {   // site-diagonal matrices in the epilogue: the self term is the matrix term
+        if (L.am != 0.0 || !L.set[0].diag || (L.nsets == 2 && !L.set[1].diag)) return KERR_UNSUPPORTED;
+        if (L.diag_mode == DIAG_POST) {
+            using P = RingPick<T, DR, REAL, false>;
+            return launch_hop_ring_cfg<T, DR, REAL, P::WARPS, P::STAGES, P::RPC, false, DIAG_POST>(g, L, s);
+        }
+        if (!L.set[0].self) return KERR_UNSUPPORTED;
+        using P = RingPick<T, DR, REAL, true>;
+        if (L.diag_mode == DIAG_HB) return launch_hop_ring_cfg<T, DR, REAL, P::WARPS, P::STAGES, P::RPC, true, DIAG_HB>(g, L, s);
+        if (L.diag_mode == DIAG_PRE) return launch_hop_ring_cfg<T, DR, REAL, P::WARPS, P::STAGES, P::RPC, true, DIAG_PRE>(g, L, s);
+        return KERR_UNSUPPORTED;
+    }
     if (self) {
         using P = RingPick<T, DR, REAL, true>;
         return launch_hop_ring_cfg<T, DR, REAL, P::WARPS, P::STAGES, P::RPC, true>(g, L, s);

@@ -15,13 +15,22 @@ struct HopSet {
     const void *self;   // spinor on parity p_out (may be null when a == 0)
     const void *links;  // gather block of parity p_out: represented (stored) or fundamental (rebuild)
     int p_out;
+    const void *diag;   // site-diagonal matrices of parity p_out when HopLaunch::diag_mode != 0 (tile-major, [tile][entry][lane] complex)
 };
+// Site-diagonal term applied inside the stencil epilogue (Eq 43 / 47 / 50: "fused into the second pass").
+// The matrices ride through the same bulk-copy ring as the links, after the eight directions of a tile.
+//   DIAG_HB   : out = (a + csw A) self + b hop(in),  A_c = [[H, B], [B^+, -H]] from the clover field (4 d_R^2 complex per site)
+//   DIAG_PRE  : out = M self + b hop(in),            M = full (2 d_R)^2 chirality blocks (8 d_R^2 complex per site)
+//   DIAG_POST : out = M (b hop(in))                  (D_oo^-1 D_oe of the Schur form; no self)
+enum { DIAG_NONE = 0, DIAG_HB = 1, DIAG_PRE = 2, DIAG_POST = 3 };
 struct HopLaunch {
     HopSet set[2];
     int nsets;          // 1 = half lattice, 2 = both parities in one launch
     double a, b;
     double am;          // twisted mass mu: the diagonal term is (a + i am gamma_5) self (Eq 51); 0 = plain Wilson
     int g5;             // multiply the result by gamma_5 = diag(1,1,-1,-1)
+    int diag_mode;      // DIAG_*: site-diagonal matrices HopSet::diag applied in the epilogue (ring / pair kernels, stored links)
+    double diag_csw;    // DIAG_HB: c_sw (a is the (4+m) of Eq 47)
     int max_ctas;       // cap on the persistent grid (0 = one CTA per SM); tests use it to force many tiles per warp
     int tile_begin, tile_end;   // tiles [begin, end) of each parity to compute (slab regions: interior / boundary); end = 0: all
     // reductions fused into the epilogue of the tile-pair kernel (hop_full.cuh; the CG on Q^2):
@@ -51,6 +60,9 @@ int k_links_rep_export(const Geo &g, int prec, int dR, int real, void *canon, co
 int k_links_to_rep(const Geo &g, int prec, int N, int rep, void *native_rep, const void *native_fund, cudaStream_t s);
 // variant: 0 default; see hop_dispatch.cu.  mode: 0 stored represented links, 1 rebuild from fundamental (N, rep).
 int k_hop(const Geo &g, int prec, int N, int rep, int mode, int variant, const HopLaunch &L, cudaStream_t s);
+// whether a launch with HopLaunch::diag_mode != 0 is instantiated for this configuration (else the caller composes the
+// operator from separate block-apply launches)
+bool k_hop_diag_supported(int prec, int dR, int real, int mode, int variant);
 // linalg.cu: spinor linear algebra / reductions on native buffers (n = complex elements incl. padding; halves = 1 | 2)
 int k_reduce_workspace_bytes();
 // second stage of a reduction whose per-CTA partials a stencil launch has written (HopLaunch::red_partial): out_dev[0..1]

@@ -20,7 +20,7 @@ F64, F32 = 0, 1
 EVEN, ODD, FULL = 0, 1, 2
 LINKS_STORED, LINKS_REBUILD = 0, 1
 OP_DPHI, OP_DPHI_EO, OP_DPHI_OE, OP_DPHI_HAT, OP_G5DPHI_SQ = 0, 1, 2, 3, 4
-TUNE_MAX_CTAS, TUNE_SUM_ALGORITHM, TUNE_PACE_WINDOW = 1, 2, 3
+TUNE_MAX_CTAS, TUNE_SUM_ALGORITHM, TUNE_PACE_WINDOW, TUNE_FUSE_DIAG = 1, 2, 3, 4
 REGION_ALL, REGION_OWNED, REGION_INTERIOR, REGION_BOUNDARY = 0, 1, 2, 3
 STATIC_SCRATCH_BYTES = 16 << 20   # HIREP_STATIC_SCRATCH_BYTES
 OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM, EBREAKDOWN = 0, -1, -2, -3, -4, -5
