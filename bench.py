@@ -559,9 +559,9 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
         by = (cb + 2 * S) * V
         out["Cphi"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3)}
         # Site-diagonal matrices inside the stencil epilogues ("fused into the second pass") where the ring kernel carries
-        # them (stored links, d_R <= 4 in fp64, <= 6 in fp32), else separate block-apply launches.  Fractions are on the compulsory bytes
+        # them (stored links, d_R <= 6: ring / pair kernels), else separate block-apply launches.  Fractions are on the compulsory bytes
         # of the fused form (every field once); the composed form moves 2S more per block application and is timed beside it.
-        fused_diag = cfg.rep != 1 and d <= (4 if prec == "f64" else 6) or (cfg.rep == 1 and d == 3)
+        fused_diag = d <= 6
 
         def both_forms(fn, by, nl_fused, nl_composed):
             ms = timeit(fn, reps=10)

@@ -171,7 +171,7 @@ int hirep_set_kernel_variant(hirep_geom *g, int variant);
  *                          off by default: 0).  Needs all CTAs of the launch co-resident (the library's grids are <= one CTA per SM).
  *   HIREP_TUNE_FUSE_DIAG   1 (default): the operators with site-diagonal matrices (clover, exponential clover, general blocks; Eq 43,
  *                          47, 50) apply them inside the stencil epilogues wherever that kernel is instantiated (stored links,
- *                          d_R <= 4 in fp64, d_R <= 6 in fp32): Dphi_clover / Dphi_blocks 1 launch, the Schur forms 2; 0: separate
+ *                          d_R <= 6, kernel variants 0, 3, 4): Dphi_clover / Dphi_blocks 1 launch, the Schur forms 2; 0: separate
  *                          block-apply launches (2 resp. 4).  The two forms sum in different orders: results agree to rounding. */
 enum { HIREP_TUNE_MAX_CTAS = 1, HIREP_TUNE_SUM_ALGORITHM = 2, HIREP_TUNE_PACE_WINDOW = 3, HIREP_TUNE_FUSE_DIAG = 4 };
 int hirep_set_tuning(hirep_geom *g, int key, int value);

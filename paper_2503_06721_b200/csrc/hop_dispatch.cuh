@@ -20,15 +20,22 @@
 
 namespace hirep {
 
-// Launches with a site-diagonal matrix term in the epilogue (HopLaunch::diag_mode): the thread-per-site ring kernel, where one
-// thread holds the whole spinor of its site -- d_R <= 4 in fp64, d_R <= 6 in fp32 (beyond: the caller applies the blocks in
-// separate launches).  k_hop_diag_supported (hop_f64.cu) states the same rule to api.cu.
+// Launches with a site-diagonal matrix term in the epilogue (HopLaunch::diag_mode), stored links, d_R <= 6: the thread-per-site
+// ring kernel where one thread can hold the whole spinor of its site (d_R <= 4 in fp64, d_R <= 6 in fp32; variant 3), the pair
+// kernel at d_R = 5, 6 (variant 4; default in fp64).  Beyond d_R = 6 the caller applies the blocks in separate launches.
+// k_hop_diag_supported (hop_f64.cu) states the same rule to api.cu.
 template <typename T, int DR> constexpr bool hop_diag_ring() { return sizeof(T) == 8 ? DR <= 4 : DR <= 6; }
+template <typename T, int DR> constexpr bool hop_diag_pair() { return DR >= 5 && DR <= 6; }
+template <typename T, int DR> constexpr bool hop_diag_pair_default() { return DR >= 5 && DR <= 6 && sizeof(T) == 8; }
 
 template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
     if (L.diag_mode != DIAG_NONE) {
+        if (variant == 0) variant = hop_diag_pair_default<T, DR>() ? 4 : 3;
         if constexpr (hop_diag_ring<T, DR>()) {
-            if (variant == 0 || variant == 3) return launch_hop_ring<T, DR, REAL>(g, L, s);
+            if (variant == 3) return launch_hop_ring<T, DR, REAL>(g, L, s);
+        }
+        if constexpr (hop_diag_pair<T, DR>()) {
+            if (variant == 4) return launch_hop_pair_diag<T, DR, REAL>(g, L, s);
         }
         return KERR_UNSUPPORTED;
     }

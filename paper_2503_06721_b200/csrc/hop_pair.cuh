@@ -47,9 +47,12 @@ template <int D> __device__ __forceinline__ int hop_sign_dir(const Geo &g, int p
     return (fwd ? (c == g.L - 1) : (c == 0)) ? g.bc[mu] : 1;
 }
 
-template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF, int REP = 0> struct PairCfg {
+template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF, int REP = 0, int DIAG = DIAG_NONE> struct PairCfg {
     using E = link_elem<T, REAL>;                                   // element type of R
     static constexpr bool REBUILD = NF > 0;
+    static_assert(DIAG == DIAG_NONE || !REBUILD, "the site-diagonal epilogue exists for stored links only");
+    static_assert(DIAG == DIAG_NONE || DIAG == DIAG_POST || SELF, "DIAG_HB / DIAG_PRE act on the self spinor");
+    static_assert(DIAG != DIAG_POST || !SELF, "DIAG_POST has no self term");
     static constexpr bool SHARED = REBUILD && REP != 0;             // the pair rebuilds R(W) once, into shared memory
     static constexpr int CPD = REBUILD ? 1 : DR / RPC;              // chunks per direction
     static constexpr uint32_t CHUNK = REBUILD ? NF * NF * TILE * sizeof(cplx<T>) : RPC * DR * TILE * sizeof(E);
@@ -58,19 +61,24 @@ template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SE
     static constexpr uint32_t X_BYTES = 2 * DR * TILE * sizeof(cplx<T>);   // cross contributions of both warps
     static constexpr uint32_t R_BYTES = SHARED ? DR * DR * TILE * sizeof(E) : 0;   // the rebuilt R(W) of one direction
     static constexpr uint32_t NBAR = 2 * STAGES + 2;                // full[S], empty[S], self full, self empty
+    // site-diagonal matrices (kernels.h DIAG_*; hop_ring.cuh): NENT complex entries per site in pieces of DE entries, NDC per tile
+    static constexpr int NENT = DIAG == DIAG_NONE ? 0 : DIAG == DIAG_HB ? 4 * DR * DR : 8 * DR * DR;
+    static constexpr int DE = (int)(CHUNK / (TILE * sizeof(cplx<T>)));
+    static constexpr int NDC = DIAG == DIAG_NONE ? 0 : (NENT + DE - 1) / DE;
     static constexpr size_t PER_PAIR = (size_t)STAGES * CHUNK + SELF_BYTES + X_BYTES + R_BYTES + NBAR * 8;
     static constexpr size_t SMEM = PER_PAIR * PAIRS;
     static_assert(CHUNK % 16 == 0 && PER_PAIR % 16 == 0, "bulk copies need 16-byte alignment");
     static_assert(SMEM <= 227 * 1024, "pair rings do not fit the 227 KB of shared memory of an sm_100 CTA");
 };
 
-template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF, int REP>
+template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF, int REP, int DIAG = DIAG_NONE>
 __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, const HopLaunch L) {
     using C = cplx<T>;
     using E = link_elem<T, REAL>;
-    using Cfg = PairCfg<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF, REP>;
+    using Cfg = PairCfg<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF, REP, DIAG>;
     constexpr bool REBUILD = NF > 0, SHARED = Cfg::SHARED;
-    constexpr int NC = 4 * DR, CPD = Cfg::CPD, CPT = 8 * CPD;
+    constexpr int NC = 4 * DR, CPD = Cfg::CPD, CPT = 8 * CPD + Cfg::NDC;   // chunks per tile: links, then the diagonal matrices
+    constexpr int NENT = Cfg::NENT, DE = Cfg::DE;
     constexpr int RPCE = REBUILD ? DR : RPC;                        // rows of R served by one chunk
     extern __shared__ __align__(128) unsigned char smem_raw[];
 
@@ -116,16 +124,26 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
     // producer state: the next chunk to issue is chunk iq_c of the pair's iq_k-th tile
     int iq_k = 0, iq_c = 0;
     const unsigned char *iq_base = nullptr;
+    const C *iq_diag = nullptr;
     auto iq_enter = [&]() {
         int s_, t_;
         locate(iq_k, s_, t_);
-        iq_base = (const unsigned char *)(s_ ? L.set[1].links : L.set[0].links) + (size_t)t_ * CPT * Cfg::CHUNK;
+        iq_base = (const unsigned char *)(s_ ? L.set[1].links : L.set[0].links) + (size_t)t_ * (8 * CPD) * Cfg::CHUNK;
+        if constexpr (DIAG != DIAG_NONE) iq_diag = (const C *)(s_ ? L.set[1].diag : L.set[0].diag) + (size_t)t_ * NENT * TILE;
     };
     auto issue = [&](int slot) {
+        if (DIAG != DIAG_NONE && iq_c >= 8 * CPD) {
+            // piece iq_c - 8 CPD of the tile's diagonal matrices: DE entries (the last piece: what is left)
+            const int e0 = (iq_c - 8 * CPD) * DE;
+            const uint32_t bytes = (uint32_t)((NENT - e0 < DE ? NENT - e0 : DE) * TILE * sizeof(C));
+            mbar_expect_tx(full_s + 8 * slot, bytes);
+            bulk_g2s(ring_s + slot * Cfg::CHUNK, iq_diag + (size_t)e0 * TILE, bytes, full_s + 8 * slot, pol);
+        } else {
         mbar_expect_tx(full_s + 8 * slot, Cfg::CHUNK);
         // chunk iq_c of the tile = step iq_c / CPD of the walk -> direction dir_of<true>(step) of the gather block
         const int step = iq_c / CPD, chunk = dir_of<true>(step) * CPD + (iq_c - step * CPD);
         bulk_g2s(ring_s + slot * Cfg::CHUNK, iq_base + (size_t)chunk * Cfg::CHUNK, Cfg::CHUNK, full_s + 8 * slot, pol);
+        }
         if (++iq_c == CPT) {
             iq_c = 0;
             if (++iq_k < my_tiles) iq_enter();
@@ -304,6 +322,75 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
             ls[c].y += o.y;
         }
         if constexpr (SELF) mbar_wait(selffull_s, k & 1);
+        if constexpr (DIAG != DIAG_NONE) {
+            // Site-diagonal term (kernels.h DIAG_*; the ring kernel's epilogue split over the pair), chirality c = spins 2c, 2c + 1.
+            // Clover H, B: warp s computes the rows of spin 2c + s -- H multiplies the warp's own spin, B the partner's, so both
+            // warps use every entry that streams by.  Full blocks: warp s computes the rows I = 2r + s of the 2 d_R x 2 d_R block
+            // (rows alternate between the warps, so both work on every piece of the stream); the scaled hop sum of the chirality
+            // is exchanged through the cross buffer -- as the vector the block multiplies (DIAG_POST) or as the row's start value
+            // (DIAG_PRE) -- and the warp stores the rows it computed (FULLROWS below).
+            const T csw = (T)L.diag_csw;
+            const T sgh = s ? T(-1) : T(1);
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+                C o[DR];
+                C v[DIAG == DIAG_HB ? DR : 2 * DR], vo[DIAG == DIAG_HB ? DR : 1];   // HB: own spin / partner's spin; full blocks: v = both
+#pragma unroll
+                for (int j = 0; j < DR; ++j) {
+                    const C h = c == 0 ? up[j] : ls[j];
+                    o[j] = mk<T>(b * h.x, b * h.y);
+                }
+                if constexpr (DIAG == DIAG_HB) {
+#pragma unroll
+                    for (int j = 0; j < DR; ++j) {
+                        const C sv = selfbuf[((2 * c + s) * DR + j) * TILE + lane], so = selfbuf[((2 * c + 1 - s) * DR + j) * TILE + lane];
+                        o[j].x = fma(a, sv.x, o[j].x); o[j].y = fma(a, sv.y, o[j].y);
+                        v[j] = mk<T>(csw * sgh * sv.x, csw * sgh * sv.y);   // +-H on spin 0 / 1 of the chirality block
+                        vo[j] = mk<T>(csw * so.x, csw * so.y);
+                    }
+                } else {
+                    pair_sync(1 + pair);   // the partner has read what the buffer held before
+#pragma unroll
+                    for (int j = 0; j < DR; ++j) xbuf[(s * DR + j) * TILE + lane] = o[j];
+                    pair_sync(1 + pair);
+#pragma unroll
+                    for (int J = 0; J < 2 * DR; ++J)
+                        v[J] = DIAG == DIAG_POST ? xbuf[J * TILE + lane] : selfbuf[(2 * c * DR + J) * TILE + lane];
+#pragma unroll
+                    for (int r = 0; r < DR; ++r) o[r] = DIAG == DIAG_POST ? mk<T>(0, 0) : xbuf[(2 * r + s) * TILE + lane];
+                }
+#pragma unroll
+                for (int e = 0; e < NENT / 2; ++e) {
+                    const int ge = c * (NENT / 2) + e;
+                    if (ge % DE == 0) mbar_wait(full_s + 8 * slot, phase);
+                    const C m = reinterpret_cast<const C *>(ring + (size_t)slot * Cfg::CHUNK)[(ge % DE) * TILE + lane];
+                    if constexpr (DIAG == DIAG_HB) {
+                        const int i = (e % (DR * DR)) / DR, j = e % DR;
+                        if (e < DR * DR) mac<T>(o[i], m, v[j]);
+                        else if (s == 0) mac<T>(o[i], m, vo[j]);              // B psi_1 -> spin 0, row i
+                        else mac<T>(o[j], mk<T>(m.x, -m.y), vo[i]);            // B^+ psi_0 -> spin 1, row j
+                    } else {
+                        if (((e / (2 * DR)) & 1) == s) mac<T>(o[(e / (2 * DR)) >> 1], m, v[e % (2 * DR)]);
+                    }
+                    if (ge % DE == DE - 1 || ge == NENT - 1) {
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(empty_s + 8 * slot);
+                        if (producer && q + STAGES < my_chunks) {
+                            mbar_wait(empty_s + 8 * slot, phase);
+                            fence_proxy_async();
+                            issue(slot);
+                        }
+                        ++q;
+                        if (++slot == STAGES) { slot = 0; phase ^= 1; }
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < DR; ++j) {
+                    if (c == 0) up[j] = o[j];
+                    else ls[j] = o[j];
+                }
+            }
+        }
         if (c_active) {
             const size_t eoff = ((size_t)c_tile * NC) * TILE + lane;
             C *out = (C *)(c_set ? L.set[1].out : L.set[0].out) + eoff;
@@ -313,9 +400,10 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
             double site[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
             for (int c = 0; c < DR; ++c) {
-                C vu = mk<T>(b * up[c].x, b * up[c].y);
-                C vl = mk<T>(b * ls[c].x, b * ls[c].y);
-                if constexpr (SELF) {
+                C vu, vl;
+                if constexpr (DIAG != DIAG_NONE) { vu = up[c]; vl = ls[c]; }
+                else { vu = mk<T>(b * up[c].x, b * up[c].y); vl = mk<T>(b * ls[c].x, b * ls[c].y); }
+                if constexpr (SELF && DIAG == DIAG_NONE) {
                     const C su = selfbuf[(s * DR + c) * TILE + lane];
                     const C sl = selfbuf[((2 + s) * DR + c) * TILE + lane];
                     vu.x = fma(a, su.x, vu.x); vu.y = fma(a, su.y, vu.y);
@@ -325,9 +413,11 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
                         vl.x = fma(am, sl.y, vl.x); vl.y = fma(-am, sl.x, vl.y);
                     }
                 }
-                red_store(L.red_mode, out + (size_t)(s * DR + c) * TILE, rp + (size_t)(s * DR + c) * TILE, al, vu, site[0], site[1]);
-                red_store(L.red_mode, out + (size_t)((2 + s) * DR + c) * TILE, rp + (size_t)((2 + s) * DR + c) * TILE, al,
-                          mk<T>(g5s * vl.x, g5s * vl.y), site[2], site[3]);
+                // component of the upper value: spin s, colour c -- or, after a full-block epilogue, row 2c + s of chirality 0
+                constexpr bool FULLROWS = DIAG == DIAG_PRE || DIAG == DIAG_POST;
+                const int cu = FULLROWS ? 2 * c + s : s * DR + c, cl = 2 * DR + cu;
+                red_store(L.red_mode, out + (size_t)cu * TILE, rp + (size_t)cu * TILE, al, vu, site[0], site[1]);
+                red_store(L.red_mode, out + (size_t)cl * TILE, rp + (size_t)cl * TILE, al, mk<T>(g5s * vl.x, g5s * vl.y), site[2], site[3]);
             }
             if (L.red_mode != 0) acc_add(racc, (site[0] + site[1]) + (site[2] + site[3]), L.red_alg);
         }
@@ -339,10 +429,10 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
     red_finish_cta(L.red_mode, L.red_alg, racc, L.red_partial, red_scratch);
 }
 
-template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF, int REP>
+template <typename T, int DR, bool REAL, int PAIRS, int STAGES, int RPC, bool SELF, int NF, int REP, int DIAG = DIAG_NONE>
 int launch_hop_pair_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
-    using Cfg = PairCfg<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF, REP>;
-    auto kern = hop_pair_kernel<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF, REP>;
+    using Cfg = PairCfg<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF, REP, DIAG>;
+    auto kern = hop_pair_kernel<T, DR, REAL, PAIRS, STAGES, RPC, SELF, NF, REP, DIAG>;
     static DevCache cache{};
     int n_sm = 0;
     if (const int rc = prepare_launch(kern, Cfg::SMEM, cache, n_sm)) return rc;
@@ -381,6 +471,22 @@ template <typename T, int DR, bool REAL, bool SELF, int NF, int REP = 0> struct 
     static constexpr int STAGES = stages_of(RPC);
     static_assert(STAGES >= 2, "pair ring needs at least two stages");
 };
+
+// stored links with the site-diagonal matrices in the epilogue (kernels.h DIAG_*)
+template <typename T, int DR, bool REAL> int launch_hop_pair_diag(const Geo &g, const HopLaunch &L, cudaStream_t s) {
+    if (L.am != 0.0 || !L.set[0].diag || (L.nsets == 2 && !L.set[1].diag)) return KERR_UNSUPPORTED;
+    if (L.diag_mode == DIAG_POST) {
+        // the shape of the passes with a self term (4 pairs in fp64): the block epilogue makes a tile long enough that the
+        // fourth pair pays, unlike in the pure hop pass
+        using P = PairPick<T, DR, REAL, true, 0, 0>;
+        return launch_hop_pair_cfg<T, DR, REAL, P::PAIRS, P::STAGES, P::RPC, false, 0, 0, DIAG_POST>(g, L, s);
+    }
+    if (!L.set[0].self) return KERR_UNSUPPORTED;
+    using P = PairPick<T, DR, REAL, true, 0, 0>;
+    if (L.diag_mode == DIAG_HB) return launch_hop_pair_cfg<T, DR, REAL, P::PAIRS, P::STAGES, P::RPC, true, 0, 0, DIAG_HB>(g, L, s);
+    if (L.diag_mode == DIAG_PRE) return launch_hop_pair_cfg<T, DR, REAL, P::PAIRS, P::STAGES, P::RPC, true, 0, 0, DIAG_PRE>(g, L, s);
+    return KERR_UNSUPPORTED;
+}
 
 template <typename T, int DR, bool REAL, int NF = 0, int REP = 0> int launch_hop_pair(const Geo &g, const HopLaunch &L, cudaStream_t s) {
     const bool self = (L.a != 0.0) && L.set[0].self != nullptr;

@@ -461,6 +461,8 @@ int launch_hop_ring_cfg(const Geo &g, const HopLaunch &L0, cudaStream_t s) {
 template <typename T, int DR, bool REAL> int launch_hop_ring(const Geo &g, const HopLaunch &L, cudaStream_t s) {
     const bool self = (L.a != 0.0) && L.set[0].self != nullptr;
     if (L.diag_mode != DIAG_NONE) {   // site-diagonal matrices in the epilogue: the self term is the matrix term
+        if constexpr (sizeof(T) == 8 && DR > 4) return KERR_UNSUPPORTED;   // one thread per site spills there: the pair kernel's job
+        else {
         if (L.am != 0.0 || !L.set[0].diag || (L.nsets == 2 && !L.set[1].diag)) return KERR_UNSUPPORTED;
         if (L.diag_mode == DIAG_POST) {
             using P = RingPick<T, DR, REAL, false>;
@@ -471,6 +473,7 @@ template <typename T, int DR, bool REAL> int launch_hop_ring(const Geo &g, const
         if (L.diag_mode == DIAG_HB) return launch_hop_ring_cfg<T, DR, REAL, P::WARPS, P::STAGES, P::RPC, true, DIAG_HB>(g, L, s);
         if (L.diag_mode == DIAG_PRE) return launch_hop_ring_cfg<T, DR, REAL, P::WARPS, P::STAGES, P::RPC, true, DIAG_PRE>(g, L, s);
         return KERR_UNSUPPORTED;
+        }
     }
     if (self) {
         using P = RingPick<T, DR, REAL, true>;

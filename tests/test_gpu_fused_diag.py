@@ -12,8 +12,9 @@ from tests.test_gpu_parity import Problem, env  # noqa: F401  (env is a fixture)
 
 pytestmark = pytest.mark.gpu
 
-# (config, T, L, fused form instantiated in fp64, in fp32): ring kernel d_R <= 4 in fp64, <= 6 in fp32; C3 has real links
-CASES = [("C1", 4, 4, True, True), ("C2", 6, 6, True, True), ("C3", 4, 8, True, True), ("C4", 4, 6, False, True), ("C5", 2, 4, False, False)]
+# (config, T, L, fused form instantiated in fp64, in fp32): ring kernel d_R <= 4 in fp64, <= 6 in fp32, pair kernel d_R = 5, 6;
+# C3 has real links; C5 (d_R = 35, row-group kernel) keeps the composed form
+CASES = [("C1", 4, 4, True, True), ("C2", 6, 6, True, True), ("C3", 4, 8, True, True), ("C4", 4, 6, True, True), ("C5", 2, 4, False, False)]
 
 
 def launches(g, fn):
@@ -74,16 +75,20 @@ def test_fused_and_composed_forms(env, name, T, L, f64_fused, f32_fused, prec, m
         assert np.abs(got - want[op]).max() < 100 * tol * np.abs(want[op]).max(), (op, fuse)
 
 
-@pytest.mark.parametrize("n,rep,T,L,prec", [(2, 3, 4, 4, "f64"), (2, 0, 2, 6, "f64"), (4, 0, 4, 4, "f64"), (2, 2, 4, 4, "f32"), (3, 3, 2, 6, "f32"),
-                                            (5, 0, 4, 2, "f32"), (3, 2, 4, 4, "f32"), (4, 0, 6, 4, "f32")])
-def test_fused_form_every_ring_instantiation(env, n, rep, T, L, prec):
-    """d_R = 1 (SU(2) 2AS: one-entry ring slots), 2, 4 in fp64; d_R = 3, 3, 5, 6, 4 in fp32 -- every d_R the fused epilogue is
-    instantiated for beyond the BASELINE configs; ragged tails (4^4: 4 tiles; 2x6^3: 6.75 tiles)."""
+@pytest.mark.parametrize("n,rep,T,L,prec,variant", [(2, 3, 4, 4, "f64", 0), (2, 0, 2, 6, "f64", 0), (4, 0, 4, 4, "f64", 0), (5, 0, 4, 2, "f64", 0),
+                                                    (3, 2, 4, 4, "f64", 0), (2, 2, 4, 4, "f32", 0), (3, 3, 2, 6, "f32", 0), (5, 0, 4, 2, "f32", 0),
+                                                    (3, 2, 4, 4, "f32", 0), (4, 0, 6, 4, "f32", 0), (5, 0, 4, 2, "f32", 4), (3, 2, 2, 6, "f32", 4),
+                                                    (3, 0, 4, 4, "f64", 3)])
+def test_fused_form_every_instantiation(env, n, rep, T, L, prec, variant):
+    """d_R = 1 (SU(2) 2AS: one-entry ring slots), 2, 4 (ring kernel), 5, 6 (pair kernel) in fp64; d_R = 3, 3, 5, 6, 4 in fp32 (ring
+    kernel) and d_R = 5, 6 on the pair kernel (variant 4) -- every d_R the fused epilogue is instantiated for beyond the BASELINE
+    configs; ragged tails (4^4: 4 tiles; 2x6^3: 6.75 tiles)."""
     from oracle import clover as oc
     hirep, oracle = env["hirep"], env["oracle"]
     cfg = synth.Config("t", T, L, n, rep, -0.15, "haar", 29, ())
     p = Problem(env, cfg, prec)
     g, m0, tol = p.geom, cfg.m0, TOL[prec]
+    g.set_kernel_variant(variant)
     cl = g.clover_field(p.links_rep)
     psi = p.spinors[0]
     x = p.to_native(psi, hirep.FULL)
@@ -96,9 +101,13 @@ def test_fused_form_every_ring_instantiation(env, n, rep, T, L, prec):
     assert nl == 2
     assert oracle.rel_l2(p.to_numpy(out, hirep.EVEN), oc.Dphi_clover_hat(T, L, m0, 0.4, p.R, psi[p.ev], BC)) < tol
     E = g.clover_exp_field(m0, 0.8, cl)
+    Ei = g.clover_exp_field(m0, 0.8, cl, inverse=True)
     out, nl = launches(g, lambda: g.Dphi_blocks(x, p.links_rep, E))
     assert nl == 1
     assert oracle.rel_l2(p.to_numpy(out, hirep.FULL), oc.Dphi_expclover(T, L, m0, 0.8, p.R, psi, BC)) < tol
+    out, nl = launches(g, lambda: g.Dphi_blocks_hat(xe, p.links_rep, E, Ei[E.numel() // 2:]))
+    assert nl == 2
+    assert oracle.rel_l2(p.to_numpy(out, hirep.EVEN), oc.Dphi_expclover_hat(T, L, m0, 0.8, p.R, psi[p.ev], BC)) < tol
 
 
 def test_fused_form_g5_squares_and_cg(env):
