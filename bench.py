@@ -594,9 +594,10 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
             _, it, res = geom.cg_g5Dphi_clover_hat_sq(m0, 0.5, x_e, lr, cl, inv, 1e-30, iters, out=y_e)
             torch.cuda.synchronize()
             ms_it = (time.perf_counter() - t0) * 1e3 / max(it, 1)
-            by_it = 2 * by + (1 + 3 + 5) * S * V / 2
+            # fused form: the CG's reductions ride in the epilogues of the second pass of each Q_hat (r read + write, x / p update, A p never stored)
+            by_it = 2 * by + ((2 + 5 - 1) if fused_diag else (1 + 3 + 5)) * S * V / 2
             out["cg_g5Dphi_clover_hat_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gbs": round(by_it / ms_it / 1e6, 1),
-                                              "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3), "launches_per_iteration": 9 if fused_diag else 13,
+                                              "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3), "launches_per_iteration": 7 if fused_diag else 13, "fused_reductions": bool(fused_diag),
                                               "relres_after": res}
         except Exception as e:
             out["cg_g5Dphi_clover_hat_sq"] = {"error": str(e)}

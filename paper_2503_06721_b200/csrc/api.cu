@@ -595,17 +595,23 @@ static bool fuse_diag(const hirep_geom *g) {
     return g->tune_fuse_diag && !g->slab && k_hop_diag_supported(g->prec == HIREP_F64 ? 0 : 1, g->dR, g->real, g->mode, g->variant);
 }
 // one stencil pass over parity p_out with the diagonal matrices `diag` of that parity in its epilogue (kernels.h DIAG_*)
+static void set_red(hirep_geom *g, HopLaunch &L, const FusedRed *red) {   // the CG's reduction in this launch's epilogue (FusedRed)
+    if (!red) return;
+    L.red_mode = red->mode; L.red_alg = g->sum_alg; L.red_partial = g->ws_red2;
+    L.red_r = red->r; L.red_num = red->num; L.red_den = red->den;
+}
 static int hop_diag_half(hirep_geom *g, int diag_mode, double a, double csw, double b, int g5, void *out, const void *in, const void *self,
-                         const void *links, const void *diag, int p_out, const char *what) {
+                         const void *links, const void *diag, int p_out, const char *what, const FusedRed *red = nullptr) {
     HopLaunch L{};
     L.nsets = 1;
     L.set[0] = HopSet{in, out, self, links_parity(g, links, p_out), p_out, diag};
     L.a = a; L.b = b; L.g5 = g5; L.diag_mode = diag_mode; L.diag_csw = csw;
+    set_red(g, L, red);
     return hop(g, L, what);
 }
 // the same over both parities in one launch: out = [gamma_5] (Diag in + b hop(in)); diag_full = both parities, even first
 static int hop_diag_full(hirep_geom *g, int diag_mode, double a, double csw, int g5, void *out_full, const void *in_full, const void *links,
-                         const void *diag_full, size_t diag_parity_bytes, const char *what) {
+                         const void *diag_full, size_t diag_parity_bytes, const char *what, const FusedRed *red = nullptr) {
     const size_t hb = g->bytes_spinor_half;
     const char *in_e = (const char *)in_full, *in_o = in_e + hb;
     char *out_e = (char *)out_full, *out_o = out_e + hb;
@@ -614,14 +620,16 @@ static int hop_diag_full(hirep_geom *g, int diag_mode, double a, double csw, int
     L.set[0] = HopSet{in_o, out_e, in_e, links_parity(g, links, 0), 0, diag_full};
     L.set[1] = HopSet{in_e, out_o, in_o, links_parity(g, links, 1), 1, (const char *)diag_full + diag_parity_bytes};
     L.a = a; L.b = -0.5; L.g5 = g5; L.diag_mode = diag_mode; L.diag_csw = csw;
+    set_red(g, L, red);
     return hop(g, L, what);
 }
 // out = [gamma_5] (Cphi in - 1/2 hop(in)).  Fused: one stencil launch whose epilogue applies (4+m) + c_sw A to the site's own
 // input.  Composed: Cphi writes out, the hopping pass accumulates onto it in place (every site's own
 // value is read before it is written, by the same tile); gamma_5 commutes with the diagonal blocks
 static int dphi_clover(hirep_geom *g, double m0, double csw, void *out_full, const void *in_full, const void *links, const void *clover, int g5,
-                       const char *what) {
-    if (fuse_diag(g)) return hop_diag_full(g, DIAG_HB, 4.0 + m0, csw, g5, out_full, in_full, links, clover, clover_bytes(g) / 2, what);
+                       const char *what, const FusedRed *red = nullptr) {
+    if (fuse_diag(g)) return hop_diag_full(g, DIAG_HB, 4.0 + m0, csw, g5, out_full, in_full, links, clover, clover_bytes(g) / 2, what, red);
+    if (red) return fail(HIREP_EINVAL, "%s: fused reductions need the fused epilogue", what);
     int rc = kern_result(g, k_cphi(g->prec, g->dR, 2 * g->geo.n_tiles, 4.0 + m0, csw, clover, in_full, out_full, g->stream), what);
     if (rc) return rc;
     const size_t hb = g->bytes_spinor_half;
@@ -710,8 +718,10 @@ extern "C" int hirep_clover_exp_field(hirep_geom *g, double m0, double csw, int 
     return kern_result(g, k_clover_exp(g->geo, g->prec, g->dR, parity, x, pref, clover, blocks, g->ws_exp, g->dev_flags, g->stream), "hirep_clover_exp_field");
 }
 // out = [gamma_5] (blocks in - 1/2 hop(in)); gamma_5 commutes with the chirality blocks
-static int dphi_blocks(hirep_geom *g, void *out_full, const void *in_full, const void *links, const void *blocks_full, int g5, const char *what) {
-    if (fuse_diag(g)) return hop_diag_full(g, DIAG_PRE, 0.0, 0.0, g5, out_full, in_full, links, blocks_full, clover_bytes(g), what);
+static int dphi_blocks(hirep_geom *g, void *out_full, const void *in_full, const void *links, const void *blocks_full, int g5, const char *what,
+                       const FusedRed *red = nullptr) {
+    if (fuse_diag(g)) return hop_diag_full(g, DIAG_PRE, 0.0, 0.0, g5, out_full, in_full, links, blocks_full, clover_bytes(g), what, red);
+    if (red) return fail(HIREP_EINVAL, "%s: fused reductions need the fused epilogue", what);
     int rc = kern_result(g, k_cblock(g->prec, g->dR, 2 * g->geo.n_tiles, blocks_full, in_full, out_full, g->stream), what);
     if (rc) return rc;
     const size_t hb = g->bytes_spinor_half;
@@ -769,15 +779,16 @@ extern "C" int hirep_Dphi_blocks_hat(hirep_geom *g, void *out_even, const void *
 // [gamma_5] D_hat for site-diagonal blocks (Eq 43): D_ee is either Cphi from the clover field (clover != NULL) or the
 // given even blocks; gamma_5 commutes with the blocks, so it is applied once in the last stencil epilogue
 static int blocks_hat(hirep_geom *g, double m0, double csw, void *out_even, const void *in_even, const void *links, const void *clover,
-                      const void *blocks_even, const void *inv_odd, int g5, const char *what) {
+                      const void *blocks_even, const void *inv_odd, int g5, const char *what, const FusedRed *red = nullptr) {
     int rc = workspace(&g->ws_half, g->bytes_spinor_half);
     if (rc) return rc;
     if (fuse_diag(g)) {
         rc = hop_diag_half(g, DIAG_POST, 0.0, 0.0, -0.5, 0, g->ws_half, in_even, nullptr, links, inv_odd, 1, what);
         if (rc) return rc;
-        return clover ? hop_diag_half(g, DIAG_HB, 4.0 + m0, csw, +0.5, g5, out_even, g->ws_half, in_even, links, clover, 0, what)
-                      : hop_diag_half(g, DIAG_PRE, 0.0, 0.0, +0.5, g5, out_even, g->ws_half, in_even, links, blocks_even, 0, what);
+        return clover ? hop_diag_half(g, DIAG_HB, 4.0 + m0, csw, +0.5, g5, out_even, g->ws_half, in_even, links, clover, 0, what, red)
+                      : hop_diag_half(g, DIAG_PRE, 0.0, 0.0, +0.5, g5, out_even, g->ws_half, in_even, links, blocks_even, 0, what, red);
     }
+    if (red) return fail(HIREP_EINVAL, "%s: fused reductions need the fused epilogue", what);
     rc = workspace(&g->ws_half2, g->bytes_spinor_half);
     if (rc) return rc;
     rc = offdiag(g, g->ws_half, in_even, links, 1, what);
@@ -986,18 +997,30 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
     // accumulated in its epilogue; pass 2 = gamma_5 D (B p) whose epilogue does r -= alpha A p and accumulates ||r||^2 without ever
     // storing A p: 3 spinor passes and 2 launches fewer per iteration (the separate ||Bp||^2 and residual-update kernels are gone).
     // Even-odd form (Q_hat^2, ring / pair kernels): the same two reductions ride on the second pass of each Q_hat application.
+    // Operators with site-diagonal matrices (clover, exponential clover; full lattice and Schur form): when their matrices ride in the
+    // stencil epilogues (fuse_diag) the last launch of each B = gamma_5 D [hat] application is a ring / pair kernel launch whose
+    // epilogue carries the same two reductions.
     const bool plain = !twisted && !clover && !blocks_even && !inv_odd;
-    const bool fused = plain && (full ? fused_cg_ok(g) : fused_cg_eo_ok(g));
+    const bool diag = !twisted && !plain;
+    const bool fused = plain ? (full ? fused_cg_ok(g) : fused_cg_eo_ok(g)) : (diag && fuse_diag(g) && fused_cg_eo_ok(g));
     const int nred = k_reduce_workspace_bytes() / (int)(2 * 3 * sizeof(double));   // Acc pairs the partial buffer holds
+    void *Bp_f = nullptr;   // B p of the fused form
     if (fused) {
-        if ((rc = workspace(&g->ws_red2, (size_t)k_reduce_workspace_bytes())) ||
-            (rc = full ? workspace(&g->ws_full, 2 * g->bytes_spinor_half) : workspace(&g->ws_half2, g->bytes_spinor_half))) return rc;
+        void **slot = inv_odd ? &g->ws_half3 : full ? &g->ws_full : &g->ws_half2;
+        if ((rc = workspace(&g->ws_red2, (size_t)k_reduce_workspace_bytes())) || (rc = workspace(slot, (full ? 2 : 1) * g->bytes_spinor_half))) return rc;
         if ((e = cudaMemsetAsync(g->ws_red2, 0, (size_t)k_reduce_workspace_bytes(), g->stream)) != cudaSuccess) return cuda_fail(e, what);
+        Bp_f = *slot;
     }
+    // one application of B with the reduction `fr` in the epilogue of its last launch
+    auto apply_B = [&](void *out, const void *in, const FusedRed *fr) -> int {
+        if (inv_odd) return blocks_hat(g, m0, csw, out, in, links, clover, blocks_even, inv_odd, 1, what, fr);
+        if (blocks_even) return dphi_blocks(g, out, in, links, blocks_even, 1, what, fr);
+        if (clover) return dphi_clover(g, m0, csw, out, in, links, clover, 1, what, fr);
+        return full ? dphi_full(g, m0, out, in, links, 1, what, 0.0, fr) : dphi_hat(g, m0, out, in, links, 1, what, fr);
+    };
     auto fused_pass1 = [&]() -> int {
         const FusedRed fr{1, nullptr, nullptr, nullptr};
-        int rc2 = full ? dphi_full(g, m0, g->ws_full, g->cg_p, links, 1, what, 0.0, &fr)
-                       : dphi_hat(g, m0, g->ws_half2, g->cg_p, links, 1, what, &fr);
+        int rc2 = apply_B(Bp_f, g->cg_p, &fr);
         if (rc2) return rc2;
         return kern_result(g, k_reduce_final(nred, g->sum_alg, g->ws_red2, d, g->stream), what);
     };
@@ -1008,8 +1031,7 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
         double *rr_old = d + 2 + 2 * (it & 1), *rr_new_d = d + 2 + 2 * ((it + 1) & 1);
         if (fused) {
             const FusedRed fr{2, g->cg_r, rr_old, d};
-            if ((rc = full ? dphi_full(g, m0, g->cg_Ap, g->ws_full, links, 1, what, 0.0, &fr)
-                           : dphi_hat(g, m0, g->cg_Ap, g->ws_half2, links, 1, what, &fr))) return rc;
+            if ((rc = apply_B(g->cg_Ap, Bp_f, &fr))) return rc;
             if ((rc = kern_result(g, k_reduce_final(nred, g->sum_alg, g->ws_red2, rr_new_d, g->stream), what))) return rc;
         } else {
             rc = kern_result(g, k_cg_update(g->geo, g->prec, g->dR, halves, g->sum_alg, 0.0, rr_old, d, nullptr, g->cg_r, g->cg_p, g->cg_Ap, g->ws_red, rr_new_d, g->stream), what, 2);
