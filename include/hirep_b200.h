@@ -265,8 +265,11 @@ int hirep_Dphi_tm_hat(hirep_geom *g, double m0, double mu, void *out_even, const
  *                        closed loops); once per gauge update.  HIREP_EINVAL in HIREP_LINKS_REBUILD mode.
  *   hirep_clover_export  canonical_out[V][2][2 d_R][2 d_R] complex (device; site index as the canonical spinor): A_0, A_1.
  *   hirep_Cphi           out_full = ((4+m) + c_sw A) in_full           (the diagonal blocks of Eq 41 with Eq 47); out != in
- *   hirep_Dphi_clover    out_full = D_m in_full with that diagonal term (Eq 8 + Eq 47): Cphi, then the hopping pass adds
- *                        -1/2 hop(in) onto it in place; out != in; `links` as for hirep_Dphi (current link mode). */
+ *   hirep_Dphi_clover    out_full = D_m in_full with that diagonal term (Eq 8 + Eq 47).  Stored links, d_R <= 6: ONE stencil launch
+ *                        whose epilogue applies (4+m) + c_sw A to the site's own input (the H, B matrices stream through the same
+ *                        shared-memory ring as the links).  Otherwise (d_R >= 8, link mode REBUILD, slabs,
+ *                        HIREP_TUNE_FUSE_DIAG = 0): Cphi, then the hopping pass adds -1/2 hop(in) onto it in place.  out != in;
+ *                        `links` as for hirep_Dphi (current link mode). */
 int hirep_clover_bytes(const hirep_geom *g, size_t *bytes);
 int hirep_clover_field(hirep_geom *g, void *clover, const void *links_rep);
 int hirep_clover_export(hirep_geom *g, void *canonical_out, const void *clover);
@@ -283,7 +286,9 @@ int hirep_cg_g5Dphi_clover_sq(hirep_geom *g, double m0, double csw, void *x_full
  *                           regime the operator is used in); depends on m0 and c_sw, so once per gauge update AND mass.
  *   hirep_Cphi_inv          out_half = that block inverse applied to in_half (spinors of the parity `inv` was built for)
  *   hirep_Dphi_clover_hat   out_even = D_ee in_even - D_eo D_oo^{-1} D_oe in_even; inv_odd = hirep_clover_inv_field(.., HIREP_ODD, ..)
- *                           for the same m0, csw; four launches (D_oe, D_oo^{-1}, D_ee, D_eo accumulated in place); out != in. */
+ *                           for the same m0, csw.  Two launches where the fused epilogue exists (see hirep_Dphi_clover): the D_oe pass
+ *                           applies D_oo^{-1} to its hop sum before storing it, the D_eo pass adds D_ee in_even; else four
+ *                           (D_oe, D_oo^{-1}, D_ee, D_eo accumulated in place).  out != in. */
 int hirep_clover_inv_bytes(const hirep_geom *g, size_t *bytes);
 int hirep_clover_inv_field(hirep_geom *g, double m0, double csw, int parity, void *inv, const void *clover);
 int hirep_Cphi_inv(hirep_geom *g, void *out_half, const void *in_half, const void *inv);
@@ -298,7 +303,8 @@ int hirep_Dphi_clover_hat(hirep_geom *g, double m0, double csw, void *out_even, 
  *                           the odd blocks is a full-lattice block field.
  *   hirep_Dphi_blocks       out_full = blocks_full in_full - 1/2 hop(in_full): Eq 8 with ANY site-diagonal chirality blocks
  *                           (the exponential clover's; also (4+m) + c_sw A written out as full blocks); out != in
- *   hirep_Dphi_blocks_hat   out_even = blocks_even in_even - D_eo inv_blocks_odd D_oe in_even (Eq 43); four launches; out != in */
+ *   hirep_Dphi_blocks_hat   out_even = blocks_even in_even - D_eo inv_blocks_odd D_oe in_even (Eq 43); two launches (fused epilogues,
+ *                           as hirep_Dphi_clover_hat) or four; out != in */
 int hirep_clover_exp_field(hirep_geom *g, double m0, double csw, int parity, int inverse, void *blocks, const void *clover);
 int hirep_Dphi_blocks(hirep_geom *g, void *out_full, const void *in_full, const void *links, const void *blocks_full);
 int hirep_Dphi_blocks_hat(hirep_geom *g, void *out_even, const void *in_even, const void *links, const void *blocks_even,
@@ -306,7 +312,8 @@ int hirep_Dphi_blocks_hat(hirep_geom *g, void *out_even, const void *in_even, co
 
 /* Even-odd preconditioned CG with a site-diagonal term (L803, L815): Q_hat = gamma_5 D_hat with D_hat of Eq 43 is Hermitian
  * when the blocks are (gamma_5 commutes with them and gamma_5 D_eo gamma_5 = D_oe^dagger), so Q_hat^2 is Hermitian positive
- * definite.  Arguments as hirep_Dphi_clover_hat / hirep_Dphi_blocks_hat; eight launches per application; out != in.
+ * definite.  Arguments as hirep_Dphi_clover_hat / hirep_Dphi_blocks_hat; four (fused epilogues) or eight launches per application;
+ * the CGs then also carry their two reductions in the epilogues of those launches (seven launches per iteration); out != in.
  *   hirep_g5Dphi_clover_hat_sq / hirep_g5Dphi_blocks_hat_sq     out_even = Q_hat^2 in_even
  *   hirep_cg_g5Dphi_clover_hat_sq / hirep_cg_g5Dphi_blocks_hat_sq   Q_hat^2 x_even = b_even; recurrence, stopping rule, iters
  *                           and relres (host pointers, may be NULL) as hirep_cg_g5Dphi_hat_sq; x != b. */
