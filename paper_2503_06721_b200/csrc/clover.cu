@@ -251,6 +251,57 @@ __global__ void __launch_bounds__(256, sizeof(T) == 8 ? 4 : 3) cphi_kernel(int n
     }
 }
 
+// Large d_R (15 ... 35): a warp computes R consecutive rows i of both spin rows of a chirality at once, so that every psi_j it
+// loads serves 4 R complex MACs (the row-pair kernel above re-reads the whole chirality half of psi for every row: as many bytes
+// through L1 / L2 as the matrices themselves) and 3 R independent matrix loads are in flight per step.  Work units (tile, c, row
+// group) are dealt round-robin over all warps of the grid.
+template <typename T, int R>
+__global__ void __launch_bounds__(256, 2) cphi_rows_kernel(int ntile_total, int dR, T a, T csw, const cplx<T> *__restrict__ clover,
+                                                           const cplx<T> *__restrict__ in, cplx<T> *__restrict__ out) {
+    const int ne = dR * dR, ncomp = 4 * dR, lane = threadIdx.x & 31;
+    const int groups = (dR + R - 1) / R, upt = 2 * groups;               // units per tile
+    const long n_units = (long)ntile_total * upt;
+    const long gw = (long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), nw = (long)gridDim.x * (blockDim.x >> 5);
+    for (long u = gw; u < n_units; u += nw) {
+        const int tile = (int)(u / upt), q = (int)(u - (long)tile * upt), c = q / groups, i0 = (q - c * groups) * R;
+        const cplx<T> *psi = in + (size_t)tile * ncomp * TILE + lane;
+        const cplx<T> *H = clover + ((size_t)tile * 4 + 2 * c) * ne * TILE + lane, *B = H + (size_t)ne * TILE;
+        const cplx<T> *p0 = psi + (size_t)(2 * c) * dR * TILE, *p1 = p0 + (size_t)dR * TILE;
+        int row[R];   // rows of this group; a ragged last group repeats row d_R - 1 (computed twice, stored once)
+#pragma unroll
+        for (int r = 0; r < R; ++r) row[r] = i0 + r < dR ? i0 + r : dR - 1;
+        cplx<T> s0[R], s1[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) s0[r] = s1[r] = mk<T>(0, 0);
+        for (int j = 0; j < dR; ++j) {
+            const cplx<T> x0 = __ldg(p0 + (size_t)j * TILE), x1 = __ldg(p1 + (size_t)j * TILE);
+            cplx<T> h[R], b[R], bt[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                h[r] = __ldcs(H + (size_t)(row[r] * dR + j) * TILE);
+                b[r] = __ldg(B + (size_t)(row[r] * dR + j) * TILE);      // B is read twice (as row and as column): keep it cacheable
+                bt[r] = __ldg(B + (size_t)(j * dR + row[r]) * TILE);
+            }
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                cfma<T>(s0[r], h[r], x0);
+                cfma<T>(s0[r], b[r], x1);
+                cfma_conj<T>(s1[r], bt[r], x0);
+                cfma<T>(s1[r], mk<T>(-h[r].x, -h[r].y), x1);
+            }
+        }
+        cplx<T> *o = out + (size_t)tile * ncomp * TILE + lane;
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (i0 + r < dR) {
+                const int i = i0 + r;
+                const cplx<T> e0 = __ldg(p0 + (size_t)i * TILE), e1 = __ldg(p1 + (size_t)i * TILE);
+                __stcs(o + (size_t)((2 * c) * dR + i) * TILE, mk<T>(a * e0.x + csw * s0[r].x, a * e0.y + csw * s0[r].y));
+                __stcs(o + (size_t)((2 * c + 1) * dR + i) * TILE, mk<T>(a * e1.x + csw * s1[r].x, a * e1.y + csw * s1[r].y));
+            }
+    }
+}
+
 // canonical export: [V][c][2 dR][2 dR] complex, A_c = [[H, B], [B^+, -H]]; one thread per (site, c, row, column)
 template <typename T> __global__ void clover_export_kernel(Geo g, int dR, cplx<T> *__restrict__ canon, const cplx<T> *__restrict__ clover) {
     const int n2 = 2 * dR, ne = dR * dR;
@@ -414,6 +465,16 @@ template <typename T> static int cphi_t(int ntile, int dR, double a, double csw,
     case 8: return cphi_site_t<T, 8>(ntile, a, csw, clover, in, out, s);
     case 10: return cphi_site_t<T, 10>(ntile, a, csw, clover, in, out, s);
     }
+    static const int generic = getenv("HIREP_CPHI_GENERIC") ? atoi(getenv("HIREP_CPHI_GENERIC")) : 0;   // measurement switch: the round-1 kernel
+    if (dR >= 12 && !generic) {   // row groups: R = 5 where it divides d_R (15, 35), else 4 (24) or 3 (21)
+        const int R = dR % 5 == 0 ? 5 : dR % 4 == 0 ? 4 : 3;
+        const long units = (long)ntile * 2 * ((dR + R - 1) / R);
+        const int grid = (int)((units + 7) / 8 < 148 * 2 ? (units + 7) / 8 : 148 * 2);
+        if (R == 5) cphi_rows_kernel<T, 5><<<grid, 256, 0, s>>>(ntile, dR, (T)a, (T)csw, (const cplx<T> *)clover, (const cplx<T> *)in, (cplx<T> *)out);
+        else if (R == 4) cphi_rows_kernel<T, 4><<<grid, 256, 0, s>>>(ntile, dR, (T)a, (T)csw, (const cplx<T> *)clover, (const cplx<T> *)in, (cplx<T> *)out);
+        else cphi_rows_kernel<T, 3><<<grid, 256, 0, s>>>(ntile, dR, (T)a, (T)csw, (const cplx<T> *)clover, (const cplx<T> *)in, (cplx<T> *)out);
+        return (int)cudaGetLastError();
+    }
     const int wy = 2 * dR < 8 ? 2 * dR : 8;      // 8 warps per CTA, 3-4 CTAs per SM (one 16-warp CTA per SM was latency bound: 2.9 TB/s)
     int grid = ntile < 148 * 16 ? ntile : 148 * 16;   // (one CTA per SM measured slower: 4.7 vs 4.1 ms at d_R = 35 fp64)
     cphi_kernel<T><<<grid, dim3(TILE, wy), 0, s>>>(ntile, dR, (T)a, (T)csw, (const cplx<T> *)clover, (const cplx<T> *)in, (cplx<T> *)out);
@@ -537,6 +598,40 @@ __global__ void __launch_bounds__(256, sizeof(T) == 8 ? 4 : 3) cblock_kernel(int
     }
 }
 
+// Large d_R: R consecutive rows of a chirality block per warp, one load of v_J serving R rows (see cphi_rows_kernel)
+template <typename T, int R>
+__global__ void __launch_bounds__(256, 2) cblock_rows_kernel(int ntile, int dR, const cplx<T> *__restrict__ blk, const cplx<T> *__restrict__ in,
+                                                             cplx<T> *__restrict__ out) {
+    const int n = 2 * dR, ncomp = 4 * dR, lane = threadIdx.x & 31;
+    const int groups = (n + R - 1) / R, upt = 2 * groups;
+    const long n_units = (long)ntile * upt;
+    const long gw = (long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), nw = (long)gridDim.x * (blockDim.x >> 5);
+    for (long u = gw; u < n_units; u += nw) {
+        const int tile = (int)(u / upt), q = (int)(u - (long)tile * upt), c = q / groups, I0 = (q - c * groups) * R;
+        const cplx<T> *v = in + ((size_t)tile * ncomp + (size_t)c * n) * TILE + lane;
+        const cplx<T> *M = blk + ((size_t)(tile * 2 + c) * n * n) * TILE + lane;
+        size_t rowoff[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) rowoff[r] = (size_t)(I0 + r < n ? I0 + r : n - 1) * n;
+        cplx<T> acc[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) acc[r] = mk<T>(0, 0);
+#pragma unroll 2
+        for (int J = 0; J < n; ++J) {
+            const cplx<T> x = __ldg(v + (size_t)J * TILE);
+            cplx<T> m[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) m[r] = __ldcs(M + (rowoff[r] + J) * TILE);
+#pragma unroll
+            for (int r = 0; r < R; ++r) cfma<T>(acc[r], m[r], x);
+        }
+        cplx<T> *o = out + ((size_t)tile * ncomp + (size_t)c * n) * TILE + lane;
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (I0 + r < n) __stcs(o + (size_t)(I0 + r) * TILE, acc[r]);
+    }
+}
+
 template <typename T, int DR> static int cblock_site_t(int ntile, const void *blk, const void *in, void *out, cudaStream_t s) {
     const int blocks = (ntile + 3) / 4;
     cblock_site_kernel<T, DR><<<blocks < 148 * 16 ? blocks : 148 * 16, 128, 0, s>>>(ntile, (const cplx<T> *)blk, (const cplx<T> *)in, (cplx<T> *)out);
@@ -549,6 +644,16 @@ template <typename T> static int cblock_t(int ntile, int dR, const void *blk, co
     case 4: return cblock_site_t<T, 4>(ntile, blk, in, out, s);
     case 5: return cblock_site_t<T, 5>(ntile, blk, in, out, s);
     case 6: return cblock_site_t<T, 6>(ntile, blk, in, out, s);
+    }
+    static const int generic = getenv("HIREP_CPHI_GENERIC") ? atoi(getenv("HIREP_CPHI_GENERIC")) : 0;   // measurement switch: the round-1 kernel
+    if (dR >= 8 && !generic) {   // row groups of 5 where that divides 2 d_R (10, 15, 35), else 6 (21, 24) or 4 (8)
+        const int n = 2 * dR, R = n % 5 == 0 ? 5 : n % 6 == 0 ? 6 : 4;
+        const long units = (long)ntile * 2 * ((n + R - 1) / R);
+        const int grid = (int)((units + 7) / 8 < 148 * 2 ? (units + 7) / 8 : 148 * 2);
+        if (R == 5) cblock_rows_kernel<T, 5><<<grid, 256, 0, s>>>(ntile, dR, (const cplx<T> *)blk, (const cplx<T> *)in, (cplx<T> *)out);
+        else if (R == 6) cblock_rows_kernel<T, 6><<<grid, 256, 0, s>>>(ntile, dR, (const cplx<T> *)blk, (const cplx<T> *)in, (cplx<T> *)out);
+        else cblock_rows_kernel<T, 4><<<grid, 256, 0, s>>>(ntile, dR, (const cplx<T> *)blk, (const cplx<T> *)in, (cplx<T> *)out);
+        return (int)cudaGetLastError();
     }
     const int wy = 4 * dR < 8 ? 4 * dR : 8;
     cblock_kernel<T><<<ntile < 148 * 16 ? ntile : 148 * 16, dim3(TILE, wy), 0, s>>>(ntile, dR, (const cplx<T> *)blk, (const cplx<T> *)in, (cplx<T> *)out);

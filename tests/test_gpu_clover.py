@@ -54,6 +54,28 @@ def test_clover_other_representations(env, n, rep, T, L):
     assert oracle.rel_l2(out, oc.Dphi_clover(T, L, cfg.m0, 0.9, p.R, psi, BC)) < 1e-13
 
 
+@pytest.mark.parametrize("n,rep,prec", [(5, 1, "f64"), (6, 2, "f64"), (6, 3, "f32"), (4, 1, "f32")])
+def test_clover_row_group_kernels(env, n, rep, prec):
+    """SU(5) adjoint (d_R = 24: row groups of 4 / 6), SU(6) symmetric (21: 3 / 6), SU(6) 2AS (15: 5 / 5), SU(4) adjoint (15, real links)
+    on 2^4 (one ragged tile per parity): Cphi, the block inverse applied by the row-group block kernel, and the Schur form."""
+    from oracle import clover as oc
+    hirep, oracle = env["hirep"], env["oracle"]
+    T, L = 2, 2
+    cfg = synth.Config("t", T, L, n, rep, 0.2, "haar", 31, ())
+    p = Problem(env, cfg, prec)
+    g, m0, tol, csw = p.geom, cfg.m0, TOL[prec], 0.3
+    cl = g.clover_field(p.links_rep)
+    psi = p.spinors[0]
+    out = p.to_numpy(g.Cphi(m0, csw, p.to_native(psi, hirep.FULL), cl), hirep.FULL)
+    assert oracle.rel_l2(out, oc.Cphi(T, L, m0, csw, p.R, psi)) < tol
+    inv_odd = g.clover_inv_field(m0, csw, hirep.ODD, cl)
+    got = p.to_numpy(g.Cphi_inv(hirep.ODD, p.to_native(psi[p.od], hirep.ODD), inv_odd), hirep.ODD)
+    assert oracle.rel_l2(got, oc.Cphi_inv(T, L, m0, csw, p.R, psi[p.od], sites=p.od)) < tol
+    xe = p.to_native(psi[p.ev], hirep.EVEN)
+    got = p.to_numpy(g.Dphi_clover_hat(m0, csw, xe, p.links_rep, cl, inv_odd), hirep.EVEN)
+    assert oracle.rel_l2(got, oc.Dphi_clover_hat(T, L, m0, csw, p.R, psi[p.ev], BC)) < tol
+
+
 def test_clover_periodic_bc_and_capped_grid(env):
     """Boundary signs cancel in the closed loops: the clover field is the same for periodic and antiperiodic links;
     Dphi_clover with a capped persistent grid (many tiles per warp in the in-place hopping pass)."""
