@@ -1296,7 +1296,7 @@ extern "C" int hirep_force_hopping(hirep_geom *g, void *force_canonical, const v
     if (g->mode != HIREP_LINKS_STORED) return fail(HIREP_EINVAL, "hirep_force_hopping: needs the stored represented links (HIREP_LINKS_STORED), or the adjoint representation in HIREP_LINKS_REBUILD mode");
     int rc = force_table(g);
     if (rc) return rc;
-    return kern_result(g, k_force_hopping(g->geo, g->prec, g->dR, g->real, eta_full, xi_full, links_rep, g->force_rowptr, g->force_jk, g->force_val,
+    return kern_result(g, k_force_hopping(g->geo, g->prec, g->dR, g->real, g->rep == HIREP_FUND, eta_full, xi_full, links_rep, g->force_rowptr, g->force_jk, g->force_val,
                                           g->force_dense, g->N * g->N - 1, force_canonical, g->stream), "hirep_force_hopping");
 }
 

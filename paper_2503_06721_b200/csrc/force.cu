@@ -173,99 +173,164 @@ __global__ void __launch_bounds__(256) force_hopping_kernel(const Geo g, int dR,
     }
 }
 
-// ---- small d_R: everything in registers, one thread per (site, mu), dense generator table read uniformly -----------------------
-// M_kj (d_R^2 complex) is accumulated in registers from the two outer products, then F^a = 2 sum_jk Im(T^a_jk M_kj) with T^a_jk
-// loaded at the same address by every lane (a broadcast).  Same arithmetic as the kernel above, without the shared-memory staging
-// that limits it to 8 warps per SM.
-template <typename T, int DR, bool REAL>
-__global__ void __launch_bounds__(128) force_site_kernel(const Geo g, const cplx<T> *eta, const cplx<T> *xi, const void *links_v,
-                                                         const double2 *dense, int NA, T *force, long n_units) {
+// ---- small d_R: M in registers, one warp per (parity, tile) walks the four mu ---------------------------------------------------
+// The site's own eta, xi (needed by all four directions) are staged ONCE per tile in shared memory -- each lane its own column, by
+// cp.async: extra register space, not an exchange -- instead of being re-read by four warps; the neighbours and the forward link
+// of each mu are loaded as before; M stays in registers.  For the fundamental representation the generators are those of reading
+// A10 in closed form (S_ij, A_ij, D_j: F = Im(M_ij + M_ji), Re(M_ij - M_ji), 2 nrm_j Im(sum_{q<j} M_qq - j M_jj)), so nothing is
+// read for them; other representations read the dense table from shared memory (a broadcast).  Round 2's first version ran one warp per
+// (parity, tile, mu) with the table read through L1: 12 warps per SM, latency bound (C2 fp64 0.67 ms; this one 0.38 ms, C4 fp32 20.9 -> 8.6 ms).
+// resident 128-thread blocks per SM the register budget is cut for: the live set grows with d_R^2 x precision
+template <typename T, int DR> constexpr int force_minb() { return DR * DR * (int)sizeof(T) <= 64 ? 4 : DR * DR * (int)sizeof(T) <= 100 ? 3 : 2; }
+template <typename T, int DR, bool REAL, bool FUND>
+__global__ void __launch_bounds__(128, force_minb<T, DR>()) force_tile_kernel(const Geo g, const cplx<T> *eta, const cplx<T> *xi, const void *links_v,
+                                                            const double2 *dense, int NA, T *force, int n_pt) {
     using C = cplx<T>;
     using E = link_elem<T, REAL>;
     constexpr int NC = 4 * DR;
-    const int lane = threadIdx.x & 31;
-    const long unit = (long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);   // (parity, tile, mu)
-    if (unit >= n_units) return;
-    const int mu = (int)(unit & 3);
-    const long pt = unit >> 2;
-    const int tile = (int)(pt % g.n_tiles), p = (int)(pt / g.n_tiles);
+    extern __shared__ __align__(16) unsigned char smem_force[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    C *tab = reinterpret_cast<C *>(smem_force + (size_t)4 * 2 * NC * TILE * sizeof(C));
+    if constexpr (!FUND) {
+        for (int i = threadIdx.x; i < NA * DR * DR; i += blockDim.x) tab[i] = mk<T>((T)dense[i].x, (T)dense[i].y);
+        __syncthreads();
+    }
+    const int pt = blockIdx.x * 4 + wib;
+    if (pt >= n_pt) return;
+    const int tile = pt % g.n_tiles, p = pt / g.n_tiles;
     int h = tile * TILE + lane;
     const bool active = h < g.Nh;
     if (!active) h = g.Nh - 1;
     int t, x, y, zh;
     decode_site(g, h, t, x, y, zh);
-    const int hn = mu == 0 ? neighbour<0>(g, p, t, x, y, zh) : mu == 1 ? neighbour<1>(g, p, t, x, y, zh)
-                 : mu == 2 ? neighbour<2>(g, p, t, x, y, zh) : neighbour<3>(g, p, t, x, y, zh);
     const size_t half = (size_t)g.n_tiles * NC * TILE;
-    const bool imag = (mu & 1), swap = (mu == 1 || mu == 2);
-    const E *W = (const E *)links_v + ((((size_t)p * g.n_tiles + tile) * 8 + mu) * (size_t)DR * DR) * TILE + lane;
-    C M[DR][DR];
+    // own[f][c][lane]: f = 0 eta, 1 xi of this site
+    C *own = reinterpret_cast<C *>(smem_force) + (size_t)wib * 2 * NC * TILE + lane;
+    {
+        const uint32_t own_s = smem_u32(own);
+        const C *e0 = eta + (size_t)p * half + ((size_t)tile * NC) * TILE + lane, *x0 = xi + (size_t)p * half + ((size_t)tile * NC) * TILE + lane;
 #pragma unroll
-    for (int k = 0; k < DR; ++k)
+        for (int c = 0; c < NC; ++c) {
+            cp_async<sizeof(C)>(own_s + (uint32_t)(c * TILE * sizeof(C)), e0 + (size_t)c * TILE);
+            cp_async<sizeof(C)>(own_s + (uint32_t)((NC + c) * TILE * sizeof(C)), x0 + (size_t)c * TILE);
+        }
+    }
+    const long ix = canonical_index(g, p, h);
+    bool staged = false;
+#pragma unroll 1
+    for (int mu = 0; mu < 4; ++mu) {
+        const int hn = mu == 0 ? neighbour<0>(g, p, t, x, y, zh) : mu == 1 ? neighbour<1>(g, p, t, x, y, zh)
+                     : mu == 2 ? neighbour<2>(g, p, t, x, y, zh) : neighbour<3>(g, p, t, x, y, zh);
+        const bool imag = (mu & 1), swap = (mu == 1 || mu == 2);
+        const E *W = (const E *)links_v + ((((size_t)p * g.n_tiles + tile) * 8 + mu) * (size_t)DR * DR) * TILE + lane;
+        E w[DR][DR];
 #pragma unroll
-        for (int j = 0; j < DR; ++j) M[k][j] = mk<T>(0, 0);
-    // M += (U h^A) (x) (k^B)^dagger for (A, B) = (eta, xi) and (xi, eta)
+        for (int k = 0; k < DR; ++k)
 #pragma unroll
-    for (int f = 0; f < 2; ++f) {
-        const C *fa = f ? xi : eta, *fb = f ? eta : xi;
-        const C *nb = fa + (size_t)(1 - p) * half + ((size_t)(hn >> 5) * NC) * TILE + (hn & 31);
-        const C *own = fb + (size_t)p * half + ((size_t)tile * NC) * TILE + lane;
+            for (int j = 0; j < DR; ++j) w[k][j] = W[(size_t)(k * DR + j) * TILE];
+        C M[DR][DR];
 #pragma unroll
-        for (int s = 0; s < 2; ++s) {
-            const int qq = swap ? 1 - s : s;
-            const T sig = (mu < 2) ? T(-1) : (s ? T(1) : T(-1));
-            C hv[DR], kv[DR];
+        for (int k = 0; k < DR; ++k)
 #pragma unroll
-            for (int c = 0; c < DR; ++c) {
-                hv[c] = proj<T>(__ldg(nb + (size_t)(s * DR + c) * TILE), __ldg(nb + (size_t)((2 + qq) * DR + c) * TILE), -sig, imag);
-                kv[c] = proj<T>(__ldg(own + (size_t)(s * DR + c) * TILE), __ldg(own + (size_t)((2 + qq) * DR + c) * TILE), sig, imag);
-            }
+            for (int j = 0; j < DR; ++j) M[k][j] = mk<T>(0, 0);
+        // M += (U h^A) (x) (k^B)^dagger for (A, B) = (eta, xi) and (xi, eta)
 #pragma unroll
-            for (int k = 0; k < DR; ++k) {
-                C chi = mk<T>(0, 0);
+        for (int f = 0; f < 2; ++f) {
+            const C *fa = f ? xi : eta;
+            const C *nb = fa + (size_t)(1 - p) * half + ((size_t)(hn >> 5) * NC) * TILE + (hn & 31);
+            C nbv[NC];
 #pragma unroll
-                for (int j = 0; j < DR; ++j) mac<T>(chi, W[(size_t)(k * DR + j) * TILE], hv[j]);
+            for (int c = 0; c < NC; ++c) nbv[c] = __ldg(nb + (size_t)c * TILE);
+            if (!staged) { cp_async_wait_all(); staged = true; }   // the lane's own column of the staged tile has landed
+            const C *ob = own + (size_t)((1 - f) * NC) * TILE;     // k comes from the OTHER field
 #pragma unroll
-                for (int j = 0; j < DR; ++j) {     // M_kj += chi_k conj(k_j)
-                    M[k][j].x += chi.x * kv[j].x + chi.y * kv[j].y;
-                    M[k][j].y += chi.y * kv[j].x - chi.x * kv[j].y;
+            for (int s = 0; s < 2; ++s) {
+                const int qq = swap ? 1 - s : s;
+                const T sig = (mu < 2) ? T(-1) : (s ? T(1) : T(-1));
+                C hv[DR], kv[DR];
+#pragma unroll
+                for (int c = 0; c < DR; ++c) {
+                    const C lo_n = qq ? nbv[3 * DR + c] : nbv[2 * DR + c];
+                    hv[c] = proj<T>(nbv[s * DR + c], lo_n, -sig, imag);
+                    kv[c] = proj<T>(ob[(size_t)(s * DR + c) * TILE], ob[(size_t)((2 + qq) * DR + c) * TILE], sig, imag);
+                }
+#pragma unroll
+                for (int k = 0; k < DR; ++k) {
+                    C chi = mk<T>(0, 0);
+#pragma unroll
+                    for (int j = 0; j < DR; ++j) mac<T>(chi, w[k][j], hv[j]);
+#pragma unroll
+                    for (int j = 0; j < DR; ++j) {     // M_kj += chi_k conj(k_j)
+                        M[k][j].x += chi.x * kv[j].x + chi.y * kv[j].y;
+                        M[k][j].y += chi.y * kv[j].x - chi.x * kv[j].y;
+                    }
                 }
             }
         }
-    }
-    if (!active) return;
-    const long ix = canonical_index(g, p, h);
-    T *out = force + ((size_t)ix * 4 + mu) * NA;
-    for (int a = 0; a < NA; ++a) {
-        const double2 *ta = dense + (size_t)a * DR * DR;
-        T acc = 0;
+        if (!active) continue;
+        T *out = force + ((size_t)ix * 4 + mu) * NA;
+        if constexpr (FUND) {
+            static_for<1, DR>([&](auto jc) {
+                constexpr int j = decltype(jc)::value;
+                T dsum = 0;
+                static_for<0, j>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    out[gen_base(j) + 2 * i] = M[i][j].y + M[j][i].y;
+                    out[gen_base(j) + 2 * i + 1] = M[i][j].x - M[j][i].x;
+                    dsum += M[i][i].y;
+                });
+                out[gen_base(j) + 2 * j] = (T)(2.0 * diag_norm(j)) * (dsum - j * M[j][j].y);
+            });
+        } else {
+            for (int a = 0; a < NA; ++a) {
+                const C *ta = tab + (size_t)a * DR * DR;
+                T acc = 0;
 #pragma unroll
-        for (int j = 0; j < DR; ++j)
+                for (int j = 0; j < DR; ++j)
 #pragma unroll
-            for (int k = 0; k < DR; ++k) {
-                const double2 tv = __ldg(ta + j * DR + k);          // T^a_jk, the same address in every lane
-                acc += (T)tv.x * M[k][j].y + (T)tv.y * M[k][j].x;   // Im(T^a_jk M_kj)
+                    for (int k = 0; k < DR; ++k) {
+                        const C tv = ta[j * DR + k];                        // T^a_jk, the same address in every lane
+                        acc += tv.x * M[k][j].y + tv.y * M[k][j].x;        // Im(T^a_jk M_kj)
+                    }
+                out[a] = 2 * acc;
             }
-        out[a] = 2 * acc;
+        }
     }
 }
 
+template <typename T, int DR, bool REAL, bool FUND>
+int launch_force_tile(const Geo &g, const void *eta, const void *xi, const void *links, const void *dense, int NA, void *force, cudaStream_t s) {
+    auto kern = force_tile_kernel<T, DR, REAL, FUND>;
+    const size_t own = (size_t)4 * 2 * 4 * DR * TILE * sizeof(cplx<T>);
+    const size_t smem = own + (FUND ? 0 : (size_t)NA * DR * DR * sizeof(cplx<T>));
+    // the opt-in size is set once per instantiation and device: for the largest generator table any group has here (SU(6): 35)
+    const size_t smem_max = own + (FUND ? 0 : (size_t)35 * DR * DR * sizeof(cplx<T>));
+    if (NA > 35) return KERR_UNSUPPORTED;
+    static DevCache cache{};
+    int n_sm = 0;
+    if (const int rc = prepare_launch(kern, smem_max, cache, n_sm)) return rc;
+    const int n_pt = 2 * g.n_tiles;
+    kern<<<(unsigned)((n_pt + 3) / 4), 128, smem, s>>>(g, (const cplx<T> *)eta, (const cplx<T> *)xi, links, (const double2 *)dense, NA, (T *)force, n_pt);
+    return (int)cudaGetLastError();
+}
 template <typename T, bool REAL>
-int force_site_dispatch(const Geo &g, int dR, const void *eta, const void *xi, const void *links, const void *dense, int NA, void *force, cudaStream_t s) {
-    const long n_units = (long)2 * g.n_tiles * 4;
-    const unsigned grid = (unsigned)((n_units + 3) / 4);
-#define FS(D) force_site_kernel<T, D, REAL><<<grid, 128, 0, s>>>(g, (const cplx<T> *)eta, (const cplx<T> *)xi, links, (const double2 *)dense, NA, (T *)force, n_units)
+int force_site_dispatch(const Geo &g, int dR, int fund, const void *eta, const void *xi, const void *links, const void *dense, int NA, void *force,
+                        cudaStream_t s) {
+#define FT(D)                                                                                                                        \
+    do {                                                                                                                             \
+        if constexpr (!REAL) { if (fund) return launch_force_tile<T, D, false, true>(g, eta, xi, links, dense, NA, force, s); }       \
+        return launch_force_tile<T, D, REAL, false>(g, eta, xi, links, dense, NA, force, s);                                         \
+    } while (0)
     switch (dR) {
-    case 1: FS(1); break;
-    case 2: FS(2); break;
-    case 3: FS(3); break;
-    case 4: FS(4); break;
-    case 5: if constexpr (sizeof(T) == 4) { FS(5); break; } else return KERR_UNSUPPORTED;
-    case 6: if constexpr (sizeof(T) == 4) { FS(6); break; } else return KERR_UNSUPPORTED;
+    case 1: return launch_force_tile<T, 1, REAL, false>(g, eta, xi, links, dense, NA, force, s);
+    case 2: FT(2);
+    case 3: FT(3);
+    case 4: FT(4);
+    case 5: if constexpr (sizeof(T) == 4) { FT(5); } else return KERR_UNSUPPORTED;
+    case 6: if constexpr (sizeof(T) == 4) { FT(6); } else return KERR_UNSUPPORTED;
     default: return KERR_UNSUPPORTED;
     }
-#undef FS
-    return (int)cudaGetLastError();
+#undef FT
 }
 
 // ---- adjoint representation, matrix-free (link mode REBUILD): the force as a commutator of N x N matrices -----------------------
@@ -503,13 +568,13 @@ int k_force_hopping_adj(const Geo &g, int prec, int N, const void *eta, const vo
     return KERR_UNSUPPORTED;
 }
 
-int k_force_hopping(const Geo &g, int prec, int dR, int real, const void *eta, const void *xi, const void *links, const int *rowptr,
+int k_force_hopping(const Geo &g, int prec, int dR, int real, int fund, const void *eta, const void *xi, const void *links, const int *rowptr,
                     const int *jk, const void *val, const void *dense, int NA, void *force, cudaStream_t s) {
-    if (dense) {   // d_R <= 4 (fp32: <= 6): the register kernel
-        const int rc = prec == 0 ? (real ? force_site_dispatch<double, true>(g, dR, eta, xi, links, dense, NA, force, s)
-                                         : force_site_dispatch<double, false>(g, dR, eta, xi, links, dense, NA, force, s))
-                                 : (real ? force_site_dispatch<float, true>(g, dR, eta, xi, links, dense, NA, force, s)
-                                         : force_site_dispatch<float, false>(g, dR, eta, xi, links, dense, NA, force, s));
+    if (dense) {   // d_R <= 4 (fp32: <= 6): the register kernels
+        const int rc = prec == 0 ? (real ? force_site_dispatch<double, true>(g, dR, fund, eta, xi, links, dense, NA, force, s)
+                                         : force_site_dispatch<double, false>(g, dR, fund, eta, xi, links, dense, NA, force, s))
+                                 : (real ? force_site_dispatch<float, true>(g, dR, fund, eta, xi, links, dense, NA, force, s)
+                                         : force_site_dispatch<float, false>(g, dR, fund, eta, xi, links, dense, NA, force, s));
         if (rc != KERR_UNSUPPORTED) return rc;
     }
     const size_t w = prec == 0 ? 16 : 8;

@@ -94,7 +94,8 @@ int k_cblock(int prec, int dR, int ntile, const void *blk, const void *in, void 
 // represented generators; k_force_hopping takes them as a sparse list (entries of generator a: rowptr[a]..rowptr[a+1], jk = j*dR+k)
 // and, for the register kernel at small d_R, the dense table itself
 int k_rep_generators(int N, int rep, void *table_dev, cudaStream_t s);
-int k_force_hopping(const Geo &g, int prec, int dR, int real, const void *eta, const void *xi, const void *links, const int *rowptr,
+// fund: the representation is the fundamental one (its generators are known in closed form, reading A10)
+int k_force_hopping(const Geo &g, int prec, int dR, int real, int fund, const void *eta, const void *xi, const void *links, const int *rowptr,
                     const int *jk, const void *val, const void *dense, int NA, void *force, cudaStream_t s);
 int k_force_hopping_adj(const Geo &g, int prec, int N, const void *eta, const void *xi, const void *links_fund, void *force, cudaStream_t s);
 // number of distinct kernel launches k_hop issues for this configuration (for launch accounting): always 1.
