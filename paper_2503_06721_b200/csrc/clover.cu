@@ -16,6 +16,7 @@
 // Kernels: clover_field_kernel -- a CTA per (part of a) tile, the plaquette leaves as path products W_d1(x) W_d2(x+d1) ... out of
 // the gather-layout links (W_d = U_mu(x) / U_mu(x-mu)^dagger) in shared memory; runs once per gauge update like
 // links_to_rep.  cphi_site_kernel / cphi_kernel -- out = ((4+m) + c_sw A) in, coalesced 32-lane rows (see there).
+#include "hop_ring.cuh"   // DevCache / prepare_launch (opt-in shared-memory size per device)
 #include "kernels.h"
 
 namespace hirep {
@@ -490,14 +491,21 @@ int k_cphi(int prec, int dR, int ntile, double a, double csw, const void *clover
 // One thread per site and chirality: the block is written to the thread's own column of the output buffer (coalesced
 // across lanes) and inverted there in place by Gauss-Jordan elimination without pivoting -- the blocks are Hermitian and,
 // for the parameters the operator is used with ((4+m) dominates c_sw |A|), positive definite.  Once per gauge update.
-template <typename T>
-__global__ void clover_inv_kernel(Geo g, int dR, int parity, T a, T csw, const cplx<T> *__restrict__ clover, cplx<T> *inv, int *flags) {
+// DRT > 0 (small d_R): compile-time d_R, one warp per block, the warp's 32 blocks live in SHARED memory [entry][lane] while they are
+// eliminated (each lane its own column: no exchange, no barrier) and are copied out at the end -- the same operations in the same
+// order as the in-place form, whose every elimination step is a round trip of the whole block through L2 (C2 fp64 3.4 -> 0.5 ms).
+// DRT = 0: run-time d_R, in place in global memory (blocks too large for shared memory).
+template <typename T, int DRT>
+__global__ void clover_inv_kernel(Geo g, int dR_rt, int parity, T a, T csw, const cplx<T> *__restrict__ clover, cplx<T> *inv, int *flags) {
+    const int dR = DRT > 0 ? DRT : dR_rt;
     const int n = 2 * dR, ne = dR * dR;
     const int slot = blockIdx.x * blockDim.x + threadIdx.x;      // padded site slot of the parity
     const int c = blockIdx.y;
     if (slot >= g.n_tiles * TILE) return;
     const int tile = slot >> 5, lane = slot & 31;
-    cplx<T> *M = inv + ((size_t)(tile * 2 + c) * n * n) * TILE + lane;
+    cplx<T> *G = inv + ((size_t)(tile * 2 + c) * n * n) * TILE + lane;
+    extern __shared__ __align__(16) unsigned char smem_blk[];
+    cplx<T> *M = DRT > 0 ? reinterpret_cast<cplx<T> *>(smem_blk) + (size_t)(threadIdx.x >> 5) * n * n * TILE + lane : G;
     const bool live = slot < g.Nh;
     T scale = 0;                                                  // largest |entry| of the block: the yardstick for the pivots
     for (int I = 0; I < n; ++I)
@@ -546,6 +554,8 @@ __global__ void clover_inv_kernel(Geo g, int dR, int parity, T a, T csw, const c
     }
     if (!live)
         for (int E = 0; E < n * n; ++E) M[(size_t)E * TILE] = mk<T>(0, 0);
+    if (DRT > 0)
+        for (int E = 0; E < n * n; ++E) G[(size_t)E * TILE] = M[(size_t)E * TILE];
     if (bad && live && flags) atomicOr(flags, 1);
 }
 
@@ -666,16 +676,23 @@ int k_cblock(int prec, int dR, int ntile, const void *blk, const void *in, void 
 // (the inverse).  Per site and chirality, in the thread's own columns of global memory (S = output, X and Tm = workspace):
 // scaling and squaring, exp(Y) = (sum_{k <= K} (Y/2^s)^k / k!)^(2^s) with the sum in Horner form; s = 4, K = 14 covers
 // |x A| <= 8 to 1e-16 (truncation 0.5^15/15!) and the four squarings amplify rounding by 16 ulp.
-template <typename T>
-__global__ void clover_exp_kernel(Geo g, int dR, int parity, T x, T pref, const cplx<T> *__restrict__ clover, cplx<T> *blocks, cplx<T> *work, int *flags) {
+// DRT > 0: compile-time d_R, one warp per block, S, X and the product buffer in shared memory (as clover_inv_kernel; the copy of
+// every product back into S is replaced by swapping the two buffers); DRT = 0: run-time d_R in global-memory columns.
+template <typename T, int DRT>
+__global__ void clover_exp_kernel(Geo g, int dR_rt, int parity, T x, T pref, const cplx<T> *__restrict__ clover, cplx<T> *blocks, cplx<T> *work, int *flags) {
     constexpr int SQ = 4, K = 14;
+    const int dR = DRT > 0 ? DRT : dR_rt;
     const int n = 2 * dR, ne = dR * dR;
     const int slot = blockIdx.x * blockDim.x + threadIdx.x;
     const int c = blockIdx.y;
     if (slot >= g.n_tiles * TILE) return;
     const int tile = slot >> 5, lane = slot & 31;
     const size_t off = ((size_t)(tile * 2 + c) * n * n) * TILE + lane;
-    cplx<T> *S = blocks + off, *X = work + off, *Tm = work + (size_t)g.n_tiles * 2 * n * n * TILE + off;
+    extern __shared__ __align__(16) unsigned char smem_blk[];
+    cplx<T> *const sm = reinterpret_cast<cplx<T> *>(smem_blk) + (size_t)(threadIdx.x >> 5) * 3 * n * n * TILE + lane;
+    cplx<T> *const G = blocks + off;
+    cplx<T> *S = DRT > 0 ? sm : G, *X = DRT > 0 ? sm + (size_t)n * n * TILE : work + off;
+    cplx<T> *Tm = DRT > 0 ? sm + (size_t)2 * n * n * TILE : work + (size_t)g.n_tiles * 2 * n * n * TILE + off;
     const bool live = slot < g.Nh;
     const T sc = x / T(1 << SQ);
     T norm = 0;                                                   // inf-norm of x A_c: the series below is accurate for <= 8
@@ -702,39 +719,97 @@ __global__ void clover_exp_kernel(Geo g, int dR, int parity, T x, T pref, const 
     if (live && flags && (!(norm <= T(8)) )) atomicOr(flags, 2);   // also catches NaN
     for (int k = K; k >= 1; --k) {            // S <- 1 + (X S)/k
         const T rk = T(1) / T(k);
-        for (int I = 0; I < n; ++I)
+        for (int I = 0; I < n; ++I) {
+            cplx<T> xr[DRT > 0 ? 2 * DRT : 1];     // shared-memory form: row I of the left factor in registers (one load per MAC instead of two)
+            if (DRT > 0) {
+#pragma unroll
+                for (int l = 0; l < 2 * DRT; ++l) xr[l] = X[(size_t)(I * n + l) * TILE];
+            }
             for (int J = 0; J < n; ++J) {
                 cplx<T> a = mk<T>(0, 0);
-                for (int l = 0; l < n; ++l) cfma<T>(a, X[(size_t)(I * n + l) * TILE], S[(size_t)(l * n + J) * TILE]);
+#pragma unroll
+                for (int l = 0; l < (DRT > 0 ? 2 * DRT : n); ++l) cfma<T>(a, DRT > 0 ? xr[DRT > 0 ? l : 0] : X[(size_t)(I * n + l) * TILE], S[(size_t)(l * n + J) * TILE]);
                 Tm[(size_t)(I * n + J) * TILE] = mk<T>(a.x * rk + (I == J ? T(1) : T(0)), a.y * rk);
             }
-        for (int E = 0; E < n * n; ++E) S[(size_t)E * TILE] = Tm[(size_t)E * TILE];
+        }
+        if (DRT > 0) { cplx<T> *t_ = S; S = Tm; Tm = t_; }
+        else for (int E = 0; E < n * n; ++E) S[(size_t)E * TILE] = Tm[(size_t)E * TILE];
     }
     for (int q = 0; q < SQ; ++q) {            // S <- S S
-        for (int I = 0; I < n; ++I)
+        for (int I = 0; I < n; ++I) {
+            cplx<T> xr[DRT > 0 ? 2 * DRT : 1];
+            if (DRT > 0) {
+#pragma unroll
+                for (int l = 0; l < 2 * DRT; ++l) xr[l] = S[(size_t)(I * n + l) * TILE];
+            }
             for (int J = 0; J < n; ++J) {
                 cplx<T> a = mk<T>(0, 0);
-                for (int l = 0; l < n; ++l) cfma<T>(a, S[(size_t)(I * n + l) * TILE], S[(size_t)(l * n + J) * TILE]);
+#pragma unroll
+                for (int l = 0; l < (DRT > 0 ? 2 * DRT : n); ++l) cfma<T>(a, DRT > 0 ? xr[DRT > 0 ? l : 0] : S[(size_t)(I * n + l) * TILE], S[(size_t)(l * n + J) * TILE]);
                 Tm[(size_t)(I * n + J) * TILE] = a;
             }
-        for (int E = 0; E < n * n; ++E) S[(size_t)E * TILE] = Tm[(size_t)E * TILE];
+        }
+        if (DRT > 0) { cplx<T> *t_ = S; S = Tm; Tm = t_; }
+        else for (int E = 0; E < n * n; ++E) S[(size_t)E * TILE] = Tm[(size_t)E * TILE];
     }
     for (int E = 0; E < n * n; ++E) {
         const cplx<T> v = S[(size_t)E * TILE];
-        S[(size_t)E * TILE] = live ? mk<T>(pref * v.x, pref * v.y) : mk<T>(0, 0);
+        G[(size_t)E * TILE] = live ? mk<T>(pref * v.x, pref * v.y) : mk<T>(0, 0);
     }
 }
+// shared-memory form where >= 2 warps' worth of matrices fit an SM (bytes per warp: nbuf x (2 d_R)^2 x 32 lanes x element)
+template <typename T, int DRT> static int clover_exp_sm(const Geo &g, int parity, double x, double pref, const void *clover, void *blocks, void *work, int *flags, cudaStream_t s) {
+    auto kern = clover_exp_kernel<T, DRT>;
+    const size_t smem = (size_t)3 * 4 * DRT * DRT * TILE * sizeof(cplx<T>);
+    static DevCache cache{};
+    int n_sm = 0;
+    if (const int rc = prepare_launch(kern, smem, cache, n_sm)) return rc;
+    kern<<<dim3(g.n_tiles, 2), 32, smem, s>>>(g, DRT, parity, (T)x, (T)pref, (const cplx<T> *)clover, (cplx<T> *)blocks, (cplx<T> *)work, flags);
+    return (int)cudaGetLastError();
+}
 template <typename T> static int clover_exp_t(const Geo &g, int dR, int parity, double x, double pref, const void *clover, void *blocks, void *work, int *flags, cudaStream_t s) {
-    clover_exp_kernel<T><<<dim3((g.n_tiles * TILE + 63) / 64, 2), 64, 0, s>>>(g, dR, parity, (T)x, (T)pref, (const cplx<T> *)clover, (cplx<T> *)blocks,
-                                                                           (cplx<T> *)work, flags);
+    static const int glob = getenv("HIREP_CLOVER_GLOBAL") ? atoi(getenv("HIREP_CLOVER_GLOBAL")) : 0;   // measurement switch: the in-place global-memory form
+    if (!glob && (size_t)3 * 4 * dR * dR * TILE * sizeof(cplx<T>) <= 112 * 1024) {
+        switch (dR) {
+        case 1: return clover_exp_sm<T, 1>(g, parity, x, pref, clover, blocks, work, flags, s);
+        case 2: return clover_exp_sm<T, 2>(g, parity, x, pref, clover, blocks, work, flags, s);
+        case 3: return clover_exp_sm<T, 3>(g, parity, x, pref, clover, blocks, work, flags, s);
+        case 4: return clover_exp_sm<T, 4>(g, parity, x, pref, clover, blocks, work, flags, s);
+        case 5: if constexpr (sizeof(T) == 4) return clover_exp_sm<T, 5>(g, parity, x, pref, clover, blocks, work, flags, s); break;
+        case 6: if constexpr (sizeof(T) == 4) return clover_exp_sm<T, 6>(g, parity, x, pref, clover, blocks, work, flags, s); break;
+        }
+    }
+    clover_exp_kernel<T, 0><<<dim3((g.n_tiles * TILE + 63) / 64, 2), 64, 0, s>>>(g, dR, parity, (T)x, (T)pref, (const cplx<T> *)clover, (cplx<T> *)blocks,
+                                                                              (cplx<T> *)work, flags);
     return (int)cudaGetLastError();
 }
 int k_clover_exp(const Geo &g, int prec, int dR, int parity, double x, double pref, const void *clover, void *blocks, void *work, int *flags, cudaStream_t s) {
     return prec == 0 ? clover_exp_t<double>(g, dR, parity, x, pref, clover, blocks, work, flags, s) : clover_exp_t<float>(g, dR, parity, x, pref, clover, blocks, work, flags, s);
 }
 
+template <typename T, int DRT> static int clover_inv_sm(const Geo &g, int parity, double a, double csw, const void *clover, void *inv, int *flags, cudaStream_t s) {
+    auto kern = clover_inv_kernel<T, DRT>;
+    const size_t smem = (size_t)4 * DRT * DRT * TILE * sizeof(cplx<T>);
+    static DevCache cache{};
+    int n_sm = 0;
+    if (const int rc = prepare_launch(kern, smem, cache, n_sm)) return rc;
+    kern<<<dim3(g.n_tiles, 2), 32, smem, s>>>(g, DRT, parity, (T)a, (T)csw, (const cplx<T> *)clover, (cplx<T> *)inv, flags);
+    return (int)cudaGetLastError();
+}
 template <typename T> static int clover_inv_t(const Geo &g, int dR, int parity, double a, double csw, const void *clover, void *inv, int *flags, cudaStream_t s) {
-    clover_inv_kernel<T><<<dim3((g.n_tiles * TILE + 63) / 64, 2), 64, 0, s>>>(g, dR, parity, (T)a, (T)csw, (const cplx<T> *)clover, (cplx<T> *)inv, flags);
+    static const int glob = getenv("HIREP_CLOVER_GLOBAL") ? atoi(getenv("HIREP_CLOVER_GLOBAL")) : 0;
+    if (!glob && (size_t)4 * dR * dR * TILE * sizeof(cplx<T>) <= 112 * 1024) {
+        switch (dR) {
+        case 1: return clover_inv_sm<T, 1>(g, parity, a, csw, clover, inv, flags, s);
+        case 2: return clover_inv_sm<T, 2>(g, parity, a, csw, clover, inv, flags, s);
+        case 3: return clover_inv_sm<T, 3>(g, parity, a, csw, clover, inv, flags, s);
+        case 4: return clover_inv_sm<T, 4>(g, parity, a, csw, clover, inv, flags, s);
+        case 5: return clover_inv_sm<T, 5>(g, parity, a, csw, clover, inv, flags, s);
+        case 6: return clover_inv_sm<T, 6>(g, parity, a, csw, clover, inv, flags, s);
+        case 8: return clover_inv_sm<T, 8>(g, parity, a, csw, clover, inv, flags, s);
+        }
+    }
+    clover_inv_kernel<T, 0><<<dim3((g.n_tiles * TILE + 63) / 64, 2), 64, 0, s>>>(g, dR, parity, (T)a, (T)csw, (const cplx<T> *)clover, (cplx<T> *)inv, flags);
     return (int)cudaGetLastError();
 }
 int k_clover_inv(const Geo &g, int prec, int dR, int parity, double a, double csw, const void *clover, void *inv, int *flags, cudaStream_t s) {
