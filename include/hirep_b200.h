@@ -102,6 +102,15 @@ int hirep_halo_unpack(hirep_geom *g, int face, void *spinor_half, const void *bu
 int hirep_geom_set_bc(hirep_geom *g, const int sign[4]);
 /* cuda_stream: a cudaStream_t / CUstream (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream */
 int hirep_geom_set_stream(hirep_geom *g, void *cuda_stream);
+/* Workspaces are allocated (cudaMalloc, zeroed once) by the first call that needs them -- which therefore must not sit inside a
+ * CUDA-graph capture or any other region where allocation is forbidden.  hirep_geom_reserve allocates them now instead:
+ *   HIREP_RESERVE_OPERATORS  the intermediate spinor fields of the two-pass operators (Dphi_hat, g5Dphi_sq, the clover / block /
+ *                            twisted-mass forms and their squares) and the device flag word: 5 half-lattice spinors
+ *   HIREP_RESERVE_SOLVERS    the reduction buffers and the work fields of the CGs and BiCGstab (5 full-lattice spinors), the pinned
+ *                            host scalars (the multi-shift CG's per-shift fields and hirep_apply_host's staging stay lazy)
+ * Flags may be or-ed.  Idempotent.  Errors: HIREP_EINVAL (flags), HIREP_ENOMEM, HIREP_ECUDA.  (hirep_Dphi_hat_static needs none.) */
+enum { HIREP_RESERVE_OPERATORS = 1, HIREP_RESERVE_SOLVERS = 2 };
+int hirep_geom_reserve(hirep_geom *g, int what);
 /* Bytes of native buffers (any pointer may be NULL): full- and half-lattice spinor, fundamental links,
  * represented links; d_R (Tbl 1); rep_is_real = 1 iff represented links are stored as real numbers (ADJ). */
 int hirep_geom_sizes(const hirep_geom *g, size_t *spinor_full, size_t *spinor_half, size_t *links_fund,

@@ -342,6 +342,36 @@ static int workspace(void **slot, size_t bytes) {
     return HIREP_OK;
 }
 
+// Allocate (and zero) now what the operator / solver entry points would otherwise allocate on their first call, so that a first call
+// may already sit inside a CUDA-graph capture or any region where cudaMalloc is not allowed (lazy allocation).
+extern "C" int hirep_geom_reserve(hirep_geom *g, int what) {
+    if (!g) return fail(HIREP_EINVAL, "hirep_geom_reserve: NULL geometry");
+    if (wrong_device(g)) return fail(HIREP_EINVAL, "hirep_geom_reserve: the geometry was created on CUDA device %d, which is not the current device", g->device);
+    if (what <= 0 || (what & ~(HIREP_RESERVE_OPERATORS | HIREP_RESERVE_SOLVERS))) return fail(HIREP_EINVAL, "hirep_geom_reserve: flags %d", what);
+    int rc = HIREP_OK;
+    const size_t hb = g->bytes_spinor_half;
+    if (what & HIREP_RESERVE_OPERATORS) {
+        if ((rc = workspace(&g->ws_half, hb)) || (rc = workspace(&g->ws_half2, hb)) || (rc = workspace(&g->ws_half3, hb)) ||
+            (rc = workspace(&g->ws_full, 2 * hb)) || (rc = workspace((void **)&g->dev_flags, 64)))
+            return rc;
+    }
+    if (what & HIREP_RESERVE_SOLVERS) {
+        if ((rc = workspace(&g->ws_red, (size_t)k_reduce_workspace_bytes() + 64)) || (rc = workspace(&g->ws_red2, (size_t)k_reduce_workspace_bytes())) ||
+            (rc = workspace(&g->cg_r, 2 * hb)) || (rc = workspace(&g->cg_p, 2 * hb)) || (rc = workspace(&g->cg_Ap, 2 * hb)) ||
+            (rc = workspace(&g->bi_s, 2 * hb)) || (rc = workspace(&g->bi_t, 2 * hb)))
+            return rc;
+        if (!g->h_scal) {
+            cudaError_t e = cudaHostAlloc((void **)&g->h_scal, 8 * sizeof(double), cudaHostAllocDefault);
+            if (e != cudaSuccess) { g->h_scal = nullptr; return cuda_fail(e, "hirep_geom_reserve"); }
+            if ((e = cudaEventCreateWithFlags(&g->ev_scal, cudaEventDisableTiming)) != cudaSuccess) {
+                cudaFreeHost(g->h_scal); g->h_scal = nullptr;
+                return cuda_fail(e, "hirep_geom_reserve");
+            }
+        }
+    }
+    return HIREP_OK;
+}
+
 static int offdiag(hirep_geom *g, void *out, const void *in, const void *links, int p_out, const char *what) {
     HopLaunch L{};
     L.nsets = 1;

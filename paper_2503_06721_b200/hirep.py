@@ -23,11 +23,12 @@ OP_DPHI, OP_DPHI_EO, OP_DPHI_OE, OP_DPHI_HAT, OP_G5DPHI_SQ = 0, 1, 2, 3, 4
 TUNE_MAX_CTAS, TUNE_SUM_ALGORITHM, TUNE_PACE_WINDOW, TUNE_FUSE_DIAG = 1, 2, 3, 4
 REGION_ALL, REGION_OWNED, REGION_INTERIOR, REGION_BOUNDARY = 0, 1, 2, 3
 STATIC_SCRATCH_BYTES = 16 << 20   # HIREP_STATIC_SCRATCH_BYTES
+RESERVE_OPERATORS, RESERVE_SOLVERS = 1, 2
 OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM, EBREAKDOWN = 0, -1, -2, -3, -4, -5
 
 # every symbol include/hirep_b200.h declares
 SYMBOLS = [
-    "hirep_geom_create", "hirep_geom_destroy", "hirep_geom_set_bc", "hirep_geom_set_stream", "hirep_geom_sizes",
+    "hirep_geom_create", "hirep_geom_destroy", "hirep_geom_set_bc", "hirep_geom_set_stream", "hirep_geom_sizes", "hirep_geom_reserve",
     "hirep_spinor_import", "hirep_spinor_export", "hirep_links_import", "hirep_links_rep_export",
     "hirep_links_rep_export_bwd", "hirep_links_to_rep", "hirep_Dphi", "hirep_Dphi_eo", "hirep_Dphi_oe",
     "hirep_Dphi_hat", "hirep_Dphi_hat_static", "hirep_g5Dphi_sq", "hirep_g5Dphi_hat", "hirep_g5Dphi_hat_sq", "hirep_cg_g5Dphi_hat_sq", "hirep_set_link_mode", "hirep_set_kernel_variant", "hirep_set_tuning", "hirep_launch_count",
@@ -72,6 +73,7 @@ def load():
     lib.hirep_geom_destroy.argtypes = [vp]
     lib.hirep_geom_set_bc.argtypes = [vp, ctypes.POINTER(ci)]
     lib.hirep_geom_set_stream.argtypes = [vp, vp]
+    lib.hirep_geom_reserve.argtypes = [vp, ci]
     lib.hirep_geom_sizes.argtypes = [vp] + [ctypes.POINTER(ctypes.c_size_t)] * 4 + [ctypes.POINTER(ci)] * 2
     for n in ("hirep_spinor_import", "hirep_spinor_export"):
         getattr(lib, n).argtypes = [vp, vp, vp, ci]
@@ -172,6 +174,10 @@ def hirep_geom_destroy(g):
 
 def hirep_geom_set_bc(g, sign):
     _check(load().hirep_geom_set_bc(g, (ctypes.c_int * 4)(*[int(s) for s in sign])))
+
+
+def hirep_geom_reserve(g, what):
+    _check(load().hirep_geom_reserve(g, int(what)))
 
 
 def hirep_geom_set_stream(g, cuda_stream):
@@ -705,6 +711,7 @@ class Geometry:
     def set_link_mode(self, mode): hirep_set_link_mode(self.handle, mode)
     def set_kernel_variant(self, v): hirep_set_kernel_variant(self.handle, v)
     def set_tuning(self, key, value): hirep_set_tuning(self.handle, key, value)
+    def reserve(self, what=RESERVE_OPERATORS | RESERVE_SOLVERS): hirep_geom_reserve(self.handle, what)
     def set_bc(self, sign): hirep_geom_set_bc(self.handle, sign)
     def sync(self): hirep_sync(self.handle)
     def launch_count(self): return hirep_launch_count(self.handle)

@@ -120,6 +120,16 @@ def test_new_entry_points_argument_errors_without_gpu(hirep):
     with pytest.raises(hirep.HirepError):
         hirep.hirep_set_tuning(g, 99, 1)
     with pytest.raises(hirep.HirepError):
+        hirep.hirep_set_tuning(g, hirep.TUNE_FUSE_DIAG, 2)
+    hirep.hirep_set_tuning(g, hirep.TUNE_FUSE_DIAG, 0)
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_geom_reserve(g, 0)                                     # no flag
+    with pytest.raises(hirep.HirepError):
+        hirep.hirep_geom_reserve(g, 8)                                     # unknown flag
+    with pytest.raises(hirep.HirepError) as ei:
+        hirep.hirep_geom_reserve(g, hirep.RESERVE_OPERATORS)               # no device here: an error, not a silent success
+    assert ei.value.rc in (hirep.ECUDA, hirep.ENOMEM)
+    with pytest.raises(hirep.HirepError):
         hirep.hirep_set_tuning(g, hirep.TUNE_MAX_CTAS, -2)
     hirep.hirep_set_tuning(g, hirep.TUNE_MAX_CTAS, 4)
     with pytest.raises(hirep.HirepError):

@@ -152,3 +152,48 @@ def test_cuda_graph_capture_and_replay(env):
             graph.replay()
         s.synchronize()
         assert torch.equal(ye, ref_e) and torch.equal(yf, ref_f)
+
+
+def test_reserve_then_first_call_inside_capture(env):
+    """hirep_geom_reserve allocates the workspaces up front: the FIRST Dphi_hat / g5Dphi_sq / Dphi_clover_hat of a geometry may then
+    be issued inside a CUDA-graph capture (no cudaMalloc in the call); the replayed results equal those of a second, eagerly used
+    geometry bit for bit."""
+    torch, hirep = env["torch"], env["hirep"]
+    cfg = synth.CONFIGS["C2"].resized(4, 6)
+    U, (psi,) = synth.make_inputs(cfg)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        outs = []
+        for captured in (False, True):
+            g = hirep.Geometry(cfg.T, cfg.L, cfg.n_g, cfg.rep, "f64", device=env["dev"])
+            lf = g.links_import(torch.from_numpy(U).to(env["dev"]))
+            lr = g.links_to_rep(lf)
+            x = g.spinor_import(torch.from_numpy(psi).to(env["dev"]))
+            cl = g.clover_field(lr)
+            inv = g.clover_inv_field(cfg.m0, 0.5, hirep.ODD, cl)
+            hb = g.sizes["spinor_half"]
+            ye, yf, yc = g.new_spinor(hirep.EVEN), g.new_spinor(hirep.FULL), g.new_spinor(hirep.EVEN)
+
+            def step():
+                g.Dphi_hat(cfg.m0, x[:hb], lr, out=ye)
+                g.g5Dphi_sq(cfg.m0, x, lr, out=yf)
+                g.Dphi_clover_hat(cfg.m0, 0.5, x[:hb], lr, cl, inv, out=yc)
+
+            if captured:
+                g.reserve(hirep.RESERVE_OPERATORS)
+                g.reserve(hirep.RESERVE_OPERATORS | hirep.RESERVE_SOLVERS)      # idempotent
+                s.synchronize()
+                graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(graph, stream=s):
+                    step()
+                graph.replay()
+            else:
+                step()
+            s.synchronize()
+            # canonical export: the padding lanes of the ragged last tile (13.5 tiles per parity) are never written and hold whatever
+            # torch.empty returned
+            outs.append((g.spinor_export(ye, hirep.EVEN), g.spinor_export(yf, hirep.FULL), g.spinor_export(yc, hirep.EVEN)))
+        for a, b in zip(*outs):
+            assert torch.equal(a, b) and bool(torch.isfinite(a.real).all()) and float(a.abs().max()) > 0
+    with pytest.raises(hirep.HirepError):
+        g.reserve(0)
