@@ -622,7 +622,7 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
         ms = timeit(lambda: geom.force_hopping(x_full, z_full, lr, out=fbuf), reps=10)
         by = (2 * S + 4 * cm["K"] + 4 * na * w) * V
         out["force_hopping"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3),
-                                "note": "compulsory bytes (2S + 4K + 4(N^2-1)w) per site; d_R <= 4 (fp32: 6): one warp per tile walks the four mu, M in registers; else one warp per (tile, mu), vectors in shared memory"}
+                                "note": "compulsory bytes (2S + 4K + 4(N^2-1)w) per site; d_R <= 4 (fp32: 6): one warp per tile walks the four mu, M in registers; fp64 d_R = 5, 6: two warps per tile; d_R >= 8: one warp per (tile, mu), vectors in shared memory"}
         del fbuf
     except Exception as e:
         out["force_hopping"] = {"error": str(e)}
