@@ -110,13 +110,16 @@ def test_fused_form_every_instantiation(env, n, rep, T, L, prec, variant):
     assert oracle.rel_l2(p.to_numpy(out, hirep.EVEN), oc.Dphi_expclover_hat(T, L, m0, 0.8, p.R, psi[p.ev], BC)) < tol
 
 
-def test_fused_form_g5_squares_and_cg(env):
+@pytest.mark.parametrize("name,T,L,prec", [("C2", 4, 6, "f64"), ("C4", 4, 4, "f64"), ("C3", 4, 4, "f64"), ("C4", 4, 4, "f32"), ("C2", 4, 4, "f32")])
+def test_fused_form_g5_squares_and_cg(env, name, T, L, prec):
     """(gamma_5 D_clover)^2 and the even-odd (gamma_5 D_hat)^2 run on the fused passes (2 resp. 4 launches) and agree with the
-    composed forms to rounding; the clover CGs converge to the same solution in both forms."""
+    composed forms to rounding; the clover CGs -- whose two reductions then ride in the epilogues of those passes (ring kernel: C2,
+    C3 with real links, C4 in fp32; pair kernel: C4 in fp64) -- converge to the same solution in both forms."""
     hirep, oracle = env["hirep"], env["oracle"]
-    cfg = synth.CONFIGS["C2"].resized(4, 6)
-    p = Problem(env, cfg, "f64")
+    cfg = synth.CONFIGS[name].resized(T, L)
+    p = Problem(env, cfg, prec)
     g, m0 = p.geom, 0.3
+    tol, cg_tol, sol_tol = (1e-13, 1e-10, 1e-7) if prec == "f64" else (1e-5, 1e-5, 2e-3)
     cl = g.clover_field(p.links_rep)
     inv_odd = g.clover_inv_field(m0, 0.6, hirep.ODD, cl)
     psi = p.spinors[0]
@@ -131,13 +134,21 @@ def test_fused_form_g5_squares_and_cg(env):
         out, n = launches(g, lambda: g.g5Dphi_clover_hat_sq(m0, 0.6, xe, p.links_rep, cl, inv_odd))
         assert n == (4 if fuse else 8)
         res[("hat_sq", fuse)] = p.to_numpy(out, hirep.EVEN)
-        sol, it, rel = g.cg_g5Dphi_clover_sq(m0, 0.6, x, p.links_rep, cl, 1e-10, 500)
-        assert rel < 1e-10
+        sol, it, rel = g.cg_g5Dphi_clover_sq(m0, 0.6, x, p.links_rep, cl, cg_tol, 500)
+        assert rel <= cg_tol
         res[("cg", fuse)] = p.to_numpy(sol, hirep.FULL)
-        sol, it, rel = g.cg_g5Dphi_clover_hat_sq(m0, 0.6, xe, p.links_rep, cl, inv_odd, 1e-10, 500)
-        assert rel < 1e-10
+        res[("cg_it", fuse)] = it
+        sol, it, rel = g.cg_g5Dphi_clover_hat_sq(m0, 0.6, xe, p.links_rep, cl, inv_odd, cg_tol, 500)
+        assert rel <= cg_tol
         res[("cg_hat", fuse)] = p.to_numpy(sol, hirep.EVEN)
-    assert oracle.rel_l2(res[("sq", 1)], res[("sq", 0)]) < 1e-13
-    assert oracle.rel_l2(res[("hat_sq", 1)], res[("hat_sq", 0)]) < 1e-13
-    assert oracle.rel_l2(res[("cg", 1)], res[("cg", 0)]) < 1e-7
-    assert oracle.rel_l2(res[("cg_hat", 1)], res[("cg_hat", 0)]) < 1e-7
+        res[("cg_hat_it", fuse)] = it
+    assert oracle.rel_l2(res[("sq", 1)], res[("sq", 0)]) < tol
+    assert oracle.rel_l2(res[("hat_sq", 1)], res[("hat_sq", 0)]) < tol
+    assert oracle.rel_l2(res[("cg", 1)], res[("cg", 0)]) < sol_tol
+    assert oracle.rel_l2(res[("cg_hat", 1)], res[("cg_hat", 0)]) < sol_tol
+    assert abs(res[("cg_it", 1)] - res[("cg_it", 0)]) <= 2 and abs(res[("cg_hat_it", 1)] - res[("cg_hat_it", 0)]) <= 2
+    # true residual of the fused solution through the composed operator
+    g.set_tuning(hirep.TUNE_FUSE_DIAG, 0)
+    Ax = p.to_numpy(g.g5Dphi_clover_hat_sq(m0, 0.6, p.to_native(res[("cg_hat", 1)], hirep.EVEN), p.links_rep, cl, inv_odd), hirep.EVEN)
+    b = psi[p.ev]
+    assert np.linalg.norm((Ax - b).ravel()) < 20 * cg_tol * np.linalg.norm(b.ravel())
