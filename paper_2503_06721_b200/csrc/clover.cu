@@ -419,6 +419,116 @@ __global__ void __launch_bounds__(128) clover_field_site_kernel(Geo g, const lin
         }
     }
 }
+// d_R = 4, 5, 6: the register scheme of clover_field_site_kernel with the ROWS of every matrix split over the NS warps of a CTA
+// (CTA = one tile, lane = site, warp w = rows w RP .. w RP + RP - 1).  A path product P <- P W needs, for the rows a thread owns,
+// only those rows of P and the whole of W: every element of W is loaded once (coalesced, straight from L1 / L2 -- the NS warps of
+// the CTA and the 12 leaves of neighbouring sites that use the same link hit there) and feeds RP complex MACs from registers; no
+// shared-memory staging of the matrices at all (the shared-memory kernel above is bound by its two loads per MAC: 10 % of the FP32
+// peak at d_R = 6).  Only C^+ in F = (C - C^+)/8 needs the other warps' rows: one exchange of the leaf sum per plane.
+template <typename T, bool REAL, int DR, int NS, int MB>
+__global__ void __launch_bounds__(32 * NS, MB) clover_field_rows_kernel(Geo g, const link_elem<T, REAL> *__restrict__ links, cplx<T> *__restrict__ clover) {
+    static_assert(DR % NS == 0, "the rows must split evenly over the warps");
+    constexpr int NE = DR * DR, RP = DR / NS, NR = RP * DR;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx<T> *exch = reinterpret_cast<cplx<T> *>(smem_raw) + (threadIdx.x & 31);      // leaf sum C of the tile, [e][lane]
+    const int lane = threadIdx.x & 31, r0 = (threadIdx.x >> 5) * RP;
+    const int p = blockIdx.x / g.n_tiles, tile = blockIdx.x - p * g.n_tiles;
+    const int hp = tile * TILE + lane;
+    const bool live = hp < g.Nh;
+    const int h = live ? hp : g.Nh - 1;
+    int t0, x0, y0, zh0;
+    decode_site(g, h, t0, x0, y0, zh0);
+    const int z0 = 2 * zh0 + ((t0 + x0 + y0 + p) & 1);
+    cplx<T> acc0[NR], acc1[NR];
+    cplx<T> *dst = clover + clover_off(g.n_tiles, p, tile, 0, 0, 0, lane, NE);
+    for (int q = 0; q < 6; ++q) {
+        const int pl = (0x415032 >> (4 * q)) & 7;                  // plane order 2,3,0,5,1,4  (03,12 | 01,23 | 02,13)
+        const int mu = (0x211000 >> (4 * pl)) & 3, nu = (0x332321 >> (4 * pl)) & 3;
+        if (q == 0 || q == 2) {
+#pragma unroll
+            for (int e = 0; e < NR; ++e) acc0[e] = acc1[e] = mk<T>(0, 0);
+        }
+        cplx<T> C[NR];
+#pragma unroll
+        for (int e = 0; e < NR; ++e) C[e] = mk<T>(0, 0);
+        for (int leaf = 0; leaf < 4; ++leaf) {
+            int t = t0, x = x0, y = y0, z = z0, cp = p, ch = h;
+            cplx<T> P[NR], Q[NR];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int sq = (leaf + k) & 3;
+                const int dmu = (sq & 1) ? nu : mu, d = dmu + ((sq & 2) ? 4 : 0);
+                const link_elem<T, REAL> *W = links + link_off(g.n_tiles, cp, ch >> 5, d, 0, ch & 31, NE);
+                if (k == 0) {
+#pragma unroll
+                    for (int rr = 0; rr < RP; ++rr)
+#pragma unroll
+                        for (int j = 0; j < DR; ++j) P[rr * DR + j] = ld_w<T, REAL>(W, (size_t)((r0 + rr) * DR + j) * TILE);
+                } else {
+#pragma unroll
+                    for (int e = 0; e < NR; ++e) Q[e] = mk<T>(0, 0);
+#pragma unroll
+                    for (int l = 0; l < DR; ++l)
+#pragma unroll
+                        for (int j = 0; j < DR; ++j) {
+                            const cplx<T> w = ld_w<T, REAL>(W, (size_t)(l * DR + j) * TILE);
+#pragma unroll
+                            for (int rr = 0; rr < RP; ++rr) cfma<T>(Q[rr * DR + j], P[rr * DR + l], w);
+                        }
+#pragma unroll
+                    for (int e = 0; e < NR; ++e) P[e] = Q[e];
+                }
+                const int dl = (sq & 2) ? -1 : 1;
+                t += dmu == 0 ? dl : 0; x += dmu == 1 ? dl : 0; y += dmu == 2 ? dl : 0; z += dmu == 3 ? dl : 0;
+                t = t == g.T ? 0 : (t < 0 ? g.T - 1 : t);
+                x = x == g.L ? 0 : (x < 0 ? g.L - 1 : x);
+                y = y == g.L ? 0 : (y < 0 ? g.L - 1 : y);
+                z = z == g.L ? 0 : (z < 0 ? g.L - 1 : z);
+                ch = encode_site(g, t, x, y, z >> 1);
+                cp ^= 1;
+            }
+#pragma unroll
+            for (int e = 0; e < NR; ++e) { C[e].x += P[e].x; C[e].y += P[e].y; }
+        }
+        // the leaf sum to shared memory: row i of C^+ is column i of C, whose entries the other warps hold
+        __syncthreads();                                            // the previous plane's reads are done
+#pragma unroll
+        for (int rr = 0; rr < RP; ++rr)
+#pragma unroll
+            for (int j = 0; j < DR; ++j) exch[(size_t)((r0 + rr) * DR + j) * TILE] = C[rr * DR + j];
+        __syncthreads();
+        // F = (C - C^+)/8; (i/2) F -> K1 (planes 01, 23) or K3 (03, 12); F/2 = -i (i/2) F -> -i K2 (02, 13)
+        const T s0 = (pl == 3 || pl == 5) ? T(-1) : T(1);          // c = 0: +F01 -F23 | +F02 +F13 | +F03 -F12
+        const T s1 = (pl == 4) ? T(1) : T(-1);                     // c = 1: -F01 -F23 | -F02 +F13 | -F03 -F12
+        const bool half = (pl == 1 || pl == 4);
+#pragma unroll
+        for (int rr = 0; rr < RP; ++rr)
+#pragma unroll
+            for (int j = 0; j < DR; ++j) {
+                const cplx<T> a = C[rr * DR + j], b = exch[(size_t)(j * DR + r0 + rr) * TILE];
+                const cplx<T> F = mk<T>((a.x - b.x) * T(0.125), (a.y + b.y) * T(0.125));
+                const cplx<T> v = half ? mk<T>(T(0.5) * F.x, T(0.5) * F.y) : mk<T>(-T(0.5) * F.y, T(0.5) * F.x);
+                acc0[rr * DR + j].x += s0 * v.x; acc0[rr * DR + j].y += s0 * v.y;
+                acc1[rr * DR + j].x += s1 * v.x; acc1[rr * DR + j].y += s1 * v.y;
+            }
+        if (q == 1 || q == 5) {                                     // H (m = 0) after 03,12; B (m = 1) after all four
+            const int m = q == 1 ? 0 : 1;
+#pragma unroll
+            for (int rr = 0; rr < RP; ++rr)
+#pragma unroll
+                for (int j = 0; j < DR; ++j) {
+                    const int e = (r0 + rr) * DR + j;
+                    dst[(size_t)((0 * 2 + m) * NE + e) * TILE] = live ? acc0[rr * DR + j] : mk<T>(0, 0);
+                    dst[(size_t)((1 * 2 + m) * NE + e) * TILE] = live ? acc1[rr * DR + j] : mk<T>(0, 0);
+                }
+        }
+    }
+}
+template <typename T, bool REAL, int DR, int NS, int MB = 1> static int clover_field_rows_t(const Geo &g, void *clover, const void *links, cudaStream_t s) {
+    clover_field_rows_kernel<T, REAL, DR, NS, MB><<<2 * g.n_tiles, 32 * NS, (size_t)DR * DR * TILE * sizeof(cplx<T>), s>>>(
+        g, (const link_elem<T, REAL> *)links, (cplx<T> *)clover);
+    return (int)cudaGetLastError();
+}
 template <typename T, bool REAL, int DR> static int clover_field_site_t(const Geo &g, void *clover, const void *links, cudaStream_t s) {
     const long slots = 2L * g.n_tiles * TILE;
     clover_field_site_kernel<T, REAL, DR><<<(unsigned)((slots + 127) / 128), 128, 0, s>>>(g, (const link_elem<T, REAL> *)links, (cplx<T> *)clover);
@@ -428,6 +538,20 @@ template <typename T, bool REAL, int DR> static int clover_field_site_t(const Ge
 template <typename T, bool REAL> static int clover_field_t(const Geo &g, int dR, void *clover, const void *links, cudaStream_t s) {
     if (dR == 2) return clover_field_site_t<T, REAL, 2>(g, clover, links, s);
     if (dR == 3) return clover_field_site_t<T, REAL, 3>(g, clover, links, s);
+    static const int smk = getenv("HIREP_CLOVER_FIELD_SMEM") ? atoi(getenv("HIREP_CLOVER_FIELD_SMEM")) : 0;   // measurement switch: the shared-memory kernel
+    if (!REAL && !smk) {   // d_R = 4, 5, 6 are complex representations; rows per thread chosen for <= ~180 registers
+        if constexpr (!REAL) {
+            constexpr bool F32 = sizeof(T) == 4;
+            if (dR == 4) return clover_field_rows_t<T, false, 4, 2>(g, clover, links, s);
+            if (dR == 5) return clover_field_rows_t<T, false, 5, 5>(g, clover, links, s);
+            // d_R = 6: fp32 two warps x 3 rows; fp64 six warps x 1 row at two CTAs per SM (three warps x 2 rows need 255 registers: 36.7 vs 24.2 ms
+            // for SU(3) SYM on 32^4; the shared-memory kernel: 40.4 ms)
+            if (dR == 6) {
+                if constexpr (F32) return clover_field_rows_t<T, false, 6, 2, 1>(g, clover, links, s);
+                else return clover_field_rows_t<T, false, 6, 6, 2>(g, clover, links, s);
+            }
+        }
+    }
     constexpr int LP = 1;
     const int ne = dR * dR;
     const size_t per_site = (size_t)(6 * LP + 5) * ne * sizeof(cplx<T>);
