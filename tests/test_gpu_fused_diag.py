@@ -152,3 +152,44 @@ def test_fused_form_g5_squares_and_cg(env, name, T, L, prec):
     Ax = p.to_numpy(g.g5Dphi_clover_hat_sq(m0, 0.6, p.to_native(res[("cg_hat", 1)], hirep.EVEN), p.links_rep, cl, inv_odd), hirep.EVEN)
     b = psi[p.ev]
     assert np.linalg.norm((Ax - b).ravel()) < 20 * cg_tol * np.linalg.norm(b.ravel())
+
+
+def test_full_size_fused_clover_C4_f64(env):
+    """The 2-index BASELINE config at full size (SU(4) 2AS, 96 x 48^3, fp64), bench launch configuration: Dphi_clover through the pair
+    kernel's fused epilogue (one launch) at sampled sites incl. the lattice corners.  The clover term at x only involves links in
+    the 3^4 neighbourhood of x: the oracle runs, as it stands, on that neighbourhood cut out as a 3 x 3^3 lattice and is read at the
+    centre; the hopping term comes from the sampled oracle of the Wilson tests (tests/gpu_helpers.py).  (The block export of
+    tests/test_gpu_clover.py::test_full_size_clover_sampled would not fit beside the 49 GB of links here.)"""
+    import itertools
+    from oracle import clover as oc
+    from tests.gpu_helpers import SampledOracle, coords_of, index_of, sample_sites, torch_field_fetch
+    from tests.test_gpu_parity import full_size_problem
+    torch, hirep, oracle = env["torch"], env["hirep"], env["oracle"]
+    cfg, geom, links, psi, lr = full_size_problem(env, "C4", "f64")
+    so = SampledOracle(oracle, cfg, links)
+    fetch = torch_field_fetch(psi)
+    tol, m0, csw, d = TOL["f64"], cfg.m0, 1.3, cfg.d_R
+    ext = np.array([cfg.T, cfg.L, cfg.L, cfg.L])
+    cl = geom.clover_field(lr)
+    x = geom.spinor_import(psi, hirep.FULL)
+    y, n = launches(geom, lambda: geom.Dphi_clover(m0, csw, x, lr, cl))
+    assert n == 1
+    out_d = geom.spinor_export(y, hirep.FULL)
+    del y, x
+    centre = index_of((1, 1, 1, 1), 3)
+    num = den = 0.0
+    for ix in sample_sites(cfg, 8, seed=11):
+        c = coords_of(ix, cfg.T, cfg.L)
+        idx = [index_of((c + np.array(off) - 1) % ext, cfg.L) for off in itertools.product(range(3), repeat=4)]
+        Up = links[torch.tensor(idx, device=links.device)].cpu().numpy().astype(np.complex128)          # [81,4,N,N]
+        Rp = np.array([[oracle.rep_matrix(cfg.n_g, cfg.rep, Up[s, mu]) for mu in range(4)] for s in range(81)])
+        pp = np.zeros((81, 4, d), dtype=np.complex128)
+        pp[centre] = fetch(ix)
+        want = oc.Cphi(3, 3, m0, csw, Rp, pp)[centre] + so.hop(fetch, ix)
+        got = out_d[ix].cpu().numpy().astype(np.complex128)
+        assert np.linalg.norm(got - want) <= 10 * tol * np.linalg.norm(want), ix
+        num += float(np.sum(np.abs(got - want) ** 2)); den += float(np.sum(np.abs(want) ** 2))
+    assert np.sqrt(num / den) < tol
+    geom.sync()
+    del cl, out_d, lr, links, psi
+    torch.cuda.empty_cache()
