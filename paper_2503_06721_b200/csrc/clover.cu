@@ -881,6 +881,116 @@ __global__ void clover_exp_kernel(Geo g, int dR_rt, int parity, T x, T pref, con
         G[(size_t)E * TILE] = live ? mk<T>(pref * v.x, pref * v.y) : mk<T>(0, 0);
     }
 }
+// Row-split form (small d_R): CTA = (tile, chirality), lane = site, warp w owns the rows w RP .. of X, S and of every product.
+// A product T = L R needs the thread's rows of L (registers) and all of R: the warps publish their rows of S to ONE shared-memory
+// copy [entry][lane], and every element read from there feeds RP complex MACs -- against three full matrices per site in shared
+// memory (two warps per SM at d_R = 6 fp32) and two loads per MAC in clover_exp_kernel<T, DRT>.  Same operations in the same order
+// per entry: bit-identical results.
+template <typename T, int DR, int RP>
+__global__ void __launch_bounds__(32 * (2 * DR / RP)) clover_exp_rows_kernel(Geo g, int parity, T x, T pref, const cplx<T> *__restrict__ clover,
+                                                                            cplx<T> *blocks, int *flags) {
+    constexpr int SQ = 4, K = 14, n = 2 * DR, ne = DR * DR;
+    static_assert(n % RP == 0, "rows must split evenly");
+    extern __shared__ __align__(16) unsigned char smem_blk[];
+    const int lane = threadIdx.x & 31, r0 = (threadIdx.x >> 5) * RP;
+    const int tile = blockIdx.x, c = blockIdx.y;
+    cplx<T> *R = reinterpret_cast<cplx<T> *>(smem_blk) + lane;               // the right factor S, [I n + J][lane]
+    const bool live = tile * TILE + lane < g.Nh;
+    const T sc = x / T(1 << SQ);
+    cplx<T> X[RP][n], S[RP][n], Tm[RP][n];
+    T norm = 0;
+#pragma unroll
+    for (int rr = 0; rr < RP; ++rr) {
+        const int I = r0 + rr, bi = I / DR, i = I - bi * DR;
+        T rowsum = 0;
+#pragma unroll
+        for (int J = 0; J < n; ++J) {
+            const int bj = J / DR, j = J - bj * DR;
+            cplx<T> v;
+            if (bi == bj) {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 0, i * DR + j, lane, ne)];
+                if (bi) { v.x = -v.x; v.y = -v.y; }
+            } else if (bi == 0) {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 1, i * DR + j, lane, ne)];
+            } else {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 1, j * DR + i, lane, ne)];
+                v.y = -v.y;
+            }
+            X[rr][J] = mk<T>(sc * v.x, sc * v.y);
+            S[rr][J] = mk<T>(I == J ? T(1) : T(0), T(0));
+            rowsum += sqrt(v.x * v.x + v.y * v.y);
+        }
+        norm = fmax(norm, fabs(x) * rowsum);
+    }
+    if (live && flags && (!(norm <= T(8)))) atomicOr(flags, 2);   // a row of |x A| beyond the range of the series (also catches NaN)
+    auto publish = [&]() {
+        __syncthreads();                                            // the previous product's reads are done
+#pragma unroll
+        for (int rr = 0; rr < RP; ++rr)
+#pragma unroll
+            for (int J = 0; J < n; ++J) R[(size_t)((r0 + rr) * n + J) * TILE] = S[rr][J];
+        __syncthreads();
+    };
+    for (int k = K; k >= 1; --k) {            // S <- 1 + (X S)/k
+        const T rk = T(1) / T(k);
+        publish();
+#pragma unroll
+        for (int J = 0; J < n; ++J) {
+            cplx<T> a[RP];
+#pragma unroll
+            for (int rr = 0; rr < RP; ++rr) a[rr] = mk<T>(0, 0);
+#pragma unroll
+            for (int l = 0; l < n; ++l) {
+                const cplx<T> s = R[(size_t)(l * n + J) * TILE];
+#pragma unroll
+                for (int rr = 0; rr < RP; ++rr) cfma<T>(a[rr], X[rr][l], s);
+            }
+#pragma unroll
+            for (int rr = 0; rr < RP; ++rr) Tm[rr][J] = mk<T>(a[rr].x * rk + (r0 + rr == J ? T(1) : T(0)), a[rr].y * rk);
+        }
+#pragma unroll
+        for (int rr = 0; rr < RP; ++rr)
+#pragma unroll
+            for (int J = 0; J < n; ++J) S[rr][J] = Tm[rr][J];
+    }
+    for (int q = 0; q < SQ; ++q) {            // S <- S S
+        publish();
+#pragma unroll
+        for (int J = 0; J < n; ++J) {
+            cplx<T> a[RP];
+#pragma unroll
+            for (int rr = 0; rr < RP; ++rr) a[rr] = mk<T>(0, 0);
+#pragma unroll
+            for (int l = 0; l < n; ++l) {
+                const cplx<T> s = R[(size_t)(l * n + J) * TILE];
+#pragma unroll
+                for (int rr = 0; rr < RP; ++rr) cfma<T>(a[rr], S[rr][l], s);
+            }
+#pragma unroll
+            for (int rr = 0; rr < RP; ++rr) Tm[rr][J] = a[rr];
+        }
+#pragma unroll
+        for (int rr = 0; rr < RP; ++rr)
+#pragma unroll
+            for (int J = 0; J < n; ++J) S[rr][J] = Tm[rr][J];
+    }
+    cplx<T> *G = blocks + ((size_t)(tile * 2 + c) * n * n) * TILE + lane;
+#pragma unroll
+    for (int rr = 0; rr < RP; ++rr)
+#pragma unroll
+        for (int J = 0; J < n; ++J) G[(size_t)((r0 + rr) * n + J) * TILE] = live ? mk<T>(pref * S[rr][J].x, pref * S[rr][J].y) : mk<T>(0, 0);
+}
+template <typename T, int DR> static int clover_exp_rows(const Geo &g, int parity, double x, double pref, const void *clover, void *blocks, int *flags, cudaStream_t s) {
+    constexpr int RP = (sizeof(T) == 4 || DR <= 3) ? 2 : 1;
+    auto kern = clover_exp_rows_kernel<T, DR, RP>;
+    const size_t smem = (size_t)4 * DR * DR * TILE * sizeof(cplx<T>);
+    static DevCache cache{};
+    int n_sm = 0;
+    if (const int rc = prepare_launch(kern, smem, cache, n_sm)) return rc;
+    kern<<<dim3(g.n_tiles, 2), 32 * (2 * DR / RP), smem, s>>>(g, parity, (T)x, (T)pref, (const cplx<T> *)clover, (cplx<T> *)blocks, flags);
+    return (int)cudaGetLastError();
+}
+
 // shared-memory form where >= 2 warps' worth of matrices fit an SM (bytes per warp: nbuf x (2 d_R)^2 x 32 lanes x element)
 template <typename T, int DRT> static int clover_exp_sm(const Geo &g, int parity, double x, double pref, const void *clover, void *blocks, void *work, int *flags, cudaStream_t s) {
     auto kern = clover_exp_kernel<T, DRT>;
@@ -892,8 +1002,17 @@ template <typename T, int DRT> static int clover_exp_sm(const Geo &g, int parity
     return (int)cudaGetLastError();
 }
 template <typename T> static int clover_exp_t(const Geo &g, int dR, int parity, double x, double pref, const void *clover, void *blocks, void *work, int *flags, cudaStream_t s) {
-    static const int glob = getenv("HIREP_CLOVER_GLOBAL") ? atoi(getenv("HIREP_CLOVER_GLOBAL")) : 0;   // measurement switch: the in-place global-memory form
-    if (!glob && (size_t)3 * 4 * dR * dR * TILE * sizeof(cplx<T>) <= 112 * 1024) {
+    static const int glob = getenv("HIREP_CLOVER_GLOBAL") ? atoi(getenv("HIREP_CLOVER_GLOBAL")) : 0;   // measurement switch: 1 = the in-place global-memory form,
+    if (glob == 0) {                                                                                      // 2 = the per-site shared-memory form
+        switch (dR) {
+        case 2: return clover_exp_rows<T, 2>(g, parity, x, pref, clover, blocks, flags, s);
+        case 3: return clover_exp_rows<T, 3>(g, parity, x, pref, clover, blocks, flags, s);
+        case 4: return clover_exp_rows<T, 4>(g, parity, x, pref, clover, blocks, flags, s);
+        case 5: return clover_exp_rows<T, 5>(g, parity, x, pref, clover, blocks, flags, s);
+        case 6: return clover_exp_rows<T, 6>(g, parity, x, pref, clover, blocks, flags, s);
+        }
+    }
+    if (glob != 1 && (size_t)3 * 4 * dR * dR * TILE * sizeof(cplx<T>) <= 112 * 1024) {
         switch (dR) {
         case 1: return clover_exp_sm<T, 1>(g, parity, x, pref, clover, blocks, work, flags, s);
         case 2: return clover_exp_sm<T, 2>(g, parity, x, pref, clover, blocks, work, flags, s);
