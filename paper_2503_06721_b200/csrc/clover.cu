@@ -1030,6 +1030,97 @@ int k_clover_exp(const Geo &g, int prec, int dR, int parity, double x, double pr
     return prec == 0 ? clover_exp_t<double>(g, dR, parity, x, pref, clover, blocks, work, flags, s) : clover_exp_t<float>(g, dR, parity, x, pref, clover, blocks, work, flags, s);
 }
 
+// Row-split Gauss-Jordan (d_R = 2 ... 6): CTA = (tile, chirality), lane = site, warp w holds the rows w RP .. of the block in registers.
+// Step k: the warp that owns row k scales it and publishes it to shared memory ([J][lane], double-buffered over k: one barrier per
+// step); every warp then eliminates column k from its own rows -- one shared-memory read per RP complex MACs, no global or shared
+// round trips of the block.  The same operations per entry as clover_inv_kernel: bit-identical inverse and the same pivot flag.
+template <typename T, int DR, int RP>
+__global__ void __launch_bounds__(32 * (2 * DR / RP)) clover_inv_rows_kernel(Geo g, int parity, T a, T csw, const cplx<T> *__restrict__ clover, cplx<T> *inv,
+                                                                            int *flags) {
+    constexpr int n = 2 * DR, ne = DR * DR, NW = n / RP;
+    static_assert(n % RP == 0, "rows must split evenly");
+    extern __shared__ __align__(16) unsigned char smem_blk[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, r0 = warp * RP;
+    const int tile = blockIdx.x, c = blockIdx.y;
+    cplx<T> *rowk = reinterpret_cast<cplx<T> *>(smem_blk) + lane;              // [2][n][lane]
+    T *smax = reinterpret_cast<T *>(smem_blk + (size_t)2 * n * TILE * sizeof(cplx<T>)) + lane;   // [NW][lane]
+    const bool live = tile * TILE + lane < g.Nh;
+    cplx<T> M[RP][n];
+    T scale = 0;
+#pragma unroll
+    for (int rr = 0; rr < RP; ++rr) {
+        const int I = r0 + rr, bi = I / DR, i = I - bi * DR;
+#pragma unroll
+        for (int J = 0; J < n; ++J) {
+            const int bj = J / DR, j = J - bj * DR;
+            cplx<T> v;
+            if (bi == bj) {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 0, i * DR + j, lane, ne)];
+                if (bi) { v.x = -v.x; v.y = -v.y; }
+            } else if (bi == 0) {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 1, i * DR + j, lane, ne)];
+            } else {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 1, j * DR + i, lane, ne)];
+                v.y = -v.y;
+            }
+            v.x *= csw; v.y *= csw;
+            if (I == J) v.x += a;
+            if (!live) v = mk<T>(I == J ? T(1) : T(0), T(0));
+            M[rr][J] = v;
+            scale = fmax(scale, fmax(fabs(v.x), fabs(v.y)));
+        }
+    }
+    smax[(size_t)warp * TILE] = scale;                              // the yardstick for the pivots is the block's largest entry
+    __syncthreads();
+#pragma unroll
+    for (int w = 0; w < NW; ++w) scale = fmax(scale, smax[(size_t)w * TILE]);
+    const T tiny = scale * (sizeof(T) == 8 ? T(1e-10) : T(1e-4));
+    bool bad = false;
+    static_for<0, n>([&](auto kc) {
+        constexpr int k = decltype(kc)::value, kw = k / RP, kk = k % RP;
+        cplx<T> *pub = rowk + (size_t)(k & 1) * n * TILE;
+        if (warp == kw) {
+            const cplx<T> d = M[kk][k];
+            const T d2 = d.x * d.x + d.y * d.y;
+            if (!(d2 > tiny * tiny) || !isfinite(d2)) bad = true;
+            const T r = T(1) / d2;
+            const cplx<T> p = mk<T>(d.x * r, -d.y * r);
+            M[kk][k] = mk<T>(1, 0);
+#pragma unroll
+            for (int J = 0; J < n; ++J) {
+                M[kk][J] = cmul<T>(M[kk][J], p);
+                pub[(size_t)J * TILE] = M[kk][J];
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int rr = 0; rr < RP; ++rr) {
+            if (!(warp == kw && rr == kk)) {
+                const cplx<T> f = M[rr][k];
+                M[rr][k] = mk<T>(0, 0);
+#pragma unroll
+                for (int J = 0; J < n; ++J) {
+                    const cplx<T> x = pub[(size_t)J * TILE];
+                    M[rr][J].x -= f.x * x.x - f.y * x.y;
+                    M[rr][J].y -= f.x * x.y + f.y * x.x;
+                }
+            }
+        }
+    });
+    cplx<T> *G = inv + ((size_t)(tile * 2 + c) * n * n) * TILE + lane;
+#pragma unroll
+    for (int rr = 0; rr < RP; ++rr)
+#pragma unroll
+        for (int J = 0; J < n; ++J) G[(size_t)((r0 + rr) * n + J) * TILE] = live ? M[rr][J] : mk<T>(0, 0);
+    if (bad && live && flags) atomicOr(flags, 1);
+}
+template <typename T, int DR> static int clover_inv_rows(const Geo &g, int parity, double a, double csw, const void *clover, void *inv, int *flags, cudaStream_t s) {
+    constexpr int RP = 2, n = 2 * DR;
+    clover_inv_rows_kernel<T, DR, RP><<<dim3(g.n_tiles, 2), 32 * (n / RP), (size_t)2 * n * TILE * sizeof(cplx<T>) + (size_t)(n / RP) * TILE * sizeof(T), s>>>(
+        g, parity, (T)a, (T)csw, (const cplx<T> *)clover, (cplx<T> *)inv, flags);
+    return (int)cudaGetLastError();
+}
+
 template <typename T, int DRT> static int clover_inv_sm(const Geo &g, int parity, double a, double csw, const void *clover, void *inv, int *flags, cudaStream_t s) {
     auto kern = clover_inv_kernel<T, DRT>;
     const size_t smem = (size_t)4 * DRT * DRT * TILE * sizeof(cplx<T>);
@@ -1040,8 +1131,17 @@ template <typename T, int DRT> static int clover_inv_sm(const Geo &g, int parity
     return (int)cudaGetLastError();
 }
 template <typename T> static int clover_inv_t(const Geo &g, int dR, int parity, double a, double csw, const void *clover, void *inv, int *flags, cudaStream_t s) {
-    static const int glob = getenv("HIREP_CLOVER_GLOBAL") ? atoi(getenv("HIREP_CLOVER_GLOBAL")) : 0;
-    if (!glob && (size_t)4 * dR * dR * TILE * sizeof(cplx<T>) <= 112 * 1024) {
+    static const int glob = getenv("HIREP_CLOVER_GLOBAL") ? atoi(getenv("HIREP_CLOVER_GLOBAL")) : 0;   // 1 = in place in global memory, 2 = per-site shared-memory form
+    if (glob == 0) {
+        switch (dR) {
+        case 2: return clover_inv_rows<T, 2>(g, parity, a, csw, clover, inv, flags, s);
+        case 3: return clover_inv_rows<T, 3>(g, parity, a, csw, clover, inv, flags, s);
+        case 4: return clover_inv_rows<T, 4>(g, parity, a, csw, clover, inv, flags, s);
+        case 5: return clover_inv_rows<T, 5>(g, parity, a, csw, clover, inv, flags, s);
+        case 6: return clover_inv_rows<T, 6>(g, parity, a, csw, clover, inv, flags, s);
+        }
+    }
+    if (glob != 1 && (size_t)4 * dR * dR * TILE * sizeof(cplx<T>) <= 112 * 1024) {
         switch (dR) {
         case 1: return clover_inv_sm<T, 1>(g, parity, a, csw, clover, inv, flags, s);
         case 2: return clover_inv_sm<T, 2>(g, parity, a, csw, clover, inv, flags, s);
