@@ -525,8 +525,12 @@ __global__ void __launch_bounds__(32 * NS, MB) clover_field_rows_kernel(Geo g, c
     }
 }
 template <typename T, bool REAL, int DR, int NS, int MB = 1> static int clover_field_rows_t(const Geo &g, void *clover, const void *links, cudaStream_t s) {
-    clover_field_rows_kernel<T, REAL, DR, NS, MB><<<2 * g.n_tiles, 32 * NS, (size_t)DR * DR * TILE * sizeof(cplx<T>), s>>>(
-        g, (const link_elem<T, REAL> *)links, (cplx<T> *)clover);
+    auto kern = clover_field_rows_kernel<T, REAL, DR, NS, MB>;
+    const size_t smem = (size_t)DR * DR * TILE * sizeof(cplx<T>);
+    static DevCache cache{};
+    int n_sm = 0;
+    if (const int rc = prepare_launch(kern, smem, cache, n_sm)) return rc;      // d_R = 10 in fp64 needs the opt-in size (51 KB)
+    kern<<<2 * g.n_tiles, 32 * NS, smem, s>>>(g, (const link_elem<T, REAL> *)links, (cplx<T> *)clover);
     return (int)cudaGetLastError();
 }
 template <typename T, bool REAL, int DR> static int clover_field_site_t(const Geo &g, void *clover, const void *links, cudaStream_t s) {
@@ -539,9 +543,15 @@ template <typename T, bool REAL> static int clover_field_t(const Geo &g, int dR,
     if (dR == 2) return clover_field_site_t<T, REAL, 2>(g, clover, links, s);
     if (dR == 3) return clover_field_site_t<T, REAL, 3>(g, clover, links, s);
     static const int smk = getenv("HIREP_CLOVER_FIELD_SMEM") ? atoi(getenv("HIREP_CLOVER_FIELD_SMEM")) : 0;   // measurement switch: the shared-memory kernel
-    if (!REAL && !smk) {   // d_R = 4, 5, 6 are complex representations; rows per thread chosen for <= ~180 registers
+    if (REAL && !smk) {    // SU(3) adjoint (d_R = 8, real links): two rows per thread in fp32, one in fp64
+        if constexpr (REAL) {
+            if (dR == 8) return clover_field_rows_t<T, true, 8, sizeof(T) == 4 ? 4 : 8, 1>(g, clover, links, s);
+        }
+    }
+    if (!REAL && !smk) {   // d_R = 4, 5, 6, 10 are complex representations; rows per thread chosen for <= ~200 registers
         if constexpr (!REAL) {
             constexpr bool F32 = sizeof(T) == 4;
+            if (dR == 10) return clover_field_rows_t<T, false, 10, F32 ? 5 : 10, 1>(g, clover, links, s);
             if (dR == 4) return clover_field_rows_t<T, false, 4, 2>(g, clover, links, s);
             if (dR == 5) return clover_field_rows_t<T, false, 5, 5>(g, clover, links, s);
             // d_R = 6: fp32 two warps x 3 rows; fp64 six warps x 1 row at two CTAs per SM (three warps x 2 rows need 255 registers: 36.7 vs 24.2 ms
