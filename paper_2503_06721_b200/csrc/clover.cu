@@ -1020,6 +1020,7 @@ template <typename T> static int clover_exp_t(const Geo &g, int dR, int parity, 
         case 4: return clover_exp_rows<T, 4>(g, parity, x, pref, clover, blocks, flags, s);
         case 5: return clover_exp_rows<T, 5>(g, parity, x, pref, clover, blocks, flags, s);
         case 6: return clover_exp_rows<T, 6>(g, parity, x, pref, clover, blocks, flags, s);
+        case 8: if constexpr (sizeof(T) == 4) return clover_exp_rows<T, 8>(g, parity, x, pref, clover, blocks, flags, s); break;   // fp64: 3 x 2 x 16 complex doubles per thread do not fit
         }
     }
     if (glob != 1 && (size_t)3 * 4 * dR * dR * TILE * sizeof(cplx<T>) <= 112 * 1024) {
@@ -1149,6 +1150,8 @@ template <typename T> static int clover_inv_t(const Geo &g, int dR, int parity, 
         case 4: return clover_inv_rows<T, 4>(g, parity, a, csw, clover, inv, flags, s);
         case 5: return clover_inv_rows<T, 5>(g, parity, a, csw, clover, inv, flags, s);
         case 6: return clover_inv_rows<T, 6>(g, parity, a, csw, clover, inv, flags, s);
+        case 8: return clover_inv_rows<T, 8>(g, parity, a, csw, clover, inv, flags, s);
+        case 10: if constexpr (sizeof(T) == 4) return clover_inv_rows<T, 10>(g, parity, a, csw, clover, inv, flags, s); break;   // fp64: the unrolled elimination spills (ptxas: 52 KB)
         }
     }
     if (glob != 1 && (size_t)4 * dR * dR * TILE * sizeof(cplx<T>) <= 112 * 1024) {
