@@ -253,7 +253,9 @@ int hirep_cg_g5Dphi_hat_sq(hirep_geom *g, double m0, void *x_even, const void *b
  *   hirep_spinor_g5_lc  xi = c1 eta + c2 gamma_5 eta             (gamma_5-fused linear combination, L447; xi may alias eta)
  *   hirep_Dphi_tm       out = D_m in + i mu gamma_5 in           (Eq 51 for the tau^3 = +1 flavour; -mu gives the other)
  *   hirep_Dphi_tm_sq    out = (D^tm)^dagger D^tm in = gamma_5 D^tm(-mu) gamma_5 D^tm(mu) in   (Hermitian positive definite)
- *   hirep_Dphi_tm_hat   out_even = D_ee in_even - D_eo D_oo^{-1} D_oe in_even, D_ee = D_oo = (4+m) + i mu gamma_5  (Eq 43) */
+ *   hirep_Dphi_tm_hat   out_even = D_ee in_even - D_eo D_oo^{-1} D_oe in_even, D_ee = D_oo = (4+m) + i mu gamma_5  (Eq 43); two stencil
+ *                       launches: D_oo^{-1} = ((4+m) - i mu gamma_5)/((4+m)^2 + mu^2) is applied in the epilogue of the D_oe pass, D_ee in that
+ *                       of the D_eo pass (kernel variants 1, 2: a separate gamma_5 combination in between) */
 int hirep_spinor_g5_lc(hirep_geom *g, int which, void *xi, const double c1[2], const double c2[2], const void *eta);
 /* gamma matrix application (Eq 34): xi = gamma_mu eta, mu = 0..3 in the basis of Eq 1-3, mu = 5 for gamma_5; xi != eta */
 int hirep_spinor_gamma(hirep_geom *g, int which, int mu, void *xi, const void *eta);

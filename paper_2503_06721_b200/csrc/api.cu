@@ -581,10 +581,20 @@ extern "C" int hirep_Dphi_tm_hat(hirep_geom *g, double m0, double mu, void *out_
     if (out_even == in_even) return fail(HIREP_EINVAL, "hirep_Dphi_tm_hat: out aliases in");
     int rc = workspace(&g->ws_half, g->bytes_spinor_half);
     if (rc) return rc;
-    if ((rc = offdiag(g, g->ws_half, in_even, links, 1, "hirep_Dphi_tm_hat (D_oe pass)"))) return rc;
     const double a = 4.0 + m0, den = a * a + mu * mu;
-    const double c1[2] = {a / den, 0.0}, c2[2] = {0.0, -mu / den};
-    if ((rc = hirep_spinor_g5_lc(g, HIREP_ODD, g->ws_half, c1, c2, g->ws_half))) return rc;
+    // D_oo^-1 = (a - i mu gamma_5)/(a^2 + mu^2) multiplies the hop sum of the D_oe pass: in the epilogue of that pass (kernel variants 0, 3, 4:
+    // the persistent kernels), else as a separate gamma_5 linear combination
+    if (g->variant == 0 || g->variant == 3 || g->variant == 4) {
+        HopLaunch L1{};
+        L1.nsets = 1;
+        L1.set[0] = HopSet{in_even, g->ws_half, nullptr, links_parity(g, links, 1), 1};
+        L1.a = 0.0; L1.b = -0.5 * a / den; L1.bi = 0.5 * mu / den;
+        if ((rc = hop(g, L1, "hirep_Dphi_tm_hat (D_oo^-1 D_oe pass)"))) return rc;
+    } else {
+        if ((rc = offdiag(g, g->ws_half, in_even, links, 1, "hirep_Dphi_tm_hat (D_oe pass)"))) return rc;
+        const double c1[2] = {a / den, 0.0}, c2[2] = {0.0, -mu / den};
+        if ((rc = hirep_spinor_g5_lc(g, HIREP_ODD, g->ws_half, c1, c2, g->ws_half))) return rc;
+    }
     HopLaunch L{};
     L.nsets = 1;
     L.set[0] = HopSet{g->ws_half, out_even, in_even, links_parity(g, links, 0), 0};

@@ -64,7 +64,7 @@ __global__ void __launch_bounds__(AdjMfCfg<T, N>::WARPS * 32, 1) hop_adjmf_kerne
     const long n_groups_set = (g.Nh + SPW - 1) / SPW;
     const long n_groups = n_groups_set * L.nsets;
     const long gw = (long)blockIdx.x * Cfg::WARPS + warp, nw = (long)gridDim.x * Cfg::WARPS;
-    const T a = (T)L.a, b = (T)L.b, am = (T)L.am;
+    const T a = (T)L.a, b = (T)L.b, bi = (T)L.bi, am = (T)L.am;
     const T g5s = L.g5 ? T(-1) : T(1);
 
     for (long grp = gw; grp < n_groups; grp += nw) {
@@ -267,6 +267,10 @@ __global__ void __launch_bounds__(AdjMfCfg<T, N>::WARPS * 32, 1) hop_adjmf_kerne
                     const int aa = r + N * m;
                     if (aa < DR) {
                         C v = mk<T>(b * res[sp][m].x, b * res[sp][m].y);
+                        if (bi != T(0)) {   // (b + i bi gamma_5) hop
+                            const T bs = sp < 2 ? bi : -bi;
+                            v = mk<T>(fma(-bs, res[sp][m].y, v.x), fma(bs, res[sp][m].x, v.y));
+                        }
                         if (use_self) {
                             const C sv = self[(size_t)(sp * DR + aa) * TILE];
                             const T tm = sp < 2 ? am : -am;                                        // + i mu gamma_5 self (Eq 51)

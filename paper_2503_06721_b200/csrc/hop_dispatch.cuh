@@ -44,6 +44,7 @@ template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int
     // 0.130 -> 0.119 ms in fp32, in bursts; on par under a sustained power-capped load), the real SU(2) adjoint in fp64 (C3: 0.98 -> 0.89 ms) and
     // complex links at d_R = 4, 6 in fp32 (C4: 4.91 -> 4.47 ms; SU(3) SYM 32^4 0.47 -> 0.34 ms; d_R = 5 has only one-row chunks and loses).  In fp64 at d_R >= 4 (half-spinor split over 4 warps: C4 10.7 vs 10.3 ms) and for real
     // links in fp32 the gather-layout kernels are faster; variant 5 forces it anywhere.
+    if (L.bi != 0.0 && variant != 0 && variant != 3 && variant != 4 && variant != 5) return KERR_UNSUPPORTED;   // direct-load kernels: no gamma_5 factor on the hop sum
     if (hop_full_eligible(L) && (variant == 5 || (variant == 0 && hop_full_default<T, DR, REAL>()))) return launch_hop_full<T, DR, REAL>(g, L, s);
     // the fused reductions exist in the tile-pair kernel and in the persistent ring / pair kernels (variants 0, 3, 4)
     if (L.red_mode != 0 && variant != 0 && variant != 3 && variant != 4) return KERR_UNSUPPORTED;
@@ -70,7 +71,7 @@ template <typename T, int DR, bool REAL> int hop_small_variant(const Geo &g, int
 template <typename T, int DR, bool REAL, int R, int TP> int hop_large_variant(const Geo &g, int variant, const HopLaunch &L, cudaStream_t s) {
     if (L.red_mode != 0 || L.diag_mode != DIAG_NONE) return KERR_UNSUPPORTED;
     if (variant == 0) return launch_hop_rows<T, DR, REAL, R, TP>(g, L, s);
-    if (variant == 1 && L.tile_end == 0) return launch_hop_large<T, DR, REAL, R>(g, L, s);
+    if (variant == 1 && L.tile_end == 0 && L.bi == 0.0) return launch_hop_large<T, DR, REAL, R>(g, L, s);
     return KERR_UNSUPPORTED;
 }
 

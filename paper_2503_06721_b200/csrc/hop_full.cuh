@@ -625,7 +625,7 @@ template <typename T, int DR, bool REAL> struct FullPick {
 // of the clover passes, whose self field is the output)
 inline bool hop_full_eligible(const HopLaunch &L) {
     return L.nsets == 2 && L.set[0].p_out == 0 && L.set[1].p_out == 1 && L.set[0].self == L.set[1].in && L.set[1].self == L.set[0].in &&
-           L.b != 0.0 && L.tile_end == 0 && L.diag_mode == DIAG_NONE;
+           L.b != 0.0 && L.tile_end == 0 && L.diag_mode == DIAG_NONE && L.bi == 0.0;
 }
 // would a full-lattice launch of this instantiation run hop_full by default?  (the fused CG asks before it relies on the epilogue hooks)
 template <typename T, int DR, bool REAL> constexpr bool hop_full_default() {

@@ -183,7 +183,7 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
     fetch(neighbour<dir_of<true>(0)>(g, p_out, t, x, y, zh), DirInfo<dir_of<true>(0)>::swap);
     int q = 0, slot = 0;
     uint32_t phase = 0;
-    const T a = (T)L.a, b = (T)L.b;
+    const T a = (T)L.a, b = (T)L.b, bi = (T)L.bi;
     const T am = (T)L.am;
     const T g5s = L.g5 ? T(-1) : T(1);
 
@@ -402,7 +402,10 @@ __global__ void __launch_bounds__(PAIRS * 64, 1) hop_pair_kernel(const Geo g, co
             for (int c = 0; c < DR; ++c) {
                 C vu, vl;
                 if constexpr (DIAG != DIAG_NONE) { vu = up[c]; vl = ls[c]; }
-                else { vu = mk<T>(b * up[c].x, b * up[c].y); vl = mk<T>(b * ls[c].x, b * ls[c].y); }
+                else if (bi != T(0)) {   // (b + i bi gamma_5) hop
+                    vu = mk<T>(fma(-bi, up[c].y, b * up[c].x), fma(bi, up[c].x, b * up[c].y));
+                    vl = mk<T>(fma(bi, ls[c].y, b * ls[c].x), fma(-bi, ls[c].x, b * ls[c].y));
+                } else { vu = mk<T>(b * up[c].x, b * up[c].y); vl = mk<T>(b * ls[c].x, b * ls[c].y); }
                 if constexpr (SELF && DIAG == DIAG_NONE) {
                     const C su = selfbuf[(s * DR + c) * TILE + lane];
                     const C sl = selfbuf[((2 + s) * DR + c) * TILE + lane];

@@ -237,7 +237,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
     fetch(neighbour<dir_of<IL>(0)>(g, p_out, t, x, y, zh));
     int q = 0, slot = 0;
     uint32_t phase = 0;
-    const T a = (T)L.a, b = (T)L.b;
+    const T a = (T)L.a, b = (T)L.b, bi = (T)L.bi;
     const T am = (T)L.am;
     const T g5s = L.g5 ? T(-1) : T(1);
 
@@ -398,7 +398,10 @@ __global__ void __launch_bounds__(WARPS * 32, 1) hop_ring_kernel(const Geo g, co
                 for (int c = 0; c < DR; ++c) {
                     C vu, vl;
                     if constexpr (DIAG != DIAG_NONE) { vu = up[s][c]; vl = lo[s][c]; }
-                    else { vu = mk<T>(b * up[s][c].x, b * up[s][c].y); vl = mk<T>(b * lo[s][c].x, b * lo[s][c].y); }
+                    else if (bi != T(0)) {   // (b + i bi gamma_5) hop: gamma_5 = +1 on the upper, -1 on the lower components
+                        vu = mk<T>(fma(-bi, up[s][c].y, b * up[s][c].x), fma(bi, up[s][c].x, b * up[s][c].y));
+                        vl = mk<T>(fma(bi, lo[s][c].y, b * lo[s][c].x), fma(-bi, lo[s][c].x, b * lo[s][c].y));
+                    } else { vu = mk<T>(b * up[s][c].x, b * up[s][c].y); vl = mk<T>(b * lo[s][c].x, b * lo[s][c].y); }
                     if constexpr (SELF && DIAG == DIAG_NONE) {
                         const C su = selfbuf[(s * DR + c) * TILE + lane];
                         const C sl = selfbuf[((2 + s) * DR + c) * TILE + lane];

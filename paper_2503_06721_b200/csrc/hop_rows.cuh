@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
     fetch(neighbour<dir_of<false>(0)>(g, p_out, t, x, y, zh));
     int q = 0, slot = 0;
     uint32_t phase = 0;
-    const T a = (T)L.a, b = (T)L.b;
+    const T a = (T)L.a, b = (T)L.b, bi = (T)L.bi;
     const T am = (T)L.am;
     const T g5s = L.g5 ? T(-1) : T(1);
 
@@ -234,6 +234,10 @@ __global__ void __launch_bounds__(32 * (DR / R) * TP, 1) hop_rows_kernel(const G
                     const int i = i0 + r;
                     C vu = mk<T>(b * up[s][r].x, b * up[s][r].y);
                     C vl = mk<T>(b * lo[s][r].x, b * lo[s][r].y);
+                    if (bi != T(0)) {   // (b + i bi gamma_5) hop
+                        vu = mk<T>(fma(-bi, up[s][r].y, vu.x), fma(bi, up[s][r].x, vu.y));
+                        vl = mk<T>(fma(bi, lo[s][r].y, vl.x), fma(-bi, lo[s][r].x, vl.y));
+                    }
                     if (use_self) {
                         const C su = self[(size_t)(s * DR + i) * TILE];
                         const C sl = self[(size_t)((2 + s) * DR + i) * TILE];

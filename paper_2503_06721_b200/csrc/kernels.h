@@ -27,6 +27,8 @@ struct HopLaunch {
     HopSet set[2];
     int nsets;          // 1 = half lattice, 2 = both parities in one launch
     double a, b;
+    double bi;          // the hop sum is scaled by (b + i bi gamma_5): D_oo^-1 = (a - i mu gamma_5)/(a^2 + mu^2) of the twisted-mass Schur form (Eq 43, 51)
+                        // fused into the D_oe pass; ring / pair / row-group / matrix-free adjoint kernels, 0 elsewhere
     double am;          // twisted mass mu: the diagonal term is (a + i am gamma_5) self (Eq 51); 0 = plain Wilson
     int g5;             // multiply the result by gamma_5 = diag(1,1,-1,-1)
     int diag_mode;      // DIAG_*: site-diagonal matrices HopSet::diag applied in the epilogue (ring / pair kernels, stored links)

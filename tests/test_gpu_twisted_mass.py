@@ -69,6 +69,36 @@ def test_twisted_mass_rebuild_mode_and_persistent_grid(env):
     assert oracle.rel_l2(p.to_numpy(p.geom.Dphi_tm_hat(cfg.m0, mu, xe, p.links_fund), hirep.EVEN), ref) < 1e-13
 
 
+def test_twisted_mass_schur_form_fused_and_fallback(env):
+    """Dphi_tm_hat applies D_oo^-1 = (a - i mu gamma_5)/(a^2 + mu^2) in the epilogue of its D_oe pass (2 launches) on the persistent
+    kernels -- here also the matrix-free adjoint (C5 in link mode REBUILD) and the explicit variants 3, 4 -- and falls back to the separate
+    gamma_5 combination (3 launches) on the direct-load kernels (variants 1, 2)."""
+    hirep, oracle = env["hirep"], env["oracle"]
+    mu = -0.7
+    cfg = synth.CONFIGS["C5"].resized(2, 4)
+    p = Problem(env, cfg, "f64")
+    psi = p.spinors[0]
+    ref = oracle.Dphi_tm_hat(cfg.T, cfg.L, cfg.d_R, cfg.m0, mu, p.R, psi[p.ev], BC)
+    xe = p.to_native(psi[p.ev], hirep.EVEN)
+    p.geom.set_link_mode(hirep.LINKS_REBUILD)
+    n0 = p.geom.launch_count()
+    y = p.geom.Dphi_tm_hat(cfg.m0, mu, xe, p.links_fund)
+    assert p.geom.launch_count() - n0 == 2
+    assert oracle.rel_l2(p.to_numpy(y, hirep.EVEN), ref) < 1e-13
+    for prec in ("f64", "f32"):
+        cfg = synth.CONFIGS["C2"].resized(4, 6)
+        p = Problem(env, cfg, prec)
+        psi = p.spinors[0]
+        ref = oracle.Dphi_tm_hat(cfg.T, cfg.L, cfg.d_R, cfg.m0, mu, p.R, psi[p.ev], BC)
+        xe = p.to_native(psi[p.ev], hirep.EVEN)
+        for variant, nl in ((0, 2), (3, 2), (4, 2), (1, 3), (2, 3)):
+            p.geom.set_kernel_variant(variant)
+            n0 = p.geom.launch_count()
+            y = p.geom.Dphi_tm_hat(cfg.m0, mu, xe, p.links_rep)
+            assert p.geom.launch_count() - n0 == nl, (prec, variant)
+            assert oracle.rel_l2(p.to_numpy(y, hirep.EVEN), ref) < TOL[prec], (prec, variant)
+
+
 def test_twisted_mass_cg(env):
     """CG on (D^tm)^dag D^tm: the twist lifts the spectrum by mu^2, so the solve needs fewer iterations than mu = 0;
     solution against the oracle's CG and the true residual through the oracle operator."""
