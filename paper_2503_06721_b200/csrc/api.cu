@@ -1042,7 +1042,8 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
     // epilogue carries the same two reductions.
     const bool plain = !twisted && !clover && !blocks_even && !inv_odd;
     const bool diag = !twisted && !plain;
-    const bool fused = plain ? (full ? fused_cg_ok(g) : fused_cg_eo_ok(g)) : (diag && fuse_diag(g) && fused_cg_eo_ok(g));
+    // Twisted mass ((D^tm)^dagger D^tm = [gamma_5 D^tm(-mu)] [gamma_5 D^tm(mu)], full lattice): the same two passes with +-mu in the epilogues.
+    const bool fused = plain ? (full ? fused_cg_ok(g) : fused_cg_eo_ok(g)) : twisted ? (full && fused_cg_ok(g)) : (diag && fuse_diag(g) && fused_cg_eo_ok(g));
     const int nred = k_reduce_workspace_bytes() / (int)(2 * 3 * sizeof(double));   // Acc pairs the partial buffer holds
     void *Bp_f = nullptr;   // B p of the fused form
     if (fused) {
@@ -1053,6 +1054,7 @@ static int cg_solve(hirep_geom *g, int full, double m0, void *x, const void *b, 
     }
     // one application of B with the reduction `fr` in the epilogue of its last launch
     auto apply_B = [&](void *out, const void *in, const FusedRed *fr) -> int {
+        if (twisted) return dphi_full(g, m0, out, in, links, 1, what, fr->mode == 1 ? mu : -mu, fr);   // pass 1: gamma_5 D^tm(mu), pass 2: gamma_5 D^tm(-mu)
         if (inv_odd) return blocks_hat(g, m0, csw, out, in, links, clover, blocks_even, inv_odd, 1, what, fr);
         if (blocks_even) return dphi_blocks(g, out, in, links, blocks_even, 1, what, fr);
         if (clover) return dphi_clover(g, m0, csw, out, in, links, clover, 1, what, fr);

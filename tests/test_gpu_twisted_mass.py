@@ -117,6 +117,18 @@ def test_twisted_mass_cg(env):
     assert np.linalg.norm((b - A(x)).ravel()) < 1e-9 * np.linalg.norm(b.ravel())
     _, it0, _ = p.geom.cg_g5Dphi_sq(m0, p.to_native(b, hirep.FULL), p.links_rep, 1e-10, 3000)
     assert it < it0
+    # the solve above ran with the reductions in the stencil epilogues (tile-pair kernel, 5 launches per iteration); the explicit
+    # ring variant runs the separate reduction kernels (7): same solution
+    n0 = p.geom.launch_count()
+    p.geom.cg_Dphi_tm_sq(m0, mu, p.to_native(b, hirep.FULL), p.links_rep, 1e-30, 4)
+    fused_launches = p.geom.launch_count() - n0
+    p.geom.set_kernel_variant(3)
+    n0 = p.geom.launch_count()
+    p.geom.cg_Dphi_tm_sq(m0, mu, p.to_native(b, hirep.FULL), p.links_rep, 1e-30, 4)
+    assert p.geom.launch_count() - n0 > fused_launches
+    xs3, it3, res3 = p.geom.cg_Dphi_tm_sq(m0, mu, p.to_native(b, hirep.FULL), p.links_rep, 1e-10, 3000)
+    assert res3 <= 1e-10 and abs(it3 - it) <= 2
+    assert oracle.rel_l2(p.to_numpy(xs3, hirep.FULL), x) < 1e-7
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
