@@ -269,6 +269,12 @@ def sweep_config(torch, hirep, synth, dev, name, prec, rebuild, peak, variant=0,
         out["ops"][k] = row
     ck = sampler.stop()
     out["clocks"] = {"sm_mhz": ck.get("sm_mhz"), "reasons": ck.get("reasons")}   # sustained back-to-back load: the power cap shows here
+    if own and not rebuild:   # the clover term per configuration (the headline configuration has the full block in next1_linalg_cg)
+        try:
+            out["clover"] = measure_clover(torch, hirep, fields.geom, cfg, prec, cm, cfg.m0, fields.x[0], fields.y[0], fields.lr, peak, light=True)
+        except Exception as e:
+            out["clover"] = {"error": "%s: %s" % (type(e).__name__, e)}
+            torch.cuda.empty_cache()
     if own:
         del fields
         torch.cuda.empty_cache()
@@ -482,6 +488,98 @@ def sweep_bytes(cfg, prec, rebuild):
     return V * (8 * KF + (0 if rebuild else 8 * K) + 4 * KF + (2 * NSETS + 3) * S) + (2 << 30)
 
 
+def measure_clover(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, peak, light=False):
+    """NEXT-2: clover set-up kernels and operators on resident fields.  light: the per_config form (no CG, no exponential clover)."""
+    V, S, d = cfg.volume, cm["S"], cfg.d_R
+    iters = 20
+
+    def timeit(fn, reps=20):
+        fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    out = {}
+    # NEXT-2, second part: clover term (Eq 47-49).  Algorithmic bytes per site: clover field 4 d^2 complex + spinor in/out.
+    d = cfg.d_R
+    cb = S * d                                          # clover bytes per site: 4 d^2 complex (S = 4 d complex)
+    if torch.cuda.mem_get_info()[0] < 2 * cb * V + (4 << 30):
+        out["clover"] = {"skipped": "clover field of %.1f GB does not fit beside the resident fields" % (cb * V / 1e9)}
+    else:
+        lbytes = geom.sizes["links_rep"] / V            # represented-link bytes per site
+        cl = geom.clover_field(lr)
+        ms = timeit(lambda: geom.clover_field(lr, out=cl), reps=3)
+        out["clover_field"] = {"ms": round(ms, 3), "note": "once per gauge update; 72 d_R^3 complex MACs per site out of the gather-layout links"}
+        ms = timeit(lambda: geom.Cphi(m0, 1.0, x_full, cl, out=y_full))
+        by = (cb + 2 * S) * V
+        out["Cphi"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3)}
+        # Site-diagonal matrices inside the stencil epilogues (SURVEY 8(f) row 2, "fused into the second pass") where the ring kernel carries
+        # them (stored links, d_R <= 6: ring / pair kernels), else separate block-apply launches.  Fractions are on the compulsory bytes
+        # of the fused form (every field once); the composed form moves 2S more per block application and is timed beside it.
+        fused_diag = d <= 6
+
+        def both_forms(fn, by, nl_fused, nl_composed):
+            ms = timeit(fn, reps=10)
+            r = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3),
+                 "launches": nl_fused if fused_diag else nl_composed, "fused_epilogue": bool(fused_diag)}
+            if fused_diag:
+                geom.set_tuning(hirep.TUNE_FUSE_DIAG, 0)
+                r["ms_composed"] = round(timeit(fn, reps=10), 4)
+                r["launches_composed"] = nl_composed
+                geom.set_tuning(hirep.TUNE_FUSE_DIAG, 1)
+            return r
+
+        out["Dphi_clover"] = both_forms(lambda: geom.Dphi_clover(m0, 1.0, x_full, lr, cl, out=y_full), (cb + lbytes + 2 * S) * V, 1, 2)   # in is both neighbour data and self term: 2S
+        # the Schur form Eq 43 with these blocks: block inverse (once per gauge update and mass), its application, D_hat
+        hb = geom.sizes["spinor_half"]
+        x_e, y_e = x_full[:hb], y_full[:hb]
+        inv = geom.clover_inv_field(m0, 0.5, hirep.ODD, cl)
+        ms = timeit(lambda: geom.clover_inv_field(m0, 0.5, hirep.ODD, cl, out=inv), reps=3)
+        out["clover_inv_field"] = {"ms": round(ms, 3), "note": "in-place Gauss-Jordan of the 2 d_R x 2 d_R blocks of the odd sites"}
+        ms = timeit(lambda: geom.Cphi_inv(hirep.ODD, x_e, inv, out=y_e))
+        by = (2 * cb + 2 * S) * V / 2                    # full blocks: 8 d^2 complex per site, one parity
+        out["Cphi_inv"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3)}
+        # two stencil passes (2S + 8K each) + the even input once more as the self term + inverse blocks (2 cb) + clover H, B (cb)
+        by = cm["ops"]["Dphi_eo"][1] * 2 + S * V / 2 + 3 * cb * V / 2
+        out["Dphi_clover_hat"] = both_forms(lambda: geom.Dphi_clover_hat(m0, 0.5, x_e, lr, cl, inv, out=y_e), by, 2, 4)
+        try:    # even-odd preconditioned CG with the clover term: Q_hat^2 = 2 x (the launches above), then the CG's linear algebra
+            if light:
+                raise StopIteration
+            geom.cg_g5Dphi_clover_hat_sq(m0, 0.5, x_e, lr, cl, inv, 1e-30, 2, out=y_e)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            _, it, res = geom.cg_g5Dphi_clover_hat_sq(m0, 0.5, x_e, lr, cl, inv, 1e-30, iters, out=y_e)
+            torch.cuda.synchronize()
+            ms_it = (time.perf_counter() - t0) * 1e3 / max(it, 1)
+            # fused form: the CG's reductions ride in the epilogues of the second pass of each Q_hat (r read + write, x / p update, A p never stored)
+            by_it = 2 * by + ((2 + 5 - 1) if fused_diag else (1 + 3 + 5)) * S * V / 2
+            out["cg_g5Dphi_clover_hat_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gbs": round(by_it / ms_it / 1e6, 1),
+                                              "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3), "launches_per_iteration": 7 if fused_diag else 13, "fused_reductions": bool(fused_diag),
+                                              "relres_after": res}
+        except StopIteration:
+            pass
+        except Exception as e:
+            out["cg_g5Dphi_clover_hat_sq"] = {"error": str(e)}
+        del inv
+        # exponential clover (Eq 50): full 2 d_R x 2 d_R blocks on both parities (8 d^2 complex per site)
+        if not light and d <= 10 and torch.cuda.mem_get_info()[0] > 6 * cb * V + (4 << 30):
+            nb = hirep.hirep_clover_inv_bytes(geom.handle)
+            E = geom.clover_exp_field(m0, 1.0, cl)
+            ms = timeit(lambda: hirep.hirep_clover_exp_field(geom.handle, m0, 1.0, hirep.ODD, 0, E[nb:].data_ptr(), cl.data_ptr()), reps=3)
+            out["clover_exp_field"] = {"ms": round(ms, 3), "note": "one parity; scaling and squaring, 18 block products per site and chirality"}
+            Ei = geom.clover_exp_field(m0, 1.0, cl, inverse=True)
+            out["Dphi_expclover"] = both_forms(lambda: geom.Dphi_blocks(x_full, lr, E, out=y_full), (2 * cb + lbytes + 2 * S) * V, 1, 2)
+            by = cm["ops"]["Dphi_eo"][1] * 2 + S * V / 2 + 4 * cb * V / 2
+            out["Dphi_expclover_hat"] = both_forms(lambda: geom.Dphi_blocks_hat(x_e, lr, E, Ei[nb:], out=y_e), by, 2, 4)
+            del E, Ei
+        del cl
+    return out
+
+
 def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, peak):
     """GB/s of the streaming kernels (full-lattice spinors) and ms per CG iteration of hirep_cg_g5Dphi_sq."""
     V, S, d = cfg.volume, cm["S"], cfg.d_R
@@ -545,75 +643,7 @@ def measure_extras(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, pe
     by = cm["ops"]["Dphi_hat"][1]                          # D_oo^-1 = (a - i mu gamma_5)/(a^2 + mu^2) rides in the epilogue of the D_oe pass
     out["Dphi_tm_hat"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3),
                           "gflops": round(cm["ops"]["Dphi_hat"][0] / ms / 1e6, 1), "launches": 2}
-    # NEXT-2, second part: clover term (Eq 47-49).  Algorithmic bytes per site: clover field 4 d^2 complex + spinor in/out.
-    d = cfg.d_R
-    cb = S * d                                          # clover bytes per site: 4 d^2 complex (S = 4 d complex)
-    if torch.cuda.mem_get_info()[0] < 2 * cb * V + (4 << 30):
-        out["clover"] = {"skipped": "clover field of %.1f GB does not fit beside the resident fields" % (cb * V / 1e9)}
-    else:
-        lbytes = geom.sizes["links_rep"] / V            # represented-link bytes per site
-        cl = geom.clover_field(lr)
-        ms = timeit(lambda: geom.clover_field(lr, out=cl), reps=3)
-        out["clover_field"] = {"ms": round(ms, 3), "note": "once per gauge update; 72 d_R^3 complex MACs per site out of the gather-layout links"}
-        ms = timeit(lambda: geom.Cphi(m0, 1.0, x_full, cl, out=y_full))
-        by = (cb + 2 * S) * V
-        out["Cphi"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3)}
-        # Site-diagonal matrices inside the stencil epilogues ("fused into the second pass") where the ring kernel carries
-        # them (stored links, d_R <= 6: ring / pair kernels), else separate block-apply launches.  Fractions are on the compulsory bytes
-        # of the fused form (every field once); the composed form moves 2S more per block application and is timed beside it.
-        fused_diag = d <= 6
-
-        def both_forms(fn, by, nl_fused, nl_composed):
-            ms = timeit(fn, reps=10)
-            r = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3),
-                 "launches": nl_fused if fused_diag else nl_composed, "fused_epilogue": bool(fused_diag)}
-            if fused_diag:
-                geom.set_tuning(hirep.TUNE_FUSE_DIAG, 0)
-                r["ms_composed"] = round(timeit(fn, reps=10), 4)
-                r["launches_composed"] = nl_composed
-                geom.set_tuning(hirep.TUNE_FUSE_DIAG, 1)
-            return r
-
-        out["Dphi_clover"] = both_forms(lambda: geom.Dphi_clover(m0, 1.0, x_full, lr, cl, out=y_full), (cb + lbytes + 2 * S) * V, 1, 2)   # in is both neighbour data and self term: 2S
-        # the Schur form Eq 43 with these blocks: block inverse (once per gauge update and mass), its application, D_hat
-        hb = geom.sizes["spinor_half"]
-        x_e, y_e = x_full[:hb], y_full[:hb]
-        inv = geom.clover_inv_field(m0, 0.5, hirep.ODD, cl)
-        ms = timeit(lambda: geom.clover_inv_field(m0, 0.5, hirep.ODD, cl, out=inv), reps=3)
-        out["clover_inv_field"] = {"ms": round(ms, 3), "note": "in-place Gauss-Jordan of the 2 d_R x 2 d_R blocks of the odd sites"}
-        ms = timeit(lambda: geom.Cphi_inv(hirep.ODD, x_e, inv, out=y_e))
-        by = (2 * cb + 2 * S) * V / 2                    # full blocks: 8 d^2 complex per site, one parity
-        out["Cphi_inv"] = {"ms": round(ms, 4), "gbs": round(by / ms / 1e6, 1), "frac_hbm": round(by / ms / 1e6 / peak, 3)}
-        # two stencil passes (2S + 8K each) + the even input once more as the self term + inverse blocks (2 cb) + clover H, B (cb)
-        by = cm["ops"]["Dphi_eo"][1] * 2 + S * V / 2 + 3 * cb * V / 2
-        out["Dphi_clover_hat"] = both_forms(lambda: geom.Dphi_clover_hat(m0, 0.5, x_e, lr, cl, inv, out=y_e), by, 2, 4)
-        try:    # even-odd preconditioned CG with the clover term: Q_hat^2 = 2 x (the launches above), then the CG's linear algebra
-            geom.cg_g5Dphi_clover_hat_sq(m0, 0.5, x_e, lr, cl, inv, 1e-30, 2, out=y_e)
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            _, it, res = geom.cg_g5Dphi_clover_hat_sq(m0, 0.5, x_e, lr, cl, inv, 1e-30, iters, out=y_e)
-            torch.cuda.synchronize()
-            ms_it = (time.perf_counter() - t0) * 1e3 / max(it, 1)
-            # fused form: the CG's reductions ride in the epilogues of the second pass of each Q_hat (r read + write, x / p update, A p never stored)
-            by_it = 2 * by + ((2 + 5 - 1) if fused_diag else (1 + 3 + 5)) * S * V / 2
-            out["cg_g5Dphi_clover_hat_sq"] = {"iterations": it, "ms_per_iteration": round(ms_it, 4), "gbs": round(by_it / ms_it / 1e6, 1),
-                                              "frac_hbm": round(by_it / ms_it / 1e6 / peak, 3), "launches_per_iteration": 7 if fused_diag else 13, "fused_reductions": bool(fused_diag),
-                                              "relres_after": res}
-        except Exception as e:
-            out["cg_g5Dphi_clover_hat_sq"] = {"error": str(e)}
-        del inv
-        # exponential clover (Eq 50): full 2 d_R x 2 d_R blocks on both parities (8 d^2 complex per site)
-        if d <= 10 and torch.cuda.mem_get_info()[0] > 6 * cb * V + (4 << 30):
-            nb = hirep.hirep_clover_inv_bytes(geom.handle)
-            E = geom.clover_exp_field(m0, 1.0, cl)
-            ms = timeit(lambda: hirep.hirep_clover_exp_field(geom.handle, m0, 1.0, hirep.ODD, 0, E[nb:].data_ptr(), cl.data_ptr()), reps=3)
-            out["clover_exp_field"] = {"ms": round(ms, 3), "note": "one parity; scaling and squaring, 18 block products per site and chirality"}
-            Ei = geom.clover_exp_field(m0, 1.0, cl, inverse=True)
-            out["Dphi_expclover"] = both_forms(lambda: geom.Dphi_blocks(x_full, lr, E, out=y_full), (2 * cb + lbytes + 2 * S) * V, 1, 2)
-            by = cm["ops"]["Dphi_eo"][1] * 2 + S * V / 2 + 4 * cb * V / 2
-            out["Dphi_expclover_hat"] = both_forms(lambda: geom.Dphi_blocks_hat(x_e, lr, E, Ei[nb:], out=y_e), by, 2, 4)
-            del E, Ei
-        del cl
+    out.update(measure_clover(torch, hirep, geom, cfg, prec, cm, m0, x_full, y_full, lr, peak))
     # NEXT-4: fermion force of the hopping term (Eq 20-21): both fields and the forward links once, N^2-1 reals per link out
     try:
         na = cfg.n_g ** 2 - 1
