@@ -1132,6 +1132,104 @@ template <typename T, int DR> static int clover_inv_rows(const Geo &g, int parit
     return (int)cudaGetLastError();
 }
 
+// Large d_R (blocks of 20 x 20 ... 70 x 70): one CTA per (site, chirality), thread = row, the block in shared memory [I][J] with an
+// odd row stride (conflict free for "thread I reads M[I][J]", a broadcast for the pivot row).  The per-thread form above sweeps the
+// whole block through DRAM once per pivot (2.5 MB per warp at d_R = 35: 418 ms at C5 fp64); here it is read and written once.  The
+// site's entries sit 32 elements apart in the native layout: the CTAs of neighbouring lanes run at the same time and share the
+// sectors through L2.  Same operations in the same order per entry: bit-identical inverse and pivot flag.
+template <typename T, int TPR>   // TPR threads per row, each a contiguous part of the columns (the threads of a row sit in one warp)
+__global__ void __launch_bounds__(192) clover_inv_cta_kernel(Geo g, int dR, int parity, T a, T csw, const cplx<T> *__restrict__ clover, cplx<T> *inv, int *flags) {
+    extern __shared__ __align__(16) unsigned char smem_blk[];
+    const int n = 2 * dR, ne = dR * dR, ld = n + 1;
+    cplx<T> *M = reinterpret_cast<cplx<T> *>(smem_blk);
+    T *rmax = reinterpret_cast<T *>(M + (size_t)n * ld);
+    const int slot = blockIdx.x, c = blockIdx.y, tile = slot >> 5, lane = slot & 31;
+    const int I = threadIdx.x / TPR, part = threadIdx.x % TPR, cw = (n + TPR - 1) / TPR;
+    const int J0 = part * cw, J1 = J0 + cw < n ? J0 + cw : n;     // this thread's columns
+    const bool live = slot < g.Nh, row = I < n;
+    cplx<T> *G = inv + ((size_t)(tile * 2 + c) * n * n) * TILE + lane;
+    if (!live) {                                                   // padding lanes hold zeros
+        if (row)
+            for (int J = J0; J < J1; ++J) G[(size_t)(I * n + J) * TILE] = mk<T>(0, 0);
+        return;
+    }
+    if (row) {
+        const int bi = I / dR, i = I - bi * dR;
+        T m = 0;
+        for (int J = J0; J < J1; ++J) {
+            const int bj = J / dR, j = J - bj * dR;
+            cplx<T> v;
+            if (bi == bj) {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 0, i * dR + j, lane, ne)];
+                if (bi) { v.x = -v.x; v.y = -v.y; }
+            } else if (bi == 0) {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 1, i * dR + j, lane, ne)];
+            } else {
+                v = clover[clover_off(g.n_tiles, parity, tile, c, 1, j * dR + i, lane, ne)];
+                v.y = -v.y;
+            }
+            v.x *= csw; v.y *= csw;
+            if (I == J) v.x += a;
+            M[(size_t)I * ld + J] = v;
+            m = fmax(m, fmax(fabs(v.x), fabs(v.y)));
+        }
+        rmax[threadIdx.x] = m;
+    }
+    __syncthreads();
+    T scale = 0;
+    for (int r = 0; r < n * TPR; ++r) scale = fmax(scale, rmax[r]);
+    const T tiny = scale * (sizeof(T) == 8 ? T(1e-10) : T(1e-4));
+    bool bad = false;
+    for (int k = 0; k < n; ++k) {
+        cplx<T> *Pk = M + (size_t)k * ld;
+        cplx<T> *Mi = M + (size_t)(row ? I : 0) * ld;
+        // every thread of a row reads the pivot resp. its multiplier before the owner of column k overwrites it
+        const cplx<T> dk = Pk[k];
+        const cplx<T> f = Mi[k];
+        __syncwarp();
+        if (I == k) {
+            const T d2 = dk.x * dk.x + dk.y * dk.y;
+            if (!(d2 > tiny * tiny) || !isfinite(d2)) bad = true;
+            const T r = T(1) / d2;
+            const cplx<T> p = mk<T>(dk.x * r, -dk.y * r);
+            if (k >= J0 && k < J1) Pk[k] = mk<T>(1, 0);
+            for (int J = J0; J < J1; ++J) Pk[J] = cmul<T>(Pk[J], p);
+        }
+        __syncthreads();
+        if (row && I != k) {
+            if (k >= J0 && k < J1) Mi[k] = mk<T>(0, 0);
+#pragma unroll 4
+            for (int J = J0; J < J1; ++J) {
+                const cplx<T> x = Pk[J];
+                cplx<T> y = Mi[J];
+                y.x -= f.x * x.x - f.y * x.y;
+                y.y -= f.x * x.y + f.y * x.x;
+                Mi[J] = y;
+            }
+        }
+        __syncthreads();
+    }
+    if (row)
+        for (int J = J0; J < J1; ++J) G[(size_t)(I * n + J) * TILE] = M[(size_t)I * ld + J];
+    if (bad && part == 0 && flags) atomicOr(flags, 1);
+}
+template <typename T, int TPR> static int clover_inv_cta_launch(const Geo &g, int dR, int parity, double a, double csw, const void *clover, void *inv, int *flags, cudaStream_t s) {
+    const int n = 2 * dR;
+    const size_t smem = (size_t)n * (n + 1) * sizeof(cplx<T>) + (size_t)n * TPR * sizeof(T);
+    auto kern = clover_inv_cta_kernel<T, TPR>;
+    static DevCache cache{};
+    int n_sm = 0;
+    if (const int rc = prepare_launch(kern, (size_t)70 * 71 * sizeof(cplx<T>) + 70 * TPR * sizeof(T), cache, n_sm)) return rc;   // opt-in size for the largest block (d_R = 35)
+    kern<<<dim3(g.n_tiles * TILE, 2), (n * TPR + 31) / 32 * 32, smem, s>>>(g, dR, parity, (T)a, (T)csw, (const cplx<T> *)clover, (cplx<T> *)inv, flags);
+    return (int)cudaGetLastError();
+}
+template <typename T> static int clover_inv_cta(const Geo &g, int dR, int parity, double a, double csw, const void *clover, void *inv, int *flags, cudaStream_t s) {
+    // two threads per row for the 70 x 70 blocks in fp64 (two CTAs of 80 KB per SM: 140 instead of 70 threads each; C5 154 -> 116 ms); one
+    // thread per row elsewhere (measured: fp32 52 vs 57 ms at C5; four threads per row at 30 x 30 in fp64: 9.3 vs 3.5 ms)
+    return (2 * dR > 48 && sizeof(T) == 8) ? clover_inv_cta_launch<T, 2>(g, dR, parity, a, csw, clover, inv, flags, s)
+                                           : clover_inv_cta_launch<T, 1>(g, dR, parity, a, csw, clover, inv, flags, s);
+}
+
 template <typename T, int DRT> static int clover_inv_sm(const Geo &g, int parity, double a, double csw, const void *clover, void *inv, int *flags, cudaStream_t s) {
     auto kern = clover_inv_kernel<T, DRT>;
     const size_t smem = (size_t)4 * DRT * DRT * TILE * sizeof(cplx<T>);
@@ -1165,6 +1263,7 @@ template <typename T> static int clover_inv_t(const Geo &g, int dR, int parity, 
         case 8: return clover_inv_sm<T, 8>(g, parity, a, csw, clover, inv, flags, s);
         }
     }
+    if (glob == 0 && dR >= 10 && dR <= 35) return clover_inv_cta<T>(g, dR, parity, a, csw, clover, inv, flags, s);
     clover_inv_kernel<T, 0><<<dim3((g.n_tiles * TILE + 63) / 64, 2), 64, 0, s>>>(g, dR, parity, (T)a, (T)csw, (const cplx<T> *)clover, (cplx<T> *)inv, flags);
     return (int)cudaGetLastError();
 }
