@@ -66,14 +66,23 @@ template <typename T, bool REAL> __device__ __forceinline__ cplx<T> ld_w(const l
 // neighbours', as in the stencil); shared-memory accesses are conflict free (s is the fastest index).
 // DRT > 0 fixes d_R at compile time (inner products unrolled); planes, leaves and path steps are unrolled so that every
 // direction is a constant (no local-memory tables, no dynamic indexing of the coordinates).
+// multiply-add on path elements: complex for complex links, real for the real (adjoint) links
+template <typename T> __device__ __forceinline__ void pfma(cplx<T> &acc, cplx<T> a, cplx<T> b) { cfma<T>(acc, a, b); }
+template <typename T> __device__ __forceinline__ void pfma(T &acc, T a, T b) { acc = fma(a, b, acc); }
+template <typename T> __device__ __forceinline__ cplx<T> as_cplx(cplx<T> v) { return v; }
+template <typename T> __device__ __forceinline__ cplx<T> as_cplx(T v) { return mk<T>(v, T(0)); }
+
 template <typename T, bool REAL, int LP, int DRT>
 __global__ void __launch_bounds__(512) clover_field_kernel(Geo g, int dR_rt, const link_elem<T, REAL> *__restrict__ links, cplx<T> *__restrict__ clover) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    // real links (adjoint): the path products are real matrices -- a quarter of the multiply-adds and half the shared memory
+    using PT = link_elem<T, REAL>;
     const int dR = DRT ? DRT : dR_rt;
     const int ne = dR * dR, S = blockDim.x, sx = threadIdx.x;
     const size_t mat = (size_t)ne * S;                                  // one matrix for the S sites
-    cplx<T> *W = reinterpret_cast<cplx<T> *>(smem_raw) + sx;
-    cplx<T> *P = W + 4 * LP * mat, *Q = P + LP * mat, *C = Q + LP * mat, *acc = C + mat;
+    cplx<T> *acc = reinterpret_cast<cplx<T> *>(smem_raw) + sx;          // [4][e][S] complex, then the path matrices
+    PT *W = reinterpret_cast<PT *>(smem_raw + 4 * mat * sizeof(cplx<T>)) + sx;
+    PT *P = W + 4 * LP * mat, *Q = P + LP * mat, *C = Q + LP * mat;
     const long slot = (long)blockIdx.x * S + sx;                        // padded site slots: [parity][tile][lane]
     const int slots_half = g.n_tiles * TILE;
     const int p = (int)(slot / slots_half), hp = (int)(slot - (long)p * slots_half);
@@ -90,7 +99,7 @@ __global__ void __launch_bounds__(512) clover_field_kernel(Geo g, int dR_rt, con
     for (int pl = 0; pl < 6; ++pl) {
         const int mu = PL[pl][0], nu = PL[pl][1];
         const int seq[4][4] = {{mu, nu, mu + 4, nu + 4}, {nu, mu + 4, nu + 4, mu}, {mu + 4, nu + 4, mu, nu}, {nu + 4, mu, nu, mu + 4}};
-        for (int i = i0; i < dR; i += r) C[(size_t)(i * dR + j) * S] = mk<T>(0, 0);
+        for (int i = i0; i < dR; i += r) C[(size_t)(i * dR + j) * S] = PT{};
 #pragma unroll
         for (int lg = 0; lg < 4; lg += LP) {
 #pragma unroll
@@ -101,8 +110,8 @@ __global__ void __launch_bounds__(512) clover_field_kernel(Geo g, int dR_rt, con
                 for (int k = 0; k < 4; ++k) {
                     const int d = seq[lg + ll][k];
                     const size_t base = link_off(g.n_tiles, cp, ch >> 5, d, 0, ch & 31, ne);
-                    cplx<T> *dst = W + (size_t)(ll * 4 + k) * mat;
-                    for (int i = i0; i < dR; i += r) dst[(size_t)(i * dR + j) * S] = ld_w<T, REAL>(links, base + (size_t)(i * dR + j) * TILE);
+                    PT *dst = W + (size_t)(ll * 4 + k) * mat;
+                    for (int i = i0; i < dR; i += r) dst[(size_t)(i * dR + j) * S] = links[base + (size_t)(i * dR + j) * TILE];
                     w.step(g, d);
                     ch = w.half_index(g);
                     cp ^= 1;
@@ -111,39 +120,39 @@ __global__ void __launch_bounds__(512) clover_field_kernel(Geo g, int dR_rt, con
             __syncthreads();
 #pragma unroll
             for (int ll = 0; ll < LP; ++ll) {
-                const cplx<T> *A = W + (size_t)(ll * 4) * mat, *B = A + mat;
+                const PT *A = W + (size_t)(ll * 4) * mat, *B = A + mat;
                 for (int i = i0; i < dR; i += r) {
                     const int e = i * dR + j;
-                    cplx<T> s = mk<T>(0, 0);
-                    const cplx<T> *a = A + (size_t)(i * dR) * S, *b = B + (size_t)j * S;
+                    PT s = PT{};
+                    const PT *a = A + (size_t)(i * dR) * S, *b = B + (size_t)j * S;
 #pragma unroll
-                    for (int l = 0; l < dR; ++l, a += S, b += (size_t)dR * S) cfma<T>(s, *a, *b);
+                    for (int l = 0; l < dR; ++l, a += S, b += (size_t)dR * S) pfma<T>(s, *a, *b);
                     P[ll * mat + (size_t)e * S] = s;
                 }
             }
             __syncthreads();
 #pragma unroll
             for (int ll = 0; ll < LP; ++ll) {
-                const cplx<T> *A = P + (size_t)ll * mat, *B = W + (size_t)(ll * 4 + 2) * mat;
+                const PT *A = P + (size_t)ll * mat, *B = W + (size_t)(ll * 4 + 2) * mat;
                 for (int i = i0; i < dR; i += r) {
                     const int e = i * dR + j;
-                    cplx<T> s = mk<T>(0, 0);
-                    const cplx<T> *a = A + (size_t)(i * dR) * S, *b = B + (size_t)j * S;
+                    PT s = PT{};
+                    const PT *a = A + (size_t)(i * dR) * S, *b = B + (size_t)j * S;
 #pragma unroll
-                    for (int l = 0; l < dR; ++l, a += S, b += (size_t)dR * S) cfma<T>(s, *a, *b);
+                    for (int l = 0; l < dR; ++l, a += S, b += (size_t)dR * S) pfma<T>(s, *a, *b);
                     Q[ll * mat + (size_t)e * S] = s;
                 }
             }
             __syncthreads();
 #pragma unroll
             for (int ll = 0; ll < LP; ++ll) {
-                const cplx<T> *A = Q + (size_t)ll * mat, *B = W + (size_t)(ll * 4 + 3) * mat;
+                const PT *A = Q + (size_t)ll * mat, *B = W + (size_t)(ll * 4 + 3) * mat;
                 for (int i = i0; i < dR; i += r) {
                     const int e = i * dR + j;
-                    cplx<T> s = C[(size_t)e * S];
-                    const cplx<T> *a = A + (size_t)(i * dR) * S, *b = B + (size_t)j * S;
+                    PT s = C[(size_t)e * S];
+                    const PT *a = A + (size_t)(i * dR) * S, *b = B + (size_t)j * S;
 #pragma unroll
-                    for (int l = 0; l < dR; ++l, a += S, b += (size_t)dR * S) cfma<T>(s, *a, *b);
+                    for (int l = 0; l < dR; ++l, a += S, b += (size_t)dR * S) pfma<T>(s, *a, *b);
                     C[(size_t)e * S] = s;
                 }
             }
@@ -152,7 +161,7 @@ __global__ void __launch_bounds__(512) clover_field_kernel(Geo g, int dR_rt, con
         // F = (C - C^+)/8 ; contribution (i/2) F (and for K2, times -i) to H_c / B_c with the signs of the header table
         for (int i = i0; i < dR; i += r) {
             const int e = i * dR + j;
-            const cplx<T> a = C[(size_t)e * S], b = C[(size_t)(j * dR + i) * S];
+            const cplx<T> a = as_cplx<T>(C[(size_t)e * S]), b = as_cplx<T>(C[(size_t)(j * dR + i) * S]);
             const cplx<T> F = mk<T>((a.x - b.x) * T(0.125), (a.y + b.y) * T(0.125));
             const cplx<T> iF = mk<T>(-T(0.5) * F.y, T(0.5) * F.x);    // (i/2) F
             const cplx<T> hF = mk<T>(T(0.5) * F.x, T(0.5) * F.y);     // -i (i/2) F = F/2
@@ -564,7 +573,7 @@ template <typename T, bool REAL> static int clover_field_t(const Geo &g, int dR,
     }
     constexpr int LP = 1;
     const int ne = dR * dR;
-    const size_t per_site = (size_t)(6 * LP + 5) * ne * sizeof(cplx<T>);
+    const size_t per_site = (size_t)(6 * LP + 1) * ne * sizeof(link_elem<T, REAL>) + (size_t)4 * ne * sizeof(cplx<T>);   // W[4 LP], P[LP], Q[LP], C + acc[4]
     int S = TILE;
     while (S > 1 && per_site * S > (size_t)200 * 1024) S >>= 1;
     int rows = 512 / S / dR;                       // blockDim.y = rows * dR: each thread owns one column of `rows`-strided rows
