@@ -71,6 +71,8 @@ template <typename T> __device__ __forceinline__ void pfma(cplx<T> &acc, cplx<T>
 template <typename T> __device__ __forceinline__ void pfma(T &acc, T a, T b) { acc = fma(a, b, acc); }
 template <typename T> __device__ __forceinline__ cplx<T> as_cplx(cplx<T> v) { return v; }
 template <typename T> __device__ __forceinline__ cplx<T> as_cplx(T v) { return mk<T>(v, T(0)); }
+template <typename T> __device__ __forceinline__ void padd(cplx<T> &acc, cplx<T> v) { acc.x += v.x; acc.y += v.y; }
+template <typename T> __device__ __forceinline__ void padd(T &acc, T v) { acc += v; }
 
 template <typename T, bool REAL, int LP, int DRT>
 __global__ void __launch_bounds__(512) clover_field_kernel(Geo g, int dR_rt, const link_elem<T, REAL> *__restrict__ links, cplx<T> *__restrict__ clover) {
@@ -364,12 +366,13 @@ __global__ void __launch_bounds__(128) clover_field_site_kernel(Geo g, const lin
 #pragma unroll
             for (int e = 0; e < NE; ++e) acc0[e] = acc1[e] = mk<T>(0, 0);
         }
-        cplx<T> C[NE];
+        using PT = link_elem<T, REAL>;   // real links: real path products (a quarter of the multiply-adds)
+        PT C[NE];
 #pragma unroll
-        for (int e = 0; e < NE; ++e) C[e] = mk<T>(0, 0);
+        for (int e = 0; e < NE; ++e) C[e] = PT{};
         for (int leaf = 0; leaf < 4; ++leaf) {
             int t = t0, x = x0, y = y0, z = z0, cp = p, ch = h;
-            cplx<T> P[NE], Q[NE];
+            PT P[NE], Q[NE];
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const int sq = (leaf + k) & 3;
@@ -377,17 +380,17 @@ __global__ void __launch_bounds__(128) clover_field_site_kernel(Geo g, const lin
                 const link_elem<T, REAL> *W = links + link_off(g.n_tiles, cp, ch >> 5, d, 0, ch & 31, NE);
                 if (k == 0) {
 #pragma unroll
-                    for (int e = 0; e < NE; ++e) P[e] = ld_w<T, REAL>(W, (size_t)e * TILE);
+                    for (int e = 0; e < NE; ++e) P[e] = W[(size_t)e * TILE];
                 } else {
 #pragma unroll
-                    for (int e = 0; e < NE; ++e) Q[e] = mk<T>(0, 0);
+                    for (int e = 0; e < NE; ++e) Q[e] = PT{};
 #pragma unroll
                     for (int l = 0; l < DR; ++l)
 #pragma unroll
                         for (int j = 0; j < DR; ++j) {
-                            const cplx<T> w = ld_w<T, REAL>(W, (size_t)(l * DR + j) * TILE);
+                            const PT w = W[(size_t)(l * DR + j) * TILE];
 #pragma unroll
-                            for (int i = 0; i < DR; ++i) cfma<T>(Q[i * DR + j], P[i * DR + l], w);
+                            for (int i = 0; i < DR; ++i) pfma<T>(Q[i * DR + j], P[i * DR + l], w);
                         }
 #pragma unroll
                     for (int e = 0; e < NE; ++e) P[e] = Q[e];
@@ -402,7 +405,7 @@ __global__ void __launch_bounds__(128) clover_field_site_kernel(Geo g, const lin
                 cp ^= 1;
             }
 #pragma unroll
-            for (int e = 0; e < NE; ++e) { C[e].x += P[e].x; C[e].y += P[e].y; }
+            for (int e = 0; e < NE; ++e) padd<T>(C[e], P[e]);
         }
         // F = (C - C^+)/8; (i/2) F -> K1 (planes 01, 23) or K3 (03, 12); F/2 = -i (i/2) F -> -i K2 (02, 13)
         const T s0 = (pl == 3 || pl == 5) ? T(-1) : T(1);          // c = 0: +F01 -F23 | +F02 +F13 | +F03 -F12
@@ -412,7 +415,7 @@ __global__ void __launch_bounds__(128) clover_field_site_kernel(Geo g, const lin
         for (int i = 0; i < DR; ++i)
 #pragma unroll
             for (int j = 0; j < DR; ++j) {
-                const cplx<T> a = C[i * DR + j], b = C[j * DR + i];
+                const cplx<T> a = as_cplx<T>(C[i * DR + j]), b = as_cplx<T>(C[j * DR + i]);
                 const cplx<T> F = mk<T>((a.x - b.x) * T(0.125), (a.y + b.y) * T(0.125));
                 const cplx<T> v = half ? mk<T>(T(0.5) * F.x, T(0.5) * F.y) : mk<T>(-T(0.5) * F.y, T(0.5) * F.x);
                 acc0[i * DR + j].x += s0 * v.x; acc0[i * DR + j].y += s0 * v.y;
@@ -439,7 +442,7 @@ __global__ void __launch_bounds__(32 * NS, MB) clover_field_rows_kernel(Geo g, c
     static_assert(DR % NS == 0, "the rows must split evenly over the warps");
     constexpr int NE = DR * DR, RP = DR / NS, NR = RP * DR;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx<T> *exch = reinterpret_cast<cplx<T> *>(smem_raw) + (threadIdx.x & 31);      // leaf sum C of the tile, [e][lane]
+    link_elem<T, REAL> *exch = reinterpret_cast<link_elem<T, REAL> *>(smem_raw) + (threadIdx.x & 31);   // leaf sum C of the tile, [e][lane]
     const int lane = threadIdx.x & 31, r0 = (threadIdx.x >> 5) * RP;
     const int p = blockIdx.x / g.n_tiles, tile = blockIdx.x - p * g.n_tiles;
     const int hp = tile * TILE + lane;
@@ -457,12 +460,13 @@ __global__ void __launch_bounds__(32 * NS, MB) clover_field_rows_kernel(Geo g, c
 #pragma unroll
             for (int e = 0; e < NR; ++e) acc0[e] = acc1[e] = mk<T>(0, 0);
         }
-        cplx<T> C[NR];
+        using PT = link_elem<T, REAL>;   // real links: real path products (a quarter of the multiply-adds)
+        PT C[NR];
 #pragma unroll
-        for (int e = 0; e < NR; ++e) C[e] = mk<T>(0, 0);
+        for (int e = 0; e < NR; ++e) C[e] = PT{};
         for (int leaf = 0; leaf < 4; ++leaf) {
             int t = t0, x = x0, y = y0, z = z0, cp = p, ch = h;
-            cplx<T> P[NR], Q[NR];
+            PT P[NR], Q[NR];
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const int sq = (leaf + k) & 3;
@@ -472,17 +476,17 @@ __global__ void __launch_bounds__(32 * NS, MB) clover_field_rows_kernel(Geo g, c
 #pragma unroll
                     for (int rr = 0; rr < RP; ++rr)
 #pragma unroll
-                        for (int j = 0; j < DR; ++j) P[rr * DR + j] = ld_w<T, REAL>(W, (size_t)((r0 + rr) * DR + j) * TILE);
+                        for (int j = 0; j < DR; ++j) P[rr * DR + j] = W[(size_t)((r0 + rr) * DR + j) * TILE];
                 } else {
 #pragma unroll
-                    for (int e = 0; e < NR; ++e) Q[e] = mk<T>(0, 0);
+                    for (int e = 0; e < NR; ++e) Q[e] = PT{};
 #pragma unroll
                     for (int l = 0; l < DR; ++l)
 #pragma unroll
                         for (int j = 0; j < DR; ++j) {
-                            const cplx<T> w = ld_w<T, REAL>(W, (size_t)(l * DR + j) * TILE);
+                            const PT w = W[(size_t)(l * DR + j) * TILE];
 #pragma unroll
-                            for (int rr = 0; rr < RP; ++rr) cfma<T>(Q[rr * DR + j], P[rr * DR + l], w);
+                            for (int rr = 0; rr < RP; ++rr) pfma<T>(Q[rr * DR + j], P[rr * DR + l], w);
                         }
 #pragma unroll
                     for (int e = 0; e < NR; ++e) P[e] = Q[e];
@@ -497,7 +501,7 @@ __global__ void __launch_bounds__(32 * NS, MB) clover_field_rows_kernel(Geo g, c
                 cp ^= 1;
             }
 #pragma unroll
-            for (int e = 0; e < NR; ++e) { C[e].x += P[e].x; C[e].y += P[e].y; }
+            for (int e = 0; e < NR; ++e) padd<T>(C[e], P[e]);
         }
         // the leaf sum to shared memory: row i of C^+ is column i of C, whose entries the other warps hold
         __syncthreads();                                            // the previous plane's reads are done
@@ -514,7 +518,7 @@ __global__ void __launch_bounds__(32 * NS, MB) clover_field_rows_kernel(Geo g, c
         for (int rr = 0; rr < RP; ++rr)
 #pragma unroll
             for (int j = 0; j < DR; ++j) {
-                const cplx<T> a = C[rr * DR + j], b = exch[(size_t)(j * DR + r0 + rr) * TILE];
+                const cplx<T> a = as_cplx<T>(C[rr * DR + j]), b = as_cplx<T>(exch[(size_t)(j * DR + r0 + rr) * TILE]);
                 const cplx<T> F = mk<T>((a.x - b.x) * T(0.125), (a.y + b.y) * T(0.125));
                 const cplx<T> v = half ? mk<T>(T(0.5) * F.x, T(0.5) * F.y) : mk<T>(-T(0.5) * F.y, T(0.5) * F.x);
                 acc0[rr * DR + j].x += s0 * v.x; acc0[rr * DR + j].y += s0 * v.y;
